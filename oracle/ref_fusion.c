@@ -1,0 +1,280 @@
+/*
+ * oracle/ref_fusion.c -- CPU ORACLE for the per-frame volumetric fusion of arXiv 1602.06645.
+ *
+ * TEST INFRASTRUCTURE ONLY.  Plain, slow, obviously-correct per-voxel loops written from the
+ * paper's equations; no pre-pass, no culling, no tiling, no code shared with the CUDA path
+ * (paper_1602_06645_b200/).  Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
+ * --impl reference legs may call it.
+ *
+ * What it computes (citations are PAPER.md lines; readings A1..A17 are SURVEY.md 8(c), restated in
+ * DESIGN.md "Readings"):
+ *   geometry volume  -- projective TSDF integration.  The paper gives NO equations for it
+ *                       (L33-35 defer to KinectFusion/PCL); the definition is reading A5/A6 and is
+ *                       pinned by BASELINE.json's closed forms.  ** paper: parity unpinned **
+ *   colour volume    -- eq. 5-10, on an asymmetrical colour volume (L87) with r x more
+ *                       voxels per axis.  Readings A11 (which point maps to the HD image) and A12
+ *                       (u8 weight encoding of eq. 10) are conventions ** parity unpinned ** by the paper.
+ *
+ * Canonical arithmetic: IEEE binary32, round-to-nearest-even, no implicit contraction
+ * (-ffp-contract=off); fmaf() where the spec says fma; / and sqrtf correctly rounded; rintf = half-even.
+ *
+ * Layout (little-endian, x fastest: index ((k*Ny + j)*Nx + i)):
+ *   geometry word = int16 tsdf_q (bytes 0-1) | int16 w (bytes 2-3), F = tsdf_q / 32767
+ *   colour word   = u8 R | u8 G | u8 B | u8 wq,                  W = wq / 255
+ *
+ * Build: gcc -O2 -fopenmp -ffp-contract=off -mfma -shared -fPIC ref_fusion.c -lm
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stddef.h>
+#include <string.h>
+
+typedef struct {
+    int32_t nx, ny, nz;      /* geometry dims */
+    int32_t r;               /* colour dims = r * geometry dims (L87) */
+    float   origin[3];       /* world position of the volume's corner (A1) */
+    float   extent;          /* side length along x, metres; cubic voxels vs = extent / nx */
+    float   mu;              /* truncation distance, metres (A5) */
+    int32_t w_max;           /* geometry weight cap (A5) */
+    float   sigma;           /* colour distance gate, metres; 0.020 in the paper (L108) */
+    float   gate;            /* weight gate factor; 0.8 in the paper (L115) */
+} ref_vol_t;
+
+typedef struct {
+    const uint16_t *depth; int32_t wd, hd;      /* depth map D_n, mm, 0 = invalid (L101-103) */
+    const uint8_t  *rgb;   int32_t wh, hh;      /* HD RGB image, interleaved R,G,B (L115) */
+    float T_world_depth[16];                    /* row-major rigid 4x4, depth-camera -> world */
+    float K_depth[9], K_rgb[9];                 /* row-major [fx 0 cx; 0 fy cy; 0 0 1] */
+    float T_depth_rgb[16];                      /* row-major rigid 4x4, RGB-camera -> depth-camera */
+} ref_frame_t;
+
+/* per-frame counters: a voxel is *read* when it reaches the load of its stored
+ * word and *changed* when the stored word differs after the store */
+enum { CNT_GEO_READ = 0, CNT_GEO_CHANGED = 1, CNT_COL_READ = 2, CNT_COL_CHANGED = 3, CNT_N = 4 };
+
+/* S0: per-frame constants, computed in fp64 and rounded once to fp32 */
+typedef struct {
+    float R[9], t[3];        /* (R_n, t_n) of eq. 5: world -> current depth camera = inverse(T_world_depth) */
+    float Rc[9], tc[3];      /* (R_calib, t_calib) of eq. 3: depth camera -> HD camera = inverse(T_depth_rgb) */
+    float fx, fy, cx, cy;    /* K_c  */
+    float fxh, fyh, cxh, cyh;/* K_hd */
+    float vs, vc;            /* geometry / colour voxel size */
+    float inv_mu, sig2;
+} consts_t;
+
+/* rigid inverse: R' = R^T, t' = -(R^T t), fp64 with left-to-right sums, one rounding to fp32 */
+static void rigid_inverse(const float T[16], float Rout[9], float tout[3])
+{
+    for (int i = 0; i < 3; ++i) {
+        for (int j = 0; j < 3; ++j) Rout[3 * i + j] = T[4 * j + i];
+        double s = (double)T[4 * 0 + i] * (double)T[4 * 0 + 3];
+        s = s + (double)T[4 * 1 + i] * (double)T[4 * 1 + 3];
+        s = s + (double)T[4 * 2 + i] * (double)T[4 * 2 + 3];
+        tout[i] = (float)(-s);
+    }
+}
+
+static void frame_consts(const ref_vol_t *v, const ref_frame_t *f, consts_t *c)
+{
+    rigid_inverse(f->T_world_depth, c->R, c->t);
+    rigid_inverse(f->T_depth_rgb, c->Rc, c->tc);
+    c->fx = f->K_depth[0]; c->fy = f->K_depth[4]; c->cx = f->K_depth[2]; c->cy = f->K_depth[5];
+    c->fxh = f->K_rgb[0]; c->fyh = f->K_rgb[4]; c->cxh = f->K_rgb[2]; c->cyh = f->K_rgb[5];
+    c->vs = v->extent / (float)v->nx;
+    c->vc = c->vs / (float)v->r;
+    c->inv_mu = 1.0f / v->mu;
+    c->sig2 = v->sigma * v->sigma;
+}
+
+/* eq. 5 (L91-94), voxel centre convention A1: centre of voxel idx in a grid of voxel size s */
+static void voxel_to_camera(const ref_vol_t *v, const consts_t *c, float s, int i, int j, int k,
+                            float *X, float *Y, float *Z)
+{
+    float px = fmaf((float)i + 0.5f, s, v->origin[0]);
+    float py = fmaf((float)j + 0.5f, s, v->origin[1]);
+    float pz = fmaf((float)k + 0.5f, s, v->origin[2]);
+    *X = fmaf(c->R[2], pz, fmaf(c->R[1], py, fmaf(c->R[0], px, c->t[0])));
+    *Y = fmaf(c->R[5], pz, fmaf(c->R[4], py, fmaf(c->R[3], px, c->t[1])));
+    *Z = fmaf(c->R[8], pz, fmaf(c->R[7], py, fmaf(c->R[6], px, c->t[2])));
+}
+
+/* eq. 1 / eq. 6 (L64-67, L96-99): pinhole projection, divide by z, nearest pixel (A2), frustum =
+ * Z > 0 and rounded pixel inside the w x h image (A3).  Returns 1 and the pixel if inside. */
+static int project(float fx, float fy, float cx, float cy, int w, int h,
+                   float X, float Y, float Z, int *x, int *y)
+{
+    if (!(Z > 0.0f)) return 0;
+    float iz = 1.0f / Z;
+    float u = fmaf(fx, X * iz, cx);
+    float vv = fmaf(fy, Y * iz, cy);
+    float uf = floorf(u + 0.5f);
+    float vf = floorf(vv + 0.5f);
+    if (!(uf >= 0.0f && uf < (float)w && vf >= 0.0f && vf < (float)h)) return 0;
+    *x = (int)uf; *y = (int)vf;
+    return 1;
+}
+
+/* O-G: one geometry voxel (L33-35; definition = readings A5, A6).  Returns bit0 = read, bit1 = changed. */
+static int update_geo_voxel(const ref_vol_t *v, const ref_frame_t *f, const consts_t *c,
+                            int i, int j, int k, uint32_t *word)
+{
+    float X, Y, Z; int x, y;
+    voxel_to_camera(v, c, c->vs, i, j, k, &X, &Y, &Z);
+    if (!project(c->fx, c->fy, c->cx, c->cy, f->wd, f->hd, X, Y, Z, &x, &y)) return 0;
+    uint16_t d = f->depth[(size_t)y * (size_t)f->wd + (size_t)x];
+    if (d == 0) return 0;                                   /* "if non-zero" (L103) */
+    float D = (float)d * 0.001f;                            /* mm -> m (A4) */
+    float sdf = D - Z;                                      /* projective signed distance (A5) */
+    if (sdf < -v->mu) return 0;                             /* behind the truncation band: unchanged */
+    float tsdf = fminf(1.0f, sdf * c->inv_mu);
+    int q = (int16_t)(*word & 0xffffu);
+    int w = (int16_t)(*word >> 16);
+    float num = fmaf((float)q, (float)w, tsdf * 32767.0f);  /* running average, per-frame weight 1 */
+    int qn = (int)rintf(num / ((float)w + 1.0f));
+    int wn = w + 1 < v->w_max ? w + 1 : v->w_max;           /* increment and saturate */
+    uint32_t nw = ((uint32_t)(uint16_t)(int16_t)qn) | ((uint32_t)(uint16_t)(int16_t)wn << 16);
+    int changed = nw != *word;
+    *word = nw;
+    return 1 | (changed << 1);
+}
+
+/* eq. 7 (L103-106): back-projection of depth pixel (x, y, D) with K_c^-1 */
+static void backproject(const consts_t *c, int x, int y, float D, float P[3])
+{
+    P[0] = (((float)x - c->cx) * D) / c->fx;
+    P[1] = (((float)y - c->cy) * D) / c->fy;
+    P[2] = D;
+}
+
+/* O-C: one colour voxel, eq. 5-10 (L91-124).  Returns bit0 = read, bit1 = changed. */
+static int update_col_voxel(const ref_vol_t *v, const ref_frame_t *f, const consts_t *c,
+                            int i, int j, int k, uint32_t *word)
+{
+    float X, Y, Z; int x, y;
+    voxel_to_camera(v, c, c->vc, i, j, k, &X, &Y, &Z);                                 /* eq. 5 */
+    if (!project(c->fx, c->fy, c->cx, c->cy, f->wd, f->hd, X, Y, Z, &x, &y)) return 0; /* eq. 6 */
+    uint16_t d0 = f->depth[(size_t)y * (size_t)f->wd + (size_t)x];
+    if (d0 == 0) return 0;                                                             /* L103 */
+    if (!(x + 1 < f->wd && y + 1 < f->hd)) return 0;                                   /* A7: no neighbour */
+    uint16_t d1 = f->depth[(size_t)y * (size_t)f->wd + (size_t)(x + 1)];
+    uint16_t d2 = f->depth[(size_t)(y + 1) * (size_t)f->wd + (size_t)x];
+    if (d1 == 0 || d2 == 0) return 0;                                                  /* A7 */
+    float Pd[3], P1[3], P2[3];
+    backproject(c, x, y, (float)d0 * 0.001f, Pd);                                      /* eq. 7 */
+    backproject(c, x + 1, y, (float)d1 * 0.001f, P1);
+    backproject(c, x, y + 1, (float)d2 * 0.001f, P2);
+    /* sigma gate (L108): Euclidean distance between voxel and depth point */
+    float dx = X - Pd[0], dy = Y - Pd[1], dz = Z - Pd[2];
+    float dist2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+    if (dist2 > c->sig2) return 0;
+    /* eq. 8 (L110-113): normal from forward differences */
+    float ax = P1[0] - Pd[0], ay = P1[1] - Pd[1], az = P1[2] - Pd[2];
+    float bx = P2[0] - Pd[0], by = P2[1] - Pd[1], bz = P2[2] - Pd[2];
+    float nx = fmaf(ay, bz, -(az * by));
+    float ny = fmaf(az, bx, -(ax * bz));
+    float nz = fmaf(ax, by, -(ay * bx));
+    /* weight (L110, A8): cosine between the normal and the viewing ray camera -> point */
+    float dot = fmaf(nz, Pd[2], fmaf(ny, Pd[1], nx * Pd[0]));
+    float nn = fmaf(nz, nz, fmaf(ny, ny, nx * nx));
+    float pp = fmaf(Pd[2], Pd[2], fmaf(Pd[1], Pd[1], Pd[0] * Pd[0]));
+    float den = sqrtf(nn * pp);
+    if (!(den > 0.0f)) return 0;
+    float W = fminf(1.0f, dot / den);
+    if (!(W > 0.0f)) return 0;
+    /* read C_pre, W_pre */
+    uint32_t old = *word;
+    int C[3] = { (int)(old & 0xffu), (int)((old >> 8) & 0xffu), (int)((old >> 16) & 0xffu) };
+    int wq = (int)(old >> 24);
+    float W255 = W * 255.0f;
+    if (!(W255 > v->gate * (float)wq)) return 1;                                       /* L115, A9 */
+    /* HD pixel of the voxel's own position (eq. 3-4; A10, A11) */
+    float Xh = fmaf(c->Rc[2], Z, fmaf(c->Rc[1], Y, fmaf(c->Rc[0], X, c->tc[0])));
+    float Yh = fmaf(c->Rc[5], Z, fmaf(c->Rc[4], Y, fmaf(c->Rc[3], X, c->tc[1])));
+    float Zh = fmaf(c->Rc[8], Z, fmaf(c->Rc[7], Y, fmaf(c->Rc[6], X, c->tc[2])));
+    int xh, yh;
+    if (!project(c->fxh, c->fyh, c->cxh, c->cyh, f->wh, f->hh, Xh, Yh, Zh, &xh, &yh)) return 1;  /* A13 */
+    const uint8_t *hd = f->rgb + ((size_t)yh * (size_t)f->wh + (size_t)xh) * 3;        /* A14: nearest */
+    uint32_t nw = 0;
+    for (int ch = 0; ch < 3; ++ch) {                                                   /* eq. 9 (L117) */
+        float num = fmaf(W255, (float)hd[ch], (float)(C[ch] * wq));
+        float cn = rintf(num / ((float)wq + W255));
+        int ci = cn < 0.0f ? 0 : (cn > 255.0f ? 255 : (int)cn);
+        nw |= (uint32_t)ci << (8 * ch);
+    }
+    int wn = (int)rintf(fmaf(W, (float)(255 - wq), (float)wq));                        /* eq. 10 (L122), A12 */
+    if (wn > 255) wn = 255;
+    nw |= (uint32_t)wn << 24;
+    *word = nw;                                                                        /* L124 */
+    return 1 | ((nw != old) << 1);
+}
+
+/* ------------------------------------------------------------------------------------------ */
+/* exported entry points (host pointers only)                                                  */
+/* ------------------------------------------------------------------------------------------ */
+
+/* ref_integrate: one frame over the WHOLE of both volumes -- a plain triple loop over the
+ * geometry voxels, then a plain triple loop over the colour voxels.  geo / col are the packed
+ * state arrays (layout above), updated in place.  counters[4] (nullable) receives this frame's
+ * CNT_* counts.  OpenMP only splits the outermost z loop; voxels are independent (A15). */
+int ref_integrate(const ref_vol_t *v, const ref_frame_t *f, uint32_t *geo, uint32_t *col, uint64_t *counters)
+{
+    if (!v || !f || !geo || !col || !f->depth || !f->rgb) return -1;
+    if (v->nx <= 0 || v->ny <= 0 || v->nz <= 0 || v->r < 1 || !(v->mu > 0.0f) || v->w_max < 1 || v->w_max > 512) return -1;
+    consts_t c; frame_consts(v, f, &c);
+    uint64_t gr = 0, gc = 0, cr = 0, cc = 0;
+#pragma omp parallel for schedule(static) reduction(+ : gr, gc)
+    for (int k = 0; k < v->nz; ++k)
+        for (int j = 0; j < v->ny; ++j)
+            for (int i = 0; i < v->nx; ++i) {
+                size_t idx = ((size_t)k * (size_t)v->ny + (size_t)j) * (size_t)v->nx + (size_t)i;
+                int s = update_geo_voxel(v, f, &c, i, j, k, &geo[idx]);
+                gr += (uint64_t)(s & 1); gc += (uint64_t)(s >> 1);
+            }
+    const int cx = v->nx * v->r, cy = v->ny * v->r, cz = v->nz * v->r;
+#pragma omp parallel for schedule(static) reduction(+ : cr, cc)
+    for (int k = 0; k < cz; ++k)
+        for (int j = 0; j < cy; ++j)
+            for (int i = 0; i < cx; ++i) {
+                size_t idx = ((size_t)k * (size_t)cy + (size_t)j) * (size_t)cx + (size_t)i;
+                int s = update_col_voxel(v, f, &c, i, j, k, &col[idx]);
+                cr += (uint64_t)(s & 1); cc += (uint64_t)(s >> 1);
+            }
+    if (counters) { counters[CNT_GEO_READ] = gr; counters[CNT_GEO_CHANGED] = gc; counters[CNT_COL_READ] = cr; counters[CNT_COL_CHANGED] = cc; }
+    return 0;
+}
+
+/* ref_integrate_subset: the same per-voxel updates applied to a LIST of voxels only (voxels never
+ * interact, so the state of any subset after any number of frames is exact -- SURVEY 8(c) "making
+ * the oracle affordable").  geo_idx / col_idx are linear voxel indices into the full grids;
+ * geo_words / col_words hold the state of just those voxels and are updated in place. */
+int ref_integrate_subset(const ref_vol_t *v, const ref_frame_t *f,
+                         const int64_t *geo_idx, int64_t n_geo, uint32_t *geo_words,
+                         const int64_t *col_idx, int64_t n_col, uint32_t *col_words)
+{
+    if (!v || !f || !f->depth || !f->rgb) return -1;
+    if (v->nx <= 0 || v->ny <= 0 || v->nz <= 0 || v->r < 1 || !(v->mu > 0.0f) || v->w_max < 1 || v->w_max > 512) return -1;
+    consts_t c; frame_consts(v, f, &c);
+#pragma omp parallel for schedule(static)
+    for (int64_t n = 0; n < n_geo; ++n) {
+        int64_t idx = geo_idx[n];
+        int i = (int)(idx % v->nx), j = (int)((idx / v->nx) % v->ny), k = (int)(idx / ((int64_t)v->nx * v->ny));
+        update_geo_voxel(v, f, &c, i, j, k, &geo_words[n]);
+    }
+    const int64_t cx = (int64_t)v->nx * v->r, cy = (int64_t)v->ny * v->r;
+#pragma omp parallel for schedule(static)
+    for (int64_t n = 0; n < n_col; ++n) {
+        int64_t idx = col_idx[n];
+        int i = (int)(idx % cx), j = (int)((idx / cx) % cy), k = (int)(idx / (cx * cy));
+        update_col_voxel(v, f, &c, i, j, k, &col_words[n]);
+    }
+    return 0;
+}
+
+/* ref_frame_constants: expose S0 (for the tests that pin the rigid inverse). out = R[9] t[3] Rc[9] tc[3] */
+int ref_frame_constants(const ref_vol_t *v, const ref_frame_t *f, float out[24])
+{
+    consts_t c; frame_consts(v, f, &c);
+    memcpy(out, c.R, 9 * sizeof(float)); memcpy(out + 9, c.t, 3 * sizeof(float));
+    memcpy(out + 12, c.Rc, 9 * sizeof(float)); memcpy(out + 21, c.tc, 3 * sizeof(float));
+    return 0;
+}
