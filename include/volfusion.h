@@ -1,0 +1,135 @@
+/*
+ * volfusion.h -- C ABI of the B200-native per-frame volumetric fusion of arXiv 1602.06645
+ * ("Creating Simplified 3D Models with High Quality Textures", Liu, Li, Ogunbona, Chow).
+ *
+ * One call, vol_integrate(), fuses one RGB-D frame into two device-resident volumes:
+ *   - the geometry volume: projective TSDF integration of the depth map (the paper defers to
+ *     KinectFusion/PCL, the exact definition is DESIGN.md readings A5/A6);
+ *   - the asymmetrical colour volume: r x more voxels per axis over the same physical cube,
+ *     updated from the calibrated HD RGB frame by eq. 5-10.
+ * Every step runs in hand-written sm_100a CUDA kernels; there is no CPU fallback.
+ *
+ * Conventions
+ *   - "T_a_b" is a row-major rigid 4x4 that maps b-coordinates to a-coordinates.
+ *     (R_n, t_n) of eq. 5 = inverse(T_world_depth); (R_calib, t_calib) of eq. 3 = inverse(T_depth_rgb).
+ *   - K matrices are row-major [fx 0 cx; 0 fy cy; 0 0 1] (eq. 1); pixel centres at integers.
+ *   - Voxel (i,j,k) of a grid with voxel size s has its centre at origin + (idx + 0.5) * s (reading A1); both
+ *     grids share origin and extent; geometry voxel i spans colour voxels r*i .. r*i + r - 1 per axis.
+ *   - Layouts (little-endian, x fastest, linear index ((k*Ny + j)*Nx + i)):
+ *       geometry word = int16 tsdf_q (bytes 0-1) | int16 w (bytes 2-3),  F = tsdf_q / 32767
+ *       colour word   = u8 R | u8 G | u8 B | u8 wq (bytes 0..3),         W = wq / 255
+ *     All-zero bytes = "never observed" (initial state).
+ *   - Pointers are marked HOST or DEVICE.  Matrix arguments are HOST and copied at call time.  Frame buffers are
+ *     borrowed and must stay valid until the stream has finished the enqueued work.
+ *   - Every function returns VOL_OK (0) or a negative VOL_E_* code; validation happens before any launch, so a
+ *     failed call leaves the volumes untouched.  Nothing throws or aborts across this boundary.
+ *   - `stream` is a cudaStream_t passed as void* (NULL = default stream).  vol_integrate* and vol_reset are
+ *     asynchronous on it; vol_download*, vol_upload and vol_frame_stats synchronise it before returning.
+ */
+#ifndef VOLFUSION_H
+#define VOLFUSION_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define VOL_OK       0
+#define VOL_E_ARG   -1   /* null pointer, dims <= 0, dims_geo[0] % 4 != 0, r not in 1..4, mu <= 0, w_max not in 1..512,
+                            non-zero skew, non-rigid T, image size <= 0, buffer too small, bad shard */
+#define VOL_E_OOM   -2   /* device allocation failed */
+#define VOL_E_CUDA  -3   /* a CUDA call failed (sticky: see vol_strerror) */
+
+/* geometry layers per shard slab (and per culling tile along z): rank `shard_rank` of `shard_world` owns the
+ * geometry layers k with (k / VOL_SLAB) % shard_world == shard_rank, and the r*VOL_SLAB colour layers under each */
+#define VOL_SLAB 8
+
+typedef struct vol vol_t;   /* opaque; owns (or borrows) the two device buffers */
+
+typedef struct {
+    float   sigma_m;        /* colour distance gate sigma, metres; <= 0 selects the paper's 0.020 */
+    float   gate;           /* weight gate factor; <= 0 selects the paper's 0.8 */
+    void   *geo_dev;        /* DEVICE, optional caller-owned storage of info.geo_bytes (e.g. a torch tensor); NULL = library allocates */
+    void   *col_dev;        /* DEVICE, optional caller-owned storage of info.col_bytes */
+    int32_t device;         /* CUDA device ordinal; < 0 = current device */
+    int32_t shard_rank;     /* multi-GPU z-slab sharding; rank 0 of world 1 = whole volume */
+    int32_t shard_world;    /* <= 0 is read as 1 */
+} vol_opts_t;
+
+typedef struct {
+    int32_t  dims_geo[3];   /* full (unsharded) geometry dims Nx, Ny, Nz */
+    int32_t  r;
+    int32_t  dims_col[3];   /* r * dims_geo */
+    int32_t  local_nz_geo;  /* geometry layers stored by this shard (== dims_geo[2] when unsharded) */
+    float    voxel_geo_m, voxel_col_m;
+    float    origin_m[3], extent_m, trunc_mu_m, sigma_m, gate;
+    int32_t  w_max, device, shard_rank, shard_world;
+    uint64_t geo_bytes, col_bytes;      /* bytes stored by this shard */
+    void    *geo_dev, *col_dev;         /* DEVICE pointers of this shard's storage */
+} vol_info_t;
+
+/* Per-frame statistics of the last vol_integrate* call.  Tile figures are always valid; the four voxel counters
+ * are only filled when counting is enabled (vol_set_counting), otherwise 0.
+ * A voxel is *read* when the method reaches the load of its stored word (geometry: passes the frustum, non-zero-depth
+ * and truncation tests; colour: passes the sigma gate with a valid view weight) and *changed* when the stored word
+ * differs after the update. */
+typedef struct {
+    uint64_t geo_read, geo_changed, col_read, col_changed;
+    uint32_t tiles_total;   /* geometry tiles owned by this shard */
+    uint32_t tiles_geo;     /* tiles whose TSDF voxels were visited */
+    uint32_t tiles_col;     /* tiles whose colour children were visited */
+    uint32_t blocks_col;    /* colour micro-blocks that survived the second-level cull */
+} vol_stats_t;
+
+/* Create a volume pair.  dims_geo: HOST int32[3] (dims_geo[0] must be a multiple of 4); r in 1..4; origin_m: HOST
+ * float[3], world position of the volume corner; extent_m: side length along x (cubic voxels of extent/dims_geo[0]);
+ * trunc_mu_m > 0; w_max in 1..512 (exactness bound of the fp32 running average); opts nullable.
+ * Both volumes start zeroed.  *out is only written on success. */
+int vol_create(vol_t **out, const int32_t dims_geo[3], int32_t r, const float origin_m[3], float extent_m,
+               float trunc_mu_m, int32_t w_max, const vol_opts_t *opts);
+
+/* Fuse one frame (PAPER.md L91-124 per colour voxel; TSDF per geometry voxel).
+ * depth_u16_dev: DEVICE, wd*hd uint16 millimetres, 0 = invalid; rgb8_dev: DEVICE, wh*hh*3 bytes
+ * interleaved R,G,B; the four matrices are HOST float arrays (see conventions).  Asynchronous on `stream`. */
+int vol_integrate(vol_t *v, const uint16_t *depth_u16_dev, int32_t wd, int32_t hd,
+                  const uint8_t *rgb8_dev, int32_t wh, int32_t hh,
+                  const float T_world_depth[16], const float K_depth[9], const float K_rgb[9],
+                  const float T_depth_rgb[16], void *stream);
+
+/* Same, with HOST frame buffers (ideally pinned): copies both images to library-owned device staging buffers on
+ * `stream`, then runs vol_integrate on them.  The host buffers may be reused once the stream has passed the copies. */
+int vol_integrate_host(vol_t *v, const uint16_t *depth_u16_host, int32_t wd, int32_t hd,
+                       const uint8_t *rgb8_host, int32_t wh, int32_t hh,
+                       const float T_world_depth[16], const float K_depth[9], const float K_rgb[9],
+                       const float T_depth_rgb[16], void *stream);
+
+/* Copy this shard's volumes to HOST buffers of at least info.geo_bytes / info.col_bytes (either may be NULL to skip). */
+int vol_download(const vol_t *v, void *geo_host, size_t geo_bytes, void *col_host, size_t col_bytes, void *stream);
+/* Gather single voxels: geo_idx / col_idx are HOST int64 linear indices into the FULL grids (must be owned by this
+ * shard); the packed words are written to HOST geo_words / col_words.  Used for sampled parity at full size. */
+int vol_download_voxels(const vol_t *v, const int64_t *geo_idx, int64_t n_geo, uint32_t *geo_words,
+                        const int64_t *col_idx, int64_t n_col, uint32_t *col_words, void *stream);
+/* Overwrite this shard's volumes from HOST buffers (resume / test seeding); either may be NULL to skip. */
+int vol_upload(vol_t *v, const void *geo_host, const void *col_host, void *stream);
+/* Zero both volumes (asynchronous). */
+int vol_reset(vol_t *v, void *stream);
+int vol_info(const vol_t *v, vol_info_t *out);
+/* Enable (1) / disable (0) the four voxel counters of vol_stats_t (a separately compiled kernel variant). */
+int vol_set_counting(vol_t *v, int32_t on);
+/* Statistics of the last frame (synchronises `stream`; copies 48 bytes device -> host). */
+int vol_frame_stats(vol_t *v, vol_stats_t *out, void *stream);
+/* Enable per-kernel CUDA-event timing of subsequent vol_integrate calls / read the last frame's kernel times in
+ * milliseconds: ms[0] pre-pass (S1), ms[1] tile classification (S9), ms[2] fused integrate (S2-S8).  Synchronises. */
+int vol_set_profiling(vol_t *v, int32_t on);
+int vol_last_kernel_ms(vol_t *v, float ms[3]);
+/* Number of kernels one vol_integrate call launches. */
+int vol_launches_per_frame(const vol_t *v);
+void vol_destroy(vol_t *v);
+const char *vol_strerror(int code);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* VOLFUSION_H */

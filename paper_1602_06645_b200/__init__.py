@@ -1,0 +1,235 @@
+"""paper_1602_06645_b200 -- B200-native fused TSDF + asymmetrical colour-volume integration (arXiv 1602.06645).
+
+Thin ctypes binding over the C ABI declared in ``include/volfusion.h`` (same names, argument marshalling only:
+every step of the path runs in the sm_100a kernels of ``csrc/``).  PyTorch is used by callers for device memory and
+streams; this module only needs ``data_ptr()`` of CUDA tensors.  There is no CPU fallback: if ``libvolfusion.so`` is
+missing or no CUDA device is usable, calls raise.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_ROOT = os.path.dirname(_HERE)
+_SRC_DIR = os.path.join(_HERE, "csrc")
+_SO = os.path.join(_HERE, "libvolfusion.so")
+_lib = None
+
+VOL_OK, VOL_E_ARG, VOL_E_OOM, VOL_E_CUDA = 0, -1, -2, -3
+VOL_SLAB = 8
+
+NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "--fmad=false", "-std=c++17",
+              "-Xcompiler", "-fPIC,-ffp-contract=off", "-shared"]
+
+EXPORTS = ["vol_create", "vol_integrate", "vol_integrate_host", "vol_download", "vol_download_voxels", "vol_upload",
+           "vol_reset", "vol_info", "vol_set_counting", "vol_frame_stats", "vol_set_profiling", "vol_last_kernel_ms",
+           "vol_launches_per_frame", "vol_destroy", "vol_strerror"]
+
+
+def build(force: bool = False, verbose: bool = False) -> str:
+    """Compile csrc/volfusion.cu for sm_100a into libvolfusion.so (in-tree; nvcc cross-compiles without a GPU)."""
+    srcs = [os.path.join(_SRC_DIR, f) for f in os.listdir(_SRC_DIR)] + [os.path.join(_ROOT, "include", "volfusion.h")]
+    newest = max(os.path.getmtime(s) for s in srcs)
+    if force or not os.path.exists(_SO) or os.path.getmtime(_SO) < newest:
+        nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
+        cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + [os.path.join(_SRC_DIR, "volfusion.cu"), "-o", _SO]
+        subprocess.run(cmd, check=True)
+    return _SO
+
+
+class VolOpts(ctypes.Structure):
+    _fields_ = [("sigma_m", ctypes.c_float), ("gate", ctypes.c_float), ("geo_dev", ctypes.c_void_p),
+                ("col_dev", ctypes.c_void_p), ("device", ctypes.c_int32), ("shard_rank", ctypes.c_int32),
+                ("shard_world", ctypes.c_int32)]
+
+
+class VolInfo(ctypes.Structure):
+    _fields_ = [("dims_geo", ctypes.c_int32 * 3), ("r", ctypes.c_int32), ("dims_col", ctypes.c_int32 * 3),
+                ("local_nz_geo", ctypes.c_int32), ("voxel_geo_m", ctypes.c_float), ("voxel_col_m", ctypes.c_float),
+                ("origin_m", ctypes.c_float * 3), ("extent_m", ctypes.c_float), ("trunc_mu_m", ctypes.c_float),
+                ("sigma_m", ctypes.c_float), ("gate", ctypes.c_float), ("w_max", ctypes.c_int32),
+                ("device", ctypes.c_int32), ("shard_rank", ctypes.c_int32), ("shard_world", ctypes.c_int32),
+                ("geo_bytes", ctypes.c_uint64), ("col_bytes", ctypes.c_uint64), ("geo_dev", ctypes.c_void_p),
+                ("col_dev", ctypes.c_void_p)]
+
+
+class VolStats(ctypes.Structure):
+    _fields_ = [("geo_read", ctypes.c_uint64), ("geo_changed", ctypes.c_uint64), ("col_read", ctypes.c_uint64),
+                ("col_changed", ctypes.c_uint64), ("tiles_total", ctypes.c_uint32), ("tiles_geo", ctypes.c_uint32),
+                ("tiles_col", ctypes.c_uint32), ("blocks_col", ctypes.c_uint32)]
+
+
+def lib():
+    """Load libvolfusion.so (building it if the sources are newer) and declare the prototypes."""
+    global _lib
+    if _lib is None:
+        build()
+        L = ctypes.CDLL(_SO)
+        P, I32, I64, F = ctypes.c_void_p, ctypes.c_int32, ctypes.c_int64, ctypes.c_float
+        L.vol_create.argtypes = [ctypes.POINTER(P), P, I32, P, F, F, I32, P]
+        L.vol_integrate.argtypes = [P, P, I32, I32, P, I32, I32, P, P, P, P, P]
+        L.vol_integrate_host.argtypes = L.vol_integrate.argtypes
+        L.vol_download.argtypes = [P, P, ctypes.c_size_t, P, ctypes.c_size_t, P]
+        L.vol_download_voxels.argtypes = [P, P, I64, P, P, I64, P, P]
+        L.vol_upload.argtypes = [P, P, P, P]
+        L.vol_reset.argtypes = [P, P]
+        L.vol_info.argtypes = [P, P]
+        L.vol_set_counting.argtypes = [P, I32]
+        L.vol_frame_stats.argtypes = [P, P, P]
+        L.vol_set_profiling.argtypes = [P, I32]
+        L.vol_last_kernel_ms.argtypes = [P, P]
+        L.vol_launches_per_frame.argtypes = [P]
+        L.vol_destroy.argtypes = [P]
+        L.vol_destroy.restype = None
+        L.vol_strerror.argtypes = [ctypes.c_int]
+        L.vol_strerror.restype = ctypes.c_char_p
+        for name in EXPORTS:
+            if name not in ("vol_destroy", "vol_strerror"):
+                getattr(L, name).restype = ctypes.c_int
+        _lib = L
+    return _lib
+
+
+class VolError(RuntimeError):
+    def __init__(self, code: int, where: str):
+        self.code = code
+        super().__init__(f"{where}: {lib().vol_strerror(code).decode()} ({code})")
+
+
+def _check(rc: int, where: str):
+    if rc != VOL_OK:
+        raise VolError(rc, where)
+
+
+def _f32(a, n):
+    a = np.ascontiguousarray(np.asarray(a, dtype=np.float32).reshape(-1))
+    if a.size != n:
+        raise ValueError(f"expected {n} floats, got {a.size}")
+    return a
+
+
+def _dev_ptr(t):
+    """Device pointer of a CUDA tensor (anything with .data_ptr() and .is_cuda) or a raw int address."""
+    if isinstance(t, int):
+        return t
+    if not getattr(t, "is_cuda", False):
+        raise TypeError("expected a CUDA tensor (or an int device address)")
+    if not t.is_contiguous():
+        raise ValueError("CUDA tensor must be contiguous")
+    return t.data_ptr()
+
+
+def _stream_ptr(stream):
+    if stream is None:
+        return None
+    return getattr(stream, "cuda_stream", stream)
+
+
+class Volume:
+    """A geometry (TSDF) volume and its asymmetrical colour volume on one GPU (or one z-slab shard of them)."""
+
+    def __init__(self, dims_geo, r, origin, extent, mu, w_max, sigma=0.0, gate=0.0, device=-1, shard_rank=0,
+                 shard_world=1, geo_dev=None, col_dev=None):
+        self._h = ctypes.c_void_p()
+        dims = (ctypes.c_int32 * 3)(*[int(d) for d in dims_geo])
+        org = (ctypes.c_float * 3)(*[float(x) for x in origin])
+        opts = VolOpts(float(sigma), float(gate), geo_dev, col_dev, int(device), int(shard_rank), int(shard_world))
+        rc = lib().vol_create(ctypes.byref(self._h), dims, int(r), org, float(extent), float(mu), int(w_max), ctypes.byref(opts))
+        if rc != VOL_OK:
+            self._h = ctypes.c_void_p()
+        _check(rc, "vol_create")
+        self.info = self._info()
+
+    def _info(self) -> VolInfo:
+        o = VolInfo()
+        _check(lib().vol_info(self._h, ctypes.byref(o)), "vol_info")
+        return o
+
+    def _mats(self, T_world_depth, K_depth, K_rgb, T_depth_rgb):
+        return (_f32(T_world_depth, 16), _f32(K_depth, 9), _f32(K_rgb, 9), _f32(T_depth_rgb, 16))
+
+    def integrate(self, depth_dev, wd, hd, rgb_dev, wh, hh, T_world_depth, K_depth, K_rgb, T_depth_rgb, stream=None):
+        """vol_integrate: fuse one frame whose images are already resident on the device."""
+        T, Kd, Kh, Tc = self._mats(T_world_depth, K_depth, K_rgb, T_depth_rgb)
+        _check(lib().vol_integrate(self._h, _dev_ptr(depth_dev), wd, hd, _dev_ptr(rgb_dev), wh, hh, T.ctypes.data,
+                                   Kd.ctypes.data, Kh.ctypes.data, Tc.ctypes.data, _stream_ptr(stream)), "vol_integrate")
+
+    def integrate_host(self, depth, rgb, T_world_depth, K_depth, K_rgb, T_depth_rgb, stream=None):
+        """vol_integrate_host: images are host arrays (numpy uint16 [hd,wd] / uint8 [hh,wh,3], or pinned CPU tensors)."""
+        T, Kd, Kh, Tc = self._mats(T_world_depth, K_depth, K_rgb, T_depth_rgb)
+        if isinstance(depth, np.ndarray):
+            assert depth.dtype == np.uint16 and depth.flags.c_contiguous and rgb.dtype == np.uint8 and rgb.flags.c_contiguous
+            dp, cp = depth.ctypes.data, rgb.ctypes.data
+        else:                                           # CPU torch tensors (pinned)
+            assert not depth.is_cuda and not rgb.is_cuda and depth.is_contiguous() and rgb.is_contiguous()
+            dp, cp = depth.data_ptr(), rgb.data_ptr()
+        hd, wd = int(depth.shape[0]), int(depth.shape[1])
+        hh, wh = int(rgb.shape[0]), int(rgb.shape[1])
+        _check(lib().vol_integrate_host(self._h, dp, wd, hd, cp, wh, hh, T.ctypes.data, Kd.ctypes.data, Kh.ctypes.data,
+                                        Tc.ctypes.data, _stream_ptr(stream)), "vol_integrate_host")
+
+    def download(self, stream=None):
+        """vol_download: (geo uint32 [local_nz, Ny, Nx], col uint32 [r*local_nz, r*Ny, r*Nx]) of this shard."""
+        i = self.info
+        geo = np.empty((i.local_nz_geo, i.dims_geo[1], i.dims_geo[0]), dtype=np.uint32)
+        col = np.empty((i.local_nz_geo * i.r, i.dims_col[1], i.dims_col[0]), dtype=np.uint32)
+        _check(lib().vol_download(self._h, geo.ctypes.data, geo.nbytes, col.ctypes.data, col.nbytes, _stream_ptr(stream)), "vol_download")
+        return geo, col
+
+    def download_voxels(self, geo_idx, col_idx, stream=None):
+        geo_idx = np.ascontiguousarray(geo_idx, dtype=np.int64)
+        col_idx = np.ascontiguousarray(col_idx, dtype=np.int64)
+        gw, cw = np.empty(geo_idx.size, np.uint32), np.empty(col_idx.size, np.uint32)
+        _check(lib().vol_download_voxels(self._h, geo_idx.ctypes.data, geo_idx.size, gw.ctypes.data, col_idx.ctypes.data,
+                                         col_idx.size, cw.ctypes.data, _stream_ptr(stream)), "vol_download_voxels")
+        return gw, cw
+
+    def upload(self, geo=None, col=None, stream=None):
+        for a, nb in ((geo, self.info.geo_bytes), (col, self.info.col_bytes)):
+            if a is not None:
+                assert a.dtype == np.uint32 and a.flags.c_contiguous and a.nbytes == nb
+        _check(lib().vol_upload(self._h, None if geo is None else geo.ctypes.data, None if col is None else col.ctypes.data,
+                                _stream_ptr(stream)), "vol_upload")
+
+    def reset(self, stream=None):
+        _check(lib().vol_reset(self._h, _stream_ptr(stream)), "vol_reset")
+
+    def set_counting(self, on: bool):
+        _check(lib().vol_set_counting(self._h, int(on)), "vol_set_counting")
+
+    def frame_stats(self, stream=None) -> VolStats:
+        s = VolStats()
+        _check(lib().vol_frame_stats(self._h, ctypes.byref(s), _stream_ptr(stream)), "vol_frame_stats")
+        return s
+
+    def set_profiling(self, on: bool):
+        _check(lib().vol_set_profiling(self._h, int(on)), "vol_set_profiling")
+
+    def last_kernel_ms(self):
+        ms = (ctypes.c_float * 3)()
+        _check(lib().vol_last_kernel_ms(self._h, ms), "vol_last_kernel_ms")
+        return [float(x) for x in ms]
+
+    def launches_per_frame(self) -> int:
+        return int(lib().vol_launches_per_frame(self._h))
+
+    def close(self):
+        if getattr(self, "_h", None) is not None and self._h:
+            lib().vol_destroy(self._h)
+            self._h = ctypes.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *a):
+        self.close()

@@ -1,0 +1,119 @@
+// params.cuh -- per-frame constants (S0) and shared device helpers of the fused integration kernels.
+//
+// Canonical arithmetic: every per-voxel decision is taken in IEEE binary32
+// with an explicit operation order -- __fmaf_rn where the method fuses, __fmul_rn/__fadd_rn elsewhere (never
+// contracted by the compiler), correctly rounded __frcp_rn/__fdiv_rn/__fsqrt_rn, floorf for the pixel rounding
+// (reading A2).  The file is compiled with --fmad=false as a second line of defence.
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+namespace vf {
+
+// geometry tile (the culling / work unit): TX x TY x TZ geometry voxels and their r^3 colour children
+constexpr int TX = 32, TY = 4, TZ = 8;
+constexpr int TILE_VOX = TX * TY * TZ;          // 1024
+constexpr int CTA = 256;                        // threads per CTA of the fused kernel; one 16-byte vector each
+static_assert(TILE_VOX == CTA * 4, "one uint4 of geometry voxels per thread");
+// colour micro-block (second-level cull unit, one warp): 16 x 4 x 2 colour voxels = 32 lanes x uint4
+constexpr int MBX = 16, MBY = 4, MBZ = 2;
+constexpr int MAX_MB = (4 * TX / MBX) * (4 * TY / MBY) * (4 * TZ / MBZ);   // r = 4: 512
+
+struct Params {
+    // volume (fixed at vol_create)
+    int   nx, ny, nz;            // full geometry dims
+    int   r;
+    int   cnx, cny;              // colour dims x, y (= r * nx, r * ny)
+    int   local_nz;              // geometry layers stored by this shard
+    int   tiles_x, tiles_y, tiles_z_local, n_tiles;
+    int   shard_rank, shard_world;
+    float ox, oy, oz;            // volume corner (world)
+    float vs, vc;                // geometry / colour voxel size
+    float mu, neg_mu, inv_mu, sig2, sigma, gate;
+    int   w_max;
+    // frame (S0: computed on the host in fp64, rounded once)
+    float R[9], t[3];            // (R_n, t_n) of eq. 5: world -> depth camera
+    float Rc[9], tc[3];          // (R_calib, t_calib) of eq. 3: depth camera -> HD camera
+    float fx, fy, cx, cy;        // K_c
+    float fxh, fyh, cxh, cyh;    // K_hd
+    int   wd, hd, wh, hh;
+    float wd_f, hd_f, wh_f, hh_f;
+    // conservative half extents (camera axes) of a tile / a micro-block, for culling only
+    float tile_ex, tile_ey, tile_ez;
+    float mb_ex, mb_ey, mb_ez;
+    // device buffers
+    const uint16_t *depth;
+    const uint8_t  *rgb;
+    uint32_t *geo;               // this shard's geometry words
+    uint32_t *col;               // this shard's colour words
+    float4   *pixmap;            // S1 output: {X_vd, Y_vd, Z_vd, W} per depth pixel; W = 0 when no colour update is possible
+    uint32_t *pyr;               // min/max valid-depth pyramid: entry = min_mm | max_mm << 16 (0xffff / 0 = empty)
+    int       pyr_off[12], pyr_w[12], pyr_h[12], pyr_levels;
+    uint32_t *work;              // tile work list: colour-flagged tiles from the front, geometry-only tiles from the back
+    uint32_t *ctrl;              // control words, see CTRL_* below
+    unsigned long long *counters;// 4 voxel counters (counting variant only)
+};
+
+enum { CTRL_FRONT = 0, CTRL_BACK = 1, CTRL_CURSOR = 2, CTRL_TICKET = 3, CTRL_BLOCKS_COL = 4, CTRL_N = 8 };
+constexpr uint32_t ITEM_GEO = 1u << 30, ITEM_COL = 1u << 31, ITEM_ID = (1u << 30) - 1u;
+
+// geometry layer (local storage index) -> global layer; slabs of VOL_SLAB = TZ layers are dealt round-robin to ranks
+__device__ __forceinline__ int local_to_global_tz(const Params &p, int tz_local) { return tz_local * p.shard_world + p.shard_rank; }
+
+// eq. 1 / eq. 6: pinhole projection + nearest pixel (A2) + frustum test (A3) in the canonical order.
+__device__ __forceinline__ bool project_px(float fx, float fy, float cx, float cy, float wf, float hf,
+                                           float X, float Y, float Z, int &x, int &y)
+{
+    if (!(Z > 0.0f)) return false;
+    const float iz = __frcp_rn(Z);
+    const float u = __fmaf_rn(fx, __fmul_rn(X, iz), cx);
+    const float v = __fmaf_rn(fy, __fmul_rn(Y, iz), cy);
+    const float uf = floorf(__fadd_rn(u, 0.5f));
+    const float vf = floorf(__fadd_rn(v, 0.5f));
+    if (!(uf >= 0.0f && uf < wf && vf >= 0.0f && vf < hf)) return false;
+    x = (int)uf; y = (int)vf;
+    return true;
+}
+
+// min/max valid depth (mm) over the inclusive pixel rectangle [x0,x1] x [y0,y1] (already clamped to the image),
+// from the coarsest-needed pyramid level: at most 3 x 3 entries are read.
+__device__ __forceinline__ void depth_range(const Params &p, int x0, int x1, int y0, int y1, uint32_t &mn, uint32_t &mx)
+{
+    int l = 0;
+    while (l + 1 < p.pyr_levels && (((x1 >> (3 + l)) - (x0 >> (3 + l))) > 2 || ((y1 >> (3 + l)) - (y0 >> (3 + l))) > 2)) ++l;
+    const int bx0 = x0 >> (3 + l), bx1 = x1 >> (3 + l), by0 = y0 >> (3 + l), by1 = y1 >> (3 + l);
+    mn = 0xffffu; mx = 0u;
+    const uint32_t *lev = p.pyr + p.pyr_off[l];
+    const int lw = p.pyr_w[l];
+    for (int by = by0; by <= by1; ++by)
+        for (int bx = bx0; bx <= bx1; ++bx) {
+            const uint32_t e = __ldg(lev + by * lw + bx);
+            mn = min(mn, e & 0xffffu); mx = max(mx, e >> 16);
+        }
+}
+
+// Conservative pixel rectangle of a camera-space box (centre c, half extents e).  Returns false if the box cannot
+// project into the image.  A box that straddles the camera plane gets the whole image.
+__device__ __forceinline__ bool box_rect(const Params &p, float cX, float cY, float cZ, float eX, float eY, float eZ,
+                                         int &x0, int &x1, int &y0, int &y1, float &zmin, float &zmax)
+{
+    zmin = cZ - eZ; zmax = cZ + eZ;
+    if (!(zmax > 0.0f)) return false;
+    if (zmin > 0.02f) {
+        const float i0 = 1.0f / zmin, i1 = 1.0f / zmax;
+        const float xa = cX - eX, xb = cX + eX, ya = cY - eY, yb = cY + eY;
+        const float umin = p.cx + p.fx * (xa >= 0.0f ? xa * i1 : xa * i0);
+        const float umax = p.cx + p.fx * (xb >= 0.0f ? xb * i0 : xb * i1);
+        const float vmin = p.cy + p.fy * (ya >= 0.0f ? ya * i1 : ya * i0);
+        const float vmax = p.cy + p.fy * (yb >= 0.0f ? yb * i0 : yb * i1);
+        if (!(umax >= -2.0f && umin <= p.wd_f + 1.0f && vmax >= -2.0f && vmin <= p.hd_f + 1.0f)) return false;
+        x0 = max(0, (int)floorf(fmaxf(umin, -4.0f)) - 1); x1 = min(p.wd - 1, (int)ceilf(fminf(umax, p.wd_f + 4.0f)) + 1);
+        y0 = max(0, (int)floorf(fmaxf(vmin, -4.0f)) - 1); y1 = min(p.hd - 1, (int)ceilf(fminf(vmax, p.hd_f + 4.0f)) + 1);
+        if (x0 > x1 || y0 > y1) return false;
+    } else {
+        x0 = 0; x1 = p.wd - 1; y0 = 0; y1 = p.hd - 1;
+    }
+    return true;
+}
+
+}  // namespace vf

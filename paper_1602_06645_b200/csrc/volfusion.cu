@@ -1,0 +1,421 @@
+// volfusion.cu -- C ABI (include/volfusion.h) and host side (S0, launches) of the fused integration.
+//
+// Build: nvcc -gencode arch=compute_100a,code=sm_100a -O3 -lineinfo --fmad=false -Xcompiler -fPIC,-ffp-contract=off
+//             -shared volfusion.cu -o libvolfusion.so
+#include "../../include/volfusion.h"
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "fused.cuh"
+#include "params.cuh"
+#include "prepass.cuh"
+
+using vf::Params;
+
+static char g_err[256] = "";
+
+#define CK(call)                                                                                         \
+    do {                                                                                                 \
+        cudaError_t e_ = (call);                                                                         \
+        if (e_ != cudaSuccess) {                                                                         \
+            snprintf(g_err, sizeof g_err, "%s:%d %s: %s", __FILE__, __LINE__, #call, cudaGetErrorString(e_)); \
+            return e_ == cudaErrorMemoryAllocation ? VOL_E_OOM : VOL_E_CUDA;                             \
+        }                                                                                                \
+    } while (0)
+
+struct vol {
+    Params p;                       // volume fields filled at create; frame fields per call
+    int device;
+    bool own_geo, own_col;
+    size_t geo_bytes, col_bytes;
+    // per-frame-size scratch
+    int scratch_wd, scratch_hd;
+    size_t pyr_entries;
+    // staging for vol_integrate_host
+    uint16_t *stage_depth; size_t stage_depth_bytes;
+    uint8_t *stage_rgb; size_t stage_rgb_bytes;
+    // fused-kernel launch shape
+    int n_sms, fused_blocks;
+    bool counting, profiling;
+    cudaEvent_t ev[4];
+    bool ev_valid;
+};
+
+static int set_device(const vol *v) { CK(cudaSetDevice(v->device)); return VOL_OK; }
+
+// rigid inverse in fp64 with left-to-right sums, rounded once to fp32 (S0).  Returns false if T is not rigid.
+static bool rigid_inverse(const float T[16], float Rout[9], float tout[3])
+{
+    if (T[12] != 0.0f || T[13] != 0.0f || T[14] != 0.0f || T[15] != 1.0f) return false;
+    for (int i = 0; i < 16; ++i) if (!std::isfinite(T[i])) return false;
+    for (int i = 0; i < 3; ++i)
+        for (int j = 0; j < 3; ++j) {
+            double s = 0.0;
+            for (int k = 0; k < 3; ++k) s += (double)T[4 * k + i] * (double)T[4 * k + j];
+            if (std::fabs(s - (i == j ? 1.0 : 0.0)) > 1e-3) return false;
+        }
+    const double det = (double)T[0] * ((double)T[5] * T[10] - (double)T[6] * T[9]) - (double)T[1] * ((double)T[4] * T[10] - (double)T[6] * T[8]) +
+                       (double)T[2] * ((double)T[4] * T[9] - (double)T[5] * T[8]);
+    if (!(det > 0.0)) return false;
+    for (int i = 0; i < 3; ++i) {
+        for (int j = 0; j < 3; ++j) Rout[3 * i + j] = T[4 * j + i];
+        double s = (double)T[4 * 0 + i] * (double)T[4 * 0 + 3];
+        s = s + (double)T[4 * 1 + i] * (double)T[4 * 1 + 3];
+        s = s + (double)T[4 * 2 + i] * (double)T[4 * 2 + 3];
+        tout[i] = (float)(-s);
+    }
+    return true;
+}
+
+static bool intrinsics_ok(const float K[9])
+{
+    for (int i = 0; i < 9; ++i) if (!std::isfinite(K[i])) return false;
+    return K[0] > 0.0f && K[4] > 0.0f && K[1] == 0.0f && K[3] == 0.0f && K[6] == 0.0f && K[7] == 0.0f && K[8] == 1.0f;
+}
+
+// conservative camera-axis half extents of a world-axis box with half sizes (hx, hy, hz)
+static void box_extents(const float R[9], double hx, double hy, double hz, double slack, float &ex, float &ey, float &ez)
+{
+    ex = (float)(std::fabs(R[0]) * hx + std::fabs(R[1]) * hy + std::fabs(R[2]) * hz + slack);
+    ey = (float)(std::fabs(R[3]) * hx + std::fabs(R[4]) * hy + std::fabs(R[5]) * hz + slack);
+    ez = (float)(std::fabs(R[6]) * hx + std::fabs(R[7]) * hy + std::fabs(R[8]) * hz + slack);
+}
+
+extern "C" const char *vol_strerror(int code)
+{
+    switch (code) {
+        case VOL_OK: return "ok";
+        case VOL_E_ARG: return "invalid argument";
+        case VOL_E_OOM: return g_err[0] ? g_err : "out of device memory";
+        case VOL_E_CUDA: return g_err[0] ? g_err : "CUDA error";
+        default: return "unknown error code";
+    }
+}
+
+extern "C" int vol_create(vol_t **out, const int32_t dims_geo[3], int32_t r, const float origin_m[3], float extent_m,
+                          float trunc_mu_m, int32_t w_max, const vol_opts_t *opts)
+{
+    if (!out || !dims_geo || !origin_m) return VOL_E_ARG;
+    if (dims_geo[0] <= 0 || dims_geo[1] <= 0 || dims_geo[2] <= 0 || dims_geo[0] % 4 != 0) return VOL_E_ARG;
+    if (r < 1 || r > 4 || !(extent_m > 0.0f) || !(trunc_mu_m > 0.0f) || w_max < 1 || w_max > 512) return VOL_E_ARG;
+    if (!std::isfinite(extent_m) || !std::isfinite(trunc_mu_m)) return VOL_E_ARG;
+    for (int i = 0; i < 3; ++i) if (!std::isfinite(origin_m[i])) return VOL_E_ARG;
+    if ((int64_t)dims_geo[0] * r > INT32_MAX / 4 || (int64_t)dims_geo[1] * r > INT32_MAX / 4 || (int64_t)dims_geo[2] * r > INT32_MAX / 4) return VOL_E_ARG;
+    int rank = 0, world = 1, device = -1;
+    float sigma = 0.020f, gate = 0.8f;
+    if (opts) {
+        if (opts->sigma_m > 0.0f) sigma = opts->sigma_m;
+        if (opts->gate > 0.0f) gate = opts->gate;
+        world = opts->shard_world > 0 ? opts->shard_world : 1;
+        rank = opts->shard_rank;
+        device = opts->device;
+        if (rank < 0 || rank >= world) return VOL_E_ARG;
+    }
+    if (device < 0) CK(cudaGetDevice(&device));
+    CK(cudaSetDevice(device));
+
+    vol *v = new (std::nothrow) vol();
+    if (!v) return VOL_E_OOM;
+    memset(v, 0, sizeof *v);
+    v->device = device;
+    Params &p = v->p;
+    p.nx = dims_geo[0]; p.ny = dims_geo[1]; p.nz = dims_geo[2]; p.r = r;
+    p.cnx = r * p.nx; p.cny = r * p.ny;
+    p.shard_rank = rank; p.shard_world = world;
+    const int slabs = (p.nz + vf::TZ - 1) / vf::TZ;
+    const int my_slabs = slabs > rank ? (slabs - rank + world - 1) / world : 0;
+    // stored layers: full slabs except a possibly partial last global slab
+    int local_nz = 0;
+    for (int s = 0; s < my_slabs; ++s) {
+        const int g = s * world + rank;
+        local_nz += (g + 1) * vf::TZ <= p.nz ? vf::TZ : p.nz - g * vf::TZ;
+    }
+    p.local_nz = local_nz;
+    p.tiles_x = (p.nx + vf::TX - 1) / vf::TX; p.tiles_y = (p.ny + vf::TY - 1) / vf::TY; p.tiles_z_local = my_slabs;
+    const int64_t n_tiles = (int64_t)p.tiles_x * p.tiles_y * my_slabs;
+    if (n_tiles >= (int64_t)vf::ITEM_ID) { delete v; return VOL_E_ARG; }
+    p.n_tiles = (int)n_tiles;
+    p.ox = origin_m[0]; p.oy = origin_m[1]; p.oz = origin_m[2];
+    p.vs = extent_m / (float)p.nx;
+    p.vc = p.vs / (float)r;
+    p.mu = trunc_mu_m; p.neg_mu = -trunc_mu_m; p.inv_mu = 1.0f / trunc_mu_m;
+    p.sigma = sigma; p.sig2 = sigma * sigma; p.gate = gate; p.w_max = w_max;
+    v->geo_bytes = (size_t)local_nz * p.ny * p.nx * 4u;
+    v->col_bytes = (size_t)local_nz * r * p.cny * p.cnx * 4u;
+
+    int rc = VOL_OK;
+    auto fail = [&](int code) { vol_destroy(v); return code; };
+    if (opts && opts->geo_dev) p.geo = (uint32_t *)opts->geo_dev;
+    else if (v->geo_bytes) {
+        if (cudaMalloc(&p.geo, v->geo_bytes) != cudaSuccess) { cudaGetLastError(); snprintf(g_err, sizeof g_err, "cudaMalloc(%zu) geometry volume failed", v->geo_bytes); return fail(VOL_E_OOM); }
+        v->own_geo = true;
+    }
+    if (opts && opts->col_dev) p.col = (uint32_t *)opts->col_dev;
+    else if (v->col_bytes) {
+        if (cudaMalloc(&p.col, v->col_bytes) != cudaSuccess) { cudaGetLastError(); snprintf(g_err, sizeof g_err, "cudaMalloc(%zu) colour volume failed", v->col_bytes); return fail(VOL_E_OOM); }
+        v->own_col = true;
+    }
+    if (((uintptr_t)p.geo | (uintptr_t)p.col) & 15u) return fail(VOL_E_ARG);       // 16-byte vector access
+    if (v->geo_bytes && cudaMemset(p.geo, 0, v->geo_bytes) != cudaSuccess) rc = VOL_E_CUDA;
+    if (v->col_bytes && cudaMemset(p.col, 0, v->col_bytes) != cudaSuccess) rc = VOL_E_CUDA;
+    if (cudaMalloc(&p.work, sizeof(uint32_t) * (size_t)(p.n_tiles > 0 ? p.n_tiles : 1)) != cudaSuccess) rc = VOL_E_OOM;
+    if (cudaMalloc(&p.ctrl, sizeof(uint32_t) * vf::CTRL_N) != cudaSuccess) rc = VOL_E_OOM;
+    if (cudaMalloc(&p.counters, sizeof(unsigned long long) * 4) != cudaSuccess) rc = VOL_E_OOM;
+    if (rc == VOL_OK && cudaMemset(p.ctrl, 0, sizeof(uint32_t) * vf::CTRL_N) != cudaSuccess) rc = VOL_E_CUDA;
+    if (rc == VOL_OK && cudaMemset(p.counters, 0, sizeof(unsigned long long) * 4) != cudaSuccess) rc = VOL_E_CUDA;
+    if (rc != VOL_OK) { cudaGetLastError(); return fail(rc); }
+
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) return fail(VOL_E_CUDA);
+    v->n_sms = prop.multiProcessorCount;
+    int occ = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, vf::k_fused<false>, vf::CTA, 0) != cudaSuccess || occ < 1) {
+        snprintf(g_err, sizeof g_err, "fused kernel cannot be resident on device %d (built for sm_100a): %s", device, cudaGetErrorString(cudaGetLastError()));
+        return fail(VOL_E_CUDA);
+    }
+    v->fused_blocks = v->n_sms * occ;
+    for (int i = 0; i < 4; ++i) if (cudaEventCreate(&v->ev[i]) != cudaSuccess) return fail(VOL_E_CUDA);
+    v->ev_valid = false;
+    if (cudaDeviceSynchronize() != cudaSuccess) return fail(VOL_E_CUDA);
+    *out = v;
+    return VOL_OK;
+}
+
+extern "C" void vol_destroy(vol_t *v)
+{
+    if (!v) return;
+    cudaSetDevice(v->device);
+    cudaDeviceSynchronize();
+    if (v->own_geo && v->p.geo) cudaFree(v->p.geo);
+    if (v->own_col && v->p.col) cudaFree(v->p.col);
+    if (v->p.work) cudaFree(v->p.work);
+    if (v->p.ctrl) cudaFree(v->p.ctrl);
+    if (v->p.counters) cudaFree(v->p.counters);
+    if (v->p.pixmap) cudaFree(v->p.pixmap);
+    if (v->p.pyr) cudaFree(v->p.pyr);
+    if (v->stage_depth) cudaFree(v->stage_depth);
+    if (v->stage_rgb) cudaFree(v->stage_rgb);
+    for (int i = 0; i < 4; ++i) if (v->ev[i]) cudaEventDestroy(v->ev[i]);
+    cudaGetLastError();
+    delete v;
+}
+
+// (re)allocate the per-frame-size scratch: pixel map + depth pyramid
+static int ensure_scratch(vol *v, int wd, int hd)
+{
+    if (v->scratch_wd == wd && v->scratch_hd == hd && v->p.pixmap) return VOL_OK;
+    Params &p = v->p;
+    if (p.pixmap) { CK(cudaDeviceSynchronize()); cudaFree(p.pixmap); p.pixmap = nullptr; }
+    if (p.pyr) { cudaFree(p.pyr); p.pyr = nullptr; }
+    CK(cudaMalloc(&p.pixmap, sizeof(float4) * (size_t)wd * hd));
+    int l = 0; size_t off = 0;
+    for (;; ++l) {
+        if (l >= 12) return VOL_E_ARG;                       // image larger than 16384 x 16384
+        const int bs = 8 << l;
+        p.pyr_w[l] = (wd + bs - 1) / bs; p.pyr_h[l] = (hd + bs - 1) / bs; p.pyr_off[l] = (int)off;
+        off += (size_t)p.pyr_w[l] * p.pyr_h[l];
+        if (p.pyr_w[l] == 1 && p.pyr_h[l] == 1) break;
+    }
+    p.pyr_levels = l + 1;
+    v->pyr_entries = off;
+    CK(cudaMalloc(&p.pyr, sizeof(uint32_t) * off));
+    v->scratch_wd = wd; v->scratch_hd = hd;
+    return VOL_OK;
+}
+
+extern "C" int vol_integrate(vol_t *v, const uint16_t *depth_u16_dev, int32_t wd, int32_t hd, const uint8_t *rgb8_dev,
+                             int32_t wh, int32_t hh, const float T_world_depth[16], const float K_depth[9],
+                             const float K_rgb[9], const float T_depth_rgb[16], void *stream)
+{
+    if (!v || !depth_u16_dev || !rgb8_dev || !T_world_depth || !K_depth || !K_rgb || !T_depth_rgb) return VOL_E_ARG;
+    if (wd <= 0 || hd <= 0 || wh <= 0 || hh <= 0 || wd > 16384 || hd > 16384 || wh > 16384 || hh > 16384) return VOL_E_ARG;
+    if (!intrinsics_ok(K_depth) || !intrinsics_ok(K_rgb)) return VOL_E_ARG;
+    Params p = v->p;
+    if (!rigid_inverse(T_world_depth, p.R, p.t) || !rigid_inverse(T_depth_rgb, p.Rc, p.tc)) return VOL_E_ARG;
+    int rc = set_device(v); if (rc) return rc;
+    rc = ensure_scratch(v, wd, hd); if (rc) return rc;
+    p = v->p;                                                  // scratch pointers / pyramid shape
+    rigid_inverse(T_world_depth, p.R, p.t); rigid_inverse(T_depth_rgb, p.Rc, p.tc);
+    p.fx = K_depth[0]; p.fy = K_depth[4]; p.cx = K_depth[2]; p.cy = K_depth[5];
+    p.fxh = K_rgb[0]; p.fyh = K_rgb[4]; p.cxh = K_rgb[2]; p.cyh = K_rgb[5];
+    p.wd = wd; p.hd = hd; p.wh = wh; p.hh = hh;
+    p.wd_f = (float)wd; p.hd_f = (float)hd; p.wh_f = (float)wh; p.hh_f = (float)hh;
+    p.depth = depth_u16_dev; p.rgb = rgb8_dev;
+    // culling extents: half the box + slack for the fp32 evaluation of the box centre
+    const double mag = std::fabs((double)p.t[0]) + std::fabs((double)p.t[1]) + std::fabs((double)p.t[2]) +
+                       std::fabs((double)p.ox) + std::fabs((double)p.oy) + std::fabs((double)p.oz) + (double)p.vs * (p.nx + p.ny + p.nz);
+    const double slack = 1e-4 + 4e-6 * mag;
+    box_extents(p.R, 0.5 * vf::TX * p.vs, 0.5 * vf::TY * p.vs, 0.5 * vf::TZ * p.vs, slack, p.tile_ex, p.tile_ey, p.tile_ez);
+    box_extents(p.R, 0.5 * vf::MBX * p.vc, 0.5 * vf::MBY * p.vc, 0.5 * vf::MBZ * p.vc, slack, p.mb_ex, p.mb_ey, p.mb_ez);
+    if (p.n_tiles == 0) return VOL_OK;
+
+    cudaStream_t s = (cudaStream_t)stream;
+    if (v->counting) CK(cudaMemsetAsync(p.counters, 0, sizeof(unsigned long long) * 4, s));
+    if (v->profiling) CK(cudaEventRecord(v->ev[0], s));
+    const dim3 g0((wd + 31) / 32, (hd + 31) / 32);
+    vf::k_prepass<<<g0, 256, 0, s>>>(p);
+    if (v->profiling) CK(cudaEventRecord(v->ev[1], s));
+    vf::k_classify<<<(p.n_tiles + 255) / 256, 256, 0, s>>>(p);
+    if (v->profiling) CK(cudaEventRecord(v->ev[2], s));
+    if (v->counting) vf::k_fused<true><<<v->fused_blocks, vf::CTA, 0, s>>>(p);
+    else             vf::k_fused<false><<<v->fused_blocks, vf::CTA, 0, s>>>(p);
+    if (v->profiling) { CK(cudaEventRecord(v->ev[3], s)); v->ev_valid = true; }
+    CK(cudaGetLastError());
+    return VOL_OK;
+}
+
+extern "C" int vol_integrate_host(vol_t *v, const uint16_t *depth_u16_host, int32_t wd, int32_t hd, const uint8_t *rgb8_host,
+                                  int32_t wh, int32_t hh, const float T_world_depth[16], const float K_depth[9],
+                                  const float K_rgb[9], const float T_depth_rgb[16], void *stream)
+{
+    if (!v || !depth_u16_host || !rgb8_host) return VOL_E_ARG;
+    if (wd <= 0 || hd <= 0 || wh <= 0 || hh <= 0 || wd > 16384 || hd > 16384 || wh > 16384 || hh > 16384) return VOL_E_ARG;
+    if (!T_world_depth || !K_depth || !K_rgb || !T_depth_rgb || !intrinsics_ok(K_depth) || !intrinsics_ok(K_rgb)) return VOL_E_ARG;
+    float Rt[9], tt[3];
+    if (!rigid_inverse(T_world_depth, Rt, tt) || !rigid_inverse(T_depth_rgb, Rt, tt)) return VOL_E_ARG;
+    int rc = set_device(v); if (rc) return rc;
+    const size_t db = (size_t)wd * hd * sizeof(uint16_t), cb = (size_t)wh * hh * 3;
+    if (v->stage_depth_bytes < db) {
+        if (v->stage_depth) { CK(cudaDeviceSynchronize()); cudaFree(v->stage_depth); v->stage_depth = nullptr; v->stage_depth_bytes = 0; }
+        CK(cudaMalloc(&v->stage_depth, db)); v->stage_depth_bytes = db;
+    }
+    if (v->stage_rgb_bytes < cb) {
+        if (v->stage_rgb) { CK(cudaDeviceSynchronize()); cudaFree(v->stage_rgb); v->stage_rgb = nullptr; v->stage_rgb_bytes = 0; }
+        CK(cudaMalloc(&v->stage_rgb, cb)); v->stage_rgb_bytes = cb;
+    }
+    cudaStream_t s = (cudaStream_t)stream;
+    CK(cudaMemcpyAsync(v->stage_depth, depth_u16_host, db, cudaMemcpyHostToDevice, s));
+    CK(cudaMemcpyAsync(v->stage_rgb, rgb8_host, cb, cudaMemcpyHostToDevice, s));
+    return vol_integrate(v, v->stage_depth, wd, hd, v->stage_rgb, wh, hh, T_world_depth, K_depth, K_rgb, T_depth_rgb, stream);
+}
+
+extern "C" int vol_download(const vol_t *v, void *geo_host, size_t geo_bytes, void *col_host, size_t col_bytes, void *stream)
+{
+    if (!v) return VOL_E_ARG;
+    if ((geo_host && geo_bytes < v->geo_bytes) || (col_host && col_bytes < v->col_bytes)) return VOL_E_ARG;
+    int rc = set_device(v); if (rc) return rc;
+    cudaStream_t s = (cudaStream_t)stream;
+    if (geo_host && v->geo_bytes) CK(cudaMemcpyAsync(geo_host, v->p.geo, v->geo_bytes, cudaMemcpyDeviceToHost, s));
+    if (col_host && v->col_bytes) CK(cudaMemcpyAsync(col_host, v->p.col, v->col_bytes, cudaMemcpyDeviceToHost, s));
+    CK(cudaStreamSynchronize(s));
+    return VOL_OK;
+}
+
+extern "C" int vol_upload(vol_t *v, const void *geo_host, const void *col_host, void *stream)
+{
+    if (!v) return VOL_E_ARG;
+    int rc = set_device(v); if (rc) return rc;
+    cudaStream_t s = (cudaStream_t)stream;
+    if (geo_host && v->geo_bytes) CK(cudaMemcpyAsync(v->p.geo, geo_host, v->geo_bytes, cudaMemcpyHostToDevice, s));
+    if (col_host && v->col_bytes) CK(cudaMemcpyAsync(v->p.col, col_host, v->col_bytes, cudaMemcpyHostToDevice, s));
+    CK(cudaStreamSynchronize(s));
+    return VOL_OK;
+}
+
+extern "C" int vol_reset(vol_t *v, void *stream)
+{
+    if (!v) return VOL_E_ARG;
+    int rc = set_device(v); if (rc) return rc;
+    cudaStream_t s = (cudaStream_t)stream;
+    if (v->geo_bytes) CK(cudaMemsetAsync(v->p.geo, 0, v->geo_bytes, s));
+    if (v->col_bytes) CK(cudaMemsetAsync(v->p.col, 0, v->col_bytes, s));
+    return VOL_OK;
+}
+
+// gather kernel for vol_download_voxels: idx are LOCAL linear indices
+__global__ void k_gather(const uint32_t *__restrict__ src, const long long *__restrict__ idx, long long n, uint32_t *__restrict__ dst)
+{
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) dst[i] = src[idx[i]];
+}
+
+// global linear index of a grid with layers of `scale` x the geometry layers -> this shard's local index (or -1)
+static long long to_local(const vol *v, long long idx, int scale)
+{
+    const Params &p = v->p;
+    const long long nx = (long long)p.nx * scale, ny = (long long)p.ny * scale, nz = (long long)p.nz * scale;
+    if (idx < 0 || idx >= nx * ny * nz) return -1;
+    const long long k = idx / (nx * ny), rem = idx % (nx * ny);
+    const long long slab = k / ((long long)vf::TZ * scale), in = k % ((long long)vf::TZ * scale);
+    if (slab % p.shard_world != p.shard_rank) return -1;
+    return ((slab / p.shard_world) * vf::TZ * scale + in) * nx * ny + rem;
+}
+
+static int gather(const vol *v, const uint32_t *src, const int64_t *idx, int64_t n, int scale, uint32_t *out, cudaStream_t s)
+{
+    if (n == 0) return VOL_OK;
+    long long *h = new (std::nothrow) long long[n];
+    if (!h) return VOL_E_OOM;
+    for (int64_t i = 0; i < n; ++i) { h[i] = to_local(v, idx[i], scale); if (h[i] < 0) { delete[] h; return VOL_E_ARG; } }
+    long long *d_idx = nullptr; uint32_t *d_out = nullptr;
+    int rc = VOL_OK;
+    if (cudaMalloc(&d_idx, sizeof(long long) * n) != cudaSuccess || cudaMalloc(&d_out, sizeof(uint32_t) * n) != cudaSuccess) rc = VOL_E_OOM;
+    if (rc == VOL_OK && cudaMemcpyAsync(d_idx, h, sizeof(long long) * n, cudaMemcpyHostToDevice, s) != cudaSuccess) rc = VOL_E_CUDA;
+    if (rc == VOL_OK) {
+        k_gather<<<(unsigned)((n + 255) / 256), 256, 0, s>>>(src, d_idx, n, d_out);
+        if (cudaMemcpyAsync(out, d_out, sizeof(uint32_t) * n, cudaMemcpyDeviceToHost, s) != cudaSuccess) rc = VOL_E_CUDA;
+        if (cudaStreamSynchronize(s) != cudaSuccess) rc = VOL_E_CUDA;
+    }
+    if (rc != VOL_OK) snprintf(g_err, sizeof g_err, "vol_download_voxels: %s", cudaGetErrorString(cudaGetLastError()));
+    cudaFree(d_idx); cudaFree(d_out); delete[] h;
+    return rc;
+}
+
+extern "C" int vol_download_voxels(const vol_t *v, const int64_t *geo_idx, int64_t n_geo, uint32_t *geo_words,
+                                   const int64_t *col_idx, int64_t n_col, uint32_t *col_words, void *stream)
+{
+    if (!v || n_geo < 0 || n_col < 0 || (n_geo && (!geo_idx || !geo_words)) || (n_col && (!col_idx || !col_words))) return VOL_E_ARG;
+    int rc = set_device(v); if (rc) return rc;
+    rc = gather(v, v->p.geo, geo_idx, n_geo, 1, geo_words, (cudaStream_t)stream); if (rc) return rc;
+    return gather(v, v->p.col, col_idx, n_col, v->p.r, col_words, (cudaStream_t)stream);
+}
+
+extern "C" int vol_info(const vol_t *v, vol_info_t *o)
+{
+    if (!v || !o) return VOL_E_ARG;
+    const Params &p = v->p;
+    memset(o, 0, sizeof *o);
+    o->dims_geo[0] = p.nx; o->dims_geo[1] = p.ny; o->dims_geo[2] = p.nz; o->r = p.r;
+    for (int i = 0; i < 3; ++i) o->dims_col[i] = o->dims_geo[i] * p.r;
+    o->local_nz_geo = p.local_nz; o->voxel_geo_m = p.vs; o->voxel_col_m = p.vc;
+    o->origin_m[0] = p.ox; o->origin_m[1] = p.oy; o->origin_m[2] = p.oz; o->extent_m = p.vs * (float)p.nx;
+    o->trunc_mu_m = p.mu; o->sigma_m = p.sigma; o->gate = p.gate; o->w_max = p.w_max; o->device = v->device;
+    o->shard_rank = p.shard_rank; o->shard_world = p.shard_world;
+    o->geo_bytes = v->geo_bytes; o->col_bytes = v->col_bytes; o->geo_dev = p.geo; o->col_dev = p.col;
+    return VOL_OK;
+}
+
+extern "C" int vol_set_counting(vol_t *v, int32_t on) { if (!v) return VOL_E_ARG; v->counting = on != 0; return VOL_OK; }
+extern "C" int vol_set_profiling(vol_t *v, int32_t on) { if (!v) return VOL_E_ARG; v->profiling = on != 0; v->ev_valid = false; return VOL_OK; }
+extern "C" int vol_launches_per_frame(const vol_t *v) { return v ? 3 : VOL_E_ARG; }
+
+extern "C" int vol_frame_stats(vol_t *v, vol_stats_t *out, void *stream)
+{
+    if (!v || !out) return VOL_E_ARG;
+    int rc = set_device(v); if (rc) return rc;
+    cudaStream_t s = (cudaStream_t)stream;
+    uint32_t ctrl[vf::CTRL_N]; unsigned long long cnt[4];
+    CK(cudaMemcpyAsync(ctrl, v->p.ctrl, sizeof ctrl, cudaMemcpyDeviceToHost, s));
+    CK(cudaMemcpyAsync(cnt, v->p.counters, sizeof cnt, cudaMemcpyDeviceToHost, s));
+    CK(cudaStreamSynchronize(s));
+    memset(out, 0, sizeof *out);
+    if (v->counting) { out->geo_read = cnt[0]; out->geo_changed = cnt[1]; out->col_read = cnt[2]; out->col_changed = cnt[3]; }
+    out->tiles_total = (uint32_t)v->p.n_tiles;
+    out->tiles_col = ctrl[vf::CTRL_FRONT];
+    out->tiles_geo = 0;       // filled below: geometry-flagged tiles = back list + colour tiles that also carry the geometry flag
+    out->blocks_col = ctrl[vf::CTRL_BLOCKS_COL];
+    out->tiles_geo = ctrl[vf::CTRL_BACK] + ctrl[vf::CTRL_FRONT];
+    return VOL_OK;
+}
+
+extern "C" int vol_last_kernel_ms(vol_t *v, float ms[3])
+{
+    if (!v || !ms || !v->ev_valid) return VOL_E_ARG;
+    int rc = set_device(v); if (rc) return rc;
+    CK(cudaEventSynchronize(v->ev[3]));
+    for (int i = 0; i < 3; ++i) CK(cudaEventElapsedTime(&ms[i], v->ev[i], v->ev[i + 1]));
+    return VOL_OK;
+}

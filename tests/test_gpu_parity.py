@@ -1,0 +1,149 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element, same seeded inputs."""
+import numpy as np
+import pytest
+
+import synth
+from parity_util import check_counters, compare_states, integrate_both, make_pair, run_sequence, to_dev
+
+pytestmark = pytest.mark.gpu
+I4 = np.eye(4, dtype=np.float32)
+
+
+def test_cfg1_full_sequence():
+    """Config 1 as specified: 64^3 / 128^3, 5 frames, state and counters checked after every frame."""
+    run_sequence(synth.config(1), range(5))
+
+
+@pytest.mark.parametrize("r", [1, 2, 3, 4])
+def test_cfg1_all_ratios(r):
+    run_sequence(synth.config(1, r=r).scaled(48, r), [0, 2, 4])
+
+
+def test_ragged_dims_and_tail_tiles():
+    """Dims that are not multiples of the tile (32 x 4 x 8) or of the micro-block: ragged tails on every axis."""
+    c = synth.config(1).scaled(40, 3)
+    c.dims_geo = (44, 38, 27)
+    run_sequence(c, [0, 1, 3])
+
+
+def test_cfg2_scaled_orbit():
+    """Config 2's scene, cameras, noise and 2 % dropouts on a 96^3 / 192^3 grid; 6 frames spread over the orbit."""
+    run_sequence(synth.config(2).scaled(96, 2), [0, 17, 34, 51, 68, 99])
+
+
+def test_cfg3_scaled_jittered():
+    run_sequence(synth.config(3).scaled(128, 2), [0, 1, 2, 150, 299])
+
+
+def test_cfg4_scaled_r3():
+    run_sequence(synth.config(4).scaled(64, 3), [0, 50, 100])
+
+
+def test_cfg5_scaled_small_object():
+    """Config 5: 0.5 m cube, mu = 4 mm << sigma = 20 mm, no background: the colour shell dominates."""
+    run_sequence(synth.config(5).scaled(96, 2), [0, 100, 200, 399])
+
+
+def test_weight_saturation_and_gate_many_frames():
+    """Same frame 12 times with w_max = 5: weights saturate, the 0.8 gate closes, stores get skipped."""
+    c = synth.config(1).scaled(32, 2)
+    c.w_max = 5
+    g, o = make_pair(c)
+    depth, rgb, T = synth.frame(c, 2)
+    for n in range(12):
+        st, cnt = integrate_both(g, o, c, depth, rgb, T)
+        check_counters(st, cnt, f"repeat {n}")
+    compare_states(g, o, "saturation")
+
+
+def test_degenerate_frames():
+    """All-zero depth is a no-op; a camera looking away touches nothing; both leave a seeded state untouched."""
+    c = synth.config(1).scaled(32, 2)
+    g, o = make_pair(c)
+    depth, rgb, T = synth.frame(c, 0)
+    integrate_both(g, o, c, depth, rgb, T)
+    before, _ = g.download()
+    st, cnt = integrate_both(g, o, c, np.zeros_like(depth), rgb, T)
+    check_counters(st, cnt)
+    assert st.tiles_geo == 0 and st.tiles_col == 0
+    Tb = I4.copy()
+    Tb[:3, :3] = np.diag([-1, 1, -1]).astype(np.float32)
+    st, cnt = integrate_both(g, o, c, depth, rgb, Tb)
+    check_counters(st, cnt)
+    geo, _ = compare_states(g, o, "degenerate")
+    assert np.array_equal(geo, before)
+
+
+def test_camera_inside_volume_and_near_plane():
+    """Camera inside the volume: tiles straddle the camera plane (Z <= 0 voxels, huge projected rectangles)."""
+    c = synth.config(2).scaled(64, 2)
+    g, o = make_pair(c)
+    T = synth.rigid32(synth.look_at((0.75, 0.6, 0.35), (0, 0, -0.2)))
+    depth, _ = synth.render(c.prims, c.K_depth, T.astype(np.float64), c.wd, c.hd, True, False)
+    depth = synth.quantise_depth(depth, np.random.default_rng(1), c.noise, 0.02)
+    rgb = synth.random_rgb(c.wh, c.hh, 3)
+    st, cnt = integrate_both(g, o, c, depth, rgb, T)
+    check_counters(st, cnt)
+    assert cnt[0] > 1000
+    compare_states(g, o, "inside")
+
+
+def test_host_entry_point_and_upload_roundtrip():
+    """vol_integrate_host (host buffers, copies inside) gives the same state; vol_upload / vol_reset round-trip."""
+    c = synth.config(1).scaled(32, 2)
+    g, o = make_pair(c)
+    for fi in (0, 4):
+        depth, rgb, T = synth.frame(c, fi)
+        g.integrate_host(depth, rgb, T, c.K_depth, c.K_rgb, c.T_depth_rgb)
+        o.integrate(depth, rgb, T, c.K_depth, c.K_rgb, c.T_depth_rgb)
+    geo, col = compare_states(g, o, "host entry")
+    g.reset()
+    z, zc = g.download()
+    assert not z.any() and not zc.any()
+    g.upload(geo, col)
+    compare_states(g, o, "after upload")
+    gi = np.array([0, 5, 32 * 32 * 16 + 77, 32 ** 3 - 1], np.int64)
+    ci = np.array([1, 64 * 64 * 30 + 64 * 31 + 29, 64 ** 3 - 1], np.int64)
+    gw, cw = g.download_voxels(gi, ci)
+    assert np.array_equal(gw, geo.reshape(-1)[gi]) and np.array_equal(cw, col.reshape(-1)[ci])
+
+
+def test_shards_reassemble_to_the_unsharded_volume():
+    """z-slab sharding (VOL_SLAB layers dealt round-robin): two shards run one after the other on this GPU hold exactly
+    the slabs of the unsharded result; no voxel is owned twice or dropped."""
+    import paper_1602_06645_b200 as vf
+    c = synth.config(1).scaled(40, 2)
+    c.dims_geo = (40, 40, 44)                          # 6 slabs, the last one partial
+    g, o = make_pair(c)
+    shards = [vf.Volume(c.dims_geo, c.r, c.origin, c.extent, c.mu, c.w_max, shard_rank=k, shard_world=2) for k in range(2)]
+    for fi in (0, 3):
+        depth, rgb, T = synth.frame(c, fi)
+        integrate_both(g, o, c, depth, rgb, T)
+        dd, dr = to_dev(depth), to_dev(rgb)
+        for s in shards:
+            s.integrate(dd, c.wd, c.hd, dr, c.wh, c.hh, T, c.K_depth, c.K_rgb, c.T_depth_rgb)
+    geo, col = compare_states(g, o, "unsharded")
+    nz, r, S = 44, c.r, vf.VOL_SLAB
+    for k, s in enumerate(shards):
+        sg, sc = s.download()
+        layers = [z for z in range(nz) if (z // S) % 2 == k]
+        assert sg.shape[0] == len(layers)
+        assert np.array_equal(sg, geo[layers])
+        clayers = [z for z in range(nz * r) if (z // (S * r)) % 2 == k]
+        assert np.array_equal(sc, col[clayers])
+
+
+def test_bad_arguments_leave_state_untouched():
+    import paper_1602_06645_b200 as vf
+    c = synth.config(1).scaled(32, 2)
+    g, o = make_pair(c)
+    depth, rgb, T = synth.frame(c, 0)
+    integrate_both(g, o, c, depth, rgb, T)
+    dd, dr = to_dev(depth), to_dev(rgb)
+    Tbad = T.copy(); Tbad[0, 0] = 2.0
+    Kbad = c.K_depth.copy(); Kbad[0, 1] = 0.5
+    for args in ((Tbad, c.K_depth), (T, Kbad)):
+        with pytest.raises(vf.VolError) as e:
+            g.integrate(dd, c.wd, c.hd, dr, c.wh, c.hh, args[0], args[1], c.K_rgb, c.T_depth_rgb)
+        assert e.value.code == vf.VOL_E_ARG
+    compare_states(g, o, "after rejected calls")
