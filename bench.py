@@ -1,0 +1,311 @@
+#!/usr/bin/env python
+"""bench.py -- fused TSDF + colour-volume integration throughput on B200 (one JSON line on stdout).
+
+A *step* is one pass of the whole hot path (S0-S9: pre-pass, tile classification, fused integrate) over one synthetic
+RGB-D frame.  Workload at N = 1: BASELINE.json configs[2] ("cfg3": geometry 512^3 over a 3 m cube, colour 1024^3,
+640x480 depth, 1920x1080 RGB, 20 primitives on a plane, jittered orbit) -- the configuration the 70 % target is quoted on.
+
+  value     whole-job voxel updates/s = (N_geo + N_col) voxels brought up to date per frame x frames / device time,
+            inputs resident in HBM, CUDA events on the launching stream, L2 flushed between timed frames
+  e2e       the same metric through vol_integrate_host (pinned HOST frames copied in, per-frame stats copied out)
+  roofline  fused kernel: algorithmic bytes per launch (4 B x voxels read + 4 B x voxels changed + the two input images)
+            / its mean launch time (CUDA events inside the library), against the measured HBM copy peak
+  cpu_baseline  the CPU oracle, as it stands, on the first full-size frames of the same workload (rank 0, N = 1 only)
+
+N > 1 (torchrun): every rank integrates an independent scan of the same configuration (replicas, no data-path
+collective), value = sum over ranks / max-over-ranks time, "scaling": "weak".
+`--impl reference` times the CPU oracle alone (rank 0), each step a bounded sample of the workload.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import synth  # noqa: E402
+
+METRIC = "fused_voxel_updates_per_s"
+UNIT = "voxel updates/s"
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=30)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--cfg", type=int, default=3, help="BASELINE config number 1..5 (default 3 = the headline workload)")
+    ap.add_argument("--r", type=int, default=None, help="colour/geometry ratio override (config 4 sweep)")
+    ap.add_argument("--no-flush", action="store_true", help="time frames back to back without flushing L2")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--first-frame", type=int, default=0)
+    return ap.parse_args()
+
+
+def peaks():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+def ncu_traffic(workload):
+    """DRAM bytes per fused-kernel launch from the committed ncu --set full capture, if one is recorded."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
+            return json.load(f).get(workload, {}).get("fused_dram_bytes_per_launch")
+    except Exception:
+        return None
+
+
+class ClockSampler(threading.Thread):
+    """nvidia-smi clocks + throttle reasons while the benchmark runs (the profiling recipe's clocks line)."""
+    Q = "clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown," \
+        "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap,utilization.gpu"
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index, self.rows, self.proc = index, [], None
+
+    def run(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            for line in self.proc.stdout:
+                self.rows.append([x.strip() for x in line.split(",")])
+        except Exception:
+            pass
+
+    def stop(self):
+        if self.proc:
+            self.proc.terminate()
+        self.join(timeout=2)
+        sm = [float(r[0]) for r in self.rows if len(r) >= 7 and r[0].replace(".", "").isdigit()]
+        busy = [float(r[0]) for r in self.rows if len(r) >= 7 and r[6].isdigit() and int(r[6]) > 0 and r[0].replace(".", "").isdigit()]
+        mx = [float(r[1]) for r in self.rows if len(r) >= 7 and r[1].replace(".", "").isdigit()]
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = sorted({n for r in self.rows if len(r) >= 7 for n, v in zip(names, r[2:6]) if v.lower().startswith("active")})
+        use = busy or sm
+        return {"sm_mhz": float(np.median(use)) if use else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": reasons, "samples": len(sm), "samples_under_load": len(busy)}
+
+
+def workload_name(c):
+    return (f"{c.name}: geometry {c.dims_geo[0]}^3 over {c.extent} m, colour {c.dims_col[0]}^3 (r={c.r}), depth {c.wd}x{c.hd}, "
+            f"rgb {c.wh}x{c.hh}")
+
+
+def oracle_sample(c, n_frames, slab_layers=None):
+    """Time the CPU oracle (as it stands) on `n_frames` frames.  slab_layers = None: the full volumes; otherwise a central
+    z-slab of that many geometry layers (and r x as many colour layers) -- a bounded sample of the same workload."""
+    import oracle
+    oracle.build()
+    nx, ny, nz = c.dims_geo
+    origin = np.array(c.origin, np.float32)
+    if slab_layers is not None and slab_layers < nz:
+        k0 = (nz - slab_layers) // 2
+        origin = origin.copy()
+        origin[2] += np.float32(k0) * np.float32(c.voxel)
+        dims = (nx, ny, slab_layers)
+        sample = f"central z-slab of {slab_layers}/{nz} geometry layers (and {slab_layers * c.r} colour layers), {n_frames} frames"
+    else:
+        dims = (nx, ny, nz)
+        sample = f"full volumes, first {n_frames} frames"
+    o = oracle.RefVolume(dims, c.r, origin, c.extent, c.mu, c.w_max, sigma=c.sigma, gate=c.gate)
+    o.desc.extent = float(np.float32(c.voxel) * np.float32(nx))
+    nvox = dims[0] * dims[1] * dims[2] * (1 + c.r ** 3)
+    times = []
+    for i in range(n_frames):
+        depth, rgb, T = synth.frame(c, i)
+        t0 = time.perf_counter()
+        o.integrate(depth, rgb, T, c.K_depth, c.K_rgb, c.T_depth_rgb)
+        times.append(time.perf_counter() - t0)
+    return nvox, times, sample
+
+
+def run_reference(args, rank):
+    """--impl reference: the CPU oracle on this box's host cores, rank 0 only; each step = one frame over a z-slab sample."""
+    if rank != 0:
+        return
+    c = synth.config(args.cfg, r=args.r)
+    cores = os.cpu_count() or 1
+    slab = max(8, c.dims_geo[2] // 16)
+    nvox, times, sample = oracle_sample(c, args.warmup + args.steps, slab_layers=slab)
+    t = times[args.warmup:]
+    ms = 1e3 * float(np.mean(t))
+    val = nvox / (ms * 1e-3)
+    out = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+           "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+           "dtype": "f32", "data": "synthetic",
+           "config": {"workload": workload_name(c), "sample_per_step": sample},
+           "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+           "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+           "gpu_launches": 0}
+    print(json.dumps(out), flush=True)
+
+
+def run_ours(args, rank, world, local_rank):
+    import torch
+    import torch.distributed as dist
+
+    import paper_1602_06645_b200 as vf
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- the product path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    c = synth.config(args.cfg, r=args.r)
+    W, K = args.warmup, args.steps
+    nfr = W + K
+    first = args.first_frame + 7 * rank                       # replicas scan different parts of the trajectory
+    sampler = ClockSampler(local_rank) if rank == 0 else None
+    if sampler:
+        sampler.start()
+
+    # ---- inputs: generated once, pinned on the host and resident on the device
+    frames = []
+    for i in range(nfr):
+        depth, rgb, T = synth.frame(c, (first + i) % c.n_frames)
+        hd_, hr_ = torch.from_numpy(depth.view(np.int16)).pin_memory(), torch.from_numpy(rgb).pin_memory()
+        frames.append((hd_, hr_, hd_.cuda(), hr_.cuda(), T))
+    vol = vf.Volume(c.dims_geo, c.r, c.origin, c.extent, c.mu, c.w_max, sigma=c.sigma, gate=c.gate, device=local_rank)
+    stream = torch.cuda.current_stream()
+    flush_buf = torch.empty(512 << 20, dtype=torch.uint8, device="cuda")      # > 126 MB L2
+
+    def integrate_dev(i):
+        _, _, dd, dr, T = frames[i]
+        vol.integrate(dd, c.wd, c.hd, dr, c.wh, c.hh, T, c.K_depth, c.K_rgb, c.T_depth_rgb, stream=stream)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- pass 1 (untimed): per-frame voxel counters of exactly this frame sequence -> algorithmic bytes
+    vol.set_counting(True)
+    counters = []
+    for i in range(nfr):
+        integrate_dev(i)
+        s = vol.frame_stats(stream)
+        counters.append((s.geo_read, s.geo_changed, s.col_read, s.col_changed, s.tiles_geo, s.tiles_col, s.blocks_col))
+    vol.set_counting(False)
+
+    # ---- pass 2 (untimed): per-kernel times of the timed frames (library-side CUDA events on the launching stream)
+    vol.reset(stream)
+    for i in range(W):
+        integrate_dev(i)
+    vol.set_profiling(True)
+    kms = []
+    for i in range(W, nfr):
+        if not args.no_flush:
+            flush_buf.zero_()
+        integrate_dev(i)
+        kms.append(vol.last_kernel_ms())
+    vol.set_profiling(False)
+    kms = np.array(kms)
+
+    # ---- pass 3: THE timed region -- K frames, device-resident inputs, events around every frame, L2 flushed between
+    vol.reset(stream)
+    for i in range(W):
+        integrate_dev(i)
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(K)]
+    barrier()
+    for n, i in enumerate(range(W, nfr)):
+        if not args.no_flush:
+            flush_buf.zero_()
+        ev[n][0].record(stream)
+        integrate_dev(i)
+        ev[n][1].record(stream)
+    barrier()
+    per_frame_ms = np.array([a.elapsed_time(b) for a, b in ev])
+    total_ms = float(per_frame_ms.sum())
+
+    # ---- pass 4: end to end through vol_integrate_host -- pinned host frames in, per-frame stats out, every step
+    vol.reset(stream)
+    for i in range(W):
+        integrate_dev(i)
+    barrier()
+    t0 = torch.cuda.Event(enable_timing=True); t1 = torch.cuda.Event(enable_timing=True)
+    t0.record(stream)
+    for i in range(W, nfr):
+        hd_, hr_, _, _, T = frames[i]
+        vol.integrate_host(hd_, hr_, T, c.K_depth, c.K_rgb, c.T_depth_rgb, stream=stream)
+        vol.frame_stats(stream)                                   # device -> host read of the step's result (synchronises)
+    t1.record(stream)
+    barrier()
+    e2e_ms = float(t0.elapsed_time(t1))
+
+    if world > 1:
+        tt = torch.tensor([total_ms, e2e_ms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        total_ms, e2e_ms = float(tt[0]), float(tt[1])
+    clocks = sampler.stop() if sampler else None
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    nvox = int(np.prod(c.dims_geo)) * (1 + c.r ** 3)
+    ms_per_step = total_ms / K
+    value = world * nvox * K / (total_ms * 1e-3)
+    e2e_value = world * nvox * K / (e2e_ms * 1e-3)
+    cnt = np.array(counters[W:], dtype=np.float64)
+    frame_bytes = c.wd * c.hd * 2 + c.wh * c.hh * 3
+    alg_bytes = 4.0 * cnt[:, :4].sum(axis=1) + frame_bytes        # per fused launch
+    fused_ms = kms[:, 2]
+    peak, peak_src = peaks()
+    achieved = float(alg_bytes.sum() / (fused_ms.sum() * 1e-3) / 1e9)
+    out = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+        "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32", "data": "synthetic",
+        "config": {"workload": workload_name(c), "frames": f"{first}..{first + nfr - 1} of the seeded trajectory",
+                   "l2": "no flush (frames back to back)" if args.no_flush else "L2 flushed (512 MiB memset) between timed frames",
+                   "parallelism": "single GPU" if world == 1 else f"{world} replicas (independent scans), no data-path collective"},
+        "frames_per_s": world * K / (total_ms * 1e-3),
+        "applied_updates_per_s": world * float(cnt[:, 0].sum() + cnt[:, 2].sum()) / (total_ms * 1e-3),
+        "per_frame_ms": {"median": float(np.median(per_frame_ms)), "p95": float(np.percentile(per_frame_ms, 95)), "min": float(per_frame_ms.min())},
+        "kernel_ms_mean": {"prepass": float(kms[:, 0].mean()), "classify": float(kms[:, 1].mean()), "fused": float(fused_ms.mean())},
+        "per_frame_mean": {"geo_read": float(cnt[:, 0].mean()), "geo_changed": float(cnt[:, 1].mean()), "col_read": float(cnt[:, 2].mean()),
+                           "col_changed": float(cnt[:, 3].mean()), "tiles_geo": float(cnt[:, 4].mean()), "tiles_col": float(cnt[:, 5].mean()),
+                           "blocks_col": float(cnt[:, 6].mean()), "algorithmic_bytes": float(alg_bytes.mean())},
+        "roofline": {"bound": "hbm", "kernel": "k_fused", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                     "traffic": ncu_traffic(c.name), "peak_source": peak_src,
+                     "dense_sweep_frac": float(8.0 * nvox / (fused_ms.mean() * 1e-3) / 1e9 / peak)},
+        "e2e": {"value": e2e_value, "unit": UNIT, "ms_per_step": e2e_ms / K, "h2d_bytes_per_step": frame_bytes,
+                "d2h_bytes_per_step": 64},
+        "gpu_launches": vol.launches_per_frame() * K,
+        "clocks": clocks,
+    }
+    if world == 1 and not args.no_cpu_baseline:
+        n = 2 if nvox > 5e8 else (4 if nvox > 5e7 else 5)
+        nv, times, sample = oracle_sample(c, min(n, c.n_frames))
+        out["cpu_baseline"] = {"value": nv * len(times) / sum(times), "unit": UNIT, "cores": os.cpu_count() or 1, "kind": "oracle",
+                               "sample": sample, "ms_per_frame": 1e3 * float(np.mean(times))}
+    print(json.dumps(out), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    args = parse()
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        run_reference(args, rank)
+    else:
+        run_ours(args, rank, world, local_rank)
+
+
+if __name__ == "__main__":
+    main()
