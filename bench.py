@@ -196,7 +196,7 @@ def run_ours(args, rank, world, local_rank):
     for i in range(nfr):
         integrate_dev(i)
         s = vol.frame_stats(stream)
-        counters.append((s.geo_read, s.geo_changed, s.col_read, s.col_changed, s.tiles_geo, s.tiles_col, s.blocks_col))
+        counters.append((s.geo_read, s.geo_changed, s.col_read, s.col_changed, s.tiles_geo, s.items_col, s.cells_col))
     vol.set_counting(False)
 
     # ---- pass 2 (untimed): per-kernel times of the timed frames (library-side CUDA events on the launching stream)
@@ -276,8 +276,8 @@ def run_ours(args, rank, world, local_rank):
         "per_frame_ms": {"median": float(np.median(per_frame_ms)), "p95": float(np.percentile(per_frame_ms, 95)), "min": float(per_frame_ms.min())},
         "kernel_ms_mean": {"prepass": float(kms[:, 0].mean()), "classify": float(kms[:, 1].mean()), "fused": float(fused_ms.mean())},
         "per_frame_mean": {"geo_read": float(cnt[:, 0].mean()), "geo_changed": float(cnt[:, 1].mean()), "col_read": float(cnt[:, 2].mean()),
-                           "col_changed": float(cnt[:, 3].mean()), "tiles_geo": float(cnt[:, 4].mean()), "tiles_col": float(cnt[:, 5].mean()),
-                           "blocks_col": float(cnt[:, 6].mean()), "algorithmic_bytes": float(alg_bytes.mean())},
+                           "col_changed": float(cnt[:, 3].mean()), "tiles_geo": float(cnt[:, 4].mean()), "items_col": float(cnt[:, 5].mean()),
+                           "cells_col": float(cnt[:, 6].mean()), "algorithmic_bytes": float(alg_bytes.mean())},
         "roofline": {"bound": "hbm", "kernel": "k_fused", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                      "traffic": ncu_traffic(c.name), "peak_source": peak_src,
                      "dense_sweep_frac": float(8.0 * nvox / (fused_ms.mean() * 1e-3) / 1e9 / peak)},

@@ -71,16 +71,16 @@ typedef struct {
 } vol_info_t;
 
 /* Per-frame statistics of the last vol_integrate* call.  Tile figures are always valid; the four voxel counters
- * are only filled when counting is enabled (vol_set_counting), otherwise 0.
+ * and cells_col are only filled when counting is enabled (vol_set_counting), otherwise 0.
  * A voxel is *read* when the method reaches the load of its stored word (geometry: passes the frustum, non-zero-depth
  * and truncation tests; colour: passes the sigma gate with a valid view weight) and *changed* when the stored word
  * differs after the update. */
 typedef struct {
     uint64_t geo_read, geo_changed, col_read, col_changed;
     uint32_t tiles_total;   /* geometry tiles owned by this shard */
-    uint32_t tiles_geo;     /* tiles whose TSDF voxels were visited */
-    uint32_t tiles_col;     /* tiles whose colour children were visited */
-    uint32_t blocks_col;    /* colour micro-blocks that survived the second-level cull */
+    uint32_t tiles_geo;     /* geometry tiles (32x4x8 voxels) whose TSDF voxels were visited */
+    uint32_t items_col;     /* colour work items (non-zero shell-mark words) */
+    uint32_t cells_col;     /* colour cells (8x4x4 colour voxels) visited; only when counting is enabled */
 } vol_stats_t;
 
 /* Create a volume pair.  dims_geo: HOST int32[3] (dims_geo[0] must be a multiple of 4); r in 1..4; origin_m: HOST

@@ -60,7 +60,7 @@ class VolInfo(ctypes.Structure):
 class VolStats(ctypes.Structure):
     _fields_ = [("geo_read", ctypes.c_uint64), ("geo_changed", ctypes.c_uint64), ("col_read", ctypes.c_uint64),
                 ("col_changed", ctypes.c_uint64), ("tiles_total", ctypes.c_uint32), ("tiles_geo", ctypes.c_uint32),
-                ("tiles_col", ctypes.c_uint32), ("blocks_col", ctypes.c_uint32)]
+                ("items_col", ctypes.c_uint32), ("cells_col", ctypes.c_uint32)]
 
 
 def lib():

@@ -1,29 +1,35 @@
-// params.cuh -- per-frame constants (S0) and shared device helpers of the fused integration kernels.
+// params.cuh -- per-frame constants (S0), work-list layout and shared device helpers of the integration kernels.
 //
 // Canonical arithmetic: every per-voxel decision is taken in IEEE binary32
 // with an explicit operation order -- __fmaf_rn where the method fuses, __fmul_rn/__fadd_rn elsewhere (never
 // contracted by the compiler), correctly rounded __frcp_rn/__fdiv_rn/__fsqrt_rn, floorf for the pixel rounding
-// (reading A2).  The file is compiled with --fmad=false as a second line of defence.
+// (reading A2).  The file is compiled with --fmad=false as a second line of defence.  Code marked "culling only"
+// is free-form arithmetic with explicit slack: it may only decide that work is skipped when no voxel can pass.
 #pragma once
 #include <cstdint>
 #include <cuda_runtime.h>
 
 namespace vf {
 
-// geometry tile (the culling / work unit): TX x TY x TZ geometry voxels and their r^3 colour children
+// geometry tile (culling / work unit, one warp): TX x TY x TZ geometry voxels = 32 lanes x uint4 x TZ layers
 constexpr int TX = 32, TY = 4, TZ = 8;
-constexpr int TILE_VOX = TX * TY * TZ;          // 1024
-constexpr int CTA = 256;                        // threads per CTA of the fused kernel; one 16-byte vector each
-static_assert(TILE_VOX == CTA * 4, "one uint4 of geometry voxels per thread");
-// colour micro-block (second-level cull unit, one warp): 16 x 4 x 2 colour voxels = 32 lanes x uint4
-constexpr int MBX = 16, MBY = 4, MBZ = 2;
-constexpr int MAX_MB = (4 * TX / MBX) * (4 * TY / MBY) * (4 * TZ / MBZ);   // r = 4: 512
+// colour cell (shell-mark / work unit, one warp pass): 8 x 4 x 4 colour voxels = 32 lanes x uint4
+constexpr int CLX = 8, CLY = 4, CLZ = 4;
+constexpr int WARPS_PER_CTA = 8;
+constexpr int CTA = 32 * WARPS_PER_CTA;
+
+// cells of one tile's colour children per axis, and 32-bit mark words per tile, for ratio r
+__host__ __device__ constexpr int cells_x(int r) { return TX * r / CLX; }   // 4r
+__host__ __device__ constexpr int cells_y(int r) { return TY * r / CLY; }   // r
+__host__ __device__ constexpr int cells_z(int r) { return TZ * r / CLZ; }   // 2r
+__host__ __device__ constexpr int cells_per_tile(int r) { return cells_x(r) * cells_y(r) * cells_z(r); }   // 8 r^3
+__host__ __device__ constexpr int words_per_tile(int r) { return (cells_per_tile(r) + 31) / 32; }          // 1, 2, 7, 16
 
 struct Params {
     // volume (fixed at vol_create)
     int   nx, ny, nz;            // full geometry dims
     int   r;
-    int   cnx, cny;              // colour dims x, y (= r * nx, r * ny)
+    int   cnx, cny, cnz;         // full colour dims
     int   local_nz;              // geometry layers stored by this shard
     int   tiles_x, tiles_y, tiles_z_local, n_tiles;
     int   shard_rank, shard_world;
@@ -38,9 +44,10 @@ struct Params {
     float fxh, fyh, cxh, cyh;    // K_hd
     int   wd, hd, wh, hh;
     float wd_f, hd_f, wh_f, hh_f;
-    // conservative half extents (camera axes) of a tile / a micro-block, for culling only
-    float tile_ex, tile_ey, tile_ez;
-    float mb_ex, mb_ey, mb_ez;
+    // culling only
+    float Rw[9], tw[3];          // depth camera -> world (the caller's T_world_depth)
+    float tile_ex, tile_ey, tile_ez;   // conservative camera-axis half extents of a geometry tile
+    float inv_vc, slack;         // 1 / colour voxel size; metres of slack for fp32 evaluation of culling geometry
     // device buffers
     const uint16_t *depth;
     const uint8_t  *rgb;
@@ -49,15 +56,16 @@ struct Params {
     float4   *pixmap;            // S1 output: {X_vd, Y_vd, Z_vd, W} per depth pixel; W = 0 when no colour update is possible
     uint32_t *pyr;               // min/max valid-depth pyramid: entry = min_mm | max_mm << 16 (0xffff / 0 = empty)
     int       pyr_off[12], pyr_w[12], pyr_h[12], pyr_levels;
-    uint32_t *work;              // tile work list: colour-flagged tiles from the front, geometry-only tiles from the back
+    uint32_t *marks;             // shell marks: words_per_tile(r) words per tile, bit = colour cell that may hold sigma-shell voxels
+    uint32_t *work_geo;          // geometry work list: local tile ids
+    uint32_t *work_col;          // colour work list: indices of non-zero mark words
     uint32_t *ctrl;              // control words, see CTRL_* below
     unsigned long long *counters;// 4 voxel counters (counting variant only)
 };
 
-enum { CTRL_FRONT = 0, CTRL_BACK = 1, CTRL_CURSOR = 2, CTRL_TICKET = 3, CTRL_BLOCKS_COL = 4, CTRL_N = 8 };
-constexpr uint32_t ITEM_GEO = 1u << 30, ITEM_COL = 1u << 31, ITEM_ID = (1u << 30) - 1u;
+enum { CTRL_NGEO = 0, CTRL_NCOL = 1, CTRL_CURSOR = 2, CTRL_TICKET = 3, CTRL_CELLS = 4, CTRL_N = 8 };
 
-// geometry layer (local storage index) -> global layer; slabs of VOL_SLAB = TZ layers are dealt round-robin to ranks
+// local slab index -> global slab index; slabs of TZ = VOL_SLAB geometry layers are dealt round-robin to ranks
 __device__ __forceinline__ int local_to_global_tz(const Params &p, int tz_local) { return tz_local * p.shard_world + p.shard_rank; }
 
 // eq. 1 / eq. 6: pinhole projection + nearest pixel (A2) + frustum test (A3) in the canonical order.
@@ -75,8 +83,8 @@ __device__ __forceinline__ bool project_px(float fx, float fy, float cx, float c
     return true;
 }
 
-// min/max valid depth (mm) over the inclusive pixel rectangle [x0,x1] x [y0,y1] (already clamped to the image),
-// from the coarsest-needed pyramid level: at most 3 x 3 entries are read.
+// culling only: min/max valid depth (mm) over the inclusive pixel rectangle [x0,x1] x [y0,y1] (already clamped to the
+// image), from the coarsest-needed pyramid level: at most 3 x 3 entries are read.
 __device__ __forceinline__ void depth_range(const Params &p, int x0, int x1, int y0, int y1, uint32_t &mn, uint32_t &mx)
 {
     int l = 0;
@@ -92,8 +100,8 @@ __device__ __forceinline__ void depth_range(const Params &p, int x0, int x1, int
         }
 }
 
-// Conservative pixel rectangle of a camera-space box (centre c, half extents e).  Returns false if the box cannot
-// project into the image.  A box that straddles the camera plane gets the whole image.
+// culling only: conservative pixel rectangle of a camera-space box (centre c, half extents e).  Returns false if the
+// box cannot project into the image.  A box that straddles the camera plane gets the whole image.
 __device__ __forceinline__ bool box_rect(const Params &p, float cX, float cY, float cZ, float eX, float eY, float eZ,
                                          int &x0, int &x1, int &y0, int &y1, float &zmin, float &zmax)
 {

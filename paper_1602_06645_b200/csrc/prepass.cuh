@@ -1,4 +1,4 @@
-// prepass.cuh -- S1 (per-pixel map) and S9 (tile classification) kernels.
+// prepass.cuh -- S1 (per-pixel map, depth pyramid, shell marks) and S9 (tile classification) kernels.
 #pragma once
 #include "params.cuh"
 
@@ -14,31 +14,79 @@ __device__ __forceinline__ float3 backproject(const Params &p, int x, int y, flo
     return P;
 }
 
-// K0 -- one CTA per 32 x 32 pixel region (256 threads x 4 rows).
+// culling only: set the mark bits of every colour cell that intersects the colour-voxel index box
+// [i0,i1] x [j0,j1] x [k0,k1] (inclusive, already clamped to the colour grid).  The (cy, cz) rows of the box are dealt
+// round-robin to `nsub` cooperating lanes; this lane is number `sub`.
+template <int R>
+__device__ __forceinline__ void mark_box(const Params &p, int i0, int i1, int j0, int j1, int k0, int k1, int sub, int nsub)
+{
+    constexpr int CX = cells_x(R), CY = cells_y(R), CZ = cells_z(R), WPT = words_per_tile(R);
+    const int cx0 = i0 / CLX, cx1 = i1 / CLX, cy0 = j0 / CLY, cy1 = j1 / CLY, cz0 = k0 / CLZ, cz1 = k1 / CLZ;
+    int cnt = 0;
+    for (int cz = cz0; cz <= cz1; ++cz) {
+        const int gz = cz / CZ, czin = cz % CZ;
+        if (gz % p.shard_world != p.shard_rank) continue;
+        const int tzl = gz / p.shard_world;
+        for (int cy = cy0; cy <= cy1; ++cy, ++cnt) {
+            if (cnt % nsub != sub) continue;
+            const int ty = cy / CY, cyin = cy % CY;
+            const int rowbit = (czin * CY + cyin) * CX;
+            for (int ttx = cx0 / CX; ttx <= cx1 / CX; ++ttx) {
+                const int a = max(cx0, ttx * CX) - ttx * CX, b = min(cx1, ttx * CX + CX - 1) - ttx * CX;
+                const int bit0 = rowbit + a;
+                const unsigned long long m64 = ((1ull << (b - a + 1)) - 1ull) << (bit0 & 31);
+                uint32_t *w = p.marks + (size_t)((tzl * p.tiles_y + ty) * p.tiles_x + ttx) * WPT + (bit0 >> 5);
+                const uint32_t lo = (uint32_t)m64, hi = (uint32_t)(m64 >> 32);
+                if ((__ldcg(w) & lo) != lo) atomicOr(w, lo);
+                if (hi && (__ldcg(w + 1) & hi) != hi) atomicOr(w + 1, hi);
+            }
+        }
+    }
+}
+
+// culling only: world-space box [lo, hi] grown by sigma -> inclusive colour-voxel index box of the voxel CENTRES inside it.
+__device__ __forceinline__ bool index_box(const Params &p, float lo, float hi, float o, int n, int &a, int &b)
+{
+    const float g = p.sigma + p.slack;
+    const float fa = fmaxf(((lo - g) - o) * p.inv_vc - 0.5f, -1.0f);
+    const float fb = fminf(((hi + g) - o) * p.inv_vc - 0.5f, (float)n);
+    a = max(0, (int)floorf(fa)); b = min(n - 1, (int)ceilf(fb));
+    return a <= b;
+}
+
+// K0 -- one CTA per 32 x 32 pixel region; thread (tx, tq) owns pixels (x = tx, y = 4 tq + m), m = 0..3.
 //  (a) pixel map: everything of eq. 7-8 and the view weight (L110) depends only on the depth pixel, so it is computed
 //      once per pixel instead of once per colour voxel: {X_vd, Y_vd, Z_vd, W}; W = 0 encodes "no colour update possible"
 //      (invalid depth, missing forward neighbour (A7), degenerate normal, W <= 0 (A8)).
 //  (b) min/max valid depth per 8x8, 16x16, 32x32 block (pyramid levels 0-2); the last CTA to finish builds the coarser
-//      levels.  Thread 0 of CTA 0 also resets the per-frame work-list counters.
+//      levels.  Used to cull geometry tiles.
+//  (c) shell marks: a colour voxel can pass the sigma gate (L108) only if it lies within sigma of the depth point of a
+//      colour-eligible pixel, so every 4 x 4 pixel patch marks the colour cells that meet the world-space bounding box
+//      of its points grown by sigma.  Marks are consumed (and cleared) by the fused kernel.
+template <int R>
 __global__ void __launch_bounds__(256) k_prepass(const __grid_constant__ Params p)
 {
     __shared__ uint32_t s_mn[16], s_mx[16];
     __shared__ bool s_last;
-    const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
-    if (threadIdx.x < 16) { s_mn[threadIdx.x] = 0xffffu; s_mx[threadIdx.x] = 0u; }
-    if (blockIdx.x == 0 && blockIdx.y == 0 && threadIdx.x == 0) {
-        p.ctrl[CTRL_FRONT] = 0; p.ctrl[CTRL_BACK] = 0; p.ctrl[CTRL_CURSOR] = 0; p.ctrl[CTRL_BLOCKS_COL] = 0;
+    const int t = threadIdx.x, tx = t & 31, tq = t >> 5;
+    if (t < 16) { s_mn[t] = 0xffffu; s_mx[t] = 0u; }
+    if (blockIdx.x == 0 && blockIdx.y == 0 && t == 0) {
+        p.ctrl[CTRL_NGEO] = 0; p.ctrl[CTRL_NCOL] = 0; p.ctrl[CTRL_CURSOR] = 0; p.ctrl[CTRL_CELLS] = 0;
     }
     __syncthreads();
     const int x = blockIdx.x * 32 + tx;
+    uint32_t mn = 0xffffu, mx = 0u;
+    float lo[3] = {1e30f, 1e30f, 1e30f}, hi[3] = {-1e30f, -1e30f, -1e30f};
+    float wpt[4][3]; bool elig[4];
 #pragma unroll
     for (int m = 0; m < 4; ++m) {
-        const int y = blockIdx.y * 32 + m * 8 + ty;
-        uint32_t d0 = 0;
+        const int y = blockIdx.y * 32 + tq * 4 + m;
+        elig[m] = false;
         if (x < p.wd && y < p.hd) {
-            d0 = __ldg(p.depth + (size_t)y * p.wd + x);
+            const uint32_t d0 = __ldg(p.depth + (size_t)y * p.wd + x);
             float4 out = make_float4(0.f, 0.f, 0.f, 0.f);
             if (d0 != 0) {
+                mn = min(mn, d0); mx = max(mx, d0);
                 const float D = __fmul_rn((float)d0, 0.001f);                      // mm -> m (A4)
                 const float3 Pd = backproject(p, x, y, D);
                 out.x = Pd.x; out.y = Pd.y; out.z = Pd.z;
@@ -63,36 +111,71 @@ __global__ void __launch_bounds__(256) k_prepass(const __grid_constant__ Params 
                         }
                     }
                 }
+                if (out.w > 0.0f) {                                                   // culling only: depth point in world space
+                    elig[m] = true;
+#pragma unroll
+                    for (int a = 0; a < 3; ++a) {
+                        wpt[m][a] = p.Rw[3 * a] * Pd.x + p.Rw[3 * a + 1] * Pd.y + p.Rw[3 * a + 2] * Pd.z + p.tw[a];
+                        lo[a] = fminf(lo[a], wpt[m][a]); hi[a] = fmaxf(hi[a], wpt[m][a]);
+                    }
+                }
             }
             p.pixmap[(size_t)y * p.wd + x] = out;
         }
-        // min / max over the 8-pixel run of this row that lies in one level-0 block, then one shared atomic per run
-        uint32_t mn = d0 ? d0 : 0xffffu, mx = d0;
-#pragma unroll
-        for (int o = 1; o < 8; o <<= 1) {
-            mn = min(mn, __shfl_xor_sync(0xffffffffu, mn, o));
-            mx = max(mx, __shfl_xor_sync(0xffffffffu, mx, o));
-        }
-        if ((tx & 7) == 0) { atomicMin(&s_mn[m * 4 + (tx >> 3)], mn); atomicMax(&s_mx[m * 4 + (tx >> 3)], mx); }
     }
+    // (c) patch = 4 lanes x 4 rows
+    {
+        const unsigned pm = 0xfu << (tx & 28);
+#pragma unroll
+        for (int o = 1; o < 4; o <<= 1)
+#pragma unroll
+            for (int a = 0; a < 3; ++a) {
+                lo[a] = fminf(lo[a], __shfl_xor_sync(0xffffffffu, lo[a], o));
+                hi[a] = fmaxf(hi[a], __shfl_xor_sync(0xffffffffu, hi[a], o));
+            }
+        (void)pm;
+        if (lo[0] <= hi[0]) {
+            int i0, i1, j0, j1, k0, k1;
+            const bool in = index_box(p, lo[0], hi[0], p.ox, p.cnx, i0, i1) && index_box(p, lo[1], hi[1], p.oy, p.cny, j0, j1) &&
+                            index_box(p, lo[2], hi[2], p.oz, p.cnz, k0, k1);
+            if (in) {
+                const int ncell = (i1 / CLX - i0 / CLX + 1) * (j1 / CLY - j0 / CLY + 1) * (k1 / CLZ - k0 / CLZ + 1);
+                if (ncell <= 128) {
+                    mark_box<R>(p, i0, i1, j0, j1, k0, k1, tx & 3, 4);
+                } else {                                  // the patch spans a depth edge: mark pixel by pixel
+#pragma unroll
+                    for (int m = 0; m < 4; ++m)
+                        if (elig[m] && index_box(p, wpt[m][0], wpt[m][0], p.ox, p.cnx, i0, i1) &&
+                            index_box(p, wpt[m][1], wpt[m][1], p.oy, p.cny, j0, j1) && index_box(p, wpt[m][2], wpt[m][2], p.oz, p.cnz, k0, k1))
+                            mark_box<R>(p, i0, i1, j0, j1, k0, k1, 0, 1);
+                }
+            }
+        }
+    }
+    // (b) level-0 block = 8 lanes x 2 threads-rows (tq pair)
+#pragma unroll
+    for (int o = 1; o < 8; o <<= 1) {
+        mn = min(mn, __shfl_xor_sync(0xffffffffu, mn, o));
+        mx = max(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+    }
+    if ((tx & 7) == 0) { atomicMin(&s_mn[(tq >> 1) * 4 + (tx >> 3)], mn); atomicMax(&s_mx[(tq >> 1) * 4 + (tx >> 3)], mx); }
     __syncthreads();
     // level 0: 4 x 4 entries, level 1: 2 x 2, level 2: 1
-    const int t = threadIdx.x;
     if (t < 16) {
         const int bx = blockIdx.x * 4 + (t & 3), by = blockIdx.y * 4 + (t >> 2);
         if (bx < p.pyr_w[0] && by < p.pyr_h[0]) p.pyr[p.pyr_off[0] + by * p.pyr_w[0] + bx] = s_mn[t] | (s_mx[t] << 16);
     } else if (t < 20 && p.pyr_levels > 1) {
         const int q = t - 16, qx = q & 1, qy = q >> 1;
-        uint32_t mn = 0xffffu, mx = 0u;
+        uint32_t a_mn = 0xffffu, a_mx = 0u;
         for (int a = 0; a < 2; ++a) for (int b = 0; b < 2; ++b) {
-            mn = min(mn, s_mn[(qy * 2 + a) * 4 + qx * 2 + b]); mx = max(mx, s_mx[(qy * 2 + a) * 4 + qx * 2 + b]);
+            a_mn = min(a_mn, s_mn[(qy * 2 + a) * 4 + qx * 2 + b]); a_mx = max(a_mx, s_mx[(qy * 2 + a) * 4 + qx * 2 + b]);
         }
         const int bx = blockIdx.x * 2 + qx, by = blockIdx.y * 2 + qy;
-        if (bx < p.pyr_w[1] && by < p.pyr_h[1]) p.pyr[p.pyr_off[1] + by * p.pyr_w[1] + bx] = mn | (mx << 16);
+        if (bx < p.pyr_w[1] && by < p.pyr_h[1]) p.pyr[p.pyr_off[1] + by * p.pyr_w[1] + bx] = a_mn | (a_mx << 16);
     } else if (t == 20 && p.pyr_levels > 2) {
-        uint32_t mn = 0xffffu, mx = 0u;
-        for (int a = 0; a < 16; ++a) { mn = min(mn, s_mn[a]); mx = max(mx, s_mx[a]); }
-        p.pyr[p.pyr_off[2] + blockIdx.y * p.pyr_w[2] + blockIdx.x] = mn | (mx << 16);
+        uint32_t a_mn = 0xffffu, a_mx = 0u;
+        for (int a = 0; a < 16; ++a) { a_mn = min(a_mn, s_mn[a]); a_mx = max(a_mx, s_mx[a]); }
+        p.pyr[p.pyr_off[2] + blockIdx.y * p.pyr_w[2] + blockIdx.x] = a_mn | (a_mx << 16);
     }
     if (p.pyr_levels <= 3) return;
     // the last CTA to arrive reduces level 2 into levels 3.. (each level halves both dimensions)
@@ -110,12 +193,12 @@ __global__ void __launch_bounds__(256) k_prepass(const __grid_constant__ Params 
         const uint32_t *src = p.pyr + p.pyr_off[l - 1];
         for (int e = t; e < w * h; e += blockDim.x) {
             const int ex = e % w, ey = e / w;
-            uint32_t mn = 0xffffu, mx = 0u;
+            uint32_t a_mn = 0xffffu, a_mx = 0u;
             for (int a = 0; a < 2; ++a) for (int b = 0; b < 2; ++b) {
                 const int sx = ex * 2 + b, sy = ey * 2 + a;
-                if (sx < pw && sy < ph) { const uint32_t v = __ldcg(src + sy * pw + sx); mn = min(mn, v & 0xffffu); mx = max(mx, v >> 16); }
+                if (sx < pw && sy < ph) { const uint32_t v = __ldcg(src + sy * pw + sx); a_mn = min(a_mn, v & 0xffffu); a_mx = max(a_mx, v >> 16); }
             }
-            p.pyr[p.pyr_off[l] + e] = mn | (mx << 16);
+            p.pyr[p.pyr_off[l] + e] = a_mn | (a_mx << 16);
         }
         __threadfence();
         __syncthreads();
@@ -123,17 +206,19 @@ __global__ void __launch_bounds__(256) k_prepass(const __grid_constant__ Params 
     if (t == 0) p.ctrl[CTRL_TICKET] = 0;
 }
 
-// K1 -- S9: one thread per geometry tile of this shard.  Conservative test against the depth pyramid; surviving tiles go
-// to the work list: tiles whose colour children may pass the sigma gate (heavier) from the front, geometry-only tiles
-// from the back, so the fused kernel pops the heavy items first.
+// K1 -- S9: one thread per geometry tile of this shard.
+//  geometry: conservative test of the tile's camera-space box against the depth pyramid (any voxel with sdf >= -mu?);
+//  colour:   one work item per non-zero shell-mark word of the tile (heavier, listed first in the fused kernel's queue).
+template <int R>
 __global__ void __launch_bounds__(256) k_classify(const __grid_constant__ Params p)
 {
+    constexpr int WPT = words_per_tile(R);
     const int tile = blockIdx.x * blockDim.x + threadIdx.x;
-    uint32_t flags = 0;
+    bool geo = false;
+    uint32_t nzw = 0;                                   // bit w set: mark word w of this tile is non-zero
     if (tile < p.n_tiles) {
         const int ttx = tile % p.tiles_x, tty = (tile / p.tiles_x) % p.tiles_y, ttz = tile / (p.tiles_x * p.tiles_y);
         const int gz = local_to_global_tz(p, ttz);
-        // tile box centre in world, then camera space (culling only: plain arithmetic with slack in tile_e*)
         const float wx = p.ox + ((float)(ttx * TX) + 0.5f * (float)TX) * p.vs;
         const float wy = p.oy + ((float)(tty * TY) + 0.5f * (float)TY) * p.vs;
         const float wz = p.oz + ((float)(gz * TZ) + 0.5f * (float)TZ) * p.vs;
@@ -144,26 +229,27 @@ __global__ void __launch_bounds__(256) k_classify(const __grid_constant__ Params
         if (box_rect(p, cX, cY, cZ, p.tile_ex, p.tile_ey, p.tile_ez, x0, x1, y0, y1, zmin, zmax)) {
             uint32_t mn, mx;
             depth_range(p, x0, x1, y0, y1, mn, mx);
-            if (mx != 0u) {
-                const float dmin = (float)mn * 0.001f - 1e-4f, dmax = (float)mx * 0.001f + 1e-4f;
-                if (zmin <= dmax + p.mu) flags |= ITEM_GEO;                          // sdf >= -mu possible
-                if (zmin <= dmax + p.sigma && zmax >= dmin - p.sigma) flags |= ITEM_COL;   // |Z - Z_vd| <= sigma possible
-            }
+            if (mx != 0u) geo = zmin <= ((float)mx * 0.001f + 1e-4f) + p.mu;          // sdf >= -mu possible
         }
+#pragma unroll
+        for (int w = 0; w < WPT; ++w) if (__ldcg(p.marks + (size_t)tile * WPT + w) != 0u) nzw |= 1u << w;
     }
-    // warp-aggregated append
-    const unsigned lane = threadIdx.x & 31;
-    const unsigned mcol = __ballot_sync(0xffffffffu, (flags & ITEM_COL) != 0u);
-    const unsigned mgeo = __ballot_sync(0xffffffffu, flags != 0u && (flags & ITEM_COL) == 0u);
-    uint32_t bf = 0, bb = 0;
+    // warp-aggregated appends
+    const unsigned lane = threadIdx.x & 31, lt = (1u << lane) - 1u;
+    const unsigned mg = __ballot_sync(0xffffffffu, geo);
+    int ncol = __popc(nzw), pre = ncol;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { const int v = __shfl_up_sync(0xffffffffu, pre, o); if ((int)lane >= o) pre += v; }
+    const int tot = __shfl_sync(0xffffffffu, pre, 31);
+    uint32_t bg = 0, bc = 0;
     if (lane == 0) {
-        if (mcol) bf = atomicAdd(&p.ctrl[CTRL_FRONT], (uint32_t)__popc(mcol));
-        if (mgeo) bb = atomicAdd(&p.ctrl[CTRL_BACK], (uint32_t)__popc(mgeo));
+        if (mg) bg = atomicAdd(&p.ctrl[CTRL_NGEO], (uint32_t)__popc(mg));
+        if (tot) bc = atomicAdd(&p.ctrl[CTRL_NCOL], (uint32_t)tot);
     }
-    bf = __shfl_sync(0xffffffffu, bf, 0); bb = __shfl_sync(0xffffffffu, bb, 0);
-    const unsigned lt = (1u << lane) - 1u;
-    if (flags & ITEM_COL) p.work[bf + __popc(mcol & lt)] = (uint32_t)tile | flags;
-    else if (flags) p.work[(uint32_t)p.n_tiles - 1u - (bb + __popc(mgeo & lt))] = (uint32_t)tile | flags;
+    bg = __shfl_sync(0xffffffffu, bg, 0); bc = __shfl_sync(0xffffffffu, bc, 0);
+    if (geo) p.work_geo[bg + __popc(mg & lt)] = (uint32_t)tile;
+    uint32_t pos = bc + (uint32_t)(pre - ncol);
+    while (nzw) { const int w = __ffs(nzw) - 1; nzw &= nzw - 1; p.work_col[pos++] = (uint32_t)tile * WPT + (uint32_t)w; }
 }
 
 }  // namespace vf

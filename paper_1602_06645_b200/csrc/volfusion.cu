@@ -55,7 +55,7 @@ static bool rigid_inverse(const float T[16], float Rout[9], float tout[3])
         for (int j = 0; j < 3; ++j) {
             double s = 0.0;
             for (int k = 0; k < 3; ++k) s += (double)T[4 * k + i] * (double)T[4 * k + j];
-            if (std::fabs(s - (i == j ? 1.0 : 0.0)) > 1e-3) return false;
+            if (std::fabs(s - (i == j ? 1.0 : 0.0)) > 1e-4) return false;
         }
     const double det = (double)T[0] * ((double)T[5] * T[10] - (double)T[6] * T[9]) - (double)T[1] * ((double)T[4] * T[10] - (double)T[6] * T[8]) +
                        (double)T[2] * ((double)T[4] * T[9] - (double)T[5] * T[8]);
@@ -82,6 +82,18 @@ static void box_extents(const float R[9], double hx, double hy, double hz, doubl
     ex = (float)(std::fabs(R[0]) * hx + std::fabs(R[1]) * hy + std::fabs(R[2]) * hz + slack);
     ey = (float)(std::fabs(R[3]) * hx + std::fabs(R[4]) * hy + std::fabs(R[5]) * hz + slack);
     ez = (float)(std::fabs(R[6]) * hx + std::fabs(R[7]) * hy + std::fabs(R[8]) * hz + slack);
+}
+
+// culling only: exact (fp64) inverse of the fp32 world->camera map (R, t), rounded to fp32: camera -> world
+static void camera_to_world(const float R[9], const float t[3], float Rw[9], float tw[3])
+{
+    const double a = R[0], b = R[1], c = R[2], d = R[3], e = R[4], f = R[5], g = R[6], h = R[7], i = R[8];
+    const double det = a * (e * i - f * h) - b * (d * i - f * g) + c * (d * h - e * g);
+    const double inv[9] = {(e * i - f * h) / det, (c * h - b * i) / det, (b * f - c * e) / det,
+                           (f * g - d * i) / det, (a * i - c * g) / det, (c * d - a * f) / det,
+                           (d * h - e * g) / det, (b * g - a * h) / det, (a * e - b * d) / det};
+    for (int k = 0; k < 9; ++k) Rw[k] = (float)inv[k];
+    for (int k = 0; k < 3; ++k) tw[k] = (float)(-(inv[3 * k] * t[0] + inv[3 * k + 1] * t[1] + inv[3 * k + 2] * t[2]));
 }
 
 extern "C" const char *vol_strerror(int code)
@@ -123,7 +135,7 @@ extern "C" int vol_create(vol_t **out, const int32_t dims_geo[3], int32_t r, con
     v->device = device;
     Params &p = v->p;
     p.nx = dims_geo[0]; p.ny = dims_geo[1]; p.nz = dims_geo[2]; p.r = r;
-    p.cnx = r * p.nx; p.cny = r * p.ny;
+    p.cnx = r * p.nx; p.cny = r * p.ny; p.cnz = r * p.nz;
     p.shard_rank = rank; p.shard_world = world;
     const int slabs = (p.nz + vf::TZ - 1) / vf::TZ;
     const int my_slabs = slabs > rank ? (slabs - rank + world - 1) / world : 0;
@@ -136,11 +148,12 @@ extern "C" int vol_create(vol_t **out, const int32_t dims_geo[3], int32_t r, con
     p.local_nz = local_nz;
     p.tiles_x = (p.nx + vf::TX - 1) / vf::TX; p.tiles_y = (p.ny + vf::TY - 1) / vf::TY; p.tiles_z_local = my_slabs;
     const int64_t n_tiles = (int64_t)p.tiles_x * p.tiles_y * my_slabs;
-    if (n_tiles >= (int64_t)vf::ITEM_ID) { delete v; return VOL_E_ARG; }
+    if (n_tiles * 16 >= (int64_t)UINT32_MAX) { delete v; return VOL_E_ARG; }
     p.n_tiles = (int)n_tiles;
     p.ox = origin_m[0]; p.oy = origin_m[1]; p.oz = origin_m[2];
     p.vs = extent_m / (float)p.nx;
     p.vc = p.vs / (float)r;
+    p.inv_vc = 1.0f / p.vc;
     p.mu = trunc_mu_m; p.neg_mu = -trunc_mu_m; p.inv_mu = 1.0f / trunc_mu_m;
     p.sigma = sigma; p.sig2 = sigma * sigma; p.gate = gate; p.w_max = w_max;
     v->geo_bytes = (size_t)local_nz * p.ny * p.nx * 4u;
@@ -161,7 +174,11 @@ extern "C" int vol_create(vol_t **out, const int32_t dims_geo[3], int32_t r, con
     if (((uintptr_t)p.geo | (uintptr_t)p.col) & 15u) return fail(VOL_E_ARG);       // 16-byte vector access
     if (v->geo_bytes && cudaMemset(p.geo, 0, v->geo_bytes) != cudaSuccess) rc = VOL_E_CUDA;
     if (v->col_bytes && cudaMemset(p.col, 0, v->col_bytes) != cudaSuccess) rc = VOL_E_CUDA;
-    if (cudaMalloc(&p.work, sizeof(uint32_t) * (size_t)(p.n_tiles > 0 ? p.n_tiles : 1)) != cudaSuccess) rc = VOL_E_OOM;
+    const size_t nt = (size_t)(p.n_tiles > 0 ? p.n_tiles : 1), nw = nt * (size_t)vf::words_per_tile(r);
+    if (cudaMalloc(&p.work_geo, sizeof(uint32_t) * nt) != cudaSuccess) rc = VOL_E_OOM;
+    if (cudaMalloc(&p.work_col, sizeof(uint32_t) * nw) != cudaSuccess) rc = VOL_E_OOM;
+    if (cudaMalloc(&p.marks, sizeof(uint32_t) * nw) != cudaSuccess) rc = VOL_E_OOM;
+    if (rc == VOL_OK && cudaMemset(p.marks, 0, sizeof(uint32_t) * nw) != cudaSuccess) rc = VOL_E_CUDA;
     if (cudaMalloc(&p.ctrl, sizeof(uint32_t) * vf::CTRL_N) != cudaSuccess) rc = VOL_E_OOM;
     if (cudaMalloc(&p.counters, sizeof(unsigned long long) * 4) != cudaSuccess) rc = VOL_E_OOM;
     if (rc == VOL_OK && cudaMemset(p.ctrl, 0, sizeof(uint32_t) * vf::CTRL_N) != cudaSuccess) rc = VOL_E_CUDA;
@@ -172,7 +189,7 @@ extern "C" int vol_create(vol_t **out, const int32_t dims_geo[3], int32_t r, con
     if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) return fail(VOL_E_CUDA);
     v->n_sms = prop.multiProcessorCount;
     int occ = 0;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, vf::k_fused<false>, vf::CTA, 0) != cudaSuccess || occ < 1) {
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, vf::k_fused<2, false>, vf::CTA, 0) != cudaSuccess || occ < 1) {
         snprintf(g_err, sizeof g_err, "fused kernel cannot be resident on device %d (built for sm_100a): %s", device, cudaGetErrorString(cudaGetLastError()));
         return fail(VOL_E_CUDA);
     }
@@ -191,7 +208,9 @@ extern "C" void vol_destroy(vol_t *v)
     cudaDeviceSynchronize();
     if (v->own_geo && v->p.geo) cudaFree(v->p.geo);
     if (v->own_col && v->p.col) cudaFree(v->p.col);
-    if (v->p.work) cudaFree(v->p.work);
+    if (v->p.work_geo) cudaFree(v->p.work_geo);
+    if (v->p.work_col) cudaFree(v->p.work_col);
+    if (v->p.marks) cudaFree(v->p.marks);
     if (v->p.ctrl) cudaFree(v->p.ctrl);
     if (v->p.counters) cudaFree(v->p.counters);
     if (v->p.pixmap) cudaFree(v->p.pixmap);
@@ -244,24 +263,37 @@ extern "C" int vol_integrate(vol_t *v, const uint16_t *depth_u16_dev, int32_t wd
     p.wd = wd; p.hd = hd; p.wh = wh; p.hh = hh;
     p.wd_f = (float)wd; p.hd_f = (float)hd; p.wh_f = (float)wh; p.hh_f = (float)hh;
     p.depth = depth_u16_dev; p.rgb = rgb8_dev;
-    // culling extents: half the box + slack for the fp32 evaluation of the box centre
+    // culling only: slack for the fp32 evaluation of box centres / world points, tile extents, camera -> world map
     const double mag = std::fabs((double)p.t[0]) + std::fabs((double)p.t[1]) + std::fabs((double)p.t[2]) +
                        std::fabs((double)p.ox) + std::fabs((double)p.oy) + std::fabs((double)p.oz) + (double)p.vs * (p.nx + p.ny + p.nz);
-    const double slack = 1e-4 + 4e-6 * mag;
+    const double slack = 1e-4 + 2e-5 * mag;
+    p.slack = (float)slack;
     box_extents(p.R, 0.5 * vf::TX * p.vs, 0.5 * vf::TY * p.vs, 0.5 * vf::TZ * p.vs, slack, p.tile_ex, p.tile_ey, p.tile_ez);
-    box_extents(p.R, 0.5 * vf::MBX * p.vc, 0.5 * vf::MBY * p.vc, 0.5 * vf::MBZ * p.vc, slack, p.mb_ex, p.mb_ey, p.mb_ez);
+    camera_to_world(p.R, p.t, p.Rw, p.tw);
     if (p.n_tiles == 0) return VOL_OK;
 
     cudaStream_t s = (cudaStream_t)stream;
     if (v->counting) CK(cudaMemsetAsync(p.counters, 0, sizeof(unsigned long long) * 4, s));
     if (v->profiling) CK(cudaEventRecord(v->ev[0], s));
     const dim3 g0((wd + 31) / 32, (hd + 31) / 32);
-    vf::k_prepass<<<g0, 256, 0, s>>>(p);
-    if (v->profiling) CK(cudaEventRecord(v->ev[1], s));
-    vf::k_classify<<<(p.n_tiles + 255) / 256, 256, 0, s>>>(p);
-    if (v->profiling) CK(cudaEventRecord(v->ev[2], s));
-    if (v->counting) vf::k_fused<true><<<v->fused_blocks, vf::CTA, 0, s>>>(p);
-    else             vf::k_fused<false><<<v->fused_blocks, vf::CTA, 0, s>>>(p);
+    const int g1 = (p.n_tiles + 255) / 256, g2 = v->fused_blocks;
+    const bool cnt = v->counting;
+#define VF_LAUNCH(RR)                                                                   \
+    do {                                                                                \
+        vf::k_prepass<RR><<<g0, 256, 0, s>>>(p);                                        \
+        if (v->profiling) CK(cudaEventRecord(v->ev[1], s));                             \
+        vf::k_classify<RR><<<g1, 256, 0, s>>>(p);                                       \
+        if (v->profiling) CK(cudaEventRecord(v->ev[2], s));                             \
+        if (cnt) vf::k_fused<RR, true><<<g2, vf::CTA, 0, s>>>(p);                       \
+        else     vf::k_fused<RR, false><<<g2, vf::CTA, 0, s>>>(p);                      \
+    } while (0)
+    switch (p.r) {
+        case 1: VF_LAUNCH(1); break;
+        case 2: VF_LAUNCH(2); break;
+        case 3: VF_LAUNCH(3); break;
+        default: VF_LAUNCH(4); break;
+    }
+#undef VF_LAUNCH
     if (v->profiling) { CK(cudaEventRecord(v->ev[3], s)); v->ev_valid = true; }
     CK(cudaGetLastError());
     return VOL_OK;
@@ -404,10 +436,9 @@ extern "C" int vol_frame_stats(vol_t *v, vol_stats_t *out, void *stream)
     memset(out, 0, sizeof *out);
     if (v->counting) { out->geo_read = cnt[0]; out->geo_changed = cnt[1]; out->col_read = cnt[2]; out->col_changed = cnt[3]; }
     out->tiles_total = (uint32_t)v->p.n_tiles;
-    out->tiles_col = ctrl[vf::CTRL_FRONT];
-    out->tiles_geo = 0;       // filled below: geometry-flagged tiles = back list + colour tiles that also carry the geometry flag
-    out->blocks_col = ctrl[vf::CTRL_BLOCKS_COL];
-    out->tiles_geo = ctrl[vf::CTRL_BACK] + ctrl[vf::CTRL_FRONT];
+    out->tiles_geo = ctrl[vf::CTRL_NGEO];
+    out->items_col = ctrl[vf::CTRL_NCOL];
+    out->cells_col = v->counting ? ctrl[vf::CTRL_CELLS] : 0u;
     return VOL_OK;
 }
 

@@ -65,7 +65,7 @@ def test_degenerate_frames():
     before, _ = g.download()
     st, cnt = integrate_both(g, o, c, np.zeros_like(depth), rgb, T)
     check_counters(st, cnt)
-    assert st.tiles_geo == 0 and st.tiles_col == 0
+    assert st.tiles_geo == 0 and st.items_col == 0
     Tb = I4.copy()
     Tb[:3, :3] = np.diag([-1, 1, -1]).astype(np.float32)
     st, cnt = integrate_both(g, o, c, depth, rgb, Tb)
