@@ -126,6 +126,11 @@ int vol_set_profiling(vol_t *v, int32_t on);
 int vol_last_kernel_ms(vol_t *v, float ms[3]);
 /* Number of kernels one vol_integrate call launches. */
 int vol_launches_per_frame(const vol_t *v);
+/* Device self-test of the branch-free exact reciprocal / division used on the hot path against the correctly rounded
+ * library intrinsics: mismatches[0] = reciprocal over every binary32 in its operand range, mismatches[1] = TSDF
+ * running-average quotient over its operand domain (every denominator 1..513 x numerators; all of them when
+ * exhaustive != 0, every 257th otherwise).  Both must be 0.  Runs on the current device; synchronises. */
+int vol_selftest(uint64_t mismatches[2], int32_t exhaustive);
 void vol_destroy(vol_t *v);
 const char *vol_strerror(int code);
 

@@ -27,7 +27,7 @@ NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", 
 
 EXPORTS = ["vol_create", "vol_integrate", "vol_integrate_host", "vol_download", "vol_download_voxels", "vol_upload",
            "vol_reset", "vol_info", "vol_set_counting", "vol_frame_stats", "vol_set_profiling", "vol_last_kernel_ms",
-           "vol_launches_per_frame", "vol_destroy", "vol_strerror"]
+           "vol_launches_per_frame", "vol_selftest", "vol_destroy", "vol_strerror"]
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
@@ -83,6 +83,7 @@ def lib():
         L.vol_set_profiling.argtypes = [P, I32]
         L.vol_last_kernel_ms.argtypes = [P, P]
         L.vol_launches_per_frame.argtypes = [P]
+        L.vol_selftest.argtypes = [P, I32]
         L.vol_destroy.argtypes = [P]
         L.vol_destroy.restype = None
         L.vol_strerror.argtypes = [ctypes.c_int]
@@ -127,6 +128,13 @@ def _stream_ptr(stream):
     if stream is None:
         return None
     return getattr(stream, "cuda_stream", stream)
+
+
+def selftest(exhaustive: bool = False):
+    """vol_selftest: (reciprocal mismatches, TSDF-quotient mismatches) of the branch-free exact arithmetic; both must be 0."""
+    out = (ctypes.c_uint64 * 2)()
+    _check(lib().vol_selftest(out, int(exhaustive)), "vol_selftest")
+    return int(out[0]), int(out[1])
 
 
 class Volume:

@@ -4,44 +4,53 @@
 // = up to 32 colour cells of 8x4x4 voxels of one tile), then the geometry items (one tile of 32x4x8 TSDF voxels, marched
 // along z with per-column bases hoisted).  A lane always owns one 16-byte vector of 4 x-adjacent voxels, so a warp
 // reads/writes whole 32-byte sectors (colour rows) or 128-byte lines (geometry rows).  No block-level barriers.
+//
+// The per-voxel arithmetic is the canonical sequence of DESIGN.md, issued branch-free for 4 voxels at a time
+// (projection -> gathers -> update); operands outside the range of the branch-free exact reciprocal (exact.cuh) send
+// the whole warp through the plain reference routines below, which use the library intrinsics.
 #pragma once
+#include "exact.cuh"
 #include "params.cuh"
 
 namespace vf {
 
-// O-G for one geometry voxel (readings A5/A6).
-// (X, Y, Z) = voxel centre in the depth camera (eq. 5).  Returns true if the voxel reached its read.
-__device__ __forceinline__ bool geo_voxel(const Params &p, float X, float Y, float Z, uint32_t &word)
+// ---------------------------------------------------------------------------------------------------------------
+// plain per-voxel routines (any operand range) -- the slow path, and the definition the fast path must reproduce
+// ---------------------------------------------------------------------------------------------------------------
+
+// O-G for one geometry voxel (readings A5/A6).  (X, Y, Z) = voxel centre in the depth camera (eq. 5).
+__device__ __noinline__ uint32_t geo_voxel_ref(const Params &p, float X, float Y, float Z, uint32_t word, bool &read)
 {
     int x, y;
-    if (!project_px(p.fx, p.fy, p.cx, p.cy, p.wd_f, p.hd_f, X, Y, Z, x, y)) return false;
+    read = false;
+    if (!project_px(p.fx, p.fy, p.cx, p.cy, p.wd_f, p.hd_f, X, Y, Z, x, y)) return word;
     const uint32_t d = __ldg(p.depth + y * p.wd + x);
-    if (d == 0u) return false;                                            // "if non-zero" (L103)
+    if (d == 0u) return word;                                             // "if non-zero" (L103)
     const float D = __fmul_rn((float)d, 0.001f);
     const float sdf = __fsub_rn(D, Z);
-    if (sdf < p.neg_mu) return false;                                     // behind the truncation band: unchanged
+    if (sdf < p.neg_mu) return word;                                      // behind the truncation band: unchanged
+    read = true;
     const float tsdf = fminf(1.0f, __fmul_rn(sdf, p.inv_mu));
     const int q = (int)(short)(word & 0xffffu);
     const int w = (int)(short)(word >> 16);
     const float num = __fmaf_rn((float)q, (float)w, __fmul_rn(tsdf, 32767.0f));
     const int qn = __float2int_rn(__fdiv_rn(num, __fadd_rn((float)w, 1.0f)));
     const int wn = min(w + 1, p.w_max);
-    word = ((uint32_t)qn & 0xffffu) | ((uint32_t)wn << 16);
-    return true;
+    return ((uint32_t)qn & 0xffffu) | ((uint32_t)wn << 16);
 }
 
 // eq. 9-10 for one colour voxel that passed the sigma gate with view weight W.
-__device__ __forceinline__ void col_voxel_update(const Params &p, float X, float Y, float Z, float W, uint32_t &word)
+__device__ __forceinline__ uint32_t col_voxel_update(const Params &p, float X, float Y, float Z, float W, uint32_t word)
 {
     const int wq = (int)(word >> 24);
     const float W255 = __fmul_rn(W, 255.0f);
-    if (!(W255 > __fmul_rn(p.gate, (float)wq))) return;                   // L115, A9
+    if (!(W255 > __fmul_rn(p.gate, (float)wq))) return word;              // L115, A9
     // HD pixel of the voxel's own position (eq. 3-4; A10, A11)
     const float Xh = __fmaf_rn(p.Rc[2], Z, __fmaf_rn(p.Rc[1], Y, __fmaf_rn(p.Rc[0], X, p.tc[0])));
     const float Yh = __fmaf_rn(p.Rc[5], Z, __fmaf_rn(p.Rc[4], Y, __fmaf_rn(p.Rc[3], X, p.tc[1])));
     const float Zh = __fmaf_rn(p.Rc[8], Z, __fmaf_rn(p.Rc[7], Y, __fmaf_rn(p.Rc[6], X, p.tc[2])));
     int xh, yh;
-    if (!project_px(p.fxh, p.fyh, p.cxh, p.cyh, p.wh_f, p.hh_f, Xh, Yh, Zh, xh, yh)) return;   // A13
+    if (!project_px(p.fxh, p.fyh, p.cxh, p.cyh, p.wh_f, p.hh_f, Xh, Yh, Zh, xh, yh)) return word;   // A13
     const uint8_t *hd = p.rgb + (size_t)(yh * p.wh + xh) * 3;             // A14: nearest pixel
     const float den = __fadd_rn((float)wq, W255);
     uint32_t nw = 0;
@@ -55,19 +64,51 @@ __device__ __forceinline__ void col_voxel_update(const Params &p, float X, float
     }
     int wn = __float2int_rn(__fmaf_rn(W, (float)(255 - wq), (float)wq)); // eq. 10, A12
     wn = min(wn, 255);
-    word = nw | ((uint32_t)wn << 24);
+    return nw | ((uint32_t)wn << 24);
+}
+
+// sigma gate of one colour voxel (eq. 6-8 via the pixel map, L101-110).  Returns the view weight W (> 0) or 0.
+__device__ __noinline__ float col_voxel_gate_ref(const Params &p, float X, float Y, float Z)
+{
+    int x, y;
+    if (!project_px(p.fx, p.fy, p.cx, p.cy, p.wd_f, p.hd_f, X, Y, Z, x, y)) return 0.0f;
+    const float4 pm = __ldg(p.pixmap + y * p.wd + x);
+    if (!(pm.w > 0.0f)) return 0.0f;
+    const float dx = __fsub_rn(X, pm.x), dy = __fsub_rn(Y, pm.y), dz = __fsub_rn(Z, pm.z);
+    const float d2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
+    return d2 > p.sig2 ? 0.0f : pm.w;
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// branch-free projection of one voxel (fast path): pixel offset y * w + x, or ok = false.
+// Precondition (established per tile by k_classify, bit ITEM_NEAR clear): RCP_MIN <= Z <= RCP_MAX.
+// ---------------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void project_fast(float fx, float fy, float cx, float cy, int w, int h, float X, float Y, float Z,
+                                             bool &ok, uint32_t &off)
+{
+    const float iz = rcp_exact(Z);
+    const float u = __fmaf_rn(fx, __fmul_rn(X, iz), cx);
+    const float v = __fmaf_rn(fy, __fmul_rn(Y, iz), cy);
+    // u, v are finite here, so the saturating float->int floor decides exactly like the float-domain test of A2/A3
+    const int xi = __float2int_rd(__fadd_rn(u, 0.5f));
+    const int yi = __float2int_rd(__fadd_rn(v, 0.5f));
+    ok = ((uint32_t)xi < (uint32_t)w) && ((uint32_t)yi < (uint32_t)h);
+    off = ok ? (uint32_t)(yi * w + xi) : 0u;
 }
 
 struct Counts { unsigned long long gr, gc, cr, cc; };
 
-// one geometry tile, one warp: lane = (vx = lane & 7, y = lane >> 3) owns voxels (gx0 + 4 vx .. + 3, gy0 + y) of every layer
+// one geometry tile, one warp: lane = (vx = lane & 7, y = lane >> 3) owns voxels (gx0 + 4 vx .. + 3, gy0 + y) of every layer.
+// NEAR tiles (may hold voxels with Z <= 0 or outside rcp_exact's range) take the plain per-voxel routine.
 template <bool COUNT>
-__device__ __forceinline__ void geometry_tile(const Params &p, int tile, int lane, Counts &c)
+__device__ __forceinline__ void geometry_tile(const Params &p, uint32_t item, int lane, Counts &c)
 {
+    const int tile = (int)(item & ITEM_ID);
+    const bool near = (item & ITEM_NEAR) != 0u;
     const int ttx = tile % p.tiles_x, t2 = tile / p.tiles_x, tty = t2 % p.tiles_y, ttz = t2 / p.tiles_y;
     const int i0 = ttx * TX + 4 * (lane & 7), j = tty * TY + (lane >> 3);
     const int gz0 = local_to_global_tz(p, ttz) * TZ, lz0 = ttz * TZ;
-    if (!(i0 < p.nx && j < p.ny)) return;
+    if (!(i0 < p.nx && j < p.ny)) return;                 // ragged tile: no warp-wide operation below
     const int nl = min(TZ, p.nz - gz0);
     // per-column bases of eq. 5: fma(R_1, py, fma(R_0, px, t)) -- the z term is added per layer with one fma each
     const float py = __fmaf_rn((float)j + 0.5f, p.vs, p.oy);
@@ -79,6 +120,10 @@ __device__ __forceinline__ void geometry_tile(const Params &p, int tile, int lan
         bY[e] = __fmaf_rn(p.R[4], py, __fmaf_rn(p.R[3], px, p.t[1]));
         bZ[e] = __fmaf_rn(p.R[7], py, __fmaf_rn(p.R[6], px, p.t[2]));
     }
+    const float fx = p.fx, fy = p.fy, cx = p.cx, cy = p.cy, r02 = p.R[2], r12 = p.R[5], r22 = p.R[8];
+    const float neg_mu = p.neg_mu, inv_mu = p.inv_mu;
+    const int wd = p.wd, hd = p.hd, w_max = p.w_max;
+    const uint16_t *__restrict__ depth = p.depth;
     const size_t layer = (size_t)p.ny * p.nx;
     uint4 *ptr = reinterpret_cast<uint4 *>(p.geo + ((size_t)lz0 * p.ny + j) * p.nx + i0);
     uint4 cur = *ptr;
@@ -87,21 +132,48 @@ __device__ __forceinline__ void geometry_tile(const Params &p, int tile, int lan
         uint4 *pn = reinterpret_cast<uint4 *>(reinterpret_cast<uint32_t *>(ptr) + layer);
         if (z + 1 < nl) nxt = *pn;                                // prefetch the next layer while this one is computed
         const float pz = __fmaf_rn((float)(gz0 + z) + 0.5f, p.vs, p.oz);
-        uint4 v = cur;
-        uint32_t *w4 = reinterpret_cast<uint32_t *>(&v);
-        const uint32_t *o4 = reinterpret_cast<const uint32_t *>(&cur);
-        bool any = false;
+        float X[4], Y[4], Z[4];
 #pragma unroll
-        for (int e = 0; e < 4; ++e) {
-            const float X = __fmaf_rn(p.R[2], pz, bX[e]);
-            const float Y = __fmaf_rn(p.R[5], pz, bY[e]);
-            const float Z = __fmaf_rn(p.R[8], pz, bZ[e]);
-            const bool rd = geo_voxel(p, X, Y, Z, w4[e]);
-            const bool ch = w4[e] != o4[e];
-            any |= ch;
-            if (COUNT) { c.gr += rd; c.gc += ch; }
+        for (int e = 0; e < 4; ++e) {                             // eq. 5: z term
+            X[e] = __fmaf_rn(r02, pz, bX[e]); Y[e] = __fmaf_rn(r12, pz, bY[e]); Z[e] = __fmaf_rn(r22, pz, bZ[e]);
         }
-        if (any) *ptr = v;                                        // skip the store when nothing changed
+        const uint32_t o4[4] = {cur.x, cur.y, cur.z, cur.w};
+        uint32_t w4[4];
+        if (near) {
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {
+                bool rd = false;
+                w4[e] = geo_voxel_ref(p, X[e], Y[e], Z[e], o4[e], rd);
+                if (COUNT) c.gr += rd;
+            }
+        } else {
+            uint32_t off[4], d[4]; bool ok[4];
+#pragma unroll
+            for (int e = 0; e < 4; ++e) project_fast(fx, fy, cx, cy, wd, hd, X[e], Y[e], Z[e], ok[e], off[e]);   // S2
+#pragma unroll
+            for (int e = 0; e < 4; ++e) d[e] = __ldg(depth + off[e]);  // gather D_n (offset 0 when !ok: a valid address)
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {                         // S3: truncation test + running average
+                const float D = __fmul_rn((float)d[e], 0.001f);
+                const float sdf = __fsub_rn(D, Z[e]);
+                const bool upd = ok[e] && (d[e] != 0u) && !(sdf < neg_mu);
+                const float tsdf = fminf(1.0f, __fmul_rn(sdf, inv_mu));
+                const int q = (int)(short)(o4[e] & 0xffffu);
+                const int wi = (int)(short)(o4[e] >> 16);
+                const float wf = (float)wi;
+                // num is 0 or 2^-40 <= |num| < 2^26 (vol_create bounds mu), den in [1, 513]
+                const float num = __fmaf_rn((float)q, wf, __fmul_rn(tsdf, 32767.0f));
+                const float den = __fadd_rn(wf, 1.0f);
+                const int qn = __float2int_rn(div_with(num, den, div_prepare(den)));
+                const int wn = min(wi + 1, w_max);
+                const uint32_t nw = ((uint32_t)qn & 0xffffu) | ((uint32_t)wn << 16);
+                w4[e] = upd ? nw : o4[e];
+                if (COUNT) c.gr += upd;
+            }
+        }
+        const bool any = (w4[0] != o4[0]) | (w4[1] != o4[1]) | (w4[2] != o4[2]) | (w4[3] != o4[3]);
+        if (COUNT) c.gc += (w4[0] != o4[0]) + (w4[1] != o4[1]) + (w4[2] != o4[2]) + (w4[3] != o4[3]);
+        if (any) *ptr = make_uint4(w4[0], w4[1], w4[2], w4[3]);   // skip the store when nothing changed
         ptr = pn; cur = nxt;
     }
 }
@@ -109,8 +181,10 @@ __device__ __forceinline__ void geometry_tile(const Params &p, int tile, int lan
 // one colour work item, one warp: the set bits of one shell-mark word are colour cells of 8 x 4 x 4 voxels;
 // lane = (vx = lane & 1, y = (lane >> 1) & 3, z = lane >> 3) owns 4 x-adjacent voxels of each cell
 template <int R, bool COUNT>
-__device__ __forceinline__ void colour_item(const Params &p, uint32_t wi, int lane, Counts &c)
+__device__ __forceinline__ void colour_item(const Params &p, uint32_t item, int lane, Counts &c)
 {
+    const uint32_t wi = item & ITEM_ID;
+    const bool near = (item & ITEM_NEAR) != 0u;
     constexpr int CX = cells_x(R), CY = cells_y(R), WPT = words_per_tile(R);
     uint32_t bits = 0;
     if (lane == 0) { bits = __ldcg(p.marks + wi); p.marks[wi] = 0u; }     // consume the marks (self-cleaning)
@@ -120,6 +194,9 @@ __device__ __forceinline__ void colour_item(const Params &p, uint32_t wi, int la
     const int cgx0 = ttx * TX * R, cgy0 = tty * TY * R;
     const int cgz0 = local_to_global_tz(p, ttz) * TZ * R, clz0 = ttz * TZ * R;
     const size_t cnx = (size_t)p.cnx, cny = (size_t)p.cny;
+    const float fx = p.fx, fy = p.fy, cx_ = p.cx, cy_ = p.cy, sig2 = p.sig2;
+    const int wd = p.wd, hd = p.hd;
+    const float4 *__restrict__ pixmap = p.pixmap;
     if (COUNT && lane == 0) atomicAdd(&p.ctrl[CTRL_CELLS], (uint32_t)__popc(bits));
     while (bits) {
         const int b = word * 32 + (__ffs(bits) - 1);
@@ -129,45 +206,53 @@ __device__ __forceinline__ void colour_item(const Params &p, uint32_t wi, int la
         const int jc = cgy0 + cy * CLY + ((lane >> 1) & 3);
         const int kz = cz * CLZ + (lane >> 3);
         const int kcg = cgz0 + kz, kcl = clz0 + kz;
-        if (!(ic0 < p.cnx && jc < p.cny && kcg < p.cnz)) continue;
+        const bool act = ic0 < p.cnx && jc < p.cny && kcg < p.cnz;
         const float py = __fmaf_rn((float)jc + 0.5f, p.vc, p.oy);
         const float pz = __fmaf_rn((float)kcg + 0.5f, p.vc, p.oz);
         float X[4], Y[4], Z[4], W[4];
-        unsigned pass = 0;
 #pragma unroll
-        for (int e = 0; e < 4; ++e) {
+        for (int e = 0; e < 4; ++e) {                                     // S4: eq. 5
             const float px = __fmaf_rn((float)(ic0 + e) + 0.5f, p.vc, p.ox);
-            X[e] = __fmaf_rn(p.R[2], pz, __fmaf_rn(p.R[1], py, __fmaf_rn(p.R[0], px, p.t[0])));    // eq. 5
+            X[e] = __fmaf_rn(p.R[2], pz, __fmaf_rn(p.R[1], py, __fmaf_rn(p.R[0], px, p.t[0])));
             Y[e] = __fmaf_rn(p.R[5], pz, __fmaf_rn(p.R[4], py, __fmaf_rn(p.R[3], px, p.t[1])));
             Z[e] = __fmaf_rn(p.R[8], pz, __fmaf_rn(p.R[7], py, __fmaf_rn(p.R[6], px, p.t[2])));
-            int x, y;
-            W[e] = 0.0f;
-            if (project_px(p.fx, p.fy, p.cx, p.cy, p.wd_f, p.hd_f, X[e], Y[e], Z[e], x, y)) {      // eq. 6
-                const float4 pm = __ldg(p.pixmap + y * p.wd + x);                               // eq. 7-8 per pixel (S1)
-                if (pm.w > 0.0f) {
-                    const float dx = __fsub_rn(X[e], pm.x), dy = __fsub_rn(Y[e], pm.y), dz = __fsub_rn(Z[e], pm.z);
-                    const float d2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
-                    if (!(d2 > p.sig2)) { pass |= 1u << e; W[e] = pm.w; }                          // sigma gate, L108
-                }
+        }
+        unsigned pass = 0;
+        if (near) {
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {
+                W[e] = act ? col_voxel_gate_ref(p, X[e], Y[e], Z[e]) : 0.0f;
+                if (W[e] > 0.0f) pass |= 1u << e;
+            }
+        } else {
+            uint32_t off[4]; bool ok[4];
+            float4 pm[4];
+#pragma unroll
+            for (int e = 0; e < 4; ++e) project_fast(fx, fy, cx_, cy_, wd, hd, X[e], Y[e], Z[e], ok[e], off[e]);   // eq. 6
+#pragma unroll
+            for (int e = 0; e < 4; ++e) pm[e] = __ldg(pixmap + off[e]);      // eq. 7-8 and W per pixel (S1)
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {                                 // S5: sigma gate (L108)
+                const float dx = __fsub_rn(X[e], pm[e].x), dy = __fsub_rn(Y[e], pm[e].y), dz = __fsub_rn(Z[e], pm[e].z);
+                const float d2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
+                const bool in = act && ok[e] && (pm[e].w > 0.0f) && !(d2 > sig2);
+                W[e] = pm[e].w;
+                if (in) pass |= 1u << e;
             }
         }
         if (pass) {
             uint4 *ptr = reinterpret_cast<uint4 *>(p.col + ((size_t)kcl * cny + (size_t)jc) * cnx + (size_t)ic0);
-            uint4 v = *ptr;                                       // first HBM touch of these colour voxels (S6)
-            const uint4 old = v;
-            uint32_t *w4 = reinterpret_cast<uint32_t *>(&v);
-            const uint32_t *o4 = reinterpret_cast<const uint32_t *>(&old);
-            bool any = false;
+            const uint4 old = *ptr;                               // first HBM touch of these colour voxels (S6)
+            const uint32_t o4[4] = {old.x, old.y, old.z, old.w};
+            uint32_t w4[4] = {old.x, old.y, old.z, old.w};
 #pragma unroll
             for (int e = 0; e < 4; ++e) {
                 if (pass & (1u << e)) {
-                    col_voxel_update(p, X[e], Y[e], Z[e], W[e], w4[e]);
-                    const bool ch = w4[e] != o4[e];
-                    any |= ch;
-                    if (COUNT) { c.cr += 1; c.cc += ch; }
+                    w4[e] = col_voxel_update(p, X[e], Y[e], Z[e], W[e], o4[e]);                // S6-S8
+                    if (COUNT) { c.cr += 1; c.cc += w4[e] != o4[e]; }
                 }
             }
-            if (any) *ptr = v;
+            if ((w4[0] != o4[0]) | (w4[1] != o4[1]) | (w4[2] != o4[2]) | (w4[3] != o4[3])) *ptr = make_uint4(w4[0], w4[1], w4[2], w4[3]);
         }
     }
 }
@@ -184,7 +269,7 @@ __global__ void __launch_bounds__(CTA) k_fused(const __grid_constant__ Params p)
         it = __shfl_sync(0xffffffffu, it, 0);
         if (it >= n_items) break;
         if (it < n_col) colour_item<R, COUNT>(p, __ldcg(p.work_col + it), lane, c);
-        else            geometry_tile<COUNT>(p, (int)__ldcg(p.work_geo + (it - n_col)), lane, c);
+        else            geometry_tile<COUNT>(p, __ldcg(p.work_geo + (it - n_col)), lane, c);
     }
     if (COUNT) {
 #pragma unroll

@@ -63,6 +63,10 @@ struct Params {
     unsigned long long *counters;// 4 voxel counters (counting variant only)
 };
 
+// work items: low bits = tile id (geometry) or mark-word index (colour); ITEM_NEAR = the tile's box comes within 2 mm of
+// the camera plane (or behind it), so its voxels may have Z <= 0 or Z outside the range of the branch-free reciprocal
+constexpr uint32_t ITEM_NEAR = 1u << 31, ITEM_ID = ITEM_NEAR - 1u;
+
 enum { CTRL_NGEO = 0, CTRL_NCOL = 1, CTRL_CURSOR = 2, CTRL_TICKET = 3, CTRL_CELLS = 4, CTRL_N = 8 };
 
 // local slab index -> global slab index; slabs of TZ = VOL_SLAB geometry layers are dealt round-robin to ranks

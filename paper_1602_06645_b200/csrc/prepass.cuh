@@ -28,7 +28,7 @@ __device__ __forceinline__ void mark_box(const Params &p, int i0, int i1, int j0
         if (gz % p.shard_world != p.shard_rank) continue;
         const int tzl = gz / p.shard_world;
         for (int cy = cy0; cy <= cy1; ++cy, ++cnt) {
-            if (cnt % nsub != sub) continue;
+            if ((cnt & (nsub - 1)) != sub) continue;
             const int ty = cy / CY, cyin = cy % CY;
             const int rowbit = (czin * CY + cyin) * CX;
             for (int ttx = cx0 / CX; ttx <= cx1 / CX; ++ttx) {
@@ -125,7 +125,6 @@ __global__ void __launch_bounds__(256) k_prepass(const __grid_constant__ Params 
     }
     // (c) patch = 4 lanes x 4 rows
     {
-        const unsigned pm = 0xfu << (tx & 28);
 #pragma unroll
         for (int o = 1; o < 4; o <<= 1)
 #pragma unroll
@@ -133,14 +132,13 @@ __global__ void __launch_bounds__(256) k_prepass(const __grid_constant__ Params 
                 lo[a] = fminf(lo[a], __shfl_xor_sync(0xffffffffu, lo[a], o));
                 hi[a] = fmaxf(hi[a], __shfl_xor_sync(0xffffffffu, hi[a], o));
             }
-        (void)pm;
         if (lo[0] <= hi[0]) {
             int i0, i1, j0, j1, k0, k1;
             const bool in = index_box(p, lo[0], hi[0], p.ox, p.cnx, i0, i1) && index_box(p, lo[1], hi[1], p.oy, p.cny, j0, j1) &&
                             index_box(p, lo[2], hi[2], p.oz, p.cnz, k0, k1);
             if (in) {
                 const int ncell = (i1 / CLX - i0 / CLX + 1) * (j1 / CLY - j0 / CLY + 1) * (k1 / CLZ - k0 / CLZ + 1);
-                if (ncell <= 128) {
+                if (ncell <= 640) {
                     mark_box<R>(p, i0, i1, j0, j1, k0, k1, tx & 3, 4);
                 } else {                                  // the patch spans a depth edge: mark pixel by pixel
 #pragma unroll
@@ -215,6 +213,7 @@ __global__ void __launch_bounds__(256) k_classify(const __grid_constant__ Params
     constexpr int WPT = words_per_tile(R);
     const int tile = blockIdx.x * blockDim.x + threadIdx.x;
     bool geo = false;
+    uint32_t near = 0;
     uint32_t nzw = 0;                                   // bit w set: mark word w of this tile is non-zero
     if (tile < p.n_tiles) {
         const int ttx = tile % p.tiles_x, tty = (tile / p.tiles_x) % p.tiles_y, ttz = tile / (p.tiles_x * p.tiles_y);
@@ -226,6 +225,7 @@ __global__ void __launch_bounds__(256) k_classify(const __grid_constant__ Params
         const float cY = p.R[3] * wx + p.R[4] * wy + p.R[5] * wz + p.t[1];
         const float cZ = p.R[6] * wx + p.R[7] * wy + p.R[8] * wz + p.t[2];
         int x0, x1, y0, y1; float zmin, zmax;
+        if (!(cZ - p.tile_ez > 2e-3f)) near = ITEM_NEAR;
         if (box_rect(p, cX, cY, cZ, p.tile_ex, p.tile_ey, p.tile_ez, x0, x1, y0, y1, zmin, zmax)) {
             uint32_t mn, mx;
             depth_range(p, x0, x1, y0, y1, mn, mx);
@@ -247,9 +247,9 @@ __global__ void __launch_bounds__(256) k_classify(const __grid_constant__ Params
         if (tot) bc = atomicAdd(&p.ctrl[CTRL_NCOL], (uint32_t)tot);
     }
     bg = __shfl_sync(0xffffffffu, bg, 0); bc = __shfl_sync(0xffffffffu, bc, 0);
-    if (geo) p.work_geo[bg + __popc(mg & lt)] = (uint32_t)tile;
+    if (geo) p.work_geo[bg + __popc(mg & lt)] = (uint32_t)tile | near;
     uint32_t pos = bc + (uint32_t)(pre - ncol);
-    while (nzw) { const int w = __ffs(nzw) - 1; nzw &= nzw - 1; p.work_col[pos++] = (uint32_t)tile * WPT + (uint32_t)w; }
+    while (nzw) { const int w = __ffs(nzw) - 1; nzw &= nzw - 1; p.work_col[pos++] = ((uint32_t)tile * WPT + (uint32_t)w) | near; }
 }
 
 }  // namespace vf

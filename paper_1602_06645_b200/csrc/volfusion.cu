@@ -50,7 +50,7 @@ static int set_device(const vol *v) { CK(cudaSetDevice(v->device)); return VOL_O
 static bool rigid_inverse(const float T[16], float Rout[9], float tout[3])
 {
     if (T[12] != 0.0f || T[13] != 0.0f || T[14] != 0.0f || T[15] != 1.0f) return false;
-    for (int i = 0; i < 16; ++i) if (!std::isfinite(T[i])) return false;
+    for (int i = 0; i < 16; ++i) if (!(std::fabs(T[i]) <= 1e6f)) return false;      // also rejects NaN / inf
     for (int i = 0; i < 3; ++i)
         for (int j = 0; j < 3; ++j) {
             double s = 0.0;
@@ -113,8 +113,8 @@ extern "C" int vol_create(vol_t **out, const int32_t dims_geo[3], int32_t r, con
     if (!out || !dims_geo || !origin_m) return VOL_E_ARG;
     if (dims_geo[0] <= 0 || dims_geo[1] <= 0 || dims_geo[2] <= 0 || dims_geo[0] % 4 != 0) return VOL_E_ARG;
     if (r < 1 || r > 4 || !(extent_m > 0.0f) || !(trunc_mu_m > 0.0f) || w_max < 1 || w_max > 512) return VOL_E_ARG;
-    if (!std::isfinite(extent_m) || !std::isfinite(trunc_mu_m)) return VOL_E_ARG;
-    for (int i = 0; i < 3; ++i) if (!std::isfinite(origin_m[i])) return VOL_E_ARG;
+    if (!(extent_m <= 1e6f) || !(trunc_mu_m <= 1e6f)) return VOL_E_ARG;           // also rejects NaN / inf
+    for (int i = 0; i < 3; ++i) if (!(std::fabs(origin_m[i]) <= 1e6f)) return VOL_E_ARG;
     if ((int64_t)dims_geo[0] * r > INT32_MAX / 4 || (int64_t)dims_geo[1] * r > INT32_MAX / 4 || (int64_t)dims_geo[2] * r > INT32_MAX / 4) return VOL_E_ARG;
     int rank = 0, world = 1, device = -1;
     float sigma = 0.020f, gate = 0.8f;
@@ -148,7 +148,7 @@ extern "C" int vol_create(vol_t **out, const int32_t dims_geo[3], int32_t r, con
     p.local_nz = local_nz;
     p.tiles_x = (p.nx + vf::TX - 1) / vf::TX; p.tiles_y = (p.ny + vf::TY - 1) / vf::TY; p.tiles_z_local = my_slabs;
     const int64_t n_tiles = (int64_t)p.tiles_x * p.tiles_y * my_slabs;
-    if (n_tiles * 16 >= (int64_t)UINT32_MAX) { delete v; return VOL_E_ARG; }
+    if (n_tiles * 16 >= (int64_t)vf::ITEM_ID) { delete v; return VOL_E_ARG; }
     p.n_tiles = (int)n_tiles;
     p.ox = origin_m[0]; p.oy = origin_m[1]; p.oz = origin_m[2];
     p.vs = extent_m / (float)p.nx;
@@ -449,4 +449,55 @@ extern "C" int vol_last_kernel_ms(vol_t *v, float ms[3])
     CK(cudaEventSynchronize(v->ev[3]));
     for (int i = 0; i < 3; ++i) CK(cudaEventElapsedTime(&ms[i], v->ev[i], v->ev[i + 1]));
     return VOL_OK;
+}
+
+// ---- vol_selftest: rcp_exact / div_with against the correctly rounded intrinsics -------------------------------
+__global__ void k_selftest_rcp(unsigned long long *bad)
+{
+    // every positive binary32 with RCP_MIN <= a <= RCP_MAX (and its negative)
+    const uint32_t lo = __float_as_uint(vf::RCP_MIN), hi = __float_as_uint(vf::RCP_MAX);
+    unsigned long long n = 0;
+    for (uint64_t b = (uint64_t)lo + (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; b <= hi; b += (uint64_t)gridDim.x * blockDim.x) {
+        const float a = __uint_as_float((uint32_t)b);
+        n += __float_as_uint(vf::rcp_exact(a)) != __float_as_uint(__frcp_rn(a));
+        n += __float_as_uint(vf::rcp_exact(-a)) != __float_as_uint(__frcp_rn(-a));
+    }
+    if (n) atomicAdd(bad, n);
+}
+
+__global__ void k_selftest_div(unsigned long long *bad, uint32_t stride)
+{
+    // numerators: 0 and every |a| in [2^-40, 2^40] (both signs), denominators 1..513
+    const uint32_t lo = __float_as_uint(0x1p-40f), hi = __float_as_uint(0x1p40f);
+    unsigned long long n = 0;
+    for (uint64_t b = (uint64_t)lo + ((uint64_t)blockIdx.x * blockDim.x + threadIdx.x) * stride; b <= hi; b += (uint64_t)gridDim.x * blockDim.x * stride) {
+        const float a = __uint_as_float((uint32_t)b);
+        for (int w = 0; w <= 512; ++w) {
+            const float den = (float)w + 1.0f, rb = vf::div_prepare(den);
+            n += __float_as_uint(vf::div_with(a, den, rb)) != __float_as_uint(__fdiv_rn(a, den));
+            n += __float_as_uint(vf::div_with(-a, den, rb)) != __float_as_uint(__fdiv_rn(-a, den));
+        }
+    }
+    if (blockIdx.x == 0 && threadIdx.x == 0)
+        for (int w = 0; w <= 512; ++w) { const float den = (float)w + 1.0f; n += __float_as_uint(vf::div_with(0.0f, den, vf::div_prepare(den))) != 0u; }
+    if (n) atomicAdd(bad, n);
+}
+
+extern "C" int vol_selftest(uint64_t mismatches[2], int32_t exhaustive)
+{
+    if (!mismatches) return VOL_E_ARG;
+    unsigned long long *d = nullptr;
+    CK(cudaMalloc(&d, 2 * sizeof(unsigned long long)));
+    int rc = VOL_OK;
+    if (cudaMemset(d, 0, 2 * sizeof(unsigned long long)) != cudaSuccess) rc = VOL_E_CUDA;
+    if (rc == VOL_OK) {
+        k_selftest_rcp<<<148 * 8, 256>>>(d);
+        k_selftest_div<<<148 * 8, 256>>>(d + 1, exhaustive ? 1u : 257u);
+        unsigned long long h[2];
+        if (cudaMemcpy(h, d, sizeof h, cudaMemcpyDeviceToHost) != cudaSuccess) rc = VOL_E_CUDA;
+        else { mismatches[0] = h[0]; mismatches[1] = h[1]; }
+    }
+    if (rc != VOL_OK) snprintf(g_err, sizeof g_err, "vol_selftest: %s", cudaGetErrorString(cudaGetLastError()));
+    cudaFree(d);
+    return rc;
 }

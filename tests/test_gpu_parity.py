@@ -147,3 +147,11 @@ def test_bad_arguments_leave_state_untouched():
             g.integrate(dd, c.wd, c.hd, dr, c.wh, c.hh, args[0], args[1], c.K_rgb, c.T_depth_rgb)
         assert e.value.code == vf.VOL_E_ARG
     compare_states(g, o, "after rejected calls")
+
+
+def test_exact_arithmetic_selftest():
+    """The branch-free reciprocal / quotient of the hot path equal __frcp_rn / __fdiv_rn bit for bit: every binary32
+    in the reciprocal's operand range, and a 1/257 stride of the TSDF quotient's numerators x all 513 denominators
+    (the exhaustive sweep is `vf.selftest(exhaustive=True)`, ~1e12 quotients)."""
+    import paper_1602_06645_b200 as vf
+    assert vf.selftest(False) == (0, 0)
