@@ -178,8 +178,65 @@ __device__ __forceinline__ void geometry_tile(const Params &p, uint32_t item, in
     }
 }
 
-// one colour work item, one warp: the set bits of one shell-mark word are colour cells of 8 x 4 x 4 voxels;
-// lane = (vx = lane & 1, y = (lane >> 1) & 3, z = lane >> 3) owns 4 x-adjacent voxels of each cell
+// one colour cell of 8 x 4 x 4 voxels, one warp: lane = (vx = lane & 1, y = (lane >> 1) & 3, z = lane >> 3) owns 4
+// x-adjacent voxels.  (ic0, jc, kcg) = the lane's first voxel in the full colour grid, kcl = its layer in this shard.
+template <bool COUNT>
+__device__ __forceinline__ void colour_cell(const Params &p, bool near, int ic0, int jc, int kcg, int kcl, Counts &c)
+{
+    const float fx = p.fx, fy = p.fy, cx_ = p.cx, cy_ = p.cy, sig2 = p.sig2;
+    const int wd = p.wd, hd = p.hd;
+    const float4 *__restrict__ pixmap = p.pixmap;
+    const bool act = ic0 < p.cnx && jc < p.cny && kcg < p.cnz;
+    const float py = __fmaf_rn((float)jc + 0.5f, p.vc, p.oy);
+    const float pz = __fmaf_rn((float)kcg + 0.5f, p.vc, p.oz);
+    float X[4], Y[4], Z[4], W[4];
+#pragma unroll
+    for (int e = 0; e < 4; ++e) {                                     // S4: eq. 5
+        const float px = __fmaf_rn((float)(ic0 + e) + 0.5f, p.vc, p.ox);
+        X[e] = __fmaf_rn(p.R[2], pz, __fmaf_rn(p.R[1], py, __fmaf_rn(p.R[0], px, p.t[0])));
+        Y[e] = __fmaf_rn(p.R[5], pz, __fmaf_rn(p.R[4], py, __fmaf_rn(p.R[3], px, p.t[1])));
+        Z[e] = __fmaf_rn(p.R[8], pz, __fmaf_rn(p.R[7], py, __fmaf_rn(p.R[6], px, p.t[2])));
+    }
+    unsigned pass = 0;
+    if (near) {
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+            W[e] = act ? col_voxel_gate_ref(p, X[e], Y[e], Z[e]) : 0.0f;
+            if (W[e] > 0.0f) pass |= 1u << e;
+        }
+    } else {
+        uint32_t off[4]; bool ok[4];
+        float4 pm[4];
+#pragma unroll
+        for (int e = 0; e < 4; ++e) project_fast(fx, fy, cx_, cy_, wd, hd, X[e], Y[e], Z[e], ok[e], off[e]);   // eq. 6
+#pragma unroll
+        for (int e = 0; e < 4; ++e) pm[e] = __ldg(pixmap + off[e]);      // eq. 7-8 and W per pixel (S1)
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {                                 // S5: sigma gate (L108)
+            const float dx = __fsub_rn(X[e], pm[e].x), dy = __fsub_rn(Y[e], pm[e].y), dz = __fsub_rn(Z[e], pm[e].z);
+            const float d2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
+            const bool in = act && ok[e] && (pm[e].w > 0.0f) && !(d2 > sig2);
+            W[e] = pm[e].w;
+            if (in) pass |= 1u << e;
+        }
+    }
+    if (pass) {
+        uint4 *ptr = reinterpret_cast<uint4 *>(p.col + ((size_t)kcl * (size_t)p.cny + (size_t)jc) * (size_t)p.cnx + (size_t)ic0);
+        const uint4 old = *ptr;                               // first HBM touch of these colour voxels (S6)
+        const uint32_t o4[4] = {old.x, old.y, old.z, old.w};
+        uint32_t w4[4] = {old.x, old.y, old.z, old.w};
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+            if (pass & (1u << e)) {
+                w4[e] = col_voxel_update(p, X[e], Y[e], Z[e], W[e], o4[e]);                // S6-S8
+                if (COUNT) { c.cr += 1; c.cc += w4[e] != o4[e]; }
+            }
+        }
+        if ((w4[0] != o4[0]) | (w4[1] != o4[1]) | (w4[2] != o4[2]) | (w4[3] != o4[3])) *ptr = make_uint4(w4[0], w4[1], w4[2], w4[3]);
+    }
+}
+
+// one colour work item, one warp: the set bits of one shell-mark word are colour cells of one tile
 template <int R, bool COUNT>
 __device__ __forceinline__ void colour_item(const Params &p, uint32_t item, int lane, Counts &c)
 {
@@ -193,67 +250,13 @@ __device__ __forceinline__ void colour_item(const Params &p, uint32_t item, int 
     const int ttx = tile % p.tiles_x, t2 = tile / p.tiles_x, tty = t2 % p.tiles_y, ttz = t2 / p.tiles_y;
     const int cgx0 = ttx * TX * R, cgy0 = tty * TY * R;
     const int cgz0 = local_to_global_tz(p, ttz) * TZ * R, clz0 = ttz * TZ * R;
-    const size_t cnx = (size_t)p.cnx, cny = (size_t)p.cny;
-    const float fx = p.fx, fy = p.fy, cx_ = p.cx, cy_ = p.cy, sig2 = p.sig2;
-    const int wd = p.wd, hd = p.hd;
-    const float4 *__restrict__ pixmap = p.pixmap;
     if (COUNT && lane == 0) atomicAdd(&p.ctrl[CTRL_CELLS], (uint32_t)__popc(bits));
     while (bits) {
         const int b = word * 32 + (__ffs(bits) - 1);
         bits &= bits - 1;
         const int cx = b % CX, cy = (b / CX) % CY, cz = b / (CX * CY);
-        const int ic0 = cgx0 + cx * CLX + 4 * (lane & 1);
-        const int jc = cgy0 + cy * CLY + ((lane >> 1) & 3);
         const int kz = cz * CLZ + (lane >> 3);
-        const int kcg = cgz0 + kz, kcl = clz0 + kz;
-        const bool act = ic0 < p.cnx && jc < p.cny && kcg < p.cnz;
-        const float py = __fmaf_rn((float)jc + 0.5f, p.vc, p.oy);
-        const float pz = __fmaf_rn((float)kcg + 0.5f, p.vc, p.oz);
-        float X[4], Y[4], Z[4], W[4];
-#pragma unroll
-        for (int e = 0; e < 4; ++e) {                                     // S4: eq. 5
-            const float px = __fmaf_rn((float)(ic0 + e) + 0.5f, p.vc, p.ox);
-            X[e] = __fmaf_rn(p.R[2], pz, __fmaf_rn(p.R[1], py, __fmaf_rn(p.R[0], px, p.t[0])));
-            Y[e] = __fmaf_rn(p.R[5], pz, __fmaf_rn(p.R[4], py, __fmaf_rn(p.R[3], px, p.t[1])));
-            Z[e] = __fmaf_rn(p.R[8], pz, __fmaf_rn(p.R[7], py, __fmaf_rn(p.R[6], px, p.t[2])));
-        }
-        unsigned pass = 0;
-        if (near) {
-#pragma unroll
-            for (int e = 0; e < 4; ++e) {
-                W[e] = act ? col_voxel_gate_ref(p, X[e], Y[e], Z[e]) : 0.0f;
-                if (W[e] > 0.0f) pass |= 1u << e;
-            }
-        } else {
-            uint32_t off[4]; bool ok[4];
-            float4 pm[4];
-#pragma unroll
-            for (int e = 0; e < 4; ++e) project_fast(fx, fy, cx_, cy_, wd, hd, X[e], Y[e], Z[e], ok[e], off[e]);   // eq. 6
-#pragma unroll
-            for (int e = 0; e < 4; ++e) pm[e] = __ldg(pixmap + off[e]);      // eq. 7-8 and W per pixel (S1)
-#pragma unroll
-            for (int e = 0; e < 4; ++e) {                                 // S5: sigma gate (L108)
-                const float dx = __fsub_rn(X[e], pm[e].x), dy = __fsub_rn(Y[e], pm[e].y), dz = __fsub_rn(Z[e], pm[e].z);
-                const float d2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
-                const bool in = act && ok[e] && (pm[e].w > 0.0f) && !(d2 > sig2);
-                W[e] = pm[e].w;
-                if (in) pass |= 1u << e;
-            }
-        }
-        if (pass) {
-            uint4 *ptr = reinterpret_cast<uint4 *>(p.col + ((size_t)kcl * cny + (size_t)jc) * cnx + (size_t)ic0);
-            const uint4 old = *ptr;                               // first HBM touch of these colour voxels (S6)
-            const uint32_t o4[4] = {old.x, old.y, old.z, old.w};
-            uint32_t w4[4] = {old.x, old.y, old.z, old.w};
-#pragma unroll
-            for (int e = 0; e < 4; ++e) {
-                if (pass & (1u << e)) {
-                    w4[e] = col_voxel_update(p, X[e], Y[e], Z[e], W[e], o4[e]);                // S6-S8
-                    if (COUNT) { c.cr += 1; c.cc += w4[e] != o4[e]; }
-                }
-            }
-            if ((w4[0] != o4[0]) | (w4[1] != o4[1]) | (w4[2] != o4[2]) | (w4[3] != o4[3])) *ptr = make_uint4(w4[0], w4[1], w4[2], w4[3]);
-        }
+        colour_cell<COUNT>(p, near, cgx0 + cx * CLX + 4 * (lane & 1), cgy0 + cy * CLY + ((lane >> 1) & 3), cgz0 + kz, clz0 + kz, c);
     }
 }
 

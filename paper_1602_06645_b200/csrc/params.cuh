@@ -15,6 +15,8 @@ namespace vf {
 constexpr int TX = 32, TY = 4, TZ = 8;
 // colour cell (shell-mark / work unit, one warp pass): 8 x 4 x 4 colour voxels = 32 lanes x uint4
 constexpr int CLX = 8, CLY = 4, CLZ = 4;
+// tile classification refines a tile that passes the coarse test on SUBX x 1 x SUBZ sub-boxes
+constexpr int SUBX = 4, SUBZ = 2;
 constexpr int WARPS_PER_CTA = 8;
 constexpr int CTA = 32 * WARPS_PER_CTA;
 
@@ -47,6 +49,8 @@ struct Params {
     // culling only
     float Rw[9], tw[3];          // depth camera -> world (the caller's T_world_depth)
     float tile_ex, tile_ey, tile_ez;   // conservative camera-axis half extents of a geometry tile
+    float sub_ex, sub_ey, sub_ez;      // ... of one of its SUBX x 1 x SUBZ sub-boxes
+    float sigma_g;                     // sigma grown by the fp32 slack
     float inv_vc, slack;         // 1 / colour voxel size; metres of slack for fp32 evaluation of culling geometry
     // device buffers
     const uint16_t *depth;
@@ -56,18 +60,19 @@ struct Params {
     float4   *pixmap;            // S1 output: {X_vd, Y_vd, Z_vd, W} per depth pixel; W = 0 when no colour update is possible
     uint32_t *pyr;               // min/max valid-depth pyramid: entry = min_mm | max_mm << 16 (0xffff / 0 = empty)
     int       pyr_off[12], pyr_w[12], pyr_h[12], pyr_levels;
-    uint32_t *marks;             // shell marks: words_per_tile(r) words per tile, bit = colour cell that may hold sigma-shell voxels
+    uint4    *jobs;              // shell-mark jobs of the frame (one per 4 x 4 pixel patch or per pixel), wd x hd (rounded up to 4) entries
     uint32_t *work_geo;          // geometry work list: local tile ids
+    uint32_t *marks;             // shell marks: words_per_tile(r) words per tile, bit = colour cell that may hold sigma-shell voxels
     uint32_t *work_col;          // colour work list: indices of non-zero mark words
     uint32_t *ctrl;              // control words, see CTRL_* below
     unsigned long long *counters;// 4 voxel counters (counting variant only)
 };
 
-// work items: low bits = tile id (geometry) or mark-word index (colour); ITEM_NEAR = the tile's box comes within 2 mm of
+// work items: low bits = local tile id (geometry) or mark-word index (colour); ITEM_NEAR = the tile's box comes within 2 mm of
 // the camera plane (or behind it), so its voxels may have Z <= 0 or Z outside the range of the branch-free reciprocal
 constexpr uint32_t ITEM_NEAR = 1u << 31, ITEM_ID = ITEM_NEAR - 1u;
 
-enum { CTRL_NGEO = 0, CTRL_NCOL = 1, CTRL_CURSOR = 2, CTRL_TICKET = 3, CTRL_CELLS = 4, CTRL_N = 8 };
+enum { CTRL_NGEO = 0, CTRL_NCOL = 1, CTRL_CURSOR = 2, CTRL_TICKET = 3, CTRL_CELLS = 4, CTRL_NJOBS = 5, CTRL_N = 8 };
 
 // local slab index -> global slab index; slabs of TZ = VOL_SLAB geometry layers are dealt round-robin to ranks
 __device__ __forceinline__ int local_to_global_tz(const Params &p, int tz_local) { return tz_local * p.shard_world + p.shard_rank; }
@@ -105,12 +110,22 @@ __device__ __forceinline__ void depth_range(const Params &p, int x0, int x1, int
 }
 
 // culling only: conservative pixel rectangle of a camera-space box (centre c, half extents e).  Returns false if the
-// box cannot project into the image.  A box that straddles the camera plane gets the whole image.
+// box cannot project into the image: first the four side planes of the view frustum (through the camera centre, grown
+// by one pixel; valid for any Z > 0, so also for boxes that straddle the camera plane), then the projected rectangle.
+// A box that comes within 2 cm of the camera plane gets the whole image.
 __device__ __forceinline__ bool box_rect(const Params &p, float cX, float cY, float cZ, float eX, float eY, float eZ,
                                          int &x0, int &x1, int &y0, int &y1, float &zmin, float &zmax)
 {
     zmin = cZ - eZ; zmax = cZ + eZ;
     if (!(zmax > 0.0f)) return false;
+    {   // u >= -1.5  <=>  fx X + (cx + 1.5) Z >= 0;   u <= wd + 0.5  <=>  -fx X + (wd + 0.5 - cx) Z >= 0   (Z > 0); same in v
+        const float kl = p.cx + 1.5f, kr = p.wd_f + 0.5f - p.cx, kt = p.cy + 1.5f, kb = p.hd_f + 0.5f - p.cy;
+        const float fxe = p.fx * eX, fye = p.fy * eY;
+        if (p.fx * cX + kl * cZ + fxe + fabsf(kl) * eZ < 0.0f) return false;
+        if (-p.fx * cX + kr * cZ + fxe + fabsf(kr) * eZ < 0.0f) return false;
+        if (p.fy * cY + kt * cZ + fye + fabsf(kt) * eZ < 0.0f) return false;
+        if (-p.fy * cY + kb * cZ + fye + fabsf(kb) * eZ < 0.0f) return false;
+    }
     if (zmin > 0.02f) {
         const float i0 = 1.0f / zmin, i1 = 1.0f / zmax;
         const float xa = cX - eX, xb = cX + eX, ya = cY - eY, yb = cY + eY;
@@ -126,6 +141,17 @@ __device__ __forceinline__ bool box_rect(const Params &p, float cX, float cY, fl
         x0 = 0; x1 = p.wd - 1; y0 = 0; y1 = p.hd - 1;
     }
     return true;
+}
+
+// culling only: can any voxel of the camera-space box (centre c, half extents e) pass the TSDF tests (frustum, valid
+// depth, sdf >= -mu)?  Conservative: max valid depth over the box's pixel rectangle against the box's nearest Z.
+__device__ __forceinline__ bool box_may_update(const Params &p, float cX, float cY, float cZ, float eX, float eY, float eZ)
+{
+    int x0, x1, y0, y1; float zmin, zmax;
+    if (!box_rect(p, cX, cY, cZ, eX, eY, eZ, x0, x1, y0, y1, zmin, zmax)) return false;
+    uint32_t mn, mx;
+    depth_range(p, x0, x1, y0, y1, mn, mx);
+    return mx != 0u && zmin <= ((float)mx * 0.001f + 1e-4f) + p.mu;
 }
 
 }  // namespace vf

@@ -15,43 +15,88 @@ __device__ __forceinline__ float3 backproject(const Params &p, int x, int y, flo
 }
 
 // culling only: set the mark bits of every colour cell that intersects the colour-voxel index box
-// [i0,i1] x [j0,j1] x [k0,k1] (inclusive, already clamped to the colour grid).  The (cy, cz) rows of the box are dealt
-// round-robin to `nsub` cooperating lanes; this lane is number `sub`.
+// [i0,i1] x [j0,j1] x [k0,k1] (inclusive, already clamped to the colour grid).  The cell layers (cz) of the box are dealt
+// round-robin to `nsub` cooperating lanes; this lane is number `sub`.  Per (cell layer, tile) the rows of the box form
+// one contiguous run of at most 4 r^2 <= 64 mark bits, which never spans more than two words: one or two
+// fire-and-forget reductions (no return value, so a lane never waits on the L2 round trip).
+// A box of more than MARK_FINE_MAX cells is marked tile by tile instead (all cells of every tile it meets): bounded work
+// for pathological frames, at the price of looser marks.
+constexpr int MARK_FINE_MAX = 1024;
+
 template <int R>
 __device__ __forceinline__ void mark_box(const Params &p, int i0, int i1, int j0, int j1, int k0, int k1, int sub, int nsub)
 {
-    constexpr int CX = cells_x(R), CY = cells_y(R), CZ = cells_z(R), WPT = words_per_tile(R);
+    constexpr int CX = cells_x(R), CY = cells_y(R), CZ = cells_z(R), NC = cells_per_tile(R), WPT = words_per_tile(R);
     const int cx0 = i0 / CLX, cx1 = i1 / CLX, cy0 = j0 / CLY, cy1 = j1 / CLY, cz0 = k0 / CLZ, cz1 = k1 / CLZ;
-    int cnt = 0;
-    for (int cz = cz0; cz <= cz1; ++cz) {
-        const int gz = cz / CZ, czin = cz % CZ;
+    const int tx0 = cx0 / CX, tx1 = cx1 / CX, ty0 = cy0 / CY, ty1 = cy1 / CY;
+    if ((cx1 - cx0 + 1) * (cy1 - cy0 + 1) * (cz1 - cz0 + 1) > MARK_FINE_MAX) {
+        for (int gz = cz0 / CZ + sub; gz <= cz1 / CZ; gz += nsub) {
+            if (gz % p.shard_world != p.shard_rank) continue;
+            const int tzl = gz / p.shard_world;
+            for (int tty = ty0; tty <= ty1; ++tty)
+                for (int ttx = tx0; ttx <= tx1; ++ttx) {
+                    uint32_t *w = p.marks + (size_t)((tzl * p.tiles_y + tty) * p.tiles_x + ttx) * WPT;
+#pragma unroll
+                    for (int k = 0; k < WPT; ++k) atomicOr(w + k, (k + 1) * 32 <= NC ? 0xffffffffu : (1u << (NC & 31)) - 1u);
+                }
+        }
+        return;
+    }
+    for (int cz = cz0 + sub; cz <= cz1; cz += nsub) {
+        const int gz = cz / CZ, czin = cz - gz * CZ;
         if (gz % p.shard_world != p.shard_rank) continue;
         const int tzl = gz / p.shard_world;
-        for (int cy = cy0; cy <= cy1; ++cy, ++cnt) {
-            if ((cnt & (nsub - 1)) != sub) continue;
-            const int ty = cy / CY, cyin = cy % CY;
-            const int rowbit = (czin * CY + cyin) * CX;
-            for (int ttx = cx0 / CX; ttx <= cx1 / CX; ++ttx) {
+        for (int tty = ty0; tty <= ty1; ++tty) {
+            const int la = max(cy0, tty * CY) - tty * CY, lb = min(cy1, tty * CY + CY - 1) - tty * CY;
+            for (int ttx = tx0; ttx <= tx1; ++ttx) {
                 const int a = max(cx0, ttx * CX) - ttx * CX, b = min(cx1, ttx * CX + CX - 1) - ttx * CX;
-                const int bit0 = rowbit + a;
-                const unsigned long long m64 = ((1ull << (b - a + 1)) - 1ull) << (bit0 & 31);
-                uint32_t *w = p.marks + (size_t)((tzl * p.tiles_y + ty) * p.tiles_x + ttx) * WPT + (bit0 >> 5);
-                const uint32_t lo = (uint32_t)m64, hi = (uint32_t)(m64 >> 32);
-                if ((__ldcg(w) & lo) != lo) atomicOr(w, lo);
-                if (hi && (__ldcg(w + 1) & hi) != hi) atomicOr(w + 1, hi);
+                const unsigned long long row = (1ull << (b - a + 1)) - 1ull;
+                const int bit0 = (czin * CY + la) * CX + a;
+                unsigned long long m = 0ull;
+                for (int cy = la; cy <= lb; ++cy) m |= row << ((bit0 & 31) + (cy - la) * CX);
+                uint32_t *w = p.marks + (size_t)((tzl * p.tiles_y + tty) * p.tiles_x + ttx) * WPT + (bit0 >> 5);
+                const uint32_t lo = (uint32_t)m, hi = (uint32_t)(m >> 32);
+                if (lo) atomicOr(w, lo);
+                if (hi) atomicOr(w + 1, hi);
             }
         }
     }
 }
 
-// culling only: world-space box [lo, hi] grown by sigma -> inclusive colour-voxel index box of the voxel CENTRES inside it.
-__device__ __forceinline__ bool index_box(const Params &p, float lo, float hi, float o, int n, int &a, int &b)
+// culling only: world interval [lo, hi] grown by g -> inclusive colour-voxel index range of the voxel CENTRES inside it.
+__device__ __forceinline__ bool index_box(const Params &p, float lo, float hi, float g, float o, int n, int &a, int &b)
 {
-    const float g = p.sigma + p.slack;
     const float fa = fmaxf(((lo - g) - o) * p.inv_vc - 0.5f, -1.0f);
     const float fb = fminf(((hi + g) - o) * p.inv_vc - 0.5f, (float)n);
     a = max(0, (int)floorf(fa)); b = min(n - 1, (int)ceilf(fb));
     return a <= b;
+}
+
+// culling only: a colour voxel passes the sigma gate (L108) of pixel (x, y) only if (i) it projects onto that pixel,
+// i.e. X/Z and Y/Z lie inside the pixel's footprint, and (ii) it is within sigma of the pixel's depth point, hence
+// |Z - Z_vd| <= sigma.  For a rectangle of pixels [xa, xb] x [ya, yb] whose eligible depths span [zmin, zmax] that set is
+// inside the frustum piece {(a Z, b Z, Z)}: a, b over the footprint (grown by 0.01 px against fp32 rounding of eq. 6),
+// Z in [zmin - sigma, zmax + sigma].  The piece is convex, so its world-space bounding box is that of its 8 corners.
+// Returns the inclusive colour-voxel index box of the centres inside it (false if empty).
+__device__ __forceinline__ bool shell_box(const Params &p, float xa, float xb, float ya, float yb, float zmin, float zmax,
+                                          int &i0, int &i1, int &j0, int &j1, int &k0, int &k1)
+{
+    const float a0 = ((xa - 0.51f) - p.cx) / p.fx, a1 = ((xb + 0.51f) - p.cx) / p.fx;
+    const float b0 = ((ya - 0.51f) - p.cy) / p.fy, b1 = ((yb + 0.51f) - p.cy) / p.fy;
+    const float z0 = fmaxf(zmin - p.sigma_g, 1e-6f), z1 = zmax + p.sigma_g;
+    float lo[3], hi[3];
+#pragma unroll
+    for (int ax = 0; ax < 3; ++ax) {
+        const float ra = p.Rw[3 * ax], rb = p.Rw[3 * ax + 1], rc = p.Rw[3 * ax + 2];
+        // direction of the four edge rays; world coordinate = tw + Z * d
+        const float d00 = ra * a0 + rb * b0 + rc, d10 = ra * a1 + rb * b0 + rc, d01 = ra * a0 + rb * b1 + rc, d11 = ra * a1 + rb * b1 + rc;
+        const float dmin = fminf(fminf(d00, d10), fminf(d01, d11)), dmax = fmaxf(fmaxf(d00, d10), fmaxf(d01, d11));
+        lo[ax] = p.tw[ax] + fminf(dmin * z0, dmin * z1);
+        hi[ax] = p.tw[ax] + fmaxf(dmax * z0, dmax * z1);
+    }
+    const float s = p.slack * (1.0f + z1);
+    return index_box(p, lo[0], hi[0], s, p.ox, p.cnx, i0, i1) && index_box(p, lo[1], hi[1], s, p.oy, p.cny, j0, j1) &&
+           index_box(p, lo[2], hi[2], s, p.oz, p.cnz, k0, k1);
 }
 
 // K0 -- one CTA per 32 x 32 pixel region; thread (tx, tq) owns pixels (x = tx, y = 4 tq + m), m = 0..3.
@@ -60,28 +105,34 @@ __device__ __forceinline__ bool index_box(const Params &p, float lo, float hi, f
 //      (invalid depth, missing forward neighbour (A7), degenerate normal, W <= 0 (A8)).
 //  (b) min/max valid depth per 8x8, 16x16, 32x32 block (pyramid levels 0-2); the last CTA to finish builds the coarser
 //      levels.  Used to cull geometry tiles.
-//  (c) shell marks: a colour voxel can pass the sigma gate (L108) only if it lies within sigma of the depth point of a
-//      colour-eligible pixel, so every 4 x 4 pixel patch marks the colour cells that meet the world-space bounding box
-//      of its points grown by sigma.  Marks are consumed (and cleared) by the fused kernel.
+//  (c) shell marks: a colour voxel can pass the sigma gate (L108) only inside the frustum piece of shell_box().  Every
+//      4 x 4 pixel patch marks the colour cells that meet the world-space bounding box of its piece if that box has at most
+//      PATCH_CELLS_MAX cells, else (depth edge, grazing surface) the boxes of its pixels' own pieces.  This kernel only
+//      queues the boxes as jobs; k_mark deals them evenly over the whole GPU (depth edges cluster in a few CTAs here).
+//      Marks are consumed (and cleared) by the fused kernel.
+constexpr int PATCH_CELLS_MAX = 96;
+
 template <int R>
 __global__ void __launch_bounds__(256) k_prepass(const __grid_constant__ Params p)
 {
     __shared__ uint32_t s_mn[16], s_mx[16];
     __shared__ bool s_last;
+    __shared__ uint32_t s_njobs, s_base;
+    __shared__ uint4 s_jobs[1024];      // mark jobs: {x | y << 15 | (4 x 4 patch ? 1 << 31 : single pixel), depth range of its eligible pixels}
     const int t = threadIdx.x, tx = t & 31, tq = t >> 5;
     if (t < 16) { s_mn[t] = 0xffffu; s_mx[t] = 0u; }
+    if (t == 0) s_njobs = 0u;
     if (blockIdx.x == 0 && blockIdx.y == 0 && t == 0) {
         p.ctrl[CTRL_NGEO] = 0; p.ctrl[CTRL_NCOL] = 0; p.ctrl[CTRL_CURSOR] = 0; p.ctrl[CTRL_CELLS] = 0;
     }
     __syncthreads();
     const int x = blockIdx.x * 32 + tx;
     uint32_t mn = 0xffffu, mx = 0u;
-    float lo[3] = {1e30f, 1e30f, 1e30f}, hi[3] = {-1e30f, -1e30f, -1e30f};
-    float wpt[4][3]; bool elig[4];
+    float zpx[4];                             // depths of this thread's colour-eligible pixels (0 = not eligible)
 #pragma unroll
     for (int m = 0; m < 4; ++m) {
         const int y = blockIdx.y * 32 + tq * 4 + m;
-        elig[m] = false;
+        zpx[m] = 0.0f;
         if (x < p.wd && y < p.hd) {
             const uint32_t d0 = __ldg(p.depth + (size_t)y * p.wd + x);
             float4 out = make_float4(0.f, 0.f, 0.f, 0.f);
@@ -111,44 +162,49 @@ __global__ void __launch_bounds__(256) k_prepass(const __grid_constant__ Params 
                         }
                     }
                 }
-                if (out.w > 0.0f) {                                                   // culling only: depth point in world space
-                    elig[m] = true;
-#pragma unroll
-                    for (int a = 0; a < 3; ++a) {
-                        wpt[m][a] = p.Rw[3 * a] * Pd.x + p.Rw[3 * a + 1] * Pd.y + p.Rw[3 * a + 2] * Pd.z + p.tw[a];
-                        lo[a] = fminf(lo[a], wpt[m][a]); hi[a] = fmaxf(hi[a], wpt[m][a]);
-                    }
-                }
+                if (out.w > 0.0f) zpx[m] = D;
             }
             p.pixmap[(size_t)y * p.wd + x] = out;
         }
     }
-    // (c) patch = 4 lanes x 4 rows
+    // (c) phase 1: every 4 x 4 patch (4 lanes x 4 rows) queues one job for its whole piece if that is compact, else one
+    //     job per colour-eligible pixel (depth edge, grazing surface).  All shuffles are executed by the whole warp.
     {
+        float zlo = 1e30f, zhi = -1e30f;
 #pragma unroll
-        for (int o = 1; o < 4; o <<= 1)
+        for (int m = 0; m < 4; ++m) if (zpx[m] > 0.0f) { zlo = fminf(zlo, zpx[m]); zhi = fmaxf(zhi, zpx[m]); }
 #pragma unroll
-            for (int a = 0; a < 3; ++a) {
-                lo[a] = fminf(lo[a], __shfl_xor_sync(0xffffffffu, lo[a], o));
-                hi[a] = fmaxf(hi[a], __shfl_xor_sync(0xffffffffu, hi[a], o));
-            }
-        if (lo[0] <= hi[0]) {
+        for (int o = 1; o < 4; o <<= 1) {
+            zlo = fminf(zlo, __shfl_xor_sync(0xffffffffu, zlo, o));
+            zhi = fmaxf(zhi, __shfl_xor_sync(0xffffffffu, zhi, o));
+        }
+        if (zlo <= zhi) {
+            const int xp = blockIdx.x * 32 + (tx & ~3), yp = blockIdx.y * 32 + tq * 4;
             int i0, i1, j0, j1, k0, k1;
-            const bool in = index_box(p, lo[0], hi[0], p.ox, p.cnx, i0, i1) && index_box(p, lo[1], hi[1], p.oy, p.cny, j0, j1) &&
-                            index_box(p, lo[2], hi[2], p.oz, p.cnz, k0, k1);
-            if (in) {
+            if (shell_box(p, (float)xp, (float)(xp + 3), (float)yp, (float)(yp + 3), zlo, zhi, i0, i1, j0, j1, k0, k1)) {
                 const int ncell = (i1 / CLX - i0 / CLX + 1) * (j1 / CLY - j0 / CLY + 1) * (k1 / CLZ - k0 / CLZ + 1);
-                if (ncell <= 640) {
-                    mark_box<R>(p, i0, i1, j0, j1, k0, k1, tx & 3, 4);
-                } else {                                  // the patch spans a depth edge: mark pixel by pixel
+                if (ncell <= PATCH_CELLS_MAX) {
+                    if ((tx & 3) == 0) {
+                        const uint32_t j = atomicAdd(&s_njobs, 1u);
+                        s_jobs[j] = make_uint4((uint32_t)xp | ((uint32_t)yp << 15) | 0x80000000u, __float_as_uint(zlo), __float_as_uint(zhi), 0u);
+                    }
+                } else {
 #pragma unroll
                     for (int m = 0; m < 4; ++m)
-                        if (elig[m] && index_box(p, wpt[m][0], wpt[m][0], p.ox, p.cnx, i0, i1) &&
-                            index_box(p, wpt[m][1], wpt[m][1], p.oy, p.cny, j0, j1) && index_box(p, wpt[m][2], wpt[m][2], p.oz, p.cnz, k0, k1))
-                            mark_box<R>(p, i0, i1, j0, j1, k0, k1, 0, 1);
+                        if (zpx[m] > 0.0f) {
+                            const uint32_t j = atomicAdd(&s_njobs, 1u);
+                            s_jobs[j] = make_uint4((uint32_t)x | ((uint32_t)(yp + m) << 15), __float_as_uint(zpx[m]), __float_as_uint(zpx[m]), 0u);
+                        }
                 }
             }
         }
+    }
+    __syncthreads();
+    {   // append this CTA's jobs to the frame's queue (one reservation per CTA)
+        const uint32_t njobs = s_njobs;
+        if (t == 0) s_base = njobs ? atomicAdd(&p.ctrl[CTRL_NJOBS], njobs) : 0u;
+        __syncthreads();
+        for (uint32_t j = (uint32_t)t; j < njobs; j += 256u) p.jobs[s_base + j] = s_jobs[j];
     }
     // (b) level-0 block = 8 lanes x 2 threads-rows (tq pair)
 #pragma unroll
@@ -204,14 +260,31 @@ __global__ void __launch_bounds__(256) k_prepass(const __grid_constant__ Params 
     if (t == 0) p.ctrl[CTRL_TICKET] = 0;
 }
 
+// K0b -- S1 (c) continued: one group of 4 lanes per queued job (grid-stride); the 4 lanes share the job's cell layers.
+template <int R>
+__global__ void __launch_bounds__(256) k_mark(const __grid_constant__ Params p)
+{
+    const uint32_t njobs = __ldcg(&p.ctrl[CTRL_NJOBS]);
+    const uint32_t g = (blockIdx.x * blockDim.x + threadIdx.x) >> 2, ng = (gridDim.x * blockDim.x) >> 2;
+    for (uint32_t j = g; j < njobs; j += ng) {
+        const uint4 job = __ldcg(p.jobs + j);
+        const float xa = (float)(job.x & 0x7fffu), ya = (float)((job.x >> 15) & 0x7fffu), ext = (job.x & 0x80000000u) ? 3.0f : 0.0f;
+        int i0, i1, j0, j1, k0, k1;
+        if (shell_box(p, xa, xa + ext, ya, ya + ext, __uint_as_float(job.y), __uint_as_float(job.z), i0, i1, j0, j1, k0, k1))
+            mark_box<R>(p, i0, i1, j0, j1, k0, k1, threadIdx.x & 3, 4);
+    }
+}
+
 // K1 -- S9: one thread per geometry tile of this shard.
-//  geometry: conservative test of the tile's camera-space box against the depth pyramid (any voxel with sdf >= -mu?);
+//  geometry: conservative test of the tile's camera-space box against the depth pyramid (any voxel with sdf >= -mu?),
+//            refined on SUBX x 1 x SUBZ sub-boxes for tiles that pass;
 //  colour:   one work item per non-zero shell-mark word of the tile (heavier, listed first in the fused kernel's queue).
 template <int R>
 __global__ void __launch_bounds__(256) k_classify(const __grid_constant__ Params p)
 {
     constexpr int WPT = words_per_tile(R);
     const int tile = blockIdx.x * blockDim.x + threadIdx.x;
+    if (tile == 0) p.ctrl[CTRL_NJOBS] = 0u;            // the mark jobs of this frame have been consumed by k_mark
     bool geo = false;
     uint32_t near = 0;
     uint32_t nzw = 0;                                   // bit w set: mark word w of this tile is non-zero
@@ -224,12 +297,17 @@ __global__ void __launch_bounds__(256) k_classify(const __grid_constant__ Params
         const float cX = p.R[0] * wx + p.R[1] * wy + p.R[2] * wz + p.t[0];
         const float cY = p.R[3] * wx + p.R[4] * wy + p.R[5] * wz + p.t[1];
         const float cZ = p.R[6] * wx + p.R[7] * wy + p.R[8] * wz + p.t[2];
-        int x0, x1, y0, y1; float zmin, zmax;
         if (!(cZ - p.tile_ez > 2e-3f)) near = ITEM_NEAR;
-        if (box_rect(p, cX, cY, cZ, p.tile_ex, p.tile_ey, p.tile_ez, x0, x1, y0, y1, zmin, zmax)) {
-            uint32_t mn, mx;
-            depth_range(p, x0, x1, y0, y1, mn, mx);
-            if (mx != 0u) geo = zmin <= ((float)mx * 0.001f + 1e-4f) + p.mu;          // sdf >= -mu possible
+        if (box_may_update(p, cX, cY, cZ, p.tile_ex, p.tile_ey, p.tile_ez)) {
+            const float sx = (float)(TX / SUBX) * p.vs, sz = (float)(TZ / SUBZ) * p.vs;
+#pragma unroll
+            for (int bz = 0; bz < SUBZ; ++bz)
+#pragma unroll
+                for (int bx = 0; bx < SUBX; ++bx) {
+                    const float dx = ((float)bx - 0.5f * (float)(SUBX - 1)) * sx, dz = ((float)bz - 0.5f * (float)(SUBZ - 1)) * sz;
+                    if (!geo) geo = box_may_update(p, cX + p.R[0] * dx + p.R[2] * dz, cY + p.R[3] * dx + p.R[5] * dz,
+                                                   cZ + p.R[6] * dx + p.R[8] * dz, p.sub_ex, p.sub_ey, p.sub_ez);
+                }
         }
 #pragma unroll
         for (int w = 0; w < WPT; ++w) if (__ldcg(p.marks + (size_t)tile * WPT + w) != 0u) nzw |= 1u << w;

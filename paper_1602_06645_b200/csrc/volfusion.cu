@@ -215,6 +215,7 @@ extern "C" void vol_destroy(vol_t *v)
     if (v->p.counters) cudaFree(v->p.counters);
     if (v->p.pixmap) cudaFree(v->p.pixmap);
     if (v->p.pyr) cudaFree(v->p.pyr);
+    if (v->p.jobs) cudaFree(v->p.jobs);
     if (v->stage_depth) cudaFree(v->stage_depth);
     if (v->stage_rgb) cudaFree(v->stage_rgb);
     for (int i = 0; i < 4; ++i) if (v->ev[i]) cudaEventDestroy(v->ev[i]);
@@ -229,6 +230,8 @@ static int ensure_scratch(vol *v, int wd, int hd)
     Params &p = v->p;
     if (p.pixmap) { CK(cudaDeviceSynchronize()); cudaFree(p.pixmap); p.pixmap = nullptr; }
     if (p.pyr) { cudaFree(p.pyr); p.pyr = nullptr; }
+    if (p.jobs) { cudaFree(p.jobs); p.jobs = nullptr; }
+    CK(cudaMalloc(&p.jobs, sizeof(uint4) * (size_t)((wd + 3) / 4 * 4) * (size_t)((hd + 3) / 4 * 4)));
     CK(cudaMalloc(&p.pixmap, sizeof(float4) * (size_t)wd * hd));
     int l = 0; size_t off = 0;
     for (;; ++l) {
@@ -269,6 +272,8 @@ extern "C" int vol_integrate(vol_t *v, const uint16_t *depth_u16_dev, int32_t wd
     const double slack = 1e-4 + 2e-5 * mag;
     p.slack = (float)slack;
     box_extents(p.R, 0.5 * vf::TX * p.vs, 0.5 * vf::TY * p.vs, 0.5 * vf::TZ * p.vs, slack, p.tile_ex, p.tile_ey, p.tile_ez);
+    box_extents(p.R, 0.5 * (vf::TX / vf::SUBX) * p.vs, 0.5 * vf::TY * p.vs, 0.5 * (vf::TZ / vf::SUBZ) * p.vs, slack, p.sub_ex, p.sub_ey, p.sub_ez);
+    p.sigma_g = (float)((double)p.sigma * 1.0001 + slack);
     camera_to_world(p.R, p.t, p.Rw, p.tw);
     if (p.n_tiles == 0) return VOL_OK;
 
@@ -276,11 +281,12 @@ extern "C" int vol_integrate(vol_t *v, const uint16_t *depth_u16_dev, int32_t wd
     if (v->counting) CK(cudaMemsetAsync(p.counters, 0, sizeof(unsigned long long) * 4, s));
     if (v->profiling) CK(cudaEventRecord(v->ev[0], s));
     const dim3 g0((wd + 31) / 32, (hd + 31) / 32);
-    const int g1 = (p.n_tiles + 255) / 256, g2 = v->fused_blocks;
+    const int g1 = (p.n_tiles + 255) / 256, g2 = v->fused_blocks, gm = v->n_sms * 4;
     const bool cnt = v->counting;
 #define VF_LAUNCH(RR)                                                                   \
     do {                                                                                \
         vf::k_prepass<RR><<<g0, 256, 0, s>>>(p);                                        \
+        vf::k_mark<RR><<<gm, 256, 0, s>>>(p);                                           \
         if (v->profiling) CK(cudaEventRecord(v->ev[1], s));                             \
         vf::k_classify<RR><<<g1, 256, 0, s>>>(p);                                       \
         if (v->profiling) CK(cudaEventRecord(v->ev[2], s));                             \
@@ -422,7 +428,7 @@ extern "C" int vol_info(const vol_t *v, vol_info_t *o)
 
 extern "C" int vol_set_counting(vol_t *v, int32_t on) { if (!v) return VOL_E_ARG; v->counting = on != 0; return VOL_OK; }
 extern "C" int vol_set_profiling(vol_t *v, int32_t on) { if (!v) return VOL_E_ARG; v->profiling = on != 0; v->ev_valid = false; return VOL_OK; }
-extern "C" int vol_launches_per_frame(const vol_t *v) { return v ? 3 : VOL_E_ARG; }
+extern "C" int vol_launches_per_frame(const vol_t *v) { return v ? 4 : VOL_E_ARG; }
 
 extern "C" int vol_frame_stats(vol_t *v, vol_stats_t *out, void *stream)
 {
