@@ -79,7 +79,7 @@ typedef struct {
     uint64_t geo_read, geo_changed, col_read, col_changed;
     uint32_t tiles_total;   /* geometry tiles owned by this shard */
     uint32_t tiles_geo;     /* geometry tiles (32x4x8 voxels) whose TSDF voxels were visited */
-    uint32_t items_col;     /* colour work items (non-zero shell-mark words) */
+    uint32_t items_col;     /* colour work items (non-zero bytes of the shell-mark words: up to 8 colour cells each) */
     uint32_t cells_col;     /* colour cells (8x4x4 colour voxels) visited; only when counting is enabled */
 } vol_stats_t;
 

@@ -1,9 +1,10 @@
 // fused.cuh -- K2: the fused integration kernel (S2-S8), warp-centric and persistent.
 //
-// Every warp pops work items from one queue until it is empty -- first the colour items (one non-zero shell-mark word
-// = up to 32 colour cells of 8x4x4 voxels of one tile), then the geometry items (one tile of 32x4x8 TSDF voxels, marched
+// Every warp pops work items from one queue until it is empty -- first the colour items (one non-zero shell-mark byte
+// = up to 8 colour cells of 8x4x4 voxels of one tile), then the geometry items (one tile of 32x4x8 TSDF voxels, marched
 // along z with per-column bases hoisted).  A lane always owns one 16-byte vector of 4 x-adjacent voxels, so a warp
-// reads/writes whole 32-byte sectors (colour rows) or 128-byte lines (geometry rows).  No block-level barriers.
+// reads whole 32-byte sectors (colour gate) or 128-byte lines (geometry rows).  Colour voxels that pass the gate are
+// compacted in a per-warp shared-memory stage and updated one per lane.  No block-level barriers.
 //
 // The per-voxel arithmetic is the canonical sequence of DESIGN.md, issued branch-free for 4 voxels at a time
 // (projection -> gathers -> update); operands outside the range of the branch-free exact reciprocal (exact.cuh) send
@@ -83,17 +84,20 @@ __device__ __noinline__ float col_voxel_gate_ref(const Params &p, float X, float
 // branch-free projection of one voxel (fast path): pixel offset y * w + x, or ok = false.
 // Precondition (established per tile by k_classify, bit ITEM_NEAR clear): RCP_MIN <= Z <= RCP_MAX.
 // ---------------------------------------------------------------------------------------------------------------
-__device__ __forceinline__ void project_fast(float fx, float fy, float cx, float cy, int w, int h, float X, float Y, float Z,
-                                             bool &ok, uint32_t &off)
+__device__ __forceinline__ void project_fast(float fx, float fy, float cx, float cy, uint32_t w, uint32_t wbits, uint32_t hbits, uint32_t koff,
+                                             float X, float Y, float Z, bool &ok, uint32_t &off)
 {
     const float iz = rcp_exact(Z);
     const float u = __fmaf_rn(fx, __fmul_rn(X, iz), cx);
     const float v = __fmaf_rn(fy, __fmul_rn(Y, iz), cy);
-    // u, v are finite here, so the saturating float->int floor decides exactly like the float-domain test of A2/A3
-    const int xi = __float2int_rd(__fadd_rn(u, 0.5f));
-    const int yi = __float2int_rd(__fadd_rn(v, 0.5f));
-    ok = ((uint32_t)xi < (uint32_t)w) && ((uint32_t)yi < (uint32_t)h);
-    off = ok ? (uint32_t)(yi * w + xi) : 0u;
+    const float tu = __fadd_rn(u, 0.5f), tv = __fadd_rn(v, 0.5f);
+    // A2/A3: floor(t) in [0, w)  <=>  0 <= t < w.  t is finite and never -0, so on the bit patterns (monotonic for t >= 0,
+    // sign bit set for t < 0) this is one unsigned compare against the bits of (float)w.
+    ok = (__float_as_uint(tu) < wbits) && (__float_as_uint(tv) < hbits);
+    // floor without the conversion pipe: for |t| < 2^22, t + 1.5 * 2^23 rounded towards -inf has floor(t) in its low
+    // mantissa bits; koff = bits(1.5 * 2^23) * (w + 1) folds both biases of y * w + x into one subtraction (mod 2^32)
+    const uint32_t bu = __float_as_uint(__fadd_rd(tu, 12582912.0f)), bv = __float_as_uint(__fadd_rd(tv, 12582912.0f));
+    off = ok ? bv * w + bu - koff : 0u;
 }
 
 struct Counts { unsigned long long gr, gc, cr, cc; };
@@ -122,7 +126,8 @@ __device__ __forceinline__ void geometry_tile(const Params &p, uint32_t item, in
     }
     const float fx = p.fx, fy = p.fy, cx = p.cx, cy = p.cy, r02 = p.R[2], r12 = p.R[5], r22 = p.R[8];
     const float neg_mu = p.neg_mu, inv_mu = p.inv_mu;
-    const int wd = p.wd, hd = p.hd, w_max = p.w_max;
+    const uint32_t wd = (uint32_t)p.wd, wbits = __float_as_uint(p.wd_f), hbits = __float_as_uint(p.hd_f), koff = 0x4B400000u * (wd + 1u);
+    const int w_max = p.w_max;
     const uint16_t *__restrict__ depth = p.depth;
     const size_t layer = (size_t)p.ny * p.nx;
     uint4 *ptr = reinterpret_cast<uint4 *>(p.geo + ((size_t)lz0 * p.ny + j) * p.nx + i0);
@@ -149,7 +154,7 @@ __device__ __forceinline__ void geometry_tile(const Params &p, uint32_t item, in
         } else {
             uint32_t off[4], d[4]; bool ok[4];
 #pragma unroll
-            for (int e = 0; e < 4; ++e) project_fast(fx, fy, cx, cy, wd, hd, X[e], Y[e], Z[e], ok[e], off[e]);   // S2
+            for (int e = 0; e < 4; ++e) project_fast(fx, fy, cx, cy, wd, wbits, hbits, koff, X[e], Y[e], Z[e], ok[e], off[e]);   // S2
 #pragma unroll
             for (int e = 0; e < 4; ++e) d[e] = __ldg(depth + off[e]);  // gather D_n (offset 0 when !ok: a valid address)
 #pragma unroll
@@ -164,9 +169,11 @@ __device__ __forceinline__ void geometry_tile(const Params &p, uint32_t item, in
                 // num is 0 or 2^-40 <= |num| < 2^26 (vol_create bounds mu), den in [1, 513]
                 const float num = __fmaf_rn((float)q, wf, __fmul_rn(tsdf, 32767.0f));
                 const float den = __fadd_rn(wf, 1.0f);
-                const int qn = __float2int_rn(div_with(num, den, div_prepare(den)));
+                // rint (half-even) without the conversion pipe: |quotient| <= 32767, so adding 1.5 * 2^23 leaves it in the
+                // low mantissa bits, already in two's complement
+                const uint32_t qn = __float_as_uint(__fadd_rn(div_with(num, den, div_prepare(den)), 12582912.0f));
                 const int wn = min(wi + 1, w_max);
-                const uint32_t nw = ((uint32_t)qn & 0xffffu) | ((uint32_t)wn << 16);
+                const uint32_t nw = (qn & 0xffffu) | ((uint32_t)wn << 16);
                 w4[e] = upd ? nw : o4[e];
                 if (COUNT) c.gr += upd;
             }
@@ -178,13 +185,67 @@ __device__ __forceinline__ void geometry_tile(const Params &p, uint32_t item, in
     }
 }
 
+// Per-warp staging buffer of colour voxels that passed the sigma gate.  The gate (S4-S5) runs on whole cells, 4 voxels
+// per lane, and only a fraction of them passes; the update (S6-S8: weight gate, HD lookup, eq. 9-10) is several times
+// longer.  Passing voxels are therefore compacted here and updated 32 at a time with every lane busy.
+constexpr int STAGE_CAP = 160;            // up to 31 carried over + 128 of one cell
+struct Stage {
+    float4 rec[STAGE_CAP];                // {X, Y, Z} = voxel centre in the depth camera (eq. 5), W = view weight of its pixel
+    uint2  adr[STAGE_CAP];                // word index of the voxel in this shard's colour volume (lo, hi)
+};
+
+// S6-S8 for up to 32 staged voxels [first, first + n): one voxel per lane.  Same arithmetic as col_voxel_update(), but
+// the HD pixel (eq. 3-4) is computed and its three bytes requested BEFORE the stored word arrives: the two gathers do
+// not depend on each other, so their latencies overlap instead of adding up (the word is a DRAM access, and one warp
+// works through its stage round after round).  A voxel that then fails the weight gate has fetched 3 bytes in vain.
+template <bool COUNT>
+__device__ __forceinline__ void colour_update_staged(const Params &p, const Stage &st, int first, int n, int lane, Counts &c)
+{
+    if (lane < n) {
+        const float4 r = st.rec[first + lane];
+        const uint2 a = st.adr[first + lane];
+        uint32_t *ptr = p.col + (((size_t)a.y << 32) | (size_t)a.x);
+        const uint32_t old = *ptr;                                // first HBM touch of this colour voxel (S6)
+        // HD pixel of the voxel's own position (eq. 3-4; A10, A11)
+        const float Xh = __fmaf_rn(p.Rc[2], r.z, __fmaf_rn(p.Rc[1], r.y, __fmaf_rn(p.Rc[0], r.x, p.tc[0])));
+        const float Yh = __fmaf_rn(p.Rc[5], r.z, __fmaf_rn(p.Rc[4], r.y, __fmaf_rn(p.Rc[3], r.x, p.tc[1])));
+        const float Zh = __fmaf_rn(p.Rc[8], r.z, __fmaf_rn(p.Rc[7], r.y, __fmaf_rn(p.Rc[6], r.x, p.tc[2])));
+        int xh = 0, yh = 0;
+        const bool okh = project_px(p.fxh, p.fyh, p.cxh, p.cyh, p.wh_f, p.hh_f, Xh, Yh, Zh, xh, yh);   // A13
+        const uint8_t *hd = p.rgb + (size_t)(yh * p.wh + xh) * 3;     // A14: nearest pixel ((0, 0) when outside: a valid address)
+        const uint32_t h0 = __ldg(hd), h1 = __ldg(hd + 1), h2 = __ldg(hd + 2);
+        const int wq = (int)(old >> 24);
+        const float W = r.w, W255 = __fmul_rn(W, 255.0f);
+        uint32_t nw = old;
+        if (okh && W255 > __fmul_rn(p.gate, (float)wq)) {         // L115, A9
+            const float den = __fadd_rn((float)wq, W255);
+            const uint32_t h[3] = {h0, h1, h2};
+            nw = 0;
+#pragma unroll
+            for (int ch = 0; ch < 3; ++ch) {                          // eq. 9
+                const int C = (int)((old >> (8 * ch)) & 0xffu);
+                const float num = __fmaf_rn(W255, (float)h[ch], (float)(C * wq));
+                const float cn = rintf(__fdiv_rn(num, den));
+                const int ci = cn < 0.0f ? 0 : (cn > 255.0f ? 255 : (int)cn);
+                nw |= (uint32_t)ci << (8 * ch);
+            }
+            int wn = __float2int_rn(__fmaf_rn(W, (float)(255 - wq), (float)wq)); // eq. 10, A12
+            nw |= (uint32_t)min(wn, 255) << 24;
+            if (nw != old) *ptr = nw;
+        }
+        if (COUNT) { c.cr += 1; c.cc += nw != old; }
+    }
+}
+
 // one colour cell of 8 x 4 x 4 voxels, one warp: lane = (vx = lane & 1, y = (lane >> 1) & 3, z = lane >> 3) owns 4
 // x-adjacent voxels.  (ic0, jc, kcg) = the lane's first voxel in the full colour grid, kcl = its layer in this shard.
+// Voxels that pass the gate are appended to the warp's stage (n = its fill level, warp-uniform); full groups of 32 are
+// updated at once.
 template <bool COUNT>
-__device__ __forceinline__ void colour_cell(const Params &p, bool near, int ic0, int jc, int kcg, int kcl, Counts &c)
+__device__ __forceinline__ void colour_cell(const Params &p, bool near, int ic0, int jc, int kcg, int kcl, Stage &st, int &n, int lane, Counts &c)
 {
     const float fx = p.fx, fy = p.fy, cx_ = p.cx, cy_ = p.cy, sig2 = p.sig2;
-    const int wd = p.wd, hd = p.hd;
+    const uint32_t wd = (uint32_t)p.wd, wbits = __float_as_uint(p.wd_f), hbits = __float_as_uint(p.hd_f), koff = 0x4B400000u * (wd + 1u);
     const float4 *__restrict__ pixmap = p.pixmap;
     const bool act = ic0 < p.cnx && jc < p.cny && kcg < p.cnz;
     const float py = __fmaf_rn((float)jc + 0.5f, p.vc, p.oy);
@@ -208,7 +269,7 @@ __device__ __forceinline__ void colour_cell(const Params &p, bool near, int ic0,
         uint32_t off[4]; bool ok[4];
         float4 pm[4];
 #pragma unroll
-        for (int e = 0; e < 4; ++e) project_fast(fx, fy, cx_, cy_, wd, hd, X[e], Y[e], Z[e], ok[e], off[e]);   // eq. 6
+        for (int e = 0; e < 4; ++e) project_fast(fx, fy, cx_, cy_, wd, wbits, hbits, koff, X[e], Y[e], Z[e], ok[e], off[e]);   // eq. 6
 #pragma unroll
         for (int e = 0; e < 4; ++e) pm[e] = __ldg(pixmap + off[e]);      // eq. 7-8 and W per pixel (S1)
 #pragma unroll
@@ -220,31 +281,43 @@ __device__ __forceinline__ void colour_cell(const Params &p, bool near, int ic0,
             if (in) pass |= 1u << e;
         }
     }
-    if (pass) {
-        uint4 *ptr = reinterpret_cast<uint4 *>(p.col + ((size_t)kcl * (size_t)p.cny + (size_t)jc) * (size_t)p.cnx + (size_t)ic0);
-        const uint4 old = *ptr;                               // first HBM touch of these colour voxels (S6)
-        const uint32_t o4[4] = {old.x, old.y, old.z, old.w};
-        uint32_t w4[4] = {old.x, old.y, old.z, old.w};
+    // compact: exclusive prefix of the per-lane counts
+    const int cnt = __popc(pass);
+    int pre = cnt;
 #pragma unroll
-        for (int e = 0; e < 4; ++e) {
-            if (pass & (1u << e)) {
-                w4[e] = col_voxel_update(p, X[e], Y[e], Z[e], W[e], o4[e]);                // S6-S8
-                if (COUNT) { c.cr += 1; c.cc += w4[e] != o4[e]; }
-            }
+    for (int o = 1; o < 32; o <<= 1) { const int v = __shfl_up_sync(0xffffffffu, pre, o); if (lane >= o) pre += v; }
+    const int total = __shfl_sync(0xffffffffu, pre, 31);
+    if (total == 0) return;
+    int slot = n + pre - cnt;
+    const size_t base = ((size_t)kcl * (size_t)p.cny + (size_t)jc) * (size_t)p.cnx + (size_t)ic0;
+    // start the DRAM access of the stored words now; the update reads them a few hundred cycles later
+    if (pass) asm volatile("prefetch.global.L2 [%0];" ::"l"(p.col + base));
+#pragma unroll
+    for (int e = 0; e < 4; ++e)
+        if (pass & (1u << e)) {
+            st.rec[slot] = make_float4(X[e], Y[e], Z[e], W[e]);
+            const size_t a = base + (size_t)e;
+            st.adr[slot] = make_uint2((uint32_t)a, (uint32_t)(a >> 32));
+            ++slot;
         }
-        if ((w4[0] != o4[0]) | (w4[1] != o4[1]) | (w4[2] != o4[2]) | (w4[3] != o4[3])) *ptr = make_uint4(w4[0], w4[1], w4[2], w4[3]);
-    }
+    n += total;
+    __syncwarp();
+    while (n >= 32) { n -= 32; colour_update_staged<COUNT>(p, st, n, 32, lane, c); }
+    __syncwarp();
 }
 
-// one colour work item, one warp: the set bits of one shell-mark word are colour cells of one tile
+// one colour work item, one warp: the set bits of one byte of a shell-mark word are up to 8 colour cells of one tile
 template <int R, bool COUNT>
-__device__ __forceinline__ void colour_item(const Params &p, uint32_t item, int lane, Counts &c)
+__device__ __forceinline__ void colour_item(const Params &p, uint32_t item, Stage &st, int &n, int lane, Counts &c)
 {
-    const uint32_t wi = item & ITEM_ID;
+    const uint32_t bi = item & ITEM_ID, wi = bi >> 2, sh = 8u * (bi & 3u);
     const bool near = (item & ITEM_NEAR) != 0u;
     constexpr int CX = cells_x(R), CY = cells_y(R), WPT = words_per_tile(R);
     uint32_t bits = 0;
-    if (lane == 0) { bits = __ldcg(p.marks + wi); p.marks[wi] = 0u; }     // consume the marks (self-cleaning)
+    if (lane == 0) {                                                      // consume this item's byte of the marks (self-cleaning)
+        bits = __ldcg(p.marks + wi) & (0xffu << sh);
+        atomicAnd(p.marks + wi, ~(0xffu << sh));
+    }
     bits = __shfl_sync(0xffffffffu, bits, 0);
     const int tile = (int)(wi / WPT), word = (int)(wi % WPT);
     const int ttx = tile % p.tiles_x, t2 = tile / p.tiles_x, tty = t2 % p.tiles_y, ttz = t2 / p.tiles_y;
@@ -256,24 +329,39 @@ __device__ __forceinline__ void colour_item(const Params &p, uint32_t item, int 
         bits &= bits - 1;
         const int cx = b % CX, cy = (b / CX) % CY, cz = b / (CX * CY);
         const int kz = cz * CLZ + (lane >> 3);
-        colour_cell<COUNT>(p, near, cgx0 + cx * CLX + 4 * (lane & 1), cgy0 + cy * CLY + ((lane >> 1) & 3), cgz0 + kz, clz0 + kz, c);
+        colour_cell<COUNT>(p, near, cgx0 + cx * CLX + 4 * (lane & 1), cgy0 + cy * CLY + ((lane >> 1) & 3), cgz0 + kz, clz0 + kz, st, n, lane, c);
     }
 }
 
-template <int R, bool COUNT>
-__global__ void __launch_bounds__(CTA) k_fused(const __grid_constant__ Params p)
+// lane 0 draws the next queue ticket.  A predicated instruction, not a branch: the warp must not diverge here, or the
+// compiler may run the whole item once for lane 0 and once for the other lanes.
+__device__ __forceinline__ void next_ticket(uint32_t *cursor, int lane, uint32_t &ticket)
 {
+    asm volatile("{\n\t.reg .pred q;\n\tsetp.eq.s32 q, %1, 0;\n\t@q atom.global.add.u32 %0, [%2], 1;\n\t}"
+                 : "+r"(ticket) : "r"(lane), "l"(cursor) : "memory");
+}
+
+template <int R, bool COUNT>
+__global__ void __launch_bounds__(CTA, 4) k_fused(const __grid_constant__ Params p)
+{
+    __shared__ Stage s_stage[WARPS_PER_CTA];
     const int lane = threadIdx.x & 31;
+    Stage &st = s_stage[threadIdx.x >> 5];
     const uint32_t n_col = __ldcg(&p.ctrl[CTRL_NCOL]), n_items = n_col + __ldcg(&p.ctrl[CTRL_NGEO]);
     Counts c = {0, 0, 0, 0};
+    int n_staged = 0;
+    // the ticket of the next item is requested before the current one is processed (the L2 round trip is hidden)
+    uint32_t ticket = 0;
+    next_ticket(&p.ctrl[CTRL_CURSOR], lane, ticket);
     for (;;) {
-        uint32_t it = 0;
-        if (lane == 0) it = atomicAdd(&p.ctrl[CTRL_CURSOR], 1u);
-        it = __shfl_sync(0xffffffffu, it, 0);
+        const uint32_t it = __shfl_sync(0xffffffffu, ticket, 0);
         if (it >= n_items) break;
-        if (it < n_col) colour_item<R, COUNT>(p, __ldcg(p.work_col + it), lane, c);
-        else            geometry_tile<COUNT>(p, __ldcg(p.work_geo + (it - n_col)), lane, c);
+        const uint32_t item = it < n_col ? __ldcg(p.work_col + it) : __ldcg(p.work_geo + (it - n_col));
+        next_ticket(&p.ctrl[CTRL_CURSOR], lane, ticket);
+        if (it < n_col) colour_item<R, COUNT>(p, item, st, n_staged, lane, c);
+        else            geometry_tile<COUNT>(p, item, lane, c);
     }
+    if (n_staged > 0) colour_update_staged<COUNT>(p, st, 0, n_staged, lane, c);
     if (COUNT) {
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) {

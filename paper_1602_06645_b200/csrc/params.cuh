@@ -63,12 +63,12 @@ struct Params {
     uint4    *jobs;              // shell-mark jobs of the frame (one per 4 x 4 pixel patch or per pixel), wd x hd (rounded up to 4) entries
     uint32_t *work_geo;          // geometry work list: local tile ids
     uint32_t *marks;             // shell marks: words_per_tile(r) words per tile, bit = colour cell that may hold sigma-shell voxels
-    uint32_t *work_col;          // colour work list: indices of non-zero mark words
+    uint32_t *work_col;          // colour work list: indices of non-zero mark BYTES (4 x word index + byte)
     uint32_t *ctrl;              // control words, see CTRL_* below
     unsigned long long *counters;// 4 voxel counters (counting variant only)
 };
 
-// work items: low bits = local tile id (geometry) or mark-word index (colour); ITEM_NEAR = the tile's box comes within 2 mm of
+// work items: low bits = local tile id (geometry) or mark-byte index (colour); ITEM_NEAR = the tile's box comes within 2 mm of
 // the camera plane (or behind it), so its voxels may have Z <= 0 or Z outside the range of the branch-free reciprocal
 constexpr uint32_t ITEM_NEAR = 1u << 31, ITEM_ID = ITEM_NEAR - 1u;
 

@@ -278,7 +278,8 @@ __global__ void __launch_bounds__(256) k_mark(const __grid_constant__ Params p)
 // K1 -- S9: one thread per geometry tile of this shard.
 //  geometry: conservative test of the tile's camera-space box against the depth pyramid (any voxel with sdf >= -mu?),
 //            refined on SUBX x 1 x SUBZ sub-boxes for tiles that pass;
-//  colour:   one work item per non-zero shell-mark word of the tile (heavier, listed first in the fused kernel's queue).
+//  colour:   one work item per non-zero BYTE of the tile's shell-mark words, i.e. up to 8 colour cells (heavier than a
+//            geometry tile, listed first in the fused kernel's queue).
 template <int R>
 __global__ void __launch_bounds__(256) k_classify(const __grid_constant__ Params p)
 {
@@ -287,7 +288,7 @@ __global__ void __launch_bounds__(256) k_classify(const __grid_constant__ Params
     if (tile == 0) p.ctrl[CTRL_NJOBS] = 0u;            // the mark jobs of this frame have been consumed by k_mark
     bool geo = false;
     uint32_t near = 0;
-    uint32_t nzw = 0;                                   // bit w set: mark word w of this tile is non-zero
+    unsigned long long nzb = 0ull;                      // bit 4 w + b set: byte b of mark word w of this tile is non-zero
     if (tile < p.n_tiles) {
         const int ttx = tile % p.tiles_x, tty = (tile / p.tiles_x) % p.tiles_y, ttz = tile / (p.tiles_x * p.tiles_y);
         const int gz = local_to_global_tz(p, ttz);
@@ -310,12 +311,16 @@ __global__ void __launch_bounds__(256) k_classify(const __grid_constant__ Params
                 }
         }
 #pragma unroll
-        for (int w = 0; w < WPT; ++w) if (__ldcg(p.marks + (size_t)tile * WPT + w) != 0u) nzw |= 1u << w;
+        for (int w = 0; w < WPT; ++w) {
+            const uint32_t m = __ldcg(p.marks + (size_t)tile * WPT + w);
+            const uint32_t nz = ((m & 0xffu) != 0u) | (((m & 0xff00u) != 0u) << 1) | (((m & 0xff0000u) != 0u) << 2) | (((m >> 24) != 0u) << 3);
+            nzb |= (unsigned long long)nz << (4 * w);
+        }
     }
     // warp-aggregated appends
     const unsigned lane = threadIdx.x & 31, lt = (1u << lane) - 1u;
     const unsigned mg = __ballot_sync(0xffffffffu, geo);
-    int ncol = __popc(nzw), pre = ncol;
+    int ncol = __popcll(nzb), pre = ncol;
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) { const int v = __shfl_up_sync(0xffffffffu, pre, o); if ((int)lane >= o) pre += v; }
     const int tot = __shfl_sync(0xffffffffu, pre, 31);
@@ -327,7 +332,7 @@ __global__ void __launch_bounds__(256) k_classify(const __grid_constant__ Params
     bg = __shfl_sync(0xffffffffu, bg, 0); bc = __shfl_sync(0xffffffffu, bc, 0);
     if (geo) p.work_geo[bg + __popc(mg & lt)] = (uint32_t)tile | near;
     uint32_t pos = bc + (uint32_t)(pre - ncol);
-    while (nzw) { const int w = __ffs(nzw) - 1; nzw &= nzw - 1; p.work_col[pos++] = ((uint32_t)tile * WPT + (uint32_t)w) | near; }
+    while (nzb) { const int b = __ffsll((long long)nzb) - 1; nzb &= nzb - 1ull; p.work_col[pos++] = ((uint32_t)tile * (4u * WPT) + (uint32_t)b) | near; }
 }
 
 }  // namespace vf

@@ -148,7 +148,7 @@ extern "C" int vol_create(vol_t **out, const int32_t dims_geo[3], int32_t r, con
     p.local_nz = local_nz;
     p.tiles_x = (p.nx + vf::TX - 1) / vf::TX; p.tiles_y = (p.ny + vf::TY - 1) / vf::TY; p.tiles_z_local = my_slabs;
     const int64_t n_tiles = (int64_t)p.tiles_x * p.tiles_y * my_slabs;
-    if (n_tiles * 16 >= (int64_t)vf::ITEM_ID) { delete v; return VOL_E_ARG; }
+    if (n_tiles * 64 >= (int64_t)vf::ITEM_ID) { delete v; return VOL_E_ARG; }
     p.n_tiles = (int)n_tiles;
     p.ox = origin_m[0]; p.oy = origin_m[1]; p.oz = origin_m[2];
     p.vs = extent_m / (float)p.nx;
@@ -176,7 +176,7 @@ extern "C" int vol_create(vol_t **out, const int32_t dims_geo[3], int32_t r, con
     if (v->col_bytes && cudaMemset(p.col, 0, v->col_bytes) != cudaSuccess) rc = VOL_E_CUDA;
     const size_t nt = (size_t)(p.n_tiles > 0 ? p.n_tiles : 1), nw = nt * (size_t)vf::words_per_tile(r);
     if (cudaMalloc(&p.work_geo, sizeof(uint32_t) * nt) != cudaSuccess) rc = VOL_E_OOM;
-    if (cudaMalloc(&p.work_col, sizeof(uint32_t) * nw) != cudaSuccess) rc = VOL_E_OOM;
+    if (cudaMalloc(&p.work_col, sizeof(uint32_t) * nw * 4) != cudaSuccess) rc = VOL_E_OOM;
     if (cudaMalloc(&p.marks, sizeof(uint32_t) * nw) != cudaSuccess) rc = VOL_E_OOM;
     if (rc == VOL_OK && cudaMemset(p.marks, 0, sizeof(uint32_t) * nw) != cudaSuccess) rc = VOL_E_CUDA;
     if (cudaMalloc(&p.ctrl, sizeof(uint32_t) * vf::CTRL_N) != cudaSuccess) rc = VOL_E_OOM;
