@@ -152,6 +152,22 @@ def run_reference(args, rank):
     print(json.dumps(out), flush=True)
 
 
+def max_over_ranks(values, world, device):
+    """Device times are reported as the MAX over ranks (one all-reduce; identity at world 1)."""
+    if world == 1:
+        return [float(v) for v in values]
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor(values, device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(v) for v in t]
+
+
+def whole_job_value(nvox_per_rank, steps, world, total_ms):
+    """Whole-job aggregate: voxels brought up to date by all ranks / max-over-ranks device time."""
+    return world * nvox_per_rank * steps / (total_ms * 1e-3)
+
+
 def run_ours(args, rank, world, local_rank):
     import torch
     import torch.distributed as dist
@@ -244,10 +260,7 @@ def run_ours(args, rank, world, local_rank):
     barrier()
     e2e_ms = float(t0.elapsed_time(t1))
 
-    if world > 1:
-        tt = torch.tensor([total_ms, e2e_ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        total_ms, e2e_ms = float(tt[0]), float(tt[1])
+    total_ms, e2e_ms = max_over_ranks([total_ms, e2e_ms], world, "cuda")
     clocks = sampler.stop() if sampler else None
     if rank != 0:
         if world > 1:
@@ -256,8 +269,8 @@ def run_ours(args, rank, world, local_rank):
 
     nvox = int(np.prod(c.dims_geo)) * (1 + c.r ** 3)
     ms_per_step = total_ms / K
-    value = world * nvox * K / (total_ms * 1e-3)
-    e2e_value = world * nvox * K / (e2e_ms * 1e-3)
+    value = whole_job_value(nvox, K, world, total_ms)
+    e2e_value = whole_job_value(nvox, K, world, e2e_ms)
     cnt = np.array(counters[W:], dtype=np.float64)
     frame_bytes = c.wd * c.hd * 2 + c.wh * c.hh * 3
     alg_bytes = 4.0 * cnt[:, :4].sum(axis=1) + frame_bytes        # per fused launch

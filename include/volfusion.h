@@ -116,6 +116,9 @@ int vol_upload(vol_t *v, const void *geo_host, const void *col_host, void *strea
 /* Zero both volumes (asynchronous). */
 int vol_reset(vol_t *v, void *stream);
 int vol_info(const vol_t *v, vol_info_t *out);
+/* Host-only helper (no CUDA call): the geometry layers rank `shard_rank` of `shard_world` owns out of nz, in storage order.
+ * Writes at most `cap` of them to layers_out (HOST, nullable) and returns how many there are, or VOL_E_ARG. */
+int vol_shard_layers(int32_t nz, int32_t shard_rank, int32_t shard_world, int32_t *layers_out, int32_t cap);
 /* Enable (1) / disable (0) the four voxel counters of vol_stats_t (a separately compiled kernel variant). */
 int vol_set_counting(vol_t *v, int32_t on);
 /* Statistics of the last frame (synchronises `stream`; copies 48 bytes device -> host). */

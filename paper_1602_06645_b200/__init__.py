@@ -26,7 +26,7 @@ NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", 
               "-Xcompiler", "-fPIC,-ffp-contract=off", "-shared"]
 
 EXPORTS = ["vol_create", "vol_integrate", "vol_integrate_host", "vol_download", "vol_download_voxels", "vol_upload",
-           "vol_reset", "vol_info", "vol_set_counting", "vol_frame_stats", "vol_set_profiling", "vol_last_kernel_ms",
+           "vol_reset", "vol_info", "vol_shard_layers", "vol_set_counting", "vol_frame_stats", "vol_set_profiling", "vol_last_kernel_ms",
            "vol_launches_per_frame", "vol_selftest", "vol_destroy", "vol_strerror"]
 
 
@@ -78,6 +78,7 @@ def lib():
         L.vol_upload.argtypes = [P, P, P, P]
         L.vol_reset.argtypes = [P, P]
         L.vol_info.argtypes = [P, P]
+        L.vol_shard_layers.argtypes = [I32, I32, I32, P, I32]
         L.vol_set_counting.argtypes = [P, I32]
         L.vol_frame_stats.argtypes = [P, P, P]
         L.vol_set_profiling.argtypes = [P, I32]
@@ -128,6 +129,15 @@ def _stream_ptr(stream):
     if stream is None:
         return None
     return getattr(stream, "cuda_stream", stream)
+
+
+def shard_layers(nz: int, shard_rank: int, shard_world: int):
+    """vol_shard_layers: the geometry layers (global indices, storage order) that rank `shard_rank` of `shard_world` owns."""
+    n = lib().vol_shard_layers(int(nz), int(shard_rank), int(shard_world), None, 0)
+    _check(min(n, 0), "vol_shard_layers")
+    out = np.empty(n, dtype=np.int32)
+    _check(min(lib().vol_shard_layers(int(nz), int(shard_rank), int(shard_world), out.ctypes.data, n), 0), "vol_shard_layers")
+    return out
 
 
 def selftest(exhaustive: bool = False):

@@ -426,6 +426,15 @@ extern "C" int vol_info(const vol_t *v, vol_info_t *o)
     return VOL_OK;
 }
 
+extern "C" int vol_shard_layers(int32_t nz, int32_t rank, int32_t world, int32_t *layers_out, int32_t cap)
+{
+    if (nz <= 0 || world <= 0 || rank < 0 || rank >= world || cap < 0) return VOL_E_ARG;
+    int n = 0;
+    for (int k = 0; k < nz; ++k)
+        if ((k / vf::TZ) % world == rank) { if (layers_out && n < cap) layers_out[n] = k; ++n; }
+    return n;
+}
+
 extern "C" int vol_set_counting(vol_t *v, int32_t on) { if (!v) return VOL_E_ARG; v->counting = on != 0; return VOL_OK; }
 extern "C" int vol_set_profiling(vol_t *v, int32_t on) { if (!v) return VOL_E_ARG; v->profiling = on != 0; v->ev_valid = false; return VOL_OK; }
 extern "C" int vol_launches_per_frame(const vol_t *v) { return v ? 4 : VOL_E_ARG; }
