@@ -104,6 +104,8 @@ struct Counts { unsigned long long gr, gc, cr, cc; };
 
 // one geometry tile, one warp: lane = (vx = lane & 7, y = lane >> 3) owns voxels (gx0 + 4 vx .. + 3, gy0 + y) of every layer.
 // NEAR tiles (may hold voxels with Z <= 0 or outside rcp_exact's range) take the plain per-voxel routine.
+// Otherwise the layers are software-pipelined: while layer z is updated, layer z + 1 has already been projected and its
+// four depth gathers and its voxel vector are in flight.
 template <bool COUNT>
 __device__ __forceinline__ void geometry_tile(const Params &p, uint32_t item, int lane, Counts &c)
 {
@@ -112,7 +114,9 @@ __device__ __forceinline__ void geometry_tile(const Params &p, uint32_t item, in
     const int ttx = tile % p.tiles_x, t2 = tile / p.tiles_x, tty = t2 % p.tiles_y, ttz = t2 / p.tiles_y;
     const int i0 = ttx * TX + 4 * (lane & 7), j = tty * TY + (lane >> 3);
     const int gz0 = local_to_global_tz(p, ttz) * TZ, lz0 = ttz * TZ;
-    if (!(i0 < p.nx && j < p.ny)) return;                 // ragged tile: no warp-wide operation below
+    const bool inside = i0 < p.nx && j < p.ny;
+    const unsigned lanes = __ballot_sync(0xffffffffu, inside);    // ragged tile: the votes below name only these lanes
+    if (!inside) return;
     const int nl = min(TZ, p.nz - gz0);
     // per-column bases of eq. 5: fma(R_1, py, fma(R_0, px, t)) -- the z term is added per layer with one fma each
     const float py = __fmaf_rn((float)j + 0.5f, p.vs, p.oy);
@@ -124,45 +128,77 @@ __device__ __forceinline__ void geometry_tile(const Params &p, uint32_t item, in
         bY[e] = __fmaf_rn(p.R[4], py, __fmaf_rn(p.R[3], px, p.t[1]));
         bZ[e] = __fmaf_rn(p.R[7], py, __fmaf_rn(p.R[6], px, p.t[2]));
     }
-    const float fx = p.fx, fy = p.fy, cx = p.cx, cy = p.cy, r02 = p.R[2], r12 = p.R[5], r22 = p.R[8];
+    const float r02 = p.R[2], r12 = p.R[5], r22 = p.R[8];
+    const size_t layer = (size_t)p.ny * p.nx;
+    uint4 *ptr = reinterpret_cast<uint4 *>(p.geo + ((size_t)lz0 * p.ny + j) * p.nx + i0);
+    if (near) {
+        for (int z = 0; z < nl; ++z) {
+            const uint4 cur = *ptr;
+            const float pz = __fmaf_rn((float)(gz0 + z) + 0.5f, p.vs, p.oz);
+            const uint32_t o4[4] = {cur.x, cur.y, cur.z, cur.w};
+            uint32_t w4[4];
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {
+                bool rd = false;
+                w4[e] = geo_voxel_ref(p, __fmaf_rn(r02, pz, bX[e]), __fmaf_rn(r12, pz, bY[e]), __fmaf_rn(r22, pz, bZ[e]), o4[e], rd);
+                if (COUNT) { c.gr += rd; c.gc += w4[e] != o4[e]; }
+            }
+            if ((w4[0] != o4[0]) | (w4[1] != o4[1]) | (w4[2] != o4[2]) | (w4[3] != o4[3])) *ptr = make_uint4(w4[0], w4[1], w4[2], w4[3]);
+            ptr = reinterpret_cast<uint4 *>(reinterpret_cast<uint32_t *>(ptr) + layer);
+        }
+        return;
+    }
+    const float fx = p.fx, fy = p.fy, cx = p.cx, cy = p.cy;
     const float neg_mu = p.neg_mu, inv_mu = p.inv_mu;
     const uint32_t wd = (uint32_t)p.wd, wbits = __float_as_uint(p.wd_f), hbits = __float_as_uint(p.hd_f), koff = 0x4B400000u * (wd + 1u);
     const int w_max = p.w_max;
     const uint16_t *__restrict__ depth = p.depth;
-    const size_t layer = (size_t)p.ny * p.nx;
-    uint4 *ptr = reinterpret_cast<uint4 *>(p.geo + ((size_t)lz0 * p.ny + j) * p.nx + i0);
+    // S2 of one layer: eq. 5 z term, projection, and the four depth gathers (offset 0 when outside: a valid address)
+    auto project_layer = [&](int z, float (&Z)[4], uint32_t (&d)[4], unsigned &okm) {
+        const float pz = __fmaf_rn((float)(gz0 + z) + 0.5f, p.vs, p.oz);
+        okm = 0u;
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+            const float X = __fmaf_rn(r02, pz, bX[e]), Y = __fmaf_rn(r12, pz, bY[e]);
+            Z[e] = __fmaf_rn(r22, pz, bZ[e]);
+            bool ok; uint32_t off;
+            project_fast(fx, fy, cx, cy, wd, wbits, hbits, koff, X, Y, Z[e], ok, off);
+            okm |= (ok ? 1u : 0u) << e;
+            d[e] = __ldg(depth + off);
+        }
+    };
+    float Zc[4]; uint32_t dc[4]; unsigned okc;
     uint4 cur = *ptr;
+    project_layer(0, Zc, dc, okc);
     for (int z = 0; z < nl; ++z) {
         uint4 nxt = cur;
         uint4 *pn = reinterpret_cast<uint4 *>(reinterpret_cast<uint32_t *>(ptr) + layer);
-        if (z + 1 < nl) nxt = *pn;                                // prefetch the next layer while this one is computed
-        const float pz = __fmaf_rn((float)(gz0 + z) + 0.5f, p.vs, p.oz);
-        float X[4], Y[4], Z[4];
-#pragma unroll
-        for (int e = 0; e < 4; ++e) {                             // eq. 5: z term
-            X[e] = __fmaf_rn(r02, pz, bX[e]); Y[e] = __fmaf_rn(r12, pz, bY[e]); Z[e] = __fmaf_rn(r22, pz, bZ[e]);
-        }
+        float Zn[4] = {0.f, 0.f, 0.f, 0.f}; uint32_t dn[4] = {0u, 0u, 0u, 0u}; unsigned okn = 0u;
+        if (z + 1 < nl) { nxt = *pn; project_layer(z + 1, Zn, dn, okn); }    // next layer in flight
         const uint32_t o4[4] = {cur.x, cur.y, cur.z, cur.w};
         uint32_t w4[4];
-        if (near) {
+        float sdf[4]; bool upd[4];
+        bool easy = true;
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {                             // S3: truncation test
+            const float D = __fmul_rn((float)dc[e], 0.001f);
+            sdf[e] = __fsub_rn(D, Zc[e]);
+            upd[e] = ((okc >> e) & 1u) && (dc[e] != 0u) && !(sdf[e] < neg_mu);
+            // saturated free space (tsdf = 1 onto q = 32767) or first touch (w = 0): the running average is 32767 exactly,
+            // fma(32767, w, 32767) / (w + 1) with every intermediate below 2^24
+            easy = easy && (!upd[e] || (__fmul_rn(sdf[e], inv_mu) >= 1.0f && ((o4[e] & 0xffffu) == 0x7fffu || (o4[e] >> 16) == 0u)));
+            if (COUNT) c.gr += upd[e];
+        }
+        if (__all_sync(lanes, easy)) {                            // whole warp in free space: no division needed
 #pragma unroll
             for (int e = 0; e < 4; ++e) {
-                bool rd = false;
-                w4[e] = geo_voxel_ref(p, X[e], Y[e], Z[e], o4[e], rd);
-                if (COUNT) c.gr += rd;
+                const int wn = min((int)(short)(o4[e] >> 16) + 1, w_max);
+                w4[e] = upd[e] ? (0x7fffu | ((uint32_t)wn << 16)) : o4[e];
             }
         } else {
-            uint32_t off[4], d[4]; bool ok[4];
 #pragma unroll
-            for (int e = 0; e < 4; ++e) project_fast(fx, fy, cx, cy, wd, wbits, hbits, koff, X[e], Y[e], Z[e], ok[e], off[e]);   // S2
-#pragma unroll
-            for (int e = 0; e < 4; ++e) d[e] = __ldg(depth + off[e]);  // gather D_n (offset 0 when !ok: a valid address)
-#pragma unroll
-            for (int e = 0; e < 4; ++e) {                         // S3: truncation test + running average
-                const float D = __fmul_rn((float)d[e], 0.001f);
-                const float sdf = __fsub_rn(D, Z[e]);
-                const bool upd = ok[e] && (d[e] != 0u) && !(sdf < neg_mu);
-                const float tsdf = fminf(1.0f, __fmul_rn(sdf, inv_mu));
+            for (int e = 0; e < 4; ++e) {                         // S3: running average
+                const float tsdf = fminf(1.0f, __fmul_rn(sdf[e], inv_mu));
                 const int q = (int)(short)(o4[e] & 0xffffu);
                 const int wi = (int)(short)(o4[e] >> 16);
                 const float wf = (float)wi;
@@ -174,14 +210,15 @@ __device__ __forceinline__ void geometry_tile(const Params &p, uint32_t item, in
                 const uint32_t qn = __float_as_uint(__fadd_rn(div_with(num, den, div_prepare(den)), 12582912.0f));
                 const int wn = min(wi + 1, w_max);
                 const uint32_t nw = (qn & 0xffffu) | ((uint32_t)wn << 16);
-                w4[e] = upd ? nw : o4[e];
-                if (COUNT) c.gr += upd;
+                w4[e] = upd[e] ? nw : o4[e];
             }
         }
         const bool any = (w4[0] != o4[0]) | (w4[1] != o4[1]) | (w4[2] != o4[2]) | (w4[3] != o4[3]);
         if (COUNT) c.gc += (w4[0] != o4[0]) + (w4[1] != o4[1]) + (w4[2] != o4[2]) + (w4[3] != o4[3]);
         if (any) *ptr = make_uint4(w4[0], w4[1], w4[2], w4[3]);   // skip the store when nothing changed
-        ptr = pn; cur = nxt;
+        ptr = pn; cur = nxt; okc = okn;
+#pragma unroll
+        for (int e = 0; e < 4; ++e) { Zc[e] = Zn[e]; dc[e] = dn[e]; }
     }
 }
 

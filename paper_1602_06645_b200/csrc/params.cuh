@@ -145,13 +145,16 @@ __device__ __forceinline__ bool box_rect(const Params &p, float cX, float cY, fl
 
 // culling only: can any voxel of the camera-space box (centre c, half extents e) pass the TSDF tests (frustum, valid
 // depth, sdf >= -mu)?  Conservative: max valid depth over the box's pixel rectangle against the box's nearest Z.
-__device__ __forceinline__ bool box_may_update(const Params &p, float cX, float cY, float cZ, float eX, float eY, float eZ)
+// Returns 0 = no, 1 = maybe, 2 = maybe and the whole box lies in front of every valid depth of its rectangle (free space:
+// a finer look at the box would find the same).
+__device__ __forceinline__ int box_may_update(const Params &p, float cX, float cY, float cZ, float eX, float eY, float eZ)
 {
     int x0, x1, y0, y1; float zmin, zmax;
-    if (!box_rect(p, cX, cY, cZ, eX, eY, eZ, x0, x1, y0, y1, zmin, zmax)) return false;
+    if (!box_rect(p, cX, cY, cZ, eX, eY, eZ, x0, x1, y0, y1, zmin, zmax)) return 0;
     uint32_t mn, mx;
     depth_range(p, x0, x1, y0, y1, mn, mx);
-    return mx != 0u && zmin <= ((float)mx * 0.001f + 1e-4f) + p.mu;
+    if (mx == 0u || !(zmin <= ((float)mx * 0.001f + 1e-4f) + p.mu)) return 0;
+    return zmax <= (float)mn * 0.001f - 1e-4f ? 2 : 1;
 }
 
 }  // namespace vf

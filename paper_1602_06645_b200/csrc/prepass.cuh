@@ -299,7 +299,8 @@ __global__ void __launch_bounds__(256) k_classify(const __grid_constant__ Params
         const float cY = p.R[3] * wx + p.R[4] * wy + p.R[5] * wz + p.t[1];
         const float cZ = p.R[6] * wx + p.R[7] * wy + p.R[8] * wz + p.t[2];
         if (!(cZ - p.tile_ez > 2e-3f)) near = ITEM_NEAR;
-        if (box_may_update(p, cX, cY, cZ, p.tile_ex, p.tile_ey, p.tile_ez)) {
+        const int coarse = box_may_update(p, cX, cY, cZ, p.tile_ex, p.tile_ey, p.tile_ez);
+        if (coarse != 0) {
             const float sx = (float)(TX / SUBX) * p.vs, sz = (float)(TZ / SUBZ) * p.vs;
 #pragma unroll
             for (int bz = 0; bz < SUBZ; ++bz)
@@ -307,7 +308,7 @@ __global__ void __launch_bounds__(256) k_classify(const __grid_constant__ Params
                 for (int bx = 0; bx < SUBX; ++bx) {
                     const float dx = ((float)bx - 0.5f * (float)(SUBX - 1)) * sx, dz = ((float)bz - 0.5f * (float)(SUBZ - 1)) * sz;
                     if (!geo) geo = box_may_update(p, cX + p.R[0] * dx + p.R[2] * dz, cY + p.R[3] * dx + p.R[5] * dz,
-                                                   cZ + p.R[6] * dx + p.R[8] * dz, p.sub_ex, p.sub_ey, p.sub_ez);
+                                                   cZ + p.R[6] * dx + p.R[8] * dz, p.sub_ex, p.sub_ey, p.sub_ez) != 0;
                 }
         }
 #pragma unroll
