@@ -384,6 +384,7 @@ __global__ void __launch_bounds__(CTA, 4) k_fused(const __grid_constant__ Params
     __shared__ Stage s_stage[WARPS_PER_CTA];
     const int lane = threadIdx.x & 31;
     Stage &st = s_stage[threadIdx.x >> 5];
+    pdl_wait();
     const uint32_t n_col = __ldcg(&p.ctrl[CTRL_NCOL]), n_items = n_col + __ldcg(&p.ctrl[CTRL_NGEO]);
     Counts c = {0, 0, 0, 0};
     int n_staged = 0;

@@ -74,6 +74,11 @@ constexpr uint32_t ITEM_NEAR = 1u << 31, ITEM_ID = ITEM_NEAR - 1u;
 
 enum { CTRL_NGEO = 0, CTRL_NCOL = 1, CTRL_CURSOR = 2, CTRL_TICKET = 3, CTRL_CELLS = 4, CTRL_NJOBS = 5, CTRL_N = 8 };
 
+// programmatic dependent launch: wait for the previous kernel of the stream (completion + memory flush) / allow the next
+// kernel's CTAs to be scheduled as this one drains
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
 // local slab index -> global slab index; slabs of TZ = VOL_SLAB geometry layers are dealt round-robin to ranks
 __device__ __forceinline__ int local_to_global_tz(const Params &p, int tz_local) { return tz_local * p.shard_world + p.shard_rank; }
 

@@ -120,6 +120,7 @@ __global__ void __launch_bounds__(256) k_prepass(const __grid_constant__ Params 
     __shared__ uint32_t s_njobs, s_base;
     __shared__ uint4 s_jobs[1024];      // mark jobs: {x | y << 15 | (4 x 4 patch ? 1 << 31 : single pixel), depth range of its eligible pixels}
     const int t = threadIdx.x, tx = t & 31, tq = t >> 5;
+    pdl_launch_dependents();
     if (t < 16) { s_mn[t] = 0xffffu; s_mx[t] = 0u; }
     if (t == 0) s_njobs = 0u;
     if (blockIdx.x == 0 && blockIdx.y == 0 && t == 0) {
@@ -264,6 +265,8 @@ __global__ void __launch_bounds__(256) k_prepass(const __grid_constant__ Params 
 template <int R>
 __global__ void __launch_bounds__(256) k_mark(const __grid_constant__ Params p)
 {
+    pdl_launch_dependents();
+    pdl_wait();
     const uint32_t njobs = __ldcg(&p.ctrl[CTRL_NJOBS]);
     const uint32_t g = (blockIdx.x * blockDim.x + threadIdx.x) >> 2, ng = (gridDim.x * blockDim.x) >> 2;
     for (uint32_t j = g; j < njobs; j += ng) {
@@ -285,6 +288,8 @@ __global__ void __launch_bounds__(256) k_classify(const __grid_constant__ Params
 {
     constexpr int WPT = words_per_tile(R);
     const int tile = blockIdx.x * blockDim.x + threadIdx.x;
+    pdl_launch_dependents();
+    pdl_wait();
     if (tile == 0) p.ctrl[CTRL_NJOBS] = 0u;            // the mark jobs of this frame have been consumed by k_mark
     bool geo = false;
     uint32_t near = 0;

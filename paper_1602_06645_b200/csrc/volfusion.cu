@@ -44,6 +44,18 @@ struct vol {
     bool ev_valid;
 };
 
+// one kernel launch; `dependent` = programmatic dependent launch on the previous kernel of the stream
+static cudaError_t launch(void (*kernel)(const Params), dim3 grid, int block, cudaStream_t s, bool dependent, const Params &p)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid; cfg.blockDim = dim3(block); cfg.dynamicSmemBytes = 0; cfg.stream = s;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at; cfg.numAttrs = dependent ? 1 : 0;
+    return cudaLaunchKernelEx(&cfg, kernel, p);
+}
+
 static int set_device(const vol *v) { CK(cudaSetDevice(v->device)); return VOL_OK; }
 
 // rigid inverse in fp64 with left-to-right sums, rounded once to fp32 (S0).  Returns false if T is not rigid.
@@ -283,15 +295,18 @@ extern "C" int vol_integrate(vol_t *v, const uint16_t *depth_u16_dev, int32_t wd
     const dim3 g0((wd + 31) / 32, (hd + 31) / 32);
     const int g1 = (p.n_tiles + 255) / 256, g2 = v->fused_blocks, gm = v->n_sms * 4;
     const bool cnt = v->counting;
+    // k_mark, k_classify and k_fused are launched with programmatic stream serialization: their CTAs may be scheduled
+    // while the predecessor drains (it signals griddepcontrol.launch_dependents), and they wait for its completion and
+    // memory flush with griddepcontrol.wait before touching anything it wrote.
 #define VF_LAUNCH(RR)                                                                   \
     do {                                                                                \
-        vf::k_prepass<RR><<<g0, 256, 0, s>>>(p);                                        \
-        vf::k_mark<RR><<<gm, 256, 0, s>>>(p);                                           \
+        CK(launch(vf::k_prepass<RR>, g0, 256, s, false, p));                            \
+        CK(launch(vf::k_mark<RR>, dim3(gm), 256, s, true, p));                          \
         if (v->profiling) CK(cudaEventRecord(v->ev[1], s));                             \
-        vf::k_classify<RR><<<g1, 256, 0, s>>>(p);                                       \
+        CK(launch(vf::k_classify<RR>, dim3(g1), 256, s, true, p));                      \
         if (v->profiling) CK(cudaEventRecord(v->ev[2], s));                             \
-        if (cnt) vf::k_fused<RR, true><<<g2, vf::CTA, 0, s>>>(p);                       \
-        else     vf::k_fused<RR, false><<<g2, vf::CTA, 0, s>>>(p);                      \
+        if (cnt) CK(launch(vf::k_fused<RR, true>, dim3(g2), vf::CTA, s, true, p));      \
+        else     CK(launch(vf::k_fused<RR, false>, dim3(g2), vf::CTA, s, true, p));     \
     } while (0)
     switch (p.r) {
         case 1: VF_LAUNCH(1); break;
