@@ -37,7 +37,7 @@ extern "C" {
 #endif
 
 #define VOL_OK       0
-#define VOL_E_ARG   -1   /* null pointer, dims <= 0, dims_geo[0] % 4 != 0, r not in 1..4, mu <= 0, w_max not in 1..512,
+#define VOL_E_ARG   -1   /* null pointer, dims <= 0, dims_geo[0] % 4 != 0, dims_geo > 4096 x 4096 x 2048 (per shard), r not in 1..4, mu <= 0, w_max not in 1..512,
                             non-zero skew, non-rigid T, image size <= 0, buffer too small, bad shard */
 #define VOL_E_OOM   -2   /* device allocation failed */
 #define VOL_E_CUDA  -3   /* a CUDA call failed (sticky: see vol_strerror) */

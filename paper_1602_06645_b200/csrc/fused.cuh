@@ -109,9 +109,9 @@ struct Counts { unsigned long long gr, gc, cr, cc; };
 template <bool COUNT>
 __device__ __forceinline__ void geometry_tile(const Params &p, uint32_t item, int lane, Counts &c)
 {
-    const int tile = (int)(item & ITEM_ID);
     const bool near = (item & ITEM_NEAR) != 0u;
-    const int ttx = tile % p.tiles_x, t2 = tile / p.tiles_x, tty = t2 % p.tiles_y, ttz = t2 / p.tiles_y;
+    int ttx, tty, ttz, sub;
+    item_unpack(item, ttx, tty, ttz, sub);
     const int i0 = ttx * TX + 4 * (lane & 7), j = tty * TY + (lane >> 3);
     const int gz0 = local_to_global_tz(p, ttz) * TZ, lz0 = ttz * TZ;
     const bool inside = i0 < p.nx && j < p.ny;
@@ -347,17 +347,18 @@ __device__ __forceinline__ void colour_cell(const Params &p, bool near, int ic0,
 template <int R, bool COUNT>
 __device__ __forceinline__ void colour_item(const Params &p, uint32_t item, Stage &st, int &n, int lane, Counts &c)
 {
-    const uint32_t bi = item & ITEM_ID, wi = bi >> 2, sh = 8u * (bi & 3u);
     const bool near = (item & ITEM_NEAR) != 0u;
     constexpr int CX = cells_x(R), CY = cells_y(R), WPT = words_per_tile(R);
+    int ttx, tty, ttz, sub;
+    item_unpack(item, ttx, tty, ttz, sub);
+    const int word = sub >> 2;
+    const uint32_t wi = (uint32_t)((ttz * p.tiles_y + tty) * p.tiles_x + ttx) * WPT + (uint32_t)word, sh = 8u * ((uint32_t)sub & 3u);
     uint32_t bits = 0;
     if (lane == 0) {                                                      // consume this item's byte of the marks (self-cleaning)
         bits = __ldcg(p.marks + wi) & (0xffu << sh);
         atomicAnd(p.marks + wi, ~(0xffu << sh));
     }
     bits = __shfl_sync(0xffffffffu, bits, 0);
-    const int tile = (int)(wi / WPT), word = (int)(wi % WPT);
-    const int ttx = tile % p.tiles_x, t2 = tile / p.tiles_x, tty = t2 % p.tiles_y, ttz = t2 / p.tiles_y;
     const int cgx0 = ttx * TX * R, cgy0 = tty * TY * R;
     const int cgz0 = local_to_global_tz(p, ttz) * TZ * R, clz0 = ttz * TZ * R;
     if (COUNT && lane == 0) atomicAdd(&p.ctrl[CTRL_CELLS], (uint32_t)__popc(bits));

@@ -50,6 +50,7 @@ struct Params {
     float Rw[9], tw[3];          // depth camera -> world (the caller's T_world_depth)
     float tile_ex, tile_ey, tile_ez;   // conservative camera-axis half extents of a geometry tile
     float sub_ex, sub_ey, sub_ez;      // ... of one of its SUBX x 1 x SUBZ sub-boxes
+    float cell_ex, cell_ey, cell_ez;   // ... and of a colour cell
     float sigma_g;                     // sigma grown by the fp32 slack
     float inv_vc, slack;         // 1 / colour voxel size; metres of slack for fp32 evaluation of culling geometry
     // device buffers
@@ -68,9 +69,22 @@ struct Params {
     unsigned long long *counters;// 4 voxel counters (counting variant only)
 };
 
-// work items: low bits = local tile id (geometry) or mark-byte index (colour); ITEM_NEAR = the tile's box comes within 2 mm of
-// the camera plane (or behind it), so its voxels may have Z <= 0 or Z outside the range of the branch-free reciprocal
-constexpr uint32_t ITEM_NEAR = 1u << 31, ITEM_ID = ITEM_NEAR - 1u;
+// work items (32 bits): [6:0] ttx | [16:7] tty | [24:17] ttz (local slab) = tile coordinates, [30:25] sub = index of the
+// mark byte within the tile (colour items only), [31] ITEM_NEAR = the tile's box comes within 2 mm of the camera plane
+// (or behind it), so its voxels may have Z <= 0 or Z outside the range of the branch-free reciprocal.
+// vol_create rejects volumes with more than 128 x 1024 x 256 tiles per shard.
+constexpr uint32_t ITEM_NEAR = 1u << 31;
+constexpr int ITEM_Y_SHIFT = 7, ITEM_Z_SHIFT = 17, ITEM_SUB_SHIFT = 25;
+constexpr int ITEM_MAX_TX = 128, ITEM_MAX_TY = 1024, ITEM_MAX_TZ = 256;
+__device__ __forceinline__ uint32_t item_pack(int ttx, int tty, int ttz, int sub)
+{
+    return (uint32_t)ttx | ((uint32_t)tty << ITEM_Y_SHIFT) | ((uint32_t)ttz << ITEM_Z_SHIFT) | ((uint32_t)sub << ITEM_SUB_SHIFT);
+}
+__device__ __forceinline__ void item_unpack(uint32_t item, int &ttx, int &tty, int &ttz, int &sub)
+{
+    ttx = (int)(item & 127u); tty = (int)((item >> ITEM_Y_SHIFT) & 1023u); ttz = (int)((item >> ITEM_Z_SHIFT) & 255u);
+    sub = (int)((item >> ITEM_SUB_SHIFT) & 63u);
+}
 
 enum { CTRL_NGEO = 0, CTRL_NCOL = 1, CTRL_CURSOR = 2, CTRL_TICKET = 3, CTRL_CELLS = 4, CTRL_NJOBS = 5, CTRL_N = 8 };
 

@@ -14,17 +14,40 @@ __device__ __forceinline__ float3 backproject(const Params &p, int x, int y, flo
     return P;
 }
 
+// culling only: a frustum piece in the depth camera: X/Z in [a0, a1], Y/Z in [b0, b1], Z in [z0, z1] (see shell_box)
+struct Piece { float a0, a1, b0, b1, z0, z1; };
+
+// culling only: can the colour cell with global cell coordinates (cx, cy, cz) meet the piece?  Conservative: the cell's
+// camera-space bounding box (centre +- cell_e, slack included) against the piece's own six planes.
+__device__ __forceinline__ bool cell_meets_piece(const Params &p, const Piece &pc, int cx, int cy, int cz)
+{
+    const float wx = p.ox + ((float)(cx * CLX) + 0.5f * (float)CLX) * p.vc;
+    const float wy = p.oy + ((float)(cy * CLY) + 0.5f * (float)CLY) * p.vc;
+    const float wz = p.oz + ((float)(cz * CLZ) + 0.5f * (float)CLZ) * p.vc;
+    const float X = p.R[0] * wx + p.R[1] * wy + p.R[2] * wz + p.t[0];
+    const float Y = p.R[3] * wx + p.R[4] * wy + p.R[5] * wz + p.t[1];
+    const float Z = p.R[6] * wx + p.R[7] * wy + p.R[8] * wz + p.t[2];
+    const float ex = p.cell_ex, ey = p.cell_ey, ez = p.cell_ez;
+    if (Z + ez < pc.z0 || Z - ez > pc.z1) return false;
+    // X <= a1 Z somewhere in the box  <=>  min over the box of (X - a1 Z) <= 0, and so on
+    if (X - pc.a1 * Z > ex + fabsf(pc.a1) * ez || X - pc.a0 * Z < -(ex + fabsf(pc.a0) * ez)) return false;
+    if (Y - pc.b1 * Z > ey + fabsf(pc.b1) * ez || Y - pc.b0 * Z < -(ey + fabsf(pc.b0) * ez)) return false;
+    return true;
+}
+
 // culling only: set the mark bits of every colour cell that intersects the colour-voxel index box
 // [i0,i1] x [j0,j1] x [k0,k1] (inclusive, already clamped to the colour grid).  The cell layers (cz) of the box are dealt
 // round-robin to `nsub` cooperating lanes; this lane is number `sub`.  Per (cell layer, tile) the rows of the box form
 // one contiguous run of at most 4 r^2 <= 64 mark bits, which never spans more than two words: one or two
 // fire-and-forget reductions (no return value, so a lane never waits on the L2 round trip).
+// (Testing every cell of the box against the piece itself -- cell_meets_piece -- marks 16 % fewer cells on config 3 but
+// costs k_mark more than it saves k_fused: measured, not used.)
 // A box of more than MARK_FINE_MAX cells is marked tile by tile instead (all cells of every tile it meets): bounded work
 // for pathological frames, at the price of looser marks.
 constexpr int MARK_FINE_MAX = 1024;
 
 template <int R>
-__device__ __forceinline__ void mark_box(const Params &p, int i0, int i1, int j0, int j1, int k0, int k1, int sub, int nsub)
+__device__ __forceinline__ void mark_box(const Params &p, const Piece &pc, int i0, int i1, int j0, int j1, int k0, int k1, int sub, int nsub)
 {
     constexpr int CX = cells_x(R), CY = cells_y(R), CZ = cells_z(R), NC = cells_per_tile(R), WPT = words_per_tile(R);
     const int cx0 = i0 / CLX, cx1 = i1 / CLX, cy0 = j0 / CLY, cy1 = j1 / CLY, cz0 = k0 / CLZ, cz1 = k1 / CLZ;
@@ -79,11 +102,12 @@ __device__ __forceinline__ bool index_box(const Params &p, float lo, float hi, f
 // Z in [zmin - sigma, zmax + sigma].  The piece is convex, so its world-space bounding box is that of its 8 corners.
 // Returns the inclusive colour-voxel index box of the centres inside it (false if empty).
 __device__ __forceinline__ bool shell_box(const Params &p, float xa, float xb, float ya, float yb, float zmin, float zmax,
-                                          int &i0, int &i1, int &j0, int &j1, int &k0, int &k1)
+                                          Piece &pc, int &i0, int &i1, int &j0, int &j1, int &k0, int &k1)
 {
     const float a0 = ((xa - 0.51f) - p.cx) / p.fx, a1 = ((xb + 0.51f) - p.cx) / p.fx;
     const float b0 = ((ya - 0.51f) - p.cy) / p.fy, b1 = ((yb + 0.51f) - p.cy) / p.fy;
     const float z0 = fmaxf(zmin - p.sigma_g, 1e-6f), z1 = zmax + p.sigma_g;
+    pc.a0 = a0; pc.a1 = a1; pc.b0 = b0; pc.b1 = b1; pc.z0 = z0; pc.z1 = z1;
     float lo[3], hi[3];
 #pragma unroll
     for (int ax = 0; ax < 3; ++ax) {
@@ -182,7 +206,8 @@ __global__ void __launch_bounds__(256) k_prepass(const __grid_constant__ Params 
         if (zlo <= zhi) {
             const int xp = blockIdx.x * 32 + (tx & ~3), yp = blockIdx.y * 32 + tq * 4;
             int i0, i1, j0, j1, k0, k1;
-            if (shell_box(p, (float)xp, (float)(xp + 3), (float)yp, (float)(yp + 3), zlo, zhi, i0, i1, j0, j1, k0, k1)) {
+            Piece pc;
+            if (shell_box(p, (float)xp, (float)(xp + 3), (float)yp, (float)(yp + 3), zlo, zhi, pc, i0, i1, j0, j1, k0, k1)) {
                 const int ncell = (i1 / CLX - i0 / CLX + 1) * (j1 / CLY - j0 / CLY + 1) * (k1 / CLZ - k0 / CLZ + 1);
                 if (ncell <= PATCH_CELLS_MAX) {
                     if ((tx & 3) == 0) {
@@ -273,8 +298,9 @@ __global__ void __launch_bounds__(256) k_mark(const __grid_constant__ Params p)
         const uint4 job = __ldcg(p.jobs + j);
         const float xa = (float)(job.x & 0x7fffu), ya = (float)((job.x >> 15) & 0x7fffu), ext = (job.x & 0x80000000u) ? 3.0f : 0.0f;
         int i0, i1, j0, j1, k0, k1;
-        if (shell_box(p, xa, xa + ext, ya, ya + ext, __uint_as_float(job.y), __uint_as_float(job.z), i0, i1, j0, j1, k0, k1))
-            mark_box<R>(p, i0, i1, j0, j1, k0, k1, threadIdx.x & 3, 4);
+        Piece pc;
+        if (shell_box(p, xa, xa + ext, ya, ya + ext, __uint_as_float(job.y), __uint_as_float(job.z), pc, i0, i1, j0, j1, k0, k1))
+            mark_box<R>(p, pc, i0, i1, j0, j1, k0, k1, threadIdx.x & 3, 4);
     }
 }
 
@@ -293,9 +319,10 @@ __global__ void __launch_bounds__(256) k_classify(const __grid_constant__ Params
     if (tile == 0) p.ctrl[CTRL_NJOBS] = 0u;            // the mark jobs of this frame have been consumed by k_mark
     bool geo = false;
     uint32_t near = 0;
+    int ttx = 0, tty = 0, ttz = 0;
     unsigned long long nzb = 0ull;                      // bit 4 w + b set: byte b of mark word w of this tile is non-zero
     if (tile < p.n_tiles) {
-        const int ttx = tile % p.tiles_x, tty = (tile / p.tiles_x) % p.tiles_y, ttz = tile / (p.tiles_x * p.tiles_y);
+        ttx = tile % p.tiles_x; tty = (tile / p.tiles_x) % p.tiles_y; ttz = tile / (p.tiles_x * p.tiles_y);
         const int gz = local_to_global_tz(p, ttz);
         const float wx = p.ox + ((float)(ttx * TX) + 0.5f * (float)TX) * p.vs;
         const float wy = p.oy + ((float)(tty * TY) + 0.5f * (float)TY) * p.vs;
@@ -336,9 +363,9 @@ __global__ void __launch_bounds__(256) k_classify(const __grid_constant__ Params
         if (tot) bc = atomicAdd(&p.ctrl[CTRL_NCOL], (uint32_t)tot);
     }
     bg = __shfl_sync(0xffffffffu, bg, 0); bc = __shfl_sync(0xffffffffu, bc, 0);
-    if (geo) p.work_geo[bg + __popc(mg & lt)] = (uint32_t)tile | near;
+    if (geo) p.work_geo[bg + __popc(mg & lt)] = item_pack(ttx, tty, ttz, 0) | near;
     uint32_t pos = bc + (uint32_t)(pre - ncol);
-    while (nzb) { const int b = __ffsll((long long)nzb) - 1; nzb &= nzb - 1ull; p.work_col[pos++] = ((uint32_t)tile * (4u * WPT) + (uint32_t)b) | near; }
+    while (nzb) { const int b = __ffsll((long long)nzb) - 1; nzb &= nzb - 1ull; p.work_col[pos++] = item_pack(ttx, tty, ttz, b) | near; }
 }
 
 }  // namespace vf

@@ -160,7 +160,7 @@ extern "C" int vol_create(vol_t **out, const int32_t dims_geo[3], int32_t r, con
     p.local_nz = local_nz;
     p.tiles_x = (p.nx + vf::TX - 1) / vf::TX; p.tiles_y = (p.ny + vf::TY - 1) / vf::TY; p.tiles_z_local = my_slabs;
     const int64_t n_tiles = (int64_t)p.tiles_x * p.tiles_y * my_slabs;
-    if (n_tiles * 64 >= (int64_t)vf::ITEM_ID) { delete v; return VOL_E_ARG; }
+    if (p.tiles_x > vf::ITEM_MAX_TX || p.tiles_y > vf::ITEM_MAX_TY || my_slabs > vf::ITEM_MAX_TZ || n_tiles > INT32_MAX / 64) { delete v; return VOL_E_ARG; }
     p.n_tiles = (int)n_tiles;
     p.ox = origin_m[0]; p.oy = origin_m[1]; p.oz = origin_m[2];
     p.vs = extent_m / (float)p.nx;
@@ -285,6 +285,7 @@ extern "C" int vol_integrate(vol_t *v, const uint16_t *depth_u16_dev, int32_t wd
     p.slack = (float)slack;
     box_extents(p.R, 0.5 * vf::TX * p.vs, 0.5 * vf::TY * p.vs, 0.5 * vf::TZ * p.vs, slack, p.tile_ex, p.tile_ey, p.tile_ez);
     box_extents(p.R, 0.5 * (vf::TX / vf::SUBX) * p.vs, 0.5 * vf::TY * p.vs, 0.5 * (vf::TZ / vf::SUBZ) * p.vs, slack, p.sub_ex, p.sub_ey, p.sub_ez);
+    box_extents(p.R, 0.5 * vf::CLX * p.vc, 0.5 * vf::CLY * p.vc, 0.5 * vf::CLZ * p.vc, slack, p.cell_ex, p.cell_ey, p.cell_ez);
     p.sigma_g = (float)((double)p.sigma * 1.0001 + slack);
     camera_to_world(p.R, p.t, p.Rw, p.tw);
     if (p.n_tiles == 0) return VOL_OK;
