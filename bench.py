@@ -58,12 +58,17 @@ def peaks():
 
 
 def ncu_traffic(workload):
-    """DRAM bytes per fused-kernel launch from the committed ncu --set full capture, if one is recorded."""
+    """DRAM bytes (dram__bytes_read.sum + dram__bytes_write.sum) per k_fused launch from the committed ncu --set full
+    capture of this workload (profiles/traffic.csv: workload,kernel,dram_bytes_per_launch), or None if none is recorded."""
     try:
-        with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
-            return json.load(f).get(workload, {}).get("fused_dram_bytes_per_launch")
+        with open(os.path.join(ROOT, "profiles", "traffic.csv")) as f:
+            for line in f:
+                cols = [c.strip() for c in line.split(",")]
+                if len(cols) >= 3 and cols[0] == workload and cols[1] == "k_fused":
+                    return float(cols[2])
     except Exception:
-        return None
+        pass
+    return None
 
 
 class ClockSampler(threading.Thread):

@@ -124,7 +124,7 @@ int vol_set_counting(vol_t *v, int32_t on);
 /* Statistics of the last frame (synchronises `stream`; copies 48 bytes device -> host). */
 int vol_frame_stats(vol_t *v, vol_stats_t *out, void *stream);
 /* Enable per-kernel CUDA-event timing of subsequent vol_integrate calls / read the last frame's kernel times in
- * milliseconds: ms[0] pre-pass + shell marks (S1), ms[1] tile classification (S9), ms[2] fused integrate (S2-S8).  Synchronises. */
+ * milliseconds: ms[0] pre-pass, shell marks and geometry tile classification (S1, S9), ms[1] colour work items (S9), ms[2] fused integrate (S2-S8).  Synchronises. */
 int vol_set_profiling(vol_t *v, int32_t on);
 int vol_last_kernel_ms(vol_t *v, float ms[3]);
 /* Number of kernels one vol_integrate call launches. */

@@ -286,63 +286,98 @@ __global__ void __launch_bounds__(256) k_prepass(const __grid_constant__ Params 
     if (t == 0) p.ctrl[CTRL_TICKET] = 0;
 }
 
-// K0b -- S1 (c) continued: one group of 4 lanes per queued job (grid-stride); the 4 lanes share the job's cell layers.
-template <int R>
-__global__ void __launch_bounds__(256) k_mark(const __grid_constant__ Params p)
+// camera-space centre of geometry tile (ttx, tty, ttz local) -- culling only
+__device__ __forceinline__ void tile_centre(const Params &p, int ttx, int tty, int ttz, float &cX, float &cY, float &cZ)
 {
-    pdl_launch_dependents();
-    pdl_wait();
-    const uint32_t njobs = __ldcg(&p.ctrl[CTRL_NJOBS]);
-    const uint32_t g = (blockIdx.x * blockDim.x + threadIdx.x) >> 2, ng = (gridDim.x * blockDim.x) >> 2;
-    for (uint32_t j = g; j < njobs; j += ng) {
-        const uint4 job = __ldcg(p.jobs + j);
-        const float xa = (float)(job.x & 0x7fffu), ya = (float)((job.x >> 15) & 0x7fffu), ext = (job.x & 0x80000000u) ? 3.0f : 0.0f;
-        int i0, i1, j0, j1, k0, k1;
-        Piece pc;
-        if (shell_box(p, xa, xa + ext, ya, ya + ext, __uint_as_float(job.y), __uint_as_float(job.z), pc, i0, i1, j0, j1, k0, k1))
-            mark_box<R>(p, pc, i0, i1, j0, j1, k0, k1, threadIdx.x & 3, 4);
-    }
+    const int gz = local_to_global_tz(p, ttz);
+    const float wx = p.ox + ((float)(ttx * TX) + 0.5f * (float)TX) * p.vs;
+    const float wy = p.oy + ((float)(tty * TY) + 0.5f * (float)TY) * p.vs;
+    const float wz = p.oz + ((float)(gz * TZ) + 0.5f * (float)TZ) * p.vs;
+    cX = p.R[0] * wx + p.R[1] * wy + p.R[2] * wz + p.t[0];
+    cY = p.R[3] * wx + p.R[4] * wy + p.R[5] * wz + p.t[1];
+    cZ = p.R[6] * wx + p.R[7] * wy + p.R[8] * wz + p.t[2];
 }
 
-// K1 -- S9: one thread per geometry tile of this shard.
-//  geometry: conservative test of the tile's camera-space box against the depth pyramid (any voxel with sdf >= -mu?),
-//            refined on SUBX x 1 x SUBZ sub-boxes for tiles that pass;
-//  colour:   one work item per non-zero BYTE of the tile's shell-mark words, i.e. up to 8 colour cells (heavier than a
-//            geometry tile, listed first in the fused kernel's queue).
+// K1 -- one launch, two roles that both depend only on k_prepass and so run side by side:
+//  blocks [0, n_geo_blocks): S9 for geometry, one thread per tile of this shard: conservative test of the tile's
+//      camera-space box against the depth pyramid (any voxel with sdf >= -mu?).  Tiles that pass are refined on their
+//      SUBX x 1 x SUBZ sub-boxes by SUBX * SUBZ threads each (second phase, through shared memory), then appended to the
+//      geometry work list with warp-aggregated atomics.
+//  the other blocks: S1 (c) continued: one group of 4 lanes per queued mark job (grid-stride); the 4 lanes share the
+//      job's cell layers.
 template <int R>
-__global__ void __launch_bounds__(256) k_classify(const __grid_constant__ Params p)
+__global__ void __launch_bounds__(256) k_mark_classify(const __grid_constant__ Params p, int n_geo_blocks)
 {
-    constexpr int WPT = words_per_tile(R);
-    const int tile = blockIdx.x * blockDim.x + threadIdx.x;
+    __shared__ float s_c[256][3];
+    __shared__ uint16_t s_surv[256];
+    __shared__ uint32_t s_nsurv, s_pass[256];
     pdl_launch_dependents();
     pdl_wait();
-    if (tile == 0) p.ctrl[CTRL_NJOBS] = 0u;            // the mark jobs of this frame have been consumed by k_mark
-    bool geo = false;
+    const int t = threadIdx.x;
+    if ((int)blockIdx.x >= n_geo_blocks) {
+        const uint32_t njobs = __ldcg(&p.ctrl[CTRL_NJOBS]);
+        const uint32_t g = ((blockIdx.x - n_geo_blocks) * blockDim.x + t) >> 2, ng = ((gridDim.x - n_geo_blocks) * blockDim.x) >> 2;
+        for (uint32_t j = g; j < njobs; j += ng) {
+            const uint4 job = __ldcg(p.jobs + j);
+            const float xa = (float)(job.x & 0x7fffu), ya = (float)((job.x >> 15) & 0x7fffu), ext = (job.x & 0x80000000u) ? 3.0f : 0.0f;
+            int i0, i1, j0, j1, k0, k1;
+            Piece pc;
+            if (shell_box(p, xa, xa + ext, ya, ya + ext, __uint_as_float(job.y), __uint_as_float(job.z), pc, i0, i1, j0, j1, k0, k1))
+                mark_box<R>(p, pc, i0, i1, j0, j1, k0, k1, t & 3, 4);
+        }
+        return;
+    }
+    const int tile = blockIdx.x * blockDim.x + t;
+    if (t == 0) s_nsurv = 0u;
+    s_pass[t] = 0u;
+    __syncthreads();
     uint32_t near = 0;
     int ttx = 0, tty = 0, ttz = 0;
-    unsigned long long nzb = 0ull;                      // bit 4 w + b set: byte b of mark word w of this tile is non-zero
     if (tile < p.n_tiles) {
         ttx = tile % p.tiles_x; tty = (tile / p.tiles_x) % p.tiles_y; ttz = tile / (p.tiles_x * p.tiles_y);
-        const int gz = local_to_global_tz(p, ttz);
-        const float wx = p.ox + ((float)(ttx * TX) + 0.5f * (float)TX) * p.vs;
-        const float wy = p.oy + ((float)(tty * TY) + 0.5f * (float)TY) * p.vs;
-        const float wz = p.oz + ((float)(gz * TZ) + 0.5f * (float)TZ) * p.vs;
-        const float cX = p.R[0] * wx + p.R[1] * wy + p.R[2] * wz + p.t[0];
-        const float cY = p.R[3] * wx + p.R[4] * wy + p.R[5] * wz + p.t[1];
-        const float cZ = p.R[6] * wx + p.R[7] * wy + p.R[8] * wz + p.t[2];
+        float cX, cY, cZ;
+        tile_centre(p, ttx, tty, ttz, cX, cY, cZ);
         if (!(cZ - p.tile_ez > 2e-3f)) near = ITEM_NEAR;
-        const int coarse = box_may_update(p, cX, cY, cZ, p.tile_ex, p.tile_ey, p.tile_ez);
-        if (coarse != 0) {
-            const float sx = (float)(TX / SUBX) * p.vs, sz = (float)(TZ / SUBZ) * p.vs;
-#pragma unroll
-            for (int bz = 0; bz < SUBZ; ++bz)
-#pragma unroll
-                for (int bx = 0; bx < SUBX; ++bx) {
-                    const float dx = ((float)bx - 0.5f * (float)(SUBX - 1)) * sx, dz = ((float)bz - 0.5f * (float)(SUBZ - 1)) * sz;
-                    if (!geo) geo = box_may_update(p, cX + p.R[0] * dx + p.R[2] * dz, cY + p.R[3] * dx + p.R[5] * dz,
-                                                   cZ + p.R[6] * dx + p.R[8] * dz, p.sub_ex, p.sub_ey, p.sub_ez) != 0;
-                }
+        if (box_may_update(p, cX, cY, cZ, p.tile_ex, p.tile_ey, p.tile_ez) != 0) {
+            const uint32_t k = atomicAdd(&s_nsurv, 1u);
+            s_surv[k] = (uint16_t)t;
+            s_c[t][0] = cX; s_c[t][1] = cY; s_c[t][2] = cZ;
         }
+    }
+    __syncthreads();
+    {   // phase 2: thread k tests sub-box (k % 8) of survivor (k / 8)
+        const uint32_t n = s_nsurv * (uint32_t)(SUBX * SUBZ);
+        const float sx = (float)(TX / SUBX) * p.vs, sz = (float)(TZ / SUBZ) * p.vs;
+        for (uint32_t k = (uint32_t)t; k < n; k += 256u) {
+            const int sv = s_surv[k / (SUBX * SUBZ)], sb = (int)(k % (SUBX * SUBZ)), bx = sb % SUBX, bz = sb / SUBX;
+            const float dx = ((float)bx - 0.5f * (float)(SUBX - 1)) * sx, dz = ((float)bz - 0.5f * (float)(SUBZ - 1)) * sz;
+            if (box_may_update(p, s_c[sv][0] + p.R[0] * dx + p.R[2] * dz, s_c[sv][1] + p.R[3] * dx + p.R[5] * dz,
+                               s_c[sv][2] + p.R[6] * dx + p.R[8] * dz, p.sub_ex, p.sub_ey, p.sub_ez) != 0)
+                s_pass[sv] = 1u;                          // benign race: every writer stores 1
+        }
+    }
+    __syncthreads();
+    const bool geo = s_pass[t] != 0u;
+    const unsigned lane = t & 31, lt = (1u << lane) - 1u;
+    const unsigned mg = __ballot_sync(0xffffffffu, geo);
+    uint32_t bg = 0;
+    if (lane == 0 && mg) bg = atomicAdd(&p.ctrl[CTRL_NGEO], (uint32_t)__popc(mg));
+    bg = __shfl_sync(0xffffffffu, bg, 0);
+    if (geo) p.work_geo[bg + __popc(mg & lt)] = item_pack(ttx, tty, ttz, 0) | near;
+}
+
+// K1b -- S9 for colour, one thread per tile: one work item per non-zero BYTE of the tile's shell-mark words, i.e. up to 8
+// colour cells (heavier than a geometry tile, listed first in the fused kernel's queue).
+template <int R>
+__global__ void __launch_bounds__(256) k_items_col(const __grid_constant__ Params p)
+{
+    constexpr int WPT = words_per_tile(R);
+    pdl_launch_dependents();
+    pdl_wait();
+    const int tile = blockIdx.x * blockDim.x + threadIdx.x;
+    if (tile == 0) p.ctrl[CTRL_NJOBS] = 0u;            // the mark jobs of this frame have been consumed
+    unsigned long long nzb = 0ull;                      // bit 4 w + b set: byte b of mark word w of this tile is non-zero
+    if (tile < p.n_tiles) {
 #pragma unroll
         for (int w = 0; w < WPT; ++w) {
             const uint32_t m = __ldcg(p.marks + (size_t)tile * WPT + w);
@@ -350,22 +385,23 @@ __global__ void __launch_bounds__(256) k_classify(const __grid_constant__ Params
             nzb |= (unsigned long long)nz << (4 * w);
         }
     }
-    // warp-aggregated appends
-    const unsigned lane = threadIdx.x & 31, lt = (1u << lane) - 1u;
-    const unsigned mg = __ballot_sync(0xffffffffu, geo);
+    const unsigned lane = threadIdx.x & 31;
     int ncol = __popcll(nzb), pre = ncol;
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) { const int v = __shfl_up_sync(0xffffffffu, pre, o); if ((int)lane >= o) pre += v; }
     const int tot = __shfl_sync(0xffffffffu, pre, 31);
-    uint32_t bg = 0, bc = 0;
-    if (lane == 0) {
-        if (mg) bg = atomicAdd(&p.ctrl[CTRL_NGEO], (uint32_t)__popc(mg));
-        if (tot) bc = atomicAdd(&p.ctrl[CTRL_NCOL], (uint32_t)tot);
+    if (tot == 0) return;
+    uint32_t bc = 0;
+    if (lane == 0) bc = atomicAdd(&p.ctrl[CTRL_NCOL], (uint32_t)tot);
+    bc = __shfl_sync(0xffffffffu, bc, 0);
+    if (nzb) {
+        const int ttx = tile % p.tiles_x, tty = (tile / p.tiles_x) % p.tiles_y, ttz = tile / (p.tiles_x * p.tiles_y);
+        float cX, cY, cZ;
+        tile_centre(p, ttx, tty, ttz, cX, cY, cZ);
+        const uint32_t near = !(cZ - p.tile_ez > 2e-3f) ? ITEM_NEAR : 0u;
+        uint32_t pos = bc + (uint32_t)(pre - ncol);
+        while (nzb) { const int b = __ffsll((long long)nzb) - 1; nzb &= nzb - 1ull; p.work_col[pos++] = item_pack(ttx, tty, ttz, b) | near; }
     }
-    bg = __shfl_sync(0xffffffffu, bg, 0); bc = __shfl_sync(0xffffffffu, bc, 0);
-    if (geo) p.work_geo[bg + __popc(mg & lt)] = item_pack(ttx, tty, ttz, 0) | near;
-    uint32_t pos = bc + (uint32_t)(pre - ncol);
-    while (nzb) { const int b = __ffsll((long long)nzb) - 1; nzb &= nzb - 1ull; p.work_col[pos++] = item_pack(ttx, tty, ttz, b) | near; }
 }
 
 }  // namespace vf

@@ -45,7 +45,8 @@ struct vol {
 };
 
 // one kernel launch; `dependent` = programmatic dependent launch on the previous kernel of the stream
-static cudaError_t launch(void (*kernel)(const Params), dim3 grid, int block, cudaStream_t s, bool dependent, const Params &p)
+template <typename... Args>
+static cudaError_t launch(void (*kernel)(const Params, Args...), dim3 grid, int block, cudaStream_t s, bool dependent, const Params &p, Args... args)
 {
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = grid; cfg.blockDim = dim3(block); cfg.dynamicSmemBytes = 0; cfg.stream = s;
@@ -53,7 +54,7 @@ static cudaError_t launch(void (*kernel)(const Params), dim3 grid, int block, cu
     at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     at[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = at; cfg.numAttrs = dependent ? 1 : 0;
-    return cudaLaunchKernelEx(&cfg, kernel, p);
+    return cudaLaunchKernelEx(&cfg, kernel, p, args...);
 }
 
 static int set_device(const vol *v) { CK(cudaSetDevice(v->device)); return VOL_OK; }
@@ -296,15 +297,15 @@ extern "C" int vol_integrate(vol_t *v, const uint16_t *depth_u16_dev, int32_t wd
     const dim3 g0((wd + 31) / 32, (hd + 31) / 32);
     const int g1 = (p.n_tiles + 255) / 256, g2 = v->fused_blocks, gm = v->n_sms * 4;
     const bool cnt = v->counting;
-    // k_mark, k_classify and k_fused are launched with programmatic stream serialization: their CTAs may be scheduled
+    // k_mark_classify, k_items_col and k_fused are launched with programmatic stream serialization: their CTAs may be scheduled
     // while the predecessor drains (it signals griddepcontrol.launch_dependents), and they wait for its completion and
     // memory flush with griddepcontrol.wait before touching anything it wrote.
 #define VF_LAUNCH(RR)                                                                   \
     do {                                                                                \
         CK(launch(vf::k_prepass<RR>, g0, 256, s, false, p));                            \
-        CK(launch(vf::k_mark<RR>, dim3(gm), 256, s, true, p));                          \
+        CK(launch(vf::k_mark_classify<RR>, dim3(g1 + gm), 256, s, true, p, g1));        \
         if (v->profiling) CK(cudaEventRecord(v->ev[1], s));                             \
-        CK(launch(vf::k_classify<RR>, dim3(g1), 256, s, true, p));                      \
+        CK(launch(vf::k_items_col<RR>, dim3(g1), 256, s, true, p));                     \
         if (v->profiling) CK(cudaEventRecord(v->ev[2], s));                             \
         if (cnt) CK(launch(vf::k_fused<RR, true>, dim3(g2), vf::CTA, s, true, p));      \
         else     CK(launch(vf::k_fused<RR, false>, dim3(g2), vf::CTA, s, true, p));     \
