@@ -44,7 +44,7 @@ __device__ __forceinline__ bool cell_meets_piece(const Params &p, const Piece &p
 // costs k_mark more than it saves k_fused: measured, not used.)
 // A box of more than MARK_FINE_MAX cells is marked tile by tile instead (all cells of every tile it meets): bounded work
 // for pathological frames, at the price of looser marks.
-constexpr int MARK_FINE_MAX = 1024;
+constexpr int MARK_FINE_MAX = 8192;
 
 template <int R>
 __device__ __forceinline__ void mark_box(const Params &p, const Piece &pc, int i0, int i1, int j0, int j1, int k0, int k1, int sub, int nsub)
@@ -130,11 +130,11 @@ __device__ __forceinline__ bool shell_box(const Params &p, float xa, float xb, f
 //  (b) min/max valid depth per 8x8, 16x16, 32x32 block (pyramid levels 0-2); the last CTA to finish builds the coarser
 //      levels.  Used to cull geometry tiles.
 //  (c) shell marks: a colour voxel can pass the sigma gate (L108) only inside the frustum piece of shell_box().  Every
-//      4 x 4 pixel patch marks the colour cells that meet the world-space bounding box of its piece if that box has at most
-//      PATCH_CELLS_MAX cells, else (depth edge, grazing surface) the boxes of its pixels' own pieces.  This kernel only
+//      4 x 4 pixel patch marks the colour cells that meet the world-space bounding box of its piece if that box is at most
+//      PATCH_SPREAD_MAX x larger than a compact piece's, else (depth edge, grazing surface) the boxes of its pixels' own pieces.  This kernel only
 //      queues the boxes as jobs; k_mark deals them evenly over the whole GPU (depth edges cluster in a few CTAs here).
 //      Marks are consumed (and cleared) by the fused kernel.
-constexpr int PATCH_CELLS_MAX = 96;
+constexpr float PATCH_SPREAD_MAX = 2.4f;
 
 template <int R>
 __global__ void __launch_bounds__(256) k_prepass(const __grid_constant__ Params p)
@@ -209,7 +209,10 @@ __global__ void __launch_bounds__(256) k_prepass(const __grid_constant__ Params 
             Piece pc;
             if (shell_box(p, (float)xp, (float)(xp + 3), (float)yp, (float)(yp + 3), zlo, zhi, pc, i0, i1, j0, j1, k0, k1)) {
                 const int ncell = (i1 / CLX - i0 / CLX + 1) * (j1 / CLY - j0 / CLY + 1) * (k1 / CLZ - k0 / CLZ + 1);
-                if (ncell <= PATCH_CELLS_MAX) {
+                // a compact piece (smooth surface seen head-on) spans about n0 cells: 2 sigma deep, the patch's footprint wide
+                const float c = (float)CLY * p.vc, wfoot = 4.0f * zhi / p.fx;
+                const float n0 = (2.0f * p.sigma / c + 2.0f) * (wfoot / c + 2.0f) * (0.5f * wfoot / c + 2.0f);
+                if ((float)ncell <= PATCH_SPREAD_MAX * n0) {
                     if ((tx & 3) == 0) {
                         const uint32_t j = atomicAdd(&s_njobs, 1u);
                         s_jobs[j] = make_uint4((uint32_t)xp | ((uint32_t)yp << 15) | 0x80000000u, __float_as_uint(zlo), __float_as_uint(zhi), 0u);
