@@ -46,6 +46,8 @@ def parse():
     ap.add_argument("--no-flush", action="store_true", help="time frames back to back without flushing L2")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--first-frame", type=int, default=0)
+    ap.add_argument("--stress", action="store_true",
+                    help="second workload: the saturating frame of SURVEY 8(d) item 5 (every geometry voxel updated) instead of the scan")
     return ap.parse_args()
 
 
@@ -195,7 +197,7 @@ def run_ours(args, rank, world, local_rank):
     # ---- inputs: generated once, pinned on the host and resident on the device
     frames = []
     for i in range(nfr):
-        depth, rgb, T = synth.frame(c, (first + i) % c.n_frames)
+        depth, rgb, T = synth.stress_frame(c, i) if args.stress else synth.frame(c, (first + i) % c.n_frames)
         hd_, hr_ = torch.from_numpy(depth.view(np.int16)).pin_memory(), torch.from_numpy(rgb).pin_memory()
         frames.append((hd_, hr_, hd_.cuda(), hr_.cuda(), T))
     vol = vf.Volume(c.dims_geo, c.r, c.origin, c.extent, c.mu, c.w_max, sigma=c.sigma, gate=c.gate, device=local_rank)
@@ -286,7 +288,8 @@ def run_ours(args, rank, world, local_rank):
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
         "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f32", "data": "synthetic",
-        "config": {"workload": workload_name(c), "frames": f"{first}..{first + nfr - 1} of the seeded trajectory",
+        "config": {"workload": workload_name(c) + (" -- STRESS: saturating frame, every geometry voxel updated" if args.stress else ""),
+                   "frames": "one saturating pose, repeated" if args.stress else f"{first}..{first + nfr - 1} of the seeded trajectory",
                    "l2": "no flush (frames back to back)" if args.no_flush else "L2 flushed (512 MiB memset) between timed frames",
                    "parallelism": "single GPU" if world == 1 else f"{world} replicas (independent scans), no data-path collective"},
         "frames_per_s": world * K / (total_ms * 1e-3),

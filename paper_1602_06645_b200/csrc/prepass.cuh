@@ -271,19 +271,30 @@ __global__ void __launch_bounds__(256) k_prepass(const __grid_constant__ Params 
     __syncthreads();
     if (!s_last) return;
     __threadfence();
+    // small images: levels 4.. are built from a shared-memory copy of the level below (block barriers only); the job
+    // staging buffer is free by now.  Larger images go level by level through global memory.
+    uint32_t *buf = reinterpret_cast<uint32_t *>(s_jobs);
+    const bool in_smem = p.pyr_w[3] * p.pyr_h[3] <= 1024;
     for (int l = 3; l < p.pyr_levels; ++l) {
         const int w = p.pyr_w[l], h = p.pyr_h[l], pw = p.pyr_w[l - 1], ph = p.pyr_h[l - 1];
         const uint32_t *src = p.pyr + p.pyr_off[l - 1];
+        const uint32_t *ssrc = buf + ((l - 1) & 1) * 1024;
+        uint32_t *sdst = buf + (l & 1) * 1024;
+        const bool from_smem = in_smem && l > 3;
         for (int e = t; e < w * h; e += blockDim.x) {
             const int ex = e % w, ey = e / w;
             uint32_t a_mn = 0xffffu, a_mx = 0u;
             for (int a = 0; a < 2; ++a) for (int b = 0; b < 2; ++b) {
                 const int sx = ex * 2 + b, sy = ey * 2 + a;
-                if (sx < pw && sy < ph) { const uint32_t v = __ldcg(src + sy * pw + sx); a_mn = min(a_mn, v & 0xffffu); a_mx = max(a_mx, v >> 16); }
+                if (sx < pw && sy < ph) {
+                    const uint32_t v = from_smem ? ssrc[sy * pw + sx] : __ldcg(src + sy * pw + sx);
+                    a_mn = min(a_mn, v & 0xffffu); a_mx = max(a_mx, v >> 16);
+                }
             }
             p.pyr[p.pyr_off[l] + e] = a_mn | (a_mx << 16);
+            if (in_smem) sdst[e] = a_mn | (a_mx << 16);
         }
-        __threadfence();
+        if (!in_smem) __threadfence();
         __syncthreads();
     }
     if (t == 0) p.ctrl[CTRL_TICKET] = 0;

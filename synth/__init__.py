@@ -344,5 +344,22 @@ def coord_rgb(wh: int, hh: int) -> np.ndarray:
     return np.stack([x % 256, y % 256, (x // 256) + 16 * (y // 256)], axis=-1).astype(np.uint8)
 
 
+def stress_frame(c: "Config", seed: int = 0):
+    """Saturating geometry frame for config ``c``: the camera is backed off along -x until the whole
+    cube is inside the depth frustum and sees a fronto-parallel wall behind the cube, so EVERY geometry voxel is updated
+    (free space); the wall is further than sigma behind the cube, so no colour voxel is.  Returns (depth, rgb, T_world_depth)."""
+    ext = float(c.extent)
+    centre = np.asarray(c.origin, np.float64) + ext / 2
+    fx, fy = float(c.K_depth[0, 0]), float(c.K_depth[1, 1])
+    half = ext / 2
+    tan_h, tan_v = (c.wd / 2 - 1.0) / fx, (c.hd / 2 - 1.0) / fy
+    d = half + 1.05 * half / min(tan_h, tan_v)                 # distance camera -> cube centre
+    T = look_at(centre + np.array([-d, 0.0, 0.0]), centre)
+    wall_mm = int(np.ceil(1000.0 * (d + half + 0.5)))
+    assert wall_mm < 65535
+    depth = np.full((c.hd, c.wd), wall_mm, dtype=np.uint16)
+    return depth, random_rgb(c.wh, c.hh, 900 + seed), rigid32(T)
+
+
 def random_rgb(wh: int, hh: int, seed: int) -> np.ndarray:
     return np.random.default_rng(SEED0 + seed).integers(0, 256, size=(hh, wh, 3), dtype=np.uint8)
