@@ -154,39 +154,32 @@ __device__ __forceinline__ void geometry_tile(const Params &p, uint32_t item, in
     const int w_max = p.w_max;
     const uint16_t *__restrict__ depth = p.depth;
     // S2 of one layer: eq. 5 z term, projection, and the four depth gathers (offset 0 when outside: a valid address)
-    auto project_layer = [&](int z, float (&Z)[4], uint32_t (&d)[4], unsigned &okm) {
+    // A voxel outside the frustum gets Z = +inf: its sdf is -inf, "behind the band", whatever pixel 0 holds.
+    auto project_layer = [&](int z, float (&Z)[4], uint32_t (&d)[4]) {
         const float pz = __fmaf_rn((float)(gz0 + z) + 0.5f, p.vs, p.oz);
-        okm = 0u;
 #pragma unroll
         for (int e = 0; e < 4; ++e) {
-            const float X = __fmaf_rn(r02, pz, bX[e]), Y = __fmaf_rn(r12, pz, bY[e]);
-            Z[e] = __fmaf_rn(r22, pz, bZ[e]);
+            const float X = __fmaf_rn(r02, pz, bX[e]), Y = __fmaf_rn(r12, pz, bY[e]), Zv = __fmaf_rn(r22, pz, bZ[e]);
             bool ok; uint32_t off;
-            project_fast(fx, fy, cx, cy, wd, wbits, hbits, koff, X, Y, Z[e], ok, off);
-            okm |= (ok ? 1u : 0u) << e;
+            project_fast(fx, fy, cx, cy, wd, wbits, hbits, koff, X, Y, Zv, ok, off);
+            Z[e] = ok ? Zv : __int_as_float(0x7f800000);
             d[e] = __ldg(depth + off);
         }
     };
-    float Zc[4]; uint32_t dc[4]; unsigned okc;
-    uint4 cur = *ptr;
-    project_layer(0, Zc, dc, okc);
-    for (int z = 0; z < nl; ++z) {
-        uint4 nxt = cur;
-        uint4 *pn = reinterpret_cast<uint4 *>(reinterpret_cast<uint32_t *>(ptr) + layer);
-        float Zn[4] = {0.f, 0.f, 0.f, 0.f}; uint32_t dn[4] = {0u, 0u, 0u, 0u}; unsigned okn = 0u;
-        if (z + 1 < nl) { nxt = *pn; project_layer(z + 1, Zn, dn, okn); }    // next layer in flight
+    // S3 of one layer: truncation test, running average, store if a word changed
+    auto update_layer = [&](uint4 *ptr, const uint4 &cur, const float (&Z)[4], const uint32_t (&d)[4]) {
         const uint32_t o4[4] = {cur.x, cur.y, cur.z, cur.w};
         uint32_t w4[4];
         float sdf[4]; bool upd[4];
         bool easy = true;
 #pragma unroll
-        for (int e = 0; e < 4; ++e) {                             // S3: truncation test
-            const float D = __fmul_rn((float)dc[e], 0.001f);
-            sdf[e] = __fsub_rn(D, Zc[e]);
-            upd[e] = ((okc >> e) & 1u) && (dc[e] != 0u) && !(sdf[e] < neg_mu);
+        for (int e = 0; e < 4; ++e) {
+            const float D = __fmul_rn((float)d[e], 0.001f);
+            sdf[e] = __fsub_rn(D, Z[e]);
+            upd[e] = (d[e] != 0u) & !(sdf[e] < neg_mu);
             // saturated free space (tsdf = 1 onto q = 32767) or first touch (w = 0): the running average is 32767 exactly,
-            // fma(32767, w, 32767) / (w + 1) with every intermediate below 2^24
-            easy = easy && (!upd[e] || (__fmul_rn(sdf[e], inv_mu) >= 1.0f && ((o4[e] & 0xffffu) == 0x7fffu || (o4[e] >> 16) == 0u)));
+            // fma(32767, w, 32767) / (w + 1) with every intermediate below 2^24.  (Bitwise on purpose: no branches.)
+            easy = easy & (!upd[e] | ((__fmul_rn(sdf[e], inv_mu) >= 1.0f) & (((o4[e] & 0xffffu) == 0x7fffu) | (o4[e] < 0x10000u))));
             if (COUNT) c.gr += upd[e];
         }
         if (__all_sync(lanes, easy)) {                            // whole warp in free space: no division needed
@@ -197,7 +190,7 @@ __device__ __forceinline__ void geometry_tile(const Params &p, uint32_t item, in
             }
         } else {
 #pragma unroll
-            for (int e = 0; e < 4; ++e) {                         // S3: running average
+            for (int e = 0; e < 4; ++e) {
                 const float tsdf = fminf(1.0f, __fmul_rn(sdf[e], inv_mu));
                 const int q = (int)(short)(o4[e] & 0xffffu);
                 const int wi = (int)(short)(o4[e] >> 16);
@@ -216,10 +209,35 @@ __device__ __forceinline__ void geometry_tile(const Params &p, uint32_t item, in
         const bool any = (w4[0] != o4[0]) | (w4[1] != o4[1]) | (w4[2] != o4[2]) | (w4[3] != o4[3]);
         if (COUNT) c.gc += (w4[0] != o4[0]) + (w4[1] != o4[1]) + (w4[2] != o4[2]) + (w4[3] != o4[3]);
         if (any) *ptr = make_uint4(w4[0], w4[1], w4[2], w4[3]);   // skip the store when nothing changed
-        ptr = pn; cur = nxt; okc = okn;
-#pragma unroll
-        for (int e = 0; e < 4; ++e) { Zc[e] = Zn[e]; dc[e] = dn[e]; }
+    };
+    // Two register sets, A (even layers) and B (odd layers), used alternately: the pipeline needs no register-to-register
+    // rotation, which would make the warp wait for the loads it has just issued.
+    float ZA[4], ZB[4]; uint32_t dA[4], dB[4];
+    uint4 curA = *ptr, curB = curA;
+    project_layer(0, ZA, dA);
+    for (int z = 0; z < nl; z += 2) {
+        uint4 *pB = reinterpret_cast<uint4 *>(reinterpret_cast<uint32_t *>(ptr) + layer);
+        uint4 *pA2 = reinterpret_cast<uint4 *>(reinterpret_cast<uint32_t *>(pB) + layer);
+        const bool hasB = z + 1 < nl, hasA2 = z + 2 < nl;
+        if (hasB) { curB = *pB; project_layer(z + 1, ZB, dB); }               // layer z + 1 in flight
+        update_layer(ptr, curA, ZA, dA);
+        if (hasB) {
+            if (hasA2) { curA = *pA2; project_layer(z + 2, ZA, dA); }         // layer z + 2 in flight
+            update_layer(pB, curB, ZB, dB);
+        }
+        ptr = pA2;
     }
+}
+
+// pull the 32 lines (8 layers x 4 rows x 128 bytes) of a geometry tile into L2: one line per lane, no register is tied up.
+// Issued when the tile is started: its later layers are then L2 hits by the time the layer pipeline reaches them.
+__device__ __forceinline__ void geometry_prefetch(const Params &p, uint32_t item, int lane)
+{
+    int ttx, tty, ttz, sub;
+    item_unpack(item, ttx, tty, ttz, sub);
+    const int j = tty * TY + (lane & 3), lz = ttz * TZ + (lane >> 2);
+    if (j < p.ny && lz < p.local_nz)
+        asm volatile("prefetch.global.L2 [%0];" ::"l"(p.geo + ((size_t)lz * p.ny + j) * p.nx + ttx * TX));
 }
 
 // Per-warp staging buffer of colour voxels that passed the sigma gate.  The gate (S4-S5) runs on whole cells, 4 voxels
@@ -389,7 +407,8 @@ __global__ void __launch_bounds__(CTA, 4) k_fused(const __grid_constant__ Params
     const uint32_t n_col = __ldcg(&p.ctrl[CTRL_NCOL]), n_items = n_col + __ldcg(&p.ctrl[CTRL_NGEO]);
     Counts c = {0, 0, 0, 0};
     int n_staged = 0;
-    // the ticket of the next item is requested before the current one is processed (the L2 round trip is hidden)
+    // the ticket of the next item is requested before the current one is processed (the L2 round trip is hidden).
+    // Only one item is reserved ahead: colour items are long, and a deeper reservation unbalances the tail.
     uint32_t ticket = 0;
     next_ticket(&p.ctrl[CTRL_CURSOR], lane, ticket);
     for (;;) {
@@ -398,7 +417,7 @@ __global__ void __launch_bounds__(CTA, 4) k_fused(const __grid_constant__ Params
         const uint32_t item = it < n_col ? __ldcg(p.work_col + it) : __ldcg(p.work_geo + (it - n_col));
         next_ticket(&p.ctrl[CTRL_CURSOR], lane, ticket);
         if (it < n_col) colour_item<R, COUNT>(p, item, st, n_staged, lane, c);
-        else            geometry_tile<COUNT>(p, item, lane, c);
+        else { geometry_prefetch(p, item, lane); geometry_tile<COUNT>(p, item, lane, c); }
     }
     if (n_staged > 0) colour_update_staged<COUNT>(p, st, 0, n_staged, lane, c);
     if (COUNT) {
