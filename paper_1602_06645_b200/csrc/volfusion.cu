@@ -42,6 +42,9 @@ struct vol {
     bool counting, profiling;
     cudaEvent_t ev[4];
     bool ev_valid;
+    // vol_integrate_host: the HD frame is copied on a stream of the library's own while the depth-only kernels run
+    cudaStream_t copy_stream;
+    cudaEvent_t ev_fork, ev_rgb;
 };
 
 // one kernel launch; `dependent` = programmatic dependent launch on the previous kernel of the stream
@@ -208,6 +211,9 @@ extern "C" int vol_create(vol_t **out, const int32_t dims_geo[3], int32_t r, con
     }
     v->fused_blocks = v->n_sms * occ;
     for (int i = 0; i < 4; ++i) if (cudaEventCreate(&v->ev[i]) != cudaSuccess) return fail(VOL_E_CUDA);
+    if (cudaStreamCreateWithFlags(&v->copy_stream, cudaStreamNonBlocking) != cudaSuccess) return fail(VOL_E_CUDA);
+    if (cudaEventCreateWithFlags(&v->ev_fork, cudaEventDisableTiming) != cudaSuccess) return fail(VOL_E_CUDA);
+    if (cudaEventCreateWithFlags(&v->ev_rgb, cudaEventDisableTiming) != cudaSuccess) return fail(VOL_E_CUDA);
     v->ev_valid = false;
     if (cudaDeviceSynchronize() != cudaSuccess) return fail(VOL_E_CUDA);
     *out = v;
@@ -232,6 +238,9 @@ extern "C" void vol_destroy(vol_t *v)
     if (v->stage_depth) cudaFree(v->stage_depth);
     if (v->stage_rgb) cudaFree(v->stage_rgb);
     for (int i = 0; i < 4; ++i) if (v->ev[i]) cudaEventDestroy(v->ev[i]);
+    if (v->ev_fork) cudaEventDestroy(v->ev_fork);
+    if (v->ev_rgb) cudaEventDestroy(v->ev_rgb);
+    if (v->copy_stream) cudaStreamDestroy(v->copy_stream);
     cudaGetLastError();
     delete v;
 }
@@ -261,9 +270,10 @@ static int ensure_scratch(vol *v, int wd, int hd)
     return VOL_OK;
 }
 
-extern "C" int vol_integrate(vol_t *v, const uint16_t *depth_u16_dev, int32_t wd, int32_t hd, const uint8_t *rgb8_dev,
-                             int32_t wh, int32_t hh, const float T_world_depth[16], const float K_depth[9],
-                             const float K_rgb[9], const float T_depth_rgb[16], void *stream)
+// rgb_ready: optional event the fused kernel (the only reader of the HD frame) has to wait for
+static int integrate_impl(vol_t *v, const uint16_t *depth_u16_dev, int32_t wd, int32_t hd, const uint8_t *rgb8_dev,
+                          int32_t wh, int32_t hh, const float T_world_depth[16], const float K_depth[9],
+                          const float K_rgb[9], const float T_depth_rgb[16], void *stream, cudaEvent_t rgb_ready)
 {
     if (!v || !depth_u16_dev || !rgb8_dev || !T_world_depth || !K_depth || !K_rgb || !T_depth_rgb) return VOL_E_ARG;
     if (wd <= 0 || hd <= 0 || wh <= 0 || hh <= 0 || wd > 16384 || hd > 16384 || wh > 16384 || hh > 16384) return VOL_E_ARG;
@@ -307,6 +317,7 @@ extern "C" int vol_integrate(vol_t *v, const uint16_t *depth_u16_dev, int32_t wd
         if (v->profiling) CK(cudaEventRecord(v->ev[1], s));                             \
         CK(launch(vf::k_items_col<RR>, dim3(g1), 256, s, true, p));                     \
         if (v->profiling) CK(cudaEventRecord(v->ev[2], s));                             \
+        if (rgb_ready) CK(cudaStreamWaitEvent(s, rgb_ready, 0));                        \
         if (cnt) CK(launch(vf::k_fused<RR, true>, dim3(g2), vf::CTA, s, true, p));      \
         else     CK(launch(vf::k_fused<RR, false>, dim3(g2), vf::CTA, s, true, p));     \
     } while (0)
@@ -320,6 +331,13 @@ extern "C" int vol_integrate(vol_t *v, const uint16_t *depth_u16_dev, int32_t wd
     if (v->profiling) { CK(cudaEventRecord(v->ev[3], s)); v->ev_valid = true; }
     CK(cudaGetLastError());
     return VOL_OK;
+}
+
+extern "C" int vol_integrate(vol_t *v, const uint16_t *depth_u16_dev, int32_t wd, int32_t hd, const uint8_t *rgb8_dev,
+                             int32_t wh, int32_t hh, const float T_world_depth[16], const float K_depth[9],
+                             const float K_rgb[9], const float T_depth_rgb[16], void *stream)
+{
+    return integrate_impl(v, depth_u16_dev, wd, hd, rgb8_dev, wh, hh, T_world_depth, K_depth, K_rgb, T_depth_rgb, stream, nullptr);
 }
 
 extern "C" int vol_integrate_host(vol_t *v, const uint16_t *depth_u16_host, int32_t wd, int32_t hd, const uint8_t *rgb8_host,
@@ -343,8 +361,13 @@ extern "C" int vol_integrate_host(vol_t *v, const uint16_t *depth_u16_host, int3
     }
     cudaStream_t s = (cudaStream_t)stream;
     CK(cudaMemcpyAsync(v->stage_depth, depth_u16_host, db, cudaMemcpyHostToDevice, s));
-    CK(cudaMemcpyAsync(v->stage_rgb, rgb8_host, cb, cudaMemcpyHostToDevice, s));
-    return vol_integrate(v, v->stage_depth, wd, hd, v->stage_rgb, wh, hh, T_world_depth, K_depth, K_rgb, T_depth_rgb, stream);
+    // fork: the HD frame (91 % of the bytes) goes over the library's copy stream, ordered after everything already queued
+    // on `stream` (the previous frame's fused kernel still reads the staging buffer); only the fused kernel waits for it
+    CK(cudaEventRecord(v->ev_fork, s));
+    CK(cudaStreamWaitEvent(v->copy_stream, v->ev_fork, 0));
+    CK(cudaMemcpyAsync(v->stage_rgb, rgb8_host, cb, cudaMemcpyHostToDevice, v->copy_stream));
+    CK(cudaEventRecord(v->ev_rgb, v->copy_stream));
+    return integrate_impl(v, v->stage_depth, wd, hd, v->stage_rgb, wh, hh, T_world_depth, K_depth, K_rgb, T_depth_rgb, stream, v->ev_rgb);
 }
 
 extern "C" int vol_download(const vol_t *v, void *geo_host, size_t geo_bytes, void *col_host, size_t col_bytes, void *stream)
