@@ -300,7 +300,7 @@ def run_ours(args, rank, world, local_rank):
                            "col_changed": float(cnt[:, 3].mean()), "tiles_geo": float(cnt[:, 4].mean()), "items_col": float(cnt[:, 5].mean()),
                            "cells_col": float(cnt[:, 6].mean()), "algorithmic_bytes": float(alg_bytes.mean())},
         "roofline": {"bound": "hbm", "kernel": "k_fused", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                     "traffic": ncu_traffic(c.name), "peak_source": peak_src,
+                     "traffic": ncu_traffic(c.name + ("-stress" if args.stress else "")), "peak_source": peak_src,
                      "dense_sweep_frac": float(8.0 * nvox / (fused_ms.mean() * 1e-3) / 1e9 / peak)},
         "e2e": {"value": e2e_value, "unit": UNIT, "ms_per_step": e2e_ms / K, "h2d_bytes_per_step": frame_bytes,
                 "d2h_bytes_per_step": 64},

@@ -100,6 +100,19 @@ __device__ __forceinline__ void project_fast(float fx, float fy, float cx, float
     off = ok ? bv * w + bu - koff : 0u;
 }
 
+// the same without the final select: off is only meaningful when ok
+__device__ __forceinline__ void project_fast_raw(float fx, float fy, float cx, float cy, uint32_t w, uint32_t wbits, uint32_t hbits, uint32_t koff,
+                                                 float X, float Y, float Z, bool &ok, uint32_t &off)
+{
+    const float iz = rcp_exact(Z);
+    const float u = __fmaf_rn(fx, __fmul_rn(X, iz), cx);
+    const float v = __fmaf_rn(fy, __fmul_rn(Y, iz), cy);
+    const float tu = __fadd_rn(u, 0.5f), tv = __fadd_rn(v, 0.5f);
+    ok = (__float_as_uint(tu) < wbits) && (__float_as_uint(tv) < hbits);
+    const uint32_t bu = __float_as_uint(__fadd_rd(tu, 12582912.0f)), bv = __float_as_uint(__fadd_rd(tv, 12582912.0f));
+    off = bv * w + bu - koff;
+}
+
 struct Counts { unsigned long long gr, gc, cr, cc; };
 
 // one geometry tile, one warp: lane = (vx = lane & 7, y = lane >> 3) owns voxels (gx0 + 4 vx .. + 3, gy0 + y) of every layer.
@@ -154,16 +167,22 @@ __device__ __forceinline__ void geometry_tile(const Params &p, uint32_t item, in
     const int w_max = p.w_max;
     const uint16_t *__restrict__ depth = p.depth;
     // S2 of one layer: eq. 5 z term, projection, and the four depth gathers (offset 0 when outside: a valid address)
-    // A voxel outside the frustum gets Z = +inf: its sdf is -inf, "behind the band", whatever pixel 0 holds.
+    // A voxel outside the frustum keeps d = 0 ("invalid depth": not updated); its gather is predicated off.  The address is
+    // one mad.wide (FMA pipe) instead of a 64-bit add pair: the ALU pipe is the busiest one in this loop.
     auto project_layer = [&](int z, float (&Z)[4], uint32_t (&d)[4]) {
         const float pz = __fmaf_rn((float)(gz0 + z) + 0.5f, p.vs, p.oz);
 #pragma unroll
         for (int e = 0; e < 4; ++e) {
-            const float X = __fmaf_rn(r02, pz, bX[e]), Y = __fmaf_rn(r12, pz, bY[e]), Zv = __fmaf_rn(r22, pz, bZ[e]);
+            const float X = __fmaf_rn(r02, pz, bX[e]), Y = __fmaf_rn(r12, pz, bY[e]);
+            Z[e] = __fmaf_rn(r22, pz, bZ[e]);
             bool ok; uint32_t off;
-            project_fast(fx, fy, cx, cy, wd, wbits, hbits, koff, X, Y, Zv, ok, off);
-            Z[e] = ok ? Zv : __int_as_float(0x7f800000);
-            d[e] = __ldg(depth + off);
+            project_fast_raw(fx, fy, cx, cy, wd, wbits, hbits, koff, X, Y, Z[e], ok, off);
+            d[e] = 0u;
+            if (ok) {
+                unsigned long long addr;
+                asm("mad.wide.u32 %0, %1, 2, %2;" : "=l"(addr) : "r"(off), "l"(depth));
+                d[e] = __ldg(reinterpret_cast<const uint16_t *>(addr));
+            }
         }
     };
     // S3 of one layer: truncation test, running average, store if a word changed
