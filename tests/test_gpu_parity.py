@@ -202,3 +202,38 @@ def test_cfg4_r4_full_size_sampled():
     """The largest configuration: 384^3 geometry, 1536^3 colour (14.5 GB, word offsets beyond 2^32 bytes), 2 frames."""
     ng, nc = _sampled_full_size(synth.config(4, r=4), [0, 100], 32, 41)
     assert ng > 10000 and nc > 1000
+
+
+def test_cfg2_full_size_every_voxel():
+    """BASELINE config 2 at full size (256^3 / 512^3): the oracle runs over both whole volumes; every word and the four
+    per-frame counters are compared after each of 3 frames spread over the orbit."""
+    run_sequence(synth.config(2), [0, 33, 66])
+
+
+def test_cfg5_full_size_sampled():
+    """Config 5 at full size (512^3 / 1024^3 over 0.5 m: 0.49 mm colour voxels, sigma = 41 voxels): thick colour shell."""
+    ng, nc = _sampled_full_size(synth.config(5), [0, 200], 48, 51)
+    assert ng > 10000 and nc > 10000
+
+
+def test_run_to_run_determinism_and_noop_repeat():
+    """T4 invariants on the GPU alone: two independent runs of the same sequence give identical bytes (no dependence on
+    the work-queue order), and a frame that changes nothing (zero depth) leaves every byte and the counters at zero."""
+    import paper_1602_06645_b200 as vf
+    c = synth.config(3).scaled(128, 2)
+    states = []
+    for _ in range(2):
+        g = vf.Volume(c.dims_geo, c.r, c.origin, c.extent, c.mu, c.w_max)
+        for fi in (0, 7, 150):
+            depth, rgb, T = synth.frame(c, fi)
+            g.integrate(to_dev(depth), c.wd, c.hd, to_dev(rgb), c.wh, c.hh, T, c.K_depth, c.K_rgb, c.T_depth_rgb)
+        states.append(g.download())
+        if len(states) == 2:
+            g.set_counting(True)
+            g.integrate(to_dev(np.zeros_like(depth)), c.wd, c.hd, to_dev(rgb), c.wh, c.hh, T, c.K_depth, c.K_rgb, c.T_depth_rgb)
+            st = g.frame_stats()
+            assert (st.geo_read, st.geo_changed, st.col_read, st.col_changed, st.tiles_geo, st.items_col) == (0, 0, 0, 0, 0, 0)
+            again = g.download()
+            assert np.array_equal(again[0], states[1][0]) and np.array_equal(again[1], states[1][1])
+        g.close()
+    assert np.array_equal(states[0][0], states[1][0]) and np.array_equal(states[0][1], states[1][1])
