@@ -37,7 +37,7 @@ extern "C" {
 #endif
 
 #define VOL_OK       0
-#define VOL_E_ARG   -1   /* null pointer, dims <= 0, dims_geo[0] % 4 != 0, dims_geo > 4096 x 4096 x 2048 (per shard), r not in 1..4, mu <= 0, w_max not in 1..512,
+#define VOL_E_ARG   -1   /* null pointer, dims <= 0, dims_geo[0] % 4 != 0, dims_geo > 4096 x 2048 x 2048 (per shard), r not in 1..4, mu <= 0, w_max not in 1..512,
                             non-zero skew, non-rigid T, image size <= 0, buffer too small, bad shard */
 #define VOL_E_OOM   -2   /* device allocation failed */
 #define VOL_E_CUDA  -3   /* a CUDA call failed (sticky: see vol_strerror) */
@@ -79,7 +79,7 @@ typedef struct {
     uint64_t geo_read, geo_changed, col_read, col_changed;
     uint32_t tiles_total;   /* geometry tiles owned by this shard */
     uint32_t tiles_geo;     /* geometry tiles (32x4x8 voxels) whose TSDF voxels were visited */
-    uint32_t items_col;     /* colour work items (non-zero bytes of the shell-mark words: up to 8 colour cells each) */
+    uint32_t items_col;     /* colour work items (non-zero nibbles of the shell-mark words: up to 4 colour cells each) */
     uint32_t cells_col;     /* colour cells (8x4x4 colour voxels) visited; only when counting is enabled */
 } vol_stats_t;
 

@@ -1,7 +1,7 @@
 // fused.cuh -- K2: the fused integration kernel (S2-S8), warp-centric and persistent.
 //
-// Every warp pops work items from one queue until it is empty -- first the colour items (one non-zero shell-mark byte
-// = up to 8 colour cells of 8x4x4 voxels of one tile), then the geometry items (one tile of 32x4x8 TSDF voxels, marched
+// Every warp pops work items from one queue until it is empty -- first the colour items (one non-zero shell-mark
+// nibble = up to 4 colour cells of 8x4x4 voxels of one tile), then the geometry items (one tile of 32x4x8 TSDF voxels, marched
 // along z with per-column bases hoisted).  A lane always owns one 16-byte vector of 4 x-adjacent voxels, so a warp
 // reads whole 32-byte sectors (colour gate) or 128-byte lines (geometry rows).  Colour voxels that pass the gate are
 // compacted in a per-warp shared-memory stage and updated one per lane.  No block-level barriers.
@@ -111,6 +111,14 @@ __device__ __forceinline__ void project_fast_raw(float fx, float fy, float cx, f
     ok = (__float_as_uint(tu) < wbits) && (__float_as_uint(tv) < hbits);
     const uint32_t bu = __float_as_uint(__fadd_rd(tu, 12582912.0f)), bv = __float_as_uint(__fadd_rd(tv, 12582912.0f));
     off = bv * w + bu - koff;
+}
+
+// lane 0 draws the next queue ticket.  A predicated instruction, not a branch: the warp must not diverge here, or the
+// compiler may run the whole item once for lane 0 and once for the other lanes.
+__device__ __forceinline__ void next_ticket(uint32_t *cursor, int lane, uint32_t &ticket)
+{
+    asm volatile("{\n\t.reg .pred q;\n\tsetp.eq.s32 q, %1, 0;\n\t@q atom.global.add.u32 %0, [%2], 1;\n\t}"
+                 : "+r"(ticket) : "r"(lane), "l"(cursor) : "memory");
 }
 
 struct Counts { unsigned long long gr, gc, cr, cc; };
@@ -380,40 +388,36 @@ __device__ __forceinline__ void colour_cell(const Params &p, bool near, int ic0,
     __syncwarp();
 }
 
-// one colour work item, one warp: the set bits of one byte of a shell-mark word are up to 8 colour cells of one tile
+// one colour work item, one warp: the set bits of one nibble of a shell-mark word are up to 4 colour cells of one tile.
+// The ticket of the next item is drawn before the LAST cell: its latency is hidden, yet no item waits reserved behind a
+// long one.
 template <int R, bool COUNT>
-__device__ __forceinline__ void colour_item(const Params &p, uint32_t item, Stage &st, int &n, int lane, Counts &c)
+__device__ __forceinline__ void colour_item(const Params &p, uint32_t item, Stage &st, int &n, int lane, Counts &c, uint32_t &ticket)
 {
     const bool near = (item & ITEM_NEAR) != 0u;
     constexpr int CX = cells_x(R), CY = cells_y(R), WPT = words_per_tile(R);
     int ttx, tty, ttz, sub;
     item_unpack(item, ttx, tty, ttz, sub);
-    const int word = sub >> 2;
-    const uint32_t wi = (uint32_t)((ttz * p.tiles_y + tty) * p.tiles_x + ttx) * WPT + (uint32_t)word, sh = 8u * ((uint32_t)sub & 3u);
+    const int word = sub >> 3;
+    const uint32_t wi = (uint32_t)((ttz * p.tiles_y + tty) * p.tiles_x + ttx) * WPT + (uint32_t)word, sh = 4u * ((uint32_t)sub & 7u);
     uint32_t bits = 0;
-    if (lane == 0) {                                                      // consume this item's byte of the marks (self-cleaning)
-        bits = __ldcg(p.marks + wi) & (0xffu << sh);
-        atomicAnd(p.marks + wi, ~(0xffu << sh));
+    if (lane == 0) {                                                      // consume this item's nibble of the marks (self-cleaning)
+        bits = __ldcg(p.marks + wi) & (0xfu << sh);
+        atomicAnd(p.marks + wi, ~(0xfu << sh));
     }
     bits = __shfl_sync(0xffffffffu, bits, 0);
     const int cgx0 = ttx * TX * R, cgy0 = tty * TY * R;
     const int cgz0 = local_to_global_tz(p, ttz) * TZ * R, clz0 = ttz * TZ * R;
     if (COUNT && lane == 0) atomicAdd(&p.ctrl[CTRL_CELLS], (uint32_t)__popc(bits));
+    if (bits == 0u) next_ticket(&p.ctrl[CTRL_CURSOR], lane, ticket);
     while (bits) {
         const int b = word * 32 + (__ffs(bits) - 1);
         bits &= bits - 1;
+        if (bits == 0u) next_ticket(&p.ctrl[CTRL_CURSOR], lane, ticket);
         const int cx = b % CX, cy = (b / CX) % CY, cz = b / (CX * CY);
         const int kz = cz * CLZ + (lane >> 3);
         colour_cell<COUNT>(p, near, cgx0 + cx * CLX + 4 * (lane & 1), cgy0 + cy * CLY + ((lane >> 1) & 3), cgz0 + kz, clz0 + kz, st, n, lane, c);
     }
-}
-
-// lane 0 draws the next queue ticket.  A predicated instruction, not a branch: the warp must not diverge here, or the
-// compiler may run the whole item once for lane 0 and once for the other lanes.
-__device__ __forceinline__ void next_ticket(uint32_t *cursor, int lane, uint32_t &ticket)
-{
-    asm volatile("{\n\t.reg .pred q;\n\tsetp.eq.s32 q, %1, 0;\n\t@q atom.global.add.u32 %0, [%2], 1;\n\t}"
-                 : "+r"(ticket) : "r"(lane), "l"(cursor) : "memory");
 }
 
 template <int R, bool COUNT>
@@ -423,7 +427,8 @@ __global__ void __launch_bounds__(CTA, 4) k_fused(const __grid_constant__ Params
     const int lane = threadIdx.x & 31;
     Stage &st = s_stage[threadIdx.x >> 5];
     pdl_wait();
-    const uint32_t n_col = __ldcg(&p.ctrl[CTRL_NCOL]), n_items = n_col + __ldcg(&p.ctrl[CTRL_NGEO]);
+    // queue order: NEAR geometry tiles (the longest items), colour items, ordinary geometry tiles (the shortest: the tail)
+    const uint32_t n_near = __ldcg(&p.ctrl[CTRL_NNEAR]), n_col = n_near + __ldcg(&p.ctrl[CTRL_NCOL]), n_items = n_col + __ldcg(&p.ctrl[CTRL_NGEO]);
     Counts c = {0, 0, 0, 0};
     int n_staged = 0;
     // the ticket of the next item is requested before the current one is processed (the L2 round trip is hidden).
@@ -433,10 +438,11 @@ __global__ void __launch_bounds__(CTA, 4) k_fused(const __grid_constant__ Params
     for (;;) {
         const uint32_t it = __shfl_sync(0xffffffffu, ticket, 0);
         if (it >= n_items) break;
-        const uint32_t item = it < n_col ? __ldcg(p.work_col + it) : __ldcg(p.work_geo + (it - n_col));
-        next_ticket(&p.ctrl[CTRL_CURSOR], lane, ticket);
-        if (it < n_col) colour_item<R, COUNT>(p, item, st, n_staged, lane, c);
-        else { geometry_prefetch(p, item, lane); geometry_tile<COUNT>(p, item, lane, c); }
+        const uint32_t item = it < n_near ? __ldcg(p.work_geo + ((uint32_t)p.n_tiles - 1u - it))
+                                          : (it < n_col ? __ldcg(p.work_col + (it - n_near)) : __ldcg(p.work_geo + (it - n_col)));
+        if (it >= n_near && it < n_col) colour_item<R, COUNT>(p, item, st, n_staged, lane, c, ticket);
+        else {
+            next_ticket(&p.ctrl[CTRL_CURSOR], lane, ticket); geometry_prefetch(p, item, lane); geometry_tile<COUNT>(p, item, lane, c); }
     }
     if (n_staged > 0) colour_update_staged<COUNT>(p, st, 0, n_staged, lane, c);
     if (COUNT) {

@@ -62,31 +62,31 @@ struct Params {
     uint32_t *pyr;               // min/max valid-depth pyramid: entry = min_mm | max_mm << 16 (0xffff / 0 = empty)
     int       pyr_off[12], pyr_w[12], pyr_h[12], pyr_levels;
     uint4    *jobs;              // shell-mark jobs of the frame (one per 4 x 4 pixel patch or per pixel), wd x hd (rounded up to 4) entries
-    uint32_t *work_geo;          // geometry work list: local tile ids
+    uint32_t *work_geo;          // geometry work list (n_tiles entries): ordinary tiles from the front, ITEM_NEAR tiles from the back
     uint32_t *marks;             // shell marks: words_per_tile(r) words per tile, bit = colour cell that may hold sigma-shell voxels
-    uint32_t *work_col;          // colour work list: indices of non-zero mark BYTES (4 x word index + byte)
+    uint32_t *work_col;          // colour work list: one item per non-zero mark NIBBLE (up to 4 colour cells)
     uint32_t *ctrl;              // control words, see CTRL_* below
     unsigned long long *counters;// 4 voxel counters (counting variant only)
 };
 
-// work items (32 bits): [6:0] ttx | [16:7] tty | [24:17] ttz (local slab) = tile coordinates, [30:25] sub = index of the
-// mark byte within the tile (colour items only), [31] ITEM_NEAR = the tile's box comes within 2 mm of the camera plane
+// work items (32 bits): [6:0] ttx | [15:7] tty | [23:16] ttz (local slab) = tile coordinates, [30:24] sub = index of the
+// mark NIBBLE within the tile (colour items only), [31] ITEM_NEAR = the tile's box comes within 2 mm of the camera plane
 // (or behind it), so its voxels may have Z <= 0 or Z outside the range of the branch-free reciprocal.
-// vol_create rejects volumes with more than 128 x 1024 x 256 tiles per shard.
+// vol_create rejects volumes with more than 128 x 512 x 256 tiles per shard.
 constexpr uint32_t ITEM_NEAR = 1u << 31;
-constexpr int ITEM_Y_SHIFT = 7, ITEM_Z_SHIFT = 17, ITEM_SUB_SHIFT = 25;
-constexpr int ITEM_MAX_TX = 128, ITEM_MAX_TY = 1024, ITEM_MAX_TZ = 256;
+constexpr int ITEM_Y_SHIFT = 7, ITEM_Z_SHIFT = 16, ITEM_SUB_SHIFT = 24;
+constexpr int ITEM_MAX_TX = 128, ITEM_MAX_TY = 512, ITEM_MAX_TZ = 256;
 __device__ __forceinline__ uint32_t item_pack(int ttx, int tty, int ttz, int sub)
 {
     return (uint32_t)ttx | ((uint32_t)tty << ITEM_Y_SHIFT) | ((uint32_t)ttz << ITEM_Z_SHIFT) | ((uint32_t)sub << ITEM_SUB_SHIFT);
 }
 __device__ __forceinline__ void item_unpack(uint32_t item, int &ttx, int &tty, int &ttz, int &sub)
 {
-    ttx = (int)(item & 127u); tty = (int)((item >> ITEM_Y_SHIFT) & 1023u); ttz = (int)((item >> ITEM_Z_SHIFT) & 255u);
-    sub = (int)((item >> ITEM_SUB_SHIFT) & 63u);
+    ttx = (int)(item & 127u); tty = (int)((item >> ITEM_Y_SHIFT) & 511u); ttz = (int)((item >> ITEM_Z_SHIFT) & 255u);
+    sub = (int)((item >> ITEM_SUB_SHIFT) & 127u);
 }
 
-enum { CTRL_NGEO = 0, CTRL_NCOL = 1, CTRL_CURSOR = 2, CTRL_TICKET = 3, CTRL_CELLS = 4, CTRL_NJOBS = 5, CTRL_N = 8 };
+enum { CTRL_NGEO = 0, CTRL_NCOL = 1, CTRL_CURSOR = 2, CTRL_TICKET = 3, CTRL_CELLS = 4, CTRL_NJOBS = 5, CTRL_NNEAR = 6, CTRL_N = 8 };
 
 // programmatic dependent launch: wait for the previous kernel of the stream (completion + memory flush) / allow the next
 // kernel's CTAs to be scheduled as this one drains

@@ -148,7 +148,7 @@ __global__ void __launch_bounds__(256) k_prepass(const __grid_constant__ Params 
     if (t < 16) { s_mn[t] = 0xffffu; s_mx[t] = 0u; }
     if (t == 0) s_njobs = 0u;
     if (blockIdx.x == 0 && blockIdx.y == 0 && t == 0) {
-        p.ctrl[CTRL_NGEO] = 0; p.ctrl[CTRL_NCOL] = 0; p.ctrl[CTRL_CURSOR] = 0; p.ctrl[CTRL_CELLS] = 0;
+        p.ctrl[CTRL_NGEO] = 0; p.ctrl[CTRL_NCOL] = 0; p.ctrl[CTRL_CURSOR] = 0; p.ctrl[CTRL_CELLS] = 0; p.ctrl[CTRL_NNEAR] = 0;
     }
     __syncthreads();
     const int x = blockIdx.x * 32 + tx;
@@ -371,17 +371,22 @@ __global__ void __launch_bounds__(256) k_mark_classify(const __grid_constant__ P
         }
     }
     __syncthreads();
-    const bool geo = s_pass[t] != 0u;
+    // NEAR tiles take the slow per-voxel routines (several times longer than an ordinary tile): they are listed from the
+    // back of the work list and the fused kernel starts with them, so that none is left for the tail
+    const bool pass = s_pass[t] != 0u, geo = pass && near == 0u, geo_near = pass && near != 0u;
     const unsigned lane = t & 31, lt = (1u << lane) - 1u;
-    const unsigned mg = __ballot_sync(0xffffffffu, geo);
-    uint32_t bg = 0;
+    const unsigned mg = __ballot_sync(0xffffffffu, geo), mn = __ballot_sync(0xffffffffu, geo_near);
+    uint32_t bg = 0, bn = 0;
     if (lane == 0 && mg) bg = atomicAdd(&p.ctrl[CTRL_NGEO], (uint32_t)__popc(mg));
-    bg = __shfl_sync(0xffffffffu, bg, 0);
-    if (geo) p.work_geo[bg + __popc(mg & lt)] = item_pack(ttx, tty, ttz, 0) | near;
+    if (lane == 0 && mn) bn = atomicAdd(&p.ctrl[CTRL_NNEAR], (uint32_t)__popc(mn));
+    bg = __shfl_sync(0xffffffffu, bg, 0); bn = __shfl_sync(0xffffffffu, bn, 0);
+    if (geo) p.work_geo[bg + __popc(mg & lt)] = item_pack(ttx, tty, ttz, 0);
+    if (geo_near) p.work_geo[(uint32_t)p.n_tiles - 1u - (bn + __popc(mn & lt))] = item_pack(ttx, tty, ttz, 0) | ITEM_NEAR;
 }
 
-// K1b -- S9 for colour, one thread per tile: one work item per non-zero BYTE of the tile's shell-mark words, i.e. up to 8
-// colour cells (heavier than a geometry tile, listed first in the fused kernel's queue).
+// K1b -- S9 for colour, one thread per tile: one work item per non-zero NIBBLE of the tile's shell-mark words, i.e. up to
+// 4 colour cells.  (A colour item is several times longer than a geometry tile; with 8 cells per item the longest ones
+// took half of the fused kernel's duration and left a tail.)  Colour items come first in the fused kernel's queue.
 template <int R>
 __global__ void __launch_bounds__(256) k_items_col(const __grid_constant__ Params p)
 {
@@ -390,17 +395,20 @@ __global__ void __launch_bounds__(256) k_items_col(const __grid_constant__ Param
     pdl_wait();
     const int tile = blockIdx.x * blockDim.x + threadIdx.x;
     if (tile == 0) p.ctrl[CTRL_NJOBS] = 0u;            // the mark jobs of this frame have been consumed
-    unsigned long long nzb = 0ull;                      // bit 4 w + b set: byte b of mark word w of this tile is non-zero
-    if (tile < p.n_tiles) {
+    uint32_t nz[WPT];                                   // bit n set: nibble n of the mark word is non-zero
+    int ncol = 0;
 #pragma unroll
-        for (int w = 0; w < WPT; ++w) {
+    for (int w = 0; w < WPT; ++w) {
+        nz[w] = 0u;
+        if (tile < p.n_tiles) {
             const uint32_t m = __ldcg(p.marks + (size_t)tile * WPT + w);
-            const uint32_t nz = ((m & 0xffu) != 0u) | (((m & 0xff00u) != 0u) << 1) | (((m & 0xff0000u) != 0u) << 2) | (((m >> 24) != 0u) << 3);
-            nzb |= (unsigned long long)nz << (4 * w);
+#pragma unroll
+            for (int n = 0; n < 8; ++n) nz[w] |= (((m >> (4 * n)) & 0xfu) != 0u ? 1u : 0u) << n;
         }
+        ncol += __popc(nz[w]);
     }
     const unsigned lane = threadIdx.x & 31;
-    int ncol = __popcll(nzb), pre = ncol;
+    int pre = ncol;
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) { const int v = __shfl_up_sync(0xffffffffu, pre, o); if ((int)lane >= o) pre += v; }
     const int tot = __shfl_sync(0xffffffffu, pre, 31);
@@ -408,13 +416,17 @@ __global__ void __launch_bounds__(256) k_items_col(const __grid_constant__ Param
     uint32_t bc = 0;
     if (lane == 0) bc = atomicAdd(&p.ctrl[CTRL_NCOL], (uint32_t)tot);
     bc = __shfl_sync(0xffffffffu, bc, 0);
-    if (nzb) {
+    if (ncol) {
         const int ttx = tile % p.tiles_x, tty = (tile / p.tiles_x) % p.tiles_y, ttz = tile / (p.tiles_x * p.tiles_y);
         float cX, cY, cZ;
         tile_centre(p, ttx, tty, ttz, cX, cY, cZ);
         const uint32_t near = !(cZ - p.tile_ez > 2e-3f) ? ITEM_NEAR : 0u;
         uint32_t pos = bc + (uint32_t)(pre - ncol);
-        while (nzb) { const int b = __ffsll((long long)nzb) - 1; nzb &= nzb - 1ull; p.work_col[pos++] = item_pack(ttx, tty, ttz, b) | near; }
+#pragma unroll
+        for (int w = 0; w < WPT; ++w) {
+            uint32_t m = nz[w];
+            while (m) { const int n = __ffs(m) - 1; m &= m - 1u; p.work_col[pos++] = item_pack(ttx, tty, ttz, 8 * w + n) | near; }
+        }
     }
 }
 

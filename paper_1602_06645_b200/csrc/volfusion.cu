@@ -164,7 +164,7 @@ extern "C" int vol_create(vol_t **out, const int32_t dims_geo[3], int32_t r, con
     p.local_nz = local_nz;
     p.tiles_x = (p.nx + vf::TX - 1) / vf::TX; p.tiles_y = (p.ny + vf::TY - 1) / vf::TY; p.tiles_z_local = my_slabs;
     const int64_t n_tiles = (int64_t)p.tiles_x * p.tiles_y * my_slabs;
-    if (p.tiles_x > vf::ITEM_MAX_TX || p.tiles_y > vf::ITEM_MAX_TY || my_slabs > vf::ITEM_MAX_TZ || n_tiles > INT32_MAX / 64) { delete v; return VOL_E_ARG; }
+    if (p.tiles_x > vf::ITEM_MAX_TX || p.tiles_y > vf::ITEM_MAX_TY || my_slabs > vf::ITEM_MAX_TZ || n_tiles > INT32_MAX / 128) { delete v; return VOL_E_ARG; }
     p.n_tiles = (int)n_tiles;
     p.ox = origin_m[0]; p.oy = origin_m[1]; p.oz = origin_m[2];
     p.vs = extent_m / (float)p.nx;
@@ -192,7 +192,7 @@ extern "C" int vol_create(vol_t **out, const int32_t dims_geo[3], int32_t r, con
     if (v->col_bytes && cudaMemset(p.col, 0, v->col_bytes) != cudaSuccess) rc = VOL_E_CUDA;
     const size_t nt = (size_t)(p.n_tiles > 0 ? p.n_tiles : 1), nw = nt * (size_t)vf::words_per_tile(r);
     if (cudaMalloc(&p.work_geo, sizeof(uint32_t) * nt) != cudaSuccess) rc = VOL_E_OOM;
-    if (cudaMalloc(&p.work_col, sizeof(uint32_t) * nw * 4) != cudaSuccess) rc = VOL_E_OOM;
+    if (cudaMalloc(&p.work_col, sizeof(uint32_t) * nw * 8) != cudaSuccess) rc = VOL_E_OOM;
     if (cudaMalloc(&p.marks, sizeof(uint32_t) * nw) != cudaSuccess) rc = VOL_E_OOM;
     if (rc == VOL_OK && cudaMemset(p.marks, 0, sizeof(uint32_t) * nw) != cudaSuccess) rc = VOL_E_CUDA;
     if (cudaMalloc(&p.ctrl, sizeof(uint32_t) * vf::CTRL_N) != cudaSuccess) rc = VOL_E_OOM;
@@ -491,7 +491,7 @@ extern "C" int vol_frame_stats(vol_t *v, vol_stats_t *out, void *stream)
     memset(out, 0, sizeof *out);
     if (v->counting) { out->geo_read = cnt[0]; out->geo_changed = cnt[1]; out->col_read = cnt[2]; out->col_changed = cnt[3]; }
     out->tiles_total = (uint32_t)v->p.n_tiles;
-    out->tiles_geo = ctrl[vf::CTRL_NGEO];
+    out->tiles_geo = ctrl[vf::CTRL_NGEO] + ctrl[vf::CTRL_NNEAR];
     out->items_col = ctrl[vf::CTRL_NCOL];
     out->cells_col = v->counting ? ctrl[vf::CTRL_CELLS] : 0u;
     return VOL_OK;
