@@ -154,21 +154,31 @@ __global__ void __launch_bounds__(256) k_prepass(const __grid_constant__ Params 
     const int x = blockIdx.x * 32 + tx;
     uint32_t mn = 0xffffu, mx = 0u;
     float zpx[4];                             // depths of this thread's colour-eligible pixels (0 = not eligible)
+    // all twelve depth loads of the thread are issued first (the frame has just arrived: they come from DRAM); a missing
+    // forward neighbour reads as 0 = invalid, which is what reading A7 makes of it
+    uint32_t dd0[4], dd1[4], dd2[4];
+#pragma unroll
+    for (int m = 0; m < 4; ++m) {
+        const int y = blockIdx.y * 32 + tq * 4 + m;
+        const bool in = x < p.wd && y < p.hd;
+        dd0[m] = in ? __ldg(p.depth + (size_t)y * p.wd + x) : 0u;
+        dd1[m] = in && x + 1 < p.wd && y + 1 < p.hd ? __ldg(p.depth + (size_t)y * p.wd + x + 1) : 0u;
+        dd2[m] = in && x + 1 < p.wd && y + 1 < p.hd ? __ldg(p.depth + (size_t)(y + 1) * p.wd + x) : 0u;
+    }
 #pragma unroll
     for (int m = 0; m < 4; ++m) {
         const int y = blockIdx.y * 32 + tq * 4 + m;
         zpx[m] = 0.0f;
         if (x < p.wd && y < p.hd) {
-            const uint32_t d0 = __ldg(p.depth + (size_t)y * p.wd + x);
+            const uint32_t d0 = dd0[m];
             float4 out = make_float4(0.f, 0.f, 0.f, 0.f);
             if (d0 != 0) {
                 mn = min(mn, d0); mx = max(mx, d0);
                 const float D = __fmul_rn((float)d0, 0.001f);                      // mm -> m (A4)
                 const float3 Pd = backproject(p, x, y, D);
                 out.x = Pd.x; out.y = Pd.y; out.z = Pd.z;
-                if (x + 1 < p.wd && y + 1 < p.hd) {
-                    const uint32_t d1 = __ldg(p.depth + (size_t)y * p.wd + x + 1);
-                    const uint32_t d2 = __ldg(p.depth + (size_t)(y + 1) * p.wd + x);
+                {
+                    const uint32_t d1 = dd1[m], d2 = dd2[m];
                     if (d1 != 0 && d2 != 0) {
                         const float3 P1 = backproject(p, x + 1, y, __fmul_rn((float)d1, 0.001f));
                         const float3 P2 = backproject(p, x, y + 1, __fmul_rn((float)d2, 0.001f));
