@@ -237,3 +237,46 @@ def test_run_to_run_determinism_and_noop_repeat():
             assert np.array_equal(again[0], states[1][0]) and np.array_equal(again[1], states[1][1])
         g.close()
     assert np.array_equal(states[0][0], states[1][0]) and np.array_equal(states[0][1], states[1][1])
+
+
+def test_large_sigma_and_odd_parameters():
+    """sigma = 150 mm on a coarse grid: every mark box exceeds MARK_FINE_MAX or spans many tiles (tile-granular marks), the
+    colour shell is thicker than the objects; plus w_max = 1, a non-default gate, and a truncation band of half a voxel."""
+    c = synth.config(2).scaled(48, 3)
+    c.w_max = 1
+    c.mu = 0.5 * c.extent / 48
+    g, o = make_pair(c, sigma=0.150, gate=0.5)
+    for fi in (0, 40):
+        depth, rgb, T = synth.frame(c, fi)
+        st, cnt = integrate_both(g, o, c, depth, rgb, T)
+        check_counters(st, cnt, f"large sigma frame {fi}")
+    compare_states(g, o, "large sigma")
+
+
+def test_minimal_volume_frame_size_change_and_streams():
+    """A 4 x 1 x 1 volume; the frame size changes between calls (scratch is reallocated); two volumes alive at once; a
+    non-default stream."""
+    import torch
+    import oracle
+    import paper_1602_06645_b200 as vf
+    c1 = synth.config(1).scaled(32, 2)
+    c2 = synth.config(2).scaled(32, 2)
+    tiny = vf.Volume((4, 1, 1), 2, (-0.1, 0.0, 1.4), 0.4, 0.3, 128)
+    otiny = oracle.RefVolume((4, 1, 1), 2, (-0.1, 0.0, 1.4), 0.4, 0.3, 128)
+    g1, o1 = make_pair(c1)
+    s = torch.cuda.Stream()
+    for c, fi in ((c1, 0), (c2, 10), (c1, 3)):                       # 160x120 -> 640x480 -> 160x120 frames into the SAME volumes
+        depth, rgb, T = synth.frame(c, fi)
+        dd, dr = to_dev(depth), to_dev(rgb)
+        torch.cuda.synchronize()
+        with torch.cuda.stream(s):
+            for vol in (g1, tiny):
+                vol.integrate(dd, c.wd, c.hd, dr, c.wh, c.hh, T, c.K_depth, c.K_rgb, c.T_depth_rgb, stream=s)
+        s.synchronize()
+        for ov in (o1, otiny):
+            ov.integrate(depth, rgb, T, c.K_depth, c.K_rgb, c.T_depth_rgb)
+    compare_states(g1, o1, "frame size change")
+    compare_states(tiny, otiny, "4x1x1 volume")
+    assert (oracle.geo_w(o1.geo) > 0).sum() > 1000
+    assert np.all(oracle.geo_w(otiny.geo) == 2) and (otiny.col > 0).sum() >= 1      # the tiny volume is really in view
+    tiny.close()
