@@ -135,6 +135,8 @@ int vol_launches_per_frame(const vol_t *v);
  * exhaustive != 0, every 257th otherwise).  Both must be 0.  Runs on the current device; synchronises. */
 int vol_selftest(uint64_t mismatches[2], int32_t exhaustive);
 void vol_destroy(vol_t *v);
+/* Text for a return code.  For VOL_E_OOM / VOL_E_CUDA it names the failing CUDA call of the most recent failure in this
+ * process (one process-global buffer: not meant to be read while other threads are making calls). */
 const char *vol_strerror(int code);
 
 #ifdef __cplusplus

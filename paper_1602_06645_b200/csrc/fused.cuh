@@ -40,34 +40,6 @@ __device__ __noinline__ uint32_t geo_voxel_ref(const Params &p, float X, float Y
     return ((uint32_t)qn & 0xffffu) | ((uint32_t)wn << 16);
 }
 
-// eq. 9-10 for one colour voxel that passed the sigma gate with view weight W.
-__device__ __forceinline__ uint32_t col_voxel_update(const Params &p, float X, float Y, float Z, float W, uint32_t word)
-{
-    const int wq = (int)(word >> 24);
-    const float W255 = __fmul_rn(W, 255.0f);
-    if (!(W255 > __fmul_rn(p.gate, (float)wq))) return word;              // L115, A9
-    // HD pixel of the voxel's own position (eq. 3-4; A10, A11)
-    const float Xh = __fmaf_rn(p.Rc[2], Z, __fmaf_rn(p.Rc[1], Y, __fmaf_rn(p.Rc[0], X, p.tc[0])));
-    const float Yh = __fmaf_rn(p.Rc[5], Z, __fmaf_rn(p.Rc[4], Y, __fmaf_rn(p.Rc[3], X, p.tc[1])));
-    const float Zh = __fmaf_rn(p.Rc[8], Z, __fmaf_rn(p.Rc[7], Y, __fmaf_rn(p.Rc[6], X, p.tc[2])));
-    int xh, yh;
-    if (!project_px(p.fxh, p.fyh, p.cxh, p.cyh, p.wh_f, p.hh_f, Xh, Yh, Zh, xh, yh)) return word;   // A13
-    const uint8_t *hd = p.rgb + (size_t)(yh * p.wh + xh) * 3;             // A14: nearest pixel
-    const float den = __fadd_rn((float)wq, W255);
-    uint32_t nw = 0;
-#pragma unroll
-    for (int ch = 0; ch < 3; ++ch) {                                      // eq. 9
-        const int C = (int)((word >> (8 * ch)) & 0xffu);
-        const float num = __fmaf_rn(W255, (float)__ldg(hd + ch), (float)(C * wq));
-        const float cn = rintf(__fdiv_rn(num, den));
-        const int ci = cn < 0.0f ? 0 : (cn > 255.0f ? 255 : (int)cn);
-        nw |= (uint32_t)ci << (8 * ch);
-    }
-    int wn = __float2int_rn(__fmaf_rn(W, (float)(255 - wq), (float)wq)); // eq. 10, A12
-    wn = min(wn, 255);
-    return nw | ((uint32_t)wn << 24);
-}
-
 // sigma gate of one colour voxel (eq. 6-8 via the pixel map, L101-110).  Returns the view weight W (> 0) or 0.
 __device__ __noinline__ float col_voxel_gate_ref(const Params &p, float X, float Y, float Z)
 {
@@ -82,7 +54,7 @@ __device__ __noinline__ float col_voxel_gate_ref(const Params &p, float X, float
 
 // ---------------------------------------------------------------------------------------------------------------
 // branch-free projection of one voxel (fast path): pixel offset y * w + x, or ok = false.
-// Precondition (established per tile by k_classify, bit ITEM_NEAR clear): RCP_MIN <= Z <= RCP_MAX.
+// Precondition (established per tile by k_mark_classify / k_items_col, bit ITEM_NEAR clear): RCP_MIN <= Z <= RCP_MAX.
 // ---------------------------------------------------------------------------------------------------------------
 __device__ __forceinline__ void project_fast(float fx, float fy, float cx, float cy, uint32_t w, uint32_t wbits, uint32_t hbits, uint32_t koff,
                                              float X, float Y, float Z, bool &ok, uint32_t &off)
@@ -276,8 +248,8 @@ struct Stage {
     uint2  adr[STAGE_CAP];                // word index of the voxel in this shard's colour volume (lo, hi)
 };
 
-// S6-S8 for up to 32 staged voxels [first, first + n): one voxel per lane.  Same arithmetic as col_voxel_update(), but
-// the HD pixel (eq. 3-4) is computed and its three bytes requested BEFORE the stored word arrives: the two gathers do
+// S6-S8 (weight gate L115, HD pixel eq. 3-4, eq. 9, eq. 10) for up to 32 staged voxels [first, first + n): one voxel per
+// lane.  The HD pixel (eq. 3-4) is computed and its three bytes requested BEFORE the stored word arrives: the two gathers do
 // not depend on each other, so their latencies overlap instead of adding up (the word is a DRAM access, and one warp
 // works through its stage round after round).  A voxel that then fails the weight gate has fetched 3 bytes in vain.
 template <bool COUNT>

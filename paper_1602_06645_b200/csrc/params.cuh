@@ -50,7 +50,6 @@ struct Params {
     float Rw[9], tw[3];          // depth camera -> world (the caller's T_world_depth)
     float tile_ex, tile_ey, tile_ez;   // conservative camera-axis half extents of a geometry tile
     float sub_ex, sub_ey, sub_ez;      // ... of one of its SUBX x 1 x SUBZ sub-boxes
-    float cell_ex, cell_ey, cell_ez;   // ... and of a colour cell
     float sigma_g;                     // sigma grown by the fp32 slack
     float inv_vc, slack;         // 1 / colour voxel size; metres of slack for fp32 evaluation of culling geometry
     // device buffers

@@ -14,40 +14,19 @@ __device__ __forceinline__ float3 backproject(const Params &p, int x, int y, flo
     return P;
 }
 
-// culling only: a frustum piece in the depth camera: X/Z in [a0, a1], Y/Z in [b0, b1], Z in [z0, z1] (see shell_box)
-struct Piece { float a0, a1, b0, b1, z0, z1; };
-
-// culling only: can the colour cell with global cell coordinates (cx, cy, cz) meet the piece?  Conservative: the cell's
-// camera-space bounding box (centre +- cell_e, slack included) against the piece's own six planes.
-__device__ __forceinline__ bool cell_meets_piece(const Params &p, const Piece &pc, int cx, int cy, int cz)
-{
-    const float wx = p.ox + ((float)(cx * CLX) + 0.5f * (float)CLX) * p.vc;
-    const float wy = p.oy + ((float)(cy * CLY) + 0.5f * (float)CLY) * p.vc;
-    const float wz = p.oz + ((float)(cz * CLZ) + 0.5f * (float)CLZ) * p.vc;
-    const float X = p.R[0] * wx + p.R[1] * wy + p.R[2] * wz + p.t[0];
-    const float Y = p.R[3] * wx + p.R[4] * wy + p.R[5] * wz + p.t[1];
-    const float Z = p.R[6] * wx + p.R[7] * wy + p.R[8] * wz + p.t[2];
-    const float ex = p.cell_ex, ey = p.cell_ey, ez = p.cell_ez;
-    if (Z + ez < pc.z0 || Z - ez > pc.z1) return false;
-    // X <= a1 Z somewhere in the box  <=>  min over the box of (X - a1 Z) <= 0, and so on
-    if (X - pc.a1 * Z > ex + fabsf(pc.a1) * ez || X - pc.a0 * Z < -(ex + fabsf(pc.a0) * ez)) return false;
-    if (Y - pc.b1 * Z > ey + fabsf(pc.b1) * ez || Y - pc.b0 * Z < -(ey + fabsf(pc.b0) * ez)) return false;
-    return true;
-}
-
 // culling only: set the mark bits of every colour cell that intersects the colour-voxel index box
 // [i0,i1] x [j0,j1] x [k0,k1] (inclusive, already clamped to the colour grid).  The cell layers (cz) of the box are dealt
 // round-robin to `nsub` cooperating lanes; this lane is number `sub`.  Per (cell layer, tile) the rows of the box form
 // one contiguous run of at most 4 r^2 <= 64 mark bits, which never spans more than two words: one or two
 // fire-and-forget reductions (no return value, so a lane never waits on the L2 round trip).
-// (Testing every cell of the box against the piece itself -- cell_meets_piece -- marks 16 % fewer cells on config 3 but
-// costs k_mark more than it saves k_fused: measured, not used.)
+// (Testing every cell of the box against the piece itself marks 16 % fewer cells on config 3 but costs the marking more
+// than it saves the fused kernel: measured, not used.)
 // A box of more than MARK_FINE_MAX cells is marked tile by tile instead (all cells of every tile it meets): bounded work
 // for pathological frames, at the price of looser marks.
 constexpr int MARK_FINE_MAX = 8192;
 
 template <int R>
-__device__ __forceinline__ void mark_box(const Params &p, const Piece &pc, int i0, int i1, int j0, int j1, int k0, int k1, int sub, int nsub)
+__device__ __forceinline__ void mark_box(const Params &p, int i0, int i1, int j0, int j1, int k0, int k1, int sub, int nsub)
 {
     constexpr int CX = cells_x(R), CY = cells_y(R), CZ = cells_z(R), NC = cells_per_tile(R), WPT = words_per_tile(R);
     const int cx0 = i0 / CLX, cx1 = i1 / CLX, cy0 = j0 / CLY, cy1 = j1 / CLY, cz0 = k0 / CLZ, cz1 = k1 / CLZ;
@@ -102,12 +81,11 @@ __device__ __forceinline__ bool index_box(const Params &p, float lo, float hi, f
 // Z in [zmin - sigma, zmax + sigma].  The piece is convex, so its world-space bounding box is that of its 8 corners.
 // Returns the inclusive colour-voxel index box of the centres inside it (false if empty).
 __device__ __forceinline__ bool shell_box(const Params &p, float xa, float xb, float ya, float yb, float zmin, float zmax,
-                                          Piece &pc, int &i0, int &i1, int &j0, int &j1, int &k0, int &k1)
+                                          int &i0, int &i1, int &j0, int &j1, int &k0, int &k1)
 {
     const float a0 = ((xa - 0.51f) - p.cx) / p.fx, a1 = ((xb + 0.51f) - p.cx) / p.fx;
     const float b0 = ((ya - 0.51f) - p.cy) / p.fy, b1 = ((yb + 0.51f) - p.cy) / p.fy;
     const float z0 = fmaxf(zmin - p.sigma_g, 1e-6f), z1 = zmax + p.sigma_g;
-    pc.a0 = a0; pc.a1 = a1; pc.b0 = b0; pc.b1 = b1; pc.z0 = z0; pc.z1 = z1;
     float lo[3], hi[3];
 #pragma unroll
     for (int ax = 0; ax < 3; ++ax) {
@@ -132,7 +110,7 @@ __device__ __forceinline__ bool shell_box(const Params &p, float xa, float xb, f
 //  (c) shell marks: a colour voxel can pass the sigma gate (L108) only inside the frustum piece of shell_box().  Every
 //      4 x 4 pixel patch marks the colour cells that meet the world-space bounding box of its piece if that box is at most
 //      PATCH_SPREAD_MAX x larger than a compact piece's, else (depth edge, grazing surface) the boxes of its pixels' own pieces.  This kernel only
-//      queues the boxes as jobs; k_mark deals them evenly over the whole GPU (depth edges cluster in a few CTAs here).
+//      queues the boxes as jobs; k_mark_classify deals them evenly over the whole GPU (depth edges cluster in a few CTAs here).
 //      Marks are consumed (and cleared) by the fused kernel.
 constexpr float PATCH_SPREAD_MAX = 2.4f;
 
@@ -216,8 +194,7 @@ __global__ void __launch_bounds__(256) k_prepass(const __grid_constant__ Params 
         if (zlo <= zhi) {
             const int xp = blockIdx.x * 32 + (tx & ~3), yp = blockIdx.y * 32 + tq * 4;
             int i0, i1, j0, j1, k0, k1;
-            Piece pc;
-            if (shell_box(p, (float)xp, (float)(xp + 3), (float)yp, (float)(yp + 3), zlo, zhi, pc, i0, i1, j0, j1, k0, k1)) {
+            if (shell_box(p, (float)xp, (float)(xp + 3), (float)yp, (float)(yp + 3), zlo, zhi, i0, i1, j0, j1, k0, k1)) {
                 const int ncell = (i1 / CLX - i0 / CLX + 1) * (j1 / CLY - j0 / CLY + 1) * (k1 / CLZ - k0 / CLZ + 1);
                 // a compact piece (smooth surface seen head-on) spans about n0 cells: 2 sigma deep, the patch's footprint wide
                 const float c = (float)CLY * p.vc, wfoot = 4.0f * zhi / p.fx;
@@ -345,9 +322,8 @@ __global__ void __launch_bounds__(256) k_mark_classify(const __grid_constant__ P
             const uint4 job = __ldcg(p.jobs + j);
             const float xa = (float)(job.x & 0x7fffu), ya = (float)((job.x >> 15) & 0x7fffu), ext = (job.x & 0x80000000u) ? 3.0f : 0.0f;
             int i0, i1, j0, j1, k0, k1;
-            Piece pc;
-            if (shell_box(p, xa, xa + ext, ya, ya + ext, __uint_as_float(job.y), __uint_as_float(job.z), pc, i0, i1, j0, j1, k0, k1))
-                mark_box<R>(p, pc, i0, i1, j0, j1, k0, k1, t & 3, 4);
+            if (shell_box(p, xa, xa + ext, ya, ya + ext, __uint_as_float(job.y), __uint_as_float(job.z), i0, i1, j0, j1, k0, k1))
+                mark_box<R>(p, i0, i1, j0, j1, k0, k1, t & 3, 4);
         }
         return;
     }

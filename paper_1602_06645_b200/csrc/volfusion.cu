@@ -250,6 +250,7 @@ static int ensure_scratch(vol *v, int wd, int hd)
 {
     if (v->scratch_wd == wd && v->scratch_hd == hd && v->p.pixmap) return VOL_OK;
     Params &p = v->p;
+    v->scratch_wd = v->scratch_hd = 0;                       // nothing is valid until every allocation below has succeeded
     if (p.pixmap) { CK(cudaDeviceSynchronize()); cudaFree(p.pixmap); p.pixmap = nullptr; }
     if (p.pyr) { cudaFree(p.pyr); p.pyr = nullptr; }
     if (p.jobs) { cudaFree(p.jobs); p.jobs = nullptr; }
@@ -296,7 +297,6 @@ static int integrate_impl(vol_t *v, const uint16_t *depth_u16_dev, int32_t wd, i
     p.slack = (float)slack;
     box_extents(p.R, 0.5 * vf::TX * p.vs, 0.5 * vf::TY * p.vs, 0.5 * vf::TZ * p.vs, slack, p.tile_ex, p.tile_ey, p.tile_ez);
     box_extents(p.R, 0.5 * (vf::TX / vf::SUBX) * p.vs, 0.5 * vf::TY * p.vs, 0.5 * (vf::TZ / vf::SUBZ) * p.vs, slack, p.sub_ex, p.sub_ey, p.sub_ez);
-    box_extents(p.R, 0.5 * vf::CLX * p.vc, 0.5 * vf::CLY * p.vc, 0.5 * vf::CLZ * p.vc, slack, p.cell_ex, p.cell_ey, p.cell_ez);
     p.sigma_g = (float)((double)p.sigma * 1.0001 + slack);
     camera_to_world(p.R, p.t, p.Rw, p.tw);
     if (p.n_tiles == 0) return VOL_OK;
