@@ -212,16 +212,17 @@ __device__ __forceinline__ void geometry_tile(const Params &p, uint32_t item, in
     // Two register sets, A (even layers) and B (odd layers), used alternately: the pipeline needs no register-to-register
     // rotation, which would make the warp wait for the loads it has just issued.
     float ZA[4], ZB[4]; uint32_t dA[4], dB[4];
-    uint4 curA = *ptr, curB = curA;
+    // the voxel stream bypasses L1 (__ldcg): every line is used once, and L1 is better spent on the depth image
+    uint4 curA = __ldcg(ptr), curB = curA;
     project_layer(0, ZA, dA);
     for (int z = 0; z < nl; z += 2) {
         uint4 *pB = reinterpret_cast<uint4 *>(reinterpret_cast<uint32_t *>(ptr) + layer);
         uint4 *pA2 = reinterpret_cast<uint4 *>(reinterpret_cast<uint32_t *>(pB) + layer);
         const bool hasB = z + 1 < nl, hasA2 = z + 2 < nl;
-        if (hasB) { curB = *pB; project_layer(z + 1, ZB, dB); }               // layer z + 1 in flight
+        if (hasB) { curB = __ldcg(pB); project_layer(z + 1, ZB, dB); }               // layer z + 1 in flight
         update_layer(ptr, curA, ZA, dA);
         if (hasB) {
-            if (hasA2) { curA = *pA2; project_layer(z + 2, ZA, dA); }         // layer z + 2 in flight
+            if (hasA2) { curA = __ldcg(pA2); project_layer(z + 2, ZA, dA); }         // layer z + 2 in flight
             update_layer(pB, curB, ZB, dB);
         }
         ptr = pA2;
@@ -259,7 +260,7 @@ __device__ __forceinline__ void colour_update_staged(const Params &p, const Stag
         const float4 r = st.rec[first + lane];
         const uint2 a = st.adr[first + lane];
         uint32_t *ptr = p.col + (((size_t)a.y << 32) | (size_t)a.x);
-        const uint32_t old = *ptr;                                // first HBM touch of this colour voxel (S6)
+        const uint32_t old = __ldcg(ptr);                         // first HBM touch of this colour voxel (S6); L2 only
         // HD pixel of the voxel's own position (eq. 3-4; A10, A11)
         const float Xh = __fmaf_rn(p.Rc[2], r.z, __fmaf_rn(p.Rc[1], r.y, __fmaf_rn(p.Rc[0], r.x, p.tc[0])));
         const float Yh = __fmaf_rn(p.Rc[5], r.z, __fmaf_rn(p.Rc[4], r.y, __fmaf_rn(p.Rc[3], r.x, p.tc[1])));
