@@ -56,6 +56,8 @@ def _load():
         lib.ref_integrate_subset.argtypes = [P, P, P, ctypes.c_int64, P, P, ctypes.c_int64, P]
         lib.ref_frame_constants.restype = ctypes.c_int
         lib.ref_frame_constants.argtypes = [P, P, P]
+        lib.ref_raycast.restype = ctypes.c_int
+        lib.ref_raycast.argtypes = [P, P, P, ctypes.c_int32, ctypes.c_int32, P, P, ctypes.c_float, ctypes.c_float, P, P]
         _lib = lib
     return _lib
 
@@ -118,6 +120,17 @@ class RefVolume:
                                           col_idx.ctypes.data, col_idx.size, col_words.ctypes.data)
         if rc != 0:
             raise ValueError("ref_integrate_subset: bad arguments")
+
+    def raycast(self, w, h, T_world_cam, K, t_near, t_far):
+        """ref_raycast: (depth float32 [h, w] metres, 0 = no surface; rgb uint8 [h, w, 3]) seen by a virtual camera."""
+        T, Kc = _f32(T_world_cam, 16), _f32(K, 9)
+        depth = np.zeros((h, w), dtype=np.float32)
+        rgb = np.zeros((h, w, 3), dtype=np.uint8)
+        rc = _load().ref_raycast(ctypes.addressof(self.desc), self.geo.ctypes.data, self.col.ctypes.data, int(w), int(h),
+                                 T.ctypes.data, Kc.ctypes.data, float(t_near), float(t_far), depth.ctypes.data, rgb.ctypes.data)
+        if rc != 0:
+            raise ValueError("ref_raycast: bad arguments")
+        return depth, rgb
 
     def frame_constants(self, T_world_depth, T_depth_rgb):
         dummy_d = np.zeros((1, 1), np.uint16)

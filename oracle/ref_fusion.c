@@ -278,3 +278,75 @@ int ref_frame_constants(const ref_vol_t *v, const ref_frame_t *f, float out[24])
     memcpy(out + 12, c.Rc, 9 * sizeof(float)); memcpy(out + 21, c.tc, 3 * sizeof(float));
     return 0;
 }
+
+/* ------------------------------------------------------------------------------------------ */
+/* ref_raycast -- NEXT row: ray casting of the geometry + colour volumes  */
+/* ------------------------------------------------------------------------------------------ */
+/* The paper names the operation only ("ray casting" of the volumes for the ICP prediction and the
+ * live preview) and gives no equations: ** parity unpinned by the paper **.  The
+ * definition below is this build's reading R1-R6, written out step by step:
+ *   R1  pixel (x, y) of a virtual pinhole camera K, pose T_world_cam: camera-space ray ((x-cx)/fx, (y-cy)/fy, 1),
+ *       so the ray parameter t IS the camera-space depth z (eq. 1, inverted as in eq. 7);
+ *   R2  samples at t_k = t_near + k * vs (one geometry voxel of depth per step), k = 0, 1, ... while t_k <= t_far;
+ *   R3  the TSDF at a sample is the value of the voxel whose cell contains the point (nearest voxel, no
+ *       interpolation); voxels never observed (w = 0) and points outside the volume are "unknown";
+ *   R4  a hit is the first pair of consecutive known samples with F_prev > 0 >= F_cur (front face only);
+ *       its depth is t_prev + vs * F_prev / (F_prev - F_cur) (linear zero crossing);
+ *   R5  the colour of a hit is the colour voxel that contains the hit point (nearest, weight > 0), else black;
+ *   R6  no hit: depth 0, colour black.
+ * Canonical arithmetic as above (binary32, explicit fmaf, correctly rounded division, floorf).
+ * depth_out: w*h float32 metres; rgb_out: w*h*3 bytes (nullable).  T_world_cam: row-major rigid 4x4. */
+int ref_raycast(const ref_vol_t *v, const uint32_t *geo, const uint32_t *col, int32_t w, int32_t h,
+                const float T_world_cam[16], const float K[9], float t_near, float t_far,
+                float *depth_out, uint8_t *rgb_out)
+{
+    if (!v || !geo || !col || !T_world_cam || !K || !depth_out || w <= 0 || h <= 0) return -1;
+    if (!(t_near >= 0.0f) || !(t_far >= t_near)) return -1;
+    const float fx = K[0], fy = K[4], cx = K[2], cy = K[5];
+    const float vs = v->extent / (float)v->nx, vc = vs / (float)v->r;
+    const float inv_vs = 1.0f / vs, inv_vc = 1.0f / vc;
+    const int cnx = v->nx * v->r, cny = v->ny * v->r, cnz = v->nz * v->r;
+#pragma omp parallel for schedule(dynamic, 4)
+    for (int y = 0; y < h; ++y)
+        for (int x = 0; x < w; ++x) {
+            const float dx = ((float)x - cx) / fx, dy = ((float)y - cy) / fy;                     /* R1 */
+            float dw[3], ow[3];
+            for (int a = 0; a < 3; ++a) {
+                dw[a] = fmaf(T_world_cam[4 * a + 1], dy, fmaf(T_world_cam[4 * a + 0], dx, T_world_cam[4 * a + 2]));
+                ow[a] = T_world_cam[4 * a + 3];
+            }
+            float depth = 0.0f, t_prev = 0.0f, f_prev = 0.0f;
+            int known_prev = 0;
+            uint8_t rgb[3] = {0, 0, 0};
+            for (int k = 0;; ++k) {
+                const float t = fmaf((float)k, vs, t_near);                                       /* R2 */
+                if (t > t_far) break;
+                const float gx = (fmaf(t, dw[0], ow[0]) - v->origin[0]) * inv_vs;
+                const float gy = (fmaf(t, dw[1], ow[1]) - v->origin[1]) * inv_vs;
+                const float gz = (fmaf(t, dw[2], ow[2]) - v->origin[2]) * inv_vs;
+                const float fi = floorf(gx), fj = floorf(gy), fk = floorf(gz);
+                int known = 0; float f = 0.0f;
+                if (fi >= 0.0f && fi < (float)v->nx && fj >= 0.0f && fj < (float)v->ny && fk >= 0.0f && fk < (float)v->nz) {
+                    const uint32_t word = geo[((size_t)(int)fk * (size_t)v->ny + (size_t)(int)fj) * (size_t)v->nx + (size_t)(int)fi];
+                    if ((int16_t)(word >> 16) != 0) { known = 1; f = (float)(int16_t)(word & 0xffffu); }   /* R3 */
+                }
+                if (known && known_prev && f_prev > 0.0f && !(f > 0.0f)) {                        /* R4 */
+                    depth = fmaf(vs, f_prev / (f_prev - f), t_prev);
+                    break;
+                }
+                known_prev = known; t_prev = t; f_prev = f;
+            }
+            if (depth > 0.0f) {                                                                   /* R5 */
+                const float hx = floorf((fmaf(depth, dw[0], ow[0]) - v->origin[0]) * inv_vc);
+                const float hy = floorf((fmaf(depth, dw[1], ow[1]) - v->origin[1]) * inv_vc);
+                const float hz = floorf((fmaf(depth, dw[2], ow[2]) - v->origin[2]) * inv_vc);
+                if (hx >= 0.0f && hx < (float)cnx && hy >= 0.0f && hy < (float)cny && hz >= 0.0f && hz < (float)cnz) {
+                    const uint32_t cw = col[((size_t)(int)hz * (size_t)cny + (size_t)(int)hy) * (size_t)cnx + (size_t)(int)hx];
+                    if ((cw >> 24) != 0) { rgb[0] = (uint8_t)cw; rgb[1] = (uint8_t)(cw >> 8); rgb[2] = (uint8_t)(cw >> 16); }
+                }
+            }
+            depth_out[(size_t)y * (size_t)w + (size_t)x] = depth;
+            if (rgb_out) { uint8_t *o = rgb_out + ((size_t)y * (size_t)w + (size_t)x) * 3; o[0] = rgb[0]; o[1] = rgb[1]; o[2] = rgb[2]; }
+        }
+    return 0;
+}
