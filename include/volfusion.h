@@ -105,6 +105,17 @@ int vol_integrate_host(vol_t *v, const uint16_t *depth_u16_host, int32_t wd, int
                        const float T_world_depth[16], const float K_depth[9], const float K_rgb[9],
                        const float T_depth_rgb[16], void *stream);
 
+/* Ray-cast both volumes into the image of a virtual pinhole camera (the prediction for tracking and the
+ * live preview; the paper gives no equations, the definition is DESIGN.md "Ray casting", readings R1-R6): per pixel the
+ * ray ((x-cx)/fx, (y-cy)/fy, 1) is sampled every geometry-voxel of camera depth from t_near_m to t_far_m; the first
+ * front-face zero crossing of the TSDF (nearest voxel, observed voxels only) gives the depth by linear interpolation, the
+ * colour voxel containing the hit point gives the colour.
+ * depth_dev: DEVICE, w*h float32, metres along the camera's z axis, 0 = no surface; rgb8_dev: DEVICE, w*h*3 bytes R,G,B
+ * (black where there is no surface or no colour), nullable.  T_world_cam / K: HOST, as for vol_integrate.  Unsharded
+ * volumes only (VOL_E_ARG otherwise).  Asynchronous on `stream`; reads the volumes, writes nothing else. */
+int vol_raycast(const vol_t *v, int32_t w, int32_t h, const float T_world_cam[16], const float K[9], float t_near_m,
+                float t_far_m, float *depth_dev, uint8_t *rgb8_dev, void *stream);
+
 /* Copy this shard's volumes to HOST buffers of at least info.geo_bytes / info.col_bytes (either may be NULL to skip). */
 int vol_download(const vol_t *v, void *geo_host, size_t geo_bytes, void *col_host, size_t col_bytes, void *stream);
 /* Gather single voxels: geo_idx / col_idx are HOST int64 linear indices into the FULL grids (must be owned by this

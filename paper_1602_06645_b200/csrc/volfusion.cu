@@ -12,6 +12,7 @@
 #include "fused.cuh"
 #include "params.cuh"
 #include "prepass.cuh"
+#include "raycast.cuh"
 
 using vf::Params;
 
@@ -368,6 +369,27 @@ extern "C" int vol_integrate_host(vol_t *v, const uint16_t *depth_u16_host, int3
     CK(cudaMemcpyAsync(v->stage_rgb, rgb8_host, cb, cudaMemcpyHostToDevice, v->copy_stream));
     CK(cudaEventRecord(v->ev_rgb, v->copy_stream));
     return integrate_impl(v, v->stage_depth, wd, hd, v->stage_rgb, wh, hh, T_world_depth, K_depth, K_rgb, T_depth_rgb, stream, v->ev_rgb);
+}
+
+extern "C" int vol_raycast(const vol_t *v, int32_t w, int32_t h, const float T_world_cam[16], const float K[9], float t_near_m,
+                           float t_far_m, float *depth_dev, uint8_t *rgb8_dev, void *stream)
+{
+    if (!v || !T_world_cam || !K || !depth_dev) return VOL_E_ARG;
+    if (w <= 0 || h <= 0 || w > 16384 || h > 16384 || !intrinsics_ok(K)) return VOL_E_ARG;
+    if (!(t_near_m >= 0.0f) || !(t_far_m >= t_near_m) || !(t_far_m <= 1e6f)) return VOL_E_ARG;
+    if (v->p.shard_world != 1) return VOL_E_ARG;               // a shard does not hold the whole volume
+    float Rt[9], tt[3];
+    if (!rigid_inverse(T_world_cam, Rt, tt)) return VOL_E_ARG;  // only used as the rigidity check
+    int rc = set_device(v); if (rc) return rc;
+    vf::RayParams q;
+    q.w = w; q.h = h; q.fx = K[0]; q.fy = K[4]; q.cx = K[2]; q.cy = K[5];
+    for (int i = 0; i < 12; ++i) q.T[i] = T_world_cam[i];
+    q.t_near = t_near_m; q.t_far = t_far_m; q.depth = depth_dev; q.rgb = rgb8_dev;
+    if (v->p.n_tiles == 0) return VOL_OK;
+    const dim3 grid((w + 7) / 8, (h + 7) / 8);
+    vf::k_raycast<<<grid, 64, 0, (cudaStream_t)stream>>>(v->p, q);
+    CK(cudaGetLastError());
+    return VOL_OK;
 }
 
 extern "C" int vol_download(const vol_t *v, void *geo_host, size_t geo_bytes, void *col_host, size_t col_bytes, void *stream)

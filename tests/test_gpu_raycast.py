@@ -1,0 +1,79 @@
+"""GPU parity of vol_raycast against the oracle's ref_raycast: depth bit for bit, colours byte for byte."""
+import numpy as np
+import pytest
+
+import synth
+from parity_util import integrate_both, make_pair
+
+pytestmark = pytest.mark.gpu
+
+
+def cast_both(g, o, w, h, T, K, t_near, t_far, with_rgb=True):
+    import torch
+    dd = torch.full((h * w,), -1.0, dtype=torch.float32, device="cuda")
+    dr = torch.full((h * w * 3,), 7, dtype=torch.uint8, device="cuda") if with_rgb else None
+    g.raycast(w, h, T, K, t_near, t_far, dd, dr)
+    torch.cuda.synchronize()
+    od, orgb = o.raycast(w, h, T, K, t_near, t_far)
+    gd = dd.cpu().numpy().reshape(h, w)
+    assert np.array_equal(gd.view(np.uint32), od.view(np.uint32)), f"{int((gd.view(np.uint32) != od.view(np.uint32)).sum())} depths differ"
+    if with_rgb:
+        assert np.array_equal(dr.cpu().numpy().reshape(h, w, 3), orgb)
+    return od, orgb
+
+
+def fused_pair(c, frames):
+    g, o = make_pair(c)
+    for fi in frames:
+        depth, rgb, T = synth.frame(c, fi)
+        integrate_both(g, o, c, depth, rgb, T, counting=False)
+    return g, o
+
+
+def test_raycast_cfg1_views():
+    """Config 1 after its 5 frames: the scan's own camera, an oblique camera, a camera inside the volume, a ragged image
+    size (not a multiple of the 8 x 8 pixel CTA), t_near on and off the voxel grid."""
+    c = synth.config(1)
+    g, o = fused_pair(c, range(5))
+    d, rgb = cast_both(g, o, c.wd, c.hd, synth.frame(c, 2)[2], c.K_depth, 0.4, 3.0)
+    assert (d > 0).sum() > 2000 and (rgb.sum(axis=2) > 0).sum() > 2000
+    T = synth.rigid32(synth.look_at((0.25, -0.15, 0.1), (0.0, 0.0, 1.5), up=(0.0, -1.0, 0.0)))
+    d, _ = cast_both(g, o, 157, 93, T, c.K_depth, 0.3125, 2.75)
+    assert (d > 0).sum() > 2000
+    T = synth.rigid32(synth.look_at((0.1, 0.3, 1.15), (0.0, 0.0, 1.5), up=(0.0, -1.0, 0.0)))     # inside the cube
+    cast_both(g, o, c.wd, c.hd, T, c.K_depth, 0.0, 1.0)
+    cast_both(g, o, c.wd, c.hd, T, c.K_depth, 0.05, 0.05)                                          # a single sample: no pair, no hit
+    cast_both(g, o, 64, 48, T, c.K_rgb, 0.0, 2.0, with_rgb=False)                                  # depth only
+
+
+def test_raycast_cfg2_r3_and_empty_volume():
+    c = synth.config(2).scaled(96, 3)
+    g, o = make_pair(c)
+    T0 = synth.frame(c, 0)[2]
+    d, rgb = cast_both(g, o, 80, 60, T0, c.K_depth / np.array([[8, 1, 8], [1, 8, 8], [1, 1, 1]], np.float32), 0.2, 4.0)
+    assert not d.any() and not rgb.any()                                                           # nothing observed yet
+    for fi in (0, 10, 20, 30):
+        depth, rgb_in, T = synth.frame(c, fi)
+        integrate_both(g, o, c, depth, rgb_in, T, counting=False)
+    d, rgb = cast_both(g, o, c.wd, c.hd, synth.frame(c, 15)[2], c.K_depth, 0.2, 4.0)
+    assert (d > 0).mean() > 0.2
+    want = synth.frame(c, 15)[0].astype(np.float32) * 1e-3
+    both = (d > 0) & (want > 0)
+    assert np.median(np.abs(d[both] - want[both])) < 2.0 * c.extent / 96                          # it is the scene that was fused
+
+
+def test_raycast_rejects_bad_arguments():
+    import torch
+    import paper_1602_06645_b200 as vf
+    c = synth.config(1).scaled(32, 2)
+    g, o = make_pair(c)
+    dd = torch.zeros(c.wd * c.hd, dtype=torch.float32, device="cuda")
+    I4 = np.eye(4, dtype=np.float32)
+    Tbad = I4.copy(); Tbad[0, 0] = 2.0
+    for args in ((Tbad, c.K_depth, 0.1, 2.0), (I4, c.K_depth, 2.0, 1.0), (I4, c.K_depth, -1.0, 1.0)):
+        with pytest.raises(vf.VolError) as e:
+            g.raycast(c.wd, c.hd, args[0], args[1], args[2], args[3], dd)
+        assert e.value.code == vf.VOL_E_ARG
+    shard = vf.Volume(c.dims_geo, c.r, c.origin, c.extent, c.mu, c.w_max, shard_rank=0, shard_world=2)
+    with pytest.raises(vf.VolError):
+        shard.raycast(c.wd, c.hd, I4, c.K_depth, 0.1, 2.0, dd)
