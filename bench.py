@@ -135,6 +135,10 @@ def oracle_sample(c, n_frames, slab_layers=None):
         t0 = time.perf_counter()
         o.integrate(depth, rgb, T, c.K_depth, c.K_rgb, c.T_depth_rgb)
         times.append(time.perf_counter() - t0)
+    # the same oracle volumes ray-cast once from the last pose (reported beside the GPU's vol_raycast time)
+    t0 = time.perf_counter()
+    o.raycast(c.wd, c.hd, T, c.K_depth, 0.3, 8.0)
+    oracle_sample.raycast_ms = 1e3 * (time.perf_counter() - t0)
     return nvox, times, sample
 
 
@@ -267,6 +271,22 @@ def run_ours(args, rank, world, local_rank):
     barrier()
     e2e_ms = float(t0.elapsed_time(t1))
 
+    # ---- NEXT row, outside the timed regions: vol_raycast of the volumes as they stand now, from the
+    #      last frame's pose, one 640 x 480 (depth-camera sized) image per call
+    rc_depth = torch.empty(c.wd * c.hd, dtype=torch.float32, device="cuda")
+    rc_rgb = torch.empty(c.wd * c.hd * 3, dtype=torch.uint8, device="cuda")
+    T_last = frames[nfr - 1][4]
+    for _ in range(3):
+        vol.raycast(c.wd, c.hd, T_last, c.K_depth, 0.3, 8.0, rc_depth, rc_rgb, stream=stream)
+    r0 = torch.cuda.Event(enable_timing=True); r1 = torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    r0.record(stream)
+    for _ in range(10):
+        vol.raycast(c.wd, c.hd, T_last, c.K_depth, 0.3, 8.0, rc_depth, rc_rgb, stream=stream)
+    r1.record(stream)
+    torch.cuda.synchronize()
+    raycast_ms = float(r0.elapsed_time(r1)) / 10.0
+    raycast_hit = float((rc_depth > 0).float().mean())
     total_ms, e2e_ms = max_over_ranks([total_ms, e2e_ms], world, "cuda")
     clocks = sampler.stop() if sampler else None
     if rank != 0:
@@ -304,6 +324,8 @@ def run_ours(args, rank, world, local_rank):
                      "dense_sweep_frac": float(8.0 * nvox / (fused_ms.mean() * 1e-3) / 1e9 / peak)},
         "e2e": {"value": e2e_value, "unit": UNIT, "ms_per_step": e2e_ms / K, "h2d_bytes_per_step": frame_bytes,
                 "d2h_bytes_per_step": 64},
+        "raycast": {"ms": raycast_ms, "rays_per_s": c.wd * c.hd / (raycast_ms * 1e-3), "image": f"{c.wd}x{c.hd}", "hit_fraction": raycast_hit,
+                    "note": "vol_raycast of the fused volumes (SURVEY 8(f) rank 1), not part of the timed step"},
         "gpu_launches": vol.launches_per_frame() * K,
         "clocks": clocks,
     }
@@ -311,7 +333,8 @@ def run_ours(args, rank, world, local_rank):
         n = 2 if nvox > 5e8 else (4 if nvox > 5e7 else 5)
         nv, times, sample = oracle_sample(c, min(n, c.n_frames))
         out["cpu_baseline"] = {"value": nv * len(times) / sum(times), "unit": UNIT, "cores": os.cpu_count() or 1, "kind": "oracle",
-                               "sample": sample, "ms_per_frame": 1e3 * float(np.mean(times))}
+                               "sample": sample, "ms_per_frame": 1e3 * float(np.mean(times)),
+                               "raycast_ms": oracle_sample.raycast_ms}
     print(json.dumps(out), flush=True)
     if world > 1:
         dist.destroy_process_group()

@@ -77,3 +77,16 @@ def test_raycast_rejects_bad_arguments():
     shard = vf.Volume(c.dims_geo, c.r, c.origin, c.extent, c.mu, c.w_max, shard_rank=0, shard_world=2)
     with pytest.raises(vf.VolError):
         shard.raycast(c.wd, c.hd, I4, c.K_depth, 0.1, 2.0, dd)
+
+
+def test_raycast_cfg3_full_size():
+    """BASELINE config 3 at full size (512^3 / 1024^3): two frames fused on both sides (the oracle over the whole volumes),
+    then a 640 x 480 ray cast from a third pose of the trajectory compared bit for bit."""
+    c = synth.config(3)
+    g, o = make_pair(c)
+    for fi in (0, 6):
+        depth, rgb, T = synth.frame(c, fi)
+        integrate_both(g, o, c, depth, rgb, T, counting=False)
+    d, rgb = cast_both(g, o, c.wd, c.hd, synth.frame(c, 3)[2], c.K_depth, 0.3, 5.0)
+    assert (d > 0).mean() > 0.5 and (rgb.sum(axis=2) > 0).mean() > 0.3
+    g.close()
