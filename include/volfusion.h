@@ -138,7 +138,8 @@ int vol_frame_stats(vol_t *v, vol_stats_t *out, void *stream);
  * milliseconds: ms[0] pre-pass, shell marks and geometry tile classification (S1, S9), ms[1] colour work items (S9), ms[2] fused integrate (S2-S8).  Synchronises. */
 int vol_set_profiling(vol_t *v, int32_t on);
 int vol_last_kernel_ms(vol_t *v, float ms[3]);
-/* Number of kernels one vol_integrate call launches. */
+/* Number of kernels one vol_integrate call launches (vol_integrate_host launches one more: its fused kernel runs as a geometry
+ * half and a colour half around the arrival of the HD frame). */
 int vol_launches_per_frame(const vol_t *v);
 /* Device self-test of the branch-free exact reciprocal / division used on the hot path against the correctly rounded
  * library intrinsics: mismatches[0] = reciprocal over every binary32 in its operand range, mismatches[1] = TSDF

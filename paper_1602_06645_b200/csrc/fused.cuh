@@ -365,7 +365,7 @@ __device__ __forceinline__ void colour_cell(const Params &p, bool near, int ic0,
 // The ticket of the next item is drawn before the LAST cell: its latency is hidden, yet no item waits reserved behind a
 // long one.
 template <int R, bool COUNT>
-__device__ __forceinline__ void colour_item(const Params &p, uint32_t item, Stage &st, int &n, int lane, Counts &c, uint32_t &ticket)
+__device__ __forceinline__ void colour_item(const Params &p, uint32_t item, Stage &st, int &n, int lane, Counts &c, uint32_t *cursor, uint32_t &ticket)
 {
     const bool near = (item & ITEM_NEAR) != 0u;
     constexpr int CX = cells_x(R), CY = cells_y(R), WPT = words_per_tile(R);
@@ -382,40 +382,52 @@ __device__ __forceinline__ void colour_item(const Params &p, uint32_t item, Stag
     const int cgx0 = ttx * TX * R, cgy0 = tty * TY * R;
     const int cgz0 = local_to_global_tz(p, ttz) * TZ * R, clz0 = ttz * TZ * R;
     if (COUNT && lane == 0) atomicAdd(&p.ctrl[CTRL_CELLS], (uint32_t)__popc(bits));
-    if (bits == 0u) next_ticket(&p.ctrl[CTRL_CURSOR], lane, ticket);
+    if (bits == 0u) next_ticket(cursor, lane, ticket);
     while (bits) {
         const int b = word * 32 + (__ffs(bits) - 1);
         bits &= bits - 1;
-        if (bits == 0u) next_ticket(&p.ctrl[CTRL_CURSOR], lane, ticket);
+        if (bits == 0u) next_ticket(cursor, lane, ticket);
         const int cx = b % CX, cy = (b / CX) % CY, cz = b / (CX * CY);
         const int kz = cz * CLZ + (lane >> 3);
         colour_cell<COUNT>(p, near, cgx0 + cx * CLX + 4 * (lane & 1), cgy0 + cy * CLY + ((lane >> 1) & 3), cgz0 + kz, clz0 + kz, st, n, lane, c);
     }
 }
 
+// phase: PHASE_ALL = the whole queue in one launch (frames already on the device); PHASE_GEO / PHASE_COL = the geometry
+// items / the colour items only, so that vol_integrate_host can run the geometry half while the HD frame is still being
+// copied (only the colour update reads it).
+enum { PHASE_ALL = 0, PHASE_GEO = 1, PHASE_COL = 2 };
+
 template <int R, bool COUNT>
-__global__ void __launch_bounds__(CTA, 4) k_fused(const __grid_constant__ Params p)
+__global__ void __launch_bounds__(CTA, 4) k_fused(const __grid_constant__ Params p, int phase)
 {
     __shared__ Stage s_stage[WARPS_PER_CTA];
     const int lane = threadIdx.x & 31;
     Stage &st = s_stage[threadIdx.x >> 5];
     pdl_wait();
-    // queue order: NEAR geometry tiles (the longest items), colour items, ordinary geometry tiles (the shortest: the tail)
-    const uint32_t n_near = __ldcg(&p.ctrl[CTRL_NNEAR]), n_col = n_near + __ldcg(&p.ctrl[CTRL_NCOL]), n_items = n_col + __ldcg(&p.ctrl[CTRL_NGEO]);
+    // queue order, longest kind first: NEAR geometry tiles, colour items, ordinary geometry tiles (the shortest: the tail)
+    const uint32_t c_near = __ldcg(&p.ctrl[CTRL_NNEAR]), c_col = __ldcg(&p.ctrl[CTRL_NCOL]), c_geo = __ldcg(&p.ctrl[CTRL_NGEO]);
+    const uint32_t n_near = phase == PHASE_COL ? 0u : c_near;
+    const uint32_t n_col = n_near + (phase == PHASE_GEO ? 0u : c_col);
+    const uint32_t n_items = n_col + (phase == PHASE_COL ? 0u : c_geo);
+    uint32_t *cursor = &p.ctrl[phase == PHASE_COL ? CTRL_CURSOR2 : CTRL_CURSOR];
     Counts c = {0, 0, 0, 0};
     int n_staged = 0;
     // the ticket of the next item is requested before the current one is processed (the L2 round trip is hidden).
     // Only one item is reserved ahead: colour items are long, and a deeper reservation unbalances the tail.
     uint32_t ticket = 0;
-    next_ticket(&p.ctrl[CTRL_CURSOR], lane, ticket);
+    next_ticket(cursor, lane, ticket);
     for (;;) {
         const uint32_t it = __shfl_sync(0xffffffffu, ticket, 0);
         if (it >= n_items) break;
         const uint32_t item = it < n_near ? __ldcg(p.work_geo + ((uint32_t)p.n_tiles - 1u - it))
                                           : (it < n_col ? __ldcg(p.work_col + (it - n_near)) : __ldcg(p.work_geo + (it - n_col)));
-        if (it >= n_near && it < n_col) colour_item<R, COUNT>(p, item, st, n_staged, lane, c, ticket);
+        if (it >= n_near && it < n_col) colour_item<R, COUNT>(p, item, st, n_staged, lane, c, cursor, ticket);
         else {
-            next_ticket(&p.ctrl[CTRL_CURSOR], lane, ticket); geometry_prefetch(p, item, lane); geometry_tile<COUNT>(p, item, lane, c); }
+            next_ticket(cursor, lane, ticket);
+            geometry_prefetch(p, item, lane);
+            geometry_tile<COUNT>(p, item, lane, c);
+        }
     }
     if (n_staged > 0) colour_update_staged<COUNT>(p, st, 0, n_staged, lane, c);
     if (COUNT) {

@@ -85,7 +85,7 @@ __device__ __forceinline__ void item_unpack(uint32_t item, int &ttx, int &tty, i
     sub = (int)((item >> ITEM_SUB_SHIFT) & 127u);
 }
 
-enum { CTRL_NGEO = 0, CTRL_NCOL = 1, CTRL_CURSOR = 2, CTRL_TICKET = 3, CTRL_CELLS = 4, CTRL_NJOBS = 5, CTRL_NNEAR = 6, CTRL_N = 8 };
+enum { CTRL_NGEO = 0, CTRL_NCOL = 1, CTRL_CURSOR = 2, CTRL_TICKET = 3, CTRL_CELLS = 4, CTRL_NJOBS = 5, CTRL_NNEAR = 6, CTRL_CURSOR2 = 7, CTRL_N = 8 };
 
 // programmatic dependent launch: wait for the previous kernel of the stream (completion + memory flush) / allow the next
 // kernel's CTAs to be scheduled as this one drains

@@ -126,7 +126,7 @@ __global__ void __launch_bounds__(256) k_prepass(const __grid_constant__ Params 
     if (t < 16) { s_mn[t] = 0xffffu; s_mx[t] = 0u; }
     if (t == 0) s_njobs = 0u;
     if (blockIdx.x == 0 && blockIdx.y == 0 && t == 0) {
-        p.ctrl[CTRL_NGEO] = 0; p.ctrl[CTRL_NCOL] = 0; p.ctrl[CTRL_CURSOR] = 0; p.ctrl[CTRL_CELLS] = 0; p.ctrl[CTRL_NNEAR] = 0;
+        p.ctrl[CTRL_NGEO] = 0; p.ctrl[CTRL_NCOL] = 0; p.ctrl[CTRL_CURSOR] = 0; p.ctrl[CTRL_CELLS] = 0; p.ctrl[CTRL_NNEAR] = 0; p.ctrl[CTRL_CURSOR2] = 0;
     }
     __syncthreads();
     const int x = blockIdx.x * 32 + tx;

@@ -318,9 +318,16 @@ static int integrate_impl(vol_t *v, const uint16_t *depth_u16_dev, int32_t wd, i
         if (v->profiling) CK(cudaEventRecord(v->ev[1], s));                             \
         CK(launch(vf::k_items_col<RR>, dim3(g1), 256, s, true, p));                     \
         if (v->profiling) CK(cudaEventRecord(v->ev[2], s));                             \
-        if (rgb_ready) CK(cudaStreamWaitEvent(s, rgb_ready, 0));                        \
-        if (cnt) CK(launch(vf::k_fused<RR, true>, dim3(g2), vf::CTA, s, true, p));      \
-        else     CK(launch(vf::k_fused<RR, false>, dim3(g2), vf::CTA, s, true, p));     \
+        if (rgb_ready) {   /* geometry half now, colour half once the HD frame has arrived */           \
+            if (cnt) CK(launch(vf::k_fused<RR, true>, dim3(g2), vf::CTA, s, true, p, (int)vf::PHASE_GEO));   \
+            else     CK(launch(vf::k_fused<RR, false>, dim3(g2), vf::CTA, s, true, p, (int)vf::PHASE_GEO));  \
+            CK(cudaStreamWaitEvent(s, rgb_ready, 0));                                    \
+            if (cnt) CK(launch(vf::k_fused<RR, true>, dim3(g2), vf::CTA, s, false, p, (int)vf::PHASE_COL));  \
+            else     CK(launch(vf::k_fused<RR, false>, dim3(g2), vf::CTA, s, false, p, (int)vf::PHASE_COL)); \
+        } else {                                                                        \
+            if (cnt) CK(launch(vf::k_fused<RR, true>, dim3(g2), vf::CTA, s, true, p, (int)vf::PHASE_ALL));   \
+            else     CK(launch(vf::k_fused<RR, false>, dim3(g2), vf::CTA, s, true, p, (int)vf::PHASE_ALL));  \
+        }                                                                               \
     } while (0)
     switch (p.r) {
         case 1: VF_LAUNCH(1); break;
