@@ -64,6 +64,9 @@ struct Params {
     uint32_t *work_geo;          // geometry work list (n_tiles entries): ordinary tiles from the front, ITEM_NEAR tiles from the back
     uint32_t *marks;             // shell marks: words_per_tile(r) words per tile, bit = colour cell that may hold sigma-shell voxels
     uint32_t *work_col;          // colour work list: one item per non-zero mark NIBBLE (up to 4 colour cells)
+    uint8_t  *tile_neg;          // per geometry tile: 1 = the tile may hold an observed voxel with tsdf <= 0.  Set by the fused
+                                 // kernel when it writes one, never cleared except by vol_reset (vol_upload sets all): a
+                                 // conservative superset, used by the ray caster to skip free space
     uint32_t *ctrl;              // control words, see CTRL_* below
     unsigned long long *counters;// 4 voxel counters (counting variant only)
 };

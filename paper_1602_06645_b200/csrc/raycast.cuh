@@ -16,8 +16,40 @@ struct RayParams {
 };
 
 // One thread per pixel; a CTA covers 8 x 8 pixels (two warps of 8 x 4), so the rays of a warp stay close together and
-// their gathers share sectors.  Samples outside the volume are "unknown" and cannot produce a hit, so only the samples
-// between the ray's entry into and exit from the volume's box (one sample of slack on both sides) are visited.
+// their gathers share sectors.  Two exact shortcuts:
+//  * samples outside the volume are "unknown" and cannot produce a hit, so only the samples between the ray's entry into
+//    and exit from the volume's box (one sample of slack on both sides) are visited;
+//  * a hit needs a sample with tsdf <= 0 in an observed voxel (R4), and p.tile_neg lists (conservatively) the geometry
+//    tiles that may hold one.  A sample in any other tile cannot complete a hit, so its voxel is not read, and the ray
+//    jumps to the last sample that is safely inside that tile.  Such a sample may still be the F_prev of the next one:
+//    it is then evaluated lazily, only if the next sample turns out to be a candidate.
+struct RaySample { float t, f; bool known; int i, j, k; };        // (i, j, k) = the voxel that contains the sample, if inside
+
+// R2-R3 for sample k: canonical arithmetic, identical to the oracle's
+__device__ __forceinline__ RaySample ray_sample(const Params &p, const float (&dw)[3], const float (&ow)[3], float vs, float inv_vs,
+                                                float t_near, int k, bool &inside, int &tile)
+{
+    RaySample s;
+    s.t = __fmaf_rn((float)k, vs, t_near); s.f = 0.0f; s.known = false;
+    const float fi = floorf(__fmul_rn(__fsub_rn(__fmaf_rn(s.t, dw[0], ow[0]), p.ox), inv_vs));
+    const float fj = floorf(__fmul_rn(__fsub_rn(__fmaf_rn(s.t, dw[1], ow[1]), p.oy), inv_vs));
+    const float fk = floorf(__fmul_rn(__fsub_rn(__fmaf_rn(s.t, dw[2], ow[2]), p.oz), inv_vs));
+    inside = fi >= 0.0f && fi < (float)p.nx && fj >= 0.0f && fj < (float)p.ny && fk >= 0.0f && fk < (float)p.nz;
+    tile = -1; s.i = s.j = s.k = 0;
+    if (inside) {
+        s.i = (int)fi; s.j = (int)fj; s.k = (int)fk;
+        tile = ((s.k / TZ) * p.tiles_y + s.j / TY) * p.tiles_x + s.i / TX;      // the voxel itself is read by ray_voxel() when needed
+    }
+    return s;
+}
+
+__device__ __forceinline__ void ray_voxel(const Params &p, RaySample &s)
+{
+    const uint32_t word = __ldg(p.geo + ((size_t)s.k * (size_t)p.ny + (size_t)s.j) * (size_t)p.nx + (size_t)s.i);
+    s.known = (word >> 16) != 0u;                                                         // R3
+    s.f = s.known ? (float)(int)(short)(word & 0xffffu) : 0.0f;
+}
+
 __global__ void __launch_bounds__(64) k_raycast(const __grid_constant__ Params p, const __grid_constant__ RayParams q)
 {
     const int x = blockIdx.x * 8 + (threadIdx.x & 7), y = blockIdx.y * 8 + (threadIdx.x >> 3);
@@ -44,28 +76,52 @@ __global__ void __launch_bounds__(64) k_raycast(const __grid_constant__ Params p
             } else if (ow[a] < lo[a] || ow[a] > hi[a]) tb = -1.0f;
         }
     }
+    // culling only: the ray in grid coordinates, g(t) = go + t * gd, for the tile-exit computation
+    float go[3], gd[3];
+#pragma unroll
+    for (int a = 0; a < 3; ++a) { go[a] = (ow[a] - org[a]) * inv_vs; gd[a] = dw[a] * inv_vs; }
+    const int tdim[3] = {TX, TY, TZ};
     float depth = 0.0f;
     if (ta <= tb) {
-        const int k0 = max(0, (int)floorf((ta - q.t_near) * inv_vs) - 1);
+        int k = max(0, (int)floorf((ta - q.t_near) * inv_vs) - 1);
         const int k1 = (int)fminf(ceilf((tb - q.t_near) * inv_vs) + 1.0f, 2.0e9f);
-        float t_prev = 0.0f, f_prev = 0.0f;
-        bool known_prev = false;
-        for (int k = k0; k <= k1; ++k) {
-            const float t = __fmaf_rn((float)k, vs, q.t_near);                                  // R2
-            if (t > q.t_far) break;
-            const float fi = floorf(__fmul_rn(__fsub_rn(__fmaf_rn(t, dw[0], ow[0]), org[0]), inv_vs));
-            const float fj = floorf(__fmul_rn(__fsub_rn(__fmaf_rn(t, dw[1], ow[1]), org[1]), inv_vs));
-            const float fk = floorf(__fmul_rn(__fsub_rn(__fmaf_rn(t, dw[2], ow[2]), org[2]), inv_vs));
-            bool known = false; float f = 0.0f;
-            if (fi >= 0.0f && fi < (float)p.nx && fj >= 0.0f && fj < (float)p.ny && fk >= 0.0f && fk < (float)p.nz) {
-                const uint32_t word = __ldg(p.geo + ((size_t)(int)fk * (size_t)p.ny + (size_t)(int)fj) * (size_t)p.nx + (size_t)(int)fi);
-                if ((word >> 16) != 0u) { known = true; f = (float)(int)(short)(word & 0xffffu); }  // R3
+        RaySample prev; prev.t = 0.0f; prev.f = 0.0f; prev.known = false;
+        bool prev_pending = false;                          // sample k - 1 was skipped: evaluate it when it is needed
+        while (k <= k1) {
+            bool inside; int tile;
+            RaySample cur = ray_sample(p, dw, ow, vs, inv_vs, q.t_near, k, inside, tile);   // R2
+            if (cur.t > q.t_far) break;
+            if (!inside) { prev = cur; prev_pending = false; ++k; continue; }             // unknown sample
+            if (__ldg(p.tile_neg + tile) == 0) {
+                // no observed voxel with tsdf <= 0 in this tile: jump to the last sample that is inside it with a margin
+                // (the tile's box comes from the sample's canonical voxel indices, the exit from free-form arithmetic: if
+                // the two disagree at a tile boundary the exit lies behind the sample and nothing is skipped)
+                const int vox[3] = {cur.i, cur.j, cur.k};
+                float t_exit = 3.0e38f;
+#pragma unroll
+                for (int a = 0; a < 3; ++a) {
+                    const float lo = (float)((vox[a] / tdim[a]) * tdim[a]);
+                    if (gd[a] > 1e-9f) t_exit = fminf(t_exit, (lo + (float)tdim[a] - 0.05f - go[a]) / gd[a]);
+                    else if (gd[a] < -1e-9f) t_exit = fminf(t_exit, (lo + 0.05f - go[a]) / gd[a]);
+                }
+                const int kk = (int)fminf(floorf((t_exit - q.t_near) * inv_vs) - 1.0f, (float)k1);
+                k = max(k, kk) + 1;
+                prev_pending = true;
+                continue;
             }
-            if (known && known_prev && f_prev > 0.0f && !(f > 0.0f)) {                          // R4
-                depth = __fmaf_rn(vs, __fdiv_rn(f_prev, __fsub_rn(f_prev, f)), t_prev);
-                break;
+            ray_voxel(p, cur);
+            if (cur.known && !(cur.f > 0.0f)) {                                            // candidate: needs F_prev
+                if (prev_pending) {
+                    bool in2; int tile2;
+                    prev = ray_sample(p, dw, ow, vs, inv_vs, q.t_near, k - 1, in2, tile2);
+                    if (in2) ray_voxel(p, prev);
+                }
+                if (prev.known && prev.f > 0.0f) {                                         // R4
+                    depth = __fmaf_rn(vs, __fdiv_rn(prev.f, __fsub_rn(prev.f, cur.f)), prev.t);
+                    break;
+                }
             }
-            known_prev = known; t_prev = t; f_prev = f;
+            prev = cur; prev_pending = false; ++k;
         }
     }
     uint32_t c = 0u;

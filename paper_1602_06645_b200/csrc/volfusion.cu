@@ -195,6 +195,8 @@ extern "C" int vol_create(vol_t **out, const int32_t dims_geo[3], int32_t r, con
     if (cudaMalloc(&p.work_geo, sizeof(uint32_t) * nt) != cudaSuccess) rc = VOL_E_OOM;
     if (cudaMalloc(&p.work_col, sizeof(uint32_t) * nw * 8) != cudaSuccess) rc = VOL_E_OOM;
     if (cudaMalloc(&p.marks, sizeof(uint32_t) * nw) != cudaSuccess) rc = VOL_E_OOM;
+    if (cudaMalloc(&p.tile_neg, nt) != cudaSuccess) rc = VOL_E_OOM;
+    if (rc == VOL_OK && cudaMemset(p.tile_neg, 0, nt) != cudaSuccess) rc = VOL_E_CUDA;
     if (rc == VOL_OK && cudaMemset(p.marks, 0, sizeof(uint32_t) * nw) != cudaSuccess) rc = VOL_E_CUDA;
     if (cudaMalloc(&p.ctrl, sizeof(uint32_t) * vf::CTRL_N) != cudaSuccess) rc = VOL_E_OOM;
     if (cudaMalloc(&p.counters, sizeof(unsigned long long) * 4) != cudaSuccess) rc = VOL_E_OOM;
@@ -231,6 +233,7 @@ extern "C" void vol_destroy(vol_t *v)
     if (v->p.work_geo) cudaFree(v->p.work_geo);
     if (v->p.work_col) cudaFree(v->p.work_col);
     if (v->p.marks) cudaFree(v->p.marks);
+    if (v->p.tile_neg) cudaFree(v->p.tile_neg);
     if (v->p.ctrl) cudaFree(v->p.ctrl);
     if (v->p.counters) cudaFree(v->p.counters);
     if (v->p.pixmap) cudaFree(v->p.pixmap);
@@ -418,6 +421,7 @@ extern "C" int vol_upload(vol_t *v, const void *geo_host, const void *col_host, 
     cudaStream_t s = (cudaStream_t)stream;
     if (geo_host && v->geo_bytes) CK(cudaMemcpyAsync(v->p.geo, geo_host, v->geo_bytes, cudaMemcpyHostToDevice, s));
     if (col_host && v->col_bytes) CK(cudaMemcpyAsync(v->p.col, col_host, v->col_bytes, cudaMemcpyHostToDevice, s));
+    if (geo_host && v->p.n_tiles > 0) CK(cudaMemsetAsync(v->p.tile_neg, 1, (size_t)v->p.n_tiles, s));   // unknown content: no tile may be skipped
     CK(cudaStreamSynchronize(s));
     return VOL_OK;
 }
@@ -429,6 +433,7 @@ extern "C" int vol_reset(vol_t *v, void *stream)
     cudaStream_t s = (cudaStream_t)stream;
     if (v->geo_bytes) CK(cudaMemsetAsync(v->p.geo, 0, v->geo_bytes, s));
     if (v->col_bytes) CK(cudaMemsetAsync(v->p.col, 0, v->col_bytes, s));
+    if (v->p.n_tiles > 0) CK(cudaMemsetAsync(v->p.tile_neg, 0, (size_t)v->p.n_tiles, s));
     return VOL_OK;
 }
 
