@@ -142,7 +142,9 @@ __device__ __forceinline__ void geometry_tile(const Params &p, uint32_t item, in
             if ((w4[0] != o4[0]) | (w4[1] != o4[1]) | (w4[2] != o4[2]) | (w4[3] != o4[3])) *ptr = make_uint4(w4[0], w4[1], w4[2], w4[3]);
             ptr = reinterpret_cast<uint4 *>(reinterpret_cast<uint32_t *>(ptr) + layer);
         }
-        if (__any_sync(lanes, neg) && lane == __ffs(lanes) - 1) p.tile_neg[tile_index] = 1;
+        if (__any_sync(lanes, neg) && lane == __ffs(lanes) - 1) {
+            p.tile_neg[tile_index] = 1; p.brick_neg[((ttz / 4) * p.bricks_y + tty / 8) * p.bricks_x + ttx] = 1;
+        }
         return;
     }
     const float fx = p.fx, fy = p.fy, cx = p.cx, cy = p.cy;
@@ -232,7 +234,9 @@ __device__ __forceinline__ void geometry_tile(const Params &p, uint32_t item, in
         }
         ptr = pA2;
     }
-    if (__any_sync(lanes, neg) && lane == __ffs(lanes) - 1) p.tile_neg[tile_index] = 1;
+    if (__any_sync(lanes, neg) && lane == __ffs(lanes) - 1) {
+        p.tile_neg[tile_index] = 1; p.brick_neg[((ttz / 4) * p.bricks_y + tty / 8) * p.bricks_x + ttx] = 1;
+    }
 }
 
 // pull the 32 lines (8 layers x 4 rows x 128 bytes) of a geometry tile into L2: one line per lane, no register is tied up.

@@ -17,6 +17,7 @@ constexpr int TX = 32, TY = 4, TZ = 8;
 constexpr int CLX = 8, CLY = 4, CLZ = 4;
 // tile classification refines a tile that passes the coarse test on SUBX x 1 x SUBZ sub-boxes
 constexpr int SUBX = 4, SUBZ = 2;
+constexpr int BRICK = 32;                                   // ray-casting skip brick: BRICK^3 geometry voxels = 1 x 8 x 4 tiles
 constexpr int WARPS_PER_CTA = 8;
 constexpr int CTA = 32 * WARPS_PER_CTA;
 
@@ -67,6 +68,8 @@ struct Params {
     uint8_t  *tile_neg;          // per geometry tile: 1 = the tile may hold an observed voxel with tsdf <= 0.  Set by the fused
                                  // kernel when it writes one, never cleared except by vol_reset (vol_upload sets all): a
                                  // conservative superset, used by the ray caster to skip free space
+    uint8_t  *brick_neg;         // the same per brick of BRICK^3 geometry voxels (1 x 8 x 4 tiles): the ray caster's coarse level
+    int       bricks_x, bricks_y, bricks_z;
     uint32_t *ctrl;              // control words, see CTRL_* below
     unsigned long long *counters;// 4 voxel counters (counting variant only)
 };

@@ -92,16 +92,19 @@ __global__ void __launch_bounds__(64) k_raycast(const __grid_constant__ Params p
             RaySample cur = ray_sample(p, dw, ow, vs, inv_vs, q.t_near, k, inside, tile);   // R2
             if (cur.t > q.t_far) break;
             if (!inside) { prev = cur; prev_pending = false; ++k; continue; }             // unknown sample
-            if (__ldg(p.tile_neg + tile) == 0) {
-                // no observed voxel with tsdf <= 0 in this tile: jump to the last sample that is inside it with a margin
+            // coarse level first: a brick of BRICK^3 voxels (1 x 8 x 4 tiles) without such a voxel is crossed in one jump
+            const bool brick_free = __ldg(p.brick_neg + ((cur.k / BRICK) * p.bricks_y + cur.j / BRICK) * p.bricks_x + cur.i / BRICK) == 0;
+            if (brick_free || __ldg(p.tile_neg + tile) == 0) {
+                // no observed voxel with tsdf <= 0 in this brick / tile: jump to the last sample safely inside it
                 // (the tile's box comes from the sample's canonical voxel indices, the exit from free-form arithmetic: if
                 // the two disagree at a tile boundary the exit lies behind the sample and nothing is skipped)
                 const int vox[3] = {cur.i, cur.j, cur.k};
                 float t_exit = 3.0e38f;
 #pragma unroll
                 for (int a = 0; a < 3; ++a) {
-                    const float lo = (float)((vox[a] / tdim[a]) * tdim[a]);
-                    if (gd[a] > 1e-9f) t_exit = fminf(t_exit, (lo + (float)tdim[a] - 0.05f - go[a]) / gd[a]);
+                    const int bd = brick_free ? BRICK : tdim[a];
+                    const float lo = (float)((vox[a] / bd) * bd);
+                    if (gd[a] > 1e-9f) t_exit = fminf(t_exit, (lo + (float)bd - 0.05f - go[a]) / gd[a]);
                     else if (gd[a] < -1e-9f) t_exit = fminf(t_exit, (lo + 0.05f - go[a]) / gd[a]);
                 }
                 const int kk = (int)fminf(floorf((t_exit - q.t_near) * inv_vs) - 1.0f, (float)k1);

@@ -197,6 +197,10 @@ extern "C" int vol_create(vol_t **out, const int32_t dims_geo[3], int32_t r, con
     if (cudaMalloc(&p.marks, sizeof(uint32_t) * nw) != cudaSuccess) rc = VOL_E_OOM;
     if (cudaMalloc(&p.tile_neg, nt) != cudaSuccess) rc = VOL_E_OOM;
     if (rc == VOL_OK && cudaMemset(p.tile_neg, 0, nt) != cudaSuccess) rc = VOL_E_CUDA;
+    p.bricks_x = p.tiles_x; p.bricks_y = (p.tiles_y + 7) / 8; p.bricks_z = (my_slabs + 3) / 4;
+    const size_t nb = (size_t)p.bricks_x * p.bricks_y * p.bricks_z + 1;
+    if (cudaMalloc(&p.brick_neg, nb) != cudaSuccess) rc = VOL_E_OOM;
+    if (rc == VOL_OK && cudaMemset(p.brick_neg, 0, nb) != cudaSuccess) rc = VOL_E_CUDA;
     if (rc == VOL_OK && cudaMemset(p.marks, 0, sizeof(uint32_t) * nw) != cudaSuccess) rc = VOL_E_CUDA;
     if (cudaMalloc(&p.ctrl, sizeof(uint32_t) * vf::CTRL_N) != cudaSuccess) rc = VOL_E_OOM;
     if (cudaMalloc(&p.counters, sizeof(unsigned long long) * 4) != cudaSuccess) rc = VOL_E_OOM;
@@ -234,6 +238,7 @@ extern "C" void vol_destroy(vol_t *v)
     if (v->p.work_col) cudaFree(v->p.work_col);
     if (v->p.marks) cudaFree(v->p.marks);
     if (v->p.tile_neg) cudaFree(v->p.tile_neg);
+    if (v->p.brick_neg) cudaFree(v->p.brick_neg);
     if (v->p.ctrl) cudaFree(v->p.ctrl);
     if (v->p.counters) cudaFree(v->p.counters);
     if (v->p.pixmap) cudaFree(v->p.pixmap);
@@ -421,7 +426,10 @@ extern "C" int vol_upload(vol_t *v, const void *geo_host, const void *col_host, 
     cudaStream_t s = (cudaStream_t)stream;
     if (geo_host && v->geo_bytes) CK(cudaMemcpyAsync(v->p.geo, geo_host, v->geo_bytes, cudaMemcpyHostToDevice, s));
     if (col_host && v->col_bytes) CK(cudaMemcpyAsync(v->p.col, col_host, v->col_bytes, cudaMemcpyHostToDevice, s));
-    if (geo_host && v->p.n_tiles > 0) CK(cudaMemsetAsync(v->p.tile_neg, 1, (size_t)v->p.n_tiles, s));   // unknown content: no tile may be skipped
+    if (geo_host && v->p.n_tiles > 0) {                       // unknown content: no tile or brick may be skipped
+        CK(cudaMemsetAsync(v->p.tile_neg, 1, (size_t)v->p.n_tiles, s));
+        CK(cudaMemsetAsync(v->p.brick_neg, 1, (size_t)v->p.bricks_x * v->p.bricks_y * v->p.bricks_z, s));
+    }
     CK(cudaStreamSynchronize(s));
     return VOL_OK;
 }
@@ -433,7 +441,10 @@ extern "C" int vol_reset(vol_t *v, void *stream)
     cudaStream_t s = (cudaStream_t)stream;
     if (v->geo_bytes) CK(cudaMemsetAsync(v->p.geo, 0, v->geo_bytes, s));
     if (v->col_bytes) CK(cudaMemsetAsync(v->p.col, 0, v->col_bytes, s));
-    if (v->p.n_tiles > 0) CK(cudaMemsetAsync(v->p.tile_neg, 0, (size_t)v->p.n_tiles, s));
+    if (v->p.n_tiles > 0) {
+        CK(cudaMemsetAsync(v->p.tile_neg, 0, (size_t)v->p.n_tiles, s));
+        CK(cudaMemsetAsync(v->p.brick_neg, 0, (size_t)v->p.bricks_x * v->p.bricks_y * v->p.bricks_z, s));
+    }
     return VOL_OK;
 }
 
