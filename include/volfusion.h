@@ -51,8 +51,10 @@ typedef struct vol vol_t;   /* opaque; owns (or borrows) the two device buffers 
 typedef struct {
     float   sigma_m;        /* colour distance gate sigma, metres; <= 0 selects the paper's 0.020 */
     float   gate;           /* weight gate factor; <= 0 selects the paper's 0.8 */
-    void   *geo_dev;        /* DEVICE, optional caller-owned storage of info.geo_bytes (e.g. a torch tensor); NULL = library allocates */
-    void   *col_dev;        /* DEVICE, optional caller-owned storage of info.col_bytes */
+    void   *geo_dev;        /* DEVICE, optional caller-owned storage of info.geo_bytes (e.g. a torch tensor); NULL = library allocates.
+                               16-byte aligned; zeroed by vol_create.  While the volume exists the library must stay its only
+                               writer (it keeps per-tile summaries of the content): change it through vol_upload / vol_reset */
+    void   *col_dev;        /* DEVICE, optional caller-owned storage of info.col_bytes; same rules */
     int32_t device;         /* CUDA device ordinal; < 0 = current device */
     int32_t shard_rank;     /* multi-GPU z-slab sharding; rank 0 of world 1 = whole volume */
     int32_t shard_world;    /* <= 0 is read as 1 */
@@ -122,7 +124,7 @@ int vol_download(const vol_t *v, void *geo_host, size_t geo_bytes, void *col_hos
  * shard); the packed words are written to HOST geo_words / col_words.  Used for sampled parity at full size. */
 int vol_download_voxels(const vol_t *v, const int64_t *geo_idx, int64_t n_geo, uint32_t *geo_words,
                         const int64_t *col_idx, int64_t n_col, uint32_t *col_words, void *stream);
-/* Overwrite this shard's volumes from HOST buffers (resume / test seeding); either may be NULL to skip. */
+/* Overwrite this shard's volumes from HOST buffers (resume / test seeding); either may be NULL to skip.  Synchronises. */
 int vol_upload(vol_t *v, const void *geo_host, const void *col_host, void *stream);
 /* Zero both volumes (asynchronous). */
 int vol_reset(vol_t *v, void *stream);
