@@ -105,6 +105,35 @@ class ClockSampler(threading.Thread):
                 "reasons": reasons, "samples": len(sm), "samples_under_load": len(busy)}
 
 
+class NvmlClocks:
+    """SM clock and throttle reasons read through NVML from this process: polled while the timed frames are still running on
+    the device (the timed region is only milliseconds long, shorter than nvidia-smi's sampling period)."""
+
+    def __init__(self, index):
+        self.h, self.sm, self.reasons = None, [], set()
+        try:
+            import pynvml
+            self.nv = pynvml
+            pynvml.nvmlInit()
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+        except Exception:
+            self.h = None
+
+    def sample(self):
+        if self.h is None:
+            return
+        try:
+            nv = self.nv
+            self.sm.append(float(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)))
+            r = int(nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)) if hasattr(nv, "nvmlDeviceGetCurrentClocksEventReasons") \
+                else int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h))
+            for name, bit in (("hw_slowdown", 0x8), ("sw_power_cap", 0x4), ("sw_thermal_slowdown", 0x20), ("hw_thermal_slowdown", 0x40)):
+                if r & bit:
+                    self.reasons.add(name)
+        except Exception:
+            pass
+
+
 def workload_name(c):
     return (f"{c.name}: geometry {c.dims_geo[0]}^3 over {c.extent} m, colour {c.dims_col[0]}^3 (r={c.r}), depth {c.wd}x{c.hd}, "
             f"rgb {c.wh}x{c.hh}")
@@ -245,6 +274,7 @@ def run_ours(args, rank, world, local_rank):
     for i in range(W):
         integrate_dev(i)
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(K)]
+    nvml = NvmlClocks(local_rank) if rank == 0 else None
     barrier()
     for n, i in enumerate(range(W, nfr)):
         if not args.no_flush:
@@ -252,6 +282,10 @@ def run_ours(args, rank, world, local_rank):
         ev[n][0].record(stream)
         integrate_dev(i)
         ev[n][1].record(stream)
+        if nvml and n % 4 == 3:
+            nvml.sample()                                         # the device is busy with the frames enqueued so far
+    while nvml and not ev[K - 1][1].query():
+        nvml.sample()
     barrier()
     per_frame_ms = np.array([a.elapsed_time(b) for a, b in ev])
     total_ms = float(per_frame_ms.sum())
@@ -289,6 +323,10 @@ def run_ours(args, rank, world, local_rank):
     raycast_hit = float((rc_depth > 0).float().mean())
     total_ms, e2e_ms = max_over_ranks([total_ms, e2e_ms], world, "cuda")
     clocks = sampler.stop() if sampler else None
+    if clocks is not None and nvml is not None and nvml.sm:
+        # clocks DURING the timed region (NVML, in-process); the nvidia-smi figures cover the whole run
+        clocks.update({"sm_mhz_whole_run": clocks["sm_mhz"], "sm_mhz": float(np.median(nvml.sm)), "samples_timed_region": len(nvml.sm),
+                       "reasons": sorted(set(clocks["reasons"]) | nvml.reasons)})
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
