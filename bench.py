@@ -59,18 +59,32 @@ def peaks():
         return 6650.0, "fallback (B200_PROFILING.md)"
 
 
-def ncu_traffic(workload):
-    """DRAM bytes (dram__bytes_read.sum + dram__bytes_write.sum) per k_fused launch from the committed ncu --set full
-    capture of this workload (profiles/traffic.csv: workload,kernel,dram_bytes_per_launch), or None if none is recorded."""
+def ncu_traffic(workload, column=2):
+    """Per k_fused launch, from the committed ncu --set full capture of this workload (profiles/traffic.csv:
+    workload,kernel,dram_bytes_per_launch,warp_instructions_per_launch): DRAM bytes (column 2) or warp instructions
+    (column 3); None if none is recorded."""
     try:
         with open(os.path.join(ROOT, "profiles", "traffic.csv")) as f:
             for line in f:
                 cols = [c.strip() for c in line.split(",")]
-                if len(cols) >= 3 and cols[0] == workload and cols[1] == "k_fused":
-                    return float(cols[2])
+                if len(cols) > column and cols[0] == workload and cols[1] == "k_fused":
+                    return float(cols[column])
     except Exception:
         pass
     return None
+
+
+def issue_roofline(workload, fused_ms_mean, sm_mhz):
+    """The bound the fused kernel actually runs into: warp instructions issued per second against
+    148 SMs x 4 schedulers x 1 instruction per cycle at the SM clock seen during the run.  The instruction count per
+    launch comes from the committed ncu capture (it cannot be measured outside a profiler)."""
+    inst = ncu_traffic(workload, 3)
+    if inst is None or not sm_mhz:
+        return None
+    peak = 148 * 4 * sm_mhz * 1e6
+    achieved = inst / (fused_ms_mean * 1e-3)
+    return {"bound": "alu", "achieved": achieved / 1e12, "peak": peak / 1e12, "unit": "T warp-instructions/s", "frac": achieved / peak,
+            "warp_instructions_per_launch": inst, "source": "profiles/traffic.csv (ncu smsp__inst_executed.sum)"}
 
 
 class ClockSampler(threading.Thread):
@@ -359,7 +373,9 @@ def run_ours(args, rank, world, local_rank):
                            "cells_col": float(cnt[:, 6].mean()), "algorithmic_bytes": float(alg_bytes.mean())},
         "roofline": {"bound": "hbm", "kernel": "k_fused", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                      "traffic": ncu_traffic(c.name + ("-stress" if args.stress else "")), "peak_source": peak_src,
-                     "dense_sweep_frac": float(8.0 * nvox / (fused_ms.mean() * 1e-3) / 1e9 / peak)},
+                     "dense_sweep_frac": float(8.0 * nvox / (fused_ms.mean() * 1e-3) / 1e9 / peak),
+                     "issue": issue_roofline(c.name + ("-stress" if args.stress else ""), float(fused_ms.mean()),
+                                             (clocks or {}).get("sm_mhz"))},
         "e2e": {"value": e2e_value, "unit": UNIT, "ms_per_step": e2e_ms / K, "h2d_bytes_per_step": frame_bytes,
                 "d2h_bytes_per_step": 64},
         "raycast": {"ms": raycast_ms, "rays_per_s": c.wd * c.hd / (raycast_ms * 1e-3), "image": f"{c.wd}x{c.hd}", "hit_fraction": raycast_hit,
