@@ -75,3 +75,18 @@ def test_tsdf_column_fixture():
     for k, (val,) in rows("tsdf_column_cfg1.txt"):
         assert q[int(k)] == val, (k, q[int(k)], val)
     assert v.geo[35, 32, 32] == 0 and np.all(q[:29] == 32767)
+
+
+def test_tsdf_column_fixture_is_the_closed_form():
+    """The fixture itself, against reading A5 evaluated in float64: q = 32767 * (d - z_k) / mu with d = 1.5 m,
+    z_k = 1 + (k + 0.5) / 64, mu = 3 / 64 -- thirds and halves of 32767.  Every stored value is within half a unit of it
+    (the two exact ties, k = 30 and k = 33, resolve upwards because D = 1500 * 0.001f is one ulp above 1.5)."""
+    for k, (val,) in rows("tsdf_column_cfg1.txt"):
+        k = int(k)
+        ideal = 32767.0 * (1.5 - (1.0 + (k + 0.5) / 64.0)) / (3.0 / 64.0)
+        if ideal > 32767.0:
+            assert val == 32767
+        elif ideal < -32767.0:
+            assert val == 0                                  # behind the band: the untouched word
+        else:
+            assert abs(val - ideal) <= 0.5 + 1e-6, (k, val, ideal)
