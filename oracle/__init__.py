@@ -56,6 +56,8 @@ def _load():
         lib.ref_integrate_subset.argtypes = [P, P, P, ctypes.c_int64, P, P, ctypes.c_int64, P]
         lib.ref_frame_constants.restype = ctypes.c_int
         lib.ref_frame_constants.argtypes = [P, P, P]
+        lib.ref_sample_colour.restype = ctypes.c_int
+        lib.ref_sample_colour.argtypes = [P, P, P, ctypes.c_int64, P]
         lib.ref_raycast.restype = ctypes.c_int
         lib.ref_raycast.argtypes = [P, P, P, ctypes.c_int32, ctypes.c_int32, P, P, ctypes.c_float, ctypes.c_float, P, P]
         _lib = lib
@@ -120,6 +122,15 @@ class RefVolume:
                                           col_idx.ctypes.data, col_idx.size, col_words.ctypes.data)
         if rc != 0:
             raise ValueError("ref_integrate_subset: bad arguments")
+
+    def sample_colour(self, pts):
+        """ref_sample_colour: packed colour words (uint32 [n]) of the colour voxels containing the world points pts [n, 3]."""
+        pts = np.ascontiguousarray(pts, dtype=np.float32).reshape(-1, 3)
+        out = np.zeros(pts.shape[0], dtype=np.uint32)
+        rc = _load().ref_sample_colour(ctypes.addressof(self.desc), self.col.ctypes.data, pts.ctypes.data, pts.shape[0], out.ctypes.data)
+        if rc != 0:
+            raise ValueError("ref_sample_colour: bad arguments")
+        return out
 
     def raycast(self, w, h, T_world_cam, K, t_near, t_far):
         """ref_raycast: (depth float32 [h, w] metres, 0 = no surface; rgb uint8 [h, w, 3]) seen by a virtual camera."""

@@ -350,3 +350,30 @@ int ref_raycast(const ref_vol_t *v, const uint32_t *geo, const uint32_t *col, in
         }
     return 0;
 }
+
+/* ------------------------------------------------------------------------------------------ */
+/* ref_sample_colour -- NEXT row: colour-volume lookup at world points     */
+/* ------------------------------------------------------------------------------------------ */
+/* The primitive under the paper's per-polygon texture maps: "Given the 3D world positions, the RGB value of any pixel
+ * can be found by accessing the colour volume" (the positions are V_a + i * V_aV_green + j * V_aV_blue of
+ * eq. 11-14, computed by the caller).  Reading S1 (the paper does not say how the volume is accessed): the
+ * colour voxel whose cell contains the point -- index floor((p - origin) / vc) per axis, evaluated in binary32 as
+ * (p - origin) * (1 / vc) -- nearest voxel, no interpolation; the packed word {R, G, B, wq} of that voxel, or 0 for a
+ * point outside the volume.  pts: n x 3 floats (world); words_out: n uint32. */
+int ref_sample_colour(const ref_vol_t *v, const uint32_t *col, const float *pts, int64_t n, uint32_t *words_out)
+{
+    if (!v || !col || (n > 0 && (!pts || !words_out)) || n < 0) return -1;
+    const float vc = (v->extent / (float)v->nx) / (float)v->r, inv_vc = 1.0f / vc;
+    const int cnx = v->nx * v->r, cny = v->ny * v->r, cnz = v->nz * v->r;
+#pragma omp parallel for schedule(static)
+    for (int64_t m = 0; m < n; ++m) {
+        const float hx = floorf((pts[3 * m + 0] - v->origin[0]) * inv_vc);
+        const float hy = floorf((pts[3 * m + 1] - v->origin[1]) * inv_vc);
+        const float hz = floorf((pts[3 * m + 2] - v->origin[2]) * inv_vc);
+        uint32_t w = 0;
+        if (hx >= 0.0f && hx < (float)cnx && hy >= 0.0f && hy < (float)cny && hz >= 0.0f && hz < (float)cnz)
+            w = col[((size_t)(int)hz * (size_t)cny + (size_t)(int)hy) * (size_t)cnx + (size_t)(int)hx];
+        words_out[m] = w;
+    }
+    return 0;
+}
