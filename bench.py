@@ -335,6 +335,28 @@ def run_ours(args, rank, world, local_rank):
     torch.cuda.synchronize()
     raycast_ms = float(r0.elapsed_time(r1)) / 10.0
     raycast_hit = float((rc_depth > 0).float().mean())
+    # ---- NEXT row: vol_sample_colour at surface points -- the ray-cast hit points, 8 jittered copies
+    #      each (about the density of a texture map with Size_pixel = one colour voxel), as a polygon texture map would ask
+    Tl = torch.from_numpy(np.asarray(T_last, np.float32)).cuda()
+    yy, xx = torch.meshgrid(torch.arange(c.hd, device="cuda", dtype=torch.float32), torch.arange(c.wd, device="cuda", dtype=torch.float32), indexing="ij")
+    zz = rc_depth.reshape(c.hd, c.wd)
+    cam = torch.stack([(xx - float(c.K_depth[0, 2])) / float(c.K_depth[0, 0]) * zz, (yy - float(c.K_depth[1, 2])) / float(c.K_depth[1, 1]) * zz, zz], dim=-1)
+    hit_pts = (cam.reshape(-1, 3) @ Tl[:3, :3].T + Tl[:3, 3])[rc_depth > 0]
+    gen = torch.Generator(device="cuda"); gen.manual_seed(1)
+    sp_pts = (hit_pts.repeat(8, 1) + (torch.rand(hit_pts.shape[0] * 8, 3, device="cuda", generator=gen) - 0.5) * (2.0 * c.voxel / c.r)).contiguous()
+    sp_out = torch.empty(sp_pts.shape[0], dtype=torch.int32, device="cuda")
+    sample_ms, sample_filled = None, None
+    if sp_pts.shape[0] > 0:
+        for _ in range(3):
+            vol.sample_colour(sp_pts, sp_pts.shape[0], sp_out, stream=stream)
+        torch.cuda.synchronize()
+        r0.record(stream)
+        for _ in range(10):
+            vol.sample_colour(sp_pts, sp_pts.shape[0], sp_out, stream=stream)
+        r1.record(stream)
+        torch.cuda.synchronize()
+        sample_ms = float(r0.elapsed_time(r1)) / 10.0
+        sample_filled = float(((sp_out.view(torch.int32) >> 24) != 0).float().mean())
     total_ms, e2e_ms = max_over_ranks([total_ms, e2e_ms], world, "cuda")
     clocks = sampler.stop() if sampler else None
     if clocks is not None and nvml is not None and nvml.sm:
@@ -380,6 +402,9 @@ def run_ours(args, rank, world, local_rank):
                 "d2h_bytes_per_step": 64},
         "raycast": {"ms": raycast_ms, "rays_per_s": c.wd * c.hd / (raycast_ms * 1e-3), "image": f"{c.wd}x{c.hd}", "hit_fraction": raycast_hit,
                     "note": "vol_raycast of the fused volumes (SURVEY 8(f) rank 1), not part of the timed step"},
+        "sample_colour": None if sample_ms is None else {
+            "ms": sample_ms, "points": int(sp_pts.shape[0]), "points_per_s": sp_pts.shape[0] / (sample_ms * 1e-3), "filled_fraction": sample_filled,
+            "note": "vol_sample_colour at jittered surface points (SURVEY 8(f) rank 3), not part of the timed step"},
         "gpu_launches": vol.launches_per_frame() * K,
         "clocks": clocks,
     }

@@ -118,6 +118,13 @@ int vol_integrate_host(vol_t *v, const uint16_t *depth_u16_host, int32_t wd, int
 int vol_raycast(const vol_t *v, int32_t w, int32_t h, const float T_world_cam[16], const float K[9], float t_near_m,
                 float t_far_m, float *depth_dev, uint8_t *rgb8_dev, void *stream);
 
+/* Look up the colour volume at n world points ("given the 3D world positions, the RGB value of any pixel can
+ * be found by accessing the colour volume" -- the positions of a polygon's texture map are V_a + i V_aV_green + j V_aV_blue
+ * of eq. 11-14, computed by the caller).  points_dev: DEVICE, n x 3 float32 (x, y, z in world metres); words_dev: DEVICE,
+ * n uint32: the packed colour word (layout above) of the colour voxel whose cell contains the point (nearest voxel), 0 for
+ * a point outside the volume.  Unsharded volumes only.  Asynchronous on `stream`. */
+int vol_sample_colour(const vol_t *v, const float *points_dev, int64_t n, uint32_t *words_dev, void *stream);
+
 /* Copy this shard's volumes to HOST buffers of at least info.geo_bytes / info.col_bytes (either may be NULL to skip). */
 int vol_download(const vol_t *v, void *geo_host, size_t geo_bytes, void *col_host, size_t col_bytes, void *stream);
 /* Gather single voxels: geo_idx / col_idx are HOST int64 linear indices into the FULL grids (must be owned by this

@@ -142,4 +142,21 @@ __global__ void __launch_bounds__(64) k_raycast(const __grid_constant__ Params p
     if (q.rgb) { q.rgb[3 * o] = (uint8_t)c; q.rgb[3 * o + 1] = (uint8_t)(c >> 8); q.rgb[3 * o + 2] = (uint8_t)(c >> 16); }
 }
 
+// NEXT row: colour-volume lookup at world points -- the primitive under the paper's per-polygon
+// texture maps (the positions come from eq. 11-14).  Reading S1: the colour voxel whose cell contains the
+// point, nearest voxel; the packed word {R, G, B, wq}, or 0 outside the volume.  One thread per point.
+__global__ void __launch_bounds__(256) k_sample_colour(const __grid_constant__ Params p, const float *__restrict__ pts, long long n,
+                                                       uint32_t *__restrict__ words)
+{
+    const long long m = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (m >= n) return;
+    const float hx = floorf(__fmul_rn(__fsub_rn(__ldg(pts + 3 * m + 0), p.ox), p.inv_vc));
+    const float hy = floorf(__fmul_rn(__fsub_rn(__ldg(pts + 3 * m + 1), p.oy), p.inv_vc));
+    const float hz = floorf(__fmul_rn(__fsub_rn(__ldg(pts + 3 * m + 2), p.oz), p.inv_vc));
+    uint32_t w = 0u;
+    if (hx >= 0.0f && hx < (float)p.cnx && hy >= 0.0f && hy < (float)p.cny && hz >= 0.0f && hz < (float)p.cnz)
+        w = __ldg(p.col + ((size_t)(int)hz * (size_t)p.cny + (size_t)(int)hy) * (size_t)p.cnx + (size_t)(int)hx);
+    words[m] = w;
+}
+
 }  // namespace vf

@@ -90,3 +90,30 @@ def test_raycast_cfg3_full_size():
     d, rgb = cast_both(g, o, c.wd, c.hd, synth.frame(c, 3)[2], c.K_depth, 0.3, 5.0)
     assert (d > 0).mean() > 0.5 and (rgb.sum(axis=2) > 0).mean() > 0.3
     g.close()
+
+
+def test_sample_colour_and_polygon_texture_map():
+    """vol_sample_colour against the oracle, word for word: random points inside and outside config 1's
+    fused colour volume, and the texture map of a polygon laid on the sphere's surface by eq. 11-14."""
+    import torch
+    c = synth.config(1)
+    g, o = fused_pair(c, range(5))
+    rng = np.random.default_rng(9)
+    pts = rng.uniform(-0.7, 0.7, size=(200000, 3)).astype(np.float32) + np.array([0, 0, 1.5], np.float32)
+    # a triangle tangent to the sphere (centre (0,0,1.5), R = 0.3) on its camera-facing side
+    Va, Vb, Vc = np.array([-0.1, -0.08, 1.225]), np.array([0.12, -0.08, 1.228]), np.array([-0.1, 0.1, 1.23])
+    size_pixel = 0.001
+    w, h = int(np.linalg.norm(Vb - Va) / size_pixel), int(np.linalg.norm(Vc - Va) / size_pixel)      # eq. 11, 12
+    green, blue = (Vb - Va) / (w - 1), (Vc - Va) / (h - 1)                                            # eq. 13, 14
+    jj, ii = np.meshgrid(np.arange(h), np.arange(w), indexing="ij")
+    tex_pts = (Va + ii[..., None] * green + jj[..., None] * blue).reshape(-1, 3).astype(np.float32)
+    allp = np.concatenate([pts, tex_pts])
+    dp = torch.from_numpy(allp).cuda()
+    dw = torch.full((allp.shape[0],), -1, dtype=torch.int32, device="cuda")
+    g.sample_colour(dp, allp.shape[0], dw)
+    torch.cuda.synchronize()
+    got = dw.cpu().numpy().view(np.uint32)
+    want = o.sample_colour(allp)
+    assert np.array_equal(got, want)
+    assert (want[: pts.shape[0]] >> 24 > 0).sum() > 500 and (want[pts.shape[0]:] >> 24 > 0).mean() > 0.3   # both hit filled voxels
+    g.sample_colour(dp, 0, dw)                                                                         # n = 0 is a no-op
