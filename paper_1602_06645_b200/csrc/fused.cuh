@@ -124,8 +124,6 @@ __device__ __forceinline__ void geometry_tile(const Params &p, uint32_t item, in
     const float r02 = p.R[2], r12 = p.R[5], r22 = p.R[8];
     const size_t layer = (size_t)p.ny * p.nx;
     uint4 *ptr = reinterpret_cast<uint4 *>(p.geo + ((size_t)lz0 * p.ny + j) * p.nx + i0);
-    const int tile_index = (ttz * p.tiles_y + tty) * p.tiles_x + ttx;
-    bool neg = false;                                     // this lane wrote an observed voxel with tsdf <= 0 (for p.tile_neg)
     if (near) {
         for (int z = 0; z < nl; ++z) {
             const uint4 cur = *ptr;
@@ -137,13 +135,9 @@ __device__ __forceinline__ void geometry_tile(const Params &p, uint32_t item, in
                 bool rd = false;
                 w4[e] = geo_voxel_ref(p, __fmaf_rn(r02, pz, bX[e]), __fmaf_rn(r12, pz, bY[e]), __fmaf_rn(r22, pz, bZ[e]), o4[e], rd);
                 if (COUNT) { c.gr += rd; c.gc += w4[e] != o4[e]; }
-                neg = neg | ((w4[e] >> 16) != 0u && (int)(short)(w4[e] & 0xffffu) <= 0);
             }
             if ((w4[0] != o4[0]) | (w4[1] != o4[1]) | (w4[2] != o4[2]) | (w4[3] != o4[3])) *ptr = make_uint4(w4[0], w4[1], w4[2], w4[3]);
             ptr = reinterpret_cast<uint4 *>(reinterpret_cast<uint32_t *>(ptr) + layer);
-        }
-        if (__any_sync(lanes, neg) && lane == __ffs(lanes) - 1) {
-            p.tile_neg[tile_index] = 1; p.brick_neg[((ttz / 4) * p.bricks_y + tty / 8) * p.bricks_x + ttx] = 1;
         }
         return;
     }
@@ -209,7 +203,6 @@ __device__ __forceinline__ void geometry_tile(const Params &p, uint32_t item, in
                 const int wn = min(wi + 1, w_max);
                 const uint32_t nw = (qn & 0xffffu) | ((uint32_t)wn << 16);
                 w4[e] = upd[e] ? nw : o4[e];
-                neg = neg | (upd[e] & ((int)(short)(qn & 0xffffu) <= 0));      // only this branch can write tsdf <= 0
             }
         }
         const bool any = (w4[0] != o4[0]) | (w4[1] != o4[1]) | (w4[2] != o4[2]) | (w4[3] != o4[3]);
@@ -233,9 +226,6 @@ __device__ __forceinline__ void geometry_tile(const Params &p, uint32_t item, in
             update_layer(pB, curB, ZB, dB);
         }
         ptr = pA2;
-    }
-    if (__any_sync(lanes, neg) && lane == __ffs(lanes) - 1) {
-        p.tile_neg[tile_index] = 1; p.brick_neg[((ttz / 4) * p.bricks_y + tty / 8) * p.bricks_x + ttx] = 1;
     }
 }
 

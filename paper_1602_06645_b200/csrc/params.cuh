@@ -65,9 +65,9 @@ struct Params {
     uint32_t *work_geo;          // geometry work list (n_tiles entries): ordinary tiles from the front, ITEM_NEAR tiles from the back
     uint32_t *marks;             // shell marks: words_per_tile(r) words per tile, bit = colour cell that may hold sigma-shell voxels
     uint32_t *work_col;          // colour work list: one item per non-zero mark NIBBLE (up to 4 colour cells)
-    uint8_t  *tile_neg;          // per geometry tile: 1 = the tile may hold an observed voxel with tsdf <= 0.  Set by the fused
-                                 // kernel when it writes one, never cleared except by vol_reset (vol_upload sets all): a
-                                 // conservative superset, used by the ray caster to skip free space
+    uint8_t  *tile_neg;          // per geometry tile: 1 = the tile may hold an observed voxel with tsdf <= 0.  Set by the tile
+                                 // classification (k_mark_classify), never cleared except by vol_reset (vol_upload sets
+                                 // all): a conservative superset, used by the ray caster to skip free space
     uint8_t  *brick_neg;         // the same per brick of BRICK^3 geometry voxels (1 x 8 x 4 tiles): the ray caster's coarse level
     int       bricks_x, bricks_y, bricks_z;
     uint32_t *ctrl;              // control words, see CTRL_* below

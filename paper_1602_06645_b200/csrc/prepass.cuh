@@ -333,12 +333,16 @@ __global__ void __launch_bounds__(256) k_mark_classify(const __grid_constant__ P
     __syncthreads();
     uint32_t near = 0;
     int ttx = 0, tty = 0, ttz = 0;
+    bool behind = false;
     if (tile < p.n_tiles) {
         ttx = tile % p.tiles_x; tty = (tile / p.tiles_x) % p.tiles_y; ttz = tile / (p.tiles_x * p.tiles_y);
         float cX, cY, cZ;
         tile_centre(p, ttx, tty, ttz, cX, cY, cZ);
         if (!(cZ - p.tile_ez > 2e-3f)) near = ITEM_NEAR;
-        if (box_may_update(p, cX, cY, cZ, p.tile_ex, p.tile_ey, p.tile_ez) != 0) {
+        const int coarse = box_may_update(p, cX, cY, cZ, p.tile_ex, p.tile_ey, p.tile_ez);
+        // not wholly (by >= 0.1 mm) in front of every depth it can see; with mu > 1 m even 0.1 mm could quantise to tsdf = 0
+        behind = coarse == 1 || (coarse == 2 && !(p.mu <= 1.0f));
+        if (coarse != 0) {
             const uint32_t k = atomicAdd(&s_nsurv, 1u);
             s_surv[k] = (uint16_t)t;
             s_c[t][0] = cX; s_c[t][1] = cY; s_c[t][2] = cZ;
@@ -360,6 +364,13 @@ __global__ void __launch_bounds__(256) k_mark_classify(const __grid_constant__ P
     // NEAR tiles take the slow per-voxel routines (several times longer than an ordinary tile): they are listed from the
     // back of the work list and the fused kernel starts with them, so that none is left for the tail
     const bool pass = s_pass[t] != 0u, geo = pass && near == 0u, geo_near = pass && near != 0u;
+    // For the ray caster (raycast.cuh): a voxel can only receive tsdf <= 0 in a visited tile that is NOT wholly in front of
+    // every depth it can see (in front by >= 0.1 mm, mu <= 1 m: every new sample is >= 3 q-units, so the running average of
+    // positive values stays >= 1).  Flag those tiles
+    // and their bricks; flags are only ever set (vol_reset clears them, vol_upload sets all): a conservative superset.
+    if (pass && behind) {
+        p.tile_neg[tile] = 1; p.brick_neg[((ttz / 4) * p.bricks_y + tty / 8) * p.bricks_x + ttx] = 1;
+    }
     const unsigned lane = t & 31, lt = (1u << lane) - 1u;
     const unsigned mg = __ballot_sync(0xffffffffu, geo), mn = __ballot_sync(0xffffffffu, geo_near);
     uint32_t bg = 0, bn = 0;
