@@ -34,7 +34,11 @@ def build(force: bool = False) -> str:
 class RefVol(ctypes.Structure):
     _fields_ = [("nx", ctypes.c_int32), ("ny", ctypes.c_int32), ("nz", ctypes.c_int32), ("r", ctypes.c_int32),
                 ("origin", ctypes.c_float * 3), ("extent", ctypes.c_float), ("mu", ctypes.c_float),
-                ("w_max", ctypes.c_int32), ("sigma", ctypes.c_float), ("gate", ctypes.c_float)]
+                ("w_max", ctypes.c_int32), ("sigma", ctypes.c_float), ("gate", ctypes.c_float), ("variant", ctypes.c_int32)]
+
+
+# alternative readings (ref_fusion.c), one at a time
+VAR_HD_FROM_DEPTH_POINT, VAR_TSDF_ALONG_RAY, VAR_ADDITIVE_WEIGHT = 1, 2, 4
 
 
 class RefFrame(ctypes.Structure):
@@ -73,13 +77,13 @@ def _f32(a, n):
 class RefVolume:
     """Host-side volume pair driven by the oracle.  Same call shapes as the CUDA binding's Volume."""
 
-    def __init__(self, dims_geo, r, origin, extent, mu, w_max, sigma=0.020, gate=0.8, allocate=True):
+    def __init__(self, dims_geo, r, origin, extent, mu, w_max, sigma=0.020, gate=0.8, allocate=True, variant=0):
         self.dims_geo = tuple(int(d) for d in dims_geo)
         self.r = int(r)
         self.dims_col = tuple(d * self.r for d in self.dims_geo)
         self.desc = RefVol(self.dims_geo[0], self.dims_geo[1], self.dims_geo[2], self.r,
                            (ctypes.c_float * 3)(*[float(x) for x in origin]), float(extent), float(mu),
-                           int(w_max), float(sigma), float(gate))
+                           int(w_max), float(sigma), float(gate), int(variant))
         nx, ny, nz = self.dims_geo
         if allocate:
             self.geo = np.zeros((nz, ny, nx), dtype=np.uint32)                     # weight 0 = never observed

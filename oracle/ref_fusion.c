@@ -38,7 +38,16 @@ typedef struct {
     int32_t w_max;           /* geometry weight cap (A5) */
     float   sigma;           /* colour distance gate, metres; 0.020 in the paper (L108) */
     float   gate;            /* weight gate factor; 0.8 in the paper (L115) */
+    int32_t variant;         /* 0 = the readings of DESIGN.md; or ONE of the alternative readings below */
 } ref_vol_t;
+
+/* Alternative readings, one at a time:
+ *   VAR_HD_FROM_DEPTH_POINT  A11 read literally: the HD pixel is located from the depth pixel's 3D point (X_vd, Y_vd, Z_vd)
+ *                            of eq. 7 through eq. 3-4 (L71-81, L115), not from the voxel's own position
+ *   VAR_TSDF_ALONG_RAY       A5: the signed distance is measured along the voxel's viewing ray, (D - Z_vc) * |P_vc| / Z_vc
+ *                            (KinectFusion's metric distance), not along the optical axis
+ *   VAR_ADDITIVE_WEIGHT      A12: W_new = min(W_pre + W, 1) instead of eq. 10 (L122) */
+enum { VAR_HD_FROM_DEPTH_POINT = 1, VAR_TSDF_ALONG_RAY = 2, VAR_ADDITIVE_WEIGHT = 4 };
 
 typedef struct {
     const uint16_t *depth; int32_t wd, hd;      /* depth map D_n, mm, 0 = invalid (L101-103) */
@@ -125,6 +134,10 @@ static int update_geo_voxel(const ref_vol_t *v, const ref_frame_t *f, const cons
     if (d == 0) return 0;                                   /* "if non-zero" (L103) */
     float D = (float)d * 0.001f;                            /* mm -> m (A4) */
     float sdf = D - Z;                                      /* projective signed distance (A5) */
+    if (v->variant == VAR_TSDF_ALONG_RAY) {                 /* ... measured along the viewing ray of the voxel */
+        float nrm = sqrtf(fmaf(Z, Z, fmaf(Y, Y, X * X)));
+        sdf = sdf * (nrm * (1.0f / Z));
+    }
     if (sdf < -v->mu) return 0;                             /* behind the truncation band: unchanged */
     float tsdf = fminf(1.0f, sdf * c->inv_mu);
     int q = (int16_t)(*word & 0xffffu);
@@ -188,6 +201,7 @@ static int update_col_voxel(const ref_vol_t *v, const ref_frame_t *f, const cons
     float W255 = W * 255.0f;
     if (!(W255 > v->gate * (float)wq)) return 1;                                       /* L115, A9 */
     /* HD pixel of the voxel's own position (eq. 3-4; A10, A11) */
+    if (v->variant == VAR_HD_FROM_DEPTH_POINT) { X = Pd[0]; Y = Pd[1]; Z = Pd[2]; }   /* ... or of its depth pixel's point */
     float Xh = fmaf(c->Rc[2], Z, fmaf(c->Rc[1], Y, fmaf(c->Rc[0], X, c->tc[0])));
     float Yh = fmaf(c->Rc[5], Z, fmaf(c->Rc[4], Y, fmaf(c->Rc[3], X, c->tc[1])));
     float Zh = fmaf(c->Rc[8], Z, fmaf(c->Rc[7], Y, fmaf(c->Rc[6], X, c->tc[2])));
@@ -202,6 +216,7 @@ static int update_col_voxel(const ref_vol_t *v, const ref_frame_t *f, const cons
         nw |= (uint32_t)ci << (8 * ch);
     }
     int wn = (int)rintf(fmaf(W, (float)(255 - wq), (float)wq));                        /* eq. 10 (L122), A12 */
+    if (v->variant == VAR_ADDITIVE_WEIGHT) wn = (int)rintf((float)wq + W255);          /* ... or W_pre + W */
     if (wn > 255) wn = 255;
     nw |= (uint32_t)wn << 24;
     *word = nw;                                                                        /* L124 */
@@ -220,6 +235,7 @@ int ref_integrate(const ref_vol_t *v, const ref_frame_t *f, uint32_t *geo, uint3
 {
     if (!v || !f || !geo || !col || !f->depth || !f->rgb) return -1;
     if (v->nx <= 0 || v->ny <= 0 || v->nz <= 0 || v->r < 1 || !(v->mu > 0.0f) || v->w_max < 1 || v->w_max > 512) return -1;
+    if (v->variant != 0 && v->variant != VAR_HD_FROM_DEPTH_POINT && v->variant != VAR_TSDF_ALONG_RAY && v->variant != VAR_ADDITIVE_WEIGHT) return -1;
     consts_t c; frame_consts(v, f, &c);
     uint64_t gr = 0, gc = 0, cr = 0, cc = 0;
 #pragma omp parallel for schedule(static) reduction(+ : gr, gc)
@@ -253,6 +269,7 @@ int ref_integrate_subset(const ref_vol_t *v, const ref_frame_t *f,
 {
     if (!v || !f || !f->depth || !f->rgb) return -1;
     if (v->nx <= 0 || v->ny <= 0 || v->nz <= 0 || v->r < 1 || !(v->mu > 0.0f) || v->w_max < 1 || v->w_max > 512) return -1;
+    if (v->variant != 0 && v->variant != VAR_HD_FROM_DEPTH_POINT && v->variant != VAR_TSDF_ALONG_RAY && v->variant != VAR_ADDITIVE_WEIGHT) return -1;
     consts_t c; frame_consts(v, f, &c);
 #pragma omp parallel for schedule(static)
     for (int64_t n = 0; n < n_geo; ++n) {

@@ -41,7 +41,10 @@ def backproject(x, y, D, K):
 
 
 class BruteVolume:
-    def __init__(self, dims_geo, r, origin, extent, mu, w_max, sigma=0.020, gate=0.8):
+    def __init__(self, dims_geo, r, origin, extent, mu, w_max, sigma=0.020, gate=0.8, variant=0):
+        # variant: 0, or one alternative reading: 1 = HD pixel from the depth pixel's 3D point,
+        # 2 = signed distance along the voxel's viewing ray, 4 = additive colour weight
+        self.variant = int(variant)
         self.dims_geo, self.r = tuple(dims_geo), int(r)
         self.dims_col = tuple(d * r for d in dims_geo)
         self.origin = np.asarray(origin, np.float64)
@@ -72,6 +75,8 @@ class BruteVolume:
         x, y, inside, frag = project(Pc, Kd, wd, hd)
         D = Dm[y, x]
         sdf = D - Pc[..., 2]
+        if self.variant == 2:                                            # metric distance along the ray through the voxel
+            sdf = sdf * np.linalg.norm(Pc, axis=-1) / np.where(Pc[..., 2] > 0, Pc[..., 2], 1.0)
         upd = inside & (D > 0) & (sdf >= -self.mu)
         frag = frag | (inside & (D > 0) & (np.abs(sdf + self.mu) < EPS_M))
         tsdf = np.minimum(1.0, sdf / self.mu)
@@ -101,7 +106,7 @@ class BruteVolume:
         W255 = W * 255.0
         passg = read & (W255 > self.gate * self.wq)                      # L115, A9
         frag = frag | (read & (np.abs(W255 - self.gate * self.wq) < EPS_W))
-        Ph = P @ Thd[:3, :3].T + Thd[:3, 3]                              # eq. 3 (A11: the voxel's own position)
+        Ph = (Pd if self.variant == 1 else P) @ Thd[:3, :3].T + Thd[:3, 3]    # eq. 3 (A11: the voxel's own position; variant 1: eq. 7's point)
         xh, yh, inside_h, frag_h = project(Ph, Kh, wh, hh)               # eq. 4
         upd = passg & inside_h                                           # A13
         frag = frag | (passg & frag_h)
@@ -110,6 +115,8 @@ class BruteVolume:
         Cn = (self.C * wqf[..., None] + W255[..., None] * HD) / np.where(upd, wqf + W255, 1.0)[..., None]   # eq. 9
         Cn = np.clip(np.rint(Cn), 0, 255).astype(np.int64)
         wn_real = wqf + W * (255.0 - wqf)                                # eq. 10 on the 0..255 scale (A12)
+        if self.variant == 4:
+            wn_real = wqf + W255                                         # W_pre + W
         frag = frag | (upd & (np.abs(wn_real - np.floor(wn_real) - 0.5) < EPS_W))
         wn = np.minimum(255, np.rint(wn_real)).astype(np.int64)
         self.C = np.where(upd[..., None], Cn, self.C)
