@@ -37,7 +37,7 @@ extern "C" {
 #endif
 
 #define VOL_OK       0
-#define VOL_E_ARG   -1   /* null pointer, dims <= 0, dims_geo[0] % 4 != 0, dims_geo > 4096 x 2048 x 2048 (per shard), r not in 1..4, mu <= 0, w_max not in 1..512,
+#define VOL_E_ARG   -1   /* null pointer, dims <= 0, dims_geo[0] % 4 != 0, dims_geo > 4096 x 2048 x 2048 (per shard), r not in 1..4, mu <= 0, unknown or combined variant, w_max not in 1..512,
                             non-zero skew, non-rigid T, image size <= 0, buffer too small, bad shard */
 #define VOL_E_OOM   -2   /* device allocation failed */
 #define VOL_E_CUDA  -3   /* a CUDA call failed (sticky: see vol_strerror) */
@@ -47,6 +47,18 @@ extern "C" {
 #define VOL_SLAB 8
 
 typedef struct vol vol_t;   /* opaque; owns (or borrows) the two device buffers */
+
+/* Alternative readings of passages the paper leaves open: each is the same
+ * per-frame path with one step read differently, selected per volume at vol_create (vol_opts_t.variant); combinations
+ * are rejected (VOL_E_ARG).
+ *   VOL_VARIANT_HD_FROM_DEPTH_POINT  PAPER.md L115 read with eq. 2-4 (L71-81) literally: the HD pixel of a colour voxel is
+ *                                    located from the 3D point of its depth pixel (eq. 7), not from the voxel's own position
+ *   VOL_VARIANT_TSDF_ALONG_RAY       L33-35: the signed distance is measured along the voxel's viewing ray,
+ *                                    (D - Z_vc) |P_vc| / Z_vc, not along the optical axis
+ *   VOL_VARIANT_ADDITIVE_WEIGHT      W_new = min(W_pre + W, 1) instead of eq. 10 (L122) */
+#define VOL_VARIANT_HD_FROM_DEPTH_POINT 1
+#define VOL_VARIANT_TSDF_ALONG_RAY      2
+#define VOL_VARIANT_ADDITIVE_WEIGHT     4
 
 typedef struct {
     float   sigma_m;        /* colour distance gate sigma, metres; <= 0 selects the paper's 0.020 */
@@ -58,6 +70,7 @@ typedef struct {
     int32_t device;         /* CUDA device ordinal; < 0 = current device */
     int32_t shard_rank;     /* multi-GPU z-slab sharding; rank 0 of world 1 = whole volume */
     int32_t shard_world;    /* <= 0 is read as 1 */
+    int32_t variant;        /* 0 = the method as DESIGN.md reads it, or ONE of VOL_VARIANT_* below */
 } vol_opts_t;
 
 typedef struct {
@@ -67,7 +80,7 @@ typedef struct {
     int32_t  local_nz_geo;  /* geometry layers stored by this shard (== dims_geo[2] when unsharded) */
     float    voxel_geo_m, voxel_col_m;
     float    origin_m[3], extent_m, trunc_mu_m, sigma_m, gate;
-    int32_t  w_max, device, shard_rank, shard_world;
+    int32_t  w_max, device, shard_rank, shard_world, variant;
     uint64_t geo_bytes, col_bytes;      /* bytes stored by this shard */
     void    *geo_dev, *col_dev;         /* DEVICE pointers of this shard's storage */
 } vol_info_t;

@@ -44,7 +44,11 @@ def build(force: bool = False, verbose: bool = False) -> str:
 class VolOpts(ctypes.Structure):
     _fields_ = [("sigma_m", ctypes.c_float), ("gate", ctypes.c_float), ("geo_dev", ctypes.c_void_p),
                 ("col_dev", ctypes.c_void_p), ("device", ctypes.c_int32), ("shard_rank", ctypes.c_int32),
-                ("shard_world", ctypes.c_int32)]
+                ("shard_world", ctypes.c_int32), ("variant", ctypes.c_int32)]
+
+
+# vol_opts_t.variant: alternative readings of the method (volfusion.h), one at a time
+VARIANT_HD_FROM_DEPTH_POINT, VARIANT_TSDF_ALONG_RAY, VARIANT_ADDITIVE_WEIGHT = 1, 2, 4
 
 
 class VolInfo(ctypes.Structure):
@@ -53,7 +57,7 @@ class VolInfo(ctypes.Structure):
                 ("origin_m", ctypes.c_float * 3), ("extent_m", ctypes.c_float), ("trunc_mu_m", ctypes.c_float),
                 ("sigma_m", ctypes.c_float), ("gate", ctypes.c_float), ("w_max", ctypes.c_int32),
                 ("device", ctypes.c_int32), ("shard_rank", ctypes.c_int32), ("shard_world", ctypes.c_int32),
-                ("geo_bytes", ctypes.c_uint64), ("col_bytes", ctypes.c_uint64), ("geo_dev", ctypes.c_void_p),
+                ("variant", ctypes.c_int32), ("geo_bytes", ctypes.c_uint64), ("col_bytes", ctypes.c_uint64), ("geo_dev", ctypes.c_void_p),
                 ("col_dev", ctypes.c_void_p)]
 
 
@@ -153,11 +157,11 @@ class Volume:
     """A geometry (TSDF) volume and its asymmetrical colour volume on one GPU (or one z-slab shard of them)."""
 
     def __init__(self, dims_geo, r, origin, extent, mu, w_max, sigma=0.0, gate=0.0, device=-1, shard_rank=0,
-                 shard_world=1, geo_dev=None, col_dev=None):
+                 shard_world=1, geo_dev=None, col_dev=None, variant=0):
         self._h = ctypes.c_void_p()
         dims = (ctypes.c_int32 * 3)(*[int(d) for d in dims_geo])
         org = (ctypes.c_float * 3)(*[float(x) for x in origin])
-        opts = VolOpts(float(sigma), float(gate), geo_dev, col_dev, int(device), int(shard_rank), int(shard_world))
+        opts = VolOpts(float(sigma), float(gate), geo_dev, col_dev, int(device), int(shard_rank), int(shard_world), int(variant))
         rc = lib().vol_create(ctypes.byref(self._h), dims, int(r), org, float(extent), float(mu), int(w_max), ctypes.byref(opts))
         if rc != VOL_OK:
             self._h = ctypes.c_void_p()

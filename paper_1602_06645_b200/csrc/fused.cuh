@@ -28,7 +28,9 @@ __device__ __noinline__ uint32_t geo_voxel_ref(const Params &p, float X, float Y
     const uint32_t d = __ldg(p.depth + y * p.wd + x);
     if (d == 0u) return word;                                             // "if non-zero" (L103)
     const float D = __fmul_rn((float)d, 0.001f);
-    const float sdf = __fsub_rn(D, Z);
+    float sdf = __fsub_rn(D, Z);
+    if (p.variant == VAR_TSDF_ALONG_RAY)                                  // measured along the voxel's viewing ray
+        sdf = __fmul_rn(sdf, __fmul_rn(__fsqrt_rn(__fmaf_rn(Z, Z, __fmaf_rn(Y, Y, __fmul_rn(X, X)))), __fdiv_rn(1.0f, Z)));
     if (sdf < p.neg_mu) return word;                                      // behind the truncation band: unchanged
     read = true;
     const float tsdf = fminf(1.0f, __fmul_rn(sdf, p.inv_mu));
@@ -40,16 +42,18 @@ __device__ __noinline__ uint32_t geo_voxel_ref(const Params &p, float X, float Y
     return ((uint32_t)qn & 0xffffu) | ((uint32_t)wn << 16);
 }
 
-// sigma gate of one colour voxel (eq. 6-8 via the pixel map, L101-110).  Returns the view weight W (> 0) or 0.
-__device__ __noinline__ float col_voxel_gate_ref(const Params &p, float X, float Y, float Z)
+// sigma gate of one colour voxel (eq. 6-8 via the pixel map, L101-110).  Returns the pixel-map entry of its depth pixel
+// (eq. 7's point; w = the view weight W > 0) if the voxel passes, w = 0 otherwise.
+__device__ __noinline__ float4 col_voxel_gate_ref(const Params &p, float X, float Y, float Z)
 {
     int x, y;
-    if (!project_px(p.fx, p.fy, p.cx, p.cy, p.wd_f, p.hd_f, X, Y, Z, x, y)) return 0.0f;
+    const float4 none = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+    if (!project_px(p.fx, p.fy, p.cx, p.cy, p.wd_f, p.hd_f, X, Y, Z, x, y)) return none;
     const float4 pm = __ldg(p.pixmap + y * p.wd + x);
-    if (!(pm.w > 0.0f)) return 0.0f;
+    if (!(pm.w > 0.0f)) return none;
     const float dx = __fsub_rn(X, pm.x), dy = __fsub_rn(Y, pm.y), dz = __fsub_rn(Z, pm.z);
     const float d2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
-    return d2 > p.sig2 ? 0.0f : pm.w;
+    return d2 > p.sig2 ? none : pm;
 }
 
 // ---------------------------------------------------------------------------------------------------------------
@@ -74,9 +78,9 @@ __device__ __forceinline__ void project_fast(float fx, float fy, float cx, float
 
 // the same without the final select: off is only meaningful when ok
 __device__ __forceinline__ void project_fast_raw(float fx, float fy, float cx, float cy, uint32_t w, uint32_t wbits, uint32_t hbits, uint32_t koff,
-                                                 float X, float Y, float Z, bool &ok, uint32_t &off)
+                                                 float X, float Y, float Z, bool &ok, uint32_t &off, float &iz)
 {
-    const float iz = rcp_exact(Z);
+    iz = rcp_exact(Z);
     const float u = __fmaf_rn(fx, __fmul_rn(X, iz), cx);
     const float v = __fmaf_rn(fy, __fmul_rn(Y, iz), cy);
     const float tu = __fadd_rn(u, 0.5f), tv = __fadd_rn(v, 0.5f);
@@ -99,7 +103,7 @@ struct Counts { unsigned long long gr, gc, cr, cc; };
 // NEAR tiles (may hold voxels with Z <= 0 or outside rcp_exact's range) take the plain per-voxel routine.
 // Otherwise the layers are software-pipelined: while layer z is updated, layer z + 1 has already been projected and its
 // four depth gathers and its voxel vector are in flight.
-template <bool COUNT>
+template <bool COUNT, int VAR>
 __device__ __forceinline__ void geometry_tile(const Params &p, uint32_t item, int lane, Counts &c)
 {
     const bool near = (item & ITEM_NEAR) != 0u;
@@ -149,14 +153,17 @@ __device__ __forceinline__ void geometry_tile(const Params &p, uint32_t item, in
     // S2 of one layer: eq. 5 z term, projection, and the four depth gathers (offset 0 when outside: a valid address)
     // A voxel outside the frustum keeps d = 0 ("invalid depth": not updated); its gather is predicated off.  The address is
     // one mad.wide (FMA pipe) instead of a 64-bit add pair: the ALU pipe is the busiest one in this loop.
-    auto project_layer = [&](int z, float (&Z)[4], uint32_t (&d)[4]) {
+    // (VAR_TSDF_ALONG_RAY only: L = |P_vc| / Z_vc, the factor from the distance along z to the distance along the ray)
+    auto project_layer = [&](int z, float (&Z)[4], uint32_t (&d)[4], float (&L)[4]) {
         const float pz = __fmaf_rn((float)(gz0 + z) + 0.5f, p.vs, p.oz);
 #pragma unroll
         for (int e = 0; e < 4; ++e) {
             const float X = __fmaf_rn(r02, pz, bX[e]), Y = __fmaf_rn(r12, pz, bY[e]);
             Z[e] = __fmaf_rn(r22, pz, bZ[e]);
-            bool ok; uint32_t off;
-            project_fast_raw(fx, fy, cx, cy, wd, wbits, hbits, koff, X, Y, Z[e], ok, off);
+            bool ok; uint32_t off; float iz;
+            project_fast_raw(fx, fy, cx, cy, wd, wbits, hbits, koff, X, Y, Z[e], ok, off, iz);
+            if (VAR == VAR_TSDF_ALONG_RAY)
+                L[e] = __fmul_rn(__fsqrt_rn(__fmaf_rn(Z[e], Z[e], __fmaf_rn(Y, Y, __fmul_rn(X, X)))), iz);
             d[e] = 0u;
             if (ok) {
                 unsigned long long addr;
@@ -166,7 +173,7 @@ __device__ __forceinline__ void geometry_tile(const Params &p, uint32_t item, in
         }
     };
     // S3 of one layer: truncation test, running average, store if a word changed
-    auto update_layer = [&](uint4 *ptr, const uint4 &cur, const float (&Z)[4], const uint32_t (&d)[4]) {
+    auto update_layer = [&](uint4 *ptr, const uint4 &cur, const float (&Z)[4], const uint32_t (&d)[4], const float (&L)[4]) {
         const uint32_t o4[4] = {cur.x, cur.y, cur.z, cur.w};
         uint32_t w4[4];
         float sdf[4]; bool upd[4];
@@ -175,6 +182,7 @@ __device__ __forceinline__ void geometry_tile(const Params &p, uint32_t item, in
         for (int e = 0; e < 4; ++e) {
             const float D = __fmul_rn((float)d[e], 0.001f);
             sdf[e] = __fsub_rn(D, Z[e]);
+            if (VAR == VAR_TSDF_ALONG_RAY) sdf[e] = __fmul_rn(sdf[e], L[e]);
             upd[e] = (d[e] != 0u) & !(sdf[e] < neg_mu);
             // saturated free space (tsdf = 1 onto q = 32767) or first touch (w = 0): the running average is 32767 exactly,
             // fma(32767, w, 32767) / (w + 1) with every intermediate below 2^24.  (Bitwise on purpose: no branches.)
@@ -211,19 +219,19 @@ __device__ __forceinline__ void geometry_tile(const Params &p, uint32_t item, in
     };
     // Two register sets, A (even layers) and B (odd layers), used alternately: the pipeline needs no register-to-register
     // rotation, which would make the warp wait for the loads it has just issued.
-    float ZA[4], ZB[4]; uint32_t dA[4], dB[4];
+    float ZA[4], ZB[4], LA[4], LB[4]; uint32_t dA[4], dB[4];
     // the voxel stream bypasses L1 (__ldcg): every line is used once, and L1 is better spent on the depth image
     uint4 curA = __ldcg(ptr), curB = curA;
-    project_layer(0, ZA, dA);
+    project_layer(0, ZA, dA, LA);
     for (int z = 0; z < nl; z += 2) {
         uint4 *pB = reinterpret_cast<uint4 *>(reinterpret_cast<uint32_t *>(ptr) + layer);
         uint4 *pA2 = reinterpret_cast<uint4 *>(reinterpret_cast<uint32_t *>(pB) + layer);
         const bool hasB = z + 1 < nl, hasA2 = z + 2 < nl;
-        if (hasB) { curB = __ldcg(pB); project_layer(z + 1, ZB, dB); }               // layer z + 1 in flight
-        update_layer(ptr, curA, ZA, dA);
+        if (hasB) { curB = __ldcg(pB); project_layer(z + 1, ZB, dB, LB); }               // layer z + 1 in flight
+        update_layer(ptr, curA, ZA, dA, LA);
         if (hasB) {
-            if (hasA2) { curA = __ldcg(pA2); project_layer(z + 2, ZA, dA); }         // layer z + 2 in flight
-            update_layer(pB, curB, ZB, dB);
+            if (hasA2) { curA = __ldcg(pA2); project_layer(z + 2, ZA, dA, LA); }         // layer z + 2 in flight
+            update_layer(pB, curB, ZB, dB, LB);
         }
         ptr = pA2;
     }
@@ -245,7 +253,8 @@ __device__ __forceinline__ void geometry_prefetch(const Params &p, uint32_t item
 // longer.  Passing voxels are therefore compacted here and updated 32 at a time with every lane busy.
 constexpr int STAGE_CAP = 160;            // up to 31 carried over + 128 of one cell
 struct Stage {
-    float4 rec[STAGE_CAP];                // {X, Y, Z} = voxel centre in the depth camera (eq. 5), W = view weight of its pixel
+    float4 rec[STAGE_CAP];                // {X, Y, Z} = voxel centre in the depth camera (eq. 5) -- or, VAR_HD_FROM_DEPTH_POINT, the
+                                          // 3D point of its depth pixel (eq. 7); W = view weight of its pixel
     uint2  adr[STAGE_CAP];                // word index of the voxel in this shard's colour volume (lo, hi)
 };
 
@@ -253,7 +262,7 @@ struct Stage {
 // lane.  The HD pixel (eq. 3-4) is computed and its three bytes requested BEFORE the stored word arrives: the two gathers do
 // not depend on each other, so their latencies overlap instead of adding up (the word is a DRAM access, and one warp
 // works through its stage round after round).  A voxel that then fails the weight gate has fetched 3 bytes in vain.
-template <bool COUNT>
+template <bool COUNT, int VAR>
 __device__ __forceinline__ void colour_update_staged(const Params &p, const Stage &st, int first, int n, int lane, Counts &c)
 {
     if (lane < n) {
@@ -284,7 +293,8 @@ __device__ __forceinline__ void colour_update_staged(const Params &p, const Stag
                 const int ci = cn < 0.0f ? 0 : (cn > 255.0f ? 255 : (int)cn);
                 nw |= (uint32_t)ci << (8 * ch);
             }
-            int wn = __float2int_rn(__fmaf_rn(W, (float)(255 - wq), (float)wq)); // eq. 10, A12
+            int wn = VAR == VAR_ADDITIVE_WEIGHT ? __float2int_rn(__fadd_rn((float)wq, W255))          // W_pre + W
+                                                : __float2int_rn(__fmaf_rn(W, (float)(255 - wq), (float)wq)); // eq. 10, A12
             nw |= (uint32_t)min(wn, 255) << 24;
             if (nw != old) *ptr = nw;
         }
@@ -296,7 +306,7 @@ __device__ __forceinline__ void colour_update_staged(const Params &p, const Stag
 // x-adjacent voxels.  (ic0, jc, kcg) = the lane's first voxel in the full colour grid, kcl = its layer in this shard.
 // Voxels that pass the gate are appended to the warp's stage (n = its fill level, warp-uniform); full groups of 32 are
 // updated at once.
-template <bool COUNT>
+template <bool COUNT, int VAR>
 __device__ __forceinline__ void colour_cell(const Params &p, bool near, int ic0, int jc, int kcg, int kcl, Stage &st, int &n, int lane, Counts &c)
 {
     const float fx = p.fx, fy = p.fy, cx_ = p.cx, cy_ = p.cy, sig2 = p.sig2;
@@ -314,15 +324,16 @@ __device__ __forceinline__ void colour_cell(const Params &p, bool near, int ic0,
         Z[e] = __fmaf_rn(p.R[8], pz, __fmaf_rn(p.R[7], py, __fmaf_rn(p.R[6], px, p.t[2])));
     }
     unsigned pass = 0;
+    float4 pm[4];
     if (near) {
 #pragma unroll
         for (int e = 0; e < 4; ++e) {
-            W[e] = act ? col_voxel_gate_ref(p, X[e], Y[e], Z[e]) : 0.0f;
+            pm[e] = act ? col_voxel_gate_ref(p, X[e], Y[e], Z[e]) : make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+            W[e] = pm[e].w;
             if (W[e] > 0.0f) pass |= 1u << e;
         }
     } else {
         uint32_t off[4]; bool ok[4];
-        float4 pm[4];
 #pragma unroll
         for (int e = 0; e < 4; ++e) project_fast(fx, fy, cx_, cy_, wd, wbits, hbits, koff, X[e], Y[e], Z[e], ok[e], off[e]);   // eq. 6
 #pragma unroll
@@ -350,21 +361,21 @@ __device__ __forceinline__ void colour_cell(const Params &p, bool near, int ic0,
 #pragma unroll
     for (int e = 0; e < 4; ++e)
         if (pass & (1u << e)) {
-            st.rec[slot] = make_float4(X[e], Y[e], Z[e], W[e]);
+            st.rec[slot] = VAR == VAR_HD_FROM_DEPTH_POINT ? make_float4(pm[e].x, pm[e].y, pm[e].z, W[e]) : make_float4(X[e], Y[e], Z[e], W[e]);
             const size_t a = base + (size_t)e;
             st.adr[slot] = make_uint2((uint32_t)a, (uint32_t)(a >> 32));
             ++slot;
         }
     n += total;
     __syncwarp();
-    while (n >= 32) { n -= 32; colour_update_staged<COUNT>(p, st, n, 32, lane, c); }
+    while (n >= 32) { n -= 32; colour_update_staged<COUNT, VAR>(p, st, n, 32, lane, c); }
     __syncwarp();
 }
 
 // one colour work item, one warp: the set bits of one nibble of a shell-mark word are up to 4 colour cells of one tile.
 // The ticket of the next item is drawn before the LAST cell: its latency is hidden, yet no item waits reserved behind a
 // long one.
-template <int R, bool COUNT>
+template <int R, bool COUNT, int VAR>
 __device__ __forceinline__ void colour_item(const Params &p, uint32_t item, Stage &st, int &n, int lane, Counts &c, uint32_t *cursor, uint32_t &ticket)
 {
     const bool near = (item & ITEM_NEAR) != 0u;
@@ -389,7 +400,7 @@ __device__ __forceinline__ void colour_item(const Params &p, uint32_t item, Stag
         if (bits == 0u) next_ticket(cursor, lane, ticket);
         const int cx = b % CX, cy = (b / CX) % CY, cz = b / (CX * CY);
         const int kz = cz * CLZ + (lane >> 3);
-        colour_cell<COUNT>(p, near, cgx0 + cx * CLX + 4 * (lane & 1), cgy0 + cy * CLY + ((lane >> 1) & 3), cgz0 + kz, clz0 + kz, st, n, lane, c);
+        colour_cell<COUNT, VAR>(p, near, cgx0 + cx * CLX + 4 * (lane & 1), cgy0 + cy * CLY + ((lane >> 1) & 3), cgz0 + kz, clz0 + kz, st, n, lane, c);
     }
 }
 
@@ -398,7 +409,7 @@ __device__ __forceinline__ void colour_item(const Params &p, uint32_t item, Stag
 // copied (only the colour update reads it).
 enum { PHASE_ALL = 0, PHASE_GEO = 1, PHASE_COL = 2 };
 
-template <int R, bool COUNT>
+template <int R, bool COUNT, int VAR>
 __global__ void __launch_bounds__(CTA, 4) k_fused(const __grid_constant__ Params p, int phase)
 {
     __shared__ Stage s_stage[WARPS_PER_CTA];
@@ -422,14 +433,14 @@ __global__ void __launch_bounds__(CTA, 4) k_fused(const __grid_constant__ Params
         if (it >= n_items) break;
         const uint32_t item = it < n_near ? __ldcg(p.work_geo + ((uint32_t)p.n_tiles - 1u - it))
                                           : (it < n_col ? __ldcg(p.work_col + (it - n_near)) : __ldcg(p.work_geo + (it - n_col)));
-        if (it >= n_near && it < n_col) colour_item<R, COUNT>(p, item, st, n_staged, lane, c, cursor, ticket);
+        if (it >= n_near && it < n_col) colour_item<R, COUNT, VAR>(p, item, st, n_staged, lane, c, cursor, ticket);
         else {
             next_ticket(cursor, lane, ticket);
             geometry_prefetch(p, item, lane);
-            geometry_tile<COUNT>(p, item, lane, c);
+            geometry_tile<COUNT, VAR>(p, item, lane, c);
         }
     }
-    if (n_staged > 0) colour_update_staged<COUNT>(p, st, 0, n_staged, lane, c);
+    if (n_staged > 0) colour_update_staged<COUNT, VAR>(p, st, 0, n_staged, lane, c);
     if (COUNT) {
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) {

@@ -21,6 +21,10 @@ constexpr int BRICK = 32;                                   // ray-casting skip 
 constexpr int WARPS_PER_CTA = 8;
 constexpr int CTA = 32 * WARPS_PER_CTA;
 
+// alternative readings of the method (volfusion.h VOL_VARIANT_*), one at a time: a template
+// parameter of the fused kernel, so the default reading's code is unchanged
+enum { VAR_PAPER = 0, VAR_HD_FROM_DEPTH_POINT = 1, VAR_TSDF_ALONG_RAY = 2, VAR_ADDITIVE_WEIGHT = 4 };
+
 // cells of one tile's colour children per axis, and 32-bit mark words per tile, for ratio r
 __host__ __device__ constexpr int cells_x(int r) { return TX * r / CLX; }   // 4r
 __host__ __device__ constexpr int cells_y(int r) { return TY * r / CLY; }   // r
@@ -40,6 +44,7 @@ struct Params {
     float vs, vc;                // geometry / colour voxel size
     float mu, neg_mu, inv_mu, sig2, sigma, gate;
     int   w_max;
+    int   variant;               // VAR_*
     // frame (S0: computed on the host in fp64, rounded once)
     float R[9], t[3];            // (R_n, t_n) of eq. 5: world -> depth camera
     float Rc[9], tc[3];          // (R_calib, t_calib) of eq. 3: depth camera -> HD camera

@@ -61,6 +61,19 @@ static cudaError_t launch(void (*kernel)(const Params, Args...), dim3 grid, int 
     return cudaLaunchKernelEx(&cfg, kernel, p, args...);
 }
 
+// the fused kernel for colour ratio R, with or without the voxel counters, in the volume's reading of the method
+using FusedFn = void (*)(const Params, int);
+template <int R>
+static FusedFn fused_kernel(bool counting, int variant)
+{
+    switch (variant) {
+        case vf::VAR_HD_FROM_DEPTH_POINT: return counting ? vf::k_fused<R, true, vf::VAR_HD_FROM_DEPTH_POINT> : vf::k_fused<R, false, vf::VAR_HD_FROM_DEPTH_POINT>;
+        case vf::VAR_TSDF_ALONG_RAY:      return counting ? vf::k_fused<R, true, vf::VAR_TSDF_ALONG_RAY> : vf::k_fused<R, false, vf::VAR_TSDF_ALONG_RAY>;
+        case vf::VAR_ADDITIVE_WEIGHT:     return counting ? vf::k_fused<R, true, vf::VAR_ADDITIVE_WEIGHT> : vf::k_fused<R, false, vf::VAR_ADDITIVE_WEIGHT>;
+        default:                          return counting ? vf::k_fused<R, true, vf::VAR_PAPER> : vf::k_fused<R, false, vf::VAR_PAPER>;
+    }
+}
+
 static int set_device(const vol *v) { CK(cudaSetDevice(v->device)); return VOL_OK; }
 
 // rigid inverse in fp64 with left-to-right sums, rounded once to fp32 (S0).  Returns false if T is not rigid.
@@ -135,7 +148,11 @@ extern "C" int vol_create(vol_t **out, const int32_t dims_geo[3], int32_t r, con
     if ((int64_t)dims_geo[0] * r > INT32_MAX / 4 || (int64_t)dims_geo[1] * r > INT32_MAX / 4 || (int64_t)dims_geo[2] * r > INT32_MAX / 4) return VOL_E_ARG;
     int rank = 0, world = 1, device = -1;
     float sigma = 0.020f, gate = 0.8f;
+    int variant = 0;
     if (opts) {
+        variant = opts->variant;
+        if (variant != 0 && variant != VOL_VARIANT_HD_FROM_DEPTH_POINT && variant != VOL_VARIANT_TSDF_ALONG_RAY &&
+            variant != VOL_VARIANT_ADDITIVE_WEIGHT) return VOL_E_ARG;
         if (opts->sigma_m > 0.0f) sigma = opts->sigma_m;
         if (opts->gate > 0.0f) gate = opts->gate;
         world = opts->shard_world > 0 ? opts->shard_world : 1;
@@ -172,7 +189,7 @@ extern "C" int vol_create(vol_t **out, const int32_t dims_geo[3], int32_t r, con
     p.vc = p.vs / (float)r;
     p.inv_vc = 1.0f / p.vc;
     p.mu = trunc_mu_m; p.neg_mu = -trunc_mu_m; p.inv_mu = 1.0f / trunc_mu_m;
-    p.sigma = sigma; p.sig2 = sigma * sigma; p.gate = gate; p.w_max = w_max;
+    p.sigma = sigma; p.sig2 = sigma * sigma; p.gate = gate; p.w_max = w_max; p.variant = variant;
     v->geo_bytes = (size_t)local_nz * p.ny * p.nx * 4u;
     v->col_bytes = (size_t)local_nz * r * p.cny * p.cnx * 4u;
 
@@ -212,7 +229,7 @@ extern "C" int vol_create(vol_t **out, const int32_t dims_geo[3], int32_t r, con
     if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) return fail(VOL_E_CUDA);
     v->n_sms = prop.multiProcessorCount;
     int occ = 0;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, vf::k_fused<2, false>, vf::CTA, 0) != cudaSuccess || occ < 1) {
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, vf::k_fused<2, false, 0>, vf::CTA, 0) != cudaSuccess || occ < 1) {
         snprintf(g_err, sizeof g_err, "fused kernel cannot be resident on device %d (built for sm_100a): %s", device, cudaGetErrorString(cudaGetLastError()));
         return fail(VOL_E_CUDA);
     }
@@ -321,20 +338,18 @@ static int integrate_impl(vol_t *v, const uint16_t *depth_u16_dev, int32_t wd, i
     // memory flush with griddepcontrol.wait before touching anything it wrote.
 #define VF_LAUNCH(RR)                                                                   \
     do {                                                                                \
+        const FusedFn kf = fused_kernel<RR>(cnt, p.variant);                            \
         CK(launch(vf::k_prepass<RR>, g0, 256, s, false, p));                            \
         CK(launch(vf::k_mark_classify<RR>, dim3(g1 + gm), 256, s, true, p, g1));        \
         if (v->profiling) CK(cudaEventRecord(v->ev[1], s));                             \
         CK(launch(vf::k_items_col<RR>, dim3(g1), 256, s, true, p));                     \
         if (v->profiling) CK(cudaEventRecord(v->ev[2], s));                             \
         if (rgb_ready) {   /* geometry half now, colour half once the HD frame has arrived */           \
-            if (cnt) CK(launch(vf::k_fused<RR, true>, dim3(g2), vf::CTA, s, true, p, (int)vf::PHASE_GEO));   \
-            else     CK(launch(vf::k_fused<RR, false>, dim3(g2), vf::CTA, s, true, p, (int)vf::PHASE_GEO));  \
+            CK(launch(kf, dim3(g2), vf::CTA, s, true, p, (int)vf::PHASE_GEO));          \
             CK(cudaStreamWaitEvent(s, rgb_ready, 0));                                    \
-            if (cnt) CK(launch(vf::k_fused<RR, true>, dim3(g2), vf::CTA, s, false, p, (int)vf::PHASE_COL));  \
-            else     CK(launch(vf::k_fused<RR, false>, dim3(g2), vf::CTA, s, false, p, (int)vf::PHASE_COL)); \
+            CK(launch(kf, dim3(g2), vf::CTA, s, false, p, (int)vf::PHASE_COL));         \
         } else {                                                                        \
-            if (cnt) CK(launch(vf::k_fused<RR, true>, dim3(g2), vf::CTA, s, true, p, (int)vf::PHASE_ALL));   \
-            else     CK(launch(vf::k_fused<RR, false>, dim3(g2), vf::CTA, s, true, p, (int)vf::PHASE_ALL));  \
+            CK(launch(kf, dim3(g2), vf::CTA, s, true, p, (int)vf::PHASE_ALL));          \
         }                                                                               \
     } while (0)
     switch (p.r) {
@@ -517,7 +532,7 @@ extern "C" int vol_info(const vol_t *v, vol_info_t *o)
     for (int i = 0; i < 3; ++i) o->dims_col[i] = o->dims_geo[i] * p.r;
     o->local_nz_geo = p.local_nz; o->voxel_geo_m = p.vs; o->voxel_col_m = p.vc;
     o->origin_m[0] = p.ox; o->origin_m[1] = p.oy; o->origin_m[2] = p.oz; o->extent_m = p.vs * (float)p.nx;
-    o->trunc_mu_m = p.mu; o->sigma_m = p.sigma; o->gate = p.gate; o->w_max = p.w_max; o->device = v->device;
+    o->trunc_mu_m = p.mu; o->sigma_m = p.sigma; o->gate = p.gate; o->w_max = p.w_max; o->device = v->device; o->variant = p.variant;
     o->shard_rank = p.shard_rank; o->shard_world = p.shard_world;
     o->geo_bytes = v->geo_bytes; o->col_bytes = v->col_bytes; o->geo_dev = p.geo; o->col_dev = p.col;
     return VOL_OK;

@@ -14,8 +14,10 @@ def to_dev(a):
 
 def make_pair(c, **kw):
     import paper_1602_06645_b200 as vf
-    g = vf.Volume(c.dims_geo, c.r, c.origin, c.extent, c.mu, c.w_max, sigma=kw.get("sigma", 0.0), gate=kw.get("gate", 0.0))
-    o = oracle.RefVolume(c.dims_geo, c.r, c.origin, c.extent, c.mu, c.w_max, sigma=kw.get("sigma", 0.020), gate=kw.get("gate", 0.8))
+    g = vf.Volume(c.dims_geo, c.r, c.origin, c.extent, c.mu, c.w_max, sigma=kw.get("sigma", 0.0), gate=kw.get("gate", 0.0),
+                  variant=kw.get("variant", 0))
+    o = oracle.RefVolume(c.dims_geo, c.r, c.origin, c.extent, c.mu, c.w_max, sigma=kw.get("sigma", 0.020), gate=kw.get("gate", 0.8),
+                         variant=kw.get("variant", 0))
     return g, o
 
 
@@ -53,8 +55,8 @@ def check_counters(st, cnt, where=""):
     assert got == [int(x) for x in cnt], f"{where}: counters {got} != oracle {list(cnt)}"
 
 
-def run_sequence(c, frames, counting=True, check_every=1):
-    g, o = make_pair(c)
+def run_sequence(c, frames, counting=True, check_every=1, **kw):
+    g, o = make_pair(c, **kw)
     for n, fi in enumerate(frames):
         depth, rgb, T = synth.frame(c, fi)
         st, cnt = integrate_both(g, o, c, depth, rgb, T, counting)
@@ -63,3 +65,43 @@ def run_sequence(c, frames, counting=True, check_every=1):
         if (n + 1) % check_every == 0 or n == len(frames) - 1:
             compare_states(g, o, f"{c.name} frame {fi}")
     return g, o
+
+
+def sampled_full_size(c, frames, n_cols, seed, alternate_host=False, variant=0):
+    """Full-size volumes in the launch configuration bench.py times (device-resident frames, counters off), compared on a
+    seeded sample: every voxel of n_cols random 8 x 8 (x, y) geometry columns and all their colour children.  Voxels never
+    interact, so the oracle run on the sample alone gives their exact state (ref_integrate_subset)."""
+    import paper_1602_06645_b200 as vf
+    nx, ny, nz = c.dims_geo
+    r = c.r
+    rng = np.random.default_rng(seed)
+    bx, by = rng.integers(0, nx // 8, n_cols), rng.integers(0, ny // 8, n_cols)
+    k = np.arange(nz, dtype=np.int64)[:, None, None, None]
+    j = (by[None, :, None, None] * 8 + np.arange(8)[None, None, :, None]).astype(np.int64)
+    i = (bx[None, :, None, None] * 8 + np.arange(8)[None, None, None, :]).astype(np.int64)
+    geo_idx = np.unique(((k * ny + j) * nx + i).reshape(-1))
+    kc = np.arange(nz * r, dtype=np.int64)[:, None, None, None]
+    jc = (by[None, :, None, None] * 8 * r + np.arange(8 * r)[None, None, :, None]).astype(np.int64)
+    ic = (bx[None, :, None, None] * 8 * r + np.arange(8 * r)[None, None, None, :]).astype(np.int64)
+    col_idx = np.unique(((kc * (ny * r) + jc) * (nx * r) + ic).reshape(-1))
+    gw, cw = np.zeros(geo_idx.size, np.uint32), np.zeros(col_idx.size, np.uint32)
+    o = oracle.RefVolume(c.dims_geo, r, c.origin, c.extent, c.mu, c.w_max, allocate=False, variant=variant)
+    g = vf.Volume(c.dims_geo, r, c.origin, c.extent, c.mu, c.w_max, variant=variant)
+    try:
+        for n, fi in enumerate(frames):
+            depth, rgb, T = synth.frame(c, fi)
+            if alternate_host and n % 2:                          # every other frame through vol_integrate_host
+                g.integrate_host(depth, rgb, T, c.K_depth, c.K_rgb, c.T_depth_rgb)
+            else:
+                g.integrate(to_dev(depth), c.wd, c.hd, to_dev(rgb), c.wh, c.hh, T, c.K_depth, c.K_rgb, c.T_depth_rgb)
+            o.integrate_subset(geo_idx, gw, col_idx, cw, depth, rgb, T, c.K_depth, c.K_rgb, c.T_depth_rgb)
+            if n % 64 == 63:                                      # intermediate states too
+                ggw, gcw = g.download_voxels(geo_idx, col_idx)
+                assert int((ggw != gw).sum()) == 0 and int((gcw != cw).sum()) == 0, f"{c.name}: differs after frame {fi}"
+        ggw, gcw = g.download_voxels(geo_idx, col_idx)
+    finally:
+        g.close()
+    assert (gw >> 16).max() == min(len(frames), c.w_max) and (cw >> 24).max() > 0   # the sample does see the surface
+    assert int((ggw != gw).sum()) == 0, f"{c.name}: {int((ggw != gw).sum())} geometry words differ on the sample"
+    assert int((gcw != cw).sum()) == 0, f"{c.name}: {int((gcw != cw).sum())} colour words differ on the sample"
+    return int((gw != 0).sum()), int((cw != 0).sum())

@@ -4,6 +4,7 @@ import pytest
 
 import synth
 from parity_util import check_counters, compare_states, integrate_both, make_pair, run_sequence, to_dev
+from parity_util import sampled_full_size as _sampled_full_size
 
 pytestmark = pytest.mark.gpu
 I4 = np.eye(4, dtype=np.float32)
@@ -155,47 +156,6 @@ def test_exact_arithmetic_selftest():
     (the exhaustive sweep is `vf.selftest(exhaustive=True)`, ~1e12 quotients)."""
     import paper_1602_06645_b200 as vf
     assert vf.selftest(False) == (0, 0)
-
-
-def _sampled_full_size(c, frames, n_cols, seed, alternate_host=False):
-    """Full-size volumes in the launch configuration bench.py times (device-resident frames, counters off), compared on a
-    seeded sample: every voxel of n_cols random 8 x 8 (x, y) geometry columns and all their colour children.  Voxels never
-    interact, so the oracle run on the sample alone gives their exact state (ref_integrate_subset)."""
-    import oracle
-    import paper_1602_06645_b200 as vf
-    nx, ny, nz = c.dims_geo
-    r = c.r
-    rng = np.random.default_rng(seed)
-    bx, by = rng.integers(0, nx // 8, n_cols), rng.integers(0, ny // 8, n_cols)
-    k = np.arange(nz, dtype=np.int64)[:, None, None, None]
-    j = (by[None, :, None, None] * 8 + np.arange(8)[None, None, :, None]).astype(np.int64)
-    i = (bx[None, :, None, None] * 8 + np.arange(8)[None, None, None, :]).astype(np.int64)
-    geo_idx = np.unique(((k * ny + j) * nx + i).reshape(-1))
-    kc = np.arange(nz * r, dtype=np.int64)[:, None, None, None]
-    jc = (by[None, :, None, None] * 8 * r + np.arange(8 * r)[None, None, :, None]).astype(np.int64)
-    ic = (bx[None, :, None, None] * 8 * r + np.arange(8 * r)[None, None, None, :]).astype(np.int64)
-    col_idx = np.unique(((kc * (ny * r) + jc) * (nx * r) + ic).reshape(-1))
-    gw, cw = np.zeros(geo_idx.size, np.uint32), np.zeros(col_idx.size, np.uint32)
-    o = oracle.RefVolume(c.dims_geo, r, c.origin, c.extent, c.mu, c.w_max, allocate=False)
-    g = vf.Volume(c.dims_geo, r, c.origin, c.extent, c.mu, c.w_max)
-    try:
-        for n, fi in enumerate(frames):
-            depth, rgb, T = synth.frame(c, fi)
-            if alternate_host and n % 2:                          # every other frame through vol_integrate_host
-                g.integrate_host(depth, rgb, T, c.K_depth, c.K_rgb, c.T_depth_rgb)
-            else:
-                g.integrate(to_dev(depth), c.wd, c.hd, to_dev(rgb), c.wh, c.hh, T, c.K_depth, c.K_rgb, c.T_depth_rgb)
-            o.integrate_subset(geo_idx, gw, col_idx, cw, depth, rgb, T, c.K_depth, c.K_rgb, c.T_depth_rgb)
-            if n % 64 == 63:                                      # intermediate states too
-                ggw, gcw = g.download_voxels(geo_idx, col_idx)
-                assert int((ggw != gw).sum()) == 0 and int((gcw != cw).sum()) == 0, f"{c.name}: differs after frame {fi}"
-        ggw, gcw = g.download_voxels(geo_idx, col_idx)
-    finally:
-        g.close()
-    assert (gw >> 16).max() == min(len(frames), c.w_max) and (cw >> 24).max() > 0   # the sample does see the surface
-    assert int((ggw != gw).sum()) == 0, f"{c.name}: {int((ggw != gw).sum())} geometry words differ on the sample"
-    assert int((gcw != cw).sum()) == 0, f"{c.name}: {int((gcw != cw).sum())} colour words differ on the sample"
-    return int((gw != 0).sum()), int((cw != 0).sum())
 
 
 def test_cfg3_full_size_whole_sequence_sampled():
