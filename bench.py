@@ -46,6 +46,8 @@ def parse():
     ap.add_argument("--no-flush", action="store_true", help="time frames back to back without flushing L2")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--first-frame", type=int, default=0)
+    ap.add_argument("--variant", type=int, default=0, choices=[0, 1, 2, 4],
+                    help="alternative reading of the method (vol_opts_t.variant; both arms); 0 = the headline path")
     ap.add_argument("--stress", action="store_true",
                     help="second workload: the saturating frame of SURVEY 8(d) item 5 (every geometry voxel updated) instead of the scan")
     return ap.parse_args()
@@ -149,8 +151,9 @@ class NvmlClocks:
 
 
 def workload_name(c):
+    var = getattr(c, "variant", 0)
     return (f"{c.name}: geometry {c.dims_geo[0]}^3 over {c.extent} m, colour {c.dims_col[0]}^3 (r={c.r}), depth {c.wd}x{c.hd}, "
-            f"rgb {c.wh}x{c.hh}")
+            f"rgb {c.wh}x{c.hh}" + (f" -- alternative reading {var} (vol_opts_t.variant)" if var else ""))
 
 
 def oracle_sample(c, n_frames, slab_layers=None):
@@ -169,7 +172,7 @@ def oracle_sample(c, n_frames, slab_layers=None):
     else:
         dims = (nx, ny, nz)
         sample = f"full volumes, first {n_frames} frames"
-    o = oracle.RefVolume(dims, c.r, origin, c.extent, c.mu, c.w_max, sigma=c.sigma, gate=c.gate)
+    o = oracle.RefVolume(dims, c.r, origin, c.extent, c.mu, c.w_max, sigma=c.sigma, gate=c.gate, variant=getattr(c, "variant", 0))
     o.desc.extent = float(np.float32(c.voxel) * np.float32(nx))
     nvox = dims[0] * dims[1] * dims[2] * (1 + c.r ** 3)
     times = []
@@ -190,6 +193,7 @@ def run_reference(args, rank):
     if rank != 0:
         return
     c = synth.config(args.cfg, r=args.r)
+    c.variant = args.variant
     cores = os.cpu_count() or 1
     slab = max(8, c.dims_geo[2] // 16)
     nvox, times, sample = oracle_sample(c, args.warmup + args.steps, slab_layers=slab)
@@ -234,6 +238,7 @@ def run_ours(args, rank, world, local_rank):
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
     c = synth.config(args.cfg, r=args.r)
+    c.variant = args.variant
     W, K = args.warmup, args.steps
     nfr = W + K
     first = args.first_frame + 7 * rank                       # replicas scan different parts of the trajectory
@@ -247,7 +252,8 @@ def run_ours(args, rank, world, local_rank):
         depth, rgb, T = synth.stress_frame(c, i) if args.stress else synth.frame(c, (first + i) % c.n_frames)
         hd_, hr_ = torch.from_numpy(depth.view(np.int16)).pin_memory(), torch.from_numpy(rgb).pin_memory()
         frames.append((hd_, hr_, hd_.cuda(), hr_.cuda(), T))
-    vol = vf.Volume(c.dims_geo, c.r, c.origin, c.extent, c.mu, c.w_max, sigma=c.sigma, gate=c.gate, device=local_rank)
+    vol = vf.Volume(c.dims_geo, c.r, c.origin, c.extent, c.mu, c.w_max, sigma=c.sigma, gate=c.gate, device=local_rank,
+                    variant=getattr(c, "variant", 0))
     stream = torch.cuda.current_stream()
     flush_buf = torch.empty(512 << 20, dtype=torch.uint8, device="cuda")      # > 126 MB L2
 
@@ -378,6 +384,8 @@ def run_ours(args, rank, world, local_rank):
     fused_ms = kms[:, 2]
     peak, peak_src = peaks()
     achieved = float(alg_bytes.sum() / (fused_ms.sum() * 1e-3) / 1e9)
+    # profiles/traffic.csv holds captures of the headline path only: other readings report traffic = null
+    traffic_key = c.name + ("-stress" if args.stress else "") + (f"-variant{args.variant}" if args.variant else "")
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
         "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -394,9 +402,9 @@ def run_ours(args, rank, world, local_rank):
                            "col_changed": float(cnt[:, 3].mean()), "tiles_geo": float(cnt[:, 4].mean()), "items_col": float(cnt[:, 5].mean()),
                            "cells_col": float(cnt[:, 6].mean()), "algorithmic_bytes": float(alg_bytes.mean())},
         "roofline": {"bound": "hbm", "kernel": "k_fused", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                     "traffic": ncu_traffic(c.name + ("-stress" if args.stress else "")), "peak_source": peak_src,
+                     "traffic": ncu_traffic(traffic_key), "peak_source": peak_src,
                      "dense_sweep_frac": float(8.0 * nvox / (fused_ms.mean() * 1e-3) / 1e9 / peak),
-                     "issue": issue_roofline(c.name + ("-stress" if args.stress else ""), float(fused_ms.mean()),
+                     "issue": issue_roofline(traffic_key, float(fused_ms.mean()),
                                              (clocks or {}).get("sm_mhz"))},
         "e2e": {"value": e2e_value, "unit": UNIT, "ms_per_step": e2e_ms / K, "h2d_bytes_per_step": frame_bytes,
                 "d2h_bytes_per_step": 64},

@@ -13,14 +13,14 @@ import synth
 pytestmark = pytest.mark.gpu
 
 
-def fidelity(r, vga):
+def fidelity(r, vga, variant=0, depth_error=False):
     import torch
     import paper_1602_06645_b200 as vf
     c = synth.config(5, r=r)
     if vga:                                             # the Kinect's own RGB camera instead of the HD camera
         c = dataclasses.replace(c)
         c.wh, c.hh, c.K_rgb = 640, 480, synth.intrinsics(525.0, 319.5, 239.5)
-    g = vf.Volume(c.dims_geo, c.r, c.origin, c.extent, c.mu, c.w_max)
+    g = vf.Volume(c.dims_geo, c.r, c.origin, c.extent, c.mu, c.w_max, variant=variant)
     for fi in range(0, 400, 4):
         d, rgb, T = synth.frame(c, fi)
         g.integrate(torch.from_numpy(d.view(np.int16)).cuda(), c.wd, c.hd, torch.from_numpy(rgb).cuda(), c.wh, c.hh, T,
@@ -39,6 +39,8 @@ def fidelity(r, vga):
     m = (depth > 0) & (gtz > 0) & (img.sum(axis=2) > 0)
     for _ in range(3):                                  # stay 3 px away from silhouettes and holes
         m[1:-1, 1:-1] &= m[:-2, 1:-1] & m[2:, 1:-1] & m[1:-1, :-2] & m[1:-1, 2:]
+    if depth_error:                                     # RMS error of the ray-cast surface against the analytic one, mm
+        return 1e3 * float(np.sqrt(((depth - gtz) ** 2)[m].mean())), int(m.sum())
     mse = ((img - gt.astype(np.float64)) ** 2)[m].mean()
     return 10.0 * np.log10(255.0 ** 2 / mse), int(m.sum())
 
@@ -51,3 +53,23 @@ def test_asymmetric_hd_volume_keeps_more_texture():
     assert min(n0, n1, n2) > 300000
     assert p_r1_vga < p_r1_hd < p_r2_hd
     assert p_r2_hd - p_r1_vga > 1.0
+
+
+def test_alternative_readings_on_the_same_scene():
+    """SURVEY 8(f) rank 2(b)-(d) on the turntable scene, r = 2 with the HD frame.  (b) Locating the HD pixel from the depth
+    pixel's point gives all colour voxels behind one depth pixel the same HD sample: the asymmetrical volume then holds no
+    more detail than the depth map's sampling, and the PSNR falls back towards the symmetric volume's -- the reason for
+    reading A11.  (d) The additive weight saturates one frame earlier than eq. 10 and ends within a fraction of a dB.
+    (c) The signed distance along the ray moves the fused surface by well under a voxel (1.95 mm)."""
+    import paper_1602_06645_b200 as vf
+    p_def, n = fidelity(2, False)
+    p_lit, n1 = fidelity(2, False, vf.VARIANT_HD_FROM_DEPTH_POINT)
+    p_add, n2 = fidelity(2, False, vf.VARIANT_ADDITIVE_WEIGHT)
+    e_def, _ = fidelity(2, False, 0, depth_error=True)
+    e_ray, n3 = fidelity(2, False, vf.VARIANT_TSDF_ALONG_RAY, depth_error=True)
+    print(f"PSNR r=2 HD: default {p_def:.2f} dB, HD pixel from depth point {p_lit:.2f} dB, additive weight {p_add:.2f} dB; "
+          f"surface RMS error: default {e_def:.3f} mm, along-ray TSDF {e_ray:.3f} mm over {n3} px")
+    assert min(n, n1, n2, n3) > 300000
+    assert p_lit < p_def - 0.3
+    assert abs(p_add - p_def) < 1.0
+    assert e_def < 2.0 and e_ray < 2.0
