@@ -113,8 +113,10 @@ int vol_integrate(vol_t *v, const uint16_t *depth_u16_dev, int32_t wd, int32_t h
                   const float T_world_depth[16], const float K_depth[9], const float K_rgb[9],
                   const float T_depth_rgb[16], void *stream);
 
-/* Same, with HOST frame buffers (ideally pinned): copies both images to library-owned device staging buffers on
- * `stream`, then runs vol_integrate on them.  The host buffers may be reused once the stream has passed the copies. */
+/* Same, with HOST frame buffers (ideally pinned): copies both images to library-owned device staging buffers, then runs
+ * vol_integrate on them, all ordered on `stream`.  The copies use a stream of the library's own and two staging sets, so
+ * frames enqueued back to back overlap: the images of frame n + 1 travel while the kernels of frame n run.  The host
+ * buffers may be reused once `stream` has passed this call's work. */
 int vol_integrate_host(vol_t *v, const uint16_t *depth_u16_host, int32_t wd, int32_t hd,
                        const uint8_t *rgb8_host, int32_t wh, int32_t hh,
                        const float T_world_depth[16], const float K_depth[9], const float K_rgb[9],
@@ -154,8 +156,13 @@ int vol_info(const vol_t *v, vol_info_t *out);
 int vol_shard_layers(int32_t nz, int32_t shard_rank, int32_t shard_world, int32_t *layers_out, int32_t cap);
 /* Enable (1) / disable (0) the four voxel counters of vol_stats_t (a separately compiled kernel variant). */
 int vol_set_counting(vol_t *v, int32_t on);
-/* Statistics of the last frame (synchronises `stream`; copies 48 bytes device -> host). */
+/* Statistics of the last frame (synchronises `stream`; copies 64 bytes device -> host). */
 int vol_frame_stats(vol_t *v, vol_stats_t *out, void *stream);
+/* The same without the synchronisation, for callers that enqueue frames back to back: copies the 64-byte raw record of the
+ * frame last enqueued on `stream` to raw_host (HOST, pinned, 8-byte aligned, >= 64 bytes), asynchronously, in stream order;
+ * once the stream has passed it, vol_stats_decode (host only, no CUDA call) turns it into a vol_stats_t. */
+int vol_frame_stats_async(vol_t *v, void *raw_host, void *stream);
+int vol_stats_decode(const vol_t *v, const void *raw_host, vol_stats_t *out);
 /* Enable per-kernel CUDA-event timing of subsequent vol_integrate calls / read the last frame's kernel times in
  * milliseconds: ms[0] pre-pass, shell marks and geometry tile classification (S1, S9), ms[1] colour work items (S9), ms[2] fused integrate (S2-S8).  Synchronises. */
 int vol_set_profiling(vol_t *v, int32_t on);

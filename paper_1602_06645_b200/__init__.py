@@ -26,7 +26,7 @@ NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", 
               "-Xcompiler", "-fPIC,-ffp-contract=off", "-shared"]
 
 EXPORTS = ["vol_create", "vol_integrate", "vol_integrate_host", "vol_raycast", "vol_sample_colour", "vol_download", "vol_download_voxels", "vol_upload",
-           "vol_reset", "vol_info", "vol_shard_layers", "vol_set_counting", "vol_frame_stats", "vol_set_profiling", "vol_last_kernel_ms",
+           "vol_reset", "vol_info", "vol_shard_layers", "vol_set_counting", "vol_frame_stats", "vol_frame_stats_async", "vol_stats_decode", "vol_set_profiling", "vol_last_kernel_ms",
            "vol_launches_per_frame", "vol_selftest", "vol_destroy", "vol_strerror"]
 
 
@@ -87,6 +87,8 @@ def lib():
         L.vol_shard_layers.argtypes = [I32, I32, I32, P, I32]
         L.vol_set_counting.argtypes = [P, I32]
         L.vol_frame_stats.argtypes = [P, P, P]
+        L.vol_frame_stats_async.argtypes = [P, P, P]
+        L.vol_stats_decode.argtypes = [P, P, P]
         L.vol_set_profiling.argtypes = [P, I32]
         L.vol_last_kernel_ms.argtypes = [P, P]
         L.vol_launches_per_frame.argtypes = [P]
@@ -238,6 +240,17 @@ class Volume:
     def frame_stats(self, stream=None) -> VolStats:
         s = VolStats()
         _check(lib().vol_frame_stats(self._h, ctypes.byref(s), _stream_ptr(stream)), "vol_frame_stats")
+        return s
+
+    def frame_stats_async(self, raw_host, stream=None):
+        """vol_frame_stats_async: raw_host = pinned CPU tensor of >= 64 bytes; filled in stream order, no synchronisation."""
+        assert not raw_host.is_cuda and raw_host.is_pinned() and raw_host.numel() * raw_host.element_size() >= 64
+        _check(lib().vol_frame_stats_async(self._h, raw_host.data_ptr(), _stream_ptr(stream)), "vol_frame_stats_async")
+
+    def decode_stats(self, raw_host) -> VolStats:
+        """vol_stats_decode of a record written by frame_stats_async (after the stream has passed it)."""
+        s = VolStats()
+        _check(lib().vol_stats_decode(self._h, raw_host.data_ptr(), ctypes.byref(s)), "vol_stats_decode")
         return s
 
     def set_profiling(self, on: bool):

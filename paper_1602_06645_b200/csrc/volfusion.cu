@@ -36,16 +36,20 @@ struct vol {
     int scratch_wd, scratch_hd;
     size_t pyr_entries;
     // staging for vol_integrate_host
-    uint16_t *stage_depth; size_t stage_depth_bytes;
-    uint8_t *stage_rgb; size_t stage_rgb_bytes;
+    // staging for vol_integrate_host: two sets used alternately, so that the copies of one frame overlap the kernels of the
+    // frame before it (ev_used[i]: the kernels that last read set i have finished)
+    uint16_t *stage_depth[2]; size_t stage_depth_bytes;
+    uint8_t *stage_rgb[2]; size_t stage_rgb_bytes;
+    cudaEvent_t ev_depth[2], ev_rgb[2], ev_used[2];
+    bool used_valid[2];
+    unsigned host_seq;
     // fused-kernel launch shape
     int n_sms, fused_blocks;
     bool counting, profiling;
     cudaEvent_t ev[4];
     bool ev_valid;
-    // vol_integrate_host: the HD frame is copied on a stream of the library's own while the depth-only kernels run
+    // vol_integrate_host: the frames are copied on a stream of the library's own
     cudaStream_t copy_stream;
-    cudaEvent_t ev_fork, ev_rgb;
 };
 
 // one kernel launch; `dependent` = programmatic dependent launch on the previous kernel of the stream
@@ -236,8 +240,10 @@ extern "C" int vol_create(vol_t **out, const int32_t dims_geo[3], int32_t r, con
     v->fused_blocks = v->n_sms * occ;
     for (int i = 0; i < 4; ++i) if (cudaEventCreate(&v->ev[i]) != cudaSuccess) return fail(VOL_E_CUDA);
     if (cudaStreamCreateWithFlags(&v->copy_stream, cudaStreamNonBlocking) != cudaSuccess) return fail(VOL_E_CUDA);
-    if (cudaEventCreateWithFlags(&v->ev_fork, cudaEventDisableTiming) != cudaSuccess) return fail(VOL_E_CUDA);
-    if (cudaEventCreateWithFlags(&v->ev_rgb, cudaEventDisableTiming) != cudaSuccess) return fail(VOL_E_CUDA);
+    for (int i = 0; i < 2; ++i)
+        if (cudaEventCreateWithFlags(&v->ev_depth[i], cudaEventDisableTiming) != cudaSuccess ||
+            cudaEventCreateWithFlags(&v->ev_rgb[i], cudaEventDisableTiming) != cudaSuccess ||
+            cudaEventCreateWithFlags(&v->ev_used[i], cudaEventDisableTiming) != cudaSuccess) return fail(VOL_E_CUDA);
     v->ev_valid = false;
     if (cudaDeviceSynchronize() != cudaSuccess) return fail(VOL_E_CUDA);
     *out = v;
@@ -261,11 +267,14 @@ extern "C" void vol_destroy(vol_t *v)
     if (v->p.pixmap) cudaFree(v->p.pixmap);
     if (v->p.pyr) cudaFree(v->p.pyr);
     if (v->p.jobs) cudaFree(v->p.jobs);
-    if (v->stage_depth) cudaFree(v->stage_depth);
-    if (v->stage_rgb) cudaFree(v->stage_rgb);
+    for (int i = 0; i < 2; ++i) {
+        if (v->stage_depth[i]) cudaFree(v->stage_depth[i]);
+        if (v->stage_rgb[i]) cudaFree(v->stage_rgb[i]);
+        if (v->ev_depth[i]) cudaEventDestroy(v->ev_depth[i]);
+        if (v->ev_rgb[i]) cudaEventDestroy(v->ev_rgb[i]);
+        if (v->ev_used[i]) cudaEventDestroy(v->ev_used[i]);
+    }
     for (int i = 0; i < 4; ++i) if (v->ev[i]) cudaEventDestroy(v->ev[i]);
-    if (v->ev_fork) cudaEventDestroy(v->ev_fork);
-    if (v->ev_rgb) cudaEventDestroy(v->ev_rgb);
     if (v->copy_stream) cudaStreamDestroy(v->copy_stream);
     cudaGetLastError();
     delete v;
@@ -297,10 +306,12 @@ static int ensure_scratch(vol *v, int wd, int hd)
     return VOL_OK;
 }
 
-// rgb_ready: optional event the fused kernel (the only reader of the HD frame) has to wait for
+// rgb_ready: optional event the colour update (the only reader of the HD frame) has to wait for.  split: run the geometry
+// half of the fused kernel before that wait and the colour half after it (worth it when the HD frame is still on its way);
+// otherwise the stream waits first and the whole queue goes in one launch.
 static int integrate_impl(vol_t *v, const uint16_t *depth_u16_dev, int32_t wd, int32_t hd, const uint8_t *rgb8_dev,
                           int32_t wh, int32_t hh, const float T_world_depth[16], const float K_depth[9],
-                          const float K_rgb[9], const float T_depth_rgb[16], void *stream, cudaEvent_t rgb_ready)
+                          const float K_rgb[9], const float T_depth_rgb[16], void *stream, cudaEvent_t rgb_ready, bool split)
 {
     if (!v || !depth_u16_dev || !rgb8_dev || !T_world_depth || !K_depth || !K_rgb || !T_depth_rgb) return VOL_E_ARG;
     if (wd <= 0 || hd <= 0 || wh <= 0 || hh <= 0 || wd > 16384 || hd > 16384 || wh > 16384 || hh > 16384) return VOL_E_ARG;
@@ -328,6 +339,7 @@ static int integrate_impl(vol_t *v, const uint16_t *depth_u16_dev, int32_t wd, i
     if (p.n_tiles == 0) return VOL_OK;
 
     cudaStream_t s = (cudaStream_t)stream;
+    if (rgb_ready && !split) { CK(cudaStreamWaitEvent(s, rgb_ready, 0)); rgb_ready = nullptr; }
     if (v->counting) CK(cudaMemsetAsync(p.counters, 0, sizeof(unsigned long long) * 4, s));
     if (v->profiling) CK(cudaEventRecord(v->ev[0], s));
     const dim3 g0((wd + 31) / 32, (hd + 31) / 32);
@@ -368,7 +380,7 @@ extern "C" int vol_integrate(vol_t *v, const uint16_t *depth_u16_dev, int32_t wd
                              int32_t wh, int32_t hh, const float T_world_depth[16], const float K_depth[9],
                              const float K_rgb[9], const float T_depth_rgb[16], void *stream)
 {
-    return integrate_impl(v, depth_u16_dev, wd, hd, rgb8_dev, wh, hh, T_world_depth, K_depth, K_rgb, T_depth_rgb, stream, nullptr);
+    return integrate_impl(v, depth_u16_dev, wd, hd, rgb8_dev, wh, hh, T_world_depth, K_depth, K_rgb, T_depth_rgb, stream, nullptr, false);
 }
 
 extern "C" int vol_integrate_host(vol_t *v, const uint16_t *depth_u16_host, int32_t wd, int32_t hd, const uint8_t *rgb8_host,
@@ -382,23 +394,40 @@ extern "C" int vol_integrate_host(vol_t *v, const uint16_t *depth_u16_host, int3
     if (!rigid_inverse(T_world_depth, Rt, tt) || !rigid_inverse(T_depth_rgb, Rt, tt)) return VOL_E_ARG;
     int rc = set_device(v); if (rc) return rc;
     const size_t db = (size_t)wd * hd * sizeof(uint16_t), cb = (size_t)wh * hh * 3;
-    if (v->stage_depth_bytes < db) {
-        if (v->stage_depth) { CK(cudaDeviceSynchronize()); cudaFree(v->stage_depth); v->stage_depth = nullptr; v->stage_depth_bytes = 0; }
-        CK(cudaMalloc(&v->stage_depth, db)); v->stage_depth_bytes = db;
-    }
-    if (v->stage_rgb_bytes < cb) {
-        if (v->stage_rgb) { CK(cudaDeviceSynchronize()); cudaFree(v->stage_rgb); v->stage_rgb = nullptr; v->stage_rgb_bytes = 0; }
-        CK(cudaMalloc(&v->stage_rgb, cb)); v->stage_rgb_bytes = cb;
+    if (v->stage_depth_bytes < db || v->stage_rgb_bytes < cb) {            // (re)allocate both sets
+        CK(cudaDeviceSynchronize());
+        const size_t nd = db > v->stage_depth_bytes ? db : v->stage_depth_bytes, nc = cb > v->stage_rgb_bytes ? cb : v->stage_rgb_bytes;
+        for (int i = 0; i < 2; ++i) {
+            if (v->stage_depth[i]) cudaFree(v->stage_depth[i]);
+            if (v->stage_rgb[i]) cudaFree(v->stage_rgb[i]);
+            v->stage_depth[i] = nullptr; v->stage_rgb[i] = nullptr; v->used_valid[i] = false;
+        }
+        v->stage_depth_bytes = v->stage_rgb_bytes = 0;
+        for (int i = 0; i < 2; ++i) { CK(cudaMalloc(&v->stage_depth[i], nd)); CK(cudaMalloc(&v->stage_rgb[i], nc)); }
+        v->stage_depth_bytes = nd; v->stage_rgb_bytes = nc;
     }
     cudaStream_t s = (cudaStream_t)stream;
-    CK(cudaMemcpyAsync(v->stage_depth, depth_u16_host, db, cudaMemcpyHostToDevice, s));
-    // fork: the HD frame (91 % of the bytes) goes over the library's copy stream, ordered after everything already queued
-    // on `stream` (the previous frame's fused kernel still reads the staging buffer); only the fused kernel waits for it
-    CK(cudaEventRecord(v->ev_fork, s));
-    CK(cudaStreamWaitEvent(v->copy_stream, v->ev_fork, 0));
-    CK(cudaMemcpyAsync(v->stage_rgb, rgb8_host, cb, cudaMemcpyHostToDevice, v->copy_stream));
-    CK(cudaEventRecord(v->ev_rgb, v->copy_stream));
-    return integrate_impl(v, v->stage_depth, wd, hd, v->stage_rgb, wh, hh, T_world_depth, K_depth, K_rgb, T_depth_rgb, stream, v->ev_rgb);
+    const int set = (int)(v->host_seq++ & 1u);
+    // Both images go over the library's copy stream into staging set `set`, ordered only after the kernels that last read
+    // that set (two frames ago) -- so they overlap the previous frame's kernels when the caller enqueues frames back to back.
+    if (v->used_valid[set]) CK(cudaStreamWaitEvent(v->copy_stream, v->ev_used[set], 0));
+    CK(cudaMemcpyAsync(v->stage_depth[set], depth_u16_host, db, cudaMemcpyHostToDevice, v->copy_stream));
+    CK(cudaEventRecord(v->ev_depth[set], v->copy_stream));
+    CK(cudaMemcpyAsync(v->stage_rgb[set], rgb8_host, cb, cudaMemcpyHostToDevice, v->copy_stream));
+    CK(cudaEventRecord(v->ev_rgb[set], v->copy_stream));
+    // Is the previous frame still being worked on?  Then this frame's HD image (91 % of the bytes) will have arrived by the
+    // time its kernels start, and the whole queue goes in one launch.  Otherwise (the caller waits for every frame) the
+    // geometry half runs while the HD image is still on its way and only the colour half waits for it.
+    const bool busy = v->used_valid[set ^ 1] && cudaEventQuery(v->ev_used[set ^ 1]) == cudaErrorNotReady;
+    cudaGetLastError();
+    CK(cudaStreamWaitEvent(s, v->ev_depth[set], 0));
+    rc = integrate_impl(v, v->stage_depth[set], wd, hd, v->stage_rgb[set], wh, hh, T_world_depth, K_depth, K_rgb, T_depth_rgb, stream,
+                        v->ev_rgb[set], !busy);
+    if (rc) return rc;
+    CK(cudaStreamWaitEvent(s, v->ev_rgb[set], 0));             // (already passed, except on a shard without tiles)
+    CK(cudaEventRecord(v->ev_used[set], s));
+    v->used_valid[set] = true;
+    return VOL_OK;
 }
 
 extern "C" int vol_raycast(const vol_t *v, int32_t w, int32_t h, const float T_world_cam[16], const float K[9], float t_near_m,
@@ -551,15 +580,22 @@ extern "C" int vol_set_counting(vol_t *v, int32_t on) { if (!v) return VOL_E_ARG
 extern "C" int vol_set_profiling(vol_t *v, int32_t on) { if (!v) return VOL_E_ARG; v->profiling = on != 0; v->ev_valid = false; return VOL_OK; }
 extern "C" int vol_launches_per_frame(const vol_t *v) { return v ? 4 : VOL_E_ARG; }
 
-extern "C" int vol_frame_stats(vol_t *v, vol_stats_t *out, void *stream)
+extern "C" int vol_frame_stats_async(vol_t *v, void *raw_host, void *stream)
 {
-    if (!v || !out) return VOL_E_ARG;
+    if (!v || !raw_host) return VOL_E_ARG;
     int rc = set_device(v); if (rc) return rc;
     cudaStream_t s = (cudaStream_t)stream;
+    static_assert(sizeof(uint32_t) * vf::CTRL_N == 32, "raw statistics record: 8 control words, then 4 counters");
+    CK(cudaMemcpyAsync(raw_host, v->p.ctrl, 32, cudaMemcpyDeviceToHost, s));
+    CK(cudaMemcpyAsync((char *)raw_host + 32, v->p.counters, 32, cudaMemcpyDeviceToHost, s));
+    return VOL_OK;
+}
+
+extern "C" int vol_stats_decode(const vol_t *v, const void *raw_host, vol_stats_t *out)
+{
+    if (!v || !raw_host || !out) return VOL_E_ARG;
     uint32_t ctrl[vf::CTRL_N]; unsigned long long cnt[4];
-    CK(cudaMemcpyAsync(ctrl, v->p.ctrl, sizeof ctrl, cudaMemcpyDeviceToHost, s));
-    CK(cudaMemcpyAsync(cnt, v->p.counters, sizeof cnt, cudaMemcpyDeviceToHost, s));
-    CK(cudaStreamSynchronize(s));
+    memcpy(ctrl, raw_host, 32); memcpy(cnt, (const char *)raw_host + 32, 32);
     memset(out, 0, sizeof *out);
     if (v->counting) { out->geo_read = cnt[0]; out->geo_changed = cnt[1]; out->col_read = cnt[2]; out->col_changed = cnt[3]; }
     out->tiles_total = (uint32_t)v->p.n_tiles;
@@ -567,6 +603,15 @@ extern "C" int vol_frame_stats(vol_t *v, vol_stats_t *out, void *stream)
     out->items_col = ctrl[vf::CTRL_NCOL];
     out->cells_col = v->counting ? ctrl[vf::CTRL_CELLS] : 0u;
     return VOL_OK;
+}
+
+extern "C" int vol_frame_stats(vol_t *v, vol_stats_t *out, void *stream)
+{
+    if (!v || !out) return VOL_E_ARG;
+    unsigned long long raw[8];
+    int rc = vol_frame_stats_async(v, raw, stream); if (rc) return rc;
+    CK(cudaStreamSynchronize((cudaStream_t)stream));
+    return vol_stats_decode(v, raw, out);
 }
 
 extern "C" int vol_last_kernel_ms(vol_t *v, float ms[3])

@@ -109,6 +109,41 @@ def test_host_entry_point_and_upload_roundtrip():
     assert np.array_equal(gw, geo.reshape(-1)[gi]) and np.array_equal(cw, col.reshape(-1)[ci])
 
 
+def test_host_frames_enqueued_back_to_back():
+    """vol_integrate_host without any synchronisation between frames: the copies of frame n + 1 (pinned host memory, the
+    library's copy stream, two staging sets) overlap the kernels of frame n.  16 frames of config 3's noisy orbit on a
+    non-default stream, statistics read back with vol_frame_stats_async; the final state and every frame's record must
+    equal the one-frame-at-a-time run's, and the oracle's."""
+    import torch
+    c = synth.config(3).scaled(160, 2)
+    frames = [synth.frame(c, fi) for fi in range(0, 160, 10)]
+    pinned = [(torch.from_numpy(d.copy()).pin_memory(), torch.from_numpy(rgb.copy()).pin_memory(), T) for d, rgb, T in frames]
+    g, o = make_pair(c)
+    g.set_counting(True)
+    serial = []
+    for d, rgb, T in frames:
+        g.integrate_host(d, rgb, T, c.K_depth, c.K_rgb, c.T_depth_rgb)
+        st = g.frame_stats()
+        serial.append((st.geo_read, st.geo_changed, st.col_read, st.col_changed, st.tiles_geo, st.items_col, st.cells_col))
+        cnt = o.integrate(d, rgb, T, c.K_depth, c.K_rgb, c.T_depth_rgb)
+        check_counters(st, cnt)
+    compare_states(g, o, "one frame at a time")
+    stream = torch.cuda.Stream()
+    raw = torch.zeros((len(frames), 8), dtype=torch.int64).pin_memory()
+    for rep in range(3):                                            # three times: whichever way the copies and kernels interleave
+        g.reset(stream)
+        for n, (d, rgb, T) in enumerate(pinned):
+            g.integrate_host(d, rgb, T, c.K_depth, c.K_rgb, c.T_depth_rgb, stream=stream)
+            g.frame_stats_async(raw[n], stream)
+        stream.synchronize()
+        got = []
+        for n in range(len(frames)):
+            st = g.decode_stats(raw[n])
+            got.append((st.geo_read, st.geo_changed, st.col_read, st.col_changed, st.tiles_geo, st.items_col, st.cells_col))
+        assert got == serial, f"repeat {rep}"
+        compare_states(g, o, f"back to back, repeat {rep}")
+
+
 def test_shards_reassemble_to_the_unsharded_volume():
     """z-slab sharding (VOL_SLAB layers dealt round-robin): two shards run one after the other on this GPU hold exactly
     the slabs of the unsharded result; no voxel is owned twice or dropped."""
