@@ -62,6 +62,8 @@ def _load():
         lib.ref_frame_constants.argtypes = [P, P, P]
         lib.ref_sample_colour.restype = ctypes.c_int
         lib.ref_sample_colour.argtypes = [P, P, P, ctypes.c_int64, P]
+        lib.ref_sample_colour_trilinear.restype = ctypes.c_int
+        lib.ref_sample_colour_trilinear.argtypes = [P, P, P, ctypes.c_int64, P]
         lib.ref_raycast.restype = ctypes.c_int
         lib.ref_raycast.argtypes = [P, P, P, ctypes.c_int32, ctypes.c_int32, P, P, ctypes.c_float, ctypes.c_float, P, P]
         _lib = lib
@@ -134,6 +136,15 @@ class RefVolume:
         rc = _load().ref_sample_colour(ctypes.addressof(self.desc), self.col.ctypes.data, pts.ctypes.data, pts.shape[0], out.ctypes.data)
         if rc != 0:
             raise ValueError("ref_sample_colour: bad arguments")
+        return out
+
+    def sample_colour_trilinear(self, pts):
+        """ref_sample_colour_trilinear: trilinearly interpolated colour words (uint32 [n]) at the world points pts [n, 3]."""
+        pts = np.ascontiguousarray(pts, dtype=np.float32).reshape(-1, 3)
+        out = np.zeros(pts.shape[0], dtype=np.uint32)
+        rc = _load().ref_sample_colour_trilinear(ctypes.addressof(self.desc), self.col.ctypes.data, pts.ctypes.data, pts.shape[0], out.ctypes.data)
+        if rc != 0:
+            raise ValueError("ref_sample_colour_trilinear: bad arguments")
         return out
 
     def raycast(self, w, h, T_world_cam, K, t_near, t_far):

@@ -394,3 +394,61 @@ int ref_sample_colour(const ref_vol_t *v, const uint32_t *col, const float *pts,
     }
     return 0;
 }
+
+/* ref_sample_colour_trilinear -- the same lookup with trilinear interpolation (second half).
+ * Reading S2 (the paper does not say how the volume is accessed; nearest voxel = S1 above): voxel centres sit at
+ * (idx + 0.5) * vc (A1), so the continuous grid coordinate of a point is g = (p - origin) / vc - 0.5 per axis; with
+ * b = floor(g) and f = g - b, the 8 voxels b + {0,1}^3 carry the weights (1-f or f) per axis, multiplied as (wz * wy) * wx.
+ * A voxel outside the volume or never observed (wq = 0) holds no colour: it contributes nothing, and the colour is
+ * normalised over the voxels that do --  C = rint(sum w C / sum w)  per channel (half-even).  The weight byte is the plain
+ * trilinear interpolation of the stored weights with unobserved voxels counted as 0:  A = rint(sum w wq)  -- so A tells how
+ * much of the footprint has been seen.  No observed voxel in the footprint (or a non-finite point): word 0.
+ * Canonical binary32, neighbours accumulated in the order z-major, then y, then x (dz, dy, dx = 0,0,0; 0,0,1; 0,1,0; ...),
+ * each sum as fmaf(w, value, sum). */
+int ref_sample_colour_trilinear(const ref_vol_t *v, const uint32_t *col, const float *pts, int64_t n, uint32_t *words_out)
+{
+    if (!v || !col || (n > 0 && (!pts || !words_out)) || n < 0) return -1;
+    const float vc = (v->extent / (float)v->nx) / (float)v->r, inv_vc = 1.0f / vc;
+    const int cn[3] = { v->nx * v->r, v->ny * v->r, v->nz * v->r };
+#pragma omp parallel for schedule(static)
+    for (int64_t m = 0; m < n; ++m) {
+        float b[3], f[3];
+        int ok = 1;
+        for (int a = 0; a < 3; ++a) {
+            const float g = (pts[3 * m + a] - v->origin[a]) * inv_vc - 0.5f;
+            b[a] = floorf(g);
+            f[a] = g - b[a];
+            /* the footprint must touch the volume: b in [-1, cn - 1]; also rejects NaN and infinities */
+            if (!(b[a] >= -1.0f && b[a] <= (float)(cn[a] - 1))) ok = 0;
+        }
+        uint32_t word = 0;
+        if (ok) {
+            float sw = 0.0f, sa = 0.0f, sc[3] = { 0.0f, 0.0f, 0.0f };
+            for (int dz = 0; dz < 2; ++dz)
+                for (int dy = 0; dy < 2; ++dy)
+                    for (int dx = 0; dx < 2; ++dx) {
+                        const int i = (int)b[0] + dx, j = (int)b[1] + dy, k = (int)b[2] + dz;
+                        if (i < 0 || i >= cn[0] || j < 0 || j >= cn[1] || k < 0 || k >= cn[2]) continue;
+                        const uint32_t cw = col[((size_t)k * (size_t)cn[1] + (size_t)j) * (size_t)cn[0] + (size_t)i];
+                        if ((cw >> 24) == 0) continue;
+                        const float wx = dx ? f[0] : 1.0f - f[0], wy = dy ? f[1] : 1.0f - f[1], wz = dz ? f[2] : 1.0f - f[2];
+                        const float w = (wz * wy) * wx;
+                        sw = sw + w;
+                        sa = fmaf(w, (float)(cw >> 24), sa);
+                        for (int ch = 0; ch < 3; ++ch) sc[ch] = fmaf(w, (float)((cw >> (8 * ch)) & 0xffu), sc[ch]);
+                    }
+            if (sw > 0.0f) {
+                for (int ch = 0; ch < 3; ++ch) {
+                    float cq = rintf(sc[ch] / sw);
+                    int ci = cq < 0.0f ? 0 : (cq > 255.0f ? 255 : (int)cq);
+                    word |= (uint32_t)ci << (8 * ch);
+                }
+                float aq = rintf(sa);
+                int ai = aq < 0.0f ? 0 : (aq > 255.0f ? 255 : (int)aq);
+                word |= (uint32_t)ai << 24;
+            }
+        }
+        words_out[m] = word;
+    }
+    return 0;
+}

@@ -27,6 +27,8 @@ static char g_err[256] = "";
         }                                                                                                \
     } while (0)
 
+constexpr int N_STAGE = 2;          // staging sets of vol_integrate_host
+
 struct vol {
     Params p;                       // volume fields filled at create; frame fields per call
     int device;
@@ -38,10 +40,10 @@ struct vol {
     // staging for vol_integrate_host
     // staging for vol_integrate_host: two sets used alternately, so that the copies of one frame overlap the kernels of the
     // frame before it (ev_used[i]: the kernels that last read set i have finished)
-    uint16_t *stage_depth[2]; size_t stage_depth_bytes;
-    uint8_t *stage_rgb[2]; size_t stage_rgb_bytes;
-    cudaEvent_t ev_depth[2], ev_rgb[2], ev_used[2];
-    bool used_valid[2];
+    uint16_t *stage_depth[N_STAGE]; size_t stage_depth_bytes;
+    uint8_t *stage_rgb[N_STAGE]; size_t stage_rgb_bytes;
+    cudaEvent_t ev_depth[N_STAGE], ev_rgb[N_STAGE], ev_used[N_STAGE];
+    bool used_valid[N_STAGE];
     unsigned host_seq;
     // fused-kernel launch shape
     int n_sms, fused_blocks;
@@ -223,10 +225,11 @@ extern "C" int vol_create(vol_t **out, const int32_t dims_geo[3], int32_t r, con
     if (cudaMalloc(&p.brick_neg, nb) != cudaSuccess) rc = VOL_E_OOM;
     if (rc == VOL_OK && cudaMemset(p.brick_neg, 0, nb) != cudaSuccess) rc = VOL_E_CUDA;
     if (rc == VOL_OK && cudaMemset(p.marks, 0, sizeof(uint32_t) * nw) != cudaSuccess) rc = VOL_E_CUDA;
-    if (cudaMalloc(&p.ctrl, sizeof(uint32_t) * vf::CTRL_N) != cudaSuccess) rc = VOL_E_OOM;
-    if (cudaMalloc(&p.counters, sizeof(unsigned long long) * 4) != cudaSuccess) rc = VOL_E_OOM;
-    if (rc == VOL_OK && cudaMemset(p.ctrl, 0, sizeof(uint32_t) * vf::CTRL_N) != cudaSuccess) rc = VOL_E_CUDA;
-    if (rc == VOL_OK && cudaMemset(p.counters, 0, sizeof(unsigned long long) * 4) != cudaSuccess) rc = VOL_E_CUDA;
+    // one 64-byte record: the 8 control words, then the 4 voxel counters (read back together by vol_frame_stats*)
+    static_assert(sizeof(uint32_t) * vf::CTRL_N == 32, "raw statistics record: 8 control words, then 4 counters");
+    if (cudaMalloc(&p.ctrl, 64) != cudaSuccess) rc = VOL_E_OOM;
+    if (rc == VOL_OK) p.counters = reinterpret_cast<unsigned long long *>(p.ctrl + vf::CTRL_N);
+    if (rc == VOL_OK && cudaMemset(p.ctrl, 0, 64) != cudaSuccess) rc = VOL_E_CUDA;
     if (rc != VOL_OK) { cudaGetLastError(); return fail(rc); }
 
     cudaDeviceProp prop;
@@ -240,7 +243,7 @@ extern "C" int vol_create(vol_t **out, const int32_t dims_geo[3], int32_t r, con
     v->fused_blocks = v->n_sms * occ;
     for (int i = 0; i < 4; ++i) if (cudaEventCreate(&v->ev[i]) != cudaSuccess) return fail(VOL_E_CUDA);
     if (cudaStreamCreateWithFlags(&v->copy_stream, cudaStreamNonBlocking) != cudaSuccess) return fail(VOL_E_CUDA);
-    for (int i = 0; i < 2; ++i)
+    for (int i = 0; i < N_STAGE; ++i)
         if (cudaEventCreateWithFlags(&v->ev_depth[i], cudaEventDisableTiming) != cudaSuccess ||
             cudaEventCreateWithFlags(&v->ev_rgb[i], cudaEventDisableTiming) != cudaSuccess ||
             cudaEventCreateWithFlags(&v->ev_used[i], cudaEventDisableTiming) != cudaSuccess) return fail(VOL_E_CUDA);
@@ -263,11 +266,10 @@ extern "C" void vol_destroy(vol_t *v)
     if (v->p.tile_neg) cudaFree(v->p.tile_neg);
     if (v->p.brick_neg) cudaFree(v->p.brick_neg);
     if (v->p.ctrl) cudaFree(v->p.ctrl);
-    if (v->p.counters) cudaFree(v->p.counters);
     if (v->p.pixmap) cudaFree(v->p.pixmap);
     if (v->p.pyr) cudaFree(v->p.pyr);
     if (v->p.jobs) cudaFree(v->p.jobs);
-    for (int i = 0; i < 2; ++i) {
+    for (int i = 0; i < N_STAGE; ++i) {
         if (v->stage_depth[i]) cudaFree(v->stage_depth[i]);
         if (v->stage_rgb[i]) cudaFree(v->stage_rgb[i]);
         if (v->ev_depth[i]) cudaEventDestroy(v->ev_depth[i]);
@@ -397,17 +399,17 @@ extern "C" int vol_integrate_host(vol_t *v, const uint16_t *depth_u16_host, int3
     if (v->stage_depth_bytes < db || v->stage_rgb_bytes < cb) {            // (re)allocate both sets
         CK(cudaDeviceSynchronize());
         const size_t nd = db > v->stage_depth_bytes ? db : v->stage_depth_bytes, nc = cb > v->stage_rgb_bytes ? cb : v->stage_rgb_bytes;
-        for (int i = 0; i < 2; ++i) {
+        for (int i = 0; i < N_STAGE; ++i) {
             if (v->stage_depth[i]) cudaFree(v->stage_depth[i]);
             if (v->stage_rgb[i]) cudaFree(v->stage_rgb[i]);
             v->stage_depth[i] = nullptr; v->stage_rgb[i] = nullptr; v->used_valid[i] = false;
         }
         v->stage_depth_bytes = v->stage_rgb_bytes = 0;
-        for (int i = 0; i < 2; ++i) { CK(cudaMalloc(&v->stage_depth[i], nd)); CK(cudaMalloc(&v->stage_rgb[i], nc)); }
+        for (int i = 0; i < N_STAGE; ++i) { CK(cudaMalloc(&v->stage_depth[i], nd)); CK(cudaMalloc(&v->stage_rgb[i], nc)); }
         v->stage_depth_bytes = nd; v->stage_rgb_bytes = nc;
     }
     cudaStream_t s = (cudaStream_t)stream;
-    const int set = (int)(v->host_seq++ & 1u);
+    const int set = (int)(v->host_seq++ % (unsigned)N_STAGE), prev = (set + N_STAGE - 1) % N_STAGE;
     // Both images go over the library's copy stream into staging set `set`, ordered only after the kernels that last read
     // that set (two frames ago) -- so they overlap the previous frame's kernels when the caller enqueues frames back to back.
     if (v->used_valid[set]) CK(cudaStreamWaitEvent(v->copy_stream, v->ev_used[set], 0));
@@ -418,7 +420,7 @@ extern "C" int vol_integrate_host(vol_t *v, const uint16_t *depth_u16_host, int3
     // Is the previous frame still being worked on?  Then this frame's HD image (91 % of the bytes) will have arrived by the
     // time its kernels start, and the whole queue goes in one launch.  Otherwise (the caller waits for every frame) the
     // geometry half runs while the HD image is still on its way and only the colour half waits for it.
-    const bool busy = v->used_valid[set ^ 1] && cudaEventQuery(v->ev_used[set ^ 1]) == cudaErrorNotReady;
+    const bool busy = v->used_valid[prev] && cudaEventQuery(v->ev_used[prev]) == cudaErrorNotReady;
     cudaGetLastError();
     CK(cudaStreamWaitEvent(s, v->ev_depth[set], 0));
     rc = integrate_impl(v, v->stage_depth[set], wd, hd, v->stage_rgb[set], wh, hh, T_world_depth, K_depth, K_rgb, T_depth_rgb, stream,
@@ -585,9 +587,7 @@ extern "C" int vol_frame_stats_async(vol_t *v, void *raw_host, void *stream)
     if (!v || !raw_host) return VOL_E_ARG;
     int rc = set_device(v); if (rc) return rc;
     cudaStream_t s = (cudaStream_t)stream;
-    static_assert(sizeof(uint32_t) * vf::CTRL_N == 32, "raw statistics record: 8 control words, then 4 counters");
-    CK(cudaMemcpyAsync(raw_host, v->p.ctrl, 32, cudaMemcpyDeviceToHost, s));
-    CK(cudaMemcpyAsync((char *)raw_host + 32, v->p.counters, 32, cudaMemcpyDeviceToHost, s));
+    CK(cudaMemcpyAsync(raw_host, v->p.ctrl, 64, cudaMemcpyDeviceToHost, s));
     return VOL_OK;
 }
 
