@@ -376,7 +376,7 @@ def run_ours(args, rank, world, local_rank):
     gen = torch.Generator(device="cuda"); gen.manual_seed(1)
     sp_pts = (hit_pts.repeat(8, 1) + (torch.rand(hit_pts.shape[0] * 8, 3, device="cuda", generator=gen) - 0.5) * (2.0 * c.voxel / c.r)).contiguous()
     sp_out = torch.empty(sp_pts.shape[0], dtype=torch.int32, device="cuda")
-    sample_ms, sample_filled = None, None
+    sample_ms, sample_filled, sample_tri_ms = None, None, None
     if sp_pts.shape[0] > 0:
         for _ in range(3):
             vol.sample_colour(sp_pts, sp_pts.shape[0], sp_out, stream=stream)
@@ -388,6 +388,15 @@ def run_ours(args, rank, world, local_rank):
         torch.cuda.synchronize()
         sample_ms = float(r0.elapsed_time(r1)) / 10.0
         sample_filled = float(((sp_out.view(torch.int32) >> 24) != 0).float().mean())
+        for _ in range(3):
+            vol.sample_colour_trilinear(sp_pts, sp_pts.shape[0], sp_out, stream=stream)
+        torch.cuda.synchronize()
+        r0.record(stream)
+        for _ in range(10):
+            vol.sample_colour_trilinear(sp_pts, sp_pts.shape[0], sp_out, stream=stream)
+        r1.record(stream)
+        torch.cuda.synchronize()
+        sample_tri_ms = float(r0.elapsed_time(r1)) / 10.0
     total_ms, e2e_ms, e2e_serial_ms = max_over_ranks([total_ms, e2e_ms, e2e_serial_ms], world, "cuda")
     clocks = sampler.stop() if sampler else None
     if clocks is not None and nvml is not None and nvml.sm:
@@ -441,6 +450,7 @@ def run_ours(args, rank, world, local_rank):
                     "note": "vol_raycast of the fused volumes (SURVEY 8(f) rank 1), not part of the timed step"},
         "sample_colour": None if sample_ms is None else {
             "ms": sample_ms, "points": int(sp_pts.shape[0]), "points_per_s": sp_pts.shape[0] / (sample_ms * 1e-3), "filled_fraction": sample_filled,
+            "trilinear_ms": sample_tri_ms,
             "note": "vol_sample_colour at jittered surface points (SURVEY 8(f) rank 3), not part of the timed step"},
         "gpu_launches": vol.launches_per_frame() * K,
         "clocks": clocks,

@@ -139,6 +139,11 @@ int vol_raycast(const vol_t *v, int32_t w, int32_t h, const float T_world_cam[16
  * n uint32: the packed colour word (layout above) of the colour voxel whose cell contains the point (nearest voxel), 0 for
  * a point outside the volume.  Unsharded volumes only.  Asynchronous on `stream`. */
 int vol_sample_colour(const vol_t *v, const float *points_dev, int64_t n, uint32_t *words_dev, void *stream);
+/* The same with trilinear interpolation between the 8 surrounding voxel centres (reading S2): voxels outside
+ * the volume or never observed (wq = 0) are left out and the colour is normalised over the others; the weight byte of the
+ * returned word is the trilinear interpolation of the stored weights with those voxels counted as 0 (coverage of the
+ * footprint).  0 where no observed voxel is in reach or the point is not finite.  Same arguments and rules. */
+int vol_sample_colour_trilinear(const vol_t *v, const float *points_dev, int64_t n, uint32_t *words_dev, void *stream);
 
 /* Copy this shard's volumes to HOST buffers of at least info.geo_bytes / info.col_bytes (either may be NULL to skip). */
 int vol_download(const vol_t *v, void *geo_host, size_t geo_bytes, void *col_host, size_t col_bytes, void *stream);

@@ -25,7 +25,7 @@ VOL_SLAB = 8
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "--fmad=false", "-std=c++17",
               "-Xcompiler", "-fPIC,-ffp-contract=off", "-shared"]
 
-EXPORTS = ["vol_create", "vol_integrate", "vol_integrate_host", "vol_raycast", "vol_sample_colour", "vol_download", "vol_download_voxels", "vol_upload",
+EXPORTS = ["vol_create", "vol_integrate", "vol_integrate_host", "vol_raycast", "vol_sample_colour", "vol_sample_colour_trilinear", "vol_download", "vol_download_voxels", "vol_upload",
            "vol_reset", "vol_info", "vol_shard_layers", "vol_set_counting", "vol_frame_stats", "vol_frame_stats_async", "vol_stats_decode", "vol_set_profiling", "vol_last_kernel_ms",
            "vol_launches_per_frame", "vol_selftest", "vol_destroy", "vol_strerror"]
 
@@ -79,6 +79,7 @@ def lib():
         L.vol_integrate_host.argtypes = L.vol_integrate.argtypes
         L.vol_raycast.argtypes = [P, I32, I32, P, P, F, F, P, P, P]
         L.vol_sample_colour.argtypes = [P, P, I64, P, P]
+        L.vol_sample_colour_trilinear.argtypes = [P, P, I64, P, P]
         L.vol_download.argtypes = [P, P, ctypes.c_size_t, P, ctypes.c_size_t, P]
         L.vol_download_voxels.argtypes = [P, P, I64, P, P, I64, P, P]
         L.vol_upload.argtypes = [P, P, P, P]
@@ -207,6 +208,11 @@ class Volume:
     def sample_colour(self, points_dev, n, words_dev, stream=None):
         """vol_sample_colour: points_dev = CUDA float32 tensor [n, 3] (world), words_dev = CUDA int32/uint32 tensor [n]."""
         _check(lib().vol_sample_colour(self._h, _dev_ptr(points_dev), int(n), _dev_ptr(words_dev), _stream_ptr(stream)), "vol_sample_colour")
+
+    def sample_colour_trilinear(self, points_dev, n, words_dev, stream=None):
+        """vol_sample_colour_trilinear: same arguments as sample_colour; trilinear interpolation over observed voxels."""
+        _check(lib().vol_sample_colour_trilinear(self._h, _dev_ptr(points_dev), int(n), _dev_ptr(words_dev), _stream_ptr(stream)),
+               "vol_sample_colour_trilinear")
 
     def download(self, stream=None):
         """vol_download: (geo uint32 [local_nz, Ny, Nx], col uint32 [r*local_nz, r*Ny, r*Nx]) of this shard."""

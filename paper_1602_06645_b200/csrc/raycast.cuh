@@ -159,4 +159,63 @@ __global__ void __launch_bounds__(256) k_sample_colour(const __grid_constant__ P
     words[m] = w;
 }
 
+// The same lookup with trilinear interpolation (reading S2): grid coordinate g = (p - origin) / vc - 1/2,
+// b = floor(g), f = g - b; the 8 voxels b + {0,1}^3 with weights (wz * wy) * wx; voxels outside the volume or never
+// observed (wq = 0) are left out and the colour is normalised over the rest, C = rint(sum w C / sum w); the weight byte
+// is rint(sum w wq) -- how much of the footprint has been seen.  The 8 words are requested first, then accumulated in
+// the canonical order (z-major, then y, then x).  One thread per point.
+__global__ void __launch_bounds__(256) k_sample_colour_trilinear(const __grid_constant__ Params p, const float *__restrict__ pts, long long n,
+                                                                 uint32_t *__restrict__ words)
+{
+    const long long m = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (m >= n) return;
+    const float o[3] = {p.ox, p.oy, p.oz};
+    const int cn[3] = {p.cnx, p.cny, p.cnz};
+    float b[3], f[3];
+    bool ok = true;
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        const float g = __fsub_rn(__fmul_rn(__fsub_rn(__ldg(pts + 3 * m + a), o[a]), p.inv_vc), 0.5f);
+        b[a] = floorf(g);
+        f[a] = __fsub_rn(g, b[a]);
+        ok = ok && (b[a] >= -1.0f) && (b[a] <= (float)(cn[a] - 1));      // the footprint touches the volume; false for NaN / inf
+    }
+    uint32_t word = 0u;
+    if (ok) {
+        const int i0 = (int)b[0], j0 = (int)b[1], k0 = (int)b[2];
+        uint32_t cw[8];
+#pragma unroll
+        for (int c = 0; c < 8; ++c) {
+            const int i = i0 + (c & 1), j = j0 + ((c >> 1) & 1), k = k0 + (c >> 2);
+            const bool in = i >= 0 && i < cn[0] && j >= 0 && j < cn[1] && k >= 0 && k < cn[2];
+            cw[c] = in ? __ldg(p.col + ((size_t)k * (size_t)cn[1] + (size_t)j) * (size_t)cn[0] + (size_t)i) : 0u;
+        }
+        float sw = 0.0f, sa = 0.0f, sc[3] = {0.0f, 0.0f, 0.0f};
+#pragma unroll
+        for (int c = 0; c < 8; ++c) {
+            if ((cw[c] >> 24) == 0u) continue;
+            const float wx = (c & 1) ? f[0] : __fsub_rn(1.0f, f[0]);
+            const float wy = (c & 2) ? f[1] : __fsub_rn(1.0f, f[1]);
+            const float wz = (c & 4) ? f[2] : __fsub_rn(1.0f, f[2]);
+            const float w = __fmul_rn(__fmul_rn(wz, wy), wx);
+            sw = __fadd_rn(sw, w);
+            sa = __fmaf_rn(w, (float)(cw[c] >> 24), sa);
+#pragma unroll
+            for (int ch = 0; ch < 3; ++ch) sc[ch] = __fmaf_rn(w, (float)((cw[c] >> (8 * ch)) & 0xffu), sc[ch]);
+        }
+        if (sw > 0.0f) {
+#pragma unroll
+            for (int ch = 0; ch < 3; ++ch) {
+                const float cq = rintf(__fdiv_rn(sc[ch], sw));
+                const int ci = cq < 0.0f ? 0 : (cq > 255.0f ? 255 : (int)cq);
+                word |= (uint32_t)ci << (8 * ch);
+            }
+            const float aq = rintf(sa);
+            const int ai = aq < 0.0f ? 0 : (aq > 255.0f ? 255 : (int)aq);
+            word |= (uint32_t)ai << 24;
+        }
+    }
+    words[m] = word;
+}
+
 }  // namespace vf

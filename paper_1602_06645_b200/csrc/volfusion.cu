@@ -465,6 +465,18 @@ extern "C" int vol_sample_colour(const vol_t *v, const float *points_dev, int64_
     return VOL_OK;
 }
 
+extern "C" int vol_sample_colour_trilinear(const vol_t *v, const float *points_dev, int64_t n, uint32_t *words_dev, void *stream)
+{
+    if (!v || n < 0 || (n > 0 && (!points_dev || !words_dev))) return VOL_E_ARG;
+    if (v->p.shard_world != 1) return VOL_E_ARG;               // a shard does not hold the whole volume
+    int rc = set_device(v); if (rc) return rc;
+    if (n == 0 || v->p.n_tiles == 0) return VOL_OK;
+    if ((n + 255) / 256 > 0x7fffffffLL) return VOL_E_ARG;
+    vf::k_sample_colour_trilinear<<<(unsigned)((n + 255) / 256), 256, 0, (cudaStream_t)stream>>>(v->p, points_dev, (long long)n, words_dev);
+    CK(cudaGetLastError());
+    return VOL_OK;
+}
+
 extern "C" int vol_download(const vol_t *v, void *geo_host, size_t geo_bytes, void *col_host, size_t col_bytes, void *stream)
 {
     if (!v) return VOL_E_ARG;

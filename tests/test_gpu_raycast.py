@@ -117,3 +117,34 @@ def test_sample_colour_and_polygon_texture_map():
     assert np.array_equal(got, want)
     assert (want[: pts.shape[0]] >> 24 > 0).sum() > 500 and (want[pts.shape[0]:] >> 24 > 0).mean() > 0.3   # both hit filled voxels
     g.sample_colour(dp, 0, dw)                                                                         # n = 0 is a no-op
+
+
+def test_sample_colour_trilinear():
+    """vol_sample_colour_trilinear (reading S2) against the oracle, word for word: 300 000 random points in and around
+    config 1's fused colour volume (most footprints are partly unobserved), points on the volume's faces and corners,
+    non-finite points, and a dense polygon map on the sphere."""
+    import torch
+    c = synth.config(1)
+    g, o = fused_pair(c, range(5))
+    rng = np.random.default_rng(19)
+    pts = rng.uniform(-0.8, 0.8, size=(300000, 3)).astype(np.float32) + np.array([0, 0, 1.5], np.float32)
+    surf = rng.normal(size=(200000, 3))
+    surf = (0.3 * surf / np.linalg.norm(surf, axis=1, keepdims=True) * rng.uniform(0.97, 1.03, size=(200000, 1))
+            + np.array([0, 0, 1.5])).astype(np.float32)                                                  # a shell around the sphere
+    lo, hi = np.asarray(c.origin, np.float64), np.asarray(c.origin, np.float64) + c.extent
+    t = rng.uniform(0, 1, size=(2000, 3))
+    face = lo + t * (hi - lo)
+    face[np.arange(2000), rng.integers(0, 3, 2000)] = np.where(rng.random(2000) < 0.5, lo[0], hi[0])    # cubic volume: on a face
+    odd = np.array([[np.nan, 0, 1.5], [0, np.inf, 1.5], [0, 0, -np.inf], [1e30, 0, 1.5], lo, hi, lo - 1e-4, hi + 1e-4], np.float32)
+    allp = np.concatenate([pts, surf, face.astype(np.float32), odd])
+    dp = torch.from_numpy(allp).cuda()
+    dw = torch.full((allp.shape[0],), -1, dtype=torch.int32, device="cuda")
+    g.sample_colour_trilinear(dp, allp.shape[0], dw)
+    torch.cuda.synchronize()
+    got = dw.cpu().numpy().view(np.uint32)
+    want = o.sample_colour_trilinear(allp)
+    assert np.array_equal(got, want), f"{int((got != want).sum())} words differ"
+    s = want[300000:500000]
+    assert (s != 0).mean() > 0.3 and ((s >> 24) < 250).sum() > 1000 and ((s >> 24) > 250).sum() > 1000   # full and partial footprints
+    assert not got[-8:-4].any()                                                                          # non-finite points
+    g.sample_colour_trilinear(dp, 0, dw)                                                                 # n = 0 is a no-op
