@@ -5,6 +5,8 @@ PAPER.md eq. 5-10 (L91-124) and the TSDF definition of readings A5/A6.  Only ``t
 ``__graft_entry__.smoke()`` and ``bench.py``'s ``cpu_baseline`` / ``--impl reference`` legs may import
 this package; the product path (``paper_1602_06645_b200``) never does, and this package never imports it.
 
+The depth front end and the ICP step are in ``oracle/frontend.py`` (numpy).
+
 Parity pins: tests/test_oracle_*.py (closed forms, fp64 brute force, invariants).  Unpinned by the
 paper itself (conventions of this build): the TSDF update (A5/A6), the HD-mapping
 reading A11 and the u8 weight encoding A12 -- "parity unpinned" w.r.t. the paper for those.
