@@ -140,6 +140,15 @@ def measure(depth_u16, K, levels=3, sigma_s_px=4.5, sigma_r_m=0.030):
     return pyramid(bilateral(depth_u16, sigma_s_px, sigma_r_m), K, levels, sigma_r_m)
 
 
+def predict(depth_m, K, levels=3, sigma_s_px=4.5, sigma_r_m=0.030):
+    """F8: the predicted side of the tracker from a ray-cast depth map (float32 metres, 0 = no surface).  The ray caster
+    samples the nearest voxel (reading R3), which leaves voxel-sized steps in the depth map and makes forward-difference
+    normals useless; the map is therefore rounded to whole millimetres (half-even, clamped to 65535) and passed through the
+    same filter as the measurement (F1) before F2-F4."""
+    q = np.minimum(np.rint((np.asarray(depth_m, F32) * F32(1000.0)).astype(F32)), F32(65535.0)).astype(np.uint16)
+    return pyramid(bilateral(q, sigma_s_px, sigma_r_m), K, levels, sigma_r_m)
+
+
 def _mat3(R, v, t=None):
     """R v (+ t) in the order ((R0 vx + R1 vy) + R2 vz) (+ t), one rounding per operation."""
     out = []

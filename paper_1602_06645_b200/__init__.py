@@ -27,7 +27,10 @@ NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", 
 
 EXPORTS = ["vol_create", "vol_integrate", "vol_integrate_host", "vol_raycast", "vol_sample_colour", "vol_sample_colour_trilinear", "vol_download", "vol_download_voxels", "vol_upload",
            "vol_reset", "vol_info", "vol_shard_layers", "vol_set_counting", "vol_frame_stats", "vol_frame_stats_async", "vol_stats_decode", "vol_set_profiling", "vol_last_kernel_ms",
-           "vol_launches_per_frame", "vol_selftest", "vol_destroy", "vol_strerror"]
+           "vol_launches_per_frame", "vol_selftest", "vol_destroy", "vol_strerror",
+           # include/volfrontend.h
+           "vol_frontend_create", "vol_frontend_destroy", "vol_frontend_measure", "vol_frontend_predict_depth", "vol_frontend_predict",
+           "vol_frontend_icp_step", "vol_frontend_track", "vol_frontend_maps"]
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
@@ -98,8 +101,17 @@ def lib():
         L.vol_destroy.restype = None
         L.vol_strerror.argtypes = [ctypes.c_int]
         L.vol_strerror.restype = ctypes.c_char_p
+        L.vol_frontend_create.argtypes = [ctypes.POINTER(P), I32, I32, I32, P]
+        L.vol_frontend_destroy.argtypes = [P]
+        L.vol_frontend_destroy.restype = None
+        L.vol_frontend_measure.argtypes = [P, P, P, P]
+        L.vol_frontend_predict_depth.argtypes = [P, P, P, I32, P]
+        L.vol_frontend_predict.argtypes = [P, P, P, P, F, F, P]
+        L.vol_frontend_icp_step.argtypes = [P, I32, P, P, P]
+        L.vol_frontend_track.argtypes = [P, P, P, P, P, P, P]
+        L.vol_frontend_maps.argtypes = [P, I32, I32, P, P, P, P]
         for name in EXPORTS:
-            if name not in ("vol_destroy", "vol_strerror"):
+            if name not in ("vol_destroy", "vol_strerror", "vol_frontend_destroy"):
                 getattr(L, name).restype = ctypes.c_int
         _lib = L
     return _lib
@@ -286,3 +298,82 @@ class Volume:
 
     def __exit__(self, *a):
         self.close()
+
+
+class FrontendOpts(ctypes.Structure):
+    _fields_ = [("sigma_s_px", ctypes.c_float), ("sigma_r_m", ctypes.c_float), ("dist_m", ctypes.c_float),
+                ("cos_min", ctypes.c_float), ("device", ctypes.c_int32)]
+
+
+ICP_SUMS = 29
+
+
+class Frontend:
+    """include/volfrontend.h: depth front end (bilateral filter, vertex / normal map pyramid) and ICP tracking against a
+    ray-cast prediction -- the measured and predicted map pyramids of one image size on one GPU."""
+
+    def __init__(self, w, h, levels=3, sigma_s_px=0.0, sigma_r_m=0.0, dist_m=0.0, cos_min=0.0, device=-1):
+        self._h = ctypes.c_void_p()
+        self.w, self.h, self.levels = int(w), int(h), int(levels)
+        opts = FrontendOpts(float(sigma_s_px), float(sigma_r_m), float(dist_m), float(cos_min), int(device))
+        rc = lib().vol_frontend_create(ctypes.byref(self._h), self.w, self.h, self.levels, ctypes.byref(opts))
+        if rc != VOL_OK:
+            self._h = ctypes.c_void_p()
+        _check(rc, "vol_frontend_create")
+
+    def measure(self, depth_dev, K, stream=None):
+        """vol_frontend_measure: depth_dev = CUDA tensor of w*h uint16 millimetres (any 2-byte dtype)."""
+        Kc = _f32(K, 9)
+        _check(lib().vol_frontend_measure(self._h, _dev_ptr(depth_dev), Kc.ctypes.data, _stream_ptr(stream)), "vol_frontend_measure")
+
+    def predict_depth(self, depth_m_dev, K, filter=False, stream=None):
+        """vol_frontend_predict_depth: depth_m_dev = CUDA float32 tensor of w*h metres; filter=True for ray-cast maps (F8)."""
+        Kc = _f32(K, 9)
+        _check(lib().vol_frontend_predict_depth(self._h, _dev_ptr(depth_m_dev), Kc.ctypes.data, int(bool(filter)), _stream_ptr(stream)),
+               "vol_frontend_predict_depth")
+
+    def predict(self, volume, T_world_cam, K, t_near, t_far, stream=None):
+        """vol_frontend_predict: ray-cast `volume` from T_world_cam and build the predicted maps."""
+        T, Kc = _f32(T_world_cam, 16), _f32(K, 9)
+        _check(lib().vol_frontend_predict(self._h, volume._h, T.ctypes.data, Kc.ctypes.data, float(t_near), float(t_far), _stream_ptr(stream)),
+               "vol_frontend_predict")
+
+    def icp_step(self, level, T_pred_cur, stream=None):
+        """vol_frontend_icp_step: (A [6,6], b [6], sum r^2, count) of one linearised step at `level`."""
+        T = _f32(T_pred_cur, 16)
+        s = np.zeros(ICP_SUMS, np.float64)
+        _check(lib().vol_frontend_icp_step(self._h, int(level), T.ctypes.data, s.ctypes.data, _stream_ptr(stream)), "vol_frontend_icp_step")
+        A = np.zeros((6, 6))
+        A[np.triu_indices(6)] = s[:21]
+        A = A + np.triu(A, 1).T
+        return A, s[21:27].copy(), float(s[27]), int(s[28])
+
+    def track(self, T_init=None, iterations=(10, 5, 4), stream=None):
+        """vol_frontend_track: (T_pred_cur float32 [4,4], rms, count); raises VolError(VOL_E_ARG) when tracking is lost."""
+        it = np.ascontiguousarray(np.asarray(iterations, np.int32))
+        assert it.size == self.levels
+        Ti = None if T_init is None else _f32(T_init, 16)
+        out = np.zeros(16, np.float32)
+        rms, cnt = ctypes.c_double(0.0), ctypes.c_int64(0)
+        _check(lib().vol_frontend_track(self._h, None if Ti is None else Ti.ctypes.data, it.ctypes.data, out.ctypes.data,
+                                        ctypes.byref(rms), ctypes.byref(cnt), _stream_ptr(stream)), "vol_frontend_track")
+        return out.reshape(4, 4), rms.value, cnt.value
+
+    def maps(self, which, level, stream=None):
+        """vol_frontend_maps: (D [h,w], V [h,w,3], N [h,w,3]) float32 of one level; which = 0 measured, 1 predicted."""
+        wl, hl = self.w >> level, self.h >> level
+        D, V, N = np.zeros((hl, wl), np.float32), np.zeros((hl, wl, 3), np.float32), np.zeros((hl, wl, 3), np.float32)
+        _check(lib().vol_frontend_maps(self._h, int(which), int(level), D.ctypes.data, V.ctypes.data, N.ctypes.data, _stream_ptr(stream)),
+               "vol_frontend_maps")
+        return D, V, N
+
+    def close(self):
+        if self._h:
+            lib().vol_frontend_destroy(self._h)
+            self._h = ctypes.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

@@ -1,0 +1,202 @@
+// frontend.cuh -- kernels of the depth front end and the ICP step (volfrontend.h readings F1-F5).
+//
+// Image-sized work (307 K pixels at most): one thread per pixel, whole-warp rows, no tiling -- these kernels are bound by
+// launch latency and L2, not by HBM.  All map arithmetic is binary32, one rounding per operation, NO fused multiply-add
+// (explicit __fmul_rn / __fadd_rn; the file is compiled with --fmad=false as well), in the order the oracle states, so
+// depth, vertex and normal maps are bit-identical to oracle/frontend.py.  The ICP sums are binary64.
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+namespace vf {
+
+constexpr int FE_RADIUS = 3;                  // F1: 7 x 7 window
+constexpr int FE_MAX_LEVELS = 6;
+constexpr int ICP_SUMS = 29;                  // 21 (upper triangle of A) + 6 (b) + sum r^2 + count
+
+struct LevelK { float fx, fy, cx, cy; };
+
+// F1: bilateral filter of the raw depth.  ws: 49 spatial weights [dy + 3][dx + 3]; wr: kmax + 1 range weights over whole mm.
+__global__ void __launch_bounds__(256) k_bilateral(const uint16_t *__restrict__ depth, int w, int h, const float *__restrict__ ws,
+                                                   const float *__restrict__ wr, int kmax, float *__restrict__ out)
+{
+    const int x = blockIdx.x * 32 + (threadIdx.x & 31), y = blockIdx.y * 8 + (threadIdx.x >> 5);
+    if (x >= w || y >= h) return;
+    const int d = (int)__ldg(depth + (size_t)y * w + x);
+    float r = 0.0f;
+    if (d > 0) {
+        float sw = 0.0f, sd = 0.0f;
+#pragma unroll
+        for (int dy = -FE_RADIUS; dy <= FE_RADIUS; ++dy) {
+            const int yy = y + dy;
+            if (yy < 0 || yy >= h) continue;
+#pragma unroll
+            for (int dx = -FE_RADIUS; dx <= FE_RADIUS; ++dx) {
+                const int xx = x + dx;
+                if (xx < 0 || xx >= w) continue;
+                const int q = (int)__ldg(depth + (size_t)yy * w + xx);
+                const int delta = abs(q - d);
+                if (q > 0 && delta <= kmax) {
+                    const float wgt = __fmul_rn(__ldg(ws + (dy + FE_RADIUS) * 7 + (dx + FE_RADIUS)), __ldg(wr + delta));
+                    sw = __fadd_rn(sw, wgt);
+                    sd = __fadd_rn(sd, __fmul_rn(wgt, (float)q));
+                }
+            }
+        }
+        r = __fmul_rn(__fdiv_rn(sd, sw), 0.001f);                         // mm -> m
+    }
+    out[(size_t)y * w + x] = r;
+}
+
+// F8: float metres -> whole millimetres (half-even, clamped), the input format of F1
+__global__ void __launch_bounds__(256) k_to_millimetres(const float *__restrict__ in, int n, uint16_t *__restrict__ out)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) out[i] = (uint16_t)fminf(rintf(__fmul_rn(__ldg(in + i), 1000.0f)), 65535.0f);
+}
+
+// F2: next pyramid level (w, h = size of the OUTPUT level)
+__global__ void __launch_bounds__(256) k_half_sample(const float *__restrict__ in, int w, int h, float thr, float *__restrict__ out)
+{
+    const int x = blockIdx.x * 32 + (threadIdx.x & 31), y = blockIdx.y * 8 + (threadIdx.x >> 5);
+    if (x >= w || y >= h) return;
+    const float2 r0 = __ldg(reinterpret_cast<const float2 *>(in + (size_t)(2 * y) * (2 * w) + 2 * x));
+    const float2 r1 = __ldg(reinterpret_cast<const float2 *>(in + (size_t)(2 * y + 1) * (2 * w) + 2 * x));
+    const float c = r0.x, v[4] = {r0.x, r0.y, r1.x, r1.y};
+    float res = 0.0f;
+    if (c > 0.0f) {
+        float s = 0.0f, n = 0.0f;
+#pragma unroll
+        for (int i = 0; i < 4; ++i)
+            if (v[i] > 0.0f && fabsf(__fsub_rn(v[i], c)) <= thr) { s = __fadd_rn(s, v[i]); n = __fadd_rn(n, 1.0f); }
+        res = __fdiv_rn(s, n);
+    }
+    out[(size_t)y * w + x] = res;
+}
+
+// F3 = eq. 7: the vertex of pixel (x, y) with depth D
+__device__ __forceinline__ float3 fe_vertex(const LevelK k, int x, int y, float D)
+{
+    return make_float3(__fdiv_rn(__fmul_rn(__fsub_rn((float)x, k.cx), D), k.fx), __fdiv_rn(__fmul_rn(__fsub_rn((float)y, k.cy), D), k.fy), D);
+}
+
+// F3 + F4 of one level: V (xyz, w = 0) and N (eq. 8 normalised; zero where a neighbour is missing or invalid)
+__global__ void __launch_bounds__(256) k_vertex_normal(const float *__restrict__ D, int w, int h, const LevelK k, float4 *__restrict__ V,
+                                                       float4 *__restrict__ N)
+{
+    const int x = blockIdx.x * 32 + (threadIdx.x & 31), y = blockIdx.y * 8 + (threadIdx.x >> 5);
+    if (x >= w || y >= h) return;
+    const size_t o = (size_t)y * w + x;
+    const float d0 = __ldg(D + o);
+    float4 v = make_float4(0.0f, 0.0f, 0.0f, 0.0f), n = v;
+    if (d0 > 0.0f) {
+        const float3 p0 = fe_vertex(k, x, y, d0);
+        v = make_float4(p0.x, p0.y, p0.z, 0.0f);
+        if (x + 1 < w && y + 1 < h) {
+            const float d1 = __ldg(D + o + 1), d2 = __ldg(D + o + w);
+            if (d1 > 0.0f && d2 > 0.0f) {
+                const float3 p1 = fe_vertex(k, x + 1, y, d1), p2 = fe_vertex(k, x, y + 1, d2);
+                const float ax = __fsub_rn(p1.x, p0.x), ay = __fsub_rn(p1.y, p0.y), az = __fsub_rn(p1.z, p0.z);
+                const float bx = __fsub_rn(p2.x, p0.x), by = __fsub_rn(p2.y, p0.y), bz = __fsub_rn(p2.z, p0.z);
+                const float nx = __fsub_rn(__fmul_rn(ay, bz), __fmul_rn(az, by));
+                const float ny = __fsub_rn(__fmul_rn(az, bx), __fmul_rn(ax, bz));
+                const float nz = __fsub_rn(__fmul_rn(ax, by), __fmul_rn(ay, bx));
+                const float ln = __fsqrt_rn(__fadd_rn(__fadd_rn(__fmul_rn(nx, nx), __fmul_rn(ny, ny)), __fmul_rn(nz, nz)));
+                if (ln > 0.0f) n = make_float4(__fdiv_rn(nx, ln), __fdiv_rn(ny, ln), __fdiv_rn(nz, ln), 0.0f);
+            }
+        }
+    }
+    V[o] = v; N[o] = n;
+}
+
+struct IcpParams {
+    const float4 *V, *N;            // measured maps (current camera's frame)
+    const float4 *Vp, *Np;          // predicted maps (prediction camera's frame)
+    int w, h;
+    LevelK k;
+    float R[9], t[3];               // current camera -> prediction camera
+    float dist2, cos_min;
+    double *sums;                   // ICP_SUMS accumulators (zeroed before the launch)
+};
+
+__device__ __forceinline__ float fe_dot3(float a0, float a1, float a2, float b0, float b1, float b2)
+{
+    return __fadd_rn(__fadd_rn(__fmul_rn(a0, b0), __fmul_rn(a1, b1)), __fmul_rn(a2, b2));
+}
+
+// F5: one thread per measured pixel; J and r in binary32 exactly as the oracle, products and sums in binary64; the block
+// reduces through warp shuffles and shared memory and issues one atomic per accumulator.
+__global__ void __launch_bounds__(256) k_icp(const __grid_constant__ IcpParams q)
+{
+    const int x = blockIdx.x * 32 + (threadIdx.x & 31), y = blockIdx.y * 8 + (threadIdx.x >> 5);
+    float J[6] = {0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0.0f}, r = 0.0f;
+    bool ok = x < q.w && y < q.h;
+    if (ok) {
+        const size_t o = (size_t)y * q.w + x;
+        const float4 n = __ldg(q.N + o);
+        ok = n.x != 0.0f || n.y != 0.0f || n.z != 0.0f;
+        if (ok) {
+            const float4 v = __ldg(q.V + o);
+            const float px = __fadd_rn(fe_dot3(q.R[0], q.R[1], q.R[2], v.x, v.y, v.z), q.t[0]);
+            const float py = __fadd_rn(fe_dot3(q.R[3], q.R[4], q.R[5], v.x, v.y, v.z), q.t[1]);
+            const float pz = __fadd_rn(fe_dot3(q.R[6], q.R[7], q.R[8], v.x, v.y, v.z), q.t[2]);
+            const float mx = fe_dot3(q.R[0], q.R[1], q.R[2], n.x, n.y, n.z);
+            const float my = fe_dot3(q.R[3], q.R[4], q.R[5], n.x, n.y, n.z);
+            const float mz = fe_dot3(q.R[6], q.R[7], q.R[8], n.x, n.y, n.z);
+            ok = pz > 0.0f;
+            if (ok) {
+                const float u = __fadd_rn(__fmul_rn(q.k.fx, __fdiv_rn(px, pz)), q.k.cx);
+                const float vv = __fadd_rn(__fmul_rn(q.k.fy, __fdiv_rn(py, pz)), q.k.cy);
+                const float xf = floorf(__fadd_rn(u, 0.5f)), yf = floorf(__fadd_rn(vv, 0.5f));
+                ok = xf >= 0.0f && xf < (float)q.w && yf >= 0.0f && yf < (float)q.h;
+                if (ok) {
+                    const size_t op = (size_t)(int)yf * q.w + (int)xf;
+                    const float4 nq = __ldg(q.Np + op);
+                    ok = nq.x != 0.0f || nq.y != 0.0f || nq.z != 0.0f;
+                    if (ok) {
+                        const float4 vq = __ldg(q.Vp + op);
+                        const float dx = __fsub_rn(vq.x, px), dy = __fsub_rn(vq.y, py), dz = __fsub_rn(vq.z, pz);
+                        const float dist2 = fe_dot3(dx, dy, dz, dx, dy, dz);
+                        const float cosang = fe_dot3(mx, my, mz, nq.x, nq.y, nq.z);
+                        ok = !(dist2 > q.dist2) && !(cosang < q.cos_min);
+                        r = fe_dot3(nq.x, nq.y, nq.z, dx, dy, dz);
+                        J[0] = __fsub_rn(__fmul_rn(py, nq.z), __fmul_rn(pz, nq.y));
+                        J[1] = __fsub_rn(__fmul_rn(pz, nq.x), __fmul_rn(px, nq.z));
+                        J[2] = __fsub_rn(__fmul_rn(px, nq.y), __fmul_rn(py, nq.x));
+                        J[3] = nq.x; J[4] = nq.y; J[5] = nq.z;
+                    }
+                }
+            }
+        }
+    }
+    double s[ICP_SUMS];
+    {
+        int idx = 0;
+#pragma unroll
+        for (int i = 0; i < 6; ++i)
+#pragma unroll
+            for (int j = i; j < 6; ++j) s[idx++] = ok ? (double)J[i] * (double)J[j] : 0.0;
+#pragma unroll
+        for (int i = 0; i < 6; ++i) s[21 + i] = ok ? (double)J[i] * (double)r : 0.0;
+        s[27] = ok ? (double)r * (double)r : 0.0;
+        s[28] = ok ? 1.0 : 0.0;
+    }
+    __shared__ double sh[8][ICP_SUMS];
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+#pragma unroll
+    for (int i = 0; i < ICP_SUMS; ++i) {
+        double a = s[i];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) a += __shfl_xor_sync(0xffffffffu, a, o);
+        if (lane == 0) sh[wid][i] = a;
+    }
+    __syncthreads();
+    if (threadIdx.x < ICP_SUMS) {
+        double a = 0.0;
+#pragma unroll
+        for (int k = 0; k < 8; ++k) a += sh[k][threadIdx.x];
+        if (a != 0.0) atomicAdd(q.sums + threadIdx.x, a);
+    }
+}
+
+}  // namespace vf

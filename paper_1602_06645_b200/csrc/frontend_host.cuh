@@ -1,0 +1,260 @@
+// frontend_host.cuh -- host side of include/volfrontend.h (included at the end of volfusion.cu: same library, same error
+// reporting).  F6 / F7 (the 6 x 6 solve, the pose update, the coarse-to-fine loop) run here in binary64.
+#pragma once
+#include "../../include/volfrontend.h"
+#include "frontend.cuh"
+
+struct vol_frontend {
+    int device, w, h, levels;
+    float sigma_s, sigma_r, dist_m, cos_min;
+    int kmax;
+    float *ws, *wr;                                         // F1 tables (device)
+    float *D[2][vf::FE_MAX_LEVELS];                         // [0] measured, [1] predicted
+    float4 *V[2][vf::FE_MAX_LEVELS], *N[2][vf::FE_MAX_LEVELS];
+    vf::LevelK k[2][vf::FE_MAX_LEVELS];
+    bool have[2];
+    float *ray_depth;                                       // vol_frontend_predict: the ray-cast depth map
+    uint16_t *pred_mm;                                      // F8: the prediction in whole millimetres
+    double *sums_dev, *sums_pinned;
+};
+
+static int fe_set_device(const vol_frontend *fe) { CK(cudaSetDevice(fe->device)); return VOL_OK; }
+
+extern "C" void vol_frontend_destroy(vol_frontend_t *fe)
+{
+    if (!fe) return;
+    cudaSetDevice(fe->device);
+    if (fe->ws) cudaFree(fe->ws);
+    if (fe->wr) cudaFree(fe->wr);
+    for (int s = 0; s < 2; ++s)
+        for (int l = 0; l < vf::FE_MAX_LEVELS; ++l) {
+            if (fe->D[s][l]) cudaFree(fe->D[s][l]);
+            if (fe->V[s][l]) cudaFree(fe->V[s][l]);
+            if (fe->N[s][l]) cudaFree(fe->N[s][l]);
+        }
+    if (fe->ray_depth) cudaFree(fe->ray_depth);
+    if (fe->pred_mm) cudaFree(fe->pred_mm);
+    if (fe->sums_dev) cudaFree(fe->sums_dev);
+    if (fe->sums_pinned) cudaFreeHost(fe->sums_pinned);
+    cudaGetLastError();
+    delete fe;
+}
+
+extern "C" int vol_frontend_create(vol_frontend_t **out, int32_t w, int32_t h, int32_t levels, const vol_frontend_opts_t *opts)
+{
+    if (!out || w <= 0 || h <= 0 || w > 16384 || h > 16384 || levels < 1 || levels > vf::FE_MAX_LEVELS) return VOL_E_ARG;
+    if (w % (1 << (levels - 1)) != 0 || h % (1 << (levels - 1)) != 0) return VOL_E_ARG;
+    float sigma_s = 4.5f, sigma_r = 0.030f, dist_m = 0.10f, cos_min = 0.94f;
+    int device = -1;
+    if (opts) {
+        if (opts->sigma_s_px > 0.0f) sigma_s = opts->sigma_s_px;
+        if (opts->sigma_r_m > 0.0f) sigma_r = opts->sigma_r_m;
+        if (opts->dist_m > 0.0f) dist_m = opts->dist_m;
+        if (opts->cos_min > 0.0f) cos_min = opts->cos_min;
+        device = opts->device;
+    }
+    if (!(sigma_s <= 1e3f) || !(sigma_r <= 1.0f) || !(dist_m <= 1e3f) || !(cos_min <= 1.0f)) return VOL_E_ARG;
+    if (device < 0) CK(cudaGetDevice(&device));
+    CK(cudaSetDevice(device));
+    vol_frontend *fe = new (std::nothrow) vol_frontend();
+    if (!fe) return VOL_E_OOM;
+    memset(fe, 0, sizeof *fe);
+    fe->device = device; fe->w = w; fe->h = h; fe->levels = levels;
+    fe->sigma_s = sigma_s; fe->sigma_r = sigma_r; fe->dist_m = dist_m; fe->cos_min = cos_min;
+    // F1 tables: binary64, rounded once
+    const double ss = (double)sigma_s, sr = (double)sigma_r * 1000.0;
+    fe->kmax = (int)std::ceil(3.0 * sr);
+    float ws[49];
+    for (int dy = -vf::FE_RADIUS; dy <= vf::FE_RADIUS; ++dy)
+        for (int dx = -vf::FE_RADIUS; dx <= vf::FE_RADIUS; ++dx)
+            ws[(dy + vf::FE_RADIUS) * 7 + dx + vf::FE_RADIUS] = (float)std::exp(-((double)(dx * dx) + (double)(dy * dy)) / (2.0 * ss * ss));
+    float *wr = new (std::nothrow) float[fe->kmax + 1];
+    if (!wr) { delete fe; return VOL_E_OOM; }
+    for (int k = 0; k <= fe->kmax; ++k) wr[k] = (float)std::exp(-((double)k * (double)k) / (2.0 * sr * sr));
+    auto fail = [&](int code) { delete[] wr; vol_frontend_destroy(fe); return code; };
+    bool okc = cudaMalloc(&fe->ws, sizeof ws) == cudaSuccess && cudaMalloc(&fe->wr, sizeof(float) * (fe->kmax + 1)) == cudaSuccess &&
+               cudaMalloc(&fe->ray_depth, sizeof(float) * (size_t)w * h) == cudaSuccess &&
+               cudaMalloc(&fe->pred_mm, sizeof(uint16_t) * (size_t)w * h) == cudaSuccess &&
+               cudaMalloc(&fe->sums_dev, sizeof(double) * vf::ICP_SUMS) == cudaSuccess &&
+               cudaMallocHost(&fe->sums_pinned, sizeof(double) * vf::ICP_SUMS) == cudaSuccess;
+    for (int s = 0; s < 2 && okc; ++s)
+        for (int l = 0; l < levels && okc; ++l) {
+            const size_t n = (size_t)(w >> l) * (h >> l);
+            okc = cudaMalloc(&fe->D[s][l], n * sizeof(float)) == cudaSuccess && cudaMalloc(&fe->V[s][l], n * sizeof(float4)) == cudaSuccess &&
+                  cudaMalloc(&fe->N[s][l], n * sizeof(float4)) == cudaSuccess;
+        }
+    if (!okc) { cudaGetLastError(); return fail(VOL_E_OOM); }
+    if (cudaMemcpy(fe->ws, ws, sizeof ws, cudaMemcpyHostToDevice) != cudaSuccess ||
+        cudaMemcpy(fe->wr, wr, sizeof(float) * (fe->kmax + 1), cudaMemcpyHostToDevice) != cudaSuccess) return fail(VOL_E_CUDA);
+    delete[] wr;
+    *out = fe;
+    return VOL_OK;
+}
+
+// F2-F4 for every level of side s, from its level-0 depth map
+static int fe_build_pyramid(vol_frontend *fe, int s, const float K[9], cudaStream_t st)
+{
+    vf::LevelK k = {K[0], K[4], K[2], K[5]};
+    const float thr = 3.0f * fe->sigma_r;
+    for (int l = 0; l < fe->levels; ++l) {
+        const int w = fe->w >> l, h = fe->h >> l;
+        const dim3 grid((w + 31) / 32, (h + 7) / 8);
+        if (l > 0) {
+            k.fx = k.fx * 0.5f; k.fy = k.fy * 0.5f;
+            k.cx = (k.cx - 0.5f) * 0.5f; k.cy = (k.cy - 0.5f) * 0.5f;
+            vf::k_half_sample<<<grid, 256, 0, st>>>(fe->D[s][l - 1], w, h, thr, fe->D[s][l]);
+        }
+        fe->k[s][l] = k;
+        vf::k_vertex_normal<<<grid, 256, 0, st>>>(fe->D[s][l], w, h, k, fe->V[s][l], fe->N[s][l]);
+    }
+    CK(cudaGetLastError());
+    fe->have[s] = true;
+    return VOL_OK;
+}
+
+extern "C" int vol_frontend_measure(vol_frontend_t *fe, const uint16_t *depth_u16_dev, const float K[9], void *stream)
+{
+    if (!fe || !depth_u16_dev || !K || !intrinsics_ok(K)) return VOL_E_ARG;
+    int rc = fe_set_device(fe); if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    vf::k_bilateral<<<dim3((fe->w + 31) / 32, (fe->h + 7) / 8), 256, 0, st>>>(depth_u16_dev, fe->w, fe->h, fe->ws, fe->wr, fe->kmax, fe->D[0][0]);
+    return fe_build_pyramid(fe, 0, K, st);
+}
+
+extern "C" int vol_frontend_predict_depth(vol_frontend_t *fe, const float *depth_m_dev, const float K[9], int32_t filter, void *stream)
+{
+    if (!fe || !depth_m_dev || !K || !intrinsics_ok(K)) return VOL_E_ARG;
+    int rc = fe_set_device(fe); if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    const int n = fe->w * fe->h;
+    if (filter) {                                            // F8
+        vf::k_to_millimetres<<<(n + 255) / 256, 256, 0, st>>>(depth_m_dev, n, fe->pred_mm);
+        vf::k_bilateral<<<dim3((fe->w + 31) / 32, (fe->h + 7) / 8), 256, 0, st>>>(fe->pred_mm, fe->w, fe->h, fe->ws, fe->wr, fe->kmax, fe->D[1][0]);
+    } else {
+        CK(cudaMemcpyAsync(fe->D[1][0], depth_m_dev, sizeof(float) * (size_t)n, cudaMemcpyDeviceToDevice, st));
+    }
+    return fe_build_pyramid(fe, 1, K, st);
+}
+
+extern "C" int vol_frontend_predict(vol_frontend_t *fe, const vol_t *v, const float T_world_cam[16], const float K[9], float t_near_m,
+                                    float t_far_m, void *stream)
+{
+    if (!fe || !v || fe->device != v->device) return VOL_E_ARG;
+    int rc = vol_raycast(v, fe->w, fe->h, T_world_cam, K, t_near_m, t_far_m, fe->ray_depth, nullptr, stream);
+    if (rc) return rc;
+    return vol_frontend_predict_depth(fe, fe->ray_depth, K, 1, stream);
+}
+
+static int fe_icp_launch(vol_frontend *fe, int level, const float T[16], cudaStream_t st)
+{
+    vf::IcpParams q;
+    q.V = fe->V[0][level]; q.N = fe->N[0][level]; q.Vp = fe->V[1][level]; q.Np = fe->N[1][level];
+    q.w = fe->w >> level; q.h = fe->h >> level; q.k = fe->k[1][level];
+    for (int i = 0; i < 3; ++i) { for (int j = 0; j < 3; ++j) q.R[3 * i + j] = T[4 * i + j]; q.t[i] = T[4 * i + 3]; }
+    q.dist2 = fe->dist_m * fe->dist_m; q.cos_min = fe->cos_min; q.sums = fe->sums_dev;
+    CK(cudaMemsetAsync(fe->sums_dev, 0, sizeof(double) * vf::ICP_SUMS, st));
+    vf::k_icp<<<dim3((q.w + 31) / 32, (q.h + 7) / 8), 256, 0, st>>>(q);
+    CK(cudaGetLastError());
+    CK(cudaMemcpyAsync(fe->sums_pinned, fe->sums_dev, sizeof(double) * vf::ICP_SUMS, cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    return VOL_OK;
+}
+
+static bool fe_rigid(const float T[16])
+{
+    float R[9], t[3];
+    return rigid_inverse(T, R, t);
+}
+
+extern "C" int vol_frontend_icp_step(vol_frontend_t *fe, int32_t level, const float T_pred_cur[16], double *sums_host, void *stream)
+{
+    if (!fe || !T_pred_cur || !sums_host || level < 0 || level >= fe->levels || !fe->have[0] || !fe->have[1]) return VOL_E_ARG;
+    if (!fe_rigid(T_pred_cur)) return VOL_E_ARG;
+    int rc = fe_set_device(fe); if (rc) return rc;
+    rc = fe_icp_launch(fe, level, T_pred_cur, (cudaStream_t)stream); if (rc) return rc;
+    memcpy(sums_host, fe->sums_pinned, sizeof(double) * vf::ICP_SUMS);
+    return VOL_OK;
+}
+
+// F6: A xi = b by Cholesky (A symmetric positive definite), then T <- [exp(omega) R, exp(omega) t + v]; binary64
+static bool fe_se3_update(double T[16], const double *sums)
+{
+    double A[6][6], L[6][6] = {}, b[6], y[6], xi[6];
+    int idx = 0;
+    for (int i = 0; i < 6; ++i) for (int j = i; j < 6; ++j) { A[i][j] = sums[idx]; A[j][i] = sums[idx]; ++idx; }
+    for (int i = 0; i < 6; ++i) b[i] = sums[21 + i];
+    for (int i = 0; i < 6; ++i)
+        for (int j = 0; j <= i; ++j) {
+            double s = A[i][j];
+            for (int k = 0; k < j; ++k) s -= L[i][k] * L[j][k];
+            if (i == j) { if (!(s > 0.0)) return false; L[i][i] = std::sqrt(s); }
+            else L[i][j] = s / L[j][j];
+        }
+    for (int i = 0; i < 6; ++i) { double s = b[i]; for (int k = 0; k < i; ++k) s -= L[i][k] * y[k]; y[i] = s / L[i][i]; }
+    for (int i = 5; i >= 0; --i) { double s = y[i]; for (int k = i + 1; k < 6; ++k) s -= L[k][i] * xi[k]; xi[i] = s / L[i][i]; }
+    const double ox = xi[0], oy = xi[1], oz = xi[2], th = std::sqrt(ox * ox + oy * oy + oz * oz);
+    const double Kx[3][3] = {{0.0, -oz, oy}, {oz, 0.0, -ox}, {-oy, ox, 0.0}};
+    double K2[3][3], Ri[3][3];
+    for (int i = 0; i < 3; ++i) for (int j = 0; j < 3; ++j) { K2[i][j] = 0.0; for (int k = 0; k < 3; ++k) K2[i][j] += Kx[i][k] * Kx[k][j]; }
+    const double a = th < 1e-12 ? 1.0 : std::sin(th) / th, c = th < 1e-12 ? 0.0 : (1.0 - std::cos(th)) / (th * th);
+    for (int i = 0; i < 3; ++i) for (int j = 0; j < 3; ++j) Ri[i][j] = (i == j ? 1.0 : 0.0) + a * Kx[i][j] + c * K2[i][j];
+    double out[16] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 1};
+    for (int i = 0; i < 3; ++i) {
+        for (int j = 0; j < 3; ++j) { double s = 0.0; for (int k = 0; k < 3; ++k) s += Ri[i][k] * T[4 * k + j]; out[4 * i + j] = s; }
+        double s = 0.0; for (int k = 0; k < 3; ++k) s += Ri[i][k] * T[4 * k + 3];
+        out[4 * i + 3] = s + xi[3 + i];
+    }
+    memcpy(T, out, sizeof out);
+    return true;
+}
+
+extern "C" int vol_frontend_track(vol_frontend_t *fe, const float T_init[16], const int32_t *iterations, float T_out[16], double *rms_out,
+                                  int64_t *count_out, void *stream)
+{
+    if (!fe || !iterations || !T_out || !fe->have[0] || !fe->have[1]) return VOL_E_ARG;
+    if (T_init && !fe_rigid(T_init)) return VOL_E_ARG;
+    for (int l = 0; l < fe->levels; ++l) if (iterations[l] < 0 || iterations[l] > 1000) return VOL_E_ARG;
+    int rc = fe_set_device(fe); if (rc) return rc;
+    double T[16] = {1, 0, 0, 0, 0, 1, 0, 0, 0, 0, 1, 0, 0, 0, 0, 1};
+    if (T_init) for (int i = 0; i < 16; ++i) T[i] = (double)T_init[i];
+    double rms = 0.0; int64_t count = 0;
+    int result = VOL_OK;
+    for (int l = fe->levels - 1; l >= 0 && result == VOL_OK; --l)
+        for (int it = 0; it < iterations[l]; ++it) {
+            float T32[16];
+            for (int i = 0; i < 16; ++i) T32[i] = (float)T[i];
+            rc = fe_icp_launch(fe, l, T32, (cudaStream_t)stream); if (rc) return rc;
+            const double *s = fe->sums_pinned;
+            count = (int64_t)s[28];
+            if (count < 100) { snprintf(g_err, sizeof g_err, "vol_frontend_track: %lld correspondences at level %d", (long long)count, l); result = VOL_E_ARG; break; }
+            rms = std::sqrt(s[27] / (double)count);
+            if (!fe_se3_update(T, s)) { snprintf(g_err, sizeof g_err, "vol_frontend_track: normal equations not positive definite"); result = VOL_E_ARG; break; }
+        }
+    for (int i = 0; i < 16; ++i) T_out[i] = (float)T[i];
+    if (rms_out) *rms_out = rms;
+    if (count_out) *count_out = count;
+    return result;
+}
+
+extern "C" int vol_frontend_maps(const vol_frontend_t *fe, int32_t which, int32_t level, float *depth_host, float *vertex_host,
+                                 float *normal_host, void *stream)
+{
+    if (!fe || which < 0 || which > 1 || level < 0 || level >= fe->levels || !fe->have[which]) return VOL_E_ARG;
+    int rc = fe_set_device(fe); if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t n = (size_t)(fe->w >> level) * (fe->h >> level);
+    if (depth_host) CK(cudaMemcpyAsync(depth_host, fe->D[which][level], n * sizeof(float), cudaMemcpyDeviceToHost, st));
+    float4 *tmp = nullptr;
+    if (vertex_host || normal_host) { tmp = new (std::nothrow) float4[n]; if (!tmp) return VOL_E_OOM; }
+    for (int m = 0; m < 2; ++m) {
+        float *dst = m == 0 ? vertex_host : normal_host;
+        if (!dst) continue;
+        cudaError_t e = cudaMemcpyAsync(tmp, m == 0 ? fe->V[which][level] : fe->N[which][level], n * sizeof(float4), cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+        if (e != cudaSuccess) { delete[] tmp; CK(e); }
+        for (size_t i = 0; i < n; ++i) { dst[3 * i] = tmp[i].x; dst[3 * i + 1] = tmp[i].y; dst[3 * i + 2] = tmp[i].z; }
+    }
+    delete[] tmp;
+    CK(cudaStreamSynchronize(st));
+    return VOL_OK;
+}

@@ -685,3 +685,5 @@ extern "C" int vol_selftest(uint64_t mismatches[2], int32_t exhaustive)
     cudaFree(d);
     return rc;
 }
+
+#include "frontend_host.cuh"

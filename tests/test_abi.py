@@ -1,4 +1,4 @@
-"""The C-ABI library loads and exports every symbol include/volfusion.h declares (no compute; runs without a GPU)."""
+"""The C-ABI library loads and exports every symbol include/*.h declares (no compute; runs without a GPU)."""
 import ctypes
 import os
 import re
@@ -12,9 +12,12 @@ ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 
 def declared_symbols():
-    src = open(os.path.join(ROOT, "include", "volfusion.h")).read()
-    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
-    return sorted(set(re.findall(r"\b(vol_[a-z_]+)\s*\(", src)))
+    names = set()
+    for header in sorted(os.listdir(os.path.join(ROOT, "include"))):
+        src = open(os.path.join(ROOT, "include", header)).read()
+        src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+        names |= set(re.findall(r"\b(vol_[a-z_]+)\s*\(", src))
+    return sorted(names)
 
 
 def test_header_symbols_are_exported():
@@ -53,6 +56,10 @@ def test_argument_validation_precedes_any_cuda_call():
     assert L.vol_create(None, None, 2, org, 1.0, 0.1, 128, None) == vf.VOL_E_ARG
     assert L.vol_strerror(vf.VOL_E_ARG) == b"invalid argument"
     assert L.vol_integrate(None, None, 1, 1, None, 1, 1, None, None, None, None, None) == vf.VOL_E_ARG
+    fe = ctypes.c_void_p()
+    for w, h, levels in ((0, 8, 1), (8, 8, 0), (8, 8, 7), (12, 8, 4), (8, 6, 3)):
+        assert L.vol_frontend_create(ctypes.byref(fe), w, h, levels, None) == vf.VOL_E_ARG and not fe
+    assert L.vol_frontend_measure(None, None, None, None) == vf.VOL_E_ARG
 
 
 def test_no_cpu_fallback_without_a_gpu():

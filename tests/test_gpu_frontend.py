@@ -1,0 +1,153 @@
+"""GPU parity of the depth front end and the ICP step (include/volfrontend.h) against oracle/frontend.py:
+maps bit for bit, normal-equation sums to binary64 rounding, tracked poses to micrometres, and the closed loop
+(ray-cast prediction -> ICP -> integration at the tracked pose) against the ground-truth trajectory."""
+import math
+
+import numpy as np
+import pytest
+
+import oracle
+import synth
+from oracle import frontend as ofe
+from parity_util import to_dev
+
+pytestmark = pytest.mark.gpu
+
+
+def bits(a):
+    return np.ascontiguousarray(a, np.float32).view(np.uint32)
+
+
+def assert_pyramids_identical(fe, which, ref, what):
+    for lv, (D, V, N) in enumerate(ref):
+        gD, gV, gN = fe.maps(which, lv)
+        assert np.array_equal(bits(gD), bits(D)), f"{what}: depth of level {lv} differs at {int((bits(gD) != bits(D)).sum())} pixels"
+        assert np.array_equal(bits(gV), bits(V)), f"{what}: vertex map of level {lv} differs"
+        assert np.array_equal(bits(gN), bits(N)), f"{what}: normal map of level {lv} differs at {int((bits(gN) != bits(N)).any(-1).sum())} pixels"
+
+
+@pytest.mark.parametrize("cfg,frame,sigma_s,sigma_r", [(3, 7, 0.0, 0.0), (2, 40, 0.0, 0.0), (5, 100, 3.0, 0.012), (4, 3, 6.0, 0.05)])
+def test_measured_maps_bit_exact(cfg, frame, sigma_s, sigma_r):
+    """F1-F4 on noisy 640 x 480 frames with 2 % dropouts, three levels, default and odd filter parameters."""
+    import paper_1602_06645_b200 as vf
+    c = synth.config(cfg)
+    depth, _, _ = synth.frame(c, frame, want_rgb=False)
+    fe = vf.Frontend(c.wd, c.hd, 3, sigma_s_px=sigma_s, sigma_r_m=sigma_r)
+    fe.measure(to_dev(depth), c.K_depth)
+    ref = ofe.measure(depth, c.K_depth, 3, sigma_s or 4.5, sigma_r or 0.030)
+    assert_pyramids_identical(fe, 0, ref, f"cfg {cfg}")
+    assert (ref[0][0] > 0).sum() > 20000 and np.any(ref[2][2] != 0, axis=-1).sum() > 1000
+    fe.close()
+
+
+def test_predicted_maps_and_small_images_bit_exact():
+    """F2-F4 from a float depth map (the prediction side); a 4-level pyramid; an image narrower than a warp; all-invalid input."""
+    import torch
+    import paper_1602_06645_b200 as vf
+    c = synth.config(2)
+    z, _ = synth.render(c.prims, c.K_depth, synth.look_at((0.9, -0.6, 0.55), (0, 0, 0)), c.wd, c.hd, True, False)
+    fe = vf.Frontend(c.wd, c.hd, 4)
+    fe.predict_depth(torch.from_numpy(z).cuda(), c.K_depth)
+    assert_pyramids_identical(fe, 1, ofe.pyramid(z, c.K_depth, 4), "predicted")
+    zz = z + np.float32(0.004) * ((np.arange(c.wd)[None, :] // 3 + np.arange(c.hd)[:, None] // 5) % 2).astype(np.float32) * (z > 0)   # steps
+    zz[5, 5] = 70.0                                                                                # clamps to 65535 mm
+    fe.predict_depth(torch.from_numpy(zz).cuda(), c.K_depth, filter=True)
+    assert_pyramids_identical(fe, 1, ofe.predict(zz, c.K_depth, 4), "predicted, filtered (F8)")
+    fe.close()
+    rng = np.random.default_rng(4)
+    small = np.rint(1500 + rng.normal(0, 3, size=(12, 20))).astype(np.uint16)
+    small[rng.random(small.shape) < 0.1] = 0
+    K = synth.intrinsics(30.0, 9.5, 5.5)
+    fe = vf.Frontend(20, 12, 3)
+    fe.measure(to_dev(small), K)
+    assert_pyramids_identical(fe, 0, ofe.measure(small, K, 3), "20 x 12")
+    fe.measure(to_dev(np.zeros((12, 20), np.uint16)), K)
+    for lv in range(3):
+        assert not any(m.any() for m in fe.maps(0, lv))
+    fe.close()
+
+
+def scene_pair(dT, w=640, h=480):
+    c = synth.config(2)
+    A = synth.look_at((0.9, -0.6, 0.55), (0.0, 0.0, 0.0))
+    za, _ = synth.render(c.prims, c.K_depth, A, w, h, True, False)
+    zb, _ = synth.render(c.prims, c.K_depth, A @ dT, w, h, True, False)
+    db = synth.quantise_depth(zb, np.random.default_rng(3), c.noise, 0.02)
+    return c, za, db
+
+
+def small_motion(rx, ry, rz, t):
+    T = np.eye(4)
+    T[:3, :3] = synth.rot_axis((1, 0, 0), rx) @ synth.rot_axis((0, 1, 0), ry) @ synth.rot_axis((0, 0, 1), rz)
+    T[:3, 3] = t
+    return T
+
+
+def test_icp_step_sums_and_track():
+    """F5 at every level for several estimates: the same correspondences (count identical) and A, b, sum r^2 equal to
+    binary64 summation order; F6/F7: the tracked pose equals the oracle's to micrometres and recovers the true motion."""
+    import torch
+    import paper_1602_06645_b200 as vf
+    dT = small_motion(0.012, -0.018, 0.009, (0.012, -0.007, 0.010))
+    c, za, db = scene_pair(dT)
+    fe = vf.Frontend(c.wd, c.hd, 3)
+    fe.measure(to_dev(db), c.K_depth)
+    fe.predict_depth(torch.from_numpy(za).cuda(), c.K_depth)
+    meas, pred = ofe.measure(db, c.K_depth, 3), ofe.pyramid(za, c.K_depth, 3)
+    for T in (np.eye(4), dT, small_motion(0.03, 0.02, -0.01, (0.03, 0.0, -0.02))):
+        for lv in range(3):
+            A, b, e, cnt = fe.icp_step(lv, T.astype(np.float32))
+            A0, b0, e0, cnt0 = ofe.icp_step(meas, pred, c.K_depth, lv, T.astype(np.float32))
+            assert cnt == cnt0 and cnt > 5000
+            assert np.abs(A - A0).max() <= 1e-11 * np.abs(A0).max() and np.abs(b - b0).max() <= 1e-11 * np.abs(A0).max()
+            assert abs(e - e0) <= 1e-11 * e0
+    Tg, rms, cnt = fe.track()
+    To, rms0, cnt0 = ofe.track(meas, pred, c.K_depth)
+    assert np.abs(Tg.astype(np.float64) - To).max() < 2e-6 and abs(rms - rms0) < 1e-7 and abs(cnt - cnt0) <= 5
+    err = np.linalg.inv(dT) @ To
+    assert np.linalg.norm(err[:3, 3]) < 2e-3 and math.degrees(math.acos(min(1.0, (np.trace(err[:3, :3]) - 1) / 2))) < 0.1
+    # tracking lost: a prediction that shows nothing gives no correspondences
+    fe.predict_depth(torch.zeros(c.wd * c.hd, dtype=torch.float32, device="cuda"), c.K_depth)
+    with pytest.raises(vf.VolError):
+        fe.track()
+    fe.close()
+
+
+def test_closed_loop_tracks_the_trajectory():
+    """The paper's per-frame loop with no pose given after the first frame: predict by ray-casting the
+    volume from the last pose, measure, ICP, integrate at the tracked pose.  Config 2 at full size (256^3 / 512^3), 16 frames
+    (1 degree and 21 mm apart).  The CUDA path and the oracle run the same loop independently: their trajectories agree to
+    0.1 mm, and both stay within millimetres of the ground truth."""
+    import torch
+    import paper_1602_06645_b200 as vf
+    c = synth.config(2)
+    n_frames = 16
+    g = vf.Volume(c.dims_geo, c.r, c.origin, c.extent, c.mu, c.w_max)
+    o = oracle.RefVolume(c.dims_geo, c.r, c.origin, c.extent, c.mu, c.w_max)
+    fe = vf.Frontend(c.wd, c.hd, 3)
+    Tg = To = None
+    worst_pair, worst_gt = 0.0, 0.0
+    for i in range(n_frames):
+        depth, rgb, T_true = synth.frame(c, i)
+        dd, dr = to_dev(depth), to_dev(rgb)
+        if i == 0:
+            Tg = To = T_true.astype(np.float32)
+        else:
+            fe.predict(g, Tg, c.K_depth, 0.3, 6.0)
+            fe.measure(dd, c.K_depth)
+            Trel, rms, cnt = fe.track()
+            Tg = synth.rigid32(Tg.astype(np.float64) @ Trel.astype(np.float64))
+            od, _ = o.raycast(c.wd, c.hd, To, c.K_depth, 0.3, 6.0)
+            Trel_o, _, _ = ofe.track(ofe.measure(depth, c.K_depth, 3), ofe.predict(od, c.K_depth, 3), c.K_depth)
+            To = synth.rigid32(To.astype(np.float64) @ Trel_o)
+            assert cnt > 100000 and rms < 3e-3
+        g.integrate(dd, c.wd, c.hd, dr, c.wh, c.hh, Tg, c.K_depth, c.K_rgb, c.T_depth_rgb)
+        o.integrate(depth, rgb, To, c.K_depth, c.K_rgb, c.T_depth_rgb)
+        worst_pair = max(worst_pair, float(np.abs(Tg - To).max()))
+        worst_gt = max(worst_gt, float(np.linalg.norm(Tg[:3, 3] - T_true[:3, 3])))
+    print(f"closed loop: CUDA vs oracle trajectory max |dT| = {worst_pair:.2e}; drift from ground truth after {n_frames} frames {1e3 * worst_gt:.2f} mm")
+    assert worst_pair < 1e-4
+    assert worst_gt < 0.004
+    ang = math.degrees(math.acos(min(1.0, (np.trace(np.linalg.inv(T_true.astype(np.float64))[:3, :3] @ Tg[:3, :3].astype(np.float64)) - 1) / 2)))
+    assert ang < 0.3
+    fe.close(); g.close()

@@ -225,3 +225,17 @@ def test_track_recovers_a_known_motion(quantised):
     A, b, _, _ = fe.icp_step(meas, pred, K, 2, np.eye(4))
     T1, _ = fe.se3_update(np.eye(4), A, b)
     assert np.linalg.norm((np.linalg.inv(dT) @ T1)[:3, 3]) < 0.6 * np.linalg.norm(dT[:3, 3])
+
+
+def test_filtered_prediction_removes_voxel_steps():
+    """F8: a plane with voxel-sized steps (what nearest-voxel ray casting leaves): unfiltered, most forward-difference normals
+    miss the plane's normal by more than the ICP gate of 20 degrees; rounded to millimetres and filtered, nearly all agree."""
+    n = np.array([0.45, 0.2, 0.87], np.float64); n /= np.linalg.norm(n)
+    D = plane_depth_exact(K, W, H, n, 1.3)
+    stepped = (np.floor(D / 0.004) * 0.004).astype(np.float32)                       # 4 mm terraces
+    raw = fe.pyramid(stepped, K, 1)[0][2].astype(np.float64)[8:-8, 8:-8]
+    fil = fe.predict(stepped, K, 1)[0][2].astype(np.float64)[8:-8, 8:-8]
+    good = lambda N: float(((N @ n) > 0.94).mean())
+    assert good(raw) < 0.6 and good(fil) > 0.99
+    q = fe.predict(np.array([[0.0, 1.2344, 70.0, 1.2345]], np.float32), K, 1)[0][0]
+    assert q[0, 0] == 0 and abs(float(q[0, 2]) - 65.535) < 1e-5                       # 0 stays invalid; clamp at 65535 mm
