@@ -366,6 +366,34 @@ def run_ours(args, rank, world, local_rank):
     torch.cuda.synchronize()
     raycast_ms = float(r0.elapsed_time(r1)) / 10.0
     raycast_hit = float((rc_depth > 0).float().mean())
+    # ---- NEXT row: the tracker -- front end of the last frame, prediction ray-cast from the pose before
+    #      it, coarse-to-fine ICP (19 steps, each a kernel and a 232-byte read-back); the tracked pose against the true one
+    tracking = None
+    if not args.stress and nfr >= 2:
+        fe = vf.Frontend(c.wd, c.hd, 3, device=local_rank)
+        T_prev, dd_last = np.asarray(frames[nfr - 2][4], np.float32), frames[nfr - 1][2]
+        tms = {"measure": [], "predict": [], "track": []}
+        evs = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
+        for rep in range(6):
+            evs[0].record(stream)
+            fe.measure(dd_last, c.K_depth, stream=stream)
+            evs[1].record(stream)
+            fe.predict(vol, T_prev, c.K_depth, 0.3, 8.0, stream=stream)
+            evs[2].record(stream)
+            T_rel, trk_rms, trk_cnt = fe.track(stream=stream)
+            evs[3].record(stream)
+            torch.cuda.synchronize()
+            if rep >= 2:
+                for k, name in enumerate(("measure", "predict", "track")):
+                    tms[name].append(float(evs[k].elapsed_time(evs[k + 1])))
+        T_trk = T_prev.astype(np.float64) @ T_rel.astype(np.float64)
+        tracking = {"measure_ms": float(np.mean(tms["measure"])), "predict_ms": float(np.mean(tms["predict"])),
+                    "track_ms": float(np.mean(tms["track"])), "icp_steps": 19, "correspondences": int(trk_cnt), "rms_mm": 1e3 * trk_rms,
+                    "pose_error_mm": 1e3 * float(np.linalg.norm(T_trk[:3, 3] - np.asarray(T_last, np.float64)[:3, 3])),
+                    "motion_mm": 1e3 * float(np.linalg.norm(T_prev[:3, 3] - np.asarray(T_last, np.float32)[:3, 3])),
+                    "note": "vol_frontend_measure / _predict / _track (SURVEY 8(f) rank 4) of the last frame against the fused volumes, "
+                            "not part of the timed step"}
+        fe.close()
     # ---- NEXT row: vol_sample_colour at surface points -- the ray-cast hit points, 8 jittered copies
     #      each (about the density of a texture map with Size_pixel = one colour voxel), as a polygon texture map would ask
     Tl = torch.from_numpy(np.asarray(T_last, np.float32)).cuda()
@@ -446,6 +474,7 @@ def run_ours(args, rank, world, local_rank):
                         "sequence): the copies of frame n + 1 overlap the kernels of frame n",
                 "one_frame_at_a_time": {"value": whole_job_value(nvox, K, world, e2e_serial_ms), "ms_per_step": e2e_serial_ms / K,
                                         "mode": "vol_integrate_host + vol_frame_stats (synchronises) per frame (a live scan)"}},
+        "tracking": tracking,
         "raycast": {"ms": raycast_ms, "rays_per_s": c.wd * c.hd / (raycast_ms * 1e-3), "image": f"{c.wd}x{c.hd}", "hit_fraction": raycast_hit,
                     "note": "vol_raycast of the fused volumes (SURVEY 8(f) rank 1), not part of the timed step"},
         "sample_colour": None if sample_ms is None else {
