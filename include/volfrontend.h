@@ -70,7 +70,7 @@ int vol_frontend_predict(vol_frontend_t *fe, const vol_t *v, const float T_world
  * VOL_ICP_SUMS doubles.  Synchronises `stream`. */
 int vol_frontend_icp_step(vol_frontend_t *fe, int32_t level, const float T_pred_cur[16], double *sums_host, void *stream);
 
-/* F7: the whole coarse-to-fine loop (F5 on the device, F6 on the host in binary64).  T_init: HOST, nullable (identity);
+/* F7: the whole coarse-to-fine loop in one cooperative launch (F5 and F6 on the device, F6 in binary64).  T_init: HOST, nullable (identity);
  * iterations: HOST int32[levels], iterations[l] steps at level l; T_out: HOST, the final estimate current camera ->
  * prediction camera (so T_world_cur = T_world_pred * T_out); rms_out / count_out: nullable, residual and number of
  * correspondences of the last step.  Returns VOL_E_ARG if a step finds fewer than 100 correspondences or A is not positive

@@ -6,6 +6,7 @@
 // depth, vertex and normal maps are bit-identical to oracle/frontend.py.  The ICP sums are binary64.
 #pragma once
 #include <cstdint>
+#include <cooperative_groups.h>
 #include <cuda_runtime.h>
 
 namespace vf {
@@ -109,79 +110,71 @@ __global__ void __launch_bounds__(256) k_vertex_normal(const float *__restrict__
     V[o] = v; N[o] = n;
 }
 
-struct IcpParams {
-    const float4 *V, *N;            // measured maps (current camera's frame)
-    const float4 *Vp, *Np;          // predicted maps (prediction camera's frame)
-    int w, h;
-    LevelK k;
-    float R[9], t[3];               // current camera -> prediction camera
-    float dist2, cos_min;
-    double *sums;                   // ICP_SUMS accumulators (zeroed before the launch)
-};
 
 __device__ __forceinline__ float fe_dot3(float a0, float a1, float a2, float b0, float b1, float b2)
 {
     return __fadd_rn(__fadd_rn(__fmul_rn(a0, b0), __fmul_rn(a1, b1)), __fmul_rn(a2, b2));
 }
 
-// F5: one thread per measured pixel; J and r in binary32 exactly as the oracle, products and sums in binary64; the block
-// reduces through warp shuffles and shared memory and issues one atomic per accumulator.
-__global__ void __launch_bounds__(256) k_icp(const __grid_constant__ IcpParams q)
+// the maps of one level, both sides
+struct IcpLevel {
+    const float4 *V, *N, *Vp, *Np;
+    int w, h;
+    LevelK k;
+};
+
+// F5 for one measured pixel: J and r in binary32 exactly as the oracle; false if the pixel has no correspondence
+__device__ __forceinline__ bool icp_pixel(const IcpLevel &q, const float (&R)[9], const float (&t)[3], float dist2_max, float cos_min,
+                                          int x, int y, float (&J)[6], float &r)
 {
-    const int x = blockIdx.x * 32 + (threadIdx.x & 31), y = blockIdx.y * 8 + (threadIdx.x >> 5);
-    float J[6] = {0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0.0f}, r = 0.0f;
-    bool ok = x < q.w && y < q.h;
-    if (ok) {
-        const size_t o = (size_t)y * q.w + x;
-        const float4 n = __ldg(q.N + o);
-        ok = n.x != 0.0f || n.y != 0.0f || n.z != 0.0f;
-        if (ok) {
-            const float4 v = __ldg(q.V + o);
-            const float px = __fadd_rn(fe_dot3(q.R[0], q.R[1], q.R[2], v.x, v.y, v.z), q.t[0]);
-            const float py = __fadd_rn(fe_dot3(q.R[3], q.R[4], q.R[5], v.x, v.y, v.z), q.t[1]);
-            const float pz = __fadd_rn(fe_dot3(q.R[6], q.R[7], q.R[8], v.x, v.y, v.z), q.t[2]);
-            const float mx = fe_dot3(q.R[0], q.R[1], q.R[2], n.x, n.y, n.z);
-            const float my = fe_dot3(q.R[3], q.R[4], q.R[5], n.x, n.y, n.z);
-            const float mz = fe_dot3(q.R[6], q.R[7], q.R[8], n.x, n.y, n.z);
-            ok = pz > 0.0f;
-            if (ok) {
-                const float u = __fadd_rn(__fmul_rn(q.k.fx, __fdiv_rn(px, pz)), q.k.cx);
-                const float vv = __fadd_rn(__fmul_rn(q.k.fy, __fdiv_rn(py, pz)), q.k.cy);
-                const float xf = floorf(__fadd_rn(u, 0.5f)), yf = floorf(__fadd_rn(vv, 0.5f));
-                ok = xf >= 0.0f && xf < (float)q.w && yf >= 0.0f && yf < (float)q.h;
-                if (ok) {
-                    const size_t op = (size_t)(int)yf * q.w + (int)xf;
-                    const float4 nq = __ldg(q.Np + op);
-                    ok = nq.x != 0.0f || nq.y != 0.0f || nq.z != 0.0f;
-                    if (ok) {
-                        const float4 vq = __ldg(q.Vp + op);
-                        const float dx = __fsub_rn(vq.x, px), dy = __fsub_rn(vq.y, py), dz = __fsub_rn(vq.z, pz);
-                        const float dist2 = fe_dot3(dx, dy, dz, dx, dy, dz);
-                        const float cosang = fe_dot3(mx, my, mz, nq.x, nq.y, nq.z);
-                        ok = !(dist2 > q.dist2) && !(cosang < q.cos_min);
-                        r = fe_dot3(nq.x, nq.y, nq.z, dx, dy, dz);
-                        J[0] = __fsub_rn(__fmul_rn(py, nq.z), __fmul_rn(pz, nq.y));
-                        J[1] = __fsub_rn(__fmul_rn(pz, nq.x), __fmul_rn(px, nq.z));
-                        J[2] = __fsub_rn(__fmul_rn(px, nq.y), __fmul_rn(py, nq.x));
-                        J[3] = nq.x; J[4] = nq.y; J[5] = nq.z;
-                    }
-                }
-            }
-        }
-    }
-    double s[ICP_SUMS];
-    {
-        int idx = 0;
+    const size_t o = (size_t)y * q.w + x;
+    const float4 n = __ldg(q.N + o);
+    if (!(n.x != 0.0f || n.y != 0.0f || n.z != 0.0f)) return false;
+    const float4 v = __ldg(q.V + o);
+    const float px = __fadd_rn(fe_dot3(R[0], R[1], R[2], v.x, v.y, v.z), t[0]);
+    const float py = __fadd_rn(fe_dot3(R[3], R[4], R[5], v.x, v.y, v.z), t[1]);
+    const float pz = __fadd_rn(fe_dot3(R[6], R[7], R[8], v.x, v.y, v.z), t[2]);
+    const float mx = fe_dot3(R[0], R[1], R[2], n.x, n.y, n.z);
+    const float my = fe_dot3(R[3], R[4], R[5], n.x, n.y, n.z);
+    const float mz = fe_dot3(R[6], R[7], R[8], n.x, n.y, n.z);
+    if (!(pz > 0.0f)) return false;
+    const float u = __fadd_rn(__fmul_rn(q.k.fx, __fdiv_rn(px, pz)), q.k.cx);
+    const float vv = __fadd_rn(__fmul_rn(q.k.fy, __fdiv_rn(py, pz)), q.k.cy);
+    const float xf = floorf(__fadd_rn(u, 0.5f)), yf = floorf(__fadd_rn(vv, 0.5f));
+    if (!(xf >= 0.0f && xf < (float)q.w && yf >= 0.0f && yf < (float)q.h)) return false;
+    const size_t op = (size_t)(int)yf * q.w + (int)xf;
+    const float4 nq = __ldg(q.Np + op);
+    if (!(nq.x != 0.0f || nq.y != 0.0f || nq.z != 0.0f)) return false;
+    const float4 vq = __ldg(q.Vp + op);
+    const float dx = __fsub_rn(vq.x, px), dy = __fsub_rn(vq.y, py), dz = __fsub_rn(vq.z, pz);
+    const float dist2 = fe_dot3(dx, dy, dz, dx, dy, dz);
+    const float cosang = fe_dot3(mx, my, mz, nq.x, nq.y, nq.z);
+    if (dist2 > dist2_max || cosang < cos_min) return false;
+    r = fe_dot3(nq.x, nq.y, nq.z, dx, dy, dz);
+    J[0] = __fsub_rn(__fmul_rn(py, nq.z), __fmul_rn(pz, nq.y));
+    J[1] = __fsub_rn(__fmul_rn(pz, nq.x), __fmul_rn(px, nq.z));
+    J[2] = __fsub_rn(__fmul_rn(px, nq.y), __fmul_rn(py, nq.x));
+    J[3] = nq.x; J[4] = nq.y; J[5] = nq.z;
+    return true;
+}
+
+// add one correspondence to a thread's 29 binary64 sums
+__device__ __forceinline__ void icp_accumulate(double (&s)[ICP_SUMS], const float (&J)[6], float r)
+{
+    int idx = 0;
 #pragma unroll
-        for (int i = 0; i < 6; ++i)
+    for (int i = 0; i < 6; ++i)
 #pragma unroll
-            for (int j = i; j < 6; ++j) s[idx++] = ok ? (double)J[i] * (double)J[j] : 0.0;
+        for (int j = i; j < 6; ++j) s[idx++] += (double)J[i] * (double)J[j];
 #pragma unroll
-        for (int i = 0; i < 6; ++i) s[21 + i] = ok ? (double)J[i] * (double)r : 0.0;
-        s[27] = ok ? (double)r * (double)r : 0.0;
-        s[28] = ok ? 1.0 : 0.0;
-    }
-    __shared__ double sh[8][ICP_SUMS];
+    for (int i = 0; i < 6; ++i) s[21 + i] += (double)J[i] * (double)r;
+    s[27] += (double)r * (double)r;
+    s[28] += 1.0;
+}
+
+// block reduction (256 threads) of the per-thread sums, one atomic per accumulator
+__device__ __forceinline__ void icp_block_reduce(const double (&s)[ICP_SUMS], double (*sh)[ICP_SUMS], double *sums)
+{
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
 #pragma unroll
     for (int i = 0; i < ICP_SUMS; ++i) {
@@ -195,7 +188,132 @@ __global__ void __launch_bounds__(256) k_icp(const __grid_constant__ IcpParams q
         double a = 0.0;
 #pragma unroll
         for (int k = 0; k < 8; ++k) a += sh[k][threadIdx.x];
-        if (a != 0.0) atomicAdd(q.sums + threadIdx.x, a);
+        if (a != 0.0) atomicAdd(sums + threadIdx.x, a);
+    }
+    __syncthreads();
+}
+
+struct IcpParams {
+    IcpLevel lv;
+    float R[9], t[3];               // current camera -> prediction camera
+    float dist2, cos_min;
+    double *sums;                   // ICP_SUMS accumulators (zeroed before the launch)
+};
+
+// F5, one step (vol_frontend_icp_step): one thread per measured pixel
+__global__ void __launch_bounds__(256) k_icp(const __grid_constant__ IcpParams q)
+{
+    __shared__ double sh[8][ICP_SUMS];
+    const int x = blockIdx.x * 32 + (threadIdx.x & 31), y = blockIdx.y * 8 + (threadIdx.x >> 5);
+    double s[ICP_SUMS];
+#pragma unroll
+    for (int i = 0; i < ICP_SUMS; ++i) s[i] = 0.0;
+    float J[6], r;
+    if (x < q.lv.w && y < q.lv.h && icp_pixel(q.lv, q.R, q.t, q.dist2, q.cos_min, x, y, J, r)) icp_accumulate(s, J, r);
+    icp_block_reduce(s, sh, q.sums);
+}
+
+// F6 in binary64: A xi = b by Cholesky, then T <- [exp(omega) R, exp(omega) t + v].  T: 12 doubles (3 x 4, row-major).
+// Returns false if A is not positive definite.
+__device__ inline bool icp_se3_update(double *T, const double *sums)
+{
+    double A[6][6], L[6][6], b[6], y[6], xi[6];
+    int idx = 0;
+    for (int i = 0; i < 6; ++i) for (int j = i; j < 6; ++j) { A[i][j] = sums[idx]; A[j][i] = sums[idx]; ++idx; }
+    for (int i = 0; i < 6; ++i) { b[i] = sums[21 + i]; for (int j = 0; j < 6; ++j) L[i][j] = 0.0; }
+    for (int i = 0; i < 6; ++i)
+        for (int j = 0; j <= i; ++j) {
+            double a = A[i][j];
+            for (int k = 0; k < j; ++k) a -= L[i][k] * L[j][k];
+            if (i == j) { if (!(a > 0.0)) return false; L[i][i] = sqrt(a); }
+            else L[i][j] = a / L[j][j];
+        }
+    for (int i = 0; i < 6; ++i) { double a = b[i]; for (int k = 0; k < i; ++k) a -= L[i][k] * y[k]; y[i] = a / L[i][i]; }
+    for (int i = 5; i >= 0; --i) { double a = y[i]; for (int k = i + 1; k < 6; ++k) a -= L[k][i] * xi[k]; xi[i] = a / L[i][i]; }
+    const double ox = xi[0], oy = xi[1], oz = xi[2], th = sqrt(ox * ox + oy * oy + oz * oz);
+    const double Kx[3][3] = {{0.0, -oz, oy}, {oz, 0.0, -ox}, {-oy, ox, 0.0}};
+    double Ri[3][3];
+    const double ca = th < 1e-12 ? 1.0 : sin(th) / th, cb = th < 1e-12 ? 0.0 : (1.0 - cos(th)) / (th * th);
+    for (int i = 0; i < 3; ++i)
+        for (int j = 0; j < 3; ++j) {
+            double k2 = 0.0;
+            for (int k = 0; k < 3; ++k) k2 += Kx[i][k] * Kx[k][j];
+            Ri[i][j] = (i == j ? 1.0 : 0.0) + ca * Kx[i][j] + cb * k2;
+        }
+    double out[12];
+    for (int i = 0; i < 3; ++i) {
+        for (int j = 0; j < 3; ++j) { double a = 0.0; for (int k = 0; k < 3; ++k) a += Ri[i][k] * T[4 * k + j]; out[4 * i + j] = a; }
+        double a = 0.0; for (int k = 0; k < 3; ++k) a += Ri[i][k] * T[4 * k + 3];
+        out[4 * i + 3] = a + xi[3 + i];
+    }
+    for (int i = 0; i < 12; ++i) T[i] = out[i];
+    return true;
+}
+
+// F7 in ONE cooperative launch (vol_frontend_track): every step is a grid-stride pass over the level's pixels into its own
+// set of accumulators (all zeroed before the launch), one grid-wide barrier, and the 6 x 6 solve -- done redundantly by one
+// thread of every block (29 values in, 12 out: cheaper than a second barrier to broadcast the result).
+struct TrackParams {
+    IcpLevel lv[FE_MAX_LEVELS];
+    int levels, iters[FE_MAX_LEVELS], min_count;
+    float dist2, cos_min;
+    double T0[12];                  // initial estimate
+    double *sums;                   // total steps x ICP_SUMS accumulators, zeroed
+    double *out;                    // 12 (T) + rms + count + status (0 ok, 1 too few correspondences, 2 not positive definite) + level
+};
+
+__global__ void __launch_bounds__(256) k_icp_track(const __grid_constant__ TrackParams q)
+{
+    __shared__ double sh[8][ICP_SUMS], shT[16];
+    cooperative_groups::grid_group grid = cooperative_groups::this_grid();
+    double T[12];
+#pragma unroll
+    for (int i = 0; i < 12; ++i) T[i] = q.T0[i];
+    double rms = 0.0, count = 0.0, status = 0.0, at_level = 0.0;
+    int step = 0;
+    for (int l = q.levels - 1; l >= 0 && status == 0.0; --l) {
+        const IcpLevel &lv = q.lv[l];
+        const int tx = (lv.w + 31) / 32, tiles = tx * ((lv.h + 7) / 8);
+        for (int it = 0; it < q.iters[l] && status == 0.0; ++it, ++step) {
+            float R[9], t[3];
+#pragma unroll
+            for (int i = 0; i < 3; ++i) { R[3 * i] = (float)T[4 * i]; R[3 * i + 1] = (float)T[4 * i + 1]; R[3 * i + 2] = (float)T[4 * i + 2]; t[i] = (float)T[4 * i + 3]; }
+            double s[ICP_SUMS];
+#pragma unroll
+            for (int i = 0; i < ICP_SUMS; ++i) s[i] = 0.0;
+            for (int tile = blockIdx.x; tile < tiles; tile += gridDim.x) {
+                const int x = (tile % tx) * 32 + (threadIdx.x & 31), y = (tile / tx) * 8 + (threadIdx.x >> 5);
+                float J[6], r;
+                if (x < lv.w && y < lv.h && icp_pixel(lv, R, t, q.dist2, q.cos_min, x, y, J, r)) icp_accumulate(s, J, r);
+            }
+            double *sums = q.sums + (size_t)step * ICP_SUMS;
+            icp_block_reduce(s, sh, sums);
+            __threadfence();
+            grid.sync();
+            if (threadIdx.x == 0) {                              // one thread per block solves; the others take its result
+                double g[ICP_SUMS];
+#pragma unroll
+                for (int i = 0; i < ICP_SUMS; ++i) g[i] = __ldcg(sums + i);
+                count = g[28];
+                if (count < (double)q.min_count) status = 1.0;
+                else {
+                    rms = sqrt(g[27] / count);
+                    if (!icp_se3_update(T, g)) status = 2.0;
+                }
+#pragma unroll
+                for (int i = 0; i < 12; ++i) shT[i] = T[i];
+                shT[12] = rms; shT[13] = count; shT[14] = status;
+            }
+            __syncthreads();
+#pragma unroll
+            for (int i = 0; i < 12; ++i) T[i] = shT[i];
+            rms = shT[12]; count = shT[13]; status = shT[14]; at_level = (double)l;
+            __syncthreads();
+        }
+    }
+    if (blockIdx.x == 0 && threadIdx.x == 0) {
+        for (int i = 0; i < 12; ++i) q.out[i] = T[i];
+        q.out[12] = rms; q.out[13] = count; q.out[14] = status; q.out[15] = at_level;
     }
 }
 

@@ -1,5 +1,5 @@
 // frontend_host.cuh -- host side of include/volfrontend.h (included at the end of volfusion.cu: same library, same error
-// reporting).  F6 / F7 (the 6 x 6 solve, the pose update, the coarse-to-fine loop) run here in binary64.
+// reporting).  The tracker's whole loop (F5-F7) is one cooperative launch, k_icp_track.
 #pragma once
 #include "../../include/volfrontend.h"
 #include "frontend.cuh"
@@ -16,6 +16,9 @@ struct vol_frontend {
     float *ray_depth;                                       // vol_frontend_predict: the ray-cast depth map
     uint16_t *pred_mm;                                      // F8: the prediction in whole millimetres
     double *sums_dev, *sums_pinned;
+    double *track_sums; size_t track_steps;                 // vol_frontend_track: one set of accumulators per step
+    double *track_out, *track_out_pinned;                   // 16 doubles: T (3 x 4), rms, count, status, level
+    int track_blocks;                                       // co-resident blocks of k_icp_track
 };
 
 static int fe_set_device(const vol_frontend *fe) { CK(cudaSetDevice(fe->device)); return VOL_OK; }
@@ -36,6 +39,9 @@ extern "C" void vol_frontend_destroy(vol_frontend_t *fe)
     if (fe->pred_mm) cudaFree(fe->pred_mm);
     if (fe->sums_dev) cudaFree(fe->sums_dev);
     if (fe->sums_pinned) cudaFreeHost(fe->sums_pinned);
+    if (fe->track_sums) cudaFree(fe->track_sums);
+    if (fe->track_out) cudaFree(fe->track_out);
+    if (fe->track_out_pinned) cudaFreeHost(fe->track_out_pinned);
     cudaGetLastError();
     delete fe;
 }
@@ -76,7 +82,9 @@ extern "C" int vol_frontend_create(vol_frontend_t **out, int32_t w, int32_t h, i
                cudaMalloc(&fe->ray_depth, sizeof(float) * (size_t)w * h) == cudaSuccess &&
                cudaMalloc(&fe->pred_mm, sizeof(uint16_t) * (size_t)w * h) == cudaSuccess &&
                cudaMalloc(&fe->sums_dev, sizeof(double) * vf::ICP_SUMS) == cudaSuccess &&
-               cudaMallocHost(&fe->sums_pinned, sizeof(double) * vf::ICP_SUMS) == cudaSuccess;
+               cudaMallocHost(&fe->sums_pinned, sizeof(double) * vf::ICP_SUMS) == cudaSuccess &&
+               cudaMalloc(&fe->track_out, sizeof(double) * 16) == cudaSuccess &&
+               cudaMallocHost(&fe->track_out_pinned, sizeof(double) * 16) == cudaSuccess;
     for (int s = 0; s < 2 && okc; ++s)
         for (int l = 0; l < levels && okc; ++l) {
             const size_t n = (size_t)(w >> l) * (h >> l);
@@ -87,6 +95,10 @@ extern "C" int vol_frontend_create(vol_frontend_t **out, int32_t w, int32_t h, i
     if (cudaMemcpy(fe->ws, ws, sizeof ws, cudaMemcpyHostToDevice) != cudaSuccess ||
         cudaMemcpy(fe->wr, wr, sizeof(float) * (fe->kmax + 1), cudaMemcpyHostToDevice) != cudaSuccess) return fail(VOL_E_CUDA);
     delete[] wr;
+    int occ = 0, sms = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, vf::k_icp_track, 256, 0) != cudaSuccess || occ < 1 ||
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device) != cudaSuccess) { vol_frontend_destroy(fe); return VOL_E_CUDA; }
+    fe->track_blocks = occ * sms;
     *out = fe;
     return VOL_OK;
 }
@@ -145,15 +157,22 @@ extern "C" int vol_frontend_predict(vol_frontend_t *fe, const vol_t *v, const fl
     return vol_frontend_predict_depth(fe, fe->ray_depth, K, 1, stream);
 }
 
+static vf::IcpLevel fe_level(const vol_frontend *fe, int level)
+{
+    vf::IcpLevel lv;
+    lv.V = fe->V[0][level]; lv.N = fe->N[0][level]; lv.Vp = fe->V[1][level]; lv.Np = fe->N[1][level];
+    lv.w = fe->w >> level; lv.h = fe->h >> level; lv.k = fe->k[1][level];
+    return lv;
+}
+
 static int fe_icp_launch(vol_frontend *fe, int level, const float T[16], cudaStream_t st)
 {
     vf::IcpParams q;
-    q.V = fe->V[0][level]; q.N = fe->N[0][level]; q.Vp = fe->V[1][level]; q.Np = fe->N[1][level];
-    q.w = fe->w >> level; q.h = fe->h >> level; q.k = fe->k[1][level];
+    q.lv = fe_level(fe, level);
     for (int i = 0; i < 3; ++i) { for (int j = 0; j < 3; ++j) q.R[3 * i + j] = T[4 * i + j]; q.t[i] = T[4 * i + 3]; }
     q.dist2 = fe->dist_m * fe->dist_m; q.cos_min = fe->cos_min; q.sums = fe->sums_dev;
     CK(cudaMemsetAsync(fe->sums_dev, 0, sizeof(double) * vf::ICP_SUMS, st));
-    vf::k_icp<<<dim3((q.w + 31) / 32, (q.h + 7) / 8), 256, 0, st>>>(q);
+    vf::k_icp<<<dim3((q.lv.w + 31) / 32, (q.lv.h + 7) / 8), 256, 0, st>>>(q);
     CK(cudaGetLastError());
     CK(cudaMemcpyAsync(fe->sums_pinned, fe->sums_dev, sizeof(double) * vf::ICP_SUMS, cudaMemcpyDeviceToHost, st));
     CK(cudaStreamSynchronize(st));
@@ -176,64 +195,43 @@ extern "C" int vol_frontend_icp_step(vol_frontend_t *fe, int32_t level, const fl
     return VOL_OK;
 }
 
-// F6: A xi = b by Cholesky (A symmetric positive definite), then T <- [exp(omega) R, exp(omega) t + v]; binary64
-static bool fe_se3_update(double T[16], const double *sums)
-{
-    double A[6][6], L[6][6] = {}, b[6], y[6], xi[6];
-    int idx = 0;
-    for (int i = 0; i < 6; ++i) for (int j = i; j < 6; ++j) { A[i][j] = sums[idx]; A[j][i] = sums[idx]; ++idx; }
-    for (int i = 0; i < 6; ++i) b[i] = sums[21 + i];
-    for (int i = 0; i < 6; ++i)
-        for (int j = 0; j <= i; ++j) {
-            double s = A[i][j];
-            for (int k = 0; k < j; ++k) s -= L[i][k] * L[j][k];
-            if (i == j) { if (!(s > 0.0)) return false; L[i][i] = std::sqrt(s); }
-            else L[i][j] = s / L[j][j];
-        }
-    for (int i = 0; i < 6; ++i) { double s = b[i]; for (int k = 0; k < i; ++k) s -= L[i][k] * y[k]; y[i] = s / L[i][i]; }
-    for (int i = 5; i >= 0; --i) { double s = y[i]; for (int k = i + 1; k < 6; ++k) s -= L[k][i] * xi[k]; xi[i] = s / L[i][i]; }
-    const double ox = xi[0], oy = xi[1], oz = xi[2], th = std::sqrt(ox * ox + oy * oy + oz * oz);
-    const double Kx[3][3] = {{0.0, -oz, oy}, {oz, 0.0, -ox}, {-oy, ox, 0.0}};
-    double K2[3][3], Ri[3][3];
-    for (int i = 0; i < 3; ++i) for (int j = 0; j < 3; ++j) { K2[i][j] = 0.0; for (int k = 0; k < 3; ++k) K2[i][j] += Kx[i][k] * Kx[k][j]; }
-    const double a = th < 1e-12 ? 1.0 : std::sin(th) / th, c = th < 1e-12 ? 0.0 : (1.0 - std::cos(th)) / (th * th);
-    for (int i = 0; i < 3; ++i) for (int j = 0; j < 3; ++j) Ri[i][j] = (i == j ? 1.0 : 0.0) + a * Kx[i][j] + c * K2[i][j];
-    double out[16] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 1};
-    for (int i = 0; i < 3; ++i) {
-        for (int j = 0; j < 3; ++j) { double s = 0.0; for (int k = 0; k < 3; ++k) s += Ri[i][k] * T[4 * k + j]; out[4 * i + j] = s; }
-        double s = 0.0; for (int k = 0; k < 3; ++k) s += Ri[i][k] * T[4 * k + 3];
-        out[4 * i + 3] = s + xi[3 + i];
-    }
-    memcpy(T, out, sizeof out);
-    return true;
-}
-
+// F7 in one cooperative launch (k_icp_track: F5 and F6 on the device); one read-back of 128 bytes
 extern "C" int vol_frontend_track(vol_frontend_t *fe, const float T_init[16], const int32_t *iterations, float T_out[16], double *rms_out,
                                   int64_t *count_out, void *stream)
 {
     if (!fe || !iterations || !T_out || !fe->have[0] || !fe->have[1]) return VOL_E_ARG;
     if (T_init && !fe_rigid(T_init)) return VOL_E_ARG;
-    for (int l = 0; l < fe->levels; ++l) if (iterations[l] < 0 || iterations[l] > 1000) return VOL_E_ARG;
+    size_t steps = 0;
+    for (int l = 0; l < fe->levels; ++l) { if (iterations[l] < 0 || iterations[l] > 1000) return VOL_E_ARG; steps += (size_t)iterations[l]; }
     int rc = fe_set_device(fe); if (rc) return rc;
-    double T[16] = {1, 0, 0, 0, 0, 1, 0, 0, 0, 0, 1, 0, 0, 0, 0, 1};
-    if (T_init) for (int i = 0; i < 16; ++i) T[i] = (double)T_init[i];
-    double rms = 0.0; int64_t count = 0;
-    int result = VOL_OK;
-    for (int l = fe->levels - 1; l >= 0 && result == VOL_OK; --l)
-        for (int it = 0; it < iterations[l]; ++it) {
-            float T32[16];
-            for (int i = 0; i < 16; ++i) T32[i] = (float)T[i];
-            rc = fe_icp_launch(fe, l, T32, (cudaStream_t)stream); if (rc) return rc;
-            const double *s = fe->sums_pinned;
-            count = (int64_t)s[28];
-            if (count < 100) { snprintf(g_err, sizeof g_err, "vol_frontend_track: %lld correspondences at level %d", (long long)count, l); result = VOL_E_ARG; break; }
-            rms = std::sqrt(s[27] / (double)count);
-            if (!fe_se3_update(T, s)) { snprintf(g_err, sizeof g_err, "vol_frontend_track: normal equations not positive definite"); result = VOL_E_ARG; break; }
-        }
-    for (int i = 0; i < 16; ++i) T_out[i] = (float)T[i];
-    if (rms_out) *rms_out = rms;
-    if (count_out) *count_out = count;
-    return result;
+    cudaStream_t st = (cudaStream_t)stream;
+    if (steps > fe->track_steps) {
+        if (fe->track_sums) { CK(cudaDeviceSynchronize()); cudaFree(fe->track_sums); fe->track_sums = nullptr; fe->track_steps = 0; }
+        CK(cudaMalloc(&fe->track_sums, steps * vf::ICP_SUMS * sizeof(double)));
+        fe->track_steps = steps;
+    }
+    vf::TrackParams q;
+    memset(&q, 0, sizeof q);
+    for (int l = 0; l < fe->levels; ++l) { q.lv[l] = fe_level(fe, l); q.iters[l] = iterations[l]; }
+    q.levels = fe->levels; q.min_count = 100;
+    q.dist2 = fe->dist_m * fe->dist_m; q.cos_min = fe->cos_min;
+    for (int i = 0; i < 12; ++i) q.T0[i] = T_init ? (double)T_init[i] : (i % 5 == 0 ? 1.0 : 0.0);
+    q.sums = fe->track_sums; q.out = fe->track_out;
+    if (steps > 0) CK(cudaMemsetAsync(fe->track_sums, 0, steps * vf::ICP_SUMS * sizeof(double), st));
+    const int tiles0 = ((fe->w + 31) / 32) * ((fe->h + 7) / 8);
+    const int blocks = fe->track_blocks < tiles0 ? fe->track_blocks : tiles0;
+    void *args[] = {&q};
+    CK(cudaLaunchCooperativeKernel((const void *)vf::k_icp_track, dim3(blocks), dim3(256), args, 0, st));
+    CK(cudaMemcpyAsync(fe->track_out_pinned, fe->track_out, sizeof(double) * 16, cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    const double *o = fe->track_out_pinned;
+    for (int i = 0; i < 12; ++i) T_out[i] = (float)o[i];
+    T_out[12] = T_out[13] = T_out[14] = 0.0f; T_out[15] = 1.0f;
+    if (rms_out) *rms_out = o[12];
+    if (count_out) *count_out = (int64_t)o[13];
+    if (o[14] == 1.0) { snprintf(g_err, sizeof g_err, "vol_frontend_track: %lld correspondences at level %d", (long long)o[13], (int)o[15]); return VOL_E_ARG; }
+    if (o[14] == 2.0) { snprintf(g_err, sizeof g_err, "vol_frontend_track: normal equations not positive definite"); return VOL_E_ARG; }
+    return VOL_OK;
 }
 
 extern "C" int vol_frontend_maps(const vol_frontend_t *fe, int32_t which, int32_t level, float *depth_host, float *vertex_host,
