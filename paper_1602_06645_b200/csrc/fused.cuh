@@ -114,7 +114,7 @@ __device__ __forceinline__ void geometry_tile(const Params &p, uint32_t item, in
     const bool inside = i0 < p.nx && j < p.ny;
     const unsigned lanes = __ballot_sync(0xffffffffu, inside);    // ragged tile: the votes below name only these lanes
     if (!inside) return;
-    const int nl = min(TZ, p.nz - gz0);
+    int nl = min(TZ, p.nz - gz0);
     // per-column bases of eq. 5: fma(R_1, py, fma(R_0, px, t)) -- the z term is added per layer with one fma each
     const float py = __fmaf_rn((float)j + 0.5f, p.vs, p.oy);
     float bX[4], bY[4], bZ[4];
@@ -145,6 +145,11 @@ __device__ __forceinline__ void geometry_tile(const Params &p, uint32_t item, in
         }
         return;
     }
+    // the classification tested the tile's two z-halves separately (bits 0 and 1 of sub): a half that failed holds no
+    // voxel this frame can update, and its four layers are skipped
+    const int zb = (sub & 1) ? 0 : TZ / 2;
+    if (!(sub & 2)) nl = min(nl, TZ / 2);
+    ptr = reinterpret_cast<uint4 *>(reinterpret_cast<uint32_t *>(ptr) + (size_t)zb * layer);
     const float fx = p.fx, fy = p.fy, cx = p.cx, cy = p.cy;
     const float neg_mu = p.neg_mu, inv_mu = p.inv_mu;
     const uint32_t wd = (uint32_t)p.wd, wbits = __float_as_uint(p.wd_f), hbits = __float_as_uint(p.hd_f), koff = 0x4B400000u * (wd + 1u);
@@ -222,8 +227,8 @@ __device__ __forceinline__ void geometry_tile(const Params &p, uint32_t item, in
     float ZA[4], ZB[4], LA[4], LB[4]; uint32_t dA[4], dB[4];
     // the voxel stream bypasses L1 (__ldcg): every line is used once, and L1 is better spent on the depth image
     uint4 curA = __ldcg(ptr), curB = curA;
-    project_layer(0, ZA, dA, LA);
-    for (int z = 0; z < nl; z += 2) {
+    project_layer(zb, ZA, dA, LA);
+    for (int z = zb; z < nl; z += 2) {
         uint4 *pB = reinterpret_cast<uint4 *>(reinterpret_cast<uint32_t *>(ptr) + layer);
         uint4 *pA2 = reinterpret_cast<uint4 *>(reinterpret_cast<uint32_t *>(pB) + layer);
         const bool hasB = z + 1 < nl, hasA2 = z + 2 < nl;
@@ -244,7 +249,8 @@ __device__ __forceinline__ void geometry_prefetch(const Params &p, uint32_t item
     int ttx, tty, ttz, sub;
     item_unpack(item, ttx, tty, ttz, sub);
     const int j = tty * TY + (lane & 3), lz = ttz * TZ + (lane >> 2);
-    if (j < p.ny && lz < p.local_nz)
+    const bool wanted = (item & ITEM_NEAR) != 0u || ((sub >> ((lane >> 2) / (TZ / 2))) & 1) != 0;   // its z-half is processed
+    if (j < p.ny && lz < p.local_nz && wanted)
         asm volatile("prefetch.global.L2 [%0];" ::"l"(p.geo + ((size_t)lz * p.ny + j) * p.nx + ttx * TX));
 }
 

@@ -357,7 +357,7 @@ __global__ void __launch_bounds__(256) k_mark_classify(const __grid_constant__ P
             const float dx = ((float)bx - 0.5f * (float)(SUBX - 1)) * sx, dz = ((float)bz - 0.5f * (float)(SUBZ - 1)) * sz;
             if (box_may_update(p, s_c[sv][0] + p.R[0] * dx + p.R[2] * dz, s_c[sv][1] + p.R[3] * dx + p.R[5] * dz,
                                s_c[sv][2] + p.R[6] * dx + p.R[8] * dz, p.sub_ex, p.sub_ey, p.sub_ez) != 0)
-                s_pass[sv] = 1u;                          // benign race: every writer stores 1
+                atomicOr(&s_pass[sv], 1u << bz);          // bit bz: the tile's z-half bz can hold an updated voxel
         }
     }
     __syncthreads();
@@ -377,7 +377,7 @@ __global__ void __launch_bounds__(256) k_mark_classify(const __grid_constant__ P
     if (lane == 0 && mg) bg = atomicAdd(&p.ctrl[CTRL_NGEO], (uint32_t)__popc(mg));
     if (lane == 0 && mn) bn = atomicAdd(&p.ctrl[CTRL_NNEAR], (uint32_t)__popc(mn));
     bg = __shfl_sync(0xffffffffu, bg, 0); bn = __shfl_sync(0xffffffffu, bn, 0);
-    if (geo) p.work_geo[bg + __popc(mg & lt)] = item_pack(ttx, tty, ttz, 0);
+    if (geo) p.work_geo[bg + __popc(mg & lt)] = item_pack(ttx, tty, ttz, (int)s_pass[t]);   // sub = z-half mask
     if (geo_near) p.work_geo[(uint32_t)p.n_tiles - 1u - (bn + __popc(mn & lt))] = item_pack(ttx, tty, ttz, 0) | ITEM_NEAR;
 }
 
