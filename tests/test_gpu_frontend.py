@@ -151,3 +151,33 @@ def test_closed_loop_tracks_the_trajectory():
     ang = math.degrees(math.acos(min(1.0, (np.trace(np.linalg.inv(T_true.astype(np.float64))[:3, :3] @ Tg[:3, :3].astype(np.float64)) - 1) / 2)))
     assert ang < 0.3
     fe.close(); g.close()
+
+
+def test_closed_loop_on_the_benchmark_workload():
+    """The same loop on config 3 at full size (512^3 / 1024^3, the benchmark workload), CUDA path only, 60 frames of the
+    jittered orbit (1.3 degrees and 33 mm apart, about 2 m of camera travel): the tracked trajectory stays within a few
+    millimetres of the true one.  (Config 4 is left out on purpose: its scene is a surface of revolution about the axis the
+    camera orbits, so the motion leaves the depth images unchanged and no geometric tracker can observe it.)"""
+    import paper_1602_06645_b200 as vf
+    c = synth.config(3)
+    g = vf.Volume(c.dims_geo, c.r, c.origin, c.extent, c.mu, c.w_max)
+    fe = vf.Frontend(c.wd, c.hd, 3)
+    Tg, worst, worst_ang = None, 0.0, 0.0
+    for i in range(60):
+        depth, rgb, T_true = synth.frame(c, i)
+        dd, dr = to_dev(depth), to_dev(rgb)
+        if i == 0:
+            Tg = T_true.astype(np.float32)
+        else:
+            fe.predict(g, Tg, c.K_depth, 0.3, 8.0)
+            fe.measure(dd, c.K_depth)
+            Trel, rms, cnt = fe.track()
+            assert cnt > 150000 and rms < 1.5e-3
+            Tg = synth.rigid32(Tg.astype(np.float64) @ Trel.astype(np.float64))
+        g.integrate(dd, c.wd, c.hd, dr, c.wh, c.hh, Tg, c.K_depth, c.K_rgb, c.T_depth_rgb)
+        err = np.linalg.inv(T_true.astype(np.float64)) @ Tg.astype(np.float64)
+        worst = max(worst, float(np.linalg.norm(Tg[:3, 3] - T_true[:3, 3])))
+        worst_ang = max(worst_ang, math.degrees(math.acos(min(1.0, (np.trace(err[:3, :3]) - 1) / 2))))
+    print(f"config 3 closed loop, 60 frames: worst drift {1e3 * worst:.2f} mm, {worst_ang:.3f} degrees")
+    assert worst < 0.005 and worst_ang < 0.3
+    fe.close(); g.close()
