@@ -110,11 +110,14 @@ __device__ __forceinline__ void geometry_tile(const Params &p, uint32_t item, in
     int ttx, tty, ttz, sub;
     item_unpack(item, ttx, tty, ttz, sub);
     const int i0 = ttx * TX + 4 * (lane & 7), j = tty * TY + (lane >> 3);
-    const int gz0 = local_to_global_tz(p, ttz) * TZ, lz0 = ttz * TZ;
+    // the classification tested the tile's two z-halves separately (bits 0 and 1 of sub): a half that failed holds no
+    // voxel this frame can update, and its four layers are left out -- the march starts at layer zb and covers nl layers
+    const int zb = (near || (sub & 1)) ? 0 : TZ / 2;
+    const int gz0 = local_to_global_tz(p, ttz) * TZ + zb, lz0 = ttz * TZ + zb;
     const bool inside = i0 < p.nx && j < p.ny;
     const unsigned lanes = __ballot_sync(0xffffffffu, inside);    // ragged tile: the votes below name only these lanes
     if (!inside) return;
-    int nl = min(TZ, p.nz - gz0);
+    const int nl = min((near || (sub & 2)) ? TZ - zb : TZ / 2, p.nz - gz0);
     // per-column bases of eq. 5: fma(R_1, py, fma(R_0, px, t)) -- the z term is added per layer with one fma each
     const float py = __fmaf_rn((float)j + 0.5f, p.vs, p.oy);
     float bX[4], bY[4], bZ[4];
@@ -145,11 +148,6 @@ __device__ __forceinline__ void geometry_tile(const Params &p, uint32_t item, in
         }
         return;
     }
-    // the classification tested the tile's two z-halves separately (bits 0 and 1 of sub): a half that failed holds no
-    // voxel this frame can update, and its four layers are skipped
-    const int zb = (sub & 1) ? 0 : TZ / 2;
-    if (!(sub & 2)) nl = min(nl, TZ / 2);
-    ptr = reinterpret_cast<uint4 *>(reinterpret_cast<uint32_t *>(ptr) + (size_t)zb * layer);
     const float fx = p.fx, fy = p.fy, cx = p.cx, cy = p.cy;
     const float neg_mu = p.neg_mu, inv_mu = p.inv_mu;
     const uint32_t wd = (uint32_t)p.wd, wbits = __float_as_uint(p.wd_f), hbits = __float_as_uint(p.hd_f), koff = 0x4B400000u * (wd + 1u);
@@ -227,8 +225,8 @@ __device__ __forceinline__ void geometry_tile(const Params &p, uint32_t item, in
     float ZA[4], ZB[4], LA[4], LB[4]; uint32_t dA[4], dB[4];
     // the voxel stream bypasses L1 (__ldcg): every line is used once, and L1 is better spent on the depth image
     uint4 curA = __ldcg(ptr), curB = curA;
-    project_layer(zb, ZA, dA, LA);
-    for (int z = zb; z < nl; z += 2) {
+    project_layer(0, ZA, dA, LA);
+    for (int z = 0; z < nl; z += 2) {
         uint4 *pB = reinterpret_cast<uint4 *>(reinterpret_cast<uint32_t *>(ptr) + layer);
         uint4 *pA2 = reinterpret_cast<uint4 *>(reinterpret_cast<uint32_t *>(pB) + layer);
         const bool hasB = z + 1 < nl, hasA2 = z + 2 < nl;
