@@ -214,26 +214,40 @@ __global__ void __launch_bounds__(256) k_icp(const __grid_constant__ IcpParams q
 }
 
 // F6 in binary64: A xi = b by Cholesky, then T <- [exp(omega) R, exp(omega) t + v].  T: 12 doubles (3 x 4, row-major).
-// Returns false if A is not positive definite.
+// Returns false if A is not positive definite.  One thread of every block runs this between two steps while the others
+// wait, so the chain of slow binary64 operations is kept short: one rsqrt per column instead of a sqrt and the divisions,
+// and the two Rodrigues coefficients from their series (ICP increments are far below 0.1 rad; sin / cos otherwise).
 __device__ inline bool icp_se3_update(double *T, const double *sums)
 {
-    double A[6][6], L[6][6], b[6], y[6], xi[6];
+    double A[6][6], L[6][6], inv[6], b[6], y[6], xi[6];
     int idx = 0;
     for (int i = 0; i < 6; ++i) for (int j = i; j < 6; ++j) { A[i][j] = sums[idx]; A[j][i] = sums[idx]; ++idx; }
     for (int i = 0; i < 6; ++i) { b[i] = sums[21 + i]; for (int j = 0; j < 6; ++j) L[i][j] = 0.0; }
-    for (int i = 0; i < 6; ++i)
-        for (int j = 0; j <= i; ++j) {
+    for (int j = 0; j < 6; ++j) {                                    // column by column
+        double d = A[j][j];
+        for (int k = 0; k < j; ++k) d -= L[j][k] * L[j][k];
+        if (!(d > 0.0)) return false;
+        inv[j] = rsqrt(d);
+        L[j][j] = d * inv[j];
+        for (int i = j + 1; i < 6; ++i) {
             double a = A[i][j];
             for (int k = 0; k < j; ++k) a -= L[i][k] * L[j][k];
-            if (i == j) { if (!(a > 0.0)) return false; L[i][i] = sqrt(a); }
-            else L[i][j] = a / L[j][j];
+            L[i][j] = a * inv[j];
         }
-    for (int i = 0; i < 6; ++i) { double a = b[i]; for (int k = 0; k < i; ++k) a -= L[i][k] * y[k]; y[i] = a / L[i][i]; }
-    for (int i = 5; i >= 0; --i) { double a = y[i]; for (int k = i + 1; k < 6; ++k) a -= L[k][i] * xi[k]; xi[i] = a / L[i][i]; }
-    const double ox = xi[0], oy = xi[1], oz = xi[2], th = sqrt(ox * ox + oy * oy + oz * oz);
+    }
+    for (int i = 0; i < 6; ++i) { double a = b[i]; for (int k = 0; k < i; ++k) a -= L[i][k] * y[k]; y[i] = a * inv[i]; }
+    for (int i = 5; i >= 0; --i) { double a = y[i]; for (int k = i + 1; k < 6; ++k) a -= L[k][i] * xi[k]; xi[i] = a * inv[i]; }
+    const double ox = xi[0], oy = xi[1], oz = xi[2], t2 = ox * ox + oy * oy + oz * oz;
+    double ca, cb;                                                   // sin(th) / th and (1 - cos(th)) / th^2, th^2 = t2
+    if (t2 < 1e-2) {
+        ca = 1.0 - t2 / 6.0 * (1.0 - t2 / 20.0 * (1.0 - t2 / 42.0 * (1.0 - t2 / 72.0 * (1.0 - t2 / 110.0))));
+        cb = 0.5 - t2 / 24.0 * (1.0 - t2 / 30.0 * (1.0 - t2 / 56.0 * (1.0 - t2 / 90.0 * (1.0 - t2 / 132.0))));
+    } else {
+        const double th = sqrt(t2);
+        ca = sin(th) / th; cb = (1.0 - cos(th)) / t2;
+    }
     const double Kx[3][3] = {{0.0, -oz, oy}, {oz, 0.0, -ox}, {-oy, ox, 0.0}};
     double Ri[3][3];
-    const double ca = th < 1e-12 ? 1.0 : sin(th) / th, cb = th < 1e-12 ? 0.0 : (1.0 - cos(th)) / (th * th);
     for (int i = 0; i < 3; ++i)
         for (int j = 0; j < 3; ++j) {
             double k2 = 0.0;
