@@ -38,7 +38,8 @@ __device__ __forceinline__ RaySample ray_sample(const Params &p, const float (&d
     tile = -1; s.i = s.j = s.k = 0;
     if (inside) {
         s.i = (int)fi; s.j = (int)fj; s.k = (int)fk;
-        tile = ((s.k / TZ) * p.tiles_y + s.j / TY) * p.tiles_x + s.i / TX;      // the voxel itself is read by ray_voxel() when needed
+        // (indices are non-negative here: unsigned shifts instead of signed divisions -- the kernel is issue-bound)
+        tile = (int)((((unsigned)s.k / TZ) * (unsigned)p.tiles_y + (unsigned)s.j / TY) * (unsigned)p.tiles_x + (unsigned)s.i / TX);   // the voxel itself is read by ray_voxel() when needed
     }
     return s;
 }
@@ -77,9 +78,10 @@ __global__ void __launch_bounds__(64) k_raycast(const __grid_constant__ Params p
         }
     }
     // culling only: the ray in grid coordinates, g(t) = go + t * gd, for the tile-exit computation
-    float go[3], gd[3];
+    // (1 / gd is taken once per ray: the exit parameter only has to be right to a few hundredths of a voxel)
+    float go[3], gd[3], rgd[3];
 #pragma unroll
-    for (int a = 0; a < 3; ++a) { go[a] = (ow[a] - org[a]) * inv_vs; gd[a] = dw[a] * inv_vs; }
+    for (int a = 0; a < 3; ++a) { go[a] = (ow[a] - org[a]) * inv_vs; gd[a] = dw[a] * inv_vs; rgd[a] = fabsf(gd[a]) > 1e-9f ? 1.0f / gd[a] : 0.0f; }
     const int tdim[3] = {TX, TY, TZ};
     float depth = 0.0f;
     if (ta <= tb) {
@@ -93,8 +95,9 @@ __global__ void __launch_bounds__(64) k_raycast(const __grid_constant__ Params p
             if (cur.t > q.t_far) break;
             if (!inside) { prev = cur; prev_pending = false; ++k; continue; }             // unknown sample
             // coarse level first: a brick of BRICK^3 voxels (1 x 8 x 4 tiles) without such a voxel is crossed in one jump
-            const bool brick_free = __ldg(p.brick_neg + ((cur.k / BRICK) * p.bricks_y + cur.j / BRICK) * p.bricks_x + cur.i / BRICK) == 0;
-            if (brick_free || __ldg(p.tile_neg + tile) == 0) {
+            const unsigned brick = (((unsigned)cur.k / BRICK) * (unsigned)p.bricks_y + (unsigned)cur.j / BRICK) * (unsigned)p.bricks_x + (unsigned)cur.i / BRICK;
+            const bool brick_free = __ldg(p.brick_neg + brick) == 0;
+            if (brick_free || __ldg(p.tile_neg + (unsigned)tile) == 0) {
                 // no observed voxel with tsdf <= 0 in this brick / tile: jump to the last sample safely inside it
                 // (the tile's box comes from the sample's canonical voxel indices, the exit from free-form arithmetic: if
                 // the two disagree at a tile boundary the exit lies behind the sample and nothing is skipped)
@@ -103,9 +106,9 @@ __global__ void __launch_bounds__(64) k_raycast(const __grid_constant__ Params p
 #pragma unroll
                 for (int a = 0; a < 3; ++a) {
                     const int bd = brick_free ? BRICK : tdim[a];
-                    const float lo = (float)((vox[a] / bd) * bd);
-                    if (gd[a] > 1e-9f) t_exit = fminf(t_exit, (lo + (float)bd - 0.05f - go[a]) / gd[a]);
-                    else if (gd[a] < -1e-9f) t_exit = fminf(t_exit, (lo + 0.05f - go[a]) / gd[a]);
+                    const float lo = (float)(vox[a] & ~(bd - 1));                           // box sizes are powers of two
+                    if (gd[a] > 1e-9f) t_exit = fminf(t_exit, (lo + (float)bd - 0.05f - go[a]) * rgd[a]);
+                    else if (gd[a] < -1e-9f) t_exit = fminf(t_exit, (lo + 0.05f - go[a]) * rgd[a]);
                 }
                 const int kk = (int)fminf(floorf((t_exit - q.t_near) * inv_vs) - 1.0f, (float)k1);
                 k = max(k, kk) + 1;
