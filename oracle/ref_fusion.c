@@ -15,6 +15,10 @@
  *                       voxels per axis.  Readings A11 (which point maps to the HD image) and A12
  *                       (u8 weight encoding of eq. 10) are conventions ** parity unpinned ** by the paper.
  *
+ *   ray casting (ref_raycast, readings R1-R6), colour sampling (ref_sample_colour*, readings S1-S2) and the alternative
+ *                       readings selected by ref_vol_t.variant: the paper gives no definition for any of them
+ *                       ** parity unpinned ** by the paper; pinned by closed forms (tests/test_oracle_*.py).
+ *
  * Canonical arithmetic: IEEE binary32, round-to-nearest-even, no implicit contraction
  * (-ffp-contract=off); fmaf() where the spec says fma; / and sqrtf correctly rounded; rintf = half-even.
  *
