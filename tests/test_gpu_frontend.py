@@ -181,3 +181,37 @@ def test_closed_loop_on_the_benchmark_workload():
     print(f"config 3 closed loop, 60 frames: worst drift {1e3 * worst:.2f} mm, {worst_ang:.3f} degrees")
     assert worst < 0.005 and worst_ang < 0.3
     fe.close(); g.close()
+
+
+def test_frontend_rejects_bad_calls():
+    """Validation precedes any launch: maps that do not exist yet, levels out of range, a non-rigid estimate, a negative
+    iteration count, a volume on shards -- each is VOL_E_ARG and leaves the front end usable."""
+    import torch
+    import paper_1602_06645_b200 as vf
+    c = synth.config(2)                                           # (not config 1: a lone sphere leaves its rotation unobservable)
+    fe = vf.Frontend(c.wd, c.hd, 2)
+    with pytest.raises(vf.VolError):
+        fe.track(iterations=(1, 1))                               # nothing measured or predicted yet
+    with pytest.raises(vf.VolError):
+        fe.maps(0, 0)
+    depth, _, T = synth.frame(c, 0, want_rgb=False)
+    fe.measure(to_dev(depth), c.K_depth)
+    with pytest.raises(vf.VolError):
+        fe.icp_step(0, np.eye(4, dtype=np.float32))               # no prediction yet
+    z, _ = synth.render(c.prims, c.K_depth, T.astype(np.float64), c.wd, c.hd, True, False)
+    fe.predict_depth(torch.from_numpy(z).cuda(), c.K_depth)
+    bad = np.eye(4, dtype=np.float32); bad[0, 0] = 1.5
+    for call in (lambda: fe.icp_step(2, np.eye(4, dtype=np.float32)), lambda: fe.icp_step(-1, np.eye(4, dtype=np.float32)),
+                 lambda: fe.icp_step(0, bad), lambda: fe.track(T_init=bad, iterations=(1, 1)), lambda: fe.track(iterations=(1, -1)),
+                 lambda: fe.maps(2, 0), lambda: fe.maps(0, 2)):
+        with pytest.raises(vf.VolError) as e:
+            call()
+        assert e.value.code == vf.VOL_E_ARG
+    shard = vf.Volume((32, 32, 32), 1, c.origin, c.extent, 0.1, 8, shard_rank=0, shard_world=2)
+    with pytest.raises(vf.VolError):
+        fe.predict(shard, T, c.K_depth, 0.3, 3.0)
+    shard.close()
+    T_rel, rms, cnt = fe.track(iterations=(4, 2))                 # still works: measured frame against its own exact depth
+    assert cnt > 1000 and np.abs(T_rel - np.eye(4)).max() < 2e-3
+    assert fe.track(iterations=(0, 0))[0].tolist() == np.eye(4).tolist()     # no steps: the initial estimate comes back
+    fe.close()
