@@ -79,3 +79,29 @@ def test_variant_is_live_and_reported():
     for bad in (3, 5, 6, 7, 8, -1):                       # combinations and unknown values are rejected
         with pytest.raises(vf.VolError):
             vf.Volume(c.dims_geo, c.r, c.origin, c.extent, c.mu, c.w_max, variant=bad)
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_variant_shards_reassemble(variant):
+    """The switches under z-slab sharding: three shards hold exactly the slabs of the unsharded volume of the same variant
+    (which is byte-identical to the oracle's)."""
+    import paper_1602_06645_b200 as vf
+    from parity_util import to_dev
+    c = synth.config(1).scaled(40, 2)
+    c.dims_geo = (40, 40, 44)                          # 6 slabs, the last one partial
+    g, o = make_pair(c, variant=variant)
+    shards = [vf.Volume(c.dims_geo, c.r, c.origin, c.extent, c.mu, c.w_max, shard_rank=k, shard_world=3, variant=variant) for k in range(3)]
+    for fi in (0, 3):
+        depth, rgb, T = synth.frame(c, fi)
+        integrate_both(g, o, c, depth, rgb, T)
+        dd, dr = to_dev(depth), to_dev(rgb)
+        for s in shards:
+            s.integrate(dd, c.wd, c.hd, dr, c.wh, c.hh, T, c.K_depth, c.K_rgb, c.T_depth_rgb)
+    geo, col = compare_states(g, o, f"unsharded, variant {variant}")
+    nz, r, S = 44, c.r, vf.VOL_SLAB
+    for k, s in enumerate(shards):
+        sg, sc = s.download()
+        layers = [z for z in range(nz) if (z // S) % 3 == k]
+        assert np.array_equal(sg, geo[layers])
+        assert np.array_equal(sc, col[[z for z in range(nz * r) if (z // (S * r)) % 3 == k]])
+        s.close()
