@@ -315,7 +315,7 @@ def run_ours(args, rank, world, local_rank):
     #      kernels of frame n run (two staging sets), and the step's result (the 64-byte statistics record) comes back with
     #      vol_frame_stats_async into pinned memory, in stream order.
     vol.reset(stream)
-    raw_stats = torch.zeros((max(K, W), 8), dtype=torch.int64).pin_memory()
+    raw_stats = torch.zeros((max(K, W), 16), dtype=torch.int64).pin_memory()
     for i in range(W):                                            # warm-up through the same entry point (staging buffers exist)
         hd_, hr_, _, _, T = frames[i]
         vol.integrate_host(hd_, hr_, T, c.K_depth, c.K_rgb, c.T_depth_rgb, stream=stream)
@@ -469,7 +469,7 @@ def run_ours(args, rank, world, local_rank):
                      "issue": issue_roofline(traffic_key, float(fused_ms.mean()),
                                              (clocks or {}).get("sm_mhz"))},
         "e2e": {"value": e2e_value, "unit": UNIT, "ms_per_step": e2e_ms / K, "h2d_bytes_per_step": frame_bytes,
-                "d2h_bytes_per_step": 64,
+                "d2h_bytes_per_step": 128,
                 "mode": "vol_integrate_host + vol_frame_stats_async per frame, frames enqueued back to back (a recorded "
                         "sequence): the copies of frame n + 1 overlap the kernels of frame n",
                 "one_frame_at_a_time": {"value": whole_job_value(nvox, K, world, e2e_serial_ms), "ms_per_step": e2e_serial_ms / K,

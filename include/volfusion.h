@@ -37,7 +37,7 @@ extern "C" {
 #endif
 
 #define VOL_OK       0
-#define VOL_E_ARG   -1   /* null pointer, dims <= 0, dims_geo[0] % 4 != 0, dims_geo > 4096 x 2048 x 2048 (per shard), r not in 1..4, mu <= 0, unknown or combined variant, w_max not in 1..512,
+#define VOL_E_ARG   -1   /* null pointer, dims <= 0, dims_geo > 4096 x 2048 x 2048 (per shard), r not in 1..4, mu <= 0, unknown or combined variant, w_max not in 1..512,
                             non-zero skew, non-rigid T, image size <= 0, buffer too small, bad shard */
 #define VOL_E_OOM   -2   /* device allocation failed */
 #define VOL_E_CUDA  -3   /* a CUDA call failed (sticky: see vol_strerror) */
@@ -85,20 +85,30 @@ typedef struct {
     void    *geo_dev, *col_dev;         /* DEVICE pointers of this shard's storage */
 } vol_info_t;
 
-/* Per-frame statistics of the last vol_integrate* call.  Tile figures are always valid; the four voxel counters
- * and cells_col are only filled when counting is enabled (vol_set_counting), otherwise 0.
+/* Per-frame statistics of the last vol_integrate* call.  tiles_total, tiles_geo and items_col are always valid; everything
+ * else is only filled when counting is enabled (vol_set_counting), otherwise 0.
  * A voxel is *read* when the method reaches the load of its stored word (geometry: passes the frustum, non-zero-depth
  * and truncation tests; colour: passes the sigma gate with a valid view weight) and *changed* when the stored word
- * differs after the update. */
+ * differs after the update.  The *_sectors_* figures count the distinct 32-byte sectors (8 x-adjacent words,
+ * aligned in this shard's storage) that hold at least one read / changed voxel: the DRAM granularity of the same sets. */
 typedef struct {
     uint64_t geo_read, geo_changed, col_read, col_changed;
     uint32_t tiles_total;   /* geometry tiles owned by this shard */
-    uint32_t tiles_geo;     /* geometry tiles (32x4x8 voxels) whose TSDF voxels were visited */
+    uint32_t tiles_geo;     /* geometry tiles (32x4x8 voxels) with at least one sub-box to visit */
     uint32_t items_col;     /* colour work items (non-zero nibbles of the shell-mark words: up to 4 colour cells each) */
-    uint32_t cells_col;     /* colour cells (8x4x4 colour voxels) visited; only when counting is enabled */
+    uint32_t cells_col;     /* colour cells (8x4x4 colour voxels) visited */
+    uint64_t geo_sectors_read, geo_sectors_written, col_sectors_read, col_sectors_written;
+    uint64_t geo_visited;   /* geometry voxels the kernel projected (the read ones are a subset) */
+    uint64_t col_gated;     /* colour voxels that went through the sigma gate (S4-S5; the read ones are a subset) */
+    uint64_t reserved64;
+    uint32_t subs_geo;      /* geometry sub-boxes (8x4x4 voxels) visited */
+    uint32_t jobs_mark;     /* shell-mark jobs (one or two per 4 x 4 pixel patch with colour-eligible pixels) */
 } vol_stats_t;
 
-/* Create a volume pair.  dims_geo: HOST int32[3] (dims_geo[0] must be a multiple of 4); r in 1..4; origin_m: HOST
+/* size of the raw record vol_frame_stats_async copies out */
+#define VOL_STATS_RAW_BYTES 128
+
+/* Create a volume pair.  dims_geo: HOST int32[3]; r in 1..4; origin_m: HOST
  * float[3], world position of the volume corner; extent_m: side length along x (cubic voxels of extent/dims_geo[0]);
  * trunc_mu_m > 0; w_max in 1..512 (exactness bound of the fp32 running average); opts nullable.
  * Both volumes start zeroed.  *out is only written on success. */
@@ -161,25 +171,28 @@ int vol_info(const vol_t *v, vol_info_t *out);
 int vol_shard_layers(int32_t nz, int32_t shard_rank, int32_t shard_world, int32_t *layers_out, int32_t cap);
 /* Enable (1) / disable (0) the four voxel counters of vol_stats_t (a separately compiled kernel variant). */
 int vol_set_counting(vol_t *v, int32_t on);
-/* Statistics of the last frame (synchronises `stream`; copies 64 bytes device -> host). */
+/* Statistics of the last frame (synchronises `stream`; copies VOL_STATS_RAW_BYTES device -> host). */
 int vol_frame_stats(vol_t *v, vol_stats_t *out, void *stream);
-/* The same without the synchronisation, for callers that enqueue frames back to back: copies the 64-byte raw record of the
- * frame last enqueued on `stream` to raw_host (HOST, pinned, 8-byte aligned, >= 64 bytes), asynchronously, in stream order;
+/* The same without the synchronisation, for callers that enqueue frames back to back: copies the raw record of the
+ * frame last enqueued on `stream` to raw_host (HOST, pinned, 8-byte aligned, >= VOL_STATS_RAW_BYTES), asynchronously, in stream order;
  * once the stream has passed it, vol_stats_decode (host only, no CUDA call) turns it into a vol_stats_t. */
 int vol_frame_stats_async(vol_t *v, void *raw_host, void *stream);
 int vol_stats_decode(const vol_t *v, const void *raw_host, vol_stats_t *out);
 /* Enable per-kernel CUDA-event timing of subsequent vol_integrate calls / read the last frame's kernel times in
- * milliseconds: ms[0] pre-pass, shell marks and geometry tile classification (S1, S9), ms[1] colour work items (S9), ms[2] fused integrate (S2-S8).  Synchronises. */
+ * milliseconds: ms[0] the per-pixel pre-pass (S1), ms[1] always 0 (kept for the layout: the classification of tiles and sub-boxes
+ * for both volumes (S9) runs inside the fused kernel), ms[2] the fused kernel (S2-S9).  Synchronises. */
 int vol_set_profiling(vol_t *v, int32_t on);
 int vol_last_kernel_ms(vol_t *v, float ms[3]);
-/* Number of kernels one vol_integrate call launches (vol_integrate_host launches one more: its fused kernel runs as a geometry
- * half and a colour half around the arrival of the HD frame). */
+/* Number of kernels one vol_integrate call launches (vol_integrate_host may launch one more: its fused kernel runs as a
+ * depth-only part and a colour part around the arrival of the HD frame). */
 int vol_launches_per_frame(const vol_t *v);
 /* Device self-test of the branch-free exact reciprocal / division used on the hot path against the correctly rounded
  * library intrinsics: mismatches[0] = reciprocal over every binary32 in its operand range, mismatches[1] = TSDF
  * running-average quotient over its operand domain (every denominator 1..513 x numerators; all of them when
- * exhaustive != 0, every 257th otherwise).  Both must be 0.  Runs on the current device; synchronises. */
-int vol_selftest(uint64_t mismatches[2], int32_t exhaustive);
+ * exhaustive != 0, every 257th otherwise), mismatches[2] = colour quotient of eq. 9 and the two weight roundings over
+ * stored weights x a sweep of new-sample weights (every binary32 in [2^-20, 255] when exhaustive != 0, every 1021st
+ * otherwise) x 16 colour / HD byte pairs.  All must be 0.  Runs on the current device; synchronises. */
+int vol_selftest(uint64_t mismatches[3], int32_t exhaustive);
 void vol_destroy(vol_t *v);
 /* Text for a return code.  For VOL_E_OOM / VOL_E_CUDA it names the failing CUDA call of the most recent failure in this
  * process (one process-global buffer: not meant to be read while other threads are making calls). */

@@ -21,6 +21,7 @@ _lib = None
 
 VOL_OK, VOL_E_ARG, VOL_E_OOM, VOL_E_CUDA = 0, -1, -2, -3
 VOL_SLAB = 8
+VOL_STATS_RAW_BYTES = 128
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "--fmad=false", "-std=c++17",
               "-Xcompiler", "-fPIC,-ffp-contract=off", "-shared"]
@@ -67,7 +68,11 @@ class VolInfo(ctypes.Structure):
 class VolStats(ctypes.Structure):
     _fields_ = [("geo_read", ctypes.c_uint64), ("geo_changed", ctypes.c_uint64), ("col_read", ctypes.c_uint64),
                 ("col_changed", ctypes.c_uint64), ("tiles_total", ctypes.c_uint32), ("tiles_geo", ctypes.c_uint32),
-                ("items_col", ctypes.c_uint32), ("cells_col", ctypes.c_uint32)]
+                ("items_col", ctypes.c_uint32), ("cells_col", ctypes.c_uint32),
+                ("geo_sectors_read", ctypes.c_uint64), ("geo_sectors_written", ctypes.c_uint64),
+                ("col_sectors_read", ctypes.c_uint64), ("col_sectors_written", ctypes.c_uint64),
+                ("geo_visited", ctypes.c_uint64), ("col_gated", ctypes.c_uint64), ("reserved64", ctypes.c_uint64),
+                ("subs_geo", ctypes.c_uint32), ("jobs_mark", ctypes.c_uint32)]
 
 
 def lib():
@@ -162,10 +167,10 @@ def shard_layers(nz: int, shard_rank: int, shard_world: int):
 
 
 def selftest(exhaustive: bool = False):
-    """vol_selftest: (reciprocal mismatches, TSDF-quotient mismatches) of the branch-free exact arithmetic; both must be 0."""
-    out = (ctypes.c_uint64 * 2)()
+    """vol_selftest: (reciprocal, TSDF-quotient, colour-quotient) mismatches of the branch-free exact arithmetic; all must be 0."""
+    out = (ctypes.c_uint64 * 3)()
     _check(lib().vol_selftest(out, int(exhaustive)), "vol_selftest")
-    return int(out[0]), int(out[1])
+    return int(out[0]), int(out[1]), int(out[2])
 
 
 class Volume:
@@ -261,8 +266,8 @@ class Volume:
         return s
 
     def frame_stats_async(self, raw_host, stream=None):
-        """vol_frame_stats_async: raw_host = pinned CPU tensor of >= 64 bytes; filled in stream order, no synchronisation."""
-        assert not raw_host.is_cuda and raw_host.is_pinned() and raw_host.numel() * raw_host.element_size() >= 64
+        """vol_frame_stats_async: raw_host = pinned CPU tensor of >= VOL_STATS_RAW_BYTES; filled in stream order, no synchronisation."""
+        assert not raw_host.is_cuda and raw_host.is_pinned() and raw_host.numel() * raw_host.element_size() >= VOL_STATS_RAW_BYTES
         _check(lib().vol_frame_stats_async(self._h, raw_host.data_ptr(), _stream_ptr(stream)), "vol_frame_stats_async")
 
     def decode_stats(self, raw_host) -> VolStats:

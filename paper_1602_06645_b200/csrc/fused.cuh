@@ -1,10 +1,16 @@
-// fused.cuh -- K2: the fused integration kernel (S2-S8), warp-centric and persistent.
+// fused.cuh -- K2: the fused integration kernel (S2-S9), warp-centric and persistent.
 //
-// Every warp pops work items from one queue until it is empty -- first the colour items (one non-zero shell-mark
-// nibble = up to 4 colour cells of 8x4x4 voxels of one tile), then the geometry items (one tile of 32x4x8 TSDF voxels, marched
-// along z with per-column bases hoisted).  A lane always owns one 16-byte vector of 4 x-adjacent voxels, so a warp
-// reads whole 32-byte sectors (colour gate) or 128-byte lines (geometry rows).  Colour voxels that pass the gate are
-// compacted in a per-warp shared-memory stage and updated one per lane.  No block-level barriers.
+// One launch does everything that follows the per-pixel pre-pass.  Every warp first helps with the producer roles
+// (prepass.cuh: geometry tile classification, shell marking -- chunks claimed from counters, so nobody waits for work that
+// has not been claimed), then consumes work items until none is left:
+//   geometry items (one tile of 32x4x8 TSDF voxels + the mask of its 8x4x4 sub-boxes that may be updated) are published by
+//     the classification as it goes and consumed from the first microsecond;
+//   colour items (one non-zero shell-mark nibble = up to 4 colour cells of 8x4x4 voxels of one tile) exist once every mark
+//     has been set and the mark words have been scanned (two grid-wide conditions, observed through counters); from then on
+//     they are taken first (they are the longer items; the geometry tiles fill the tail).
+// A lane owns an (x, y) column of a sub-box (4 voxels along z), so a warp reads whole 32-byte sectors and the per-column
+// part of eq. 5 is hoisted.  Colour voxels that pass the gate are compacted in a per-warp shared-memory stage and updated
+// one per lane.  No block-level barriers.
 //
 // The per-voxel arithmetic is the canonical sequence of DESIGN.md, issued branch-free for 4 voxels at a time
 // (projection -> gathers -> update); operands outside the range of the branch-free exact reciprocal (exact.cuh) send
@@ -12,6 +18,7 @@
 #pragma once
 #include "exact.cuh"
 #include "params.cuh"
+#include "prepass.cuh"
 
 namespace vf {
 
@@ -58,7 +65,7 @@ __device__ __noinline__ float4 col_voxel_gate_ref(const Params &p, float X, floa
 
 // ---------------------------------------------------------------------------------------------------------------
 // branch-free projection of one voxel (fast path): pixel offset y * w + x, or ok = false.
-// Precondition (established per tile by k_mark_classify / k_items_col, bit ITEM_NEAR clear): RCP_MIN <= Z <= RCP_MAX.
+// Precondition (tile_is_near() false for the voxel's tile): RCP_MIN <= Z <= RCP_MAX.
 // ---------------------------------------------------------------------------------------------------------------
 __device__ __forceinline__ void project_fast(float fx, float fy, float cx, float cy, uint32_t w, uint32_t wbits, uint32_t hbits, uint32_t koff,
                                              float X, float Y, float Z, bool &ok, uint32_t &off)
@@ -96,28 +103,171 @@ __device__ __forceinline__ void next_ticket(uint32_t *cursor, int lane, uint32_t
     asm volatile("{\n\t.reg .pred q;\n\tsetp.eq.s32 q, %1, 0;\n\t@q atom.global.add.u32 %0, [%2], 1;\n\t}"
                  : "+r"(ticket) : "r"(lane), "l"(cursor) : "memory");
 }
-
-struct Counts { unsigned long long gr, gc, cr, cc; };
-
-// one geometry tile, one warp: lane = (vx = lane & 7, y = lane >> 3) owns voxels (gx0 + 4 vx .. + 3, gy0 + y) of every layer.
-// NEAR tiles (may hold voxels with Z <= 0 or outside rcp_exact's range) take the plain per-voxel routine.
-// Otherwise the layers are software-pipelined: while layer z is updated, layer z + 1 has already been projected and its
-// four depth gathers and its voxel vector are in flight.
-template <bool COUNT, int VAR>
-__device__ __forceinline__ void geometry_tile(const Params &p, uint32_t item, int lane, Counts &c)
+// the same for `n` consecutive tickets
+__device__ __forceinline__ void next_tickets(uint32_t *cursor, uint32_t n, int lane, uint32_t &ticket)
 {
-    const bool near = (item & ITEM_NEAR) != 0u;
-    int ttx, tty, ttz, sub;
-    item_unpack(item, ttx, tty, ttz, sub);
+    asm volatile("{\n\t.reg .pred q;\n\tsetp.eq.s32 q, %1, 0;\n\t@q atom.global.add.u32 %0, [%2], %3;\n\t}"
+                 : "+r"(ticket) : "r"(lane), "l"(cursor), "r"(n) : "memory");
+}
+// n consecutive tickets, the first one returned to every lane at once
+__device__ __forceinline__ uint32_t claim_n(uint32_t *counter, uint32_t n, int lane)
+{
+    uint32_t t = 0;
+    next_tickets(counter, n, lane, t);
+    return __shfl_sync(0xffffffffu, t, 0);
+}
+// one ticket, returned to every lane at once (producer chunks: the result is needed right away)
+__device__ __forceinline__ uint32_t claim(uint32_t *counter, int lane)
+{
+    uint32_t t = 0;
+    next_ticket(counter, lane, t);
+    return __shfl_sync(0xffffffffu, t, 0);
+}
+// a chunk of producer work is finished: the counter the consumers watch is bumped with release semantics (a MEMBAR before
+// the reduction, and -- unlike __threadfence() -- no invalidation of this SM's L1, which the other warps' gathers live on)
+__device__ __forceinline__ void chunk_done(uint32_t *counter, int lane)
+{
+    __syncwarp();
+    if (lane == 0) asm volatile("red.release.gpu.global.add.u32 [%0], 1;" ::"l"(counter) : "memory");
+}
+// polling load of a control word or a work-list slot: served by L2, no acquire (an acquire invalidates L1 every time).
+// What the flag guards is only ever read through L2 afterwards (ld.cg, atomics), and only in code that is control-dependent
+// on the polled value.
+__device__ __forceinline__ uint32_t ld_relaxed(const uint32_t *ptr)
+{
+    uint32_t v;
+    asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(ptr) : "memory");
+    return v;
+}
+
+struct Counts { unsigned long long n[CNT_N]; };
+
+// ptr + e layers (e = 0..3 a compile-time constant after unrolling): one mad.wide with an immediate
+__device__ __forceinline__ uint32_t *layer_ptr(uint32_t *ptr, int e, uint32_t layer_b)
+{
+    unsigned long long a = (unsigned long long)ptr;
+    if (e == 1) asm("mad.wide.u32 %0, %1, 1, %2;" : "=l"(a) : "r"(layer_b), "l"(a));
+    if (e == 2) asm("mad.wide.u32 %0, %1, 2, %2;" : "=l"(a) : "r"(layer_b), "l"(a));
+    if (e == 3) asm("mad.wide.u32 %0, %1, 3, %2;" : "=l"(a) : "r"(layer_b), "l"(a));
+    return reinterpret_cast<uint32_t *>(a);
+}
+
+// development aid (compile with -DVF_TRACE): per-warp timestamps of the phase transitions of k_fused, 16 words per warp
+#ifdef VF_TRACE
+__device__ unsigned long long g_trace[8192 * 16];
+__device__ __forceinline__ unsigned long long vf_now() { unsigned long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); return t; }
+#define VF_T(slot) do { if (lane == 0 && gw < 8192u) g_trace[gw * 16u + (slot)] = vf_now(); } while (0)
+#define VF_TC(slot, v) do { if (lane == 0 && gw < 8192u) g_trace[gw * 16u + (slot)] = (v); } while (0)
+#else
+#define VF_T(slot) do { } while (0)
+#define VF_TC(slot, v) do { } while (0)
+#endif
+
+// COUNT only: how many distinct 32-byte sectors (8 words) the lanes with `pred` touch at word index `word`
+__device__ __forceinline__ unsigned sectors_touched(bool pred, unsigned long long word, int lane)
+{
+    const unsigned act = __ballot_sync(0xffffffffu, pred);
+    unsigned first = 0;
+    if (pred) {
+        const unsigned peers = __match_any_sync(act, word >> 3);
+        first = (__ffs(peers) - 1 == lane) ? 1u : 0u;
+    }
+    return first;
+}
+
+// S3 for four voxels of one lane (stored words o, camera depth Z of the voxel, depth D of its pixel -- 0 = none --, and, for
+// VAR_TSDF_ALONG_RAY, the factor L from the distance along z to the distance along the ray): truncation test and running
+// average; w4 = the new words.  Votes with the whole warp: every lane must call it.
+template <bool COUNT, int VAR>
+__device__ __forceinline__ void tsdf_update4(const uint32_t (&o)[4], const float (&Z)[4], const float (&D)[4], const float (&L)[4],
+                                             float neg_mu, float inv_mu, int w_max, uint32_t (&w4)[4], bool (&upd)[4])
+{
+    float sdf[4];
+    bool easy = true;
+#pragma unroll
+    for (int e = 0; e < 4; ++e) {
+        sdf[e] = __fsub_rn(D[e], Z[e]);
+        if (VAR == VAR_TSDF_ALONG_RAY) sdf[e] = __fmul_rn(sdf[e], L[e]);
+        upd[e] = (D[e] != 0.0f) & !(sdf[e] < neg_mu);
+        // saturated free space (tsdf = 1 onto q = 32767) or first touch (w = 0): the running average is 32767 exactly,
+        // fma(32767, w, 32767) / (w + 1) with every intermediate below 2^24.  (Bitwise on purpose: no branches.)
+        easy = easy & (!upd[e] | ((__fmul_rn(sdf[e], inv_mu) >= 1.0f) & (((o[e] & 0xffffu) == 0x7fffu) | (o[e] < 0x10000u))));
+    }
+    if (__all_sync(0xffffffffu, easy)) {                              // whole warp in free space: no division needed
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+            const int wn = min((int)(short)(o[e] >> 16) + 1, w_max);
+            w4[e] = upd[e] ? (0x7fffu | ((uint32_t)wn << 16)) : o[e];
+        }
+    } else {
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+            const float tsdf = fminf(1.0f, __fmul_rn(sdf[e], inv_mu));
+            const int q = (int)(short)(o[e] & 0xffffu);
+            const int wi = (int)(short)(o[e] >> 16);
+            const float wf = (float)wi;
+            // num is 0 or 2^-40 <= |num| < 2^26 (vol_create bounds mu), den in [1, 513]
+            const float num = __fmaf_rn((float)q, wf, __fmul_rn(tsdf, 32767.0f));
+            const float den = __fadd_rn(wf, 1.0f);
+            // rint (half-even) without the conversion pipe: |quotient| <= 32767, so adding 1.5 * 2^23 leaves it in the
+            // low mantissa bits, already in two's complement
+            const uint32_t qn = __float_as_uint(__fadd_rn(div_with(num, den, div_prepare(den)), 12582912.0f));
+            const int wn = min(wi + 1, w_max);
+            const uint32_t nw = (qn & 0xffffu) | ((uint32_t)wn << 16);
+            w4[e] = upd[e] ? nw : o[e];
+        }
+    }
+}
+
+// NEAR tiles (may hold voxels with Z <= 0 or outside rcp_exact's range) take the plain per-voxel routine, whole.
+template <bool COUNT>
+__device__ __noinline__ void geometry_tile_near(const Params &p, int ttx, int tty, int ttz, int lane, Counts &c)
+{
+    const int xl = lane & 7, j = tty * TY + (lane >> 3);
+    const int gz0 = local_to_global_tz(p, ttz) * TZ, lz0 = ttz * TZ;
+    const float py = __fmaf_rn((float)j + 0.5f, p.vs, p.oy);
+    for (int bx = 0; bx < SUBX; ++bx) {
+        const int i = ttx * TX + 8 * bx + xl;
+        if (!(i < p.nx && j < p.ny)) continue;
+        const float px = __fmaf_rn((float)i + 0.5f, p.vs, p.ox);
+        const float bX = __fmaf_rn(p.R[1], py, __fmaf_rn(p.R[0], px, p.t[0]));
+        const float bY = __fmaf_rn(p.R[4], py, __fmaf_rn(p.R[3], px, p.t[1]));
+        const float bZ = __fmaf_rn(p.R[7], py, __fmaf_rn(p.R[6], px, p.t[2]));
+#pragma unroll 1
+        for (int z = 0; z < TZ && gz0 + z < p.nz; ++z) {
+            uint32_t *ptr = p.geo + ((size_t)(lz0 + z) * p.ny + j) * p.nx + i;
+            const uint32_t o = *ptr;
+            const float pz = __fmaf_rn((float)(gz0 + z) + 0.5f, p.vs, p.oz);
+            bool rd = false;
+            const uint32_t w = geo_voxel_ref(p, __fmaf_rn(p.R[2], pz, bX), __fmaf_rn(p.R[5], pz, bY), __fmaf_rn(p.R[8], pz, bZ), o, rd);
+            if (COUNT) {
+                c.n[CNT_GEO_VISITED] += 1; c.n[CNT_GEO_READ] += rd; c.n[CNT_GEO_CHANGED] += w != o;
+                const unsigned long long wi = (unsigned long long)(ptr - p.geo);
+                const unsigned act = __activemask();
+                const unsigned pr = __match_any_sync(act, rd ? wi >> 3 : ~0ull), pw = __match_any_sync(act, w != o ? wi >> 3 : ~0ull);
+                c.n[CNT_GEO_SEC_READ] += rd && __ffs(pr) - 1 == lane; c.n[CNT_GEO_SEC_WRITTEN] += w != o && __ffs(pw) - 1 == lane;
+            }
+            if (w != o) *ptr = w;
+        }
+    }
+}
+
+// One z half (4 layers) of a geometry tile whose four x sub-boxes are all wanted: the whole 32 x 4 footprint.
+// lane = (vx = lane & 7, y = lane >> 3) owns voxels (gx0 + 4 vx .. + 3, gy0 + y) of every layer as one 16-byte vector, so a
+// warp access is four full 128-byte lines and everything per layer (z term of eq. 5, pointer, load, store) is shared by four
+// voxels.  The layers are software-pipelined over two alternating register sets: while layer z is updated, layer z + 1 has
+// already been projected and its four depth gathers and its voxel vector are in flight.  Needs nx % 4 == 0.
+template <bool COUNT, int VAR>
+__device__ __forceinline__ void geometry_half_rows(const Params &p, int ttx, int tty, int gz0, int lz0, int lane, Counts &c)
+{
     const int i0 = ttx * TX + 4 * (lane & 7), j = tty * TY + (lane >> 3);
-    // the classification tested the tile's two z-halves separately (bits 0 and 1 of sub): a half that failed holds no
-    // voxel this frame can update, and its four layers are left out -- the march starts at layer zb and covers nl layers
-    const int zb = (near || (sub & 1)) ? 0 : TZ / 2;
-    const int gz0 = local_to_global_tz(p, ttz) * TZ + zb, lz0 = ttz * TZ + zb;
     const bool inside = i0 < p.nx && j < p.ny;
-    const unsigned lanes = __ballot_sync(0xffffffffu, inside);    // ragged tile: the votes below name only these lanes
-    if (!inside) return;
-    const int nl = min((near || (sub & 2)) ? TZ - zb : TZ / 2, p.nz - gz0);
+    const int nl = inside ? min(TZ / SUBZ, p.nz - gz0) : 0;
+    const float fx = p.fx, fy = p.fy, cx = p.cx, cy = p.cy;
+    const float neg_mu = p.neg_mu, inv_mu = p.inv_mu;
+    const uint32_t wd = (uint32_t)p.wd, wbits = __float_as_uint(p.wd_f), hbits = __float_as_uint(p.hd_f), koff = 0x4B400000u * (wd + 1u);
+    const int w_max = p.w_max;
+    const float *__restrict__ depthf = p.depthf;
     // per-column bases of eq. 5: fma(R_1, py, fma(R_0, px, t)) -- the z term is added per layer with one fma each
     const float py = __fmaf_rn((float)j + 0.5f, p.vs, p.oy);
     float bX[4], bY[4], bZ[4];
@@ -129,35 +279,10 @@ __device__ __forceinline__ void geometry_tile(const Params &p, uint32_t item, in
         bZ[e] = __fmaf_rn(p.R[7], py, __fmaf_rn(p.R[6], px, p.t[2]));
     }
     const float r02 = p.R[2], r12 = p.R[5], r22 = p.R[8];
-    const size_t layer = (size_t)p.ny * p.nx;
-    uint4 *ptr = reinterpret_cast<uint4 *>(p.geo + ((size_t)lz0 * p.ny + j) * p.nx + i0);
-    if (near) {
-        for (int z = 0; z < nl; ++z) {
-            const uint4 cur = *ptr;
-            const float pz = __fmaf_rn((float)(gz0 + z) + 0.5f, p.vs, p.oz);
-            const uint32_t o4[4] = {cur.x, cur.y, cur.z, cur.w};
-            uint32_t w4[4];
-#pragma unroll
-            for (int e = 0; e < 4; ++e) {
-                bool rd = false;
-                w4[e] = geo_voxel_ref(p, __fmaf_rn(r02, pz, bX[e]), __fmaf_rn(r12, pz, bY[e]), __fmaf_rn(r22, pz, bZ[e]), o4[e], rd);
-                if (COUNT) { c.gr += rd; c.gc += w4[e] != o4[e]; }
-            }
-            if ((w4[0] != o4[0]) | (w4[1] != o4[1]) | (w4[2] != o4[2]) | (w4[3] != o4[3])) *ptr = make_uint4(w4[0], w4[1], w4[2], w4[3]);
-            ptr = reinterpret_cast<uint4 *>(reinterpret_cast<uint32_t *>(ptr) + layer);
-        }
-        return;
-    }
-    const float fx = p.fx, fy = p.fy, cx = p.cx, cy = p.cy;
-    const float neg_mu = p.neg_mu, inv_mu = p.inv_mu;
-    const uint32_t wd = (uint32_t)p.wd, wbits = __float_as_uint(p.wd_f), hbits = __float_as_uint(p.hd_f), koff = 0x4B400000u * (wd + 1u);
-    const int w_max = p.w_max;
-    const uint16_t *__restrict__ depth = p.depth;
-    // S2 of one layer: eq. 5 z term, projection, and the four depth gathers (offset 0 when outside: a valid address)
-    // A voxel outside the frustum keeps d = 0 ("invalid depth": not updated); its gather is predicated off.  The address is
-    // one mad.wide (FMA pipe) instead of a 64-bit add pair: the ALU pipe is the busiest one in this loop.
-    // (VAR_TSDF_ALONG_RAY only: L = |P_vc| / Z_vc, the factor from the distance along z to the distance along the ray)
-    auto project_layer = [&](int z, float (&Z)[4], uint32_t (&d)[4], float (&L)[4]) {
+    const uint32_t layer_b = (uint32_t)((size_t)p.ny * p.nx * 4u);
+    uint32_t *ptr0 = p.geo + ((size_t)lz0 * p.ny + j) * p.nx + i0;
+    // S2 of one layer: eq. 5 z term, projection, and the four depth gathers
+    auto project_layer = [&](int z, float (&Z)[4], float (&D)[4], float (&L)[4]) {
         const float pz = __fmaf_rn((float)(gz0 + z) + 0.5f, p.vs, p.oz);
 #pragma unroll
         for (int e = 0; e < 4; ++e) {
@@ -167,87 +292,173 @@ __device__ __forceinline__ void geometry_tile(const Params &p, uint32_t item, in
             project_fast_raw(fx, fy, cx, cy, wd, wbits, hbits, koff, X, Y, Z[e], ok, off, iz);
             if (VAR == VAR_TSDF_ALONG_RAY)
                 L[e] = __fmul_rn(__fsqrt_rn(__fmaf_rn(Z[e], Z[e], __fmaf_rn(Y, Y, __fmul_rn(X, X)))), iz);
-            d[e] = 0u;
+            D[e] = 0.0f;
             if (ok) {
                 unsigned long long addr;
-                asm("mad.wide.u32 %0, %1, 2, %2;" : "=l"(addr) : "r"(off), "l"(depth));
-                d[e] = __ldg(reinterpret_cast<const uint16_t *>(addr));
+                asm("mad.wide.u32 %0, %1, 4, %2;" : "=l"(addr) : "r"(off), "l"(depthf));
+                D[e] = __ldg(reinterpret_cast<const float *>(addr));
             }
         }
     };
-    // S3 of one layer: truncation test, running average, store if a word changed
-    auto update_layer = [&](uint4 *ptr, const uint4 &cur, const float (&Z)[4], const uint32_t (&d)[4], const float (&L)[4]) {
-        const uint32_t o4[4] = {cur.x, cur.y, cur.z, cur.w};
-        uint32_t w4[4];
-        float sdf[4]; bool upd[4];
-        bool easy = true;
-#pragma unroll
-        for (int e = 0; e < 4; ++e) {
-            const float D = __fmul_rn((float)d[e], 0.001f);
-            sdf[e] = __fsub_rn(D, Z[e]);
-            if (VAR == VAR_TSDF_ALONG_RAY) sdf[e] = __fmul_rn(sdf[e], L[e]);
-            upd[e] = (d[e] != 0u) & !(sdf[e] < neg_mu);
-            // saturated free space (tsdf = 1 onto q = 32767) or first touch (w = 0): the running average is 32767 exactly,
-            // fma(32767, w, 32767) / (w + 1) with every intermediate below 2^24.  (Bitwise on purpose: no branches.)
-            easy = easy & (!upd[e] | ((__fmul_rn(sdf[e], inv_mu) >= 1.0f) & (((o4[e] & 0xffffu) == 0x7fffu) | (o4[e] < 0x10000u))));
-            if (COUNT) c.gr += upd[e];
+    auto update_layer = [&](int z, const uint4 &cur, const float (&Z)[4], const float (&D)[4], const float (&L)[4]) {
+        const uint32_t o[4] = {cur.x, cur.y, cur.z, cur.w};
+        uint32_t w4[4]; bool upd[4];
+        const float Dm[4] = {z < nl ? D[0] : 0.0f, z < nl ? D[1] : 0.0f, z < nl ? D[2] : 0.0f, z < nl ? D[3] : 0.0f};
+        tsdf_update4<COUNT, VAR>(o, Z, Dm, L, neg_mu, inv_mu, w_max, w4, upd);
+        const bool any = (w4[0] != o[0]) | (w4[1] != o[1]) | (w4[2] != o[2]) | (w4[3] != o[3]);
+        uint4 *ptr = reinterpret_cast<uint4 *>(layer_ptr(ptr0, z, layer_b));
+        if (COUNT && z < nl) {
+            c.n[CNT_GEO_VISITED] += 4; c.n[CNT_GEO_READ] += upd[0] + upd[1] + upd[2] + upd[3];
+            c.n[CNT_GEO_CHANGED] += (w4[0] != o[0]) + (w4[1] != o[1]) + (w4[2] != o[2]) + (w4[3] != o[3]);
         }
-        if (__all_sync(lanes, easy)) {                            // whole warp in free space: no division needed
-#pragma unroll
-            for (int e = 0; e < 4; ++e) {
-                const int wn = min((int)(short)(o4[e] >> 16) + 1, w_max);
-                w4[e] = upd[e] ? (0x7fffu | ((uint32_t)wn << 16)) : o4[e];
-            }
-        } else {
-#pragma unroll
-            for (int e = 0; e < 4; ++e) {
-                const float tsdf = fminf(1.0f, __fmul_rn(sdf[e], inv_mu));
-                const int q = (int)(short)(o4[e] & 0xffffu);
-                const int wi = (int)(short)(o4[e] >> 16);
-                const float wf = (float)wi;
-                // num is 0 or 2^-40 <= |num| < 2^26 (vol_create bounds mu), den in [1, 513]
-                const float num = __fmaf_rn((float)q, wf, __fmul_rn(tsdf, 32767.0f));
-                const float den = __fadd_rn(wf, 1.0f);
-                // rint (half-even) without the conversion pipe: |quotient| <= 32767, so adding 1.5 * 2^23 leaves it in the
-                // low mantissa bits, already in two's complement
-                const uint32_t qn = __float_as_uint(__fadd_rn(div_with(num, den, div_prepare(den)), 12582912.0f));
-                const int wn = min(wi + 1, w_max);
-                const uint32_t nw = (qn & 0xffffu) | ((uint32_t)wn << 16);
-                w4[e] = upd[e] ? nw : o4[e];
-            }
+        if (COUNT) {                                                  // (a 16-byte aligned vector lies in one 32-byte sector)
+            const unsigned long long wi = (unsigned long long)(reinterpret_cast<uint32_t *>(ptr) - p.geo);
+            c.n[CNT_GEO_SEC_READ] += sectors_touched(z < nl && (upd[0] | upd[1] | upd[2] | upd[3]), wi, lane);
+            c.n[CNT_GEO_SEC_WRITTEN] += sectors_touched(any, wi, lane);
         }
-        const bool any = (w4[0] != o4[0]) | (w4[1] != o4[1]) | (w4[2] != o4[2]) | (w4[3] != o4[3]);
-        if (COUNT) c.gc += (w4[0] != o4[0]) + (w4[1] != o4[1]) + (w4[2] != o4[2]) + (w4[3] != o4[3]);
-        if (any) *ptr = make_uint4(w4[0], w4[1], w4[2], w4[3]);   // skip the store when nothing changed
+        if (any) __stcg(ptr, make_uint4(w4[0], w4[1], w4[2], w4[3]));   // skip the store when nothing changed
     };
     // Two register sets, A (even layers) and B (odd layers), used alternately: the pipeline needs no register-to-register
-    // rotation, which would make the warp wait for the loads it has just issued.
-    float ZA[4], ZB[4], LA[4], LB[4]; uint32_t dA[4], dB[4];
+    // rotation, which would make the warp wait for the loads it has just issued.  Lanes outside the volume (nl = 0) go
+    // through the motions with D = 0 (nothing is loaded or stored): the update votes with the whole warp.
+    float ZA[4], ZB[4], DA[4], DB[4], LA[4], LB[4];
+    const uint4 zero = make_uint4(0u, 0u, 0u, 0u);
     // the voxel stream bypasses L1 (__ldcg): every line is used once, and L1 is better spent on the depth image
-    uint4 curA = __ldcg(ptr), curB = curA;
-    project_layer(0, ZA, dA, LA);
-    for (int z = 0; z < nl; z += 2) {
-        uint4 *pB = reinterpret_cast<uint4 *>(reinterpret_cast<uint32_t *>(ptr) + layer);
-        uint4 *pA2 = reinterpret_cast<uint4 *>(reinterpret_cast<uint32_t *>(pB) + layer);
-        const bool hasB = z + 1 < nl, hasA2 = z + 2 < nl;
-        if (hasB) { curB = __ldcg(pB); project_layer(z + 1, ZB, dB, LB); }               // layer z + 1 in flight
-        update_layer(ptr, curA, ZA, dA, LA);
-        if (hasB) {
-            if (hasA2) { curA = __ldcg(pA2); project_layer(z + 2, ZA, dA, LA); }         // layer z + 2 in flight
-            update_layer(pB, curB, ZB, dB, LB);
+    uint4 curA = nl > 0 ? __ldcg(reinterpret_cast<const uint4 *>(ptr0)) : zero, curB = zero;
+    project_layer(0, ZA, DA, LA);
+#pragma unroll
+    for (int z = 0; z < TZ / SUBZ; z += 2) {
+        curB = z + 1 < nl ? __ldcg(reinterpret_cast<const uint4 *>(layer_ptr(ptr0, z + 1, layer_b))) : zero;
+        project_layer(z + 1, ZB, DB, LB);                                    // layer z + 1 in flight
+        update_layer(z, curA, ZA, DA, LA);
+        if (z + 2 < TZ / SUBZ) {
+            curA = z + 2 < nl ? __ldcg(reinterpret_cast<const uint4 *>(layer_ptr(ptr0, z + 2, layer_b))) : zero;
+            project_layer(z + 2, ZA, DA, LA);                                // layer z + 2 in flight
         }
-        ptr = pA2;
+        update_layer(z + 1, curB, ZB, DB, LB);
     }
 }
 
-// pull the 32 lines (8 layers x 4 rows x 128 bytes) of a geometry tile into L2: one line per lane, no register is tied up.
-// Issued when the tile is started: its later layers are then L2 hits by the time the layer pipeline reaches them.
+// The wanted sub-boxes (bits of m4: bx = 0..3) of one z half of a geometry tile, one warp pass each: lane = (x = lane & 7,
+// y = lane >> 3) owns the column of 4 voxels along z, so every access of the warp is four whole 32-byte sectors and the
+// per-column part of eq. 5 is hoisted.  The passes are software-pipelined over two alternating register sets: while
+// sub-box n is updated, sub-box n + 1 has already been projected and its depth gathers and voxel loads are in flight.
+template <bool COUNT, int VAR>
+__device__ __forceinline__ void geometry_half_boxes(const Params &p, int ttx, int tty, int gz0, int lz0, uint32_t m4, int lane, Counts &c)
+{
+    const int xl = lane & 7, j = tty * TY + (lane >> 3);
+    const float fx = p.fx, fy = p.fy, cx = p.cx, cy = p.cy, vs = p.vs;
+    const float neg_mu = p.neg_mu, inv_mu = p.inv_mu;
+    const uint32_t wd = (uint32_t)p.wd, wbits = __float_as_uint(p.wd_f), hbits = __float_as_uint(p.hd_f), koff = 0x4B400000u * (wd + 1u);
+    const int w_max = p.w_max;
+    const float *__restrict__ depthf = p.depthf;
+    const float py = __fmaf_rn((float)j + 0.5f, vs, p.oy);
+    const float r02 = p.R[2], r12 = p.R[5], r22 = p.R[8];
+    const uint32_t layer_b = (uint32_t)((size_t)p.ny * p.nx * 4u);
+    const int nrem_row = j < p.ny ? p.nz - gz0 : 0;                    // layers of this half the lane's row really has
+    float pz[4];
+#pragma unroll
+    for (int e = 0; e < 4; ++e) pz[e] = __fmaf_rn((float)(gz0 + e) + 0.5f, vs, p.oz);
+    // S2 of one sub-box: eq. 5, projection, the four depth gathers and the four voxel loads.  A voxel outside the frustum
+    // or the volume keeps D = 0 ("invalid depth": not updated); its gather is predicated off.
+    auto load_project = [&](int bx, uint32_t *&ptr, uint32_t (&o)[4], float (&Z)[4], float (&D)[4], float (&L)[4]) {
+        const int i = ttx * TX + 8 * bx + xl;
+        const int nrem = i < p.nx ? nrem_row : 0;
+        const float px = __fmaf_rn((float)i + 0.5f, vs, p.ox);
+        const float bX = __fmaf_rn(p.R[1], py, __fmaf_rn(p.R[0], px, p.t[0]));
+        const float bY = __fmaf_rn(p.R[4], py, __fmaf_rn(p.R[3], px, p.t[1]));
+        const float bZ = __fmaf_rn(p.R[7], py, __fmaf_rn(p.R[6], px, p.t[2]));
+        ptr = p.geo + ((size_t)lz0 * p.ny + j) * p.nx + i;
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+            const bool in = e < nrem;
+            // the voxel stream bypasses L1 (__ldcg): every sector is used once, and L1 is better spent on the depth image
+            o[e] = 0u;
+            if (in) o[e] = __ldcg(layer_ptr(ptr, e, layer_b));
+            const float X = __fmaf_rn(r02, pz[e], bX), Y = __fmaf_rn(r12, pz[e], bY);
+            Z[e] = __fmaf_rn(r22, pz[e], bZ);
+            bool ok; uint32_t off; float iz;
+            project_fast_raw(fx, fy, cx, cy, wd, wbits, hbits, koff, X, Y, Z[e], ok, off, iz);
+            if (VAR == VAR_TSDF_ALONG_RAY)
+                L[e] = __fmul_rn(__fsqrt_rn(__fmaf_rn(Z[e], Z[e], __fmaf_rn(Y, Y, __fmul_rn(X, X)))), iz);
+            D[e] = 0.0f;
+            if (ok && in) {
+                unsigned long long addr;                              // one mad.wide (FMA pipe) instead of a 64-bit add pair
+                asm("mad.wide.u32 %0, %1, 4, %2;" : "=l"(addr) : "r"(off), "l"(depthf));
+                D[e] = __ldg(reinterpret_cast<const float *>(addr));
+            }
+        }
+    };
+    // S3 of one sub-box: truncation test, running average, store of the words that changed
+    auto update = [&](uint32_t *ptr, const uint32_t (&o)[4], const float (&Z)[4], const float (&D)[4], const float (&L)[4]) {
+        uint32_t w4[4]; bool upd[4];
+        tsdf_update4<COUNT, VAR>(o, Z, D, L, neg_mu, inv_mu, w_max, w4, upd);
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+            if (COUNT) {
+                const unsigned long long wi = (unsigned long long)(layer_ptr(ptr, e, layer_b) - p.geo);
+                c.n[CNT_GEO_VISITED] += 1; c.n[CNT_GEO_READ] += upd[e]; c.n[CNT_GEO_CHANGED] += w4[e] != o[e];
+                c.n[CNT_GEO_SEC_READ] += sectors_touched(upd[e], wi, lane);
+                c.n[CNT_GEO_SEC_WRITTEN] += sectors_touched(w4[e] != o[e], wi, lane);
+            }
+            if (w4[e] != o[e]) __stcg(layer_ptr(ptr, e, layer_b), w4[e]);   // skip the store when nothing changed
+        }
+    };
+    // Two register sets, A and B, used alternately (no register-to-register rotation)
+    uint32_t *pA, *pB, oA[4], oB[4];
+    float ZA[4], ZB[4], DA[4], DB[4], LA[4], LB[4];
+    uint32_t m = m4;
+    if (COUNT && lane == 0) atomicAdd(&p.ctrl[ST_SUBS], (uint32_t)__popc(m));
+    int b = __ffs(m) - 1; m &= m - 1u;
+    load_project(b, pA, oA, ZA, DA, LA);
+    for (;;) {
+        const bool hasB = m != 0u;
+        if (hasB) { b = __ffs(m) - 1; m &= m - 1u; load_project(b, pB, oB, ZB, DB, LB); }      // sub-box n + 1 in flight
+        update(pA, oA, ZA, DA, LA);
+        if (!hasB) break;
+        const bool hasA = m != 0u;
+        if (hasA) { b = __ffs(m) - 1; m &= m - 1u; load_project(b, pA, oA, ZA, DA, LA); }      // sub-box n + 2 in flight
+        update(pB, oB, ZB, DB, LB);
+        if (!hasA) break;
+    }
+}
+
+#ifndef VF_ROWS_PATH
+#define VF_ROWS_PATH 0
+#endif
+// one geometry tile, one warp.  The item names the tile's 8x4x4 sub-boxes that may hold a voxel this frame updates.  Each z
+// half of the tile (4 layers) is processed either as whole rows, when all four of its sub-boxes are wanted (the common
+// case: free space), or sub-box by sub-box.
+template <bool COUNT, int VAR>
+__device__ __forceinline__ void geometry_tile(const Params &p, uint32_t item, int lane, Counts &c)
+{
+    int ttx, tty, ttz, mask;
+    item_unpack(item, ttx, tty, ttz, mask);
+    if (tile_is_near(p, ttx, tty, ttz)) { geometry_tile_near<COUNT>(p, ttx, tty, ttz, lane, c); return; }
+    const int gz0 = local_to_global_tz(p, ttz) * TZ, lz0 = ttz * TZ;
+    const bool vec_ok = (p.nx & 3) == 0;
+#pragma unroll 1
+    for (int zh = 0; zh < SUBZ; ++zh) {
+        uint32_t m = ((uint32_t)mask >> zh) & 0x55u;                  // bit 2 bx: sub-box bx of this half
+        if (m == 0u) continue;
+        if (VF_ROWS_PATH && m == 0x55u && vec_ok) {
+            if (COUNT && lane == 0) atomicAdd(&p.ctrl[ST_SUBS], 4u);
+            geometry_half_rows<COUNT, VAR>(p, ttx, tty, gz0 + zh * (TZ / SUBZ), lz0 + zh * (TZ / SUBZ), lane, c);
+        } else {
+            m = (m | (m >> 1)) & 0x33u; m = (m | (m >> 2)) & 0x0fu;   // bit bx
+            geometry_half_boxes<COUNT, VAR>(p, ttx, tty, gz0 + zh * (TZ / SUBZ), lz0 + zh * (TZ / SUBZ), m, lane, c);
+        }
+    }
+}
+
+// pull the sectors of a geometry tile into L2 when the tile is started: lane = (row, layer); a layer is wanted when its z
+// half holds a sub-box of the mask.  (Whole 128-byte lines: the x sub-boxes a tile leaves out are the minority.)
 __device__ __forceinline__ void geometry_prefetch(const Params &p, uint32_t item, int lane)
 {
-    int ttx, tty, ttz, sub;
-    item_unpack(item, ttx, tty, ttz, sub);
+    int ttx, tty, ttz, mask;
+    item_unpack(item, ttx, tty, ttz, mask);
     const int j = tty * TY + (lane & 3), lz = ttz * TZ + (lane >> 2);
-    const bool wanted = (item & ITEM_NEAR) != 0u || ((sub >> ((lane >> 2) / (TZ / 2))) & 1) != 0;   // its z-half is processed
+    const bool wanted = ((mask >> ((lane >> 2) / (TZ / SUBZ))) & 0x55) != 0;
     if (j < p.ny && lz < p.local_nz && wanted)
         asm volatile("prefetch.global.L2 [%0];" ::"l"(p.geo + ((size_t)lz * p.ny + j) * p.nx + ttx * TX));
 }
@@ -255,7 +466,7 @@ __device__ __forceinline__ void geometry_prefetch(const Params &p, uint32_t item
 // Per-warp staging buffer of colour voxels that passed the sigma gate.  The gate (S4-S5) runs on whole cells, 4 voxels
 // per lane, and only a fraction of them passes; the update (S6-S8: weight gate, HD lookup, eq. 9-10) is several times
 // longer.  Passing voxels are therefore compacted here and updated 32 at a time with every lane busy.
-constexpr int STAGE_CAP = 160;            // up to 31 carried over + 128 of one cell
+constexpr int STAGE_CAP = 64;             // up to 31 carried over + the 32 of one layer of a cell
 struct Stage {
     float4 rec[STAGE_CAP];                // {X, Y, Z} = voxel centre in the depth camera (eq. 5) -- or, VAR_HD_FROM_DEPTH_POINT, the
                                           // 3D point of its depth pixel (eq. 7); W = view weight of its pixel
@@ -266,26 +477,68 @@ struct Stage {
 // lane.  The HD pixel (eq. 3-4) is computed and its three bytes requested BEFORE the stored word arrives: the two gathers do
 // not depend on each other, so their latencies overlap instead of adding up (the word is a DRAM access, and one warp
 // works through its stage round after round).  A voxel that then fails the weight gate has fetched 3 bytes in vain.
+// Like the gate, the update issues the exact reciprocal / quotient sequences directly (exact.cuh) when every lane's operands
+// are in their range -- Z_hd in [RCP_MIN, RCP_MAX] or <= 0, and a new-sample weight 255 W >= 2^-20 -- and integer
+// conversions as magic-number additions; otherwise the whole round takes the plain routines.
 template <bool COUNT, int VAR>
 __device__ __forceinline__ void colour_update_staged(const Params &p, const Stage &st, int first, int n, int lane, Counts &c)
 {
-    if (lane < n) {
-        const float4 r = st.rec[first + lane];
+    const bool have = lane < n;
+    uint32_t old = 0u, nw = 0u;
+    unsigned long long wi = 0ull;
+    float4 r = make_float4(0.f, 0.f, 1.f, 1.f);
+    uint32_t *ptr = p.col;
+    if (have) {
+        r = st.rec[first + lane];
         const uint2 a = st.adr[first + lane];
-        uint32_t *ptr = p.col + (((size_t)a.y << 32) | (size_t)a.x);
-        const uint32_t old = __ldcg(ptr);                         // first HBM touch of this colour voxel (S6); L2 only
-        // HD pixel of the voxel's own position (eq. 3-4; A10, A11)
-        const float Xh = __fmaf_rn(p.Rc[2], r.z, __fmaf_rn(p.Rc[1], r.y, __fmaf_rn(p.Rc[0], r.x, p.tc[0])));
-        const float Yh = __fmaf_rn(p.Rc[5], r.z, __fmaf_rn(p.Rc[4], r.y, __fmaf_rn(p.Rc[3], r.x, p.tc[1])));
-        const float Zh = __fmaf_rn(p.Rc[8], r.z, __fmaf_rn(p.Rc[7], r.y, __fmaf_rn(p.Rc[6], r.x, p.tc[2])));
+        wi = ((unsigned long long)a.y << 32) | (unsigned long long)a.x;
+        ptr = p.col + wi;
+        old = __ldcg(ptr);                                            // first HBM touch of this colour voxel (S6); L2 only
+    }
+    // HD pixel of the voxel's own position (eq. 3-4; A10, A11)
+    const float Xh = __fmaf_rn(p.Rc[2], r.z, __fmaf_rn(p.Rc[1], r.y, __fmaf_rn(p.Rc[0], r.x, p.tc[0])));
+    const float Yh = __fmaf_rn(p.Rc[5], r.z, __fmaf_rn(p.Rc[4], r.y, __fmaf_rn(p.Rc[3], r.x, p.tc[1])));
+    const float Zh = __fmaf_rn(p.Rc[8], r.z, __fmaf_rn(p.Rc[7], r.y, __fmaf_rn(p.Rc[6], r.x, p.tc[2])));
+    const float W = r.w, W255 = __fmul_rn(W, 255.0f);
+    const bool tame = !have || ((!(Zh > 0.0f) || (Zh >= RCP_MIN && Zh <= RCP_MAX)) && W255 >= 0x1p-20f);
+    if (__all_sync(0xffffffffu, tame)) {
+        const uint32_t wh = (uint32_t)p.wh;
+        bool okh; uint32_t off;
+        project_fast(p.fxh, p.fyh, p.cxh, p.cyh, wh, __float_as_uint(p.wh_f), __float_as_uint(p.hh_f), 0x4B400000u * (wh + 1u),
+                     Xh, Yh, Zh > 0.0f ? Zh : 1.0f, okh, off);                 // A13; A14: nearest pixel (offset 0 when outside: a valid address)
+        okh = okh && Zh > 0.0f && have;
+        unsigned long long addr;
+        asm("mad.wide.u32 %0, %1, 3, %2;" : "=l"(addr) : "r"(okh ? off : 0u), "l"(p.rgb));
+        const uint8_t *hd = reinterpret_cast<const uint8_t *>(addr);
+        const uint32_t h0 = __ldg(hd), h1 = __ldg(hd + 1), h2 = __ldg(hd + 2);
+        const uint32_t wq = old >> 24;
+        const float wqf = (float)wq;
+        nw = old;
+        if (okh && W255 > __fmul_rn(p.gate, wqf)) {                   // L115, A9
+            const float den = __fadd_rn(wqf, W255), rden = div_prepare(den);   // den in [2^-20, 510]
+            const uint32_t h[3] = {h0, h1, h2};
+            nw = 0u;
+#pragma unroll
+            for (int ch = 0; ch < 3; ++ch) {                          // eq. 9: the quotient lies in [0, 255], so the clamp is idle
+                const uint32_t C = (old >> (8 * ch)) & 0xffu;
+                const float num = __fmaf_rn(W255, (float)h[ch], (float)(C * wq));   // 0 or in [2^-20, 2^17]
+                const uint32_t ci = __float_as_uint(__fadd_rn(div_with(num, den, rden), 12582912.0f)) & 0x1ffu;   // rint, half-even
+                nw |= min(ci, 255u) << (8 * ch);
+            }
+            const float wnf = VAR == VAR_ADDITIVE_WEIGHT ? __fadd_rn(wqf, W255)                    // W_pre + W
+                                                         : __fmaf_rn(W, (float)(255u - wq), wqf); // eq. 10, A12
+            const uint32_t wn = __float_as_uint(__fadd_rn(wnf, 12582912.0f)) & 0x3ffu;             // rint; wnf in [0, 510]
+            nw |= min(wn, 255u) << 24;
+            if (nw != old) *ptr = nw;
+        }
+    } else if (have) {
         int xh = 0, yh = 0;
         const bool okh = project_px(p.fxh, p.fyh, p.cxh, p.cyh, p.wh_f, p.hh_f, Xh, Yh, Zh, xh, yh);   // A13
         const uint8_t *hd = p.rgb + (size_t)(yh * p.wh + xh) * 3;     // A14: nearest pixel ((0, 0) when outside: a valid address)
         const uint32_t h0 = __ldg(hd), h1 = __ldg(hd + 1), h2 = __ldg(hd + 2);
         const int wq = (int)(old >> 24);
-        const float W = r.w, W255 = __fmul_rn(W, 255.0f);
-        uint32_t nw = old;
-        if (okh && W255 > __fmul_rn(p.gate, (float)wq)) {         // L115, A9
+        nw = old;
+        if (okh && W255 > __fmul_rn(p.gate, (float)wq)) {             // L115, A9
             const float den = __fadd_rn((float)wq, W255);
             const uint32_t h[3] = {h0, h1, h2};
             nw = 0;
@@ -302,160 +555,311 @@ __device__ __forceinline__ void colour_update_staged(const Params &p, const Stag
             nw |= (uint32_t)min(wn, 255) << 24;
             if (nw != old) *ptr = nw;
         }
-        if (COUNT) { c.cr += 1; c.cc += nw != old; }
+    }
+    if (COUNT) {
+        c.n[CNT_COL_READ] += have; c.n[CNT_COL_CHANGED] += have && nw != old;
+        c.n[CNT_COL_SEC_READ] += sectors_touched(have, wi, lane);
+        c.n[CNT_COL_SEC_WRITTEN] += sectors_touched(have && nw != old, wi, lane);
     }
 }
 
-// one colour cell of 8 x 4 x 4 voxels, one warp: lane = (vx = lane & 1, y = (lane >> 1) & 3, z = lane >> 3) owns 4
-// x-adjacent voxels.  (ic0, jc, kcg) = the lane's first voxel in the full colour grid, kcl = its layer in this shard.
-// Voxels that pass the gate are appended to the warp's stage (n = its fill level, warp-uniform); full groups of 32 are
-// updated at once.
+// one colour cell of 8 x 4 x 4 voxels, one warp: lane = (x = lane & 7, y = lane >> 3) owns the column of 4 voxels along z,
+// so the per-column part of eq. 5 is hoisted.  (ic, jc) = the lane's column in the full colour grid, kcg / kcl = the cell's
+// first layer in the full grid / in this shard.  Voxels that pass the gate are appended to the warp's stage, layer by
+// layer (n = its fill level, warp-uniform); full groups of 32 are updated at once.
 template <bool COUNT, int VAR>
-__device__ __forceinline__ void colour_cell(const Params &p, bool near, int ic0, int jc, int kcg, int kcl, Stage &st, int &n, int lane, Counts &c)
+__device__ __forceinline__ void colour_cell(const Params &p, bool near, int ic, int jc, int kcg, int kcl, Stage &st, int &n, int lane, Counts &c)
 {
     const float fx = p.fx, fy = p.fy, cx_ = p.cx, cy_ = p.cy, sig2 = p.sig2;
     const uint32_t wd = (uint32_t)p.wd, wbits = __float_as_uint(p.wd_f), hbits = __float_as_uint(p.hd_f), koff = 0x4B400000u * (wd + 1u);
     const float4 *__restrict__ pixmap = p.pixmap;
-    const bool act = ic0 < p.cnx && jc < p.cny && kcg < p.cnz;
+    const bool in_xy = ic < p.cnx && jc < p.cny;
+    const float px = __fmaf_rn((float)ic + 0.5f, p.vc, p.ox);
     const float py = __fmaf_rn((float)jc + 0.5f, p.vc, p.oy);
-    const float pz = __fmaf_rn((float)kcg + 0.5f, p.vc, p.oz);
-    float X[4], Y[4], Z[4], W[4];
-#pragma unroll
-    for (int e = 0; e < 4; ++e) {                                     // S4: eq. 5
-        const float px = __fmaf_rn((float)(ic0 + e) + 0.5f, p.vc, p.ox);
-        X[e] = __fmaf_rn(p.R[2], pz, __fmaf_rn(p.R[1], py, __fmaf_rn(p.R[0], px, p.t[0])));
-        Y[e] = __fmaf_rn(p.R[5], pz, __fmaf_rn(p.R[4], py, __fmaf_rn(p.R[3], px, p.t[1])));
-        Z[e] = __fmaf_rn(p.R[8], pz, __fmaf_rn(p.R[7], py, __fmaf_rn(p.R[6], px, p.t[2])));
-    }
-    unsigned pass = 0;
+    const float bX = __fmaf_rn(p.R[1], py, __fmaf_rn(p.R[0], px, p.t[0]));      // S4: eq. 5, the part that does not depend on z
+    const float bY = __fmaf_rn(p.R[4], py, __fmaf_rn(p.R[3], px, p.t[1]));
+    const float bZ = __fmaf_rn(p.R[7], py, __fmaf_rn(p.R[6], px, p.t[2]));
+    const float kf0 = (float)kcg + 0.5f;
+    float X[4], Y[4], Z[4];
     float4 pm[4];
+    bool pass[4];
     if (near) {
 #pragma unroll
         for (int e = 0; e < 4; ++e) {
+            const float pz = __fmaf_rn(__fadd_rn(kf0, (float)e), p.vc, p.oz);
+            X[e] = __fmaf_rn(p.R[2], pz, bX); Y[e] = __fmaf_rn(p.R[5], pz, bY); Z[e] = __fmaf_rn(p.R[8], pz, bZ);
+            const bool act = in_xy && kcg + e < p.cnz;
             pm[e] = act ? col_voxel_gate_ref(p, X[e], Y[e], Z[e]) : make_float4(0.0f, 0.0f, 0.0f, 0.0f);
-            W[e] = pm[e].w;
-            if (W[e] > 0.0f) pass |= 1u << e;
+            pass[e] = pm[e].w > 0.0f;
         }
     } else {
         uint32_t off[4]; bool ok[4];
 #pragma unroll
-        for (int e = 0; e < 4; ++e) project_fast(fx, fy, cx_, cy_, wd, wbits, hbits, koff, X[e], Y[e], Z[e], ok[e], off[e]);   // eq. 6
+        for (int e = 0; e < 4; ++e) {
+            const float pz = __fmaf_rn(__fadd_rn(kf0, (float)e), p.vc, p.oz);
+            X[e] = __fmaf_rn(p.R[2], pz, bX); Y[e] = __fmaf_rn(p.R[5], pz, bY); Z[e] = __fmaf_rn(p.R[8], pz, bZ);
+            project_fast(fx, fy, cx_, cy_, wd, wbits, hbits, koff, X[e], Y[e], Z[e], ok[e], off[e]);   // eq. 6
+        }
 #pragma unroll
         for (int e = 0; e < 4; ++e) pm[e] = __ldg(pixmap + off[e]);      // eq. 7-8 and W per pixel (S1)
 #pragma unroll
         for (int e = 0; e < 4; ++e) {                                 // S5: sigma gate (L108)
             const float dx = __fsub_rn(X[e], pm[e].x), dy = __fsub_rn(Y[e], pm[e].y), dz = __fsub_rn(Z[e], pm[e].z);
             const float d2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
-            const bool in = act && ok[e] && (pm[e].w > 0.0f) && !(d2 > sig2);
-            W[e] = pm[e].w;
-            if (in) pass |= 1u << e;
+            pass[e] = in_xy && kcg + e < p.cnz && ok[e] && (pm[e].w > 0.0f) && !(d2 > sig2);
         }
     }
-    // compact: exclusive prefix of the per-lane counts
-    const int cnt = __popc(pass);
-    int pre = cnt;
+    if (COUNT) c.n[CNT_COL_GATED] += in_xy ? (unsigned long long)max(0, min(4, p.cnz - kcg)) : 0ull;
+    // compact, layer by layer: one vote each; a full group of 32 is updated at once
+    const unsigned lt = (1u << lane) - 1u;
+    const size_t col0 = ((size_t)kcl * (size_t)p.cny + (size_t)jc) * (size_t)p.cnx + (size_t)ic, clayer = (size_t)p.cny * (size_t)p.cnx;
 #pragma unroll
-    for (int o = 1; o < 32; o <<= 1) { const int v = __shfl_up_sync(0xffffffffu, pre, o); if (lane >= o) pre += v; }
-    const int total = __shfl_sync(0xffffffffu, pre, 31);
-    if (total == 0) return;
-    int slot = n + pre - cnt;
-    const size_t base = ((size_t)kcl * (size_t)p.cny + (size_t)jc) * (size_t)p.cnx + (size_t)ic0;
-    // start the DRAM access of the stored words now; the update reads them a few hundred cycles later
-    if (pass) asm volatile("prefetch.global.L2 [%0];" ::"l"(p.col + base));
-#pragma unroll
-    for (int e = 0; e < 4; ++e)
-        if (pass & (1u << e)) {
-            st.rec[slot] = VAR == VAR_HD_FROM_DEPTH_POINT ? make_float4(pm[e].x, pm[e].y, pm[e].z, W[e]) : make_float4(X[e], Y[e], Z[e], W[e]);
-            const size_t a = base + (size_t)e;
+    for (int e = 0; e < 4; ++e) {
+        const unsigned b = __ballot_sync(0xffffffffu, pass[e]);
+        if (b == 0u) continue;                                        // warp-uniform
+        if (pass[e]) {
+            const size_t a = col0 + (size_t)e * clayer;
+            // start the DRAM access of the stored word now; the update reads it a few hundred cycles later
+            asm volatile("prefetch.global.L2 [%0];" ::"l"(p.col + a));
+            const int slot = n + __popc(b & lt);
+            st.rec[slot] = VAR == VAR_HD_FROM_DEPTH_POINT ? pm[e] : make_float4(X[e], Y[e], Z[e], pm[e].w);
             st.adr[slot] = make_uint2((uint32_t)a, (uint32_t)(a >> 32));
-            ++slot;
         }
-    n += total;
-    __syncwarp();
-    while (n >= 32) { n -= 32; colour_update_staged<COUNT, VAR>(p, st, n, 32, lane, c); }
-    __syncwarp();
+        n += __popc(b);
+        __syncwarp();
+        if (n >= 32) { n -= 32; colour_update_staged<COUNT, VAR>(p, st, n, 32, lane, c); __syncwarp(); }
+    }
 }
 
 // one colour work item, one warp: the set bits of one nibble of a shell-mark word are up to 4 colour cells of one tile.
-// The ticket of the next item is drawn before the LAST cell: its latency is hidden, yet no item waits reserved behind a
-// long one.
 template <int R, bool COUNT, int VAR>
-__device__ __forceinline__ void colour_item(const Params &p, uint32_t item, Stage &st, int &n, int lane, Counts &c, uint32_t *cursor, uint32_t &ticket)
+__device__ __forceinline__ void colour_item(const Params &p, uint2 item, Stage &st, int &n, int lane, Counts &c)
 {
-    const bool near = (item & ITEM_NEAR) != 0u;
-    constexpr int CX = cells_x(R), CY = cells_y(R), WPT = words_per_tile(R);
+    constexpr int CX = cells_x(R), CY = cells_y(R);
     int ttx, tty, ttz, sub;
-    item_unpack(item, ttx, tty, ttz, sub);
+    item_unpack(item.x, ttx, tty, ttz, sub);
+    const bool near = tile_is_near(p, ttx, tty, ttz);
     const int word = sub >> 3;
-    const uint32_t wi = (uint32_t)((ttz * p.tiles_y + tty) * p.tiles_x + ttx) * WPT + (uint32_t)word, sh = 4u * ((uint32_t)sub & 7u);
-    uint32_t bits = 0;
-    if (lane == 0) {                                                      // consume this item's nibble of the marks (self-cleaning)
-        bits = __ldcg(p.marks + wi) & (0xfu << sh);
-        atomicAnd(p.marks + wi, ~(0xfu << sh));
-    }
-    bits = __shfl_sync(0xffffffffu, bits, 0);
+    uint32_t bits = item.y;
     const int cgx0 = ttx * TX * R, cgy0 = tty * TY * R;
     const int cgz0 = local_to_global_tz(p, ttz) * TZ * R, clz0 = ttz * TZ * R;
-    if (COUNT && lane == 0) atomicAdd(&p.ctrl[CTRL_CELLS], (uint32_t)__popc(bits));
-    if (bits == 0u) next_ticket(cursor, lane, ticket);
+    if (COUNT && lane == 0) atomicAdd(&p.ctrl[ST_CELLS], (uint32_t)__popc(bits));
     while (bits) {
         const int b = word * 32 + (__ffs(bits) - 1);
         bits &= bits - 1;
-        if (bits == 0u) next_ticket(cursor, lane, ticket);
         const int cx = b % CX, cy = (b / CX) % CY, cz = b / (CX * CY);
-        const int kz = cz * CLZ + (lane >> 3);
-        colour_cell<COUNT, VAR>(p, near, cgx0 + cx * CLX + 4 * (lane & 1), cgy0 + cy * CLY + ((lane >> 1) & 3), cgz0 + kz, clz0 + kz, st, n, lane, c);
+        colour_cell<COUNT, VAR>(p, near, cgx0 + cx * CLX + (lane & 7), cgy0 + cy * CLY + (lane >> 3), cgz0 + cz * CLZ, clz0 + cz * CLZ, st, n, lane, c);
     }
 }
 
-// phase: PHASE_ALL = the whole queue in one launch (frames already on the device); PHASE_GEO / PHASE_COL = the geometry
-// items / the colour items only, so that vol_integrate_host can run the geometry half while the HD frame is still being
-// copied (only the colour update reads it).
+// phase: PHASE_ALL = everything in one launch (frames already on the device); PHASE_GEO = the producer roles and the
+// geometry items; PHASE_COL = the colour items only -- so that vol_integrate_host can run everything that only needs the
+// depth image while the HD frame is still being copied (only the colour update reads it).
 enum { PHASE_ALL = 0, PHASE_GEO = 1, PHASE_COL = 2 };
+#ifndef VF_COL_BATCH
+#define VF_COL_BATCH 4
+#endif
+constexpr uint32_t COL_BATCH = VF_COL_BATCH, COL_BATCH_TAIL = 12, GEO_BATCH = 2;
+// per-warp state of the consumer loop (shared memory; written by lane 0 between __syncwarp()s, read by every lane)
+enum : uint32_t { F_GEO_DONE = 1u, F_COL_DONE = 2u, F_MARKS_SET = 4u, F_SCAN_CLAIMED = 8u, F_COL_READY = 16u, F_CLS_COMPLETE = 32u };
+struct WarpState {
+    uint32_t flags;                 // F_*
+    uint32_t gt, gt_left;           // next geometry ticket of the warp and how many of its batch are left
+    uint32_t ct, ct_size;           // first ticket and size of the NEXT batch of colour items
+    uint32_t cb_left, cb_idx;       // the current batch: items left, index of the next one
+    uint32_t n_col;                 // length of the colour work list (once it is final)
+    int      n_staged;              // fill level of the warp's stage
+    uint32_t cb_item[COL_BATCH][2]; // the current batch
+};
+#ifndef VF_MIN_CTAS
+#define VF_MIN_CTAS 4
+#endif
 
 template <int R, bool COUNT, int VAR>
-__global__ void __launch_bounds__(CTA, 4) k_fused(const __grid_constant__ Params p, int phase)
+__global__ void __launch_bounds__(CTA, VF_MIN_CTAS) k_fused(const __grid_constant__ Params p, int phase)
 {
     __shared__ Stage s_stage[WARPS_PER_CTA];
+    __shared__ WarpState s_state[WARPS_PER_CTA];
     const int lane = threadIdx.x & 31;
     Stage &st = s_stage[threadIdx.x >> 5];
     pdl_wait();
-    // queue order, longest kind first: NEAR geometry tiles, colour items, ordinary geometry tiles (the shortest: the tail)
-    const uint32_t c_near = __ldcg(&p.ctrl[CTRL_NNEAR]), c_col = __ldcg(&p.ctrl[CTRL_NCOL]), c_geo = __ldcg(&p.ctrl[CTRL_NGEO]);
-    const uint32_t n_near = phase == PHASE_COL ? 0u : c_near;
-    const uint32_t n_col = n_near + (phase == PHASE_GEO ? 0u : c_col);
-    const uint32_t n_items = n_col + (phase == PHASE_COL ? 0u : c_geo);
-    uint32_t *cursor = &p.ctrl[phase == PHASE_COL ? CTRL_CURSOR2 : CTRL_CURSOR];
-    Counts c = {0, 0, 0, 0};
-    int n_staged = 0;
-    // the ticket of the next item is requested before the current one is processed (the L2 round trip is hidden).
-    // Only one item is reserved ahead: colour items are long, and a deeper reservation unbalances the tail.
-    uint32_t ticket = 0;
-    next_ticket(cursor, lane, ticket);
-    for (;;) {
-        const uint32_t it = __shfl_sync(0xffffffffu, ticket, 0);
-        if (it >= n_items) break;
-        const uint32_t item = it < n_near ? __ldcg(p.work_geo + ((uint32_t)p.n_tiles - 1u - it))
-                                          : (it < n_col ? __ldcg(p.work_col + (it - n_near)) : __ldcg(p.work_geo + (it - n_col)));
-        if (it >= n_near && it < n_col) colour_item<R, COUNT, VAR>(p, item, st, n_staged, lane, c, cursor, ticket);
-        else {
-            next_ticket(cursor, lane, ticket);
-            geometry_prefetch(p, item, lane);
-            geometry_tile<COUNT, VAR>(p, item, lane, c);
+    uint32_t *ctrl = p.ctrl;
+    const uint32_t n_tiles = (uint32_t)p.n_tiles;
+    const uint32_t n_cls = (n_tiles + CLS_CHUNK - 1) / CLS_CHUNK, n_scan = (n_tiles + SCAN_CHUNK - 1) / SCAN_CHUNK;
+    uint32_t n_mark = 0;
+    Counts c;
+    if (COUNT) {
+#pragma unroll
+        for (int k = 0; k < CNT_N; ++k) c.n[k] = 0ull;
+    }
+    const uint32_t gw = blockIdx.x * WARPS_PER_CTA + (threadIdx.x >> 5), n_warps = gridDim.x * WARPS_PER_CTA;
+    VF_T(0);
+    // ---- producer roles: the classification (it feeds the geometry queue), then the shell marks.  The first classification
+    //      chunk of a warp is its own number in the grid (no atomic: thousands of warps start at the same moment); every other
+    //      chunk is claimed from a counter, so that no chunk ever waits for a warp that is busy with an item.
+    if (phase != PHASE_COL) {
+        const uint32_t njobs = min(__ldcg(&ctrl[Q_NJOBS0 + p.parity]), p.jobs_cap);
+        n_mark = (njobs + MARK_CHUNK - 1) / MARK_CHUNK;
+        if (gw == 0 && lane == 0) ctrl[ST_NJOBS] = njobs;
+        for (uint32_t k = gw; k < n_cls; k = n_cls <= n_warps ? n_cls : n_warps + claim(&ctrl[Q_CLS_CLAIM], lane)) {
+            classify_chunk(p, k, lane);
+            chunk_done(&ctrl[Q_CLS_DONE], lane);
+        }
+        VF_T(1);
+        for (;;) {
+            const uint32_t k = claim(&ctrl[Q_MARK_CLAIM], lane);
+            if (k >= n_mark) break;
+            mark_chunk<R>(p, k, njobs, lane);
+            chunk_done(&ctrl[Q_MARK_DONE], lane);
         }
     }
+    VF_T(2);
+#ifdef VF_TRACE
+    unsigned long long tr_ngeo = 0, tr_ncol = 0, tr_sleep = 0, tr_tgeo = 0, tr_tcol = 0, tr_tscan = 0, tr_ovg = 0, tr_ovc = 0, tr_top = 0;
+#endif
+    // ---- consumer: colour items once they exist (they are the longer ones), geometry items otherwise.
+    // Every access to the queues is an L2 round trip of the order of a microsecond under load, so a round of the loop first
+    // ISSUES whatever it may need (the progress counter it is watching, the slot of its geometry ticket) and only then looks at
+    // the answers; tickets are drawn for several items at once.  The state of the loop lives in shared memory: the items need
+    // every register, and what is kept in shared memory is not spilled to (cached, evictable) local memory around them.
+    volatile WarpState &ws = s_state[threadIdx.x >> 5];
+    if (lane == 0) {
+        ws.flags = phase == PHASE_COL ? (F_GEO_DONE | F_MARKS_SET | F_SCAN_CLAIMED) : 0u;
+        ws.gt = 0u; ws.gt_left = 0u; ws.ct = 0u; ws.ct_size = 1u; ws.cb_left = 0u; ws.cb_idx = 0u; ws.n_col = 0u; ws.n_staged = 0;
+    }
+    __syncwarp();
+    for (;;) {
+#ifdef VF_TRACE
+        tr_top = clock64();
+#endif
+        uint32_t flags = ws.flags;
+        // -- requests
+        uint32_t v_poll = 0u, v_slot = 0u;
+        const int watching = (flags & (F_COL_DONE | F_COL_READY)) ? 0 : (!(flags & F_MARKS_SET) ? 1 : ((flags & F_SCAN_CLAIMED) ? 2 : 0));
+        if (watching == 1) v_poll = ld_relaxed(&ctrl[Q_MARK_DONE]);
+        if (watching == 2) v_poll = ld_relaxed(&ctrl[Q_SCAN_DONE]);
+        const bool geo_turn = !(flags & F_GEO_DONE) && (flags & (F_COL_READY | F_COL_DONE)) != F_COL_READY;   // colour items, when there are any, come first
+        uint32_t gt = ws.gt;
+        if (geo_turn && ws.gt_left == 0u) {
+            gt = claim_n(&ctrl[Q_GEO_CURSOR], GEO_BATCH, lane);
+            __syncwarp();
+            if (lane == 0) { ws.gt = gt; ws.gt_left = GEO_BATCH; }
+        }
+        if (geo_turn && gt < n_tiles) v_slot = ld_relaxed(p.work_geo + gt);
+        // -- answers
+        if (watching == 1 && v_poll >= n_mark) { flags |= F_MARKS_SET; VF_T(3); }
+        if (watching == 2 && v_poll >= (phase == PHASE_COL ? 0u : n_scan)) {
+            flags |= F_COL_READY;
+            VF_T(5);
+            const uint32_t nc = __ldcg(&ctrl[ST_NCOL]), t = claim_n(&ctrl[Q_COL_CURSOR], 1u, lane);
+            __syncwarp();
+            if (lane == 0) { ws.n_col = nc; ws.ct = t; ws.ct_size = 1u; }
+        }
+        if ((flags & (F_MARKS_SET | F_SCAN_CLAIMED)) == F_MARKS_SET) {
+            const uint32_t k = claim(&ctrl[Q_SCAN_CLAIM], lane);
+            if (k < n_scan) {
+#ifdef VF_TRACE
+                const unsigned long long t0 = clock64();
+#endif
+                scan_chunk<R>(p, k, lane);
+                chunk_done(&ctrl[Q_SCAN_DONE], lane);
+#ifdef VF_TRACE
+                tr_tscan += clock64() - t0;
+#endif
+            } else {
+                flags |= F_SCAN_CLAIMED;
+                VF_T(4);
+                if (phase == PHASE_GEO) flags |= F_COL_DONE;          // the colour items are left to the next launch
+            }
+        }
+        __syncwarp();
+        if (lane == 0) ws.flags = flags;
+        __syncwarp();
+        if ((flags & (F_COL_READY | F_COL_DONE)) == F_COL_READY) {
+            // Colour items are taken in batches: one ticket and one load for up to COL_BATCH of them; single items towards
+            // the end of the list, where balance matters.
+            uint32_t cb_left = ws.cb_left;
+            if (cb_left == 0u) {
+                const uint32_t ct = ws.ct, n_col = ws.n_col;
+                if (ct < n_col) {
+                    cb_left = min(ws.ct_size, n_col - ct);
+                    if ((uint32_t)lane < cb_left) { const uint2 it = __ldcg(p.work_col + ct + lane); ws.cb_item[lane][0] = it.x; ws.cb_item[lane][1] = it.y; }
+                    const uint32_t sz = n_col - ct > COL_BATCH_TAIL * n_warps ? COL_BATCH : 1u;
+                    const uint32_t t = claim_n(&ctrl[Q_COL_CURSOR], sz, lane);
+                    __syncwarp();
+                    if (lane == 0) { ws.ct = t; ws.ct_size = sz; ws.cb_idx = 0u; ws.cb_left = cb_left; }
+                } else {
+                    if (lane == 0) ws.flags = flags | F_COL_DONE;
+                    VF_T(6);
+                }
+                __syncwarp();
+            }
+            if (cb_left != 0u) {
+                const uint32_t idx = ws.cb_idx;
+                const uint2 item = make_uint2(ws.cb_item[idx][0], ws.cb_item[idx][1]);
+                int n_staged = ws.n_staged;
+                __syncwarp();
+                if (lane == 0) { ws.cb_idx = idx + 1u; ws.cb_left = cb_left - 1u; }
+#ifdef VF_TRACE
+                const unsigned long long t0 = clock64();
+                tr_ovc += t0 - tr_top;
+#endif
+                colour_item<R, COUNT, VAR>(p, item, st, n_staged, lane, c);
+#ifdef VF_TRACE
+                tr_ncol++; tr_tcol += clock64() - t0;
+#endif
+                __syncwarp();
+                if (lane == 0) ws.n_staged = n_staged;
+                __syncwarp();
+            }
+            continue;
+        }
+        if (geo_turn) {
+            bool complete = (flags & F_CLS_COMPLETE) != 0u || gt >= n_tiles;
+            if (v_slot == 0u && !complete) {                          // not published yet -- or beyond the end of the list?
+                complete = ld_relaxed(&ctrl[Q_CLS_DONE]) >= n_cls;
+                if (complete && gt < n_tiles) v_slot = ld_relaxed(p.work_geo + gt);
+            }
+            if (v_slot != 0u) {
+                if (lane == 0) { p.work_geo[gt] = 0u; ws.gt = gt + 1u; ws.gt_left = ws.gt_left - 1u; }   // the list is all zero again when the frame is done
+                geometry_prefetch(p, v_slot, lane);
+#ifdef VF_TRACE
+                const unsigned long long t0 = clock64();
+                tr_ovg += t0 - tr_top;
+#endif
+                geometry_tile<COUNT, VAR>(p, v_slot, lane, c);
+#ifdef VF_TRACE
+                tr_ngeo++; tr_tgeo += clock64() - t0;
+#endif
+                __syncwarp();
+                continue;
+            }
+            if (complete) {                                           // every item below the final count has been taken
+                flags |= F_CLS_COMPLETE | F_GEO_DONE;
+                __syncwarp();
+                if (lane == 0) ws.flags = flags;
+                __syncwarp();
+            }
+        }
+        if ((flags & (F_GEO_DONE | F_COL_DONE)) == (F_GEO_DONE | F_COL_DONE)) break;
+        if (watching == 0 && !geo_turn) continue;
+        if (flags & F_GEO_DONE || v_slot == 0u) {
+            __nanosleep(100);                                         // waiting for claimed producer chunks to finish
+#ifdef VF_TRACE
+            tr_sleep++;
+#endif
+        }
+    }
+    int n_staged = ws.n_staged;
+    VF_T(8);
+    VF_TC(9, tr_ngeo); VF_TC(10, tr_ncol); VF_TC(11, tr_sleep); VF_TC(12, tr_tgeo); VF_TC(13, tr_tcol); VF_TC(14, tr_tscan); VF_TC(15, tr_ovg); VF_TC(7, tr_ovc);
     if (n_staged > 0) colour_update_staged<COUNT, VAR>(p, st, 0, n_staged, lane, c);
     if (COUNT) {
 #pragma unroll
-        for (int o = 16; o > 0; o >>= 1) {
-            c.gr += __shfl_xor_sync(0xffffffffu, c.gr, o); c.gc += __shfl_xor_sync(0xffffffffu, c.gc, o);
-            c.cr += __shfl_xor_sync(0xffffffffu, c.cr, o); c.cc += __shfl_xor_sync(0xffffffffu, c.cc, o);
-        }
-        if (lane == 0) {
-            if (c.gr) atomicAdd(&p.counters[0], c.gr);
-            if (c.gc) atomicAdd(&p.counters[1], c.gc);
-            if (c.cr) atomicAdd(&p.counters[2], c.cr);
-            if (c.cc) atomicAdd(&p.counters[3], c.cc);
+        for (int k = 0; k < CNT_N; ++k) {
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) c.n[k] += __shfl_xor_sync(0xffffffffu, c.n[k], o);
+            if (lane == 0 && c.n[k]) atomicAdd(&p.counters[k], c.n[k]);
         }
     }
 }

@@ -15,7 +15,8 @@ namespace vf {
 constexpr int TX = 32, TY = 4, TZ = 8;
 // colour cell (shell-mark / work unit, one warp pass): 8 x 4 x 4 colour voxels = 32 lanes x uint4
 constexpr int CLX = 8, CLY = 4, CLZ = 4;
-// tile classification refines a tile that passes the coarse test on SUBX x 1 x SUBZ sub-boxes
+// tile classification refines a tile that passes the coarse test on SUBX x 1 x SUBZ sub-boxes of 8 x 4 x 4 voxels; the
+// fused kernel visits only the sub-boxes that pass (one warp pass each: lane = (x, y) column of 4 voxels along z)
 constexpr int SUBX = 4, SUBZ = 2;
 constexpr int BRICK = 32;                                   // ray-casting skip brick: BRICK^3 geometry voxels = 1 x 8 x 4 tiles
 constexpr int WARPS_PER_CTA = 8;
@@ -63,27 +64,32 @@ struct Params {
     const uint8_t  *rgb;
     uint32_t *geo;               // this shard's geometry words
     uint32_t *col;               // this shard's colour words
+    float    *depthf;            // S1 output: D = depth_mm * 0.001f per depth pixel (0 = invalid), what the TSDF update gathers
     float4   *pixmap;            // S1 output: {X_vd, Y_vd, Z_vd, W} per depth pixel; W = 0 when no colour update is possible
     uint32_t *pyr;               // min/max valid-depth pyramid: entry = min_mm | max_mm << 16 (0xffff / 0 = empty)
-    int       pyr_off[12], pyr_w[12], pyr_h[12], pyr_levels;
-    uint4    *jobs;              // shell-mark jobs of the frame (one per 4 x 4 pixel patch or per pixel), wd x hd (rounded up to 4) entries
-    uint32_t *work_geo;          // geometry work list (n_tiles entries): ordinary tiles from the front, ITEM_NEAR tiles from the back
+    int       pyr_off[3], pyr_w[3], pyr_h[3], pyr_levels;   // levels: blocks of 8, 16, 32 pixels (fewer for tiny images)
+    uint4    *jobs;              // shell-mark jobs of the frame (per 4 x 4 pixel patch: one, or one per strip, or one per pixel), jobs_cap entries
+    uint32_t  jobs_cap;
+    int       parity;            // frame parity: which of the two job counters this frame uses (the other one is zeroed)
+    uint32_t *work_geo;          // geometry work list (n_tiles entries, all zero between frames: a slot is cleared by the warp that takes it)
     uint32_t *marks;             // shell marks: words_per_tile(r) words per tile, bit = colour cell that may hold sigma-shell voxels
-    uint32_t *work_col;          // colour work list: one item per non-zero mark NIBBLE (up to 4 colour cells)
+    uint2    *work_col;          // colour work list: one item per non-zero mark NIBBLE (up to 4 colour cells): {tile | nibble index, the nibble's bits}
     uint8_t  *tile_neg;          // per geometry tile: 1 = the tile may hold an observed voxel with tsdf <= 0.  Set by the tile
                                  // classification (k_mark_classify), never cleared except by vol_reset (vol_upload sets
                                  // all): a conservative superset, used by the ray caster to skip free space
     uint8_t  *brick_neg;         // the same per brick of BRICK^3 geometry voxels (1 x 8 x 4 tiles): the ray caster's coarse level
     int       bricks_x, bricks_y, bricks_z;
-    uint32_t *ctrl;              // control words, see CTRL_* below
-    unsigned long long *counters;// 4 voxel counters (counting variant only)
+    uint32_t *ctrl;              // statistics record and queue control words, see ST_* / Q_* below
+    unsigned long long *counters;// voxel and sector counters (counting variant only), see CNT_*
 };
 
-// work items (32 bits): [6:0] ttx | [15:7] tty | [23:16] ttz (local slab) = tile coordinates, [30:24] sub = index of the
-// mark NIBBLE within the tile (colour items only), [31] ITEM_NEAR = the tile's box comes within 2 mm of the camera plane
-// (or behind it), so its voxels may have Z <= 0 or Z outside the range of the branch-free reciprocal.
+// work items (32 bits): [6:0] ttx | [15:7] tty | [23:16] ttz (local slab) = tile coordinates, and
+//   geometry items: [31:24] = mask of the tile's SUBX x 1 x SUBZ sub-boxes (bit bx * SUBZ + bz) that may hold a voxel this frame
+//                   updates (never 0, so a non-zero slot of the geometry work list is a published item);
+//   colour items:   [30:24] = index of the mark NIBBLE within the tile.
+// Whether a tile is NEAR (its box comes within 2 mm of the camera plane, or behind it: voxels may have Z <= 0 or Z outside
+// the range of the branch-free reciprocal) is recomputed by the consumer from the tile's coordinates (tile_is_near).
 // vol_create rejects volumes with more than 128 x 512 x 256 tiles per shard.
-constexpr uint32_t ITEM_NEAR = 1u << 31;
 constexpr int ITEM_Y_SHIFT = 7, ITEM_Z_SHIFT = 16, ITEM_SUB_SHIFT = 24;
 constexpr int ITEM_MAX_TX = 128, ITEM_MAX_TY = 512, ITEM_MAX_TZ = 256;
 __device__ __forceinline__ uint32_t item_pack(int ttx, int tty, int ttz, int sub)
@@ -93,10 +99,27 @@ __device__ __forceinline__ uint32_t item_pack(int ttx, int tty, int ttz, int sub
 __device__ __forceinline__ void item_unpack(uint32_t item, int &ttx, int &tty, int &ttz, int &sub)
 {
     ttx = (int)(item & 127u); tty = (int)((item >> ITEM_Y_SHIFT) & 511u); ttz = (int)((item >> ITEM_Z_SHIFT) & 255u);
-    sub = (int)((item >> ITEM_SUB_SHIFT) & 127u);
+    sub = (int)(item >> ITEM_SUB_SHIFT);
 }
 
-enum { CTRL_NGEO = 0, CTRL_NCOL = 1, CTRL_CURSOR = 2, CTRL_TICKET = 3, CTRL_CELLS = 4, CTRL_NJOBS = 5, CTRL_NNEAR = 6, CTRL_CURSOR2 = 7, CTRL_N = 8 };
+// ctrl[]: the first VOL_STATS_RAW_BYTES (128) are the statistics record vol_frame_stats* copies out: 8 words ST_*, then 12
+// 64-bit counters CNT_* (p.counters).  The queue control words Q_* follow; all of them are zeroed by k_prepass (the two job
+// counters alternately, see Params::parity).
+enum { ST_NGEO = 0, ST_NCOL = 1, ST_CELLS = 2, ST_SUBS = 3, ST_NJOBS = 4, ST_N = 8 };
+enum { CNT_GEO_READ = 0, CNT_GEO_CHANGED, CNT_COL_READ, CNT_COL_CHANGED, CNT_GEO_SEC_READ, CNT_GEO_SEC_WRITTEN, CNT_COL_SEC_READ,
+       CNT_COL_SEC_WRITTEN, CNT_GEO_VISITED, CNT_COL_GATED, CNT_SPARE0, CNT_SPARE1, CNT_N = 12 };
+constexpr int CTRL_Q0 = 32;                                  // first queue-control word (byte 128)
+// every queue-control word has a 128-byte line (and so, by the address hash, most likely an L2 slice) of its own: thousands
+// of warps draw tickets from and poll these words, and requests to one line are served one after the other
+constexpr int QS = 32;
+enum { Q_CLS_CLAIM = CTRL_Q0, Q_CLS_DONE = CTRL_Q0 + QS, Q_MARK_CLAIM = CTRL_Q0 + 2 * QS, Q_MARK_DONE = CTRL_Q0 + 3 * QS,
+       Q_SCAN_CLAIM = CTRL_Q0 + 4 * QS, Q_SCAN_DONE = CTRL_Q0 + 5 * QS, Q_GEO_CURSOR = CTRL_Q0 + 6 * QS, Q_COL_CURSOR = CTRL_Q0 + 7 * QS,
+       Q_NJOBS0 = CTRL_Q0 + 8 * QS, Q_NJOBS1 = Q_NJOBS0 + 1,
+       // min / max valid depth (mm) of the whole frame, two sets used alternately like the job counters
+       Q_DMIN0 = CTRL_Q0 + 9 * QS, Q_DMIN1, Q_DMAX0, Q_DMAX1, CTRL_N = CTRL_Q0 + 10 * QS };
+constexpr int CLS_CHUNK = 32;                                // tiles per classification chunk (one lane each)
+constexpr int SCAN_CHUNK = 128;                              // tiles per scan chunk (four per lane)
+constexpr int MARK_CHUNK = 8;                                // mark jobs per chunk (4 lanes each)
 
 // programmatic dependent launch: wait for the previous kernel of the stream (completion + memory flush) / allow the next
 // kernel's CTAs to be scheduled as this one drains
@@ -122,12 +145,14 @@ __device__ __forceinline__ bool project_px(float fx, float fy, float cx, float c
 }
 
 // culling only: min/max valid depth (mm) over the inclusive pixel rectangle [x0,x1] x [y0,y1] (already clamped to the
-// image), from the coarsest-needed pyramid level: at most 3 x 3 entries are read.
+// image), from the coarsest-needed pyramid level (blocks of 8, 16 or 32 pixels): at most 3 x 3 entries are read.  A rectangle
+// larger than 3 x 3 blocks of the top level gets the range of the whole frame.
 __device__ __forceinline__ void depth_range(const Params &p, int x0, int x1, int y0, int y1, uint32_t &mn, uint32_t &mx)
 {
     int l = 0;
     while (l + 1 < p.pyr_levels && (((x1 >> (3 + l)) - (x0 >> (3 + l))) > 2 || ((y1 >> (3 + l)) - (y0 >> (3 + l))) > 2)) ++l;
     const int bx0 = x0 >> (3 + l), bx1 = x1 >> (3 + l), by0 = y0 >> (3 + l), by1 = y1 >> (3 + l);
+    if (bx1 - bx0 > 2 || by1 - by0 > 2) { mn = __ldcg(&p.ctrl[Q_DMIN0 + p.parity]); mx = __ldcg(&p.ctrl[Q_DMAX0 + p.parity]); return; }
     mn = 0xffffu; mx = 0u;
     const uint32_t *lev = p.pyr + p.pyr_off[l];
     const int lw = p.pyr_w[l];
@@ -170,20 +195,6 @@ __device__ __forceinline__ bool box_rect(const Params &p, float cX, float cY, fl
         x0 = 0; x1 = p.wd - 1; y0 = 0; y1 = p.hd - 1;
     }
     return true;
-}
-
-// culling only: can any voxel of the camera-space box (centre c, half extents e) pass the TSDF tests (frustum, valid
-// depth, sdf >= -mu)?  Conservative: max valid depth over the box's pixel rectangle against the box's nearest Z.
-// Returns 0 = no, 1 = maybe, 2 = maybe and the whole box lies in front of every valid depth of its rectangle (free space:
-// a finer look at the box would find the same).
-__device__ __forceinline__ int box_may_update(const Params &p, float cX, float cY, float cZ, float eX, float eY, float eZ)
-{
-    int x0, x1, y0, y1; float zmin, zmax;
-    if (!box_rect(p, cX, cY, cZ, eX, eY, eZ, x0, x1, y0, y1, zmin, zmax)) return 0;
-    uint32_t mn, mx;
-    depth_range(p, x0, x1, y0, y1, mn, mx);
-    if (mx == 0u || !(zmin <= ((float)mx * 0.001f + 1e-4f) + p.mu)) return 0;
-    return zmax <= (float)mn * 0.001f - 1e-4f ? 2 : 1;
 }
 
 }  // namespace vf

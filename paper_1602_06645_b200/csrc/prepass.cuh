@@ -1,4 +1,6 @@
-// prepass.cuh -- S1 (per-pixel map, depth pyramid, shell marks) and S9 (tile classification) kernels.
+// prepass.cuh -- S1 (per-pixel map, depth pyramid, shell-mark jobs: kernel k_prepass) and the producer roles of the fused
+// kernel: S9 for geometry (classification of tiles and their sub-boxes), the shell marks (S1 continued) and S9 for colour
+// (work items from the marks).
 #pragma once
 #include "params.cuh"
 
@@ -105,28 +107,38 @@ __device__ __forceinline__ bool shell_box(const Params &p, float xa, float xb, f
 //  (a) pixel map: everything of eq. 7-8 and the view weight (L110) depends only on the depth pixel, so it is computed
 //      once per pixel instead of once per colour voxel: {X_vd, Y_vd, Z_vd, W}; W = 0 encodes "no colour update possible"
 //      (invalid depth, missing forward neighbour (A7), degenerate normal, W <= 0 (A8)).
-//  (b) min/max valid depth per 8x8, 16x16, 32x32 block (pyramid levels 0-2); the last CTA to finish builds the coarser
-//      levels.  Used to cull geometry tiles.
-//  (c) shell marks: a colour voxel can pass the sigma gate (L108) only inside the frustum piece of shell_box().  Every
-//      4 x 4 pixel patch marks the colour cells that meet the world-space bounding box of its piece if that box is at most
-//      PATCH_SPREAD_MAX x larger than a compact piece's, else (depth edge, grazing surface) the boxes of its pixels' own pieces.  This kernel only
-//      queues the boxes as jobs; k_mark_classify deals them evenly over the whole GPU (depth edges cluster in a few CTAs here).
-//      Marks are consumed (and cleared) by the fused kernel.
-constexpr float PATCH_SPREAD_MAX = 2.4f;
+//      Beside it the depth in metres as a float map (what the TSDF update gathers).
+//  (b) min/max valid depth per 8x8, 16x16, 32x32 block (pyramid levels 0-2) and of the whole frame (two atomics per CTA).
+//      Used to cull geometry tiles.
+//  (c) shell-mark jobs: a colour voxel can pass the sigma gate (L108) only inside the frustum piece of shell_box().  Every
+//      4 x 4 pixel patch queues the world-space bounding box of its piece as ONE job if that box is at most PATCH_SPREAD_MAX x
+//      larger than a compact piece's (a smooth surface seen head-on).  Otherwise the patch is cut into its 4 rows or its 4
+//      columns, whichever have the smaller depth ranges (a surface seen at a grazing angle: the pieces of the strips are
+//      staggered along the view direction, and their boxes follow the shear that one box for the patch would fill in) --
+//      or, if even those ranges exceed STRIP_RANGE_MAX (a depth edge), into its pixels.
+//      The fused kernel's warps turn the jobs into marks: bits of the colour cells that meet a job's box.  Marks are
+//      consumed (and cleared) by the fused kernel.
+constexpr float PATCH_SPREAD_MAX = 2.4f, STRIP_RANGE_MAX = 0.02f;
+enum { JOB_PATCH = 0, JOB_ROW = 1, JOB_COLUMN = 2, JOB_PIXEL = 3 };      // bits 31:30 of a job's first word: the pixels it covers
 
 template <int R>
 __global__ void __launch_bounds__(256) k_prepass(const __grid_constant__ Params p)
 {
     __shared__ uint32_t s_mn[16], s_mx[16];
-    __shared__ bool s_last;
     __shared__ uint32_t s_njobs, s_base;
-    __shared__ uint4 s_jobs[1024];      // mark jobs: {x | y << 15 | (4 x 4 patch ? 1 << 31 : single pixel), depth range of its eligible pixels}
+    __shared__ uint4 s_jobs[1024];      // mark jobs: {x | y << 15 | JOB_* << 30 of the first pixel, depth range of its eligible pixels}
     const int t = threadIdx.x, tx = t & 31, tq = t >> 5;
     pdl_launch_dependents();
     if (t < 16) { s_mn[t] = 0xffffu; s_mx[t] = 0u; }
     if (t == 0) s_njobs = 0u;
-    if (blockIdx.x == 0 && blockIdx.y == 0 && t == 0) {
-        p.ctrl[CTRL_NGEO] = 0; p.ctrl[CTRL_NCOL] = 0; p.ctrl[CTRL_CURSOR] = 0; p.ctrl[CTRL_CELLS] = 0; p.ctrl[CTRL_NNEAR] = 0; p.ctrl[CTRL_CURSOR2] = 0;
+    // statistics words and queue control of this frame start at zero (the previous frame's kernels have completed: this
+    // kernel is not a programmatic dependent launch)
+    // The job counter of the NEXT frame is zeroed here too, so that a frame that fails half-way never leaves a stale count
+    // behind for the frame that follows it.
+    if (blockIdx.x == 0 && blockIdx.y == 0) {
+        if (t < ST_N) p.ctrl[t] = 0u;
+        if (t < Q_NJOBS0 - CTRL_Q0 && t % QS == 0) p.ctrl[CTRL_Q0 + t] = 0u;
+        if (t == 0) { p.ctrl[Q_NJOBS0 + 1 - p.parity] = 0u; p.ctrl[Q_DMIN0 + 1 - p.parity] = 0xffffu; p.ctrl[Q_DMAX0 + 1 - p.parity] = 0u; }
     }
     __syncthreads();
     const int x = blockIdx.x * 32 + tx;
@@ -178,11 +190,10 @@ __global__ void __launch_bounds__(256) k_prepass(const __grid_constant__ Params 
                 if (out.w > 0.0f) zpx[m] = D;
             }
             p.pixmap[(size_t)y * p.wd + x] = out;
+            p.depthf[(size_t)y * p.wd + x] = out.z;                              // D, or 0 = invalid
         }
     }
-    // (c) phase 1: every 4 x 4 patch (4 lanes x 4 rows) queues one job for its whole piece if that is compact, else one
-    //     job per colour-eligible pixel (depth edge, grazing surface).  All shuffles are executed by the whole warp.
-    {
+    {   // (c) every 4 x 4 patch = 4 lanes x the thread's 4 rows.  All shuffles are executed by the whole warp.
         float zlo = 1e30f, zhi = -1e30f;
 #pragma unroll
         for (int m = 0; m < 4; ++m) if (zpx[m] > 0.0f) { zlo = fminf(zlo, zpx[m]); zhi = fmaxf(zhi, zpx[m]); }
@@ -191,6 +202,23 @@ __global__ void __launch_bounds__(256) k_prepass(const __grid_constant__ Params 
             zlo = fminf(zlo, __shfl_xor_sync(0xffffffffu, zlo, o));
             zhi = fmaxf(zhi, __shfl_xor_sync(0xffffffffu, zhi, o));
         }
+        // depth ranges of the patch's rows (over the 4 lanes) and of its columns (this lane's 4 pixels)
+        float rlo[4], rhi[4], clo = 1e30f, chi = -1e30f;
+#pragma unroll
+        for (int m = 0; m < 4; ++m) {
+            rlo[m] = zpx[m] > 0.0f ? zpx[m] : 1e30f; rhi[m] = zpx[m] > 0.0f ? zpx[m] : -1e30f;
+            clo = fminf(clo, rlo[m]); chi = fmaxf(chi, rhi[m]);
+#pragma unroll
+            for (int o = 1; o < 4; o <<= 1) {
+                rlo[m] = fminf(rlo[m], __shfl_xor_sync(0xffffffffu, rlo[m], o));
+                rhi[m] = fmaxf(rhi[m], __shfl_xor_sync(0xffffffffu, rhi[m], o));
+            }
+        }
+        float rmax = 0.0f, cmax = chi >= clo ? chi - clo : 0.0f;
+#pragma unroll
+        for (int m = 0; m < 4; ++m) if (rhi[m] >= rlo[m]) rmax = fmaxf(rmax, rhi[m] - rlo[m]);
+#pragma unroll
+        for (int o = 1; o < 4; o <<= 1) cmax = fmaxf(cmax, __shfl_xor_sync(0xffffffffu, cmax, o));
         if (zlo <= zhi) {
             const int xp = blockIdx.x * 32 + (tx & ~3), yp = blockIdx.y * 32 + tq * 4;
             int i0, i1, j0, j1, k0, k1;
@@ -199,18 +227,24 @@ __global__ void __launch_bounds__(256) k_prepass(const __grid_constant__ Params 
                 // a compact piece (smooth surface seen head-on) spans about n0 cells: 2 sigma deep, the patch's footprint wide
                 const float c = (float)CLY * p.vc, wfoot = 4.0f * zhi / p.fx;
                 const float n0 = (2.0f * p.sigma / c + 2.0f) * (wfoot / c + 2.0f) * (0.5f * wfoot / c + 2.0f);
+                const uint32_t xy = (uint32_t)xp | ((uint32_t)yp << 15);
                 if ((float)ncell <= PATCH_SPREAD_MAX * n0) {
-                    if ((tx & 3) == 0) {
-                        const uint32_t j = atomicAdd(&s_njobs, 1u);
-                        s_jobs[j] = make_uint4((uint32_t)xp | ((uint32_t)yp << 15) | 0x80000000u, __float_as_uint(zlo), __float_as_uint(zhi), 0u);
+                    if ((tx & 3) == 0) s_jobs[atomicAdd(&s_njobs, 1u)] = make_uint4(xy | ((uint32_t)JOB_PATCH << 30), __float_as_uint(zlo), __float_as_uint(zhi), 0u);
+                } else if (fminf(rmax, cmax) <= STRIP_RANGE_MAX) {
+                    if (rmax <= cmax) {                               // rows: lane m of the patch queues row m
+                        const int m = tx & 3;
+                        const float lo = m == 0 ? rlo[0] : m == 1 ? rlo[1] : m == 2 ? rlo[2] : rlo[3];
+                        const float hi = m == 0 ? rhi[0] : m == 1 ? rhi[1] : m == 2 ? rhi[2] : rhi[3];
+                        if (lo <= hi)
+                            s_jobs[atomicAdd(&s_njobs, 1u)] = make_uint4((uint32_t)xp | ((uint32_t)(yp + m) << 15) | ((uint32_t)JOB_ROW << 30), __float_as_uint(lo), __float_as_uint(hi), 0u);
+                    } else if (clo <= chi) {                          // columns: every lane queues its own
+                        s_jobs[atomicAdd(&s_njobs, 1u)] = make_uint4((uint32_t)x | ((uint32_t)yp << 15) | ((uint32_t)JOB_COLUMN << 30), __float_as_uint(clo), __float_as_uint(chi), 0u);
                     }
                 } else {
 #pragma unroll
                     for (int m = 0; m < 4; ++m)
-                        if (zpx[m] > 0.0f) {
-                            const uint32_t j = atomicAdd(&s_njobs, 1u);
-                            s_jobs[j] = make_uint4((uint32_t)x | ((uint32_t)(yp + m) << 15), __float_as_uint(zpx[m]), __float_as_uint(zpx[m]), 0u);
-                        }
+                        if (zpx[m] > 0.0f)
+                            s_jobs[atomicAdd(&s_njobs, 1u)] = make_uint4((uint32_t)x | ((uint32_t)(yp + m) << 15) | ((uint32_t)JOB_PIXEL << 30), __float_as_uint(zpx[m]), __float_as_uint(zpx[m]), 0u);
                 }
             }
         }
@@ -218,9 +252,10 @@ __global__ void __launch_bounds__(256) k_prepass(const __grid_constant__ Params 
     __syncthreads();
     {   // append this CTA's jobs to the frame's queue (one reservation per CTA)
         const uint32_t njobs = s_njobs;
-        if (t == 0) s_base = njobs ? atomicAdd(&p.ctrl[CTRL_NJOBS], njobs) : 0u;
+        if (t == 0) s_base = njobs ? atomicAdd(&p.ctrl[Q_NJOBS0 + p.parity], njobs) : 0u;
         __syncthreads();
-        for (uint32_t j = (uint32_t)t; j < njobs; j += 256u) p.jobs[s_base + j] = s_jobs[j];
+        for (uint32_t j = (uint32_t)t; j < njobs; j += 256u)
+            if (s_base + j < p.jobs_cap) p.jobs[s_base + j] = s_jobs[j];       // (always true: at most one job per pixel)
     }
     // (b) level-0 block = 8 lanes x 2 threads-rows (tq pair)
 #pragma unroll
@@ -242,49 +277,12 @@ __global__ void __launch_bounds__(256) k_prepass(const __grid_constant__ Params 
         }
         const int bx = blockIdx.x * 2 + qx, by = blockIdx.y * 2 + qy;
         if (bx < p.pyr_w[1] && by < p.pyr_h[1]) p.pyr[p.pyr_off[1] + by * p.pyr_w[1] + bx] = a_mn | (a_mx << 16);
-    } else if (t == 20 && p.pyr_levels > 2) {
+    } else if (t == 20) {
         uint32_t a_mn = 0xffffu, a_mx = 0u;
         for (int a = 0; a < 16; ++a) { a_mn = min(a_mn, s_mn[a]); a_mx = max(a_mx, s_mx[a]); }
-        p.pyr[p.pyr_off[2] + blockIdx.y * p.pyr_w[2] + blockIdx.x] = a_mn | (a_mx << 16);
+        if (p.pyr_levels > 2) p.pyr[p.pyr_off[2] + blockIdx.y * p.pyr_w[2] + blockIdx.x] = a_mn | (a_mx << 16);
+        if (a_mx != 0u) { atomicMin(&p.ctrl[Q_DMIN0 + p.parity], a_mn); atomicMax(&p.ctrl[Q_DMAX0 + p.parity], a_mx); }
     }
-    if (p.pyr_levels <= 3) return;
-    // the last CTA to arrive reduces level 2 into levels 3.. (each level halves both dimensions)
-    __threadfence();
-    __syncthreads();
-    if (t == 0) {
-        const uint32_t n = gridDim.x * gridDim.y;
-        s_last = (atomicAdd(&p.ctrl[CTRL_TICKET], 1u) == n - 1u);
-    }
-    __syncthreads();
-    if (!s_last) return;
-    __threadfence();
-    // small images: levels 4.. are built from a shared-memory copy of the level below (block barriers only); the job
-    // staging buffer is free by now.  Larger images go level by level through global memory.
-    uint32_t *buf = reinterpret_cast<uint32_t *>(s_jobs);
-    const bool in_smem = p.pyr_w[3] * p.pyr_h[3] <= 1024;
-    for (int l = 3; l < p.pyr_levels; ++l) {
-        const int w = p.pyr_w[l], h = p.pyr_h[l], pw = p.pyr_w[l - 1], ph = p.pyr_h[l - 1];
-        const uint32_t *src = p.pyr + p.pyr_off[l - 1];
-        const uint32_t *ssrc = buf + ((l - 1) & 1) * 1024;
-        uint32_t *sdst = buf + (l & 1) * 1024;
-        const bool from_smem = in_smem && l > 3;
-        for (int e = t; e < w * h; e += blockDim.x) {
-            const int ex = e % w, ey = e / w;
-            uint32_t a_mn = 0xffffu, a_mx = 0u;
-            for (int a = 0; a < 2; ++a) for (int b = 0; b < 2; ++b) {
-                const int sx = ex * 2 + b, sy = ey * 2 + a;
-                if (sx < pw && sy < ph) {
-                    const uint32_t v = from_smem ? ssrc[sy * pw + sx] : __ldcg(src + sy * pw + sx);
-                    a_mn = min(a_mn, v & 0xffffu); a_mx = max(a_mx, v >> 16);
-                }
-            }
-            p.pyr[p.pyr_off[l] + e] = a_mn | (a_mx << 16);
-            if (in_smem) sdst[e] = a_mn | (a_mx << 16);
-        }
-        if (!in_smem) __threadfence();
-        __syncthreads();
-    }
-    if (t == 0) p.ctrl[CTRL_TICKET] = 0;
 }
 
 // camera-space centre of geometry tile (ttx, tty, ttz local) -- culling only
@@ -299,130 +297,148 @@ __device__ __forceinline__ void tile_centre(const Params &p, int ttx, int tty, i
     cZ = p.R[6] * wx + p.R[7] * wy + p.R[8] * wz + p.t[2];
 }
 
-// K1 -- one launch, two roles that both depend only on k_prepass and so run side by side:
-//  blocks [0, n_geo_blocks): S9 for geometry, one thread per tile of this shard: conservative test of the tile's
-//      camera-space box against the depth pyramid (any voxel with sdf >= -mu?).  Tiles that pass are refined on their
-//      SUBX x 1 x SUBZ sub-boxes by SUBX * SUBZ threads each (second phase, through shared memory), then appended to the
-//      geometry work list with warp-aggregated atomics.
-//  the other blocks: S1 (c) continued: one group of 4 lanes per queued mark job (grid-stride); the 4 lanes share the
-//      job's cell layers.
-template <int R>
-__global__ void __launch_bounds__(256) k_mark_classify(const __grid_constant__ Params p, int n_geo_blocks)
+// is this geometry tile NEAR: does its box come within 2 mm of the camera plane (or behind it)?  Its voxels may then have
+// Z <= 0 or Z outside the range of the branch-free reciprocal, and the fused kernel takes the plain per-voxel routines.
+// Evaluated identically by the classification and by the consumers of geometry and colour items.
+__device__ __forceinline__ bool tile_is_near(const Params &p, int ttx, int tty, int ttz)
 {
-    __shared__ float s_c[256][3];
-    __shared__ uint16_t s_surv[256];
-    __shared__ uint32_t s_nsurv, s_pass[256];
-    pdl_launch_dependents();
-    pdl_wait();
-    const int t = threadIdx.x;
-    if ((int)blockIdx.x >= n_geo_blocks) {
-        const uint32_t njobs = __ldcg(&p.ctrl[CTRL_NJOBS]);
-        const uint32_t g = ((blockIdx.x - n_geo_blocks) * blockDim.x + t) >> 2, ng = ((gridDim.x - n_geo_blocks) * blockDim.x) >> 2;
-        for (uint32_t j = g; j < njobs; j += ng) {
-            const uint4 job = __ldcg(p.jobs + j);
-            const float xa = (float)(job.x & 0x7fffu), ya = (float)((job.x >> 15) & 0x7fffu), ext = (job.x & 0x80000000u) ? 3.0f : 0.0f;
-            int i0, i1, j0, j1, k0, k1;
-            if (shell_box(p, xa, xa + ext, ya, ya + ext, __uint_as_float(job.y), __uint_as_float(job.z), i0, i1, j0, j1, k0, k1))
-                mark_box<R>(p, i0, i1, j0, j1, k0, k1, t & 3, 4);
-        }
-        return;
-    }
-    const int tile = blockIdx.x * blockDim.x + t;
-    if (t == 0) s_nsurv = 0u;
-    s_pass[t] = 0u;
-    __syncthreads();
-    uint32_t near = 0;
-    int ttx = 0, tty = 0, ttz = 0;
-    bool behind = false;
-    if (tile < p.n_tiles) {
-        ttx = tile % p.tiles_x; tty = (tile / p.tiles_x) % p.tiles_y; ttz = tile / (p.tiles_x * p.tiles_y);
-        float cX, cY, cZ;
-        tile_centre(p, ttx, tty, ttz, cX, cY, cZ);
-        if (!(cZ - p.tile_ez > 2e-3f)) near = ITEM_NEAR;
-        const int coarse = box_may_update(p, cX, cY, cZ, p.tile_ex, p.tile_ey, p.tile_ez);
-        // not wholly (by >= 0.1 mm) in front of every depth it can see; with mu > 1 m even 0.1 mm could quantise to tsdf = 0
-        behind = coarse == 1 || (coarse == 2 && !(p.mu <= 1.0f));
-        if (coarse != 0) {
-            const uint32_t k = atomicAdd(&s_nsurv, 1u);
-            s_surv[k] = (uint16_t)t;
-            s_c[t][0] = cX; s_c[t][1] = cY; s_c[t][2] = cZ;
-        }
-    }
-    __syncthreads();
-    {   // phase 2: thread k tests sub-box (k % 8) of survivor (k / 8)
-        const uint32_t n = s_nsurv * (uint32_t)(SUBX * SUBZ);
-        const float sx = (float)(TX / SUBX) * p.vs, sz = (float)(TZ / SUBZ) * p.vs;
-        for (uint32_t k = (uint32_t)t; k < n; k += 256u) {
-            const int sv = s_surv[k / (SUBX * SUBZ)], sb = (int)(k % (SUBX * SUBZ)), bx = sb % SUBX, bz = sb / SUBX;
-            const float dx = ((float)bx - 0.5f * (float)(SUBX - 1)) * sx, dz = ((float)bz - 0.5f * (float)(SUBZ - 1)) * sz;
-            if (box_may_update(p, s_c[sv][0] + p.R[0] * dx + p.R[2] * dz, s_c[sv][1] + p.R[3] * dx + p.R[5] * dz,
-                               s_c[sv][2] + p.R[6] * dx + p.R[8] * dz, p.sub_ex, p.sub_ey, p.sub_ez) != 0)
-                atomicOr(&s_pass[sv], 1u << bz);          // bit bz: the tile's z-half bz can hold an updated voxel
-        }
-    }
-    __syncthreads();
-    // NEAR tiles take the slow per-voxel routines (several times longer than an ordinary tile): they are listed from the
-    // back of the work list and the fused kernel starts with them, so that none is left for the tail
-    const bool pass = s_pass[t] != 0u, geo = pass && near == 0u, geo_near = pass && near != 0u;
-    // For the ray caster (raycast.cuh): a voxel can only receive tsdf <= 0 in a visited tile that is NOT wholly in front of
-    // every depth it can see (in front by >= 0.1 mm, mu <= 1 m: every new sample is >= 3 q-units, so the running average of
-    // positive values stays >= 1).  Flag those tiles
-    // and their bricks; flags are only ever set (vol_reset clears them, vol_upload sets all): a conservative superset.
-    if (pass && behind) {
-        p.tile_neg[tile] = 1; p.brick_neg[((ttz / 4) * p.bricks_y + tty / 8) * p.bricks_x + ttx] = 1;
-    }
-    const unsigned lane = t & 31, lt = (1u << lane) - 1u;
-    const unsigned mg = __ballot_sync(0xffffffffu, geo), mn = __ballot_sync(0xffffffffu, geo_near);
-    uint32_t bg = 0, bn = 0;
-    if (lane == 0 && mg) bg = atomicAdd(&p.ctrl[CTRL_NGEO], (uint32_t)__popc(mg));
-    if (lane == 0 && mn) bn = atomicAdd(&p.ctrl[CTRL_NNEAR], (uint32_t)__popc(mn));
-    bg = __shfl_sync(0xffffffffu, bg, 0); bn = __shfl_sync(0xffffffffu, bn, 0);
-    if (geo) p.work_geo[bg + __popc(mg & lt)] = item_pack(ttx, tty, ttz, (int)s_pass[t]);   // sub = z-half mask
-    if (geo_near) p.work_geo[(uint32_t)p.n_tiles - 1u - (bn + __popc(mn & lt))] = item_pack(ttx, tty, ttz, 0) | ITEM_NEAR;
+    float cX, cY, cZ;
+    tile_centre(p, ttx, tty, ttz, cX, cY, cZ);
+    return !(cZ - p.tile_ez > 2e-3f);
 }
 
-// K1b -- S9 for colour, one thread per tile: one work item per non-zero NIBBLE of the tile's shell-mark words, i.e. up to
-// 4 colour cells.  (A colour item is several times longer than a geometry tile; with 8 cells per item the longest ones
-// took half of the fused kernel's duration and left a tail.)  Colour items come first in the fused kernel's queue.
-template <int R>
-__global__ void __launch_bounds__(256) k_items_col(const __grid_constant__ Params p)
+// culling only: can any voxel of the camera-space box (centre c, half extents e) pass the TSDF tests (frustum, valid
+// depth, sdf >= -mu)?  Conservative: max valid depth over the box's pixel rectangle against the box's nearest Z.
+// Returns 0 = no, 1 = maybe, 2 = maybe and the whole box lies in front of every valid depth of its rectangle (free space:
+// a finer look at the box would find the same).
+__device__ __forceinline__ int box_may_update(const Params &p, float cX, float cY, float cZ, float eX, float eY, float eZ)
 {
-    constexpr int WPT = words_per_tile(R);
-    pdl_launch_dependents();
-    pdl_wait();
-    const int tile = blockIdx.x * blockDim.x + threadIdx.x;
-    if (tile == 0) p.ctrl[CTRL_NJOBS] = 0u;            // the mark jobs of this frame have been consumed
-    uint32_t nz[WPT];                                   // bit n set: nibble n of the mark word is non-zero
+    int x0, x1, y0, y1; float zmin, zmax;
+    if (!box_rect(p, cX, cY, cZ, eX, eY, eZ, x0, x1, y0, y1, zmin, zmax)) return 0;
+    uint32_t mn, mx;
+    depth_range(p, x0, x1, y0, y1, mn, mx);
+    if (mx == 0u || !(zmin <= ((float)mx * 0.001f + 1e-4f) + p.mu)) return 0;
+    return zmax <= (float)mn * 0.001f - 1e-4f ? 2 : 1;
+}
+
+// The three producer roles of the fused kernel.  Each is one CHUNK of work for one warp; chunks are claimed from counters
+// in ctrl[], so every warp of the grid helps and nobody ever waits for work that has not been claimed.
+
+// S9 for geometry, 32 tiles of this shard, one lane per tile: conservative test of the tile's
+// camera-space box against the depth pyramid (any voxel with sdf >= -mu?).  Tiles that pass are refined on their
+// SUBX x 1 x SUBZ sub-boxes, 8 lanes per tile, and appended to the geometry work list together with the mask of the sub-boxes
+// that passed (warp-aggregated reservation).  The item is published by the store itself: a consumer polls its slot.
+__device__ __forceinline__ void classify_chunk(const Params &p, uint32_t chunk, int lane)
+{
+    // lane l takes tile chunk + l * n_chunks: a sample spread over the whole volume, so that the tiles near the surface
+    // (whose sub-boxes have to be looked at) are dealt evenly to the chunks
+    const int tile = (int)chunk + lane * ((p.n_tiles + CLS_CHUNK - 1) / CLS_CHUNK);
+    int ttx = 0, tty = 0, ttz = 0, coarse = 0;
+    float cX = 0.f, cY = 0.f, cZ = 0.f;
+    bool near = false;
+    if (tile < p.n_tiles) {
+        ttx = tile % p.tiles_x; tty = (tile / p.tiles_x) % p.tiles_y; ttz = tile / (p.tiles_x * p.tiles_y);
+        tile_centre(p, ttx, tty, ttz, cX, cY, cZ);
+        near = !(cZ - p.tile_ez > 2e-3f);
+        coarse = box_may_update(p, cX, cY, cZ, p.tile_ex, p.tile_ey, p.tile_ez);
+    }
+    unsigned surv = __ballot_sync(0xffffffffu, coarse != 0);
+    uint32_t mask = 0u;
+    const float sx = (float)(TX / SUBX) * p.vs, sz = (float)(TZ / SUBZ) * p.vs;
+    const int sb = lane & 7, bx = sb / SUBZ, bz = sb % SUBZ;        // item mask bit = bx * SUBZ + bz
+    const float dx = ((float)bx - 0.5f * (float)(SUBX - 1)) * sx, dz = ((float)bz - 0.5f * (float)(SUBZ - 1)) * sz;
+    while (surv) {                                   // four survivors at a time: lane = (survivor, sub-box)
+        int src[4];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) { src[k] = surv ? __ffs(surv) - 1 : -1; surv &= surv - 1u; }
+        const int mine = src[lane >> 3];
+        const float sX = __shfl_sync(0xffffffffu, cX, mine & 31), sY = __shfl_sync(0xffffffffu, cY, mine & 31), sZ = __shfl_sync(0xffffffffu, cZ, mine & 31);
+        const bool ok = mine >= 0 && box_may_update(p, sX + p.R[0] * dx + p.R[2] * dz, sY + p.R[3] * dx + p.R[5] * dz,
+                                                    sZ + p.R[6] * dx + p.R[8] * dz, p.sub_ex, p.sub_ey, p.sub_ez) != 0;
+        const unsigned b = __ballot_sync(0xffffffffu, ok);
+#pragma unroll
+        for (int k = 0; k < 4; ++k) if (lane == src[k]) mask = (b >> (8 * k)) & 0xffu;
+    }
+    // a partial last slab: sub-boxes whose first layer lies beyond the volume are not queued at all
+    if (local_to_global_tz(p, ttz) * TZ + TZ / SUBZ >= p.nz) mask &= 0x55u;
+    if (near && mask) mask = 0xffu;                  // NEAR tiles are processed whole, by the plain routines
+    // For the ray caster (raycast.cuh): a voxel can only receive tsdf <= 0 in a visited tile that is NOT wholly in front of
+    // every depth it can see (in front by >= 0.1 mm, mu <= 1 m: every new sample is >= 3 q-units, so the running average of
+    // positive values stays >= 1).  Flag those tiles and their bricks; flags are only ever set (vol_reset clears them,
+    // vol_upload sets all): a conservative superset.
+    const bool behind = coarse == 1 || (coarse == 2 && !(p.mu <= 1.0f));
+    if (mask && behind) {
+        p.tile_neg[tile] = 1; p.brick_neg[((ttz / 4) * p.bricks_y + tty / 8) * p.bricks_x + ttx] = 1;
+    }
+    const unsigned mg = __ballot_sync(0xffffffffu, mask != 0u), lt = (1u << lane) - 1u;
+    uint32_t bg = 0;
+    if (lane == 0 && mg) bg = atomicAdd(&p.ctrl[ST_NGEO], (uint32_t)__popc(mg));
+    bg = __shfl_sync(0xffffffffu, bg, 0);
+    if (mask) __stcg(p.work_geo + bg + __popc(mg & lt), item_pack(ttx, tty, ttz, (int)mask));
+}
+
+// S1 (c) continued: mark jobs [8 chunk, 8 chunk + 8), 4 lanes per job; the 4 lanes share the job's cell layers.
+template <int R>
+__device__ __forceinline__ void mark_chunk(const Params &p, uint32_t chunk, uint32_t njobs, int lane)
+{
+    const uint32_t j = chunk * MARK_CHUNK + ((uint32_t)lane >> 2);
+    if (j >= njobs) return;
+    const uint4 job = __ldcg(p.jobs + j);
+    const float xa = (float)(job.x & 0x7fffu), ya = (float)((job.x >> 15) & 0x7fffu);
+    const uint32_t shape = job.x >> 30;
+    const float ex = shape == JOB_PATCH || shape == JOB_ROW ? 3.0f : 0.0f, ey = shape == JOB_PATCH || shape == JOB_COLUMN ? 3.0f : 0.0f;
+    int i0, i1, j0, j1, k0, k1;
+    if (shell_box(p, xa, xa + ex, ya, ya + ey, __uint_as_float(job.y), __uint_as_float(job.z), i0, i1, j0, j1, k0, k1))
+        mark_box<R>(p, i0, i1, j0, j1, k0, k1, lane & 3, 4);
+}
+
+// S9 for colour, tiles [128 chunk, 128 chunk + 128), four consecutive tiles per lane, once every mark has been set: one work
+// item per non-zero NIBBLE of a tile's shell-mark words, i.e. up to 4 colour cells; the item carries the nibble's bits, and the
+// mark words are cleared here.  (A colour item is several times longer
+// than a geometry sub-box; with 8 cells per item the longest ones left a tail.)
+template <int R>
+__device__ __forceinline__ void scan_chunk(const Params &p, uint32_t chunk, int lane)
+{
+    constexpr int WPT = words_per_tile(R), TPL = SCAN_CHUNK / 32;
+    const int tile0 = (int)chunk * SCAN_CHUNK + lane * TPL;
+    uint32_t nz[TPL][WPT], mk[TPL][WPT];                // the mark words; bit n of nz set: nibble n of the word is non-zero
     int ncol = 0;
 #pragma unroll
-    for (int w = 0; w < WPT; ++w) {
-        nz[w] = 0u;
-        if (tile < p.n_tiles) {
-            const uint32_t m = __ldcg(p.marks + (size_t)tile * WPT + w);
+    for (int k = 0; k < TPL; ++k)
 #pragma unroll
-            for (int n = 0; n < 8; ++n) nz[w] |= (((m >> (4 * n)) & 0xfu) != 0u ? 1u : 0u) << n;
+        for (int w = 0; w < WPT; ++w) {
+            nz[k][w] = 0u; mk[k][w] = 0u;
+            if (tile0 + k < p.n_tiles) {
+                uint32_t m = __ldcg(p.marks + (size_t)(tile0 + k) * WPT + w);
+                mk[k][w] = m;
+                if (m) p.marks[(size_t)(tile0 + k) * WPT + w] = 0u;      // consumed: the marks are all zero again for the next frame
+                m |= m >> 1; m |= m >> 2; m &= 0x11111111u;          // bit 4n set: nibble n is non-zero
+                m = (m | (m >> 3)) & 0x03030303u; m = (m | (m >> 6)) & 0x000f000fu; nz[k][w] = (m | (m >> 12)) & 0xffu;
+            }
+            ncol += __popc(nz[k][w]);
         }
-        ncol += __popc(nz[w]);
-    }
-    const unsigned lane = threadIdx.x & 31;
     int pre = ncol;
 #pragma unroll
-    for (int o = 1; o < 32; o <<= 1) { const int v = __shfl_up_sync(0xffffffffu, pre, o); if ((int)lane >= o) pre += v; }
+    for (int o = 1; o < 32; o <<= 1) { const int v = __shfl_up_sync(0xffffffffu, pre, o); if (lane >= o) pre += v; }
     const int tot = __shfl_sync(0xffffffffu, pre, 31);
     if (tot == 0) return;
     uint32_t bc = 0;
-    if (lane == 0) bc = atomicAdd(&p.ctrl[CTRL_NCOL], (uint32_t)tot);
+    if (lane == 0) bc = atomicAdd(&p.ctrl[ST_NCOL], (uint32_t)tot);
     bc = __shfl_sync(0xffffffffu, bc, 0);
     if (ncol) {
-        const int ttx = tile % p.tiles_x, tty = (tile / p.tiles_x) % p.tiles_y, ttz = tile / (p.tiles_x * p.tiles_y);
-        float cX, cY, cZ;
-        tile_centre(p, ttx, tty, ttz, cX, cY, cZ);
-        const uint32_t near = !(cZ - p.tile_ez > 2e-3f) ? ITEM_NEAR : 0u;
         uint32_t pos = bc + (uint32_t)(pre - ncol);
 #pragma unroll
-        for (int w = 0; w < WPT; ++w) {
-            uint32_t m = nz[w];
-            while (m) { const int n = __ffs(m) - 1; m &= m - 1u; p.work_col[pos++] = item_pack(ttx, tty, ttz, 8 * w + n) | near; }
+        for (int k = 0; k < TPL; ++k) {
+            const int tile = tile0 + k;
+            const int ttx = tile % p.tiles_x, tty = (tile / p.tiles_x) % p.tiles_y, ttz = tile / (p.tiles_x * p.tiles_y);
+#pragma unroll
+            for (int w = 0; w < WPT; ++w) {
+                uint32_t m = nz[k][w];
+                while (m) {
+                    const int n = __ffs(m) - 1; m &= m - 1u;
+                    p.work_col[pos++] = make_uint2(item_pack(ttx, tty, ttz, 8 * w + n), mk[k][w] & (0xfu << (4 * n)));
+                }
+            }
         }
     }
 }

@@ -48,6 +48,7 @@ struct vol {
     // fused-kernel launch shape
     int n_sms, fused_blocks;
     bool counting, profiling;
+    unsigned frame_seq;             // frames enqueued so far: its parity selects the job counter (Params::parity)
     cudaEvent_t ev[4];
     bool ev_valid;
     // vol_integrate_host: the frames are copied on a stream of the library's own
@@ -147,7 +148,7 @@ extern "C" int vol_create(vol_t **out, const int32_t dims_geo[3], int32_t r, con
                           float trunc_mu_m, int32_t w_max, const vol_opts_t *opts)
 {
     if (!out || !dims_geo || !origin_m) return VOL_E_ARG;
-    if (dims_geo[0] <= 0 || dims_geo[1] <= 0 || dims_geo[2] <= 0 || dims_geo[0] % 4 != 0) return VOL_E_ARG;
+    if (dims_geo[0] <= 0 || dims_geo[1] <= 0 || dims_geo[2] <= 0) return VOL_E_ARG;
     if (r < 1 || r > 4 || !(extent_m > 0.0f) || !(trunc_mu_m > 0.0f) || w_max < 1 || w_max > 512) return VOL_E_ARG;
     if (!(extent_m <= 1e6f) || !(trunc_mu_m <= 1e6f)) return VOL_E_ARG;           // also rejects NaN / inf
     for (int i = 0; i < 3; ++i) if (!(std::fabs(origin_m[i]) <= 1e6f)) return VOL_E_ARG;
@@ -211,25 +212,28 @@ extern "C" int vol_create(vol_t **out, const int32_t dims_geo[3], int32_t r, con
         if (cudaMalloc(&p.col, v->col_bytes) != cudaSuccess) { cudaGetLastError(); snprintf(g_err, sizeof g_err, "cudaMalloc(%zu) colour volume failed", v->col_bytes); return fail(VOL_E_OOM); }
         v->own_col = true;
     }
-    if (((uintptr_t)p.geo | (uintptr_t)p.col) & 15u) return fail(VOL_E_ARG);       // 16-byte vector access
+    if (((uintptr_t)p.geo | (uintptr_t)p.col) & 15u) return fail(VOL_E_ARG);       // whole sectors per warp access
     if (v->geo_bytes && cudaMemset(p.geo, 0, v->geo_bytes) != cudaSuccess) rc = VOL_E_CUDA;
     if (v->col_bytes && cudaMemset(p.col, 0, v->col_bytes) != cudaSuccess) rc = VOL_E_CUDA;
     const size_t nt = (size_t)(p.n_tiles > 0 ? p.n_tiles : 1), nw = nt * (size_t)vf::words_per_tile(r);
     if (cudaMalloc(&p.work_geo, sizeof(uint32_t) * nt) != cudaSuccess) rc = VOL_E_OOM;
-    if (cudaMalloc(&p.work_col, sizeof(uint32_t) * nw * 8) != cudaSuccess) rc = VOL_E_OOM;
+    if (rc == VOL_OK && cudaMemset(p.work_geo, 0, sizeof(uint32_t) * nt) != cudaSuccess) rc = VOL_E_CUDA;   // empty slots are zero
+    if (cudaMalloc(&p.work_col, sizeof(uint2) * nw * 8) != cudaSuccess) rc = VOL_E_OOM;
     if (cudaMalloc(&p.marks, sizeof(uint32_t) * nw) != cudaSuccess) rc = VOL_E_OOM;
+    if (rc == VOL_OK && cudaMemset(p.marks, 0, sizeof(uint32_t) * nw) != cudaSuccess) rc = VOL_E_CUDA;
     if (cudaMalloc(&p.tile_neg, nt) != cudaSuccess) rc = VOL_E_OOM;
     if (rc == VOL_OK && cudaMemset(p.tile_neg, 0, nt) != cudaSuccess) rc = VOL_E_CUDA;
     p.bricks_x = p.tiles_x; p.bricks_y = (p.tiles_y + 7) / 8; p.bricks_z = (my_slabs + 3) / 4;
     const size_t nb = (size_t)p.bricks_x * p.bricks_y * p.bricks_z + 1;
     if (cudaMalloc(&p.brick_neg, nb) != cudaSuccess) rc = VOL_E_OOM;
     if (rc == VOL_OK && cudaMemset(p.brick_neg, 0, nb) != cudaSuccess) rc = VOL_E_CUDA;
-    if (rc == VOL_OK && cudaMemset(p.marks, 0, sizeof(uint32_t) * nw) != cudaSuccess) rc = VOL_E_CUDA;
-    // one 64-byte record: the 8 control words, then the 4 voxel counters (read back together by vol_frame_stats*)
-    static_assert(sizeof(uint32_t) * vf::CTRL_N == 32, "raw statistics record: 8 control words, then 4 counters");
-    if (cudaMalloc(&p.ctrl, 64) != cudaSuccess) rc = VOL_E_OOM;
-    if (rc == VOL_OK) p.counters = reinterpret_cast<unsigned long long *>(p.ctrl + vf::CTRL_N);
-    if (rc == VOL_OK && cudaMemset(p.ctrl, 0, 64) != cudaSuccess) rc = VOL_E_CUDA;
+    // one 128-byte statistics record (8 words, then 12 counters: read back together by vol_frame_stats*), then the queue control words
+    static_assert(sizeof(uint32_t) * vf::ST_N + sizeof(unsigned long long) * vf::CNT_N == VOL_STATS_RAW_BYTES && vf::CTRL_Q0 * 4 == VOL_STATS_RAW_BYTES,
+                  "raw statistics record: 8 words, then 12 counters");
+    if (cudaMalloc(&p.ctrl, sizeof(uint32_t) * vf::CTRL_N) != cudaSuccess) rc = VOL_E_OOM;
+    if (rc == VOL_OK) p.counters = reinterpret_cast<unsigned long long *>(p.ctrl + vf::ST_N);
+    if (rc == VOL_OK && cudaMemset(p.ctrl, 0, sizeof(uint32_t) * vf::CTRL_N) != cudaSuccess) rc = VOL_E_CUDA;
+    if (rc == VOL_OK && cudaMemset(p.ctrl + vf::Q_DMIN0, 0xff, sizeof(uint32_t) * 2) != cudaSuccess) rc = VOL_E_CUDA;   // "no valid depth yet"
     if (rc != VOL_OK) { cudaGetLastError(); return fail(rc); }
 
     cudaDeviceProp prop;
@@ -263,12 +267,13 @@ extern "C" void vol_destroy(vol_t *v)
     if (v->p.work_geo) cudaFree(v->p.work_geo);
     if (v->p.work_col) cudaFree(v->p.work_col);
     if (v->p.marks) cudaFree(v->p.marks);
+    if (v->p.jobs) cudaFree(v->p.jobs);
     if (v->p.tile_neg) cudaFree(v->p.tile_neg);
     if (v->p.brick_neg) cudaFree(v->p.brick_neg);
     if (v->p.ctrl) cudaFree(v->p.ctrl);
     if (v->p.pixmap) cudaFree(v->p.pixmap);
     if (v->p.pyr) cudaFree(v->p.pyr);
-    if (v->p.jobs) cudaFree(v->p.jobs);
+    if (v->p.depthf) cudaFree(v->p.depthf);
     for (int i = 0; i < N_STAGE; ++i) {
         if (v->stage_depth[i]) cudaFree(v->stage_depth[i]);
         if (v->stage_rgb[i]) cudaFree(v->stage_rgb[i]);
@@ -290,18 +295,19 @@ static int ensure_scratch(vol *v, int wd, int hd)
     v->scratch_wd = v->scratch_hd = 0;                       // nothing is valid until every allocation below has succeeded
     if (p.pixmap) { CK(cudaDeviceSynchronize()); cudaFree(p.pixmap); p.pixmap = nullptr; }
     if (p.pyr) { cudaFree(p.pyr); p.pyr = nullptr; }
+    if (p.depthf) { cudaFree(p.depthf); p.depthf = nullptr; }
     if (p.jobs) { cudaFree(p.jobs); p.jobs = nullptr; }
-    CK(cudaMalloc(&p.jobs, sizeof(uint4) * (size_t)((wd + 3) / 4 * 4) * (size_t)((hd + 3) / 4 * 4)));
+    CK(cudaMalloc(&p.depthf, sizeof(float) * (size_t)wd * hd));
+    p.jobs_cap = (uint32_t)((size_t)((wd + 3) / 4 * 4) * (size_t)((hd + 3) / 4 * 4));     // one per pixel at most
+    CK(cudaMalloc(&p.jobs, sizeof(uint4) * (size_t)p.jobs_cap));
     CK(cudaMalloc(&p.pixmap, sizeof(float4) * (size_t)wd * hd));
     int l = 0; size_t off = 0;
-    for (;; ++l) {
-        if (l >= 12) return VOL_E_ARG;                       // image larger than 16384 x 16384
+    for (; l < 3; ++l) {                                     // blocks of 8, 16, 32 pixels
         const int bs = 8 << l;
         p.pyr_w[l] = (wd + bs - 1) / bs; p.pyr_h[l] = (hd + bs - 1) / bs; p.pyr_off[l] = (int)off;
         off += (size_t)p.pyr_w[l] * p.pyr_h[l];
-        if (p.pyr_w[l] == 1 && p.pyr_h[l] == 1) break;
     }
-    p.pyr_levels = l + 1;
+    p.pyr_levels = 3;
     v->pyr_entries = off;
     CK(cudaMalloc(&p.pyr, sizeof(uint32_t) * off));
     v->scratch_wd = wd; v->scratch_hd = hd;
@@ -336,29 +342,28 @@ static int integrate_impl(vol_t *v, const uint16_t *depth_u16_dev, int32_t wd, i
     p.slack = (float)slack;
     box_extents(p.R, 0.5 * vf::TX * p.vs, 0.5 * vf::TY * p.vs, 0.5 * vf::TZ * p.vs, slack, p.tile_ex, p.tile_ey, p.tile_ez);
     box_extents(p.R, 0.5 * (vf::TX / vf::SUBX) * p.vs, 0.5 * vf::TY * p.vs, 0.5 * (vf::TZ / vf::SUBZ) * p.vs, slack, p.sub_ex, p.sub_ey, p.sub_ez);
+    p.parity = (int)(v->frame_seq & 1u);
     p.sigma_g = (float)((double)p.sigma * 1.0001 + slack);
     camera_to_world(p.R, p.t, p.Rw, p.tw);
     if (p.n_tiles == 0) return VOL_OK;
 
     cudaStream_t s = (cudaStream_t)stream;
     if (rgb_ready && !split) { CK(cudaStreamWaitEvent(s, rgb_ready, 0)); rgb_ready = nullptr; }
-    if (v->counting) CK(cudaMemsetAsync(p.counters, 0, sizeof(unsigned long long) * 4, s));
+    if (v->counting) CK(cudaMemsetAsync(p.counters, 0, sizeof(unsigned long long) * vf::CNT_N, s));
     if (v->profiling) CK(cudaEventRecord(v->ev[0], s));
     const dim3 g0((wd + 31) / 32, (hd + 31) / 32);
-    const int g1 = (p.n_tiles + 255) / 256, g2 = v->fused_blocks, gm = v->n_sms * 4;
+    const int g2 = v->fused_blocks;
     const bool cnt = v->counting;
-    // k_mark_classify, k_items_col and k_fused are launched with programmatic stream serialization: their CTAs may be scheduled
-    // while the predecessor drains (it signals griddepcontrol.launch_dependents), and they wait for its completion and
-    // memory flush with griddepcontrol.wait before touching anything it wrote.
+    // k_fused is launched with programmatic stream serialization: its CTAs may be scheduled while the pre-pass drains (it
+    // signals griddepcontrol.launch_dependents), and they wait for its completion and memory flush with griddepcontrol.wait
+    // before touching anything it wrote.
 #define VF_LAUNCH(RR)                                                                   \
     do {                                                                                \
         const FusedFn kf = fused_kernel<RR>(cnt, p.variant);                            \
         CK(launch(vf::k_prepass<RR>, g0, 256, s, false, p));                            \
-        CK(launch(vf::k_mark_classify<RR>, dim3(g1 + gm), 256, s, true, p, g1));        \
-        if (v->profiling) CK(cudaEventRecord(v->ev[1], s));                             \
-        CK(launch(vf::k_items_col<RR>, dim3(g1), 256, s, true, p));                     \
-        if (v->profiling) CK(cudaEventRecord(v->ev[2], s));                             \
-        if (rgb_ready) {   /* geometry half now, colour half once the HD frame has arrived */           \
+        ++v->frame_seq;                                                                 \
+        if (v->profiling) { CK(cudaEventRecord(v->ev[1], s)); CK(cudaEventRecord(v->ev[2], s)); } \
+        if (rgb_ready) {   /* everything but the colour items now, those once the HD frame has arrived */ \
             CK(launch(kf, dim3(g2), vf::CTA, s, true, p, (int)vf::PHASE_GEO));          \
             CK(cudaStreamWaitEvent(s, rgb_ready, 0));                                    \
             CK(launch(kf, dim3(g2), vf::CTA, s, false, p, (int)vf::PHASE_COL));         \
@@ -592,35 +597,42 @@ extern "C" int vol_shard_layers(int32_t nz, int32_t rank, int32_t world, int32_t
 
 extern "C" int vol_set_counting(vol_t *v, int32_t on) { if (!v) return VOL_E_ARG; v->counting = on != 0; return VOL_OK; }
 extern "C" int vol_set_profiling(vol_t *v, int32_t on) { if (!v) return VOL_E_ARG; v->profiling = on != 0; v->ev_valid = false; return VOL_OK; }
-extern "C" int vol_launches_per_frame(const vol_t *v) { return v ? 4 : VOL_E_ARG; }
+extern "C" int vol_launches_per_frame(const vol_t *v) { return v ? 2 : VOL_E_ARG; }
 
 extern "C" int vol_frame_stats_async(vol_t *v, void *raw_host, void *stream)
 {
     if (!v || !raw_host) return VOL_E_ARG;
     int rc = set_device(v); if (rc) return rc;
     cudaStream_t s = (cudaStream_t)stream;
-    CK(cudaMemcpyAsync(raw_host, v->p.ctrl, 64, cudaMemcpyDeviceToHost, s));
+    CK(cudaMemcpyAsync(raw_host, v->p.ctrl, VOL_STATS_RAW_BYTES, cudaMemcpyDeviceToHost, s));
     return VOL_OK;
 }
 
 extern "C" int vol_stats_decode(const vol_t *v, const void *raw_host, vol_stats_t *out)
 {
     if (!v || !raw_host || !out) return VOL_E_ARG;
-    uint32_t ctrl[vf::CTRL_N]; unsigned long long cnt[4];
-    memcpy(ctrl, raw_host, 32); memcpy(cnt, (const char *)raw_host + 32, 32);
+    uint32_t st[vf::ST_N]; unsigned long long cnt[vf::CNT_N];
+    memcpy(st, raw_host, sizeof st); memcpy(cnt, (const char *)raw_host + sizeof st, sizeof cnt);
     memset(out, 0, sizeof *out);
-    if (v->counting) { out->geo_read = cnt[0]; out->geo_changed = cnt[1]; out->col_read = cnt[2]; out->col_changed = cnt[3]; }
+    if (v->counting) {
+        out->geo_read = cnt[vf::CNT_GEO_READ]; out->geo_changed = cnt[vf::CNT_GEO_CHANGED];
+        out->col_read = cnt[vf::CNT_COL_READ]; out->col_changed = cnt[vf::CNT_COL_CHANGED];
+        out->geo_sectors_read = cnt[vf::CNT_GEO_SEC_READ]; out->geo_sectors_written = cnt[vf::CNT_GEO_SEC_WRITTEN];
+        out->col_sectors_read = cnt[vf::CNT_COL_SEC_READ]; out->col_sectors_written = cnt[vf::CNT_COL_SEC_WRITTEN];
+        out->geo_visited = cnt[vf::CNT_GEO_VISITED]; out->col_gated = cnt[vf::CNT_COL_GATED];
+        out->cells_col = st[vf::ST_CELLS]; out->subs_geo = st[vf::ST_SUBS];
+    }
     out->tiles_total = (uint32_t)v->p.n_tiles;
-    out->tiles_geo = ctrl[vf::CTRL_NGEO] + ctrl[vf::CTRL_NNEAR];
-    out->items_col = ctrl[vf::CTRL_NCOL];
-    out->cells_col = v->counting ? ctrl[vf::CTRL_CELLS] : 0u;
+    out->tiles_geo = st[vf::ST_NGEO];
+    out->items_col = st[vf::ST_NCOL];
+    out->jobs_mark = st[vf::ST_NJOBS];
     return VOL_OK;
 }
 
 extern "C" int vol_frame_stats(vol_t *v, vol_stats_t *out, void *stream)
 {
     if (!v || !out) return VOL_E_ARG;
-    unsigned long long raw[8];
+    unsigned long long raw[VOL_STATS_RAW_BYTES / 8];
     int rc = vol_frame_stats_async(v, raw, stream); if (rc) return rc;
     CK(cudaStreamSynchronize((cudaStream_t)stream));
     return vol_stats_decode(v, raw, out);
@@ -667,23 +679,62 @@ __global__ void k_selftest_div(unsigned long long *bad, uint32_t stride)
     if (n) atomicAdd(bad, n);
 }
 
-extern "C" int vol_selftest(uint64_t mismatches[2], int32_t exhaustive)
+// the colour quotient of eq. 9 and its rounding, as issued by the fast path of colour_update_staged, against the plain
+// expression: every stored weight wq, colour C and HD byte h with a sweep of new-sample weights 255 W >= 2^-20
+__global__ void k_selftest_colour(unsigned long long *bad, uint32_t stride)
+{
+    unsigned long long n = 0;
+    const uint32_t lo = __float_as_uint(0x1p-20f), hi = __float_as_uint(255.0f);
+    for (uint64_t b = (uint64_t)lo + ((uint64_t)blockIdx.x * blockDim.x + threadIdx.x) * stride; b <= hi; b += (uint64_t)gridDim.x * blockDim.x * stride) {
+        const float W255 = __uint_as_float((uint32_t)b);
+        for (uint32_t wq = 0; wq < 256u; wq += 1u + (uint32_t)(b % 3u)) {
+            const float wqf = (float)wq, den = __fadd_rn(wqf, W255), rden = vf::div_prepare(den);
+            for (uint32_t k = 0; k < 16u; ++k) {
+                const uint32_t C = (uint32_t)((b >> 3) + 37u * k + wq) & 0xffu, h = (uint32_t)((b >> 7) + 101u * k) & 0xffu;
+                const float num = __fmaf_rn(W255, (float)h, (float)(C * wq));
+                const uint32_t fast = min(__float_as_uint(__fadd_rn(vf::div_with(num, den, rden), 12582912.0f)) & 0x1ffu, 255u);
+                const float cn = rintf(__fdiv_rn(num, den));
+                const uint32_t ref = (uint32_t)(cn < 0.0f ? 0 : (cn > 255.0f ? 255 : (int)cn));
+                n += fast != ref;
+            }
+            const float W = __fdiv_rn(W255, 255.0f) > 1.0f ? 1.0f : __fdiv_rn(W255, 255.0f);
+            const float wnf = __fmaf_rn(W, (float)(255u - wq), wqf);
+            n += min(__float_as_uint(__fadd_rn(wnf, 12582912.0f)) & 0x3ffu, 255u) != (uint32_t)min(__float2int_rn(wnf), 255);
+            const float wna = __fadd_rn(wqf, W255);
+            n += min(__float_as_uint(__fadd_rn(wna, 12582912.0f)) & 0x3ffu, 255u) != (uint32_t)min(__float2int_rn(wna), 255);
+        }
+    }
+    if (n) atomicAdd(bad, n);
+}
+
+extern "C" int vol_selftest(uint64_t mismatches[3], int32_t exhaustive)
 {
     if (!mismatches) return VOL_E_ARG;
     unsigned long long *d = nullptr;
-    CK(cudaMalloc(&d, 2 * sizeof(unsigned long long)));
+    CK(cudaMalloc(&d, 3 * sizeof(unsigned long long)));
     int rc = VOL_OK;
-    if (cudaMemset(d, 0, 2 * sizeof(unsigned long long)) != cudaSuccess) rc = VOL_E_CUDA;
+    if (cudaMemset(d, 0, 3 * sizeof(unsigned long long)) != cudaSuccess) rc = VOL_E_CUDA;
     if (rc == VOL_OK) {
         k_selftest_rcp<<<148 * 8, 256>>>(d);
         k_selftest_div<<<148 * 8, 256>>>(d + 1, exhaustive ? 1u : 257u);
-        unsigned long long h[2];
+        k_selftest_colour<<<148 * 8, 256>>>(d + 2, exhaustive ? 1u : 1021u);
+        unsigned long long h[3];
         if (cudaMemcpy(h, d, sizeof h, cudaMemcpyDeviceToHost) != cudaSuccess) rc = VOL_E_CUDA;
-        else { mismatches[0] = h[0]; mismatches[1] = h[1]; }
+        else { mismatches[0] = h[0]; mismatches[1] = h[1]; mismatches[2] = h[2]; }
     }
     if (rc != VOL_OK) snprintf(g_err, sizeof g_err, "vol_selftest: %s", cudaGetErrorString(cudaGetLastError()));
     cudaFree(d);
     return rc;
 }
+
+#ifdef VF_TRACE
+// development aid: copy the per-warp trace of the last k_fused launch (8192 x 16 words) to the host
+extern "C" int vol_trace_dump(unsigned long long *host)
+{
+    CK(cudaDeviceSynchronize());
+    CK(cudaMemcpyFromSymbol(host, vf::g_trace, sizeof(unsigned long long) * 8192 * 16));
+    return VOL_OK;
+}
+#endif
 
 #include "frontend_host.cuh"

@@ -46,7 +46,7 @@ def test_argument_validation_precedes_any_cuda_call():
     L = vf.lib()
     h = ctypes.c_void_p()
     org = (ctypes.c_float * 3)(0, 0, 0)
-    bad = [((0, 8, 8), 2, 1.0, 0.1, 128), ((10, 8, 8), 2, 1.0, 0.1, 128), ((8, 8, 8), 0, 1.0, 0.1, 128),
+    bad = [((0, 8, 8), 2, 1.0, 0.1, 128), ((8, -3, 8), 2, 1.0, 0.1, 128), ((8, 8, 8), 0, 1.0, 0.1, 128),
            ((8, 8, 8), 5, 1.0, 0.1, 128), ((8, 8, 8), 2, -1.0, 0.1, 128), ((8, 8, 8), 2, 1.0, 0.0, 128),
            ((8, 8, 8), 2, 1.0, 0.1, 0), ((8, 8, 8), 2, 1.0, 0.1, 513)]
     for dims, r, ext, mu, wmax in bad:

@@ -129,7 +129,7 @@ def test_host_frames_enqueued_back_to_back():
         check_counters(st, cnt)
     compare_states(g, o, "one frame at a time")
     stream = torch.cuda.Stream()
-    raw = torch.zeros((len(frames), 8), dtype=torch.int64).pin_memory()
+    raw = torch.zeros((len(frames), 16), dtype=torch.int64).pin_memory()
     for rep in range(3):                                            # three times: whichever way the copies and kernels interleave
         g.reset(stream)
         for n, (d, rgb, T) in enumerate(pinned):
@@ -187,10 +187,11 @@ def test_bad_arguments_leave_state_untouched():
 
 def test_exact_arithmetic_selftest():
     """The branch-free reciprocal / quotient of the hot path equal __frcp_rn / __fdiv_rn bit for bit: every binary32
-    in the reciprocal's operand range, and a 1/257 stride of the TSDF quotient's numerators x all 513 denominators
-    (the exhaustive sweep is `vf.selftest(exhaustive=True)`, ~1e12 quotients)."""
+    in the reciprocal's operand range, a 1/257 stride of the TSDF quotient's numerators x all 513 denominators, and a
+    1/1021 stride of the colour quotient's new-sample weights x stored weights x colour / HD byte pairs, with both weight
+    roundings (the exhaustive sweep is `vf.selftest(exhaustive=True)`, ~1e12 quotients)."""
     import paper_1602_06645_b200 as vf
-    assert vf.selftest(False) == (0, 0)
+    assert vf.selftest(False) == (0, 0, 0)
 
 
 def test_cfg3_full_size_whole_sequence_sampled():
