@@ -100,7 +100,10 @@ typedef struct {
     uint64_t geo_sectors_read, geo_sectors_written, col_sectors_read, col_sectors_written;
     uint64_t geo_visited;   /* geometry voxels the kernel projected (the read ones are a subset) */
     uint64_t col_gated;     /* colour voxels that went through the sigma gate (S4-S5; the read ones are a subset) */
-    uint64_t reserved64;
+    uint64_t geo_skippable; /* of geo_read: voxels of sub-boxes that hold nothing but saturated free space (tsdf_q = 32767,
+                               w = w_max) and stay in free space this frame -- read and unchanged by definition; the plain
+                               (non-counting) kernel leaves those sub-boxes out, so it touches geo_read - geo_skippable */
+    uint64_t geo_sectors_skippable;  /* the same in 32-byte sectors (of geo_sectors_read) */
     uint32_t subs_geo;      /* geometry sub-boxes (8x4x4 voxels) visited */
     uint32_t jobs_mark;     /* shell-mark jobs (one or two per 4 x 4 pixel patch with colour-eligible pixels) */
 } vol_stats_t;

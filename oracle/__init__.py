@@ -58,6 +58,10 @@ def _load():
         P = ctypes.c_void_p
         lib.ref_integrate.restype = ctypes.c_int
         lib.ref_integrate.argtypes = [P, P, P, P, P]
+        lib.ref_integrate_sectors.restype = ctypes.c_int
+        lib.ref_integrate_sectors.argtypes = [P, P, P, P, P, P, P, P, P]
+        lib.ref_threads.restype = ctypes.c_int
+        lib.ref_threads.argtypes = []
         lib.ref_integrate_subset.restype = ctypes.c_int
         lib.ref_integrate_subset.argtypes = [P, P, P, ctypes.c_int64, P, P, ctypes.c_int64, P]
         lib.ref_frame_constants.restype = ctypes.c_int
@@ -119,6 +123,20 @@ class RefVolume:
         self.counters.append(cnt)
         return cnt
 
+    def integrate_sectors(self, depth, rgb, T_world_depth, K_depth, K_rgb, T_depth_rgb):
+        """integrate() that also counts the distinct 32-byte sectors (8 consecutive words) holding a read / changed voxel:
+        returns [geo_read, geo_changed, col_read, col_changed, geo_sectors_read, geo_sectors_written, col_sectors_read,
+        col_sectors_written]."""
+        fr, keep = self._frame(depth, rgb, T_world_depth, K_depth, K_rgb, T_depth_rgb)
+        cnt = np.zeros(4, dtype=np.uint64)
+        maps = [np.zeros((a.size + 7) // 8, np.uint8) for a in (self.geo, self.geo, self.col, self.col)]
+        rc = _load().ref_integrate_sectors(ctypes.addressof(self.desc), ctypes.addressof(fr), self.geo.ctypes.data, self.col.ctypes.data,
+                                           cnt.ctypes.data, *[m.ctypes.data for m in maps])
+        if rc != 0:
+            raise ValueError("ref_integrate_sectors: bad arguments")
+        self.counters.append(cnt)
+        return np.concatenate([cnt, np.array([int(m.sum(dtype=np.uint64)) for m in maps], np.uint64)])
+
     def integrate_subset(self, geo_idx, geo_words, col_idx, col_words, depth, rgb, T_world_depth, K_depth, K_rgb,
                          T_depth_rgb):
         """One frame applied only to the listed voxels (linear indices; words updated in place)."""
@@ -170,6 +188,11 @@ class RefVolume:
 
 
 # unpack helpers (layout only; used by tests on either side's downloaded state)
+def threads() -> int:
+    """OpenMP threads the oracle's loops use (omp_get_max_threads)."""
+    return int(_load().ref_threads())
+
+
 def geo_q(words):
     return (words & np.uint32(0xffff)).astype(np.uint16).view(np.int16).astype(np.int32)
 

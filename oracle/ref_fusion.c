@@ -29,6 +29,9 @@
  * Build: gcc -O2 -fopenmp -ffp-contract=off -mfma -shared -fPIC ref_fusion.c -lm
  */
 #include <math.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
 #include <stdint.h>
 #include <stddef.h>
 #include <string.h>
@@ -234,8 +237,12 @@ static int update_col_voxel(const ref_vol_t *v, const ref_frame_t *f, const cons
 /* ref_integrate: one frame over the WHOLE of both volumes -- a plain triple loop over the
  * geometry voxels, then a plain triple loop over the colour voxels.  geo / col are the packed
  * state arrays (layout above), updated in place.  counters[4] (nullable) receives this frame's
- * CNT_* counts.  OpenMP only splits the outermost z loop; voxels are independent (A15). */
-int ref_integrate(const ref_vol_t *v, const ref_frame_t *f, uint32_t *geo, uint32_t *col, uint64_t *counters)
+ * CNT_* counts.  OpenMP only splits the outermost z loop; voxels are independent (A15).
+ * sec (nullable): four byte maps, one byte per 32-byte SECTOR (8 consecutive words of the linear
+ * layout) of the geometry / colour array, set to 1 where a voxel of the sector was read / changed
+ * (sec[0] geometry read, sec[1] geometry changed, sec[2] colour read, sec[3] colour changed): the
+ * DRAM granularity of the same sets (SURVEY 8(d) "report both voxel-exact and sector-exact"). */
+static int integrate_all(const ref_vol_t *v, const ref_frame_t *f, uint32_t *geo, uint32_t *col, uint64_t *counters, uint8_t *const sec[4])
 {
     if (!v || !f || !geo || !col || !f->depth || !f->rgb) return -1;
     if (v->nx <= 0 || v->ny <= 0 || v->nz <= 0 || v->r < 1 || !(v->mu > 0.0f) || v->w_max < 1 || v->w_max > 512) return -1;
@@ -249,6 +256,16 @@ int ref_integrate(const ref_vol_t *v, const ref_frame_t *f, uint32_t *geo, uint3
                 size_t idx = ((size_t)k * (size_t)v->ny + (size_t)j) * (size_t)v->nx + (size_t)i;
                 int s = update_geo_voxel(v, f, &c, i, j, k, &geo[idx]);
                 gr += (uint64_t)(s & 1); gc += (uint64_t)(s >> 1);
+                if (sec) {                      /* (a sector can straddle two layers, i.e. two threads: same value, atomic store) */
+                    if (s & 1) {
+#pragma omp atomic write
+                        sec[0][idx >> 3] = 1;
+                    }
+                    if (s >> 1) {
+#pragma omp atomic write
+                        sec[1][idx >> 3] = 1;
+                    }
+                }
             }
     const int cx = v->nx * v->r, cy = v->ny * v->r, cz = v->nz * v->r;
 #pragma omp parallel for schedule(static) reduction(+ : cr, cc)
@@ -258,9 +275,43 @@ int ref_integrate(const ref_vol_t *v, const ref_frame_t *f, uint32_t *geo, uint3
                 size_t idx = ((size_t)k * (size_t)cy + (size_t)j) * (size_t)cx + (size_t)i;
                 int s = update_col_voxel(v, f, &c, i, j, k, &col[idx]);
                 cr += (uint64_t)(s & 1); cc += (uint64_t)(s >> 1);
+                if (sec) {
+                    if (s & 1) {
+#pragma omp atomic write
+                        sec[2][idx >> 3] = 1;
+                    }
+                    if (s >> 1) {
+#pragma omp atomic write
+                        sec[3][idx >> 3] = 1;
+                    }
+                }
             }
     if (counters) { counters[CNT_GEO_READ] = gr; counters[CNT_GEO_CHANGED] = gc; counters[CNT_COL_READ] = cr; counters[CNT_COL_CHANGED] = cc; }
     return 0;
+}
+
+int ref_integrate(const ref_vol_t *v, const ref_frame_t *f, uint32_t *geo, uint32_t *col, uint64_t *counters)
+{
+    return integrate_all(v, f, geo, col, counters, NULL);
+}
+
+/* the same, with the sector maps (caller-zeroed; sizes ceil(N / 8) bytes each) */
+int ref_integrate_sectors(const ref_vol_t *v, const ref_frame_t *f, uint32_t *geo, uint32_t *col, uint64_t *counters,
+                          uint8_t *geo_read, uint8_t *geo_changed, uint8_t *col_read, uint8_t *col_changed)
+{
+    uint8_t *const sec[4] = {geo_read, geo_changed, col_read, col_changed};
+    if (!geo_read || !geo_changed || !col_read || !col_changed) return -1;
+    return integrate_all(v, f, geo, col, counters, sec);
+}
+
+/* how many threads the loops above use (reported beside the timed CPU baseline) */
+int ref_threads(void)
+{
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
 }
 
 /* ref_integrate_subset: the same per-voxel updates applied to a LIST of voxels only (voxels never

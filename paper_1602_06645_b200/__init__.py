@@ -71,7 +71,8 @@ class VolStats(ctypes.Structure):
                 ("items_col", ctypes.c_uint32), ("cells_col", ctypes.c_uint32),
                 ("geo_sectors_read", ctypes.c_uint64), ("geo_sectors_written", ctypes.c_uint64),
                 ("col_sectors_read", ctypes.c_uint64), ("col_sectors_written", ctypes.c_uint64),
-                ("geo_visited", ctypes.c_uint64), ("col_gated", ctypes.c_uint64), ("reserved64", ctypes.c_uint64),
+                ("geo_visited", ctypes.c_uint64), ("col_gated", ctypes.c_uint64), ("geo_skippable", ctypes.c_uint64),
+                ("geo_sectors_skippable", ctypes.c_uint64),
                 ("subs_geo", ctypes.c_uint32), ("jobs_mark", ctypes.c_uint32)]
 
 

@@ -142,6 +142,27 @@ __device__ __forceinline__ uint32_t ld_relaxed(const uint32_t *ptr)
 
 struct Counts { unsigned long long n[CNT_N]; };
 
+// development aid (compile with -DVF_TRACE): per-warp timestamps of the phase transitions of k_fused, 16 words per warp
+#ifdef VF_TRACE
+__device__ unsigned long long g_trace[8192 * 16];
+__device__ __forceinline__ unsigned long long vf_now() { unsigned long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); return t; }
+#define VF_T(slot) do { if (lane == 0 && gw < 8192u) g_trace[gw * 16u + (slot)] = vf_now(); } while (0)
+#define VF_TC(slot, v) do { if (lane == 0 && gw < 8192u) g_trace[gw * 16u + (slot)] = (v); } while (0)
+#else
+#define VF_T(slot) do { } while (0)
+#define VF_TC(slot, v) do { } while (0)
+#endif
+
+// COUNT only: 1 if the lane is the first of the whole frame to touch the 32-byte sector (8 words) of word index `word` in
+// volume map `which` (Params::sec_map)
+__device__ __forceinline__ unsigned sector_first(const Params &p, int which, bool pred, unsigned long long word)
+{
+    if (!pred) return 0u;
+    const unsigned long long s = word >> 3;
+    const uint32_t bit = 1u << (unsigned)(s & 31ull);
+    return (atomicOr(p.sec_map[which] + (s >> 5), bit) & bit) ? 0u : 1u;
+}
+
 // ptr + e layers (e = 0..3 a compile-time constant after unrolling): one mad.wide with an immediate
 __device__ __forceinline__ uint32_t *layer_ptr(uint32_t *ptr, int e, uint32_t layer_b)
 {
@@ -243,99 +264,10 @@ __device__ __noinline__ void geometry_tile_near(const Params &p, int ttx, int tt
             if (COUNT) {
                 c.n[CNT_GEO_VISITED] += 1; c.n[CNT_GEO_READ] += rd; c.n[CNT_GEO_CHANGED] += w != o;
                 const unsigned long long wi = (unsigned long long)(ptr - p.geo);
-                const unsigned act = __activemask();
-                const unsigned pr = __match_any_sync(act, rd ? wi >> 3 : ~0ull), pw = __match_any_sync(act, w != o ? wi >> 3 : ~0ull);
-                c.n[CNT_GEO_SEC_READ] += rd && __ffs(pr) - 1 == lane; c.n[CNT_GEO_SEC_WRITTEN] += w != o && __ffs(pw) - 1 == lane;
+                c.n[CNT_GEO_SEC_READ] += sector_first(p, 0, rd, wi); c.n[CNT_GEO_SEC_WRITTEN] += sector_first(p, 1, w != o, wi);
             }
             if (w != o) *ptr = w;
         }
-    }
-}
-
-// One z half (4 layers) of a geometry tile whose four x sub-boxes are all wanted: the whole 32 x 4 footprint.
-// lane = (vx = lane & 7, y = lane >> 3) owns voxels (gx0 + 4 vx .. + 3, gy0 + y) of every layer as one 16-byte vector, so a
-// warp access is four full 128-byte lines and everything per layer (z term of eq. 5, pointer, load, store) is shared by four
-// voxels.  The layers are software-pipelined over two alternating register sets: while layer z is updated, layer z + 1 has
-// already been projected and its four depth gathers and its voxel vector are in flight.  Needs nx % 4 == 0.
-template <bool COUNT, int VAR>
-__device__ __forceinline__ void geometry_half_rows(const Params &p, int ttx, int tty, int gz0, int lz0, int lane, Counts &c)
-{
-    const int i0 = ttx * TX + 4 * (lane & 7), j = tty * TY + (lane >> 3);
-    const bool inside = i0 < p.nx && j < p.ny;
-    const int nl = inside ? min(TZ / SUBZ, p.nz - gz0) : 0;
-    const float fx = p.fx, fy = p.fy, cx = p.cx, cy = p.cy;
-    const float neg_mu = p.neg_mu, inv_mu = p.inv_mu;
-    const uint32_t wd = (uint32_t)p.wd, wbits = __float_as_uint(p.wd_f), hbits = __float_as_uint(p.hd_f), koff = 0x4B400000u * (wd + 1u);
-    const int w_max = p.w_max;
-    const float *__restrict__ depthf = p.depthf;
-    // per-column bases of eq. 5: fma(R_1, py, fma(R_0, px, t)) -- the z term is added per layer with one fma each
-    const float py = __fmaf_rn((float)j + 0.5f, p.vs, p.oy);
-    float bX[4], bY[4], bZ[4];
-#pragma unroll
-    for (int e = 0; e < 4; ++e) {
-        const float px = __fmaf_rn((float)(i0 + e) + 0.5f, p.vs, p.ox);
-        bX[e] = __fmaf_rn(p.R[1], py, __fmaf_rn(p.R[0], px, p.t[0]));
-        bY[e] = __fmaf_rn(p.R[4], py, __fmaf_rn(p.R[3], px, p.t[1]));
-        bZ[e] = __fmaf_rn(p.R[7], py, __fmaf_rn(p.R[6], px, p.t[2]));
-    }
-    const float r02 = p.R[2], r12 = p.R[5], r22 = p.R[8];
-    const uint32_t layer_b = (uint32_t)((size_t)p.ny * p.nx * 4u);
-    uint32_t *ptr0 = p.geo + ((size_t)lz0 * p.ny + j) * p.nx + i0;
-    // S2 of one layer: eq. 5 z term, projection, and the four depth gathers
-    auto project_layer = [&](int z, float (&Z)[4], float (&D)[4], float (&L)[4]) {
-        const float pz = __fmaf_rn((float)(gz0 + z) + 0.5f, p.vs, p.oz);
-#pragma unroll
-        for (int e = 0; e < 4; ++e) {
-            const float X = __fmaf_rn(r02, pz, bX[e]), Y = __fmaf_rn(r12, pz, bY[e]);
-            Z[e] = __fmaf_rn(r22, pz, bZ[e]);
-            bool ok; uint32_t off; float iz;
-            project_fast_raw(fx, fy, cx, cy, wd, wbits, hbits, koff, X, Y, Z[e], ok, off, iz);
-            if (VAR == VAR_TSDF_ALONG_RAY)
-                L[e] = __fmul_rn(__fsqrt_rn(__fmaf_rn(Z[e], Z[e], __fmaf_rn(Y, Y, __fmul_rn(X, X)))), iz);
-            D[e] = 0.0f;
-            if (ok) {
-                unsigned long long addr;
-                asm("mad.wide.u32 %0, %1, 4, %2;" : "=l"(addr) : "r"(off), "l"(depthf));
-                D[e] = __ldg(reinterpret_cast<const float *>(addr));
-            }
-        }
-    };
-    auto update_layer = [&](int z, const uint4 &cur, const float (&Z)[4], const float (&D)[4], const float (&L)[4]) {
-        const uint32_t o[4] = {cur.x, cur.y, cur.z, cur.w};
-        uint32_t w4[4]; bool upd[4];
-        const float Dm[4] = {z < nl ? D[0] : 0.0f, z < nl ? D[1] : 0.0f, z < nl ? D[2] : 0.0f, z < nl ? D[3] : 0.0f};
-        tsdf_update4<COUNT, VAR>(o, Z, Dm, L, neg_mu, inv_mu, w_max, w4, upd);
-        const bool any = (w4[0] != o[0]) | (w4[1] != o[1]) | (w4[2] != o[2]) | (w4[3] != o[3]);
-        uint4 *ptr = reinterpret_cast<uint4 *>(layer_ptr(ptr0, z, layer_b));
-        if (COUNT && z < nl) {
-            c.n[CNT_GEO_VISITED] += 4; c.n[CNT_GEO_READ] += upd[0] + upd[1] + upd[2] + upd[3];
-            c.n[CNT_GEO_CHANGED] += (w4[0] != o[0]) + (w4[1] != o[1]) + (w4[2] != o[2]) + (w4[3] != o[3]);
-        }
-        if (COUNT) {                                                  // (a 16-byte aligned vector lies in one 32-byte sector)
-            const unsigned long long wi = (unsigned long long)(reinterpret_cast<uint32_t *>(ptr) - p.geo);
-            c.n[CNT_GEO_SEC_READ] += sectors_touched(z < nl && (upd[0] | upd[1] | upd[2] | upd[3]), wi, lane);
-            c.n[CNT_GEO_SEC_WRITTEN] += sectors_touched(any, wi, lane);
-        }
-        if (any) __stcg(ptr, make_uint4(w4[0], w4[1], w4[2], w4[3]));   // skip the store when nothing changed
-    };
-    // Two register sets, A (even layers) and B (odd layers), used alternately: the pipeline needs no register-to-register
-    // rotation, which would make the warp wait for the loads it has just issued.  Lanes outside the volume (nl = 0) go
-    // through the motions with D = 0 (nothing is loaded or stored): the update votes with the whole warp.
-    float ZA[4], ZB[4], DA[4], DB[4], LA[4], LB[4];
-    const uint4 zero = make_uint4(0u, 0u, 0u, 0u);
-    // the voxel stream bypasses L1 (__ldcg): every line is used once, and L1 is better spent on the depth image
-    uint4 curA = nl > 0 ? __ldcg(reinterpret_cast<const uint4 *>(ptr0)) : zero, curB = zero;
-    project_layer(0, ZA, DA, LA);
-#pragma unroll
-    for (int z = 0; z < TZ / SUBZ; z += 2) {
-        curB = z + 1 < nl ? __ldcg(reinterpret_cast<const uint4 *>(layer_ptr(ptr0, z + 1, layer_b))) : zero;
-        project_layer(z + 1, ZB, DB, LB);                                    // layer z + 1 in flight
-        update_layer(z, curA, ZA, DA, LA);
-        if (z + 2 < TZ / SUBZ) {
-            curA = z + 2 < nl ? __ldcg(reinterpret_cast<const uint4 *>(layer_ptr(ptr0, z + 2, layer_b))) : zero;
-            project_layer(z + 2, ZA, DA, LA);                                // layer z + 2 in flight
-        }
-        update_layer(z + 1, curB, ZB, DB, LB);
     }
 }
 
@@ -343,9 +275,13 @@ __device__ __forceinline__ void geometry_half_rows(const Params &p, int ttx, int
 // y = lane >> 3) owns the column of 4 voxels along z, so every access of the warp is four whole 32-byte sectors and the
 // per-column part of eq. 5 is hoisted.  The passes are software-pipelined over two alternating register sets: while
 // sub-box n is updated, sub-box n + 1 has already been projected and its depth gathers and voxel loads are in flight.
+// Returns the sub-boxes (bits bx) all of whose voxels hold the saturated free-space word afterwards.  COUNT: sk4 = the
+// sub-boxes the plain variant would not have been given (their voxels are counted as skippable too).
 template <bool COUNT, int VAR>
-__device__ __forceinline__ void geometry_half_boxes(const Params &p, int ttx, int tty, int gz0, int lz0, uint32_t m4, int lane, Counts &c)
+__device__ __forceinline__ uint32_t geometry_half_boxes(const Params &p, int ttx, int tty, int gz0, int lz0, uint32_t m4, uint32_t sk4, int lane, Counts &c)
 {
+    const uint32_t sat_word = 0x7fffu | ((uint32_t)p.w_max << 16);
+    uint32_t sat4 = 0u;
     const int xl = lane & 7, j = tty * TY + (lane >> 3);
     const float fx = p.fx, fy = p.fy, cx = p.cx, cy = p.cy, vs = p.vs;
     const float neg_mu = p.neg_mu, inv_mu = p.inv_mu;
@@ -361,9 +297,9 @@ __device__ __forceinline__ void geometry_half_boxes(const Params &p, int ttx, in
     for (int e = 0; e < 4; ++e) pz[e] = __fmaf_rn((float)(gz0 + e) + 0.5f, vs, p.oz);
     // S2 of one sub-box: eq. 5, projection, the four depth gathers and the four voxel loads.  A voxel outside the frustum
     // or the volume keeps D = 0 ("invalid depth": not updated); its gather is predicated off.
-    auto load_project = [&](int bx, uint32_t *&ptr, uint32_t (&o)[4], float (&Z)[4], float (&D)[4], float (&L)[4]) {
+    auto load_project = [&](int bx, int &nrem, uint32_t *&ptr, uint32_t (&o)[4], float (&Z)[4], float (&D)[4], float (&L)[4]) {
         const int i = ttx * TX + 8 * bx + xl;
-        const int nrem = i < p.nx ? nrem_row : 0;
+        nrem = i < p.nx ? nrem_row : 0;
         const float px = __fmaf_rn((float)i + 0.5f, vs, p.ox);
         const float bX = __fmaf_rn(p.R[1], py, __fmaf_rn(p.R[0], px, p.t[0]));
         const float bY = __fmaf_rn(p.R[4], py, __fmaf_rn(p.R[3], px, p.t[1]));
@@ -390,65 +326,77 @@ __device__ __forceinline__ void geometry_half_boxes(const Params &p, int ttx, in
         }
     };
     // S3 of one sub-box: truncation test, running average, store of the words that changed
-    auto update = [&](uint32_t *ptr, const uint32_t (&o)[4], const float (&Z)[4], const float (&D)[4], const float (&L)[4]) {
+    // (nrem = how many of the four voxels of the lane exist: the others count as saturated)
+    auto update = [&](int bx, int nrem, uint32_t *ptr, const uint32_t (&o)[4], const float (&Z)[4], const float (&D)[4], const float (&L)[4]) {
         uint32_t w4[4]; bool upd[4];
         tsdf_update4<COUNT, VAR>(o, Z, D, L, neg_mu, inv_mu, w_max, w4, upd);
+        bool sat = true;
 #pragma unroll
         for (int e = 0; e < 4; ++e) {
             if (COUNT) {
                 const unsigned long long wi = (unsigned long long)(layer_ptr(ptr, e, layer_b) - p.geo);
                 c.n[CNT_GEO_VISITED] += 1; c.n[CNT_GEO_READ] += upd[e]; c.n[CNT_GEO_CHANGED] += w4[e] != o[e];
-                c.n[CNT_GEO_SEC_READ] += sectors_touched(upd[e], wi, lane);
-                c.n[CNT_GEO_SEC_WRITTEN] += sectors_touched(w4[e] != o[e], wi, lane);
+                const unsigned sr = sector_first(p, 0, upd[e], wi);
+                c.n[CNT_GEO_SEC_READ] += sr;
+                c.n[CNT_GEO_SEC_WRITTEN] += sector_first(p, 1, w4[e] != o[e], wi);
+                if ((sk4 >> bx) & 1u) { c.n[CNT_GEO_SKIPPABLE] += upd[e]; c.n[CNT_GEO_SEC_SKIPPABLE] += sr; }
             }
+            sat = sat & ((w4[e] == sat_word) | (e >= nrem));
             if (w4[e] != o[e]) __stcg(layer_ptr(ptr, e, layer_b), w4[e]);   // skip the store when nothing changed
         }
+        if (__all_sync(0xffffffffu, sat)) sat4 |= 1u << bx;
     };
     // Two register sets, A and B, used alternately (no register-to-register rotation)
     uint32_t *pA, *pB, oA[4], oB[4];
     float ZA[4], ZB[4], DA[4], DB[4], LA[4], LB[4];
+    int bA, bB, nA, nB;
     uint32_t m = m4;
     if (COUNT && lane == 0) atomicAdd(&p.ctrl[ST_SUBS], (uint32_t)__popc(m));
-    int b = __ffs(m) - 1; m &= m - 1u;
-    load_project(b, pA, oA, ZA, DA, LA);
+    bA = __ffs(m) - 1; m &= m - 1u;
+    load_project(bA, nA, pA, oA, ZA, DA, LA);
     for (;;) {
         const bool hasB = m != 0u;
-        if (hasB) { b = __ffs(m) - 1; m &= m - 1u; load_project(b, pB, oB, ZB, DB, LB); }      // sub-box n + 1 in flight
-        update(pA, oA, ZA, DA, LA);
+        if (hasB) { bB = __ffs(m) - 1; m &= m - 1u; load_project(bB, nB, pB, oB, ZB, DB, LB); }   // sub-box n + 1 in flight
+        update(bA, nA, pA, oA, ZA, DA, LA);
         if (!hasB) break;
         const bool hasA = m != 0u;
-        if (hasA) { b = __ffs(m) - 1; m &= m - 1u; load_project(b, pA, oA, ZA, DA, LA); }      // sub-box n + 2 in flight
-        update(pB, oB, ZB, DB, LB);
+        if (hasA) { bA = __ffs(m) - 1; m &= m - 1u; load_project(bA, nA, pA, oA, ZA, DA, LA); }   // sub-box n + 2 in flight
+        update(bB, nB, pB, oB, ZB, DB, LB);
         if (!hasA) break;
     }
+    return sat4;
 }
 
-#ifndef VF_ROWS_PATH
-#define VF_ROWS_PATH 0
-#endif
-// one geometry tile, one warp.  The item names the tile's 8x4x4 sub-boxes that may hold a voxel this frame updates.  Each z
-// half of the tile (4 layers) is processed either as whole rows, when all four of its sub-boxes are wanted (the common
-// case: free space), or sub-box by sub-box.
+// one geometry tile, one warp.  The item names the tile's 8x4x4 sub-boxes that may hold a voxel this frame updates; they
+// are visited z half by z half (4 layers).
+// (A whole-row path for z halves whose four sub-boxes are all wanted -- 16-byte vectors, everything per layer shared by four
+// voxels -- was measured: 14 % faster on a saturating frame, but its registers cost the scan frames 8 % even when it is not
+// taken, so it is not in the kernel.)
 template <bool COUNT, int VAR>
 __device__ __forceinline__ void geometry_tile(const Params &p, uint32_t item, int lane, Counts &c)
 {
     int ttx, tty, ttz, mask;
     item_unpack(item, ttx, tty, ttz, mask);
-    if (tile_is_near(p, ttx, tty, ttz)) { geometry_tile_near<COUNT>(p, ttx, tty, ttz, lane, c); return; }
+    const uint32_t tile = (uint32_t)((ttz * p.tiles_y + tty) * p.tiles_x + ttx);
+    if (tile_is_near(p, ttx, tty, ttz)) {
+        if (lane == 0) p.tile_sat[tile] = 0;
+        geometry_tile_near<COUNT>(p, ttx, tty, ttz, lane, c);
+        return;
+    }
     const int gz0 = local_to_global_tz(p, ttz) * TZ, lz0 = ttz * TZ;
-    const bool vec_ok = (p.nx & 3) == 0;
+    uint32_t sat = (uint32_t)__ldg(p.tile_sat + tile) & ~(uint32_t)mask;   // the visited sub-boxes are looked at afresh
+    const uint32_t skippable = COUNT ? (uint32_t)__ldcg(p.tile_skip + tile) : 0u;
 #pragma unroll 1
     for (int zh = 0; zh < SUBZ; ++zh) {
         uint32_t m = ((uint32_t)mask >> zh) & 0x55u;                  // bit 2 bx: sub-box bx of this half
         if (m == 0u) continue;
-        if (VF_ROWS_PATH && m == 0x55u && vec_ok) {
-            if (COUNT && lane == 0) atomicAdd(&p.ctrl[ST_SUBS], 4u);
-            geometry_half_rows<COUNT, VAR>(p, ttx, tty, gz0 + zh * (TZ / SUBZ), lz0 + zh * (TZ / SUBZ), lane, c);
-        } else {
-            m = (m | (m >> 1)) & 0x33u; m = (m | (m >> 2)) & 0x0fu;   // bit bx
-            geometry_half_boxes<COUNT, VAR>(p, ttx, tty, gz0 + zh * (TZ / SUBZ), lz0 + zh * (TZ / SUBZ), m, lane, c);
-        }
+        m = (m | (m >> 1)) & 0x33u; m = (m | (m >> 2)) & 0x0fu;       // bit bx
+        uint32_t sk = (skippable >> zh) & 0x55u;
+        sk = (sk | (sk >> 1)) & 0x33u; sk = (sk | (sk >> 2)) & 0x0fu;
+        const uint32_t s4 = geometry_half_boxes<COUNT, VAR>(p, ttx, tty, gz0 + zh * (TZ / SUBZ), lz0 + zh * (TZ / SUBZ), m, sk, lane, c);
+        sat |= (((s4 & 1u) | ((s4 & 2u) << 1) | ((s4 & 4u) << 2) | ((s4 & 8u) << 3)) << zh);   // bit bx -> bit 2 bx + zh
     }
+    if (lane == 0) p.tile_sat[tile] = (uint8_t)sat;
 }
 
 // pull the sectors of a geometry tile into L2 when the tile is started: lane = (row, layer); a layer is wanted when its z
@@ -558,8 +506,8 @@ __device__ __forceinline__ void colour_update_staged(const Params &p, const Stag
     }
     if (COUNT) {
         c.n[CNT_COL_READ] += have; c.n[CNT_COL_CHANGED] += have && nw != old;
-        c.n[CNT_COL_SEC_READ] += sectors_touched(have, wi, lane);
-        c.n[CNT_COL_SEC_WRITTEN] += sectors_touched(have && nw != old, wi, lane);
+        c.n[CNT_COL_SEC_READ] += sector_first(p, 2, have, wi);
+        c.n[CNT_COL_SEC_WRITTEN] += sector_first(p, 3, have && nw != old, wi);
     }
 }
 

@@ -74,6 +74,14 @@ struct Params {
     uint32_t *work_geo;          // geometry work list (n_tiles entries, all zero between frames: a slot is cleared by the warp that takes it)
     uint32_t *marks;             // shell marks: words_per_tile(r) words per tile, bit = colour cell that may hold sigma-shell voxels
     uint2    *work_col;          // colour work list: one item per non-zero mark NIBBLE (up to 4 colour cells): {tile | nibble index, the nibble's bits}
+    uint8_t  *tile_sat;          // per geometry tile: bit bx * SUBZ + bz = every voxel of that sub-box holds the saturated free-space word
+                                 // (tsdf_q = 32767, w = w_max).  Kept by the fused kernel for the sub-boxes it visits; a sub-box
+                                 // with its bit set that lies in front of every depth it can see by more than mu cannot change
+                                 // this frame and is not queued (vol_reset / vol_upload clear the bits)
+    uint8_t  *tile_skip;         // counting variant only: the sub-boxes of the tile that would not have been queued for that reason
+    int       counting;          // the counting variant visits them all the same: its counters are the method's, not the kernel's
+    uint32_t *sec_map[4];        // counting variant only: one bit per 32-byte sector of the geometry (read, written) and the colour
+                                 // volume (read, written), zeroed before every frame: a sector is counted when its bit is first set
     uint8_t  *tile_neg;          // per geometry tile: 1 = the tile may hold an observed voxel with tsdf <= 0.  Set by the tile
                                  // classification (k_mark_classify), never cleared except by vol_reset (vol_upload sets
                                  // all): a conservative superset, used by the ray caster to skip free space
@@ -107,7 +115,7 @@ __device__ __forceinline__ void item_unpack(uint32_t item, int &ttx, int &tty, i
 // counters alternately, see Params::parity).
 enum { ST_NGEO = 0, ST_NCOL = 1, ST_CELLS = 2, ST_SUBS = 3, ST_NJOBS = 4, ST_N = 8 };
 enum { CNT_GEO_READ = 0, CNT_GEO_CHANGED, CNT_COL_READ, CNT_COL_CHANGED, CNT_GEO_SEC_READ, CNT_GEO_SEC_WRITTEN, CNT_COL_SEC_READ,
-       CNT_COL_SEC_WRITTEN, CNT_GEO_VISITED, CNT_COL_GATED, CNT_SPARE0, CNT_SPARE1, CNT_N = 12 };
+       CNT_COL_SEC_WRITTEN, CNT_GEO_VISITED, CNT_COL_GATED, CNT_GEO_SKIPPABLE, CNT_GEO_SEC_SKIPPABLE, CNT_N = 12 };
 constexpr int CTRL_Q0 = 32;                                  // first queue-control word (byte 128)
 // every queue-control word has a 128-byte line (and so, by the address hash, most likely an L2 slice) of its own: thousands
 // of warps draw tickets from and poll these words, and requests to one line are served one after the other

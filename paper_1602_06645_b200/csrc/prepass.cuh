@@ -310,7 +310,8 @@ __device__ __forceinline__ bool tile_is_near(const Params &p, int ttx, int tty, 
 // culling only: can any voxel of the camera-space box (centre c, half extents e) pass the TSDF tests (frustum, valid
 // depth, sdf >= -mu)?  Conservative: max valid depth over the box's pixel rectangle against the box's nearest Z.
 // Returns 0 = no, 1 = maybe, 2 = maybe and the whole box lies in front of every valid depth of its rectangle (free space:
-// a finer look at the box would find the same).
+// a finer look at the box would find the same), 3 = ... by more than mu: every voxel of the box that is updated at all gets
+// tsdf = 1 exactly (sdf >= mu + 0.1 mm, against the slack of this fp32 evaluation and the rounding of sdf / mu).
 __device__ __forceinline__ int box_may_update(const Params &p, float cX, float cY, float cZ, float eX, float eY, float eZ)
 {
     int x0, x1, y0, y1; float zmin, zmax;
@@ -318,7 +319,8 @@ __device__ __forceinline__ int box_may_update(const Params &p, float cX, float c
     uint32_t mn, mx;
     depth_range(p, x0, x1, y0, y1, mn, mx);
     if (mx == 0u || !(zmin <= ((float)mx * 0.001f + 1e-4f) + p.mu)) return 0;
-    return zmax <= (float)mn * 0.001f - 1e-4f ? 2 : 1;
+    const float dmin = (float)mn * 0.001f - 1e-4f;
+    return zmax <= dmin ? (zmax + p.mu * 1.0001f + 1e-4f <= dmin ? 3 : 2) : 1;
 }
 
 // The three producer roles of the fused kernel.  Each is one CHUNK of work for one warp; chunks are claimed from counters
@@ -343,7 +345,7 @@ __device__ __forceinline__ void classify_chunk(const Params &p, uint32_t chunk, 
         coarse = box_may_update(p, cX, cY, cZ, p.tile_ex, p.tile_ey, p.tile_ez);
     }
     unsigned surv = __ballot_sync(0xffffffffu, coarse != 0);
-    uint32_t mask = 0u;
+    uint32_t mask = 0u, free3 = 0u;                  // sub-boxes to visit; sub-boxes in free space by more than mu
     const float sx = (float)(TX / SUBX) * p.vs, sz = (float)(TZ / SUBZ) * p.vs;
     const int sb = lane & 7, bx = sb / SUBZ, bz = sb % SUBZ;        // item mask bit = bx * SUBZ + bz
     const float dx = ((float)bx - 0.5f * (float)(SUBX - 1)) * sx, dz = ((float)bz - 0.5f * (float)(SUBZ - 1)) * sz;
@@ -353,15 +355,20 @@ __device__ __forceinline__ void classify_chunk(const Params &p, uint32_t chunk, 
         for (int k = 0; k < 4; ++k) { src[k] = surv ? __ffs(surv) - 1 : -1; surv &= surv - 1u; }
         const int mine = src[lane >> 3];
         const float sX = __shfl_sync(0xffffffffu, cX, mine & 31), sY = __shfl_sync(0xffffffffu, cY, mine & 31), sZ = __shfl_sync(0xffffffffu, cZ, mine & 31);
-        const bool ok = mine >= 0 && box_may_update(p, sX + p.R[0] * dx + p.R[2] * dz, sY + p.R[3] * dx + p.R[5] * dz,
-                                                    sZ + p.R[6] * dx + p.R[8] * dz, p.sub_ex, p.sub_ey, p.sub_ez) != 0;
-        const unsigned b = __ballot_sync(0xffffffffu, ok);
+        const int cls = mine < 0 ? 0 : box_may_update(p, sX + p.R[0] * dx + p.R[2] * dz, sY + p.R[3] * dx + p.R[5] * dz,
+                                                      sZ + p.R[6] * dx + p.R[8] * dz, p.sub_ex, p.sub_ey, p.sub_ez);
+        const unsigned b = __ballot_sync(0xffffffffu, cls != 0), b3 = __ballot_sync(0xffffffffu, cls == 3);
 #pragma unroll
-        for (int k = 0; k < 4; ++k) if (lane == src[k]) mask = (b >> (8 * k)) & 0xffu;
+        for (int k = 0; k < 4; ++k) if (lane == src[k]) { mask = (b >> (8 * k)) & 0xffu; free3 = (b3 >> (8 * k)) & 0xffu; }
     }
     // a partial last slab: sub-boxes whose first layer lies beyond the volume are not queued at all
     if (local_to_global_tz(p, ttz) * TZ + TZ / SUBZ >= p.nz) mask &= 0x55u;
     if (near && mask) mask = 0xffu;                  // NEAR tiles are processed whole, by the plain routines
+    else if (mask) {
+        // saturated free space stays what it is: (32767 w_max + 32767) / (w_max + 1) = 32767 exactly, w = min(w_max + 1, w_max)
+        const uint32_t skip = mask & free3 & (uint32_t)p.tile_sat[tile];
+        if (p.counting) p.tile_skip[tile] = (uint8_t)skip; else mask &= ~skip;
+    }
     // For the ray caster (raycast.cuh): a voxel can only receive tsdf <= 0 in a visited tile that is NOT wholly in front of
     // every depth it can see (in front by >= 0.1 mm, mu <= 1 m: every new sample is >= 3 q-units, so the running average of
     // positive values stays >= 1).  Flag those tiles and their bricks; flags are only ever set (vol_reset clears them,

@@ -83,6 +83,13 @@ static FusedFn fused_kernel(bool counting, int variant)
 
 static int set_device(const vol *v) { CK(cudaSetDevice(v->device)); return VOL_OK; }
 
+// counting variant: bytes of sector map i (one bit per 8 words of the geometry (i < 2) or colour volume, rounded up to words)
+static size_t sec_map_bytes(const vol *v, int i)
+{
+    const size_t words = (i < 2 ? v->geo_bytes : v->col_bytes) / 4u;
+    return ((words + 7u) / 8u + 31u) / 32u * 4u + 4u;
+}
+
 // rigid inverse in fp64 with left-to-right sums, rounded once to fp32 (S0).  Returns false if T is not rigid.
 static bool rigid_inverse(const float T[16], float Rout[9], float tout[3])
 {
@@ -221,6 +228,8 @@ extern "C" int vol_create(vol_t **out, const int32_t dims_geo[3], int32_t r, con
     if (cudaMalloc(&p.work_col, sizeof(uint2) * nw * 8) != cudaSuccess) rc = VOL_E_OOM;
     if (cudaMalloc(&p.marks, sizeof(uint32_t) * nw) != cudaSuccess) rc = VOL_E_OOM;
     if (rc == VOL_OK && cudaMemset(p.marks, 0, sizeof(uint32_t) * nw) != cudaSuccess) rc = VOL_E_CUDA;
+    if (cudaMalloc(&p.tile_sat, nt) != cudaSuccess || cudaMalloc(&p.tile_skip, nt) != cudaSuccess) rc = VOL_E_OOM;
+    if (rc == VOL_OK && (cudaMemset(p.tile_sat, 0, nt) != cudaSuccess || cudaMemset(p.tile_skip, 0, nt) != cudaSuccess)) rc = VOL_E_CUDA;
     if (cudaMalloc(&p.tile_neg, nt) != cudaSuccess) rc = VOL_E_OOM;
     if (rc == VOL_OK && cudaMemset(p.tile_neg, 0, nt) != cudaSuccess) rc = VOL_E_CUDA;
     p.bricks_x = p.tiles_x; p.bricks_y = (p.tiles_y + 7) / 8; p.bricks_z = (my_slabs + 3) / 4;
@@ -269,6 +278,9 @@ extern "C" void vol_destroy(vol_t *v)
     if (v->p.marks) cudaFree(v->p.marks);
     if (v->p.jobs) cudaFree(v->p.jobs);
     if (v->p.tile_neg) cudaFree(v->p.tile_neg);
+    if (v->p.tile_sat) cudaFree(v->p.tile_sat);
+    if (v->p.tile_skip) cudaFree(v->p.tile_skip);
+    for (int i = 0; i < 4; ++i) if (v->p.sec_map[i]) cudaFree(v->p.sec_map[i]);
     if (v->p.brick_neg) cudaFree(v->p.brick_neg);
     if (v->p.ctrl) cudaFree(v->p.ctrl);
     if (v->p.pixmap) cudaFree(v->p.pixmap);
@@ -343,13 +355,17 @@ static int integrate_impl(vol_t *v, const uint16_t *depth_u16_dev, int32_t wd, i
     box_extents(p.R, 0.5 * vf::TX * p.vs, 0.5 * vf::TY * p.vs, 0.5 * vf::TZ * p.vs, slack, p.tile_ex, p.tile_ey, p.tile_ez);
     box_extents(p.R, 0.5 * (vf::TX / vf::SUBX) * p.vs, 0.5 * vf::TY * p.vs, 0.5 * (vf::TZ / vf::SUBZ) * p.vs, slack, p.sub_ex, p.sub_ey, p.sub_ez);
     p.parity = (int)(v->frame_seq & 1u);
+    p.counting = v->counting ? 1 : 0;
     p.sigma_g = (float)((double)p.sigma * 1.0001 + slack);
     camera_to_world(p.R, p.t, p.Rw, p.tw);
     if (p.n_tiles == 0) return VOL_OK;
 
     cudaStream_t s = (cudaStream_t)stream;
     if (rgb_ready && !split) { CK(cudaStreamWaitEvent(s, rgb_ready, 0)); rgb_ready = nullptr; }
-    if (v->counting) CK(cudaMemsetAsync(p.counters, 0, sizeof(unsigned long long) * vf::CNT_N, s));
+    if (v->counting) {
+        CK(cudaMemsetAsync(p.counters, 0, sizeof(unsigned long long) * vf::CNT_N, s));
+        for (int i = 0; i < 4; ++i) CK(cudaMemsetAsync(p.sec_map[i], 0, sec_map_bytes(v, i), s));
+    }
     if (v->profiling) CK(cudaEventRecord(v->ev[0], s));
     const dim3 g0((wd + 31) / 32, (hd + 31) / 32);
     const int g2 = v->fused_blocks;
@@ -502,6 +518,7 @@ extern "C" int vol_upload(vol_t *v, const void *geo_host, const void *col_host, 
     if (geo_host && v->geo_bytes) CK(cudaMemcpyAsync(v->p.geo, geo_host, v->geo_bytes, cudaMemcpyHostToDevice, s));
     if (col_host && v->col_bytes) CK(cudaMemcpyAsync(v->p.col, col_host, v->col_bytes, cudaMemcpyHostToDevice, s));
     if (geo_host && v->p.n_tiles > 0) {                       // unknown content: no tile or brick may be skipped
+        CK(cudaMemsetAsync(v->p.tile_sat, 0, (size_t)v->p.n_tiles, s));
         CK(cudaMemsetAsync(v->p.tile_neg, 1, (size_t)v->p.n_tiles, s));
         CK(cudaMemsetAsync(v->p.brick_neg, 1, (size_t)v->p.bricks_x * v->p.bricks_y * v->p.bricks_z, s));
     }
@@ -517,6 +534,7 @@ extern "C" int vol_reset(vol_t *v, void *stream)
     if (v->geo_bytes) CK(cudaMemsetAsync(v->p.geo, 0, v->geo_bytes, s));
     if (v->col_bytes) CK(cudaMemsetAsync(v->p.col, 0, v->col_bytes, s));
     if (v->p.n_tiles > 0) {
+        CK(cudaMemsetAsync(v->p.tile_sat, 0, (size_t)v->p.n_tiles, s));
         CK(cudaMemsetAsync(v->p.tile_neg, 0, (size_t)v->p.n_tiles, s));
         CK(cudaMemsetAsync(v->p.brick_neg, 0, (size_t)v->p.bricks_x * v->p.bricks_y * v->p.bricks_z, s));
     }
@@ -595,7 +613,22 @@ extern "C" int vol_shard_layers(int32_t nz, int32_t rank, int32_t world, int32_t
     return n;
 }
 
-extern "C" int vol_set_counting(vol_t *v, int32_t on) { if (!v) return VOL_E_ARG; v->counting = on != 0; return VOL_OK; }
+extern "C" int vol_set_counting(vol_t *v, int32_t on)
+{
+    if (!v) return VOL_E_ARG;
+    if (on && !v->p.sec_map[0]) {                              // the sector maps of the counting variant, on first use
+        int rc = set_device(v); if (rc) return rc;
+        for (int i = 0; i < 4; ++i) {
+            if (cudaMalloc(&v->p.sec_map[i], sec_map_bytes(v, i)) != cudaSuccess) {
+                cudaGetLastError();
+                for (int k = 0; k < 4; ++k) if (v->p.sec_map[k]) { cudaFree(v->p.sec_map[k]); v->p.sec_map[k] = nullptr; }
+                return VOL_E_OOM;
+            }
+        }
+    }
+    v->counting = on != 0;
+    return VOL_OK;
+}
 extern "C" int vol_set_profiling(vol_t *v, int32_t on) { if (!v) return VOL_E_ARG; v->profiling = on != 0; v->ev_valid = false; return VOL_OK; }
 extern "C" int vol_launches_per_frame(const vol_t *v) { return v ? 2 : VOL_E_ARG; }
 
@@ -620,6 +653,7 @@ extern "C" int vol_stats_decode(const vol_t *v, const void *raw_host, vol_stats_
         out->geo_sectors_read = cnt[vf::CNT_GEO_SEC_READ]; out->geo_sectors_written = cnt[vf::CNT_GEO_SEC_WRITTEN];
         out->col_sectors_read = cnt[vf::CNT_COL_SEC_READ]; out->col_sectors_written = cnt[vf::CNT_COL_SEC_WRITTEN];
         out->geo_visited = cnt[vf::CNT_GEO_VISITED]; out->col_gated = cnt[vf::CNT_COL_GATED];
+        out->geo_skippable = cnt[vf::CNT_GEO_SKIPPABLE]; out->geo_sectors_skippable = cnt[vf::CNT_GEO_SEC_SKIPPABLE];
         out->cells_col = st[vf::ST_CELLS]; out->subs_geo = st[vf::ST_SUBS];
     }
     out->tiles_total = (uint32_t)v->p.n_tiles;

@@ -344,10 +344,26 @@ def coord_rgb(wh: int, hh: int) -> np.ndarray:
     return np.stack([x % 256, y % 256, (x // 256) + 16 * (y // 256)], axis=-1).astype(np.uint8)
 
 
-def stress_frame(c: "Config", seed: int = 0):
-    """Saturating geometry frame for config ``c``: the camera is backed off along -x until the whole
-    cube is inside the depth frustum and sees a fronto-parallel wall behind the cube, so EVERY geometry voxel is updated
-    (free space); the wall is further than sigma behind the cube, so no colour voxel is.  Returns (depth, rgb, T_world_depth)."""
+STRESS_KINDS = ("free_space", "in_band", "colour")
+
+
+def stress_params(c: "Config", kind: str):
+    """(mu, sigma) a volume needs for the saturating frame of this kind: the configuration's own,
+    except mu = extent for "in_band" (the wall cuts the cube: every voxel lies inside the truncation band) and
+    sigma = extent for "colour" ("sigma raised to cover the cube": every colour voxel passes the gate)."""
+    assert kind in STRESS_KINDS
+    return (float(c.extent) if kind == "in_band" else c.mu), (float(c.extent) if kind == "colour" else c.sigma)
+
+
+def stress_frame(c: "Config", seed: int = 0, kind: str = "free_space"):
+    """Saturating frame for config ``c``.  The camera is backed off along -x until the whole cube is
+    inside the depth frustum and sees a fronto-parallel wall,
+      "free_space": behind the cube, further than sigma: EVERY geometry voxel is updated with tsdf = 1, no colour voxel is;
+      "in_band":    through the centre of the cube, for a volume with mu = extent (stress_params): every geometry voxel is
+                    updated with a tsdf strictly inside (-1, 1), i.e. through the general running average;
+      "colour":     the same wall for a volume with sigma = extent: every colour voxel passes the sigma gate as well.
+    The wall moves by 3 mm per ``seed`` so that repeated frames differ.  Returns (depth, rgb, T_world_depth)."""
+    assert kind in STRESS_KINDS
     ext = float(c.extent)
     centre = np.asarray(c.origin, np.float64) + ext / 2
     fx, fy = float(c.K_depth[0, 0]), float(c.K_depth[1, 1])
@@ -355,7 +371,7 @@ def stress_frame(c: "Config", seed: int = 0):
     tan_h, tan_v = (c.wd / 2 - 1.0) / fx, (c.hd / 2 - 1.0) / fy
     d = half + 1.05 * half / min(tan_h, tan_v)                 # distance camera -> cube centre
     T = look_at(centre + np.array([-d, 0.0, 0.0]), centre)
-    wall_mm = int(np.ceil(1000.0 * (d + half + 0.5)))
+    wall_mm = int(np.ceil(1000.0 * (d + half + 0.5 if kind == "free_space" else d))) + 3 * int(seed)
     assert wall_mm < 65535
     depth = np.full((c.hd, c.wd), wall_mm, dtype=np.uint16)
     return depth, random_rgb(c.wh, c.hh, 900 + seed), rigid32(T)

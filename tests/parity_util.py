@@ -22,12 +22,15 @@ def make_pair(c, **kw):
 
 
 def integrate_both(g, o, c, depth, rgb, T, counting=True):
-    """One frame on both sides; returns (gpu stats, oracle counters)."""
+    """One frame on both sides; returns (gpu stats, oracle counters -- with the four sector counters when counting)."""
     dd, dr = to_dev(depth), to_dev(rgb)
     g.set_counting(counting)
     g.integrate(dd, depth.shape[1], depth.shape[0], dr, rgb.shape[1], rgb.shape[0], T, c.K_depth, c.K_rgb, c.T_depth_rgb)
     st = g.frame_stats()
-    cnt = o.integrate(depth, rgb, T, c.K_depth, c.K_rgb, c.T_depth_rgb)
+    if counting:
+        cnt = o.integrate_sectors(depth, rgb, T, c.K_depth, c.K_rgb, c.T_depth_rgb)
+    else:
+        cnt = o.integrate(depth, rgb, T, c.K_depth, c.K_rgb, c.T_depth_rgb)
     return st, cnt
 
 
@@ -51,8 +54,11 @@ def compare_states(g, o, where=""):
 
 
 def check_counters(st, cnt, where=""):
-    got = [st.geo_read, st.geo_changed, st.col_read, st.col_changed]
+    """The four voxel counters of the frame -- and, when the oracle counted them, the four sector counters -- are the oracle's."""
+    got = [st.geo_read, st.geo_changed, st.col_read, st.col_changed,
+           st.geo_sectors_read, st.geo_sectors_written, st.col_sectors_read, st.col_sectors_written][:len(cnt)]
     assert got == [int(x) for x in cnt], f"{where}: counters {got} != oracle {list(cnt)}"
+    assert st.geo_visited >= st.geo_read and st.col_gated >= st.col_read
 
 
 def run_sequence(c, frames, counting=True, check_every=1, **kw):
@@ -67,11 +73,15 @@ def run_sequence(c, frames, counting=True, check_every=1, **kw):
     return g, o
 
 
-def sampled_full_size(c, frames, n_cols, seed, alternate_host=False, variant=0):
+def sampled_full_size(c, frames, n_cols, seed, alternate_host=False, variant=0, frame_fn=None, mu=None, sigma=None, expect_colour=True):
     """Full-size volumes in the launch configuration bench.py times (device-resident frames, counters off), compared on a
     seeded sample: every voxel of n_cols random 8 x 8 (x, y) geometry columns and all their colour children.  Voxels never
-    interact, so the oracle run on the sample alone gives their exact state (ref_integrate_subset)."""
+    interact, so the oracle run on the sample alone gives their exact state (ref_integrate_subset).
+    frame_fn(c, i) supplies frame i (default: the configuration's scan); mu / sigma override the configuration's."""
     import paper_1602_06645_b200 as vf
+    frame_fn = frame_fn or synth.frame
+    mu = c.mu if mu is None else mu
+    sigma = c.sigma if sigma is None else sigma
     nx, ny, nz = c.dims_geo
     r = c.r
     rng = np.random.default_rng(seed)
@@ -85,11 +95,11 @@ def sampled_full_size(c, frames, n_cols, seed, alternate_host=False, variant=0):
     ic = (bx[None, :, None, None] * 8 * r + np.arange(8 * r)[None, None, None, :]).astype(np.int64)
     col_idx = np.unique(((kc * (ny * r) + jc) * (nx * r) + ic).reshape(-1))
     gw, cw = np.zeros(geo_idx.size, np.uint32), np.zeros(col_idx.size, np.uint32)
-    o = oracle.RefVolume(c.dims_geo, r, c.origin, c.extent, c.mu, c.w_max, allocate=False, variant=variant)
-    g = vf.Volume(c.dims_geo, r, c.origin, c.extent, c.mu, c.w_max, variant=variant)
+    o = oracle.RefVolume(c.dims_geo, r, c.origin, c.extent, mu, c.w_max, sigma=sigma, allocate=False, variant=variant)
+    g = vf.Volume(c.dims_geo, r, c.origin, c.extent, mu, c.w_max, sigma=sigma, variant=variant)
     try:
         for n, fi in enumerate(frames):
-            depth, rgb, T = synth.frame(c, fi)
+            depth, rgb, T = frame_fn(c, fi)
             if alternate_host and n % 2:                          # every other frame through vol_integrate_host
                 g.integrate_host(depth, rgb, T, c.K_depth, c.K_rgb, c.T_depth_rgb)
             else:
@@ -101,7 +111,7 @@ def sampled_full_size(c, frames, n_cols, seed, alternate_host=False, variant=0):
         ggw, gcw = g.download_voxels(geo_idx, col_idx)
     finally:
         g.close()
-    assert (gw >> 16).max() == min(len(frames), c.w_max) and (cw >> 24).max() > 0   # the sample does see the surface
+    assert (gw >> 16).max() == min(len(frames), c.w_max) and ((cw >> 24).max() > 0) == expect_colour   # the sample does see the surface
     assert int((ggw != gw).sum()) == 0, f"{c.name}: {int((ggw != gw).sum())} geometry words differ on the sample"
     assert int((gcw != cw).sum()) == 0, f"{c.name}: {int((gcw != cw).sum())} colour words differ on the sample"
     return int((gw != 0).sum()), int((cw != 0).sum())

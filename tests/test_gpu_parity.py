@@ -27,6 +27,16 @@ def test_ragged_dims_and_tail_tiles():
     run_sequence(c, [0, 1, 3])
 
 
+def test_odd_x_dimension():
+    """dims_geo[0] that is not a multiple of 4 or 8: rows are not aligned to 32-byte sectors (SURVEY 8(b) has no such rule)."""
+    c = synth.config(1).scaled(40, 2)
+    c.dims_geo = (45, 39, 29)
+    run_sequence(c, [0, 2, 4])
+    c = synth.config(2).scaled(64, 3)
+    c.dims_geo = (61, 66, 50)
+    run_sequence(c, [0, 50])
+
+
 def test_cfg2_scaled_orbit():
     """Config 2's scene, cameras, noise and 2 % dropouts on a 96^3 / 192^3 grid; 6 frames spread over the orbit."""
     run_sequence(synth.config(2).scaled(96, 2), [0, 17, 34, 51, 68, 99])
@@ -55,6 +65,26 @@ def test_weight_saturation_and_gate_many_frames():
         st, cnt = integrate_both(g, o, c, depth, rgb, T)
         check_counters(st, cnt, f"repeat {n}")
     compare_states(g, o, "saturation")
+
+
+def test_saturated_free_space_is_left_out_exactly():
+    """Steady state of a long scan: sub-boxes that hold nothing but saturated free space (tsdf_q = 32767, w = w_max) and
+    stay in free space are not visited by the plain kernel.  w_max = 3 so that it happens within a few frames; frames of a
+    moving camera, counters off (the launch configuration of bench.py), every word compared with the oracle after every
+    frame; then one counted frame: the counters are still the method's, and they say how much was left out."""
+    c = synth.config(2).scaled(96, 2)
+    c.w_max = 3
+    g, o = make_pair(c)
+    for n, fi in enumerate([0, 0, 0, 0, 1, 2, 3, 4, 5, 6, 30, 31]):
+        depth, rgb, T = synth.frame(c, fi)
+        integrate_both(g, o, c, depth, rgb, T, counting=False)
+        compare_states(g, o, f"frame {fi} (#{n})")
+    depth, rgb, T = synth.frame(c, 32)
+    st, cnt = integrate_both(g, o, c, depth, rgb, T, counting=True)
+    check_counters(st, cnt, "counted frame")
+    compare_states(g, o, "after the counted frame")
+    assert 5000 < st.geo_skippable < st.geo_read, (st.geo_skippable, st.geo_read)    # a part of the free space is left out by now
+    assert st.geo_changed <= st.geo_read - st.geo_skippable and 0 < st.geo_sectors_skippable <= st.geo_sectors_read
 
 
 def test_degenerate_frames():
@@ -210,9 +240,47 @@ def test_cfg2_cfg4_cfg5_full_size_whole_sequences_sampled():
 
 
 def test_cfg4_r4_full_size_sampled():
-    """The largest configuration: 384^3 geometry, 1536^3 colour (14.5 GB, word offsets beyond 2^32 bytes), 2 frames."""
-    ng, nc = _sampled_full_size(synth.config(4, r=4), [0, 100], 32, 41)
-    assert ng > 10000 and nc > 1000
+    """The largest configuration: 384^3 geometry, 1536^3 colour (14.5 GB, word offsets beyond 2^32 bytes), 24 frames spread
+    over the orbit, device and host entry points alternating."""
+    ng, nc = _sampled_full_size(synth.config(4, r=4), list(range(0, 200, 9)) + [199, 199], 32, 41, alternate_host=True)
+    assert ng > 50000 and nc > 50000
+
+
+@pytest.mark.parametrize("kind", synth.STRESS_KINDS)
+def test_stress_frames_full_size_sampled(kind):
+    """The saturating frames bench.py times on the benchmark volumes, 512^3 / 1024^3, in bench.py's
+    launch configuration: the wall behind the cube (every geometry voxel updated in free space), the wall through the cube
+    with mu = extent (every geometry voxel through the general running average) and the same with sigma = extent (every
+    colour voxel updated as well).  Six frames each -- the wall moves, the RGB image is random, weights grow and the 0.8 gate
+    starts to act -- against the oracle on a seeded sample of columns."""
+    c = synth.config(3)
+    mu, sigma = synth.stress_params(c, kind)
+    ng, nc = _sampled_full_size(c, range(6), 24, 77, frame_fn=lambda cc, i: synth.stress_frame(cc, i, kind), mu=mu, sigma=sigma,
+                                expect_colour=kind == "colour")
+    col = 64 * 512                                               # voxels of one sampled 8 x 8 column
+    if kind == "colour":
+        assert 8 * col <= ng <= 16 * col                         # (mu is the configuration's: the voxels behind the wall's band are not)
+    else:
+        assert ng >= 20 * col and ng % col == 0                  # every geometry voxel of the sample was updated
+    assert (nc >= 20 * col * 8 * 0.99) if kind == "colour" else nc == 0
+
+
+def test_stress_frames_every_voxel_small():
+    """The same three frames on a 64^3 / 128^3 grid, every voxel and the counters: a saturating frame reads every voxel."""
+    import paper_1602_06645_b200 as vf
+    import oracle
+    c = synth.config(3).scaled(64, 2)
+    for kind in synth.STRESS_KINDS:
+        mu, sigma = synth.stress_params(c, kind)
+        g = vf.Volume(c.dims_geo, c.r, c.origin, c.extent, mu, c.w_max, sigma=sigma)
+        o = oracle.RefVolume(c.dims_geo, c.r, c.origin, c.extent, mu, c.w_max, sigma=sigma)
+        for i in range(3):
+            depth, rgb, T = synth.stress_frame(c, i, kind)
+            st, cnt = integrate_both(g, o, c, depth, rgb, T)
+            check_counters(st, cnt, f"{kind} frame {i}")
+            assert (st.geo_read == 64 ** 3) == (kind != "colour") and (st.col_read > 0.9 * 128 ** 3) == (kind == "colour"), (kind, st.geo_read, st.col_read)
+        compare_states(g, o, kind)
+        g.close()
 
 
 def test_cfg2_full_size_every_voxel():

@@ -80,13 +80,18 @@ def test_raycast_rejects_bad_arguments():
 
 
 def test_raycast_cfg3_full_size():
-    """BASELINE config 3 at full size (512^3 / 1024^3): two frames fused on both sides (the oracle over the whole volumes),
-    then a 640 x 480 ray cast from a third pose of the trajectory compared bit for bit."""
+    """BASELINE config 3 at full size (512^3 / 1024^3): two frames fused on both sides, the oracle over the WHOLE volumes --
+    every one of the 1.2 G words and the eight per-frame counters (voxels and 32-byte sectors read / changed) are compared
+    (the every-voxel comparison at the headline size) -- then a 640 x 480 ray cast from a third pose of the
+    trajectory compared bit for bit."""
+    from parity_util import check_counters, compare_states
     c = synth.config(3)
     g, o = make_pair(c)
     for fi in (0, 6):
         depth, rgb, T = synth.frame(c, fi)
-        integrate_both(g, o, c, depth, rgb, T, counting=False)
+        st, cnt = integrate_both(g, o, c, depth, rgb, T, counting=True)
+        check_counters(st, cnt, f"cfg3 full size, frame {fi}")
+    compare_states(g, o, "cfg3 full size, every voxel")
     d, rgb = cast_both(g, o, c.wd, c.hd, synth.frame(c, 3)[2], c.K_depth, 0.3, 5.0)
     assert (d > 0).mean() > 0.5 and (rgb.sum(axis=2) > 0).mean() > 0.3
     g.close()
