@@ -48,8 +48,12 @@ def parse():
     ap.add_argument("--first-frame", type=int, default=0)
     ap.add_argument("--variant", type=int, default=0, choices=[0, 1, 2, 4],
                     help="alternative reading of the method (vol_opts_t.variant; both arms); 0 = the headline path")
-    ap.add_argument("--stress", action="store_true",
-                    help="second workload: the saturating frame of SURVEY 8(d) item 5 (every geometry voxel updated) instead of the scan")
+    ap.add_argument("--stress", default=None, choices=list(synth.STRESS_KINDS),
+                    help="time ONE saturating frame kind of SURVEY 8(d) item 5 as the main workload instead of the scan "
+                         "(the default run reports all three under \"stress\")")
+    ap.add_argument("--no-stress", action="store_true", help="skip the three saturating frames")
+    ap.add_argument("--steady-frames", type=int, default=150,
+                    help="frames swept back and forth over the arc before the steady-state window (0 = skip it)")
     return ap.parse_args()
 
 
@@ -61,32 +65,45 @@ def peaks():
         return 6650.0, "fallback (B200_PROFILING.md)"
 
 
-def ncu_traffic(workload, column=2):
-    """Per k_fused launch, from the committed ncu --set full capture of this workload (profiles/traffic.csv:
-    workload,kernel,dram_bytes_per_launch,warp_instructions_per_launch): DRAM bytes (column 2) or warp instructions
-    (column 3); None if none is recorded."""
+def kernel_source_hash():
+    """sha256 (first 16 hex digits) over the CUDA sources of the library: ncu figures recorded for another build are not quoted."""
+    import hashlib
+    h = hashlib.sha256()
+    d = os.path.join(ROOT, "paper_1602_06645_b200", "csrc")
+    for name in sorted(os.listdir(d)):
+        with open(os.path.join(d, name), "rb") as f:
+            h.update(name.encode() + b"\0" + f.read())
+    return h.hexdigest()[:16]
+
+
+def ncu_record(workload):
+    """The committed ncu --set full figures of k_fused for this workload (profiles/traffic.csv:
+    workload,kernel,dram_bytes_per_launch,warp_instructions_per_launch,source_hash) -- only if they were captured with the
+    kernel sources this run was built from (source_hash = kernel_source_hash()); None otherwise, so that a stale capture is
+    never quoted beside a live timing."""
     try:
+        want = kernel_source_hash()
         with open(os.path.join(ROOT, "profiles", "traffic.csv")) as f:
             for line in f:
                 cols = [c.strip() for c in line.split(",")]
-                if len(cols) > column and cols[0] == workload and cols[1] == "k_fused":
-                    return float(cols[column])
+                if len(cols) >= 5 and cols[0] == workload and cols[1] == "k_fused" and cols[4] == want:
+                    return {"dram_bytes": float(cols[2]), "warp_instructions": float(cols[3])}
     except Exception:
         pass
     return None
 
 
-def issue_roofline(workload, fused_ms_mean, sm_mhz):
+def issue_roofline(rec, fused_ms_mean, sm_mhz, n_sms):
     """The bound the fused kernel actually runs into: warp instructions issued per second against
-    148 SMs x 4 schedulers x 1 instruction per cycle at the SM clock seen during the run.  The instruction count per
-    launch comes from the committed ncu capture (it cannot be measured outside a profiler)."""
-    inst = ncu_traffic(workload, 3)
-    if inst is None or not sm_mhz:
+    SMs x 4 schedulers x 1 instruction per cycle at the SM clock seen during the run.  The instruction count per launch comes
+    from the committed ncu capture of the same build (it cannot be measured outside a profiler)."""
+    if rec is None or not sm_mhz:
         return None
-    peak = 148 * 4 * sm_mhz * 1e6
-    achieved = inst / (fused_ms_mean * 1e-3)
+    peak = n_sms * 4 * sm_mhz * 1e6
+    achieved = rec["warp_instructions"] / (fused_ms_mean * 1e-3)
     return {"bound": "alu", "achieved": achieved / 1e12, "peak": peak / 1e12, "unit": "T warp-instructions/s", "frac": achieved / peak,
-            "warp_instructions_per_launch": inst, "source": "profiles/traffic.csv (ncu smsp__inst_executed.sum)"}
+            "warp_instructions_per_launch": rec["warp_instructions"], "sms": n_sms,
+            "source": "profiles/traffic.csv (ncu smsp__inst_executed.sum, same kernel sources)"}
 
 
 class ClockSampler(threading.Thread):
@@ -194,7 +211,8 @@ def run_reference(args, rank):
         return
     c = synth.config(args.cfg, r=args.r)
     c.variant = args.variant
-    cores = os.cpu_count() or 1
+    import oracle
+    cores = oracle.threads()
     slab = max(8, c.dims_geo[2] // 16)
     nvox, times, sample = oracle_sample(c, args.warmup + args.steps, slab_layers=slab)
     t = times[args.warmup:]
@@ -226,6 +244,94 @@ def whole_job_value(nvox_per_rank, steps, world, total_ms):
     return world * nvox_per_rank * steps / (total_ms * 1e-3)
 
 
+STAT_KEYS = ("geo_read", "geo_changed", "col_read", "col_changed", "geo_sectors_read", "geo_sectors_written", "col_sectors_read",
+             "col_sectors_written", "geo_visited", "col_gated", "geo_skippable", "geo_sectors_skippable", "tiles_geo", "subs_geo",
+             "items_col", "cells_col", "jobs_mark")
+NOMINAL_HBM_GBS = 8000.0          # BASELINE.json: "B200's ~8 TB/s peak"
+
+
+def stats_row(s):
+    return [float(getattr(s, k)) for k in STAT_KEYS]
+
+
+def bytes_of(cnt, frame_bytes):
+    """Algorithmic bytes per fused launch from a (frames x STAT_KEYS) array: voxel-exact
+    4 (geo_read + geo_changed + col_read + col_changed) + the two images, the same at 32-byte sector granularity, and what
+    the plain kernel really has to touch (without the saturated free space it leaves out)."""
+    k = {n: cnt[:, i] for i, n in enumerate(STAT_KEYS)}
+    voxel = 4.0 * (k["geo_read"] + k["geo_changed"] + k["col_read"] + k["col_changed"]) + frame_bytes
+    sector = 32.0 * (k["geo_sectors_read"] + k["geo_sectors_written"] + k["col_sectors_read"] + k["col_sectors_written"]) + frame_bytes
+    touched = voxel - 4.0 * k["geo_skippable"]
+    touched_sector = sector - 32.0 * k["geo_sectors_skippable"]
+    return voxel, sector, touched, touched_sector
+
+
+class Window:
+    """Counts, per-kernel times and the timed pass of one list of frames on one volume."""
+
+    def __init__(self, vol, frames, c, stream, flush_buf, flush):
+        self.vol, self.frames, self.c, self.stream, self.flush_buf, self.flush = vol, frames, c, stream, flush_buf, flush
+
+    def integrate(self, fr):
+        _, _, dd, dr, T = fr
+        c = self.c
+        self.vol.integrate(dd, c.wd, c.hd, dr, c.wh, c.hh, T, c.K_depth, c.K_rgb, c.T_depth_rgb, stream=self.stream)
+
+    def count(self):
+        """(untimed) per-frame counters of exactly these frames, from the counting variant"""
+        self.vol.set_counting(True)
+        rows = []
+        for fr in self.frames:
+            self.integrate(fr)
+            rows.append(stats_row(self.vol.frame_stats(self.stream)))
+        self.vol.set_counting(False)
+        return np.array(rows, dtype=np.float64)
+
+    def kernel_times(self):
+        """(untimed) per-kernel times (library-side CUDA events on the launching stream)"""
+        self.vol.set_profiling(True)
+        kms = []
+        for fr in self.frames:
+            if self.flush:
+                self.flush_buf.zero_()
+            self.integrate(fr)
+            kms.append(self.vol.last_kernel_ms())
+        self.vol.set_profiling(False)
+        return np.array(kms)
+
+    def timed(self, torch, barrier, nvml=None):
+        """THE timed pass: events around every frame, L2 flushed between frames"""
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in self.frames]
+        barrier()
+        for n, fr in enumerate(self.frames):
+            if self.flush:
+                self.flush_buf.zero_()
+            ev[n][0].record(self.stream)
+            self.integrate(fr)
+            ev[n][1].record(self.stream)
+            if nvml and n % 4 == 3:
+                nvml.sample()                                     # the device is busy with the frames enqueued so far
+        while nvml and not ev[-1][1].query():
+            nvml.sample()
+        barrier()
+        return np.array([a.elapsed_time(b) for a, b in ev])
+
+
+def roofline_block(alg_voxel, alg_sector, touched, touched_sector, fused_ms, step_ms, peak):
+    """Fractions of the HBM roofline of one window: algorithmic bytes over the fused kernel's time (and over the whole step)."""
+    t_f, t_s = fused_ms.sum() * 1e-3, step_ms.sum() * 1e-3
+    gbs = lambda b, t: float(b.sum() / t / 1e9)
+    out = {"achieved": gbs(alg_voxel, t_f), "frac": gbs(alg_voxel, t_f) / peak, "frac_of_nominal_8tbs": gbs(alg_voxel, t_f) / NOMINAL_HBM_GBS,
+           "step_frac": gbs(alg_voxel, t_s) / peak,
+           "sector_exact": {"bytes": float(alg_sector.mean()), "achieved": gbs(alg_sector, t_f), "frac": gbs(alg_sector, t_f) / peak}}
+    if float((alg_voxel - touched).sum()) > 0.0:
+        out["touched"] = {"bytes": float(touched.mean()), "sector_bytes": float(touched_sector.mean()),
+                          "frac": gbs(touched, t_f) / peak, "sector_frac": gbs(touched_sector, t_f) / peak,
+                          "note": "without the saturated free space the plain kernel leaves out (read and unchanged by definition): "
+                                  "the bytes it really has to move"}
+    return out
+
+
 def run_ours(args, rank, world, local_rank):
     import torch
     import torch.distributed as dist
@@ -245,77 +351,74 @@ def run_ours(args, rank, world, local_rank):
     sampler = ClockSampler(local_rank) if rank == 0 else None
     if sampler:
         sampler.start()
-
-    # ---- inputs: generated once, pinned on the host and resident on the device
-    frames = []
-    for i in range(nfr):
-        depth, rgb, T = synth.stress_frame(c, i) if args.stress else synth.frame(c, (first + i) % c.n_frames)
-        hd_, hr_ = torch.from_numpy(depth.view(np.int16)).pin_memory(), torch.from_numpy(rgb).pin_memory()
-        frames.append((hd_, hr_, hd_.cuda(), hr_.cuda(), T))
-    vol = vf.Volume(c.dims_geo, c.r, c.origin, c.extent, c.mu, c.w_max, sigma=c.sigma, gate=c.gate, device=local_rank,
-                    variant=getattr(c, "variant", 0))
+    n_sms = torch.cuda.get_device_properties(local_rank).multi_processor_count
+    peak, peak_src = peaks()
+    frame_bytes = c.wd * c.hd * 2 + c.wh * c.hh * 3
     stream = torch.cuda.current_stream()
     flush_buf = torch.empty(512 << 20, dtype=torch.uint8, device="cuda")      # > 126 MB L2
-
-    def integrate_dev(i):
-        _, _, dd, dr, T = frames[i]
-        vol.integrate(dd, c.wd, c.hd, dr, c.wh, c.hh, T, c.K_depth, c.K_rgb, c.T_depth_rgb, stream=stream)
 
     def barrier():
         if world > 1:
             dist.barrier()
         torch.cuda.synchronize()
 
-    # ---- pass 1 (untimed): per-frame voxel counters of exactly this frame sequence -> algorithmic bytes
-    vol.set_counting(True)
-    counters = []
-    for i in range(nfr):
-        integrate_dev(i)
-        s = vol.frame_stats(stream)
-        counters.append((s.geo_read, s.geo_changed, s.col_read, s.col_changed, s.tiles_geo, s.items_col, s.cells_col))
-    vol.set_counting(False)
+    def upload(fr):
+        depth, rgb, T = fr
+        hd_, hr_ = torch.from_numpy(depth.view(np.int16)).pin_memory(), torch.from_numpy(rgb).pin_memory()
+        return (hd_, hr_, hd_.cuda(), hr_.cuda(), T)
 
-    # ---- pass 2 (untimed): per-kernel times of the timed frames (library-side CUDA events on the launching stream)
-    vol.reset(stream)
-    for i in range(W):
-        integrate_dev(i)
-    vol.set_profiling(True)
-    kms = []
-    for i in range(W, nfr):
-        if not args.no_flush:
-            flush_buf.zero_()
-        integrate_dev(i)
-        kms.append(vol.last_kernel_ms())
-    vol.set_profiling(False)
-    kms = np.array(kms)
+    # ---- inputs: generated once, pinned on the host and resident on the device
+    stress_kind = args.stress if args.stress in synth.STRESS_KINDS else None
+    mu, sigma = synth.stress_params(c, stress_kind) if stress_kind else (c.mu, c.sigma)
+    frames = [upload(synth.stress_frame(c, i, stress_kind) if stress_kind else synth.frame(c, (first + i) % c.n_frames)) for i in range(nfr)]
+    vol = vf.Volume(c.dims_geo, c.r, c.origin, c.extent, mu, c.w_max, sigma=sigma, gate=c.gate, device=local_rank,
+                    variant=getattr(c, "variant", 0))
+    warm, timed = frames[:W], frames[W:]
+    win = Window(vol, timed, c, stream, flush_buf, not args.no_flush)
 
+    def warm_up():
+        vol.reset(stream)
+        for fr in warm:
+            win.integrate(fr)
+
+    # ---- pass 1 (untimed): per-frame voxel and sector counters of exactly the timed frames -> algorithmic bytes
+    warm_up()
+    cnt = win.count()
+    # ---- pass 2 (untimed): per-kernel times of the timed frames
+    warm_up()
+    kms = win.kernel_times()
     # ---- pass 3: THE timed region -- K frames, device-resident inputs, events around every frame, L2 flushed between
-    vol.reset(stream)
-    for i in range(W):
-        integrate_dev(i)
-    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(K)]
+    warm_up()
     nvml = NvmlClocks(local_rank) if rank == 0 else None
-    barrier()
-    for n, i in enumerate(range(W, nfr)):
-        if not args.no_flush:
-            flush_buf.zero_()
-        ev[n][0].record(stream)
-        integrate_dev(i)
-        ev[n][1].record(stream)
-        if nvml and n % 4 == 3:
-            nvml.sample()                                         # the device is busy with the frames enqueued so far
-    while nvml and not ev[K - 1][1].query():
-        nvml.sample()
-    barrier()
-    per_frame_ms = np.array([a.elapsed_time(b) for a, b in ev])
+    per_frame_ms = win.timed(torch, barrier, nvml)
     total_ms = float(per_frame_ms.sum())
+
+    # ---- steady state of a long scan (same volume): the arc is swept back and forth until the weights are saturated
+    #      (w = w_max wherever the arc sees free space or the surface, the 0.8 gate mostly closed), then the same frames
+    #      are counted, profiled and timed again
+    steady = None
+    if args.steady_frames > 0 and not stress_kind:
+        order = list(range(nfr)) + list(range(nfr - 2, 0, -1))
+        for n in range(args.steady_frames):
+            win.integrate(frames[order[n % len(order)]])
+        s_cnt = win.count()
+        s_kms = win.kernel_times()
+        s_ms = win.timed(torch, barrier)
+        av, asec, tch, tchs = bytes_of(s_cnt, frame_bytes)
+        steady = {"frames_before": nfr * 3 + args.steady_frames + 2 * K, "ms_per_step": float(s_ms.mean()),
+                  "kernel_ms_mean": {"prepass": float(s_kms[:, 0].mean()), "fused": float(s_kms[:, 2].mean())},
+                  "per_frame_mean": {k: float(s_cnt[:, i].mean()) for i, k in enumerate(STAT_KEYS)},
+                  "algorithmic_bytes": float(av.mean()),
+                  "roofline": roofline_block(av, asec, tch, tchs, s_kms[:, 2], s_ms, peak),
+                  "note": "the timed frames again after the arc has been swept back and forth: geometry weights saturated at w_max, "
+                          "colour gate mostly closed (col_changed << col_read), stores skipped where the word does not change"}
 
     # ---- pass 4: end to end through vol_integrate_host -- pinned host frames in, per-frame stats out, every step.
     #      Frames are enqueued back to back, as when a recorded sequence is fused: the library copies frame n + 1 while the
-    #      kernels of frame n run (two staging sets), and the step's result (the 64-byte statistics record) comes back with
+    #      kernels of frame n run (two staging sets), and the step's result (the 128-byte statistics record) comes back with
     #      vol_frame_stats_async into pinned memory, in stream order.
     vol.reset(stream)
-    raw_stats = torch.zeros((max(K, W), 16), dtype=torch.int64).pin_memory()
+    raw_stats = torch.zeros((max(K, W), vf.VOL_STATS_RAW_BYTES // 8), dtype=torch.int64).pin_memory()
     for i in range(W):                                            # warm-up through the same entry point (staging buffers exist)
         hd_, hr_, _, _, T = frames[i]
         vol.integrate_host(hd_, hr_, T, c.K_depth, c.K_rgb, c.T_depth_rgb, stream=stream)
@@ -331,7 +434,7 @@ def run_ours(args, rank, world, local_rank):
     barrier()
     e2e_ms = float(t0.elapsed_time(t1))
     e2e_tiles = [vol.decode_stats(raw_stats[n]).tiles_geo for n in range(K)]
-    assert min(e2e_tiles) > 0 or args.stress, "a frame of the end-to-end pass visited no tile"
+    assert min(e2e_tiles) > 0, "a frame of the end-to-end pass visited no tile"
 
     # ---- pass 4b: the same, one frame at a time (a live scan: the caller waits for every frame's result before the next)
     vol.reset(stream)
@@ -349,6 +452,33 @@ def run_ours(args, rank, world, local_rank):
     t3.record(stream)
     barrier()
     e2e_serial_ms = float(t2.elapsed_time(t3))
+
+    # ---- the saturating frames of SURVEY 8(d) item 5, on volumes of the same size (each kind with the mu / sigma it needs):
+    #      counted, profiled and timed like the scan, a few frames each.  Parity: tests/test_gpu_parity.py::test_stress_*.
+    stress = None
+    if world == 1 and not stress_kind and not args.no_stress:
+        stress = {}
+        for kind in synth.STRESS_KINDS:
+            s_mu, s_sigma = synth.stress_params(c, kind)
+            nw_, nt_ = (1, 2) if kind == "colour" else (2, 4)
+            sfr = [upload(synth.stress_frame(c, i, kind)) for i in range(nw_ + nt_)]
+            svol = vf.Volume(c.dims_geo, c.r, c.origin, c.extent, s_mu, c.w_max, sigma=s_sigma, gate=c.gate, device=local_rank)
+            swin = Window(svol, sfr[nw_:], c, stream, flush_buf, not args.no_flush)
+            res = []
+            for what in ("count", "kernel_times", "timed"):
+                svol.reset(stream)
+                for fr in sfr[:nw_]:
+                    swin.integrate(fr)
+                res.append(swin.count() if what == "count" else swin.kernel_times() if what == "kernel_times" else swin.timed(torch, barrier))
+            s_cnt, s_kms, s_ms = res
+            av, asec, tch, tchs = bytes_of(s_cnt, frame_bytes)
+            stress[kind] = {"frames": nt_, "ms_per_step": float(s_ms.mean()), "fused_ms": float(s_kms[:, 2].mean()),
+                            "mu_m": s_mu, "sigma_m": s_sigma, "algorithmic_bytes": float(av.mean()),
+                            "geo_read": float(s_cnt[:, 0].mean()), "col_read": float(s_cnt[:, 2].mean()),
+                            "roofline": roofline_block(av, asec, tch, tchs, s_kms[:, 2], s_ms, peak)}
+            svol.close()
+            del svol, sfr
+            torch.cuda.empty_cache()
 
     # ---- NEXT row, outside the timed regions: vol_raycast of the volumes as they stand now, from the
     #      last frame's pose, one 640 x 480 (depth-camera sized) image per call
@@ -369,7 +499,7 @@ def run_ours(args, rank, world, local_rank):
     # ---- NEXT row: the tracker -- front end of the last frame, prediction ray-cast from the pose before
     #      it, coarse-to-fine ICP (19 steps, each a kernel and a 232-byte read-back); the tracked pose against the true one
     tracking = None
-    if not args.stress and nfr >= 2:
+    if not stress_kind and nfr >= 2:
         fe = vf.Frontend(c.wd, c.hd, 3, device=local_rank)
         T_prev, dd_last = np.asarray(frames[nfr - 2][4], np.float32), frames[nfr - 1][2]
         tms = {"measure": [], "predict": [], "track": []}
@@ -440,36 +570,43 @@ def run_ours(args, rank, world, local_rank):
     ms_per_step = total_ms / K
     value = whole_job_value(nvox, K, world, total_ms)
     e2e_value = whole_job_value(nvox, K, world, e2e_ms)
-    cnt = np.array(counters[W:], dtype=np.float64)
-    frame_bytes = c.wd * c.hd * 2 + c.wh * c.hh * 3
-    alg_bytes = 4.0 * cnt[:, :4].sum(axis=1) + frame_bytes        # per fused launch
     fused_ms = kms[:, 2]
-    peak, peak_src = peaks()
-    achieved = float(alg_bytes.sum() / (fused_ms.sum() * 1e-3) / 1e9)
-    # profiles/traffic.csv holds captures of the headline path only: other readings report traffic = null
-    traffic_key = c.name + ("-stress" if args.stress else "") + (f"-variant{args.variant}" if args.variant else "")
+    av, asec, tch, tchs = bytes_of(cnt, frame_bytes)
+    wl_key = c.name + (f"-stress-{stress_kind}" if stress_kind else "") + (f"-variant{args.variant}" if args.variant else "")
+    rec = ncu_record(wl_key)
+    roof = {"bound": "hbm", "kernel": "k_fused", "peak": peak, "unit": "GB/s", "peak_source": peak_src}
+    roof.update(roofline_block(av, asec, tch, tchs, fused_ms, per_frame_ms, peak))
+    roof.update({"traffic": rec["dram_bytes"] if rec else None,
+                 "traffic_source": "profiles/traffic.csv: ncu dram__bytes_read.sum + dram__bytes_write.sum per k_fused launch, captured with "
+                                   "these kernel sources (hash " + kernel_source_hash() + ")" if rec else
+                                   "null: no ncu capture of these kernel sources is committed (hash " + kernel_source_hash() + ")",
+                 "dense_sweep_frac": float(8.0 * nvox / (fused_ms.mean() * 1e-3) / 1e9 / peak),
+                 "issue": issue_roofline(rec, float(fused_ms.mean()), (clocks or {}).get("sm_mhz"), n_sms)})
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
         "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f32", "data": "synthetic",
-        "config": {"workload": workload_name(c) + (" -- STRESS: saturating frame, every geometry voxel updated" if args.stress else ""),
-                   "frames": "one saturating pose, repeated" if args.stress else f"{first}..{first + nfr - 1} of the seeded trajectory",
+        "config": {"workload": workload_name(c) + (f" -- STRESS: saturating frame ({stress_kind})" if stress_kind else ""),
+                   "value_kind": "visited: (N_geo + N_col) voxels brought up to date per frame x frames / device time -- about 1 % of them "
+                                 "are touched (applied_updates_per_s counts those); the reference arm uses the same convention",
+                   "frames": "one saturating pose, the wall moving" if stress_kind else f"{first}..{first + nfr - 1} of the seeded trajectory",
                    "l2": "no flush (frames back to back)" if args.no_flush else "L2 flushed (512 MiB memset) between timed frames",
                    "parallelism": "single GPU" if world == 1 else f"{world} replicas (independent scans), no data-path collective"},
         "frames_per_s": world * K / (total_ms * 1e-3),
         "applied_updates_per_s": world * float(cnt[:, 0].sum() + cnt[:, 2].sum()) / (total_ms * 1e-3),
         "per_frame_ms": {"median": float(np.median(per_frame_ms)), "p95": float(np.percentile(per_frame_ms, 95)), "min": float(per_frame_ms.min())},
-        "kernel_ms_mean": {"prepass": float(kms[:, 0].mean()), "classify": float(kms[:, 1].mean()), "fused": float(fused_ms.mean())},
-        "per_frame_mean": {"geo_read": float(cnt[:, 0].mean()), "geo_changed": float(cnt[:, 1].mean()), "col_read": float(cnt[:, 2].mean()),
-                           "col_changed": float(cnt[:, 3].mean()), "tiles_geo": float(cnt[:, 4].mean()), "items_col": float(cnt[:, 5].mean()),
-                           "cells_col": float(cnt[:, 6].mean()), "algorithmic_bytes": float(alg_bytes.mean())},
-        "roofline": {"bound": "hbm", "kernel": "k_fused", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                     "traffic": ncu_traffic(traffic_key), "peak_source": peak_src,
-                     "dense_sweep_frac": float(8.0 * nvox / (fused_ms.mean() * 1e-3) / 1e9 / peak),
-                     "issue": issue_roofline(traffic_key, float(fused_ms.mean()),
-                                             (clocks or {}).get("sm_mhz"))},
+        "kernel_ms_mean": {"prepass": float(kms[:, 0].mean()), "fused": float(fused_ms.mean())},
+        "per_frame_mean": dict({k: float(cnt[:, i].mean()) for i, k in enumerate(STAT_KEYS)}, algorithmic_bytes=float(av.mean()),
+                               sector_exact_bytes=float(asec.mean())),
+        "instructions_hint": None if rec is None else {
+            "warp_instructions_per_launch": rec["warp_instructions"],
+            "thread_instructions_per_visited_voxel": 32.0 * rec["warp_instructions"] / float(cnt[:, 8].mean() + cnt[:, 9].mean()),
+            "note": "ncu smsp__inst_executed.sum x 32 / (geometry voxels projected + colour voxels gated); all roles of the kernel included"},
+        "roofline": roof,
+        "steady_state": steady,
+        "stress": stress,
         "e2e": {"value": e2e_value, "unit": UNIT, "ms_per_step": e2e_ms / K, "h2d_bytes_per_step": frame_bytes,
-                "d2h_bytes_per_step": 128,
+                "d2h_bytes_per_step": vf.VOL_STATS_RAW_BYTES,
                 "mode": "vol_integrate_host + vol_frame_stats_async per frame, frames enqueued back to back (a recorded "
                         "sequence): the copies of frame n + 1 overlap the kernels of frame n",
                 "one_frame_at_a_time": {"value": whole_job_value(nvox, K, world, e2e_serial_ms), "ms_per_step": e2e_serial_ms / K,
@@ -485,11 +622,23 @@ def run_ours(args, rank, world, local_rank):
         "clocks": clocks,
     }
     if world == 1 and not args.no_cpu_baseline:
+        import oracle
         n = 2 if nvox > 5e8 else (4 if nvox > 5e7 else 5)
         nv, times, sample = oracle_sample(c, min(n, c.n_frames))
-        out["cpu_baseline"] = {"value": nv * len(times) / sum(times), "unit": UNIT, "cores": os.cpu_count() or 1, "kind": "oracle",
+        out["cpu_baseline"] = {"value": nv * len(times) / sum(times), "unit": UNIT, "cores": oracle.threads(), "kind": "oracle",
                                "sample": sample, "ms_per_frame": 1e3 * float(np.mean(times)),
+                               "omp_get_max_threads": oracle.threads(), "nproc": os.cpu_count() or 1,
                                "raycast_ms": oracle_sample.raycast_ms}
+        # plus a 1-thread figure on config 1 (a subprocess: the thread count is fixed when the OpenMP runtime starts)
+        try:
+            r = subprocess.run([sys.executable, "-c",
+                                "import sys, json; sys.path.insert(0, %r); import bench, synth\n"
+                                "nv, t, s = bench.oracle_sample(synth.config(1), 5)\n"
+                                "print(json.dumps({'value': nv * len(t) / sum(t), 'ms_per_frame': 1e3 * sum(t) / len(t), 'sample': 'config 1, ' + s}))" % ROOT],
+                               env=dict(os.environ, OMP_NUM_THREADS="1"), capture_output=True, text=True, timeout=120)
+            out["cpu_baseline"]["one_thread_cfg1"] = dict(json.loads(r.stdout.strip().splitlines()[-1]), unit=UNIT, cores=1)
+        except Exception as e:                                     # reported, never fatal
+            out["cpu_baseline"]["one_thread_cfg1"] = {"error": repr(e)[:200]}
     print(json.dumps(out), flush=True)
     if world > 1:
         dist.destroy_process_group()

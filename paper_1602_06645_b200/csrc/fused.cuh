@@ -142,6 +142,25 @@ __device__ __forceinline__ uint32_t ld_relaxed(const uint32_t *ptr)
 
 struct Counts { unsigned long long n[CNT_N]; };
 
+#ifndef VF_COL_BATCH
+#define VF_COL_BATCH 4
+#endif
+constexpr uint32_t COL_BATCH = VF_COL_BATCH, COL_BATCH_TAIL = 12, GEO_BATCH = 2;
+// per-warp state of the consumer loop (shared memory; written by lane 0 between __syncwarp()s, read by every lane): the items
+// need every register, and what is kept in shared memory is not spilled to (cached, evictable) local memory around them
+enum : uint32_t { F_GEO_DONE = 1u, F_COL_DONE = 2u, F_MARKS_SET = 4u, F_SCAN_CLAIMED = 8u, F_COL_READY = 16u, F_CLS_COMPLETE = 32u };
+struct WarpState {
+    uint32_t flags;                 // F_*
+    uint32_t gt, gt_left;           // next geometry ticket of the warp and how many of its batch are left
+    uint32_t ct, ct_size;           // first ticket and size of the NEXT batch of colour items
+    uint32_t cb_left, cb_idx;       // the current batch: items left, index of the next one
+    uint32_t n_col, n_col_big;      // length of the colour work list (once it is final), and how many of its items are long ones
+    int      n_staged;              // fill level of the warp's stage
+    uint32_t cb_item[COL_BATCH][2]; // the current batch
+    uint32_t sat;                   // geometry tile in progress: its sub-boxes (item mask bits) found to hold only saturated free space
+    uint32_t box[2];                // ... and the sub-box (item mask bit) in each of the two register sets of the pipeline
+};
+
 // development aid (compile with -DVF_TRACE): per-warp timestamps of the phase transitions of k_fused, 16 words per warp
 #ifdef VF_TRACE
 __device__ unsigned long long g_trace[8192 * 16];
@@ -173,16 +192,6 @@ __device__ __forceinline__ uint32_t *layer_ptr(uint32_t *ptr, int e, uint32_t la
     return reinterpret_cast<uint32_t *>(a);
 }
 
-// development aid (compile with -DVF_TRACE): per-warp timestamps of the phase transitions of k_fused, 16 words per warp
-#ifdef VF_TRACE
-__device__ unsigned long long g_trace[8192 * 16];
-__device__ __forceinline__ unsigned long long vf_now() { unsigned long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); return t; }
-#define VF_T(slot) do { if (lane == 0 && gw < 8192u) g_trace[gw * 16u + (slot)] = vf_now(); } while (0)
-#define VF_TC(slot, v) do { if (lane == 0 && gw < 8192u) g_trace[gw * 16u + (slot)] = (v); } while (0)
-#else
-#define VF_T(slot) do { } while (0)
-#define VF_TC(slot, v) do { } while (0)
-#endif
 
 // COUNT only: how many distinct 32-byte sectors (8 words) the lanes with `pred` touch at word index `word`
 __device__ __forceinline__ unsigned sectors_touched(bool pred, unsigned long long word, int lane)
@@ -275,13 +284,13 @@ __device__ __noinline__ void geometry_tile_near(const Params &p, int ttx, int tt
 // y = lane >> 3) owns the column of 4 voxels along z, so every access of the warp is four whole 32-byte sectors and the
 // per-column part of eq. 5 is hoisted.  The passes are software-pipelined over two alternating register sets: while
 // sub-box n is updated, sub-box n + 1 has already been projected and its depth gathers and voxel loads are in flight.
-// Returns the sub-boxes (bits bx) all of whose voxels hold the saturated free-space word afterwards.  COUNT: sk4 = the
-// sub-boxes the plain variant would not have been given (their voxels are counted as skippable too).
+// ws.sat collects the sub-boxes (item mask bits) all of whose voxels hold the saturated free-space word afterwards; like the
+// number of the sub-box in each register set it lives in shared memory, not in a register the pipeline would have to spill.
+// COUNT: sk4 = the sub-boxes the plain variant would not have been given (their voxels are counted as skippable too).
 template <bool COUNT, int VAR>
-__device__ __forceinline__ uint32_t geometry_half_boxes(const Params &p, int ttx, int tty, int gz0, int lz0, uint32_t m4, uint32_t sk4, int lane, Counts &c)
+__device__ __forceinline__ void geometry_half_boxes(const Params &p, int ttx, int tty, int gz0, int lz0, int zh, uint32_t m4, uint32_t sk4, int lane,
+                                                    volatile WarpState &ws, Counts &c)
 {
-    const uint32_t sat_word = 0x7fffu | ((uint32_t)p.w_max << 16);
-    uint32_t sat4 = 0u;
     const int xl = lane & 7, j = tty * TY + (lane >> 3);
     const float fx = p.fx, fy = p.fy, cx = p.cx, cy = p.cy, vs = p.vs;
     const float neg_mu = p.neg_mu, inv_mu = p.inv_mu;
@@ -297,9 +306,9 @@ __device__ __forceinline__ uint32_t geometry_half_boxes(const Params &p, int ttx
     for (int e = 0; e < 4; ++e) pz[e] = __fmaf_rn((float)(gz0 + e) + 0.5f, vs, p.oz);
     // S2 of one sub-box: eq. 5, projection, the four depth gathers and the four voxel loads.  A voxel outside the frustum
     // or the volume keeps D = 0 ("invalid depth": not updated); its gather is predicated off.
-    auto load_project = [&](int bx, int &nrem, uint32_t *&ptr, uint32_t (&o)[4], float (&Z)[4], float (&D)[4], float (&L)[4]) {
+    auto load_project = [&](int bx, uint32_t *&ptr, uint32_t (&o)[4], float (&Z)[4], float (&D)[4], float (&L)[4]) {
         const int i = ttx * TX + 8 * bx + xl;
-        nrem = i < p.nx ? nrem_row : 0;
+        const int nrem = i < p.nx ? nrem_row : 0;
         const float px = __fmaf_rn((float)i + 0.5f, vs, p.ox);
         const float bX = __fmaf_rn(p.R[1], py, __fmaf_rn(p.R[0], px, p.t[0]));
         const float bY = __fmaf_rn(p.R[4], py, __fmaf_rn(p.R[3], px, p.t[1]));
@@ -326,11 +335,9 @@ __device__ __forceinline__ uint32_t geometry_half_boxes(const Params &p, int ttx
         }
     };
     // S3 of one sub-box: truncation test, running average, store of the words that changed
-    // (nrem = how many of the four voxels of the lane exist: the others count as saturated)
-    auto update = [&](int bx, int nrem, uint32_t *ptr, const uint32_t (&o)[4], const float (&Z)[4], const float (&D)[4], const float (&L)[4]) {
+    auto update = [&](int set, uint32_t *ptr, const uint32_t (&o)[4], const float (&Z)[4], const float (&D)[4], const float (&L)[4]) {
         uint32_t w4[4]; bool upd[4];
         tsdf_update4<COUNT, VAR>(o, Z, D, L, neg_mu, inv_mu, w_max, w4, upd);
-        bool sat = true;
 #pragma unroll
         for (int e = 0; e < 4; ++e) {
             if (COUNT) {
@@ -339,32 +346,42 @@ __device__ __forceinline__ uint32_t geometry_half_boxes(const Params &p, int ttx
                 const unsigned sr = sector_first(p, 0, upd[e], wi);
                 c.n[CNT_GEO_SEC_READ] += sr;
                 c.n[CNT_GEO_SEC_WRITTEN] += sector_first(p, 1, w4[e] != o[e], wi);
-                if ((sk4 >> bx) & 1u) { c.n[CNT_GEO_SKIPPABLE] += upd[e]; c.n[CNT_GEO_SEC_SKIPPABLE] += sr; }
+                if ((sk4 >> (ws.box[set] >> 1)) & 1u) { c.n[CNT_GEO_SKIPPABLE] += upd[e]; c.n[CNT_GEO_SEC_SKIPPABLE] += sr; }
             }
-            sat = sat & ((w4[e] == sat_word) | (e >= nrem));
             if (w4[e] != o[e]) __stcg(layer_ptr(ptr, e, layer_b), w4[e]);   // skip the store when nothing changed
         }
-        if (__all_sync(0xffffffffu, sat)) sat4 |= 1u << bx;
+        // does the sub-box hold nothing but the saturated free-space word now?  (A column that is partly outside the volume
+        // never does: its missing voxels read as 0.)
+        const uint32_t sat_word = 0x7fffu | ((uint32_t)w_max << 16);
+        if (__all_sync(0xffffffffu, (((w4[0] ^ sat_word) | (w4[1] ^ sat_word)) | ((w4[2] ^ sat_word) | (w4[3] ^ sat_word))) == 0u) && lane == 0)
+            ws.sat = ws.sat | (1u << ws.box[set]);
     };
     // Two register sets, A and B, used alternately (no register-to-register rotation)
     uint32_t *pA, *pB, oA[4], oB[4];
     float ZA[4], ZB[4], DA[4], DB[4], LA[4], LB[4];
-    int bA, bB, nA, nB;
     uint32_t m = m4;
     if (COUNT && lane == 0) atomicAdd(&p.ctrl[ST_SUBS], (uint32_t)__popc(m));
-    bA = __ffs(m) - 1; m &= m - 1u;
-    load_project(bA, nA, pA, oA, ZA, DA, LA);
+    int b = __ffs(m) - 1; m &= m - 1u;
+    if (lane == 0) ws.box[0] = (uint32_t)(2 * b + zh);
+    load_project(b, pA, oA, ZA, DA, LA);
     for (;;) {
         const bool hasB = m != 0u;
-        if (hasB) { bB = __ffs(m) - 1; m &= m - 1u; load_project(bB, nB, pB, oB, ZB, DB, LB); }   // sub-box n + 1 in flight
-        update(bA, nA, pA, oA, ZA, DA, LA);
+        if (hasB) {                                                                            // sub-box n + 1 in flight
+            b = __ffs(m) - 1; m &= m - 1u;
+            if (lane == 0) ws.box[1] = (uint32_t)(2 * b + zh);
+            load_project(b, pB, oB, ZB, DB, LB);
+        }
+        update(0, pA, oA, ZA, DA, LA);
         if (!hasB) break;
         const bool hasA = m != 0u;
-        if (hasA) { bA = __ffs(m) - 1; m &= m - 1u; load_project(bA, nA, pA, oA, ZA, DA, LA); }   // sub-box n + 2 in flight
-        update(bB, nB, pB, oB, ZB, DB, LB);
+        if (hasA) {                                                                            // sub-box n + 2 in flight
+            b = __ffs(m) - 1; m &= m - 1u;
+            if (lane == 0) ws.box[0] = (uint32_t)(2 * b + zh);
+            load_project(b, pA, oA, ZA, DA, LA);
+        }
+        update(1, pB, oB, ZB, DB, LB);
         if (!hasA) break;
     }
-    return sat4;
 }
 
 // one geometry tile, one warp.  The item names the tile's 8x4x4 sub-boxes that may hold a voxel this frame updates; they
@@ -373,7 +390,7 @@ __device__ __forceinline__ uint32_t geometry_half_boxes(const Params &p, int ttx
 // voxels -- was measured: 14 % faster on a saturating frame, but its registers cost the scan frames 8 % even when it is not
 // taken, so it is not in the kernel.)
 template <bool COUNT, int VAR>
-__device__ __forceinline__ void geometry_tile(const Params &p, uint32_t item, int lane, Counts &c)
+__device__ __forceinline__ void geometry_tile(const Params &p, uint32_t item, int lane, volatile WarpState &ws, Counts &c)
 {
     int ttx, tty, ttz, mask;
     item_unpack(item, ttx, tty, ttz, mask);
@@ -384,7 +401,7 @@ __device__ __forceinline__ void geometry_tile(const Params &p, uint32_t item, in
         return;
     }
     const int gz0 = local_to_global_tz(p, ttz) * TZ, lz0 = ttz * TZ;
-    uint32_t sat = (uint32_t)__ldg(p.tile_sat + tile) & ~(uint32_t)mask;   // the visited sub-boxes are looked at afresh
+    if (lane == 0) ws.sat = (uint32_t)__ldg(p.tile_sat + tile) & ~(uint32_t)mask;   // the visited sub-boxes are looked at afresh
     const uint32_t skippable = COUNT ? (uint32_t)__ldcg(p.tile_skip + tile) : 0u;
 #pragma unroll 1
     for (int zh = 0; zh < SUBZ; ++zh) {
@@ -393,10 +410,9 @@ __device__ __forceinline__ void geometry_tile(const Params &p, uint32_t item, in
         m = (m | (m >> 1)) & 0x33u; m = (m | (m >> 2)) & 0x0fu;       // bit bx
         uint32_t sk = (skippable >> zh) & 0x55u;
         sk = (sk | (sk >> 1)) & 0x33u; sk = (sk | (sk >> 2)) & 0x0fu;
-        const uint32_t s4 = geometry_half_boxes<COUNT, VAR>(p, ttx, tty, gz0 + zh * (TZ / SUBZ), lz0 + zh * (TZ / SUBZ), m, sk, lane, c);
-        sat |= (((s4 & 1u) | ((s4 & 2u) << 1) | ((s4 & 4u) << 2) | ((s4 & 8u) << 3)) << zh);   // bit bx -> bit 2 bx + zh
+        geometry_half_boxes<COUNT, VAR>(p, ttx, tty, gz0 + zh * (TZ / SUBZ), lz0 + zh * (TZ / SUBZ), zh, m, sk, lane, ws, c);
     }
-    if (lane == 0) p.tile_sat[tile] = (uint8_t)sat;
+    if (lane == 0) p.tile_sat[tile] = (uint8_t)ws.sat;
 }
 
 // pull the sectors of a geometry tile into L2 when the tile is started: lane = (row, layer); a layer is wanted when its z
@@ -604,21 +620,6 @@ __device__ __forceinline__ void colour_item(const Params &p, uint2 item, Stage &
 // geometry items; PHASE_COL = the colour items only -- so that vol_integrate_host can run everything that only needs the
 // depth image while the HD frame is still being copied (only the colour update reads it).
 enum { PHASE_ALL = 0, PHASE_GEO = 1, PHASE_COL = 2 };
-#ifndef VF_COL_BATCH
-#define VF_COL_BATCH 4
-#endif
-constexpr uint32_t COL_BATCH = VF_COL_BATCH, COL_BATCH_TAIL = 12, GEO_BATCH = 2;
-// per-warp state of the consumer loop (shared memory; written by lane 0 between __syncwarp()s, read by every lane)
-enum : uint32_t { F_GEO_DONE = 1u, F_COL_DONE = 2u, F_MARKS_SET = 4u, F_SCAN_CLAIMED = 8u, F_COL_READY = 16u, F_CLS_COMPLETE = 32u };
-struct WarpState {
-    uint32_t flags;                 // F_*
-    uint32_t gt, gt_left;           // next geometry ticket of the warp and how many of its batch are left
-    uint32_t ct, ct_size;           // first ticket and size of the NEXT batch of colour items
-    uint32_t cb_left, cb_idx;       // the current batch: items left, index of the next one
-    uint32_t n_col;                 // length of the colour work list (once it is final)
-    int      n_staged;              // fill level of the warp's stage
-    uint32_t cb_item[COL_BATCH][2]; // the current batch
-};
 #ifndef VF_MIN_CTAS
 #define VF_MIN_CTAS 4
 #endif
@@ -686,7 +687,7 @@ __global__ void __launch_bounds__(CTA, VF_MIN_CTAS) k_fused(const __grid_constan
         const int watching = (flags & (F_COL_DONE | F_COL_READY)) ? 0 : (!(flags & F_MARKS_SET) ? 1 : ((flags & F_SCAN_CLAIMED) ? 2 : 0));
         if (watching == 1) v_poll = ld_relaxed(&ctrl[Q_MARK_DONE]);
         if (watching == 2) v_poll = ld_relaxed(&ctrl[Q_SCAN_DONE]);
-        const bool geo_turn = !(flags & F_GEO_DONE) && (flags & (F_COL_READY | F_COL_DONE)) != F_COL_READY;   // colour items, when there are any, come first
+        const bool geo_turn = !(flags & F_GEO_DONE);              // geometry tiles first: the colour list ends on short items
         uint32_t gt = ws.gt;
         if (geo_turn && ws.gt_left == 0u) {
             gt = claim_n(&ctrl[Q_GEO_CURSOR], GEO_BATCH, lane);
@@ -699,9 +700,9 @@ __global__ void __launch_bounds__(CTA, VF_MIN_CTAS) k_fused(const __grid_constan
         if (watching == 2 && v_poll >= (phase == PHASE_COL ? 0u : n_scan)) {
             flags |= F_COL_READY;
             VF_T(5);
-            const uint32_t nc = __ldcg(&ctrl[ST_NCOL]), t = claim_n(&ctrl[Q_COL_CURSOR], 1u, lane);
+            const uint32_t nb = __ldcg(&ctrl[ST_NCOL]), nc = nb + __ldcg(&ctrl[ST_NCOL_SMALL]), t = claim_n(&ctrl[Q_COL_CURSOR], 1u, lane);
             __syncwarp();
-            if (lane == 0) { ws.n_col = nc; ws.ct = t; ws.ct_size = 1u; }
+            if (lane == 0) { ws.n_col = nc; ws.n_col_big = nb; ws.ct = t; ws.ct_size = 1u; }
         }
         if ((flags & (F_MARKS_SET | F_SCAN_CLAIMED)) == F_MARKS_SET) {
             const uint32_t k = claim(&ctrl[Q_SCAN_CLAIM], lane);
@@ -713,6 +714,7 @@ __global__ void __launch_bounds__(CTA, VF_MIN_CTAS) k_fused(const __grid_constan
                 chunk_done(&ctrl[Q_SCAN_DONE], lane);
 #ifdef VF_TRACE
                 tr_tscan += clock64() - t0;
+                VF_T(11);
 #endif
             } else {
                 flags |= F_SCAN_CLAIMED;
@@ -723,7 +725,7 @@ __global__ void __launch_bounds__(CTA, VF_MIN_CTAS) k_fused(const __grid_constan
         __syncwarp();
         if (lane == 0) ws.flags = flags;
         __syncwarp();
-        if ((flags & (F_COL_READY | F_COL_DONE)) == F_COL_READY) {
+        if ((flags & (F_COL_READY | F_COL_DONE)) == F_COL_READY && !geo_turn) {
             // Colour items are taken in batches: one ticket and one load for up to COL_BATCH of them; single items towards
             // the end of the list, where balance matters.
             uint32_t cb_left = ws.cb_left;
@@ -731,7 +733,11 @@ __global__ void __launch_bounds__(CTA, VF_MIN_CTAS) k_fused(const __grid_constan
                 const uint32_t ct = ws.ct, n_col = ws.n_col;
                 if (ct < n_col) {
                     cb_left = min(ws.ct_size, n_col - ct);
-                    if ((uint32_t)lane < cb_left) { const uint2 it = __ldcg(p.work_col + ct + lane); ws.cb_item[lane][0] = it.x; ws.cb_item[lane][1] = it.y; }
+                    if ((uint32_t)lane < cb_left) {                 // the long items from the front of the list, then the short ones from its back
+                        const uint32_t t = ct + (uint32_t)lane, nb = ws.n_col_big;
+                        const uint2 it = __ldcg(p.work_col + (t < nb ? t : p.work_col_cap - 1u - (t - nb)));
+                        ws.cb_item[lane][0] = it.x; ws.cb_item[lane][1] = it.y;
+                    }
                     const uint32_t sz = n_col - ct > COL_BATCH_TAIL * n_warps ? COL_BATCH : 1u;
                     const uint32_t t = claim_n(&ctrl[Q_COL_CURSOR], sz, lane);
                     __syncwarp();
@@ -775,7 +781,7 @@ __global__ void __launch_bounds__(CTA, VF_MIN_CTAS) k_fused(const __grid_constan
                 const unsigned long long t0 = clock64();
                 tr_ovg += t0 - tr_top;
 #endif
-                geometry_tile<COUNT, VAR>(p, v_slot, lane, c);
+                geometry_tile<COUNT, VAR>(p, v_slot, lane, ws, c);
 #ifdef VF_TRACE
                 tr_ngeo++; tr_tgeo += clock64() - t0;
 #endif
@@ -800,7 +806,7 @@ __global__ void __launch_bounds__(CTA, VF_MIN_CTAS) k_fused(const __grid_constan
     }
     int n_staged = ws.n_staged;
     VF_T(8);
-    VF_TC(9, tr_ngeo); VF_TC(10, tr_ncol); VF_TC(11, tr_sleep); VF_TC(12, tr_tgeo); VF_TC(13, tr_tcol); VF_TC(14, tr_tscan); VF_TC(15, tr_ovg); VF_TC(7, tr_ovc);
+    VF_TC(9, tr_ngeo); VF_TC(10, tr_ncol); VF_TC(12, tr_tgeo); VF_TC(13, tr_tcol); VF_TC(14, tr_tscan); VF_TC(15, tr_ovg); VF_TC(7, tr_ovc);
     if (n_staged > 0) colour_update_staged<COUNT, VAR>(p, st, 0, n_staged, lane, c);
     if (COUNT) {
 #pragma unroll

@@ -73,7 +73,9 @@ struct Params {
     int       parity;            // frame parity: which of the two job counters this frame uses (the other one is zeroed)
     uint32_t *work_geo;          // geometry work list (n_tiles entries, all zero between frames: a slot is cleared by the warp that takes it)
     uint32_t *marks;             // shell marks: words_per_tile(r) words per tile, bit = colour cell that may hold sigma-shell voxels
-    uint2    *work_col;          // colour work list: one item per non-zero mark NIBBLE (up to 4 colour cells): {tile | nibble index, the nibble's bits}
+    uint2    *work_col;          // colour work list: one item per non-zero mark NIBBLE (up to 4 colour cells): {tile | nibble index, the nibble's
+                                 // bits}; items of 3 or 4 cells from the front (ST_NCOL of them), items of 1 or 2 cells from the back
+    uint32_t  work_col_cap;      // its capacity
     uint8_t  *tile_sat;          // per geometry tile: bit bx * SUBZ + bz = every voxel of that sub-box holds the saturated free-space word
                                  // (tsdf_q = 32767, w = w_max).  Kept by the fused kernel for the sub-boxes it visits; a sub-box
                                  // with its bit set that lies in front of every depth it can see by more than mu cannot change
@@ -113,7 +115,7 @@ __device__ __forceinline__ void item_unpack(uint32_t item, int &ttx, int &tty, i
 // ctrl[]: the first VOL_STATS_RAW_BYTES (128) are the statistics record vol_frame_stats* copies out: 8 words ST_*, then 12
 // 64-bit counters CNT_* (p.counters).  The queue control words Q_* follow; all of them are zeroed by k_prepass (the two job
 // counters alternately, see Params::parity).
-enum { ST_NGEO = 0, ST_NCOL = 1, ST_CELLS = 2, ST_SUBS = 3, ST_NJOBS = 4, ST_N = 8 };
+enum { ST_NGEO = 0, ST_NCOL = 1, ST_CELLS = 2, ST_SUBS = 3, ST_NJOBS = 4, ST_NCOL_SMALL = 5, ST_N = 8 };
 enum { CNT_GEO_READ = 0, CNT_GEO_CHANGED, CNT_COL_READ, CNT_COL_CHANGED, CNT_GEO_SEC_READ, CNT_GEO_SEC_WRITTEN, CNT_COL_SEC_READ,
        CNT_COL_SEC_WRITTEN, CNT_GEO_VISITED, CNT_COL_GATED, CNT_GEO_SKIPPABLE, CNT_GEO_SEC_SKIPPABLE, CNT_N = 12 };
 constexpr int CTRL_Q0 = 32;                                  // first queue-control word (byte 128)

@@ -408,42 +408,54 @@ __device__ __forceinline__ void scan_chunk(const Params &p, uint32_t chunk, int 
 {
     constexpr int WPT = words_per_tile(R), TPL = SCAN_CHUNK / 32;
     const int tile0 = (int)chunk * SCAN_CHUNK + lane * TPL;
-    uint32_t nz[TPL][WPT], mk[TPL][WPT];                // the mark words; bit n of nz set: nibble n of the word is non-zero
-    int ncol = 0;
+    uint32_t mk[TPL][WPT];                              // the mark words
+    int nbig = 0, nsmall = 0;                           // nibbles with 3-4 / 1-2 bits set
 #pragma unroll
     for (int k = 0; k < TPL; ++k)
 #pragma unroll
         for (int w = 0; w < WPT; ++w) {
-            nz[k][w] = 0u; mk[k][w] = 0u;
+            uint32_t m = 0u;
             if (tile0 + k < p.n_tiles) {
-                uint32_t m = __ldcg(p.marks + (size_t)(tile0 + k) * WPT + w);
-                mk[k][w] = m;
+                m = __ldcg(p.marks + (size_t)(tile0 + k) * WPT + w);
                 if (m) p.marks[(size_t)(tile0 + k) * WPT + w] = 0u;      // consumed: the marks are all zero again for the next frame
-                m |= m >> 1; m |= m >> 2; m &= 0x11111111u;          // bit 4n set: nibble n is non-zero
-                m = (m | (m >> 3)) & 0x03030303u; m = (m | (m >> 6)) & 0x000f000fu; nz[k][w] = (m | (m >> 12)) & 0xffu;
             }
-            ncol += __popc(nz[k][w]);
+            mk[k][w] = m;
+            // per nibble: number of bits, 0..4, in place (SWAR)
+            uint32_t c2 = (m & 0x55555555u) + ((m >> 1) & 0x55555555u);
+            c2 = (c2 & 0x33333333u) + ((c2 >> 2) & 0x33333333u);
+            const uint32_t ge3 = ((c2 + 0x11111111u) >> 2) & 0x11111111u & ~(c2 >> 2 & 0x11111111u) | ((c2 >> 2) & 0x11111111u);   // count >= 3
+            const uint32_t nzn = (c2 | (c2 >> 1) | (c2 >> 2)) & 0x11111111u;                                                       // count >= 1
+            nbig += __popc(ge3); nsmall += __popc(nzn & ~ge3);
         }
-    int pre = ncol;
+    // the long items (3 or 4 cells) go to the front of the list, the short ones to its back: the consumers take the front
+    // first, so that the kernel ends on short items
+    int preb = nbig, pres = nsmall;
 #pragma unroll
-    for (int o = 1; o < 32; o <<= 1) { const int v = __shfl_up_sync(0xffffffffu, pre, o); if (lane >= o) pre += v; }
-    const int tot = __shfl_sync(0xffffffffu, pre, 31);
-    if (tot == 0) return;
-    uint32_t bc = 0;
-    if (lane == 0) bc = atomicAdd(&p.ctrl[ST_NCOL], (uint32_t)tot);
-    bc = __shfl_sync(0xffffffffu, bc, 0);
-    if (ncol) {
-        uint32_t pos = bc + (uint32_t)(pre - ncol);
+    for (int o = 1; o < 32; o <<= 1) {
+        const int vb = __shfl_up_sync(0xffffffffu, preb, o), vs = __shfl_up_sync(0xffffffffu, pres, o);
+        if (lane >= o) { preb += vb; pres += vs; }
+    }
+    const int totb = __shfl_sync(0xffffffffu, preb, 31), tots = __shfl_sync(0xffffffffu, pres, 31);
+    if (totb + tots == 0) return;
+    uint32_t bb = 0, bs = 0;
+    if (lane == 0 && totb) bb = atomicAdd(&p.ctrl[ST_NCOL], (uint32_t)totb);
+    if (lane == 0 && tots) bs = atomicAdd(&p.ctrl[ST_NCOL_SMALL], (uint32_t)tots);
+    bb = __shfl_sync(0xffffffffu, bb, 0); bs = __shfl_sync(0xffffffffu, bs, 0);
+    if (nbig + nsmall) {
+        uint32_t posb = bb + (uint32_t)(preb - nbig), poss = p.work_col_cap - 1u - (bs + (uint32_t)(pres - nsmall));
 #pragma unroll
         for (int k = 0; k < TPL; ++k) {
             const int tile = tile0 + k;
             const int ttx = tile % p.tiles_x, tty = (tile / p.tiles_x) % p.tiles_y, ttz = tile / (p.tiles_x * p.tiles_y);
 #pragma unroll
             for (int w = 0; w < WPT; ++w) {
-                uint32_t m = nz[k][w];
-                while (m) {
-                    const int n = __ffs(m) - 1; m &= m - 1u;
-                    p.work_col[pos++] = make_uint2(item_pack(ttx, tty, ttz, 8 * w + n), mk[k][w] & (0xfu << (4 * n)));
+                const uint32_t m = mk[k][w];
+#pragma unroll 1
+                for (int n = 0; n < 8 && (m >> (4 * n)) != 0u; ++n) {
+                    const uint32_t bits = m & (0xfu << (4 * n));
+                    if (bits == 0u) continue;
+                    const uint2 item = make_uint2(item_pack(ttx, tty, ttz, 8 * w + n), bits);
+                    if (__popc(bits) >= 3) p.work_col[posb++] = item; else p.work_col[poss--] = item;
                 }
             }
         }

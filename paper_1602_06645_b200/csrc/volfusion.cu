@@ -225,6 +225,7 @@ extern "C" int vol_create(vol_t **out, const int32_t dims_geo[3], int32_t r, con
     const size_t nt = (size_t)(p.n_tiles > 0 ? p.n_tiles : 1), nw = nt * (size_t)vf::words_per_tile(r);
     if (cudaMalloc(&p.work_geo, sizeof(uint32_t) * nt) != cudaSuccess) rc = VOL_E_OOM;
     if (rc == VOL_OK && cudaMemset(p.work_geo, 0, sizeof(uint32_t) * nt) != cudaSuccess) rc = VOL_E_CUDA;   // empty slots are zero
+    p.work_col_cap = (uint32_t)(nw * 8);
     if (cudaMalloc(&p.work_col, sizeof(uint2) * nw * 8) != cudaSuccess) rc = VOL_E_OOM;
     if (cudaMalloc(&p.marks, sizeof(uint32_t) * nw) != cudaSuccess) rc = VOL_E_OOM;
     if (rc == VOL_OK && cudaMemset(p.marks, 0, sizeof(uint32_t) * nw) != cudaSuccess) rc = VOL_E_CUDA;
@@ -658,7 +659,7 @@ extern "C" int vol_stats_decode(const vol_t *v, const void *raw_host, vol_stats_
     }
     out->tiles_total = (uint32_t)v->p.n_tiles;
     out->tiles_geo = st[vf::ST_NGEO];
-    out->items_col = st[vf::ST_NCOL];
+    out->items_col = st[vf::ST_NCOL] + st[vf::ST_NCOL_SMALL];
     out->jobs_mark = st[vf::ST_NJOBS];
     return VOL_OK;
 }
