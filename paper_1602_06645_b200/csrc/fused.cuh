@@ -157,8 +157,6 @@ struct WarpState {
     uint32_t n_col, n_col_big;      // length of the colour work list (once it is final), and how many of its items are long ones
     int      n_staged;              // fill level of the warp's stage
     uint32_t cb_item[COL_BATCH][2]; // the current batch
-    uint32_t sat;                   // geometry tile in progress: its sub-boxes (item mask bits) found to hold only saturated free space
-    uint32_t box[2];                // ... and the sub-box (item mask bit) in each of the two register sets of the pipeline
 };
 
 // development aid (compile with -DVF_TRACE): per-warp timestamps of the phase transitions of k_fused, 16 words per warp
@@ -284,12 +282,12 @@ __device__ __noinline__ void geometry_tile_near(const Params &p, int ttx, int tt
 // y = lane >> 3) owns the column of 4 voxels along z, so every access of the warp is four whole 32-byte sectors and the
 // per-column part of eq. 5 is hoisted.  The passes are software-pipelined over two alternating register sets: while
 // sub-box n is updated, sub-box n + 1 has already been projected and its depth gathers and voxel loads are in flight.
-// ws.sat collects the sub-boxes (item mask bits) all of whose voxels hold the saturated free-space word afterwards; like the
-// number of the sub-box in each register set it lives in shared memory, not in a register the pipeline would have to spill.
-// COUNT: sk4 = the sub-boxes the plain variant would not have been given (their voxels are counted as skippable too).
-template <bool COUNT, int VAR>
-__device__ __forceinline__ void geometry_half_boxes(const Params &p, int ttx, int tty, int gz0, int lz0, int zh, uint32_t m4, uint32_t sk4, int lane,
-                                                    volatile WarpState &ws, Counts &c)
+// FULL: the half lies wholly inside the volume (no voxel of it needs a bounds test).
+// Returns, in visiting order (bit n = the n-th wanted sub-box), which sub-boxes hold nothing but the saturated free-space
+// word afterwards.  COUNT: sk4 = the sub-boxes (bits bx) the plain variant would not have been given (their voxels are
+// counted as skippable too).
+template <bool COUNT, int VAR, bool FULL>
+__device__ __forceinline__ uint32_t geometry_half_boxes(const Params &p, int ttx, int tty, int gz0, int lz0, uint32_t m4, uint32_t sk4, int lane, Counts &c)
 {
     const int xl = lane & 7, j = tty * TY + (lane >> 3);
     const float fx = p.fx, fy = p.fy, cx = p.cx, cy = p.cy, vs = p.vs;
@@ -300,26 +298,28 @@ __device__ __forceinline__ void geometry_half_boxes(const Params &p, int ttx, in
     const float py = __fmaf_rn((float)j + 0.5f, vs, p.oy);
     const float r02 = p.R[2], r12 = p.R[5], r22 = p.R[8];
     const uint32_t layer_b = (uint32_t)((size_t)p.ny * p.nx * 4u);
-    const int nrem_row = j < p.ny ? p.nz - gz0 : 0;                    // layers of this half the lane's row really has
+    const int nrem_row = FULL ? 4 : (j < p.ny ? p.nz - gz0 : 0);      // layers of this half the lane's row really has
+    const int i0 = ttx * TX + xl;
+    uint32_t *const row_ptr = p.geo + ((size_t)lz0 * p.ny + j) * p.nx + i0;   // the lane's voxel of the half's first layer in sub-box 0
     float pz[4];
 #pragma unroll
     for (int e = 0; e < 4; ++e) pz[e] = __fmaf_rn((float)(gz0 + e) + 0.5f, vs, p.oz);
     // S2 of one sub-box: eq. 5, projection, the four depth gathers and the four voxel loads.  A voxel outside the frustum
     // or the volume keeps D = 0 ("invalid depth": not updated); its gather is predicated off.
     auto load_project = [&](int bx, uint32_t *&ptr, uint32_t (&o)[4], float (&Z)[4], float (&D)[4], float (&L)[4]) {
-        const int i = ttx * TX + 8 * bx + xl;
-        const int nrem = i < p.nx ? nrem_row : 0;
+        const int i = i0 + 8 * bx;
+        const int nrem = FULL ? 4 : (i < p.nx ? nrem_row : 0);
         const float px = __fmaf_rn((float)i + 0.5f, vs, p.ox);
         const float bX = __fmaf_rn(p.R[1], py, __fmaf_rn(p.R[0], px, p.t[0]));
         const float bY = __fmaf_rn(p.R[4], py, __fmaf_rn(p.R[3], px, p.t[1]));
         const float bZ = __fmaf_rn(p.R[7], py, __fmaf_rn(p.R[6], px, p.t[2]));
-        ptr = p.geo + ((size_t)lz0 * p.ny + j) * p.nx + i;
+        ptr = row_ptr + 8 * bx;
 #pragma unroll
         for (int e = 0; e < 4; ++e) {
-            const bool in = e < nrem;
+            const bool in = FULL || e < nrem;
             // the voxel stream bypasses L1 (__ldcg): every sector is used once, and L1 is better spent on the depth image
-            o[e] = 0u;
-            if (in) o[e] = __ldcg(layer_ptr(ptr, e, layer_b));
+            if (FULL) o[e] = __ldcg(layer_ptr(ptr, e, layer_b));
+            else { o[e] = 0u; if (in) o[e] = __ldcg(layer_ptr(ptr, e, layer_b)); }
             const float X = __fmaf_rn(r02, pz[e], bX), Y = __fmaf_rn(r12, pz[e], bY);
             Z[e] = __fmaf_rn(r22, pz[e], bZ);
             bool ok; uint32_t off; float iz;
@@ -327,15 +327,13 @@ __device__ __forceinline__ void geometry_half_boxes(const Params &p, int ttx, in
             if (VAR == VAR_TSDF_ALONG_RAY)
                 L[e] = __fmul_rn(__fsqrt_rn(__fmaf_rn(Z[e], Z[e], __fmaf_rn(Y, Y, __fmul_rn(X, X)))), iz);
             D[e] = 0.0f;
-            if (ok && in) {
-                unsigned long long addr;                              // one mad.wide (FMA pipe) instead of a 64-bit add pair
-                asm("mad.wide.u32 %0, %1, 4, %2;" : "=l"(addr) : "r"(off), "l"(depthf));
-                D[e] = __ldg(reinterpret_cast<const float *>(addr));
-            }
+            if (ok && in) D[e] = __ldg(depthf + off);
         }
     };
-    // S3 of one sub-box: truncation test, running average, store of the words that changed
-    auto update = [&](int set, uint32_t *ptr, const uint32_t (&o)[4], const float (&Z)[4], const float (&D)[4], const float (&L)[4]) {
+    // S3 of one sub-box (the n-th of the half, bx its number): truncation test, running average, store of the words that
+    // changed; true if the sub-box holds nothing but the saturated free-space word afterwards.  (A column that is partly
+    // outside the volume never does: its missing voxels read as 0.)
+    auto update = [&](int bx, uint32_t *ptr, const uint32_t (&o)[4], const float (&Z)[4], const float (&D)[4], const float (&L)[4]) -> bool {
         uint32_t w4[4]; bool upd[4];
         tsdf_update4<COUNT, VAR>(o, Z, D, L, neg_mu, inv_mu, w_max, w4, upd);
 #pragma unroll
@@ -346,42 +344,46 @@ __device__ __forceinline__ void geometry_half_boxes(const Params &p, int ttx, in
                 const unsigned sr = sector_first(p, 0, upd[e], wi);
                 c.n[CNT_GEO_SEC_READ] += sr;
                 c.n[CNT_GEO_SEC_WRITTEN] += sector_first(p, 1, w4[e] != o[e], wi);
-                if ((sk4 >> (ws.box[set] >> 1)) & 1u) { c.n[CNT_GEO_SKIPPABLE] += upd[e]; c.n[CNT_GEO_SEC_SKIPPABLE] += sr; }
+                if ((sk4 >> bx) & 1u) { c.n[CNT_GEO_SKIPPABLE] += upd[e]; c.n[CNT_GEO_SEC_SKIPPABLE] += sr; }
             }
             if (w4[e] != o[e]) __stcg(layer_ptr(ptr, e, layer_b), w4[e]);   // skip the store when nothing changed
         }
-        // does the sub-box hold nothing but the saturated free-space word now?  (A column that is partly outside the volume
-        // never does: its missing voxels read as 0.)
         const uint32_t sat_word = 0x7fffu | ((uint32_t)w_max << 16);
-        if (__all_sync(0xffffffffu, (((w4[0] ^ sat_word) | (w4[1] ^ sat_word)) | ((w4[2] ^ sat_word) | (w4[3] ^ sat_word))) == 0u) && lane == 0)
-            ws.sat = ws.sat | (1u << ws.box[set]);
+        return __all_sync(0xffffffffu, (((w4[0] ^ sat_word) | (w4[1] ^ sat_word)) | ((w4[2] ^ sat_word) | (w4[3] ^ sat_word))) == 0u);
     };
-    // Two register sets, A and B, used alternately (no register-to-register rotation)
+    if (COUNT && lane == 0) atomicAdd(&p.ctrl[ST_SUBS], (uint32_t)__popc(m4));
+    uint32_t m = m4, satseq = 0u;
+    if (!FULL) {
+        // a half that sticks out of the volume (the last tiles of an axis): one sub-box after the other, no pipeline
+        uint32_t *pA, oA[4];
+        float ZA[4], DA[4], LA[4];
+#pragma unroll 1
+        for (uint32_t n = 0; m != 0u; ++n) {
+            const int bx = __ffs(m) - 1; m &= m - 1u;
+            load_project(bx, pA, oA, ZA, DA, LA);
+            satseq |= (update(bx, pA, oA, ZA, DA, LA) ? 1u : 0u) << n;
+        }
+        return satseq;
+    }
+    // Two register sets, A and B, used alternately (no register-to-register rotation).  n = position of set A's sub-box in
+    // the visiting order (set B's is n + 1).
     uint32_t *pA, *pB, oA[4], oB[4];
     float ZA[4], ZB[4], DA[4], DB[4], LA[4], LB[4];
-    uint32_t m = m4;
-    if (COUNT && lane == 0) atomicAdd(&p.ctrl[ST_SUBS], (uint32_t)__popc(m));
-    int b = __ffs(m) - 1; m &= m - 1u;
-    if (lane == 0) ws.box[0] = (uint32_t)(2 * b + zh);
+    int b = __ffs(m) - 1, bxA = b, bxB = 0;                              // (bxA / bxB: only the counting variant keeps them)
+    m &= m - 1u;
     load_project(b, pA, oA, ZA, DA, LA);
-    for (;;) {
+#pragma unroll 1
+    for (uint32_t n = 0;; n += 2) {
         const bool hasB = m != 0u;
-        if (hasB) {                                                                            // sub-box n + 1 in flight
-            b = __ffs(m) - 1; m &= m - 1u;
-            if (lane == 0) ws.box[1] = (uint32_t)(2 * b + zh);
-            load_project(b, pB, oB, ZB, DB, LB);
-        }
-        update(0, pA, oA, ZA, DA, LA);
+        if (hasB) { b = __ffs(m) - 1; m &= m - 1u; bxB = b; load_project(b, pB, oB, ZB, DB, LB); }   // sub-box n + 1 in flight
+        satseq |= (update(COUNT ? bxA : 0, pA, oA, ZA, DA, LA) ? 1u : 0u) << n;
         if (!hasB) break;
         const bool hasA = m != 0u;
-        if (hasA) {                                                                            // sub-box n + 2 in flight
-            b = __ffs(m) - 1; m &= m - 1u;
-            if (lane == 0) ws.box[0] = (uint32_t)(2 * b + zh);
-            load_project(b, pA, oA, ZA, DA, LA);
-        }
-        update(1, pB, oB, ZB, DB, LB);
+        if (hasA) { b = __ffs(m) - 1; m &= m - 1u; bxA = b; load_project(b, pA, oA, ZA, DA, LA); }   // sub-box n + 2 in flight
+        satseq |= (update(COUNT ? bxB : 0, pB, oB, ZB, DB, LB) ? 2u : 0u) << n;
         if (!hasA) break;
     }
+    return satseq;
 }
 
 // one geometry tile, one warp.  The item names the tile's 8x4x4 sub-boxes that may hold a voxel this frame updates; they
@@ -390,7 +392,7 @@ __device__ __forceinline__ void geometry_half_boxes(const Params &p, int ttx, in
 // voxels -- was measured: 14 % faster on a saturating frame, but its registers cost the scan frames 8 % even when it is not
 // taken, so it is not in the kernel.)
 template <bool COUNT, int VAR>
-__device__ __forceinline__ void geometry_tile(const Params &p, uint32_t item, int lane, volatile WarpState &ws, Counts &c)
+__device__ __forceinline__ void geometry_tile(const Params &p, uint32_t item, int lane, Counts &c)
 {
     int ttx, tty, ttz, mask;
     item_unpack(item, ttx, tty, ttz, mask);
@@ -401,8 +403,9 @@ __device__ __forceinline__ void geometry_tile(const Params &p, uint32_t item, in
         return;
     }
     const int gz0 = local_to_global_tz(p, ttz) * TZ, lz0 = ttz * TZ;
-    if (lane == 0) ws.sat = (uint32_t)__ldg(p.tile_sat + tile) & ~(uint32_t)mask;   // the visited sub-boxes are looked at afresh
+    uint32_t sat = (uint32_t)__ldg(p.tile_sat + tile) & ~(uint32_t)mask;   // the visited sub-boxes are looked at afresh
     const uint32_t skippable = COUNT ? (uint32_t)__ldcg(p.tile_skip + tile) : 0u;
+    const bool full_xy = ttx * TX + TX <= p.nx && tty * TY + TY <= p.ny;
 #pragma unroll 1
     for (int zh = 0; zh < SUBZ; ++zh) {
         uint32_t m = ((uint32_t)mask >> zh) & 0x55u;                  // bit 2 bx: sub-box bx of this half
@@ -410,9 +413,13 @@ __device__ __forceinline__ void geometry_tile(const Params &p, uint32_t item, in
         m = (m | (m >> 1)) & 0x33u; m = (m | (m >> 2)) & 0x0fu;       // bit bx
         uint32_t sk = (skippable >> zh) & 0x55u;
         sk = (sk | (sk >> 1)) & 0x33u; sk = (sk | (sk >> 2)) & 0x0fu;
-        geometry_half_boxes<COUNT, VAR>(p, ttx, tty, gz0 + zh * (TZ / SUBZ), lz0 + zh * (TZ / SUBZ), zh, m, sk, lane, ws, c);
+        const int g = gz0 + zh * (TZ / SUBZ), l = lz0 + zh * (TZ / SUBZ);
+        uint32_t seq = full_xy && g + TZ / SUBZ <= p.nz ? geometry_half_boxes<COUNT, VAR, true>(p, ttx, tty, g, l, m, sk, lane, c)
+                                                        : geometry_half_boxes<COUNT, VAR, false>(p, ttx, tty, g, l, m, sk, lane, c);
+        for (; seq != 0u && m != 0u; seq >>= 1, m &= m - 1u)           // visiting order -> item mask bit 2 bx + zh
+            if (seq & 1u) sat |= 1u << (2 * (__ffs(m) - 1) + zh);
     }
-    if (lane == 0) p.tile_sat[tile] = (uint8_t)ws.sat;
+    if (lane == 0) p.tile_sat[tile] = (uint8_t)sat;
 }
 
 // pull the sectors of a geometry tile into L2 when the tile is started: lane = (row, layer); a layer is wanted when its z
@@ -781,7 +788,7 @@ __global__ void __launch_bounds__(CTA, VF_MIN_CTAS) k_fused(const __grid_constan
                 const unsigned long long t0 = clock64();
                 tr_ovg += t0 - tr_top;
 #endif
-                geometry_tile<COUNT, VAR>(p, v_slot, lane, ws, c);
+                geometry_tile<COUNT, VAR>(p, v_slot, lane, c);
 #ifdef VF_TRACE
                 tr_ngeo++; tr_tgeo += clock64() - t0;
 #endif
