@@ -25,6 +25,10 @@
  *     failed call leaves the volumes untouched.  Nothing throws or aborts across this boundary.
  *   - `stream` is a cudaStream_t passed as void* (NULL = default stream).  vol_integrate* and vol_reset are
  *     asynchronous on it; vol_download*, vol_upload and vol_frame_stats synchronise it before returning.
+ *   - All calls on ONE vol_t must be ordered with respect to each other (one stream, or events between streams): the
+ *     per-frame scratch of a volume -- control words, shell marks, work lists, pixel map, depth pyramid, staging sets,
+ *     per-tile summaries -- exists once per volume, and two vol_integrate* / vol_frame_stats* / vol_raycast calls in
+ *     flight on unordered streams would corrupt it (and the volumes).  Different vol_t are independent.
  */
 #ifndef VOLFUSION_H
 #define VOLFUSION_H

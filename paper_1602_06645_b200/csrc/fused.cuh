@@ -4,13 +4,13 @@
 // (prepass.cuh: geometry tile classification, shell marking -- chunks claimed from counters, so nobody waits for work that
 // has not been claimed), then consumes work items until none is left:
 //   geometry items (one tile of 32x4x8 TSDF voxels + the mask of its 8x4x4 sub-boxes that may be updated) are published by
-//     the classification as it goes and consumed from the first microsecond;
+//     the classification as it goes and consumed from the first microsecond; a warp takes them while there are any;
 //   colour items (one non-zero shell-mark nibble = up to 4 colour cells of 8x4x4 voxels of one tile) exist once every mark
-//     has been set and the mark words have been scanned (two grid-wide conditions, observed through counters); from then on
-//     they are taken first (they are the longer items; the geometry tiles fill the tail).
-// A lane owns an (x, y) column of a sub-box (4 voxels along z), so a warp reads whole 32-byte sectors and the per-column
-// part of eq. 5 is hoisted.  Colour voxels that pass the gate are compacted in a per-warp shared-memory stage and updated
-// one per lane.  No block-level barriers.
+//     has been set and the mark words have been scanned (two grid-wide conditions, observed through counters); the items of
+//     3-4 cells are taken first, those of 1-2 cells last, so that the kernel ends on short items.
+// A lane owns an (x, y) column of a sub-box or cell (4 voxels along z), so a warp reads whole 32-byte sectors and the
+// per-column part of eq. 5 is hoisted.  Colour voxels that pass the gate are compacted in a per-warp shared-memory stage and
+// updated one per lane.  No block-level barriers; the state of a warp's loop lives in shared memory.
 //
 // The per-voxel arithmetic is the canonical sequence of DESIGN.md, issued branch-free for 4 voxels at a time
 // (projection -> gathers -> update); operands outside the range of the branch-free exact reciprocal (exact.cuh) send
@@ -805,7 +805,7 @@ __global__ void __launch_bounds__(CTA, VF_MIN_CTAS) k_fused(const __grid_constan
         if ((flags & (F_GEO_DONE | F_COL_DONE)) == (F_GEO_DONE | F_COL_DONE)) break;
         if (watching == 0 && !geo_turn) continue;
         if (flags & F_GEO_DONE || v_slot == 0u) {
-            __nanosleep(100);                                         // waiting for claimed producer chunks to finish
+            __nanosleep(1000);                                        // waiting for claimed producer chunks to finish (a round costs ~100 instructions)
 #ifdef VF_TRACE
             tr_sleep++;
 #endif
