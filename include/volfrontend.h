@@ -44,8 +44,10 @@ typedef struct {
     float   dist_m;         /* F5 distance gate; <= 0 selects 0.10 */
     float   cos_min;        /* F5 normal gate (cosine); <= 0 selects 0.94 */
     int32_t device;         /* CUDA device ordinal; < 0 = current device */
+    float   cond_min;       /* F6 conditioning gate, see vol_frontend_track; <= 0 selects VOL_ICP_COND_MIN; must be < 1 */
 } vol_frontend_opts_t;
 
+#define VOL_ICP_COND_MIN 1e-3f
 #define VOL_ICP_SUMS 29     /* 21 = upper triangle of A row by row (A00 A01 .. A05 A11 ..), 6 = b, sum r^2, count */
 
 /* w, h: size of level 0; both must be divisible by 2^(levels-1); levels in 1..6; opts nullable. */
@@ -67,16 +69,32 @@ int vol_frontend_predict(vol_frontend_t *fe, const vol_t *v, const float T_world
                          float t_far_m, void *stream);
 
 /* One F5 step at `level` with the estimate T_pred_cur (HOST: current camera -> prediction camera).  sums_host: HOST,
- * VOL_ICP_SUMS doubles.  Synchronises `stream`. */
+ * VOL_ICP_SUMS doubles.  The sums are bit-reproducible from run to run on one device: threads, warps and blocks add in a
+ * fixed order and the blocks' partial sums meet in integer accumulators (resolution 2^-60), whose result does not depend
+ * on the order of arrival.  Synchronises `stream`. */
 int vol_frontend_icp_step(vol_frontend_t *fe, int32_t level, const float T_pred_cur[16], double *sums_host, void *stream);
 
 /* F7: the whole coarse-to-fine loop in one cooperative launch (F5 and F6 on the device, F6 in binary64).  T_init: HOST, nullable (identity);
  * iterations: HOST int32[levels], iterations[l] steps at level l; T_out: HOST, the final estimate current camera ->
  * prediction camera (so T_world_cur = T_world_pred * T_out); rms_out / count_out: nullable, residual and number of
- * correspondences of the last step.  Returns VOL_E_ARG if a step finds fewer than 100 correspondences or A is not positive
- * definite (tracking lost; T_out then holds the last estimate).  Synchronises `stream`. */
+ * correspondences of the last step.  Returns VOL_E_ARG for invalid arguments (nothing was launched) and VOL_E_LOST when
+ * tracking is lost: a step found fewer than 100 correspondences (status 1), A was not positive definite (2), or A was
+ * too close to singular (3): the smallest Cholesky pivot relative to its diagonal entry, min_j d_j / A_jj in (0, 1], fell
+ * below cond_min -- some motion is then not observable from the maps (a sphere, a plane, a scene symmetric about the axis
+ * the camera turns about) and the solve would return noise along it.  The default, 1e-3, lies between what structured
+ * scenes give (0.3 .. 0.5 for rooms and table tops, 8e-3 for a 10 cm object filling a twentieth of the image) and what a
+ * sphere or a wall gives through sensor noise (1e-4 .. 4e-4 at the coarsest level; below 1e-6 on exact depth).  What the
+ * gate cannot see: sensor noise in the normals adds information that is not there, so a NOISY surface of revolution turned
+ * about its axis reads 0.3 like any scene, the images carry no trace of the motion, and F7 returns "no motion" with a small
+ * residual; no geometric tracker can do better.  T_out then holds the last estimate that was
+ * accepted, rms / count those of the failing step.  The result is bit-reproducible (see vol_frontend_icp_step).
+ * Synchronises `stream`. */
 int vol_frontend_track(vol_frontend_t *fe, const float T_init[16], const int32_t *iterations, float T_out[16], double *rms_out,
                        int64_t *count_out, void *stream);
+
+/* Status (0 ok, 1, 2, 3 as above), pyramid level and conditioning min_j d_j / A_jj of the last step of the most recent
+ * vol_frontend_track; every pointer nullable.  HOST values, no device work. */
+int vol_frontend_track_info(const vol_frontend_t *fe, int32_t *status_out, int32_t *level_out, double *conditioning_out);
 
 /* Copy the maps of one level to the host (tests, debugging): which = 0 measured, 1 predicted; depth_host: wl*hl floats,
  * vertex_host / normal_host: wl*hl*3 floats; any may be NULL.  Synchronises `stream`. */

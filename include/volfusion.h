@@ -45,6 +45,9 @@ extern "C" {
                             non-zero skew, non-rigid T, image size <= 0, buffer too small, bad shard */
 #define VOL_E_OOM   -2   /* device allocation failed */
 #define VOL_E_CUDA  -3   /* a CUDA call failed (sticky: see vol_strerror) */
+#define VOL_E_LOST  -4   /* vol_frontend_track only: the arguments were valid but the pose could not be estimated (too few
+                            correspondences, normal equations not positive definite or too close to singular); the
+                            volumes and the front end are intact and the caller may re-localise or skip the frame */
 
 /* geometry layers per shard slab (and per culling tile along z): rank `shard_rank` of `shard_world` owns the
  * geometry layers k with (k / VOL_SLAB) % shard_world == shard_rank, and the r*VOL_SLAB colour layers under each */

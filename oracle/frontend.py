@@ -223,16 +223,46 @@ def se3_update(T, A, b):
     return out, xi
 
 
-def track(meas, pred, K, T_init=None, iterations=(10, 5, 4), dist_m=0.10, cos_min=0.94, min_count=100):
+class TrackingLost(ValueError):
+    """F7: the pose could not be estimated; .status = 1 too few correspondences, 2 A not positive definite, 3 A too close to singular."""
+
+    def __init__(self, status, what):
+        super().__init__("tracking lost: " + what)
+        self.status = status
+
+
+COND_MIN = float(F32(1e-3))     # F6: the default gate on conditioning(A)
+
+
+def conditioning(A):
+    """F6: min_j d_j / A_jj, d_j = L_jj^2 the j-th pivot of the Cholesky factorisation A = L L^T in the order of the
+    parameters (omega, v): the share of parameter j's information that parameters 0 .. j-1 do not already explain.  1 for
+    a diagonal A, -> 0 as A becomes singular, unchanged when a parameter is rescaled (A -> S A S, S diagonal), so radians
+    against metres does not matter.  0 if A is not positive definite."""
+    A = np.asarray(A, np.float64)
+    try:
+        L = np.linalg.cholesky(A)
+    except np.linalg.LinAlgError:
+        return 0.0
+    return float(np.min(np.diag(L) ** 2 / np.diag(A)))
+
+
+def track(meas, pred, K, T_init=None, iterations=(10, 5, 4), dist_m=0.10, cos_min=0.94, min_count=100, cond_min=COND_MIN):
     """F7: coarse to fine -- iterations[l] steps at level l, from the coarsest level down; the estimate is kept in binary64
-    and rounded to binary32 for each step.  Returns (T_pred_cur [4,4] float64, rms residual of the last step, its count)."""
+    and rounded to binary32 for each step.  A step with fewer than min_count correspondences, or whose A fails the
+    conditioning gate, raises TrackingLost.  Returns (T_pred_cur [4,4] float64, rms residual of the last step, its count)."""
     T = np.eye(4) if T_init is None else np.asarray(T_init, np.float64).reshape(4, 4).copy()
     rms, cnt = 0.0, 0
     for level in range(len(iterations) - 1, -1, -1):
         for _ in range(iterations[level]):
             A, b, e, cnt = icp_step(meas, pred, K, level, T.astype(F32), dist_m, cos_min)
             if cnt < min_count:
-                raise ValueError("tracking lost: too few correspondences")
+                raise TrackingLost(1, "too few correspondences")
             rms = float(np.sqrt(e / cnt))
+            cond = conditioning(A)
+            if cond == 0.0:
+                raise TrackingLost(2, "normal equations not positive definite")
+            if cond < cond_min:
+                raise TrackingLost(3, "motion unobservable (conditioning %.3g)" % cond)
             T, _ = se3_update(T, A, b)
     return T, rms, cnt

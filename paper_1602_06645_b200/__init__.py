@@ -19,7 +19,7 @@ _SRC_DIR = os.path.join(_HERE, "csrc")
 _SO = os.path.join(_HERE, "libvolfusion.so")
 _lib = None
 
-VOL_OK, VOL_E_ARG, VOL_E_OOM, VOL_E_CUDA = 0, -1, -2, -3
+VOL_OK, VOL_E_ARG, VOL_E_OOM, VOL_E_CUDA, VOL_E_LOST = 0, -1, -2, -3, -4
 VOL_SLAB = 8
 VOL_STATS_RAW_BYTES = 128
 
@@ -31,12 +31,12 @@ EXPORTS = ["vol_create", "vol_integrate", "vol_integrate_host", "vol_raycast", "
            "vol_launches_per_frame", "vol_selftest", "vol_destroy", "vol_strerror",
            # include/volfrontend.h
            "vol_frontend_create", "vol_frontend_destroy", "vol_frontend_measure", "vol_frontend_predict_depth", "vol_frontend_predict",
-           "vol_frontend_icp_step", "vol_frontend_track", "vol_frontend_maps"]
+           "vol_frontend_icp_step", "vol_frontend_track", "vol_frontend_track_info", "vol_frontend_maps"]
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
     """Compile csrc/volfusion.cu for sm_100a into libvolfusion.so (in-tree; nvcc cross-compiles without a GPU)."""
-    srcs = [os.path.join(_SRC_DIR, f) for f in os.listdir(_SRC_DIR)] + [os.path.join(_ROOT, "include", "volfusion.h")]
+    srcs = [os.path.join(_SRC_DIR, f) for f in os.listdir(_SRC_DIR)] + [os.path.join(_ROOT, "include", f) for f in os.listdir(os.path.join(_ROOT, "include"))]
     newest = max(os.path.getmtime(s) for s in srcs)
     if force or not os.path.exists(_SO) or os.path.getmtime(_SO) < newest:
         nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
@@ -115,6 +115,7 @@ def lib():
         L.vol_frontend_predict.argtypes = [P, P, P, P, F, F, P]
         L.vol_frontend_icp_step.argtypes = [P, I32, P, P, P]
         L.vol_frontend_track.argtypes = [P, P, P, P, P, P, P]
+        L.vol_frontend_track_info.argtypes = [P, P, P, P]
         L.vol_frontend_maps.argtypes = [P, I32, I32, P, P, P, P]
         for name in EXPORTS:
             if name not in ("vol_destroy", "vol_strerror", "vol_frontend_destroy"):
@@ -308,7 +309,7 @@ class Volume:
 
 class FrontendOpts(ctypes.Structure):
     _fields_ = [("sigma_s_px", ctypes.c_float), ("sigma_r_m", ctypes.c_float), ("dist_m", ctypes.c_float),
-                ("cos_min", ctypes.c_float), ("device", ctypes.c_int32)]
+                ("cos_min", ctypes.c_float), ("device", ctypes.c_int32), ("cond_min", ctypes.c_float)]
 
 
 ICP_SUMS = 29
@@ -318,10 +319,10 @@ class Frontend:
     """include/volfrontend.h: depth front end (bilateral filter, vertex / normal map pyramid) and ICP tracking against a
     ray-cast prediction -- the measured and predicted map pyramids of one image size on one GPU."""
 
-    def __init__(self, w, h, levels=3, sigma_s_px=0.0, sigma_r_m=0.0, dist_m=0.0, cos_min=0.0, device=-1):
+    def __init__(self, w, h, levels=3, sigma_s_px=0.0, sigma_r_m=0.0, dist_m=0.0, cos_min=0.0, device=-1, cond_min=0.0):
         self._h = ctypes.c_void_p()
         self.w, self.h, self.levels = int(w), int(h), int(levels)
-        opts = FrontendOpts(float(sigma_s_px), float(sigma_r_m), float(dist_m), float(cos_min), int(device))
+        opts = FrontendOpts(float(sigma_s_px), float(sigma_r_m), float(dist_m), float(cos_min), int(device), float(cond_min))
         rc = lib().vol_frontend_create(ctypes.byref(self._h), self.w, self.h, self.levels, ctypes.byref(opts))
         if rc != VOL_OK:
             self._h = ctypes.c_void_p()
@@ -355,7 +356,7 @@ class Frontend:
         return A, s[21:27].copy(), float(s[27]), int(s[28])
 
     def track(self, T_init=None, iterations=(10, 5, 4), stream=None):
-        """vol_frontend_track: (T_pred_cur float32 [4,4], rms, count); raises VolError(VOL_E_ARG) when tracking is lost."""
+        """vol_frontend_track: (T_pred_cur float32 [4,4], rms, count); raises VolError(VOL_E_LOST) when tracking is lost."""
         it = np.ascontiguousarray(np.asarray(iterations, np.int32))
         assert it.size == self.levels
         Ti = None if T_init is None else _f32(T_init, 16)
@@ -364,6 +365,12 @@ class Frontend:
         _check(lib().vol_frontend_track(self._h, None if Ti is None else Ti.ctypes.data, it.ctypes.data, out.ctypes.data,
                                         ctypes.byref(rms), ctypes.byref(cnt), _stream_ptr(stream)), "vol_frontend_track")
         return out.reshape(4, 4), rms.value, cnt.value
+
+    def track_info(self):
+        """vol_frontend_track_info: (status, level, conditioning) of the last step of the most recent track()."""
+        st, lv, cond = ctypes.c_int32(0), ctypes.c_int32(0), ctypes.c_double(0.0)
+        _check(lib().vol_frontend_track_info(self._h, ctypes.byref(st), ctypes.byref(lv), ctypes.byref(cond)), "vol_frontend_track_info")
+        return st.value, lv.value, cond.value
 
     def maps(self, which, level, stream=None):
         """vol_frontend_maps: (D [h,w], V [h,w,3], N [h,w,3]) float32 of one level; which = 0 measured, 1 predicted."""

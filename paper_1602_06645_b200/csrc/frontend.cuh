@@ -172,8 +172,27 @@ __device__ __forceinline__ void icp_accumulate(double (&s)[ICP_SUMS], const floa
     s[28] += 1.0;
 }
 
-// block reduction (256 threads) of the per-thread sums, one atomic per accumulator
-__device__ __forceinline__ void icp_block_reduce(const double (&s)[ICP_SUMS], double (*sh)[ICP_SUMS], double *sums)
+// A block's partial sum a goes into TWO 64-bit integer accumulators, a = hi * 2^-20 + lo * 2^-60: hi = rint(a * 2^20), the
+// remainder a - hi * 2^-20 is exact in binary64 (|.| <= 2^-21) and lo = rint(remainder * 2^60) drops only bits below 2^-60.
+// Integer addition is associative, so the totals -- and with them the estimated pose -- do not depend on the order in which
+// the blocks arrive (binary64 atomicAdd would).  |a| is far below 2^42 for maps in metres (at most 2^19 pixels x (10 m)^2);
+// it is clamped there so that a corrupt map cannot overflow the integers.
+constexpr int ICP_ACC = 2 * ICP_SUMS;          // int64 words per set of accumulators: hi[ICP_SUMS], lo[ICP_SUMS]
+
+__device__ __forceinline__ void icp_publish(double a, unsigned long long *acc)
+{
+    a = fmin(fmax(a, -0x1p42), 0x1p42);
+    const double hi = rint(a * 0x1p20);
+    const double lo = rint((a - hi * 0x1p-20) * 0x1p60);
+    atomicAdd(acc, (unsigned long long)(long long)hi);
+    atomicAdd(acc + ICP_SUMS, (unsigned long long)(long long)lo);
+}
+
+__host__ __device__ __forceinline__ double icp_total(long long hi, long long lo) { return (double)hi * 0x1p-20 + (double)lo * 0x1p-60; }
+
+// block reduction (256 threads) of the per-thread sums in a fixed order (shuffle tree, then the 8 warps in turn), then
+// icp_publish of the block's 29 partial sums
+__device__ __forceinline__ void icp_block_reduce(const double (&s)[ICP_SUMS], double (*sh)[ICP_SUMS], unsigned long long *acc)
 {
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
 #pragma unroll
@@ -188,7 +207,7 @@ __device__ __forceinline__ void icp_block_reduce(const double (&s)[ICP_SUMS], do
         double a = 0.0;
 #pragma unroll
         for (int k = 0; k < 8; ++k) a += sh[k][threadIdx.x];
-        if (a != 0.0) atomicAdd(sums + threadIdx.x, a);
+        if (a != 0.0) icp_publish(a, acc + threadIdx.x);
     }
     __syncthreads();
 }
@@ -197,7 +216,7 @@ struct IcpParams {
     IcpLevel lv;
     float R[9], t[3];               // current camera -> prediction camera
     float dist2, cos_min;
-    double *sums;                   // ICP_SUMS accumulators (zeroed before the launch)
+    unsigned long long *acc;        // ICP_ACC integer accumulators (zeroed before the launch), see icp_publish
 };
 
 // F5, one step (vol_frontend_icp_step): one thread per measured pixel
@@ -210,23 +229,29 @@ __global__ void __launch_bounds__(256) k_icp(const __grid_constant__ IcpParams q
     for (int i = 0; i < ICP_SUMS; ++i) s[i] = 0.0;
     float J[6], r;
     if (x < q.lv.w && y < q.lv.h && icp_pixel(q.lv, q.R, q.t, q.dist2, q.cos_min, x, y, J, r)) icp_accumulate(s, J, r);
-    icp_block_reduce(s, sh, q.sums);
+    icp_block_reduce(s, sh, q.acc);
 }
 
 // F6 in binary64: A xi = b by Cholesky, then T <- [exp(omega) R, exp(omega) t + v].  T: 12 doubles (3 x 4, row-major).
-// Returns false if A is not positive definite.  One thread of every block runs this between two steps while the others
+// Returns 0, or 2 if A is not positive definite, or 3 if A is too close to singular: *cond = min_j d_j / A_jj, the smallest
+// Cholesky pivot relative to its diagonal entry (the part of parameter j's information that the parameters before it do
+// not already explain; 1 for a diagonal A, 0 for a singular one, and invariant under rescaling the parameters), and a
+// motion is unobservable where it falls below cond_min -- a sphere seen from its centre line, a scene that is
+// symmetric about the axis the camera turns about.  T is left alone in both failure cases.  One thread of every block runs this between two steps while the others
 // wait, so the chain of slow binary64 operations is kept short: one rsqrt per column instead of a sqrt and the divisions,
 // and the two Rodrigues coefficients from their series (ICP increments are far below 0.1 rad; sin / cos otherwise).
-__device__ inline bool icp_se3_update(double *T, const double *sums)
+__device__ inline int icp_se3_update(double *T, const double *sums, double cond_min, double *cond)
 {
     double A[6][6], L[6][6], inv[6], b[6], y[6], xi[6];
     int idx = 0;
     for (int i = 0; i < 6; ++i) for (int j = i; j < 6; ++j) { A[i][j] = sums[idx]; A[j][i] = sums[idx]; ++idx; }
     for (int i = 0; i < 6; ++i) { b[i] = sums[21 + i]; for (int j = 0; j < 6; ++j) L[i][j] = 0.0; }
+    double worst = 1.0;
     for (int j = 0; j < 6; ++j) {                                    // column by column
         double d = A[j][j];
         for (int k = 0; k < j; ++k) d -= L[j][k] * L[j][k];
-        if (!(d > 0.0)) return false;
+        if (!(d > 0.0)) { *cond = 0.0; return 2; }
+        worst = fmin(worst, d / A[j][j]);
         inv[j] = rsqrt(d);
         L[j][j] = d * inv[j];
         for (int i = j + 1; i < 6; ++i) {
@@ -235,6 +260,8 @@ __device__ inline bool icp_se3_update(double *T, const double *sums)
             L[i][j] = a * inv[j];
         }
     }
+    *cond = worst;
+    if (worst < cond_min) return 3;
     for (int i = 0; i < 6; ++i) { double a = b[i]; for (int k = 0; k < i; ++k) a -= L[i][k] * y[k]; y[i] = a * inv[i]; }
     for (int i = 5; i >= 0; --i) { double a = y[i]; for (int k = i + 1; k < 6; ++k) a -= L[k][i] * xi[k]; xi[i] = a * inv[i]; }
     const double ox = xi[0], oy = xi[1], oz = xi[2], t2 = ox * ox + oy * oy + oz * oz;
@@ -261,7 +288,7 @@ __device__ inline bool icp_se3_update(double *T, const double *sums)
         out[4 * i + 3] = a + xi[3 + i];
     }
     for (int i = 0; i < 12; ++i) T[i] = out[i];
-    return true;
+    return 0;
 }
 
 // F7 in ONE cooperative launch (vol_frontend_track): every step is a grid-stride pass over the level's pixels into its own
@@ -272,8 +299,10 @@ struct TrackParams {
     int levels, iters[FE_MAX_LEVELS], min_count;
     float dist2, cos_min;
     double T0[12];                  // initial estimate
-    double *sums;                   // total steps x ICP_SUMS accumulators, zeroed
-    double *out;                    // 12 (T) + rms + count + status (0 ok, 1 too few correspondences, 2 not positive definite) + level
+    double cond_min;                // icp_se3_update's threshold
+    unsigned long long *acc;        // total steps x ICP_ACC integer accumulators, zeroed
+    double *out;                    // 12 (T) + rms + count + status (0 ok, 1 too few correspondences, 2 not positive definite,
+                                    // 3 unobservable) + level + conditioning of the last step solved
 };
 
 __global__ void __launch_bounds__(256) k_icp_track(const __grid_constant__ TrackParams q)
@@ -283,7 +312,7 @@ __global__ void __launch_bounds__(256) k_icp_track(const __grid_constant__ Track
     double T[12];
 #pragma unroll
     for (int i = 0; i < 12; ++i) T[i] = q.T0[i];
-    double rms = 0.0, count = 0.0, status = 0.0, at_level = 0.0;
+    double rms = 0.0, count = 0.0, status = 0.0, at_level = 0.0, cond = 1.0;
     int step = 0;
     for (int l = q.levels - 1; l >= 0 && status == 0.0; --l) {
         const IcpLevel &lv = q.lv[l];
@@ -300,34 +329,34 @@ __global__ void __launch_bounds__(256) k_icp_track(const __grid_constant__ Track
                 float J[6], r;
                 if (x < lv.w && y < lv.h && icp_pixel(lv, R, t, q.dist2, q.cos_min, x, y, J, r)) icp_accumulate(s, J, r);
             }
-            double *sums = q.sums + (size_t)step * ICP_SUMS;
-            icp_block_reduce(s, sh, sums);
+            unsigned long long *acc = q.acc + (size_t)step * ICP_ACC;
+            icp_block_reduce(s, sh, acc);
             __threadfence();
             grid.sync();
             if (threadIdx.x == 0) {                              // one thread per block solves; the others take its result
                 double g[ICP_SUMS];
 #pragma unroll
-                for (int i = 0; i < ICP_SUMS; ++i) g[i] = __ldcg(sums + i);
+                for (int i = 0; i < ICP_SUMS; ++i) g[i] = icp_total((long long)__ldcg(acc + i), (long long)__ldcg(acc + ICP_SUMS + i));
                 count = g[28];
                 if (count < (double)q.min_count) status = 1.0;
                 else {
                     rms = sqrt(g[27] / count);
-                    if (!icp_se3_update(T, g)) status = 2.0;
+                    status = (double)icp_se3_update(T, g, q.cond_min, &cond);
                 }
 #pragma unroll
                 for (int i = 0; i < 12; ++i) shT[i] = T[i];
-                shT[12] = rms; shT[13] = count; shT[14] = status;
+                shT[12] = rms; shT[13] = count; shT[14] = status; shT[15] = cond;
             }
             __syncthreads();
 #pragma unroll
             for (int i = 0; i < 12; ++i) T[i] = shT[i];
-            rms = shT[12]; count = shT[13]; status = shT[14]; at_level = (double)l;
+            rms = shT[12]; count = shT[13]; status = shT[14]; cond = shT[15]; at_level = (double)l;
             __syncthreads();
         }
     }
     if (blockIdx.x == 0 && threadIdx.x == 0) {
         for (int i = 0; i < 12; ++i) q.out[i] = T[i];
-        q.out[12] = rms; q.out[13] = count; q.out[14] = status; q.out[15] = at_level;
+        q.out[12] = rms; q.out[13] = count; q.out[14] = status; q.out[15] = at_level; q.out[16] = cond;
     }
 }
 

@@ -4,6 +4,8 @@
 #include "../../include/volfrontend.h"
 #include "frontend.cuh"
 
+constexpr int FE_TRACK_OUT = 24;                            // doubles read back by vol_frontend_track (17 used)
+
 struct vol_frontend {
     int device, w, h, levels;
     float sigma_s, sigma_r, dist_m, cos_min;
@@ -15,9 +17,11 @@ struct vol_frontend {
     bool have[2];
     float *ray_depth;                                       // vol_frontend_predict: the ray-cast depth map
     uint16_t *pred_mm;                                      // F8: the prediction in whole millimetres
-    double *sums_dev, *sums_pinned;
-    double *track_sums; size_t track_steps;                 // vol_frontend_track: one set of accumulators per step
-    double *track_out, *track_out_pinned;                   // 16 doubles: T (3 x 4), rms, count, status, level
+    unsigned long long *acc_dev, *acc_pinned;               // vol_frontend_icp_step: ICP_ACC integer accumulators
+    unsigned long long *track_acc; size_t track_steps;      // vol_frontend_track: one set of accumulators per step
+    double *track_out, *track_out_pinned;                   // FE_TRACK_OUT doubles: T (3 x 4), rms, count, status, level, conditioning
+    double cond_min;
+    int last_status, last_level; double last_cond;          // of the most recent vol_frontend_track
     int track_blocks;                                       // co-resident blocks of k_icp_track
 };
 
@@ -37,9 +41,9 @@ extern "C" void vol_frontend_destroy(vol_frontend_t *fe)
         }
     if (fe->ray_depth) cudaFree(fe->ray_depth);
     if (fe->pred_mm) cudaFree(fe->pred_mm);
-    if (fe->sums_dev) cudaFree(fe->sums_dev);
-    if (fe->sums_pinned) cudaFreeHost(fe->sums_pinned);
-    if (fe->track_sums) cudaFree(fe->track_sums);
+    if (fe->acc_dev) cudaFree(fe->acc_dev);
+    if (fe->acc_pinned) cudaFreeHost(fe->acc_pinned);
+    if (fe->track_acc) cudaFree(fe->track_acc);
     if (fe->track_out) cudaFree(fe->track_out);
     if (fe->track_out_pinned) cudaFreeHost(fe->track_out_pinned);
     cudaGetLastError();
@@ -50,23 +54,24 @@ extern "C" int vol_frontend_create(vol_frontend_t **out, int32_t w, int32_t h, i
 {
     if (!out || w <= 0 || h <= 0 || w > 16384 || h > 16384 || levels < 1 || levels > vf::FE_MAX_LEVELS) return VOL_E_ARG;
     if (w % (1 << (levels - 1)) != 0 || h % (1 << (levels - 1)) != 0) return VOL_E_ARG;
-    float sigma_s = 4.5f, sigma_r = 0.030f, dist_m = 0.10f, cos_min = 0.94f;
+    float sigma_s = 4.5f, sigma_r = 0.030f, dist_m = 0.10f, cos_min = 0.94f, cond_min = VOL_ICP_COND_MIN;
     int device = -1;
     if (opts) {
         if (opts->sigma_s_px > 0.0f) sigma_s = opts->sigma_s_px;
         if (opts->sigma_r_m > 0.0f) sigma_r = opts->sigma_r_m;
         if (opts->dist_m > 0.0f) dist_m = opts->dist_m;
         if (opts->cos_min > 0.0f) cos_min = opts->cos_min;
+        if (opts->cond_min > 0.0f) cond_min = opts->cond_min;
         device = opts->device;
     }
-    if (!(sigma_s <= 1e3f) || !(sigma_r <= 1.0f) || !(dist_m <= 1e3f) || !(cos_min <= 1.0f)) return VOL_E_ARG;
+    if (!(sigma_s <= 1e3f) || !(sigma_r <= 1.0f) || !(dist_m <= 1e3f) || !(cos_min <= 1.0f) || !(cond_min < 1.0f)) return VOL_E_ARG;
     if (device < 0) CK(cudaGetDevice(&device));
     CK(cudaSetDevice(device));
     vol_frontend *fe = new (std::nothrow) vol_frontend();
     if (!fe) return VOL_E_OOM;
     memset(fe, 0, sizeof *fe);
     fe->device = device; fe->w = w; fe->h = h; fe->levels = levels;
-    fe->sigma_s = sigma_s; fe->sigma_r = sigma_r; fe->dist_m = dist_m; fe->cos_min = cos_min;
+    fe->sigma_s = sigma_s; fe->sigma_r = sigma_r; fe->dist_m = dist_m; fe->cos_min = cos_min; fe->cond_min = (double)cond_min;
     // F1 tables: binary64, rounded once
     const double ss = (double)sigma_s, sr = (double)sigma_r * 1000.0;
     fe->kmax = (int)std::ceil(3.0 * sr);
@@ -81,10 +86,10 @@ extern "C" int vol_frontend_create(vol_frontend_t **out, int32_t w, int32_t h, i
     bool okc = cudaMalloc(&fe->ws, sizeof ws) == cudaSuccess && cudaMalloc(&fe->wr, sizeof(float) * (fe->kmax + 1)) == cudaSuccess &&
                cudaMalloc(&fe->ray_depth, sizeof(float) * (size_t)w * h) == cudaSuccess &&
                cudaMalloc(&fe->pred_mm, sizeof(uint16_t) * (size_t)w * h) == cudaSuccess &&
-               cudaMalloc(&fe->sums_dev, sizeof(double) * vf::ICP_SUMS) == cudaSuccess &&
-               cudaMallocHost(&fe->sums_pinned, sizeof(double) * vf::ICP_SUMS) == cudaSuccess &&
-               cudaMalloc(&fe->track_out, sizeof(double) * 16) == cudaSuccess &&
-               cudaMallocHost(&fe->track_out_pinned, sizeof(double) * 16) == cudaSuccess;
+               cudaMalloc(&fe->acc_dev, sizeof(unsigned long long) * vf::ICP_ACC) == cudaSuccess &&
+               cudaMallocHost(&fe->acc_pinned, sizeof(unsigned long long) * vf::ICP_ACC) == cudaSuccess &&
+               cudaMalloc(&fe->track_out, sizeof(double) * FE_TRACK_OUT) == cudaSuccess &&
+               cudaMallocHost(&fe->track_out_pinned, sizeof(double) * FE_TRACK_OUT) == cudaSuccess;
     for (int s = 0; s < 2 && okc; ++s)
         for (int l = 0; l < levels && okc; ++l) {
             const size_t n = (size_t)(w >> l) * (h >> l);
@@ -170,11 +175,11 @@ static int fe_icp_launch(vol_frontend *fe, int level, const float T[16], cudaStr
     vf::IcpParams q;
     q.lv = fe_level(fe, level);
     for (int i = 0; i < 3; ++i) { for (int j = 0; j < 3; ++j) q.R[3 * i + j] = T[4 * i + j]; q.t[i] = T[4 * i + 3]; }
-    q.dist2 = fe->dist_m * fe->dist_m; q.cos_min = fe->cos_min; q.sums = fe->sums_dev;
-    CK(cudaMemsetAsync(fe->sums_dev, 0, sizeof(double) * vf::ICP_SUMS, st));
+    q.dist2 = fe->dist_m * fe->dist_m; q.cos_min = fe->cos_min; q.acc = fe->acc_dev;
+    CK(cudaMemsetAsync(fe->acc_dev, 0, sizeof(unsigned long long) * vf::ICP_ACC, st));
     vf::k_icp<<<dim3((q.lv.w + 31) / 32, (q.lv.h + 7) / 8), 256, 0, st>>>(q);
     CK(cudaGetLastError());
-    CK(cudaMemcpyAsync(fe->sums_pinned, fe->sums_dev, sizeof(double) * vf::ICP_SUMS, cudaMemcpyDeviceToHost, st));
+    CK(cudaMemcpyAsync(fe->acc_pinned, fe->acc_dev, sizeof(unsigned long long) * vf::ICP_ACC, cudaMemcpyDeviceToHost, st));
     CK(cudaStreamSynchronize(st));
     return VOL_OK;
 }
@@ -191,7 +196,7 @@ extern "C" int vol_frontend_icp_step(vol_frontend_t *fe, int32_t level, const fl
     if (!fe_rigid(T_pred_cur)) return VOL_E_ARG;
     int rc = fe_set_device(fe); if (rc) return rc;
     rc = fe_icp_launch(fe, level, T_pred_cur, (cudaStream_t)stream); if (rc) return rc;
-    memcpy(sums_host, fe->sums_pinned, sizeof(double) * vf::ICP_SUMS);
+    for (int i = 0; i < vf::ICP_SUMS; ++i) sums_host[i] = vf::icp_total((long long)fe->acc_pinned[i], (long long)fe->acc_pinned[vf::ICP_SUMS + i]);
     return VOL_OK;
 }
 
@@ -206,8 +211,8 @@ extern "C" int vol_frontend_track(vol_frontend_t *fe, const float T_init[16], co
     int rc = fe_set_device(fe); if (rc) return rc;
     cudaStream_t st = (cudaStream_t)stream;
     if (steps > fe->track_steps) {
-        if (fe->track_sums) { CK(cudaDeviceSynchronize()); cudaFree(fe->track_sums); fe->track_sums = nullptr; fe->track_steps = 0; }
-        CK(cudaMalloc(&fe->track_sums, steps * vf::ICP_SUMS * sizeof(double)));
+        if (fe->track_acc) { CK(cudaDeviceSynchronize()); cudaFree(fe->track_acc); fe->track_acc = nullptr; fe->track_steps = 0; }
+        CK(cudaMalloc(&fe->track_acc, steps * vf::ICP_ACC * sizeof(unsigned long long)));
         fe->track_steps = steps;
     }
     vf::TrackParams q;
@@ -216,21 +221,32 @@ extern "C" int vol_frontend_track(vol_frontend_t *fe, const float T_init[16], co
     q.levels = fe->levels; q.min_count = 100;
     q.dist2 = fe->dist_m * fe->dist_m; q.cos_min = fe->cos_min;
     for (int i = 0; i < 12; ++i) q.T0[i] = T_init ? (double)T_init[i] : (i % 5 == 0 ? 1.0 : 0.0);
-    q.sums = fe->track_sums; q.out = fe->track_out;
-    if (steps > 0) CK(cudaMemsetAsync(fe->track_sums, 0, steps * vf::ICP_SUMS * sizeof(double), st));
+    q.acc = fe->track_acc; q.out = fe->track_out; q.cond_min = fe->cond_min;
+    if (steps > 0) CK(cudaMemsetAsync(fe->track_acc, 0, steps * vf::ICP_ACC * sizeof(unsigned long long), st));
     const int tiles0 = ((fe->w + 31) / 32) * ((fe->h + 7) / 8);
     const int blocks = fe->track_blocks < tiles0 ? fe->track_blocks : tiles0;
     void *args[] = {&q};
     CK(cudaLaunchCooperativeKernel((const void *)vf::k_icp_track, dim3(blocks), dim3(256), args, 0, st));
-    CK(cudaMemcpyAsync(fe->track_out_pinned, fe->track_out, sizeof(double) * 16, cudaMemcpyDeviceToHost, st));
+    CK(cudaMemcpyAsync(fe->track_out_pinned, fe->track_out, sizeof(double) * FE_TRACK_OUT, cudaMemcpyDeviceToHost, st));
     CK(cudaStreamSynchronize(st));
     const double *o = fe->track_out_pinned;
+    fe->last_status = (int)o[14]; fe->last_level = (int)o[15]; fe->last_cond = o[16];
     for (int i = 0; i < 12; ++i) T_out[i] = (float)o[i];
     T_out[12] = T_out[13] = T_out[14] = 0.0f; T_out[15] = 1.0f;
     if (rms_out) *rms_out = o[12];
     if (count_out) *count_out = (int64_t)o[13];
-    if (o[14] == 1.0) { snprintf(g_err, sizeof g_err, "vol_frontend_track: %lld correspondences at level %d", (long long)o[13], (int)o[15]); return VOL_E_ARG; }
-    if (o[14] == 2.0) { snprintf(g_err, sizeof g_err, "vol_frontend_track: normal equations not positive definite"); return VOL_E_ARG; }
+    if (o[14] == 1.0) { snprintf(g_err, sizeof g_err, "vol_frontend_track: %lld correspondences at level %d", (long long)o[13], (int)o[15]); return VOL_E_LOST; }
+    if (o[14] == 2.0) { snprintf(g_err, sizeof g_err, "vol_frontend_track: normal equations not positive definite at level %d", (int)o[15]); return VOL_E_LOST; }
+    if (o[14] == 3.0) { snprintf(g_err, sizeof g_err, "vol_frontend_track: motion unobservable at level %d (conditioning %.3g < %.3g)", (int)o[15], o[16], fe->cond_min); return VOL_E_LOST; }
+    return VOL_OK;
+}
+
+extern "C" int vol_frontend_track_info(const vol_frontend_t *fe, int32_t *status_out, int32_t *level_out, double *conditioning_out)
+{
+    if (!fe) return VOL_E_ARG;
+    if (status_out) *status_out = fe->last_status;
+    if (level_out) *level_out = fe->last_level;
+    if (conditioning_out) *conditioning_out = fe->last_cond;
     return VOL_OK;
 }
 

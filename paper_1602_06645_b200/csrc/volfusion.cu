@@ -147,6 +147,7 @@ extern "C" const char *vol_strerror(int code)
         case VOL_E_ARG: return "invalid argument";
         case VOL_E_OOM: return g_err[0] ? g_err : "out of device memory";
         case VOL_E_CUDA: return g_err[0] ? g_err : "CUDA error";
+        case VOL_E_LOST: return g_err[0] ? g_err : "tracking lost";
         default: return "unknown error code";
     }
 }

@@ -101,15 +101,62 @@ def test_icp_step_sums_and_track():
             assert cnt == cnt0 and cnt > 5000
             assert np.abs(A - A0).max() <= 1e-11 * np.abs(A0).max() and np.abs(b - b0).max() <= 1e-11 * np.abs(A0).max()
             assert abs(e - e0) <= 1e-11 * e0
+            A1, b1, e1, cnt1 = fe.icp_step(lv, T.astype(np.float32))            # bit-reproducible, not only close
+            assert A1.tobytes() == A.tobytes() and b1.tobytes() == b.tobytes() and e1 == e and cnt1 == cnt
     Tg, rms, cnt = fe.track()
     To, rms0, cnt0 = ofe.track(meas, pred, c.K_depth)
     assert np.abs(Tg.astype(np.float64) - To).max() < 2e-6 and abs(rms - rms0) < 1e-7 and abs(cnt - cnt0) <= 5
+    status, level, cond = fe.track_info()
+    A0, _, _, _ = ofe.icp_step(meas, pred, c.K_depth, 0, To.astype(np.float32))
+    assert (status, level) == (0, 0) and cond > 1e-3 and abs(cond - ofe.conditioning(A0)) < 0.05 * cond
+    for _ in range(5):                                                       # the whole loop: the same bits every time
+        Tg2, rms2, cnt2 = fe.track()
+        assert Tg2.tobytes() == Tg.tobytes() and rms2 == rms and cnt2 == cnt
     err = np.linalg.inv(dT) @ To
     assert np.linalg.norm(err[:3, 3]) < 2e-3 and math.degrees(math.acos(min(1.0, (np.trace(err[:3, :3]) - 1) / 2))) < 0.1
     # tracking lost: a prediction that shows nothing gives no correspondences
     fe.predict_depth(torch.zeros(c.wd * c.hd, dtype=torch.float32, device="cuda"), c.K_depth)
-    with pytest.raises(vf.VolError):
+    with pytest.raises(vf.VolError) as e:
         fe.track()
+    assert e.value.code == vf.VOL_E_LOST and fe.track_info()[0] == 1
+    fe.close()
+
+
+def test_track_refuses_an_unobservable_motion():
+    """F6's conditioning gate on the device takes the oracle's decision: a camera facing a wall (three unobservable
+    parameters) is VOL_E_LOST with status 3 and the initial estimate comes back untouched; with the gate lowered far enough
+    the same call goes through."""
+    import torch
+    import paper_1602_06645_b200 as vf
+    c = synth.config(2)
+    n = np.array([0.1, -0.2, 0.97], np.float64); n /= np.linalg.norm(n)
+    x, y = np.meshgrid(np.arange(c.wd, dtype=np.float64), np.arange(c.hd, dtype=np.float64))
+    K = np.asarray(c.K_depth, np.float64).reshape(3, 3)
+    ray = np.stack([(x - K[0, 2]) / K[0, 0], (y - K[1, 2]) / K[1, 1], np.ones_like(x)], -1)
+    D = (1.4 / (ray @ n)).astype(np.float32)
+    mm = np.clip(np.rint(D * 1000.0), 0, 65535).astype(np.uint16)            # both sides: the wall in millimetres through F1
+    meas = ofe.measure(mm, c.K_depth, 3)
+    with pytest.raises(ofe.TrackingLost) as eo:
+        ofe.track(meas, meas, c.K_depth)
+    assert eo.value.status == 3
+    A0, _, _, _ = ofe.icp_step(meas, meas, c.K_depth, 2, np.eye(4, dtype=np.float32))
+    fe = vf.Frontend(c.wd, c.hd, 3)
+    fe.measure(to_dev(mm), c.K_depth)
+    fe.predict_depth(torch.from_numpy(mm.astype(np.float32) / np.float32(1000.0)).cuda(), c.K_depth, filter=True)
+    with pytest.raises(vf.VolError) as e:
+        fe.track()
+    status, level, cond = fe.track_info()
+    print(f"wall: conditioning {cond:.3g} (oracle {ofe.conditioning(A0):.3g})")
+    assert e.value.code == vf.VOL_E_LOST and status == 3 and level == 2 and 0.0 < cond < 1e-3 and abs(cond - ofe.conditioning(A0)) < 0.05 * cond, (status, level, cond)
+    fe.close()
+    fe = vf.Frontend(c.wd, c.hd, 3, cond_min=1e-30)                           # gate as good as off: the solve goes ahead
+    fe.measure(to_dev(mm), c.K_depth)
+    fe.predict_depth(torch.from_numpy(mm.astype(np.float32) / np.float32(1000.0)).cuda(), c.K_depth, filter=True)
+    try:
+        fe.track(iterations=(0, 0, 1))
+        assert fe.track_info()[0] == 0
+    except vf.VolError as e2:                                                 # or A is singular outright in this rounding
+        assert e2.code == vf.VOL_E_LOST and fe.track_info()[0] == 2
     fe.close()
 
 

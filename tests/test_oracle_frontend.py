@@ -227,6 +227,40 @@ def test_track_recovers_a_known_motion(quantised):
     assert np.linalg.norm((np.linalg.inv(dT) @ T1)[:3, 3]) < 0.6 * np.linalg.norm(dT[:3, 3])
 
 
+def test_conditioning_closed_forms():
+    """F6's gate: 1 for a diagonal A; 1 - c^2 / (a b) for one coupled pair (the second pivot is b - c^2 / a); unchanged by a
+    rescaling of the parameters; 0 for a singular or indefinite A."""
+    assert abs(fe.conditioning(np.diag([2.0, 3.0, 4.0, 5.0, 6.0, 7.0])) - 1.0) < 1e-15
+    A = np.diag([2.0, 3.0, 4.0, 5.0, 6.0, 7.0]); A[1, 4] = A[4, 1] = 3.0
+    assert abs(fe.conditioning(A) - (1.0 - 9.0 / 18.0)) < 1e-15
+    S = np.diag([1.0, 1e3, 1.0, 1e-3, 10.0, 1.0])
+    assert abs(fe.conditioning(S @ A @ S) - 0.5) < 1e-12
+    J = np.array([1.0, 2.0, 0.5, -1.0, 0.3, 0.7])
+    assert fe.conditioning(np.outer(J, J)) == 0.0                               # rank 1
+    assert fe.conditioning(np.diag([1.0, 1.0, -1.0, 1.0, 1.0, 1.0])) == 0.0     # indefinite
+
+
+def test_track_refuses_an_unobservable_motion():
+    """A camera facing a wall: sliding along the wall and turning about its normal change nothing, so three of the six
+    parameters are unobservable; A is singular up to rounding and F7 reports status 3 instead of solving.  (Exact depth: the
+    normals are the plane's to rounding; on a structured scene the same gate stays far from its threshold.)"""
+    n = np.array([0.1, -0.2, 0.97], np.float64); n /= np.linalg.norm(n)
+    D = plane_depth_exact(K, W, H, n, 1.4)
+    pyr = fe.pyramid(D.astype(np.float32), K, 3)
+    A, _, _, cnt = fe.icp_step(pyr, pyr, K, 2, np.eye(4))
+    assert cnt > 3000 and fe.conditioning(A) < 1e-6
+    with pytest.raises(fe.TrackingLost) as e:
+        fe.track(pyr, pyr, K)
+    assert e.value.status == 3
+    meas, pred = scene_pair(np.eye(4))
+    A, _, _, _ = fe.icp_step(meas, pred, K, 0, np.eye(4))
+    assert fe.conditioning(A) > 1e-3
+    empty = [(np.zeros_like(d), np.zeros_like(v), np.zeros_like(nn)) for d, v, nn in pred]
+    with pytest.raises(fe.TrackingLost) as e:
+        fe.track(meas, empty, K)
+    assert e.value.status == 1
+
+
 def test_filtered_prediction_removes_voxel_steps():
     """F8: a plane with voxel-sized steps (what nearest-voxel ray casting leaves): unfiltered, most forward-difference normals
     miss the plane's normal by more than the ICP gate of 20 degrees; rounded to millimetres and filtered, nearly all agree."""
