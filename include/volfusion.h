@@ -29,6 +29,13 @@
  *     per-frame scratch of a volume -- control words, shell marks, work lists, pixel map, depth pyramid, staging sets,
  *     per-tile summaries -- exists once per volume, and two vol_integrate* / vol_frame_stats* / vol_raycast calls in
  *     flight on unordered streams would corrupt it (and the volumes).  Different vol_t are independent.
+ *   - Frames enqueued directly one after the other are pipelined: the first kernel of vol_integrate (the per-pixel
+ *     pre-pass, which reads only the frame and writes scratch kept in two sets) is a programmatic dependent launch, so
+ *     behind the fused kernel of the previous frame it starts as that kernel's thread blocks retire, and it completes
+ *     only after that kernel has.  Behind a copy, an event or any kernel that does not itself issue
+ *     griddepcontrol.launch_dependents it starts in plain stream order.  The one obligation this puts on a caller: a
+ *     kernel of the caller's own that PRODUCES the frame buffers, is enqueued immediately before vol_integrate and
+ *     issues griddepcontrol.launch_dependents must issue it after its last write to them (as for any dependent).
  */
 #ifndef VOLFUSION_H
 #define VOLFUSION_H

@@ -639,6 +639,7 @@ __global__ void __launch_bounds__(CTA, VF_MIN_CTAS) k_fused(const __grid_constan
     const int lane = threadIdx.x & 31;
     Stage &st = s_stage[threadIdx.x >> 5];
     pdl_wait();
+    pdl_launch_dependents();      // the next frame's pre-pass may fill the SMs as this grid's CTAs retire (k_prepass)
     uint32_t *ctrl = p.ctrl;
     const uint32_t n_tiles = (uint32_t)p.n_tiles;
     const uint32_t n_cls = (n_tiles + CLS_CHUNK - 1) / CLS_CHUNK, n_scan = (n_tiles + SCAN_CHUNK - 1) / SCAN_CHUNK;
@@ -654,7 +655,7 @@ __global__ void __launch_bounds__(CTA, VF_MIN_CTAS) k_fused(const __grid_constan
     //      chunk of a warp is its own number in the grid (no atomic: thousands of warps start at the same moment); every other
     //      chunk is claimed from a counter, so that no chunk ever waits for a warp that is busy with an item.
     if (phase != PHASE_COL) {
-        const uint32_t njobs = min(__ldcg(&ctrl[Q_NJOBS0 + p.parity]), p.jobs_cap);
+        const uint32_t njobs = min(__ldcg(&ctrl[Q_NJOBS]), p.jobs_cap);
         n_mark = (njobs + MARK_CHUNK - 1) / MARK_CHUNK;
         if (gw == 0 && lane == 0) ctrl[ST_NJOBS] = njobs;
         for (uint32_t k = gw; k < n_cls; k = n_cls <= n_warps ? n_cls : n_warps + claim(&ctrl[Q_CLS_CLAIM], lane)) {

@@ -70,7 +70,7 @@ struct Params {
     int       pyr_off[3], pyr_w[3], pyr_h[3], pyr_levels;   // levels: blocks of 8, 16, 32 pixels (fewer for tiny images)
     uint4    *jobs;              // shell-mark jobs of the frame (per 4 x 4 pixel patch: one, or one per strip, or one per pixel), jobs_cap entries
     uint32_t  jobs_cap;
-    int       parity;            // frame parity: which of the two job counters this frame uses (the other one is zeroed)
+    int       parity;            // frame parity: which of the two sets of per-frame scratch (pixmap, depthf, pyr, jobs) this frame uses
     uint32_t *work_geo;          // geometry work list (n_tiles entries, all zero between frames: a slot is cleared by the warp that takes it)
     uint32_t *marks;             // shell marks: words_per_tile(r) words per tile, bit = colour cell that may hold sigma-shell voxels
     uint2    *work_col;          // colour work list: one item per non-zero mark NIBBLE (up to 4 colour cells): {tile | nibble index, the nibble's
@@ -89,7 +89,8 @@ struct Params {
                                  // all): a conservative superset, used by the ray caster to skip free space
     uint8_t  *brick_neg;         // the same per brick of BRICK^3 geometry voxels (1 x 8 x 4 tiles): the ray caster's coarse level
     int       bricks_x, bricks_y, bricks_z;
-    uint32_t *ctrl;              // statistics record and queue control words, see ST_* / Q_* below
+    uint32_t *ctrl;              // statistics record and queue control words of this frame, see ST_* / Q_* below
+    uint32_t *ctrl_next;         // the next frame's block, cleared by this frame's pre-pass
     unsigned long long *counters;// voxel and sector counters (counting variant only), see CNT_*
 };
 
@@ -124,9 +125,14 @@ constexpr int CTRL_Q0 = 32;                                  // first queue-cont
 constexpr int QS = 32;
 enum { Q_CLS_CLAIM = CTRL_Q0, Q_CLS_DONE = CTRL_Q0 + QS, Q_MARK_CLAIM = CTRL_Q0 + 2 * QS, Q_MARK_DONE = CTRL_Q0 + 3 * QS,
        Q_SCAN_CLAIM = CTRL_Q0 + 4 * QS, Q_SCAN_DONE = CTRL_Q0 + 5 * QS, Q_GEO_CURSOR = CTRL_Q0 + 6 * QS, Q_COL_CURSOR = CTRL_Q0 + 7 * QS,
-       Q_NJOBS0 = CTRL_Q0 + 8 * QS, Q_NJOBS1 = Q_NJOBS0 + 1,
-       // min / max valid depth (mm) of the whole frame, two sets used alternately like the job counters
-       Q_DMIN0 = CTRL_Q0 + 9 * QS, Q_DMIN1, Q_DMAX0, Q_DMAX1, CTRL_N = CTRL_Q0 + 10 * QS };
+       Q_NJOBS = CTRL_Q0 + 8 * QS,
+       // min / max valid depth (mm) of the whole frame
+       Q_DMIN = CTRL_Q0 + 9 * QS, Q_DMAX, CTRL_N = CTRL_Q0 + 10 * QS };
+// There are CTRL_SETS such blocks, used in turn by successive frames.  The pre-pass of frame n accumulates into block
+// n % 3 (job counter, depth range) and cannot zero it first (its CTAs run in no particular order), so every pre-pass clears
+// the block of the frame AFTER it instead: (n + 1) % 3, last used by frame n - 2, which has completed -- frame n - 1 may
+// still be running when the pre-pass of frame n starts (see k_prepass), hence three blocks and not two.
+constexpr int CTRL_SETS = 3;
 constexpr int CLS_CHUNK = 32;                                // tiles per classification chunk (one lane each)
 constexpr int SCAN_CHUNK = 128;                              // tiles per scan chunk (four per lane)
 constexpr int MARK_CHUNK = 8;                                // mark jobs per chunk (4 lanes each)
@@ -162,7 +168,7 @@ __device__ __forceinline__ void depth_range(const Params &p, int x0, int x1, int
     int l = 0;
     while (l + 1 < p.pyr_levels && (((x1 >> (3 + l)) - (x0 >> (3 + l))) > 2 || ((y1 >> (3 + l)) - (y0 >> (3 + l))) > 2)) ++l;
     const int bx0 = x0 >> (3 + l), bx1 = x1 >> (3 + l), by0 = y0 >> (3 + l), by1 = y1 >> (3 + l);
-    if (bx1 - bx0 > 2 || by1 - by0 > 2) { mn = __ldcg(&p.ctrl[Q_DMIN0 + p.parity]); mx = __ldcg(&p.ctrl[Q_DMAX0 + p.parity]); return; }
+    if (bx1 - bx0 > 2 || by1 - by0 > 2) { mn = __ldcg(&p.ctrl[Q_DMIN]); mx = __ldcg(&p.ctrl[Q_DMAX]); return; }
     mn = 0xffffu; mx = 0u;
     const uint32_t *lev = p.pyr + p.pyr_off[l];
     const int lw = p.pyr_w[l];

@@ -131,15 +131,10 @@ __global__ void __launch_bounds__(256) k_prepass(const __grid_constant__ Params 
     pdl_launch_dependents();
     if (t < 16) { s_mn[t] = 0xffffu; s_mx[t] = 0u; }
     if (t == 0) s_njobs = 0u;
-    // statistics words and queue control of this frame start at zero (the previous frame's kernels have completed: this
-    // kernel is not a programmatic dependent launch)
-    // The job counter of the NEXT frame is zeroed here too, so that a frame that fails half-way never leaves a stale count
-    // behind for the frame that follows it.
-    if (blockIdx.x == 0 && blockIdx.y == 0) {
-        if (t < ST_N) p.ctrl[t] = 0u;
-        if (t < Q_NJOBS0 - CTRL_Q0 && t % QS == 0) p.ctrl[CTRL_Q0 + t] = 0u;
-        if (t == 0) { p.ctrl[Q_NJOBS0 + 1 - p.parity] = 0u; p.ctrl[Q_DMIN0 + 1 - p.parity] = 0xffffu; p.ctrl[Q_DMAX0 + 1 - p.parity] = 0u; }
-    }
+    // the control block of the NEXT frame starts at zero ("no valid depth yet" for the minimum); this frame's was cleared by the
+    // pre-pass before it (params.cuh, CTRL_SETS)
+    if (blockIdx.x == 0 && blockIdx.y == 0)
+        for (int i = t; i < CTRL_N; i += 256) p.ctrl_next[i] = i == Q_DMIN ? 0xffffu : 0u;
     __syncthreads();
     const int x = blockIdx.x * 32 + tx;
     uint32_t mn = 0xffffu, mx = 0u;
@@ -252,7 +247,7 @@ __global__ void __launch_bounds__(256) k_prepass(const __grid_constant__ Params 
     __syncthreads();
     {   // append this CTA's jobs to the frame's queue (one reservation per CTA)
         const uint32_t njobs = s_njobs;
-        if (t == 0) s_base = njobs ? atomicAdd(&p.ctrl[Q_NJOBS0 + p.parity], njobs) : 0u;
+        if (t == 0) s_base = njobs ? atomicAdd(&p.ctrl[Q_NJOBS], njobs) : 0u;
         __syncthreads();
         for (uint32_t j = (uint32_t)t; j < njobs; j += 256u)
             if (s_base + j < p.jobs_cap) p.jobs[s_base + j] = s_jobs[j];       // (always true: at most one job per pixel)
@@ -281,8 +276,13 @@ __global__ void __launch_bounds__(256) k_prepass(const __grid_constant__ Params 
         uint32_t a_mn = 0xffffu, a_mx = 0u;
         for (int a = 0; a < 16; ++a) { a_mn = min(a_mn, s_mn[a]); a_mx = max(a_mx, s_mx[a]); }
         if (p.pyr_levels > 2) p.pyr[p.pyr_off[2] + blockIdx.y * p.pyr_w[2] + blockIdx.x] = a_mn | (a_mx << 16);
-        if (a_mx != 0u) { atomicMin(&p.ctrl[Q_DMIN0 + p.parity], a_mn); atomicMax(&p.ctrl[Q_DMAX0 + p.parity], a_mx); }
+        if (a_mx != 0u) { atomicMin(&p.ctrl[Q_DMIN], a_mn); atomicMax(&p.ctrl[Q_DMAX], a_mx); }
     }
+    // This kernel is itself a programmatic dependent launch: it reads only the frame and writes only this frame's scratch set
+    // and control block, so its CTAs may run beside the last warps of the previous frame's fused kernel.  It must not
+    // COMPLETE before that kernel has, though: this frame's fused kernel waits for this grid alone, and it works on the
+    // volumes and the work lists the previous one is still using.
+    pdl_wait();
 }
 
 // camera-space centre of geometry tile (ttx, tty, ttz local) -- culling only

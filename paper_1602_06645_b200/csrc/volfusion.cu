@@ -48,13 +48,21 @@ struct vol {
     // fused-kernel launch shape
     int n_sms, fused_blocks;
     bool counting, profiling;
-    unsigned frame_seq;             // frames enqueued so far: its parity selects the job counter (Params::parity)
+    unsigned frame_seq;             // frames enqueued so far: selects the scratch set (parity) and the control block (mod CTRL_SETS)
+    // per-frame scratch, two sets used alternately (Params::pixmap, depthf, pyr, jobs point into set frame_seq & 1), and the
+    // CTRL_SETS control blocks (Params::ctrl = ctrl_base + (frame_seq % CTRL_SETS) * CTRL_N): the pre-pass of a frame may run
+    // while the fused kernel of the frame before it is still reading its own set
+    float4 *scr_pixmap[2]; float *scr_depthf[2]; uint32_t *scr_pyr[2]; uint4 *scr_jobs[2];
+    uint32_t *ctrl_base, *ctrl_last;    // ctrl_last: block of the most recent frame (vol_frame_stats*)
     cudaEvent_t ev[4];
     bool ev_valid;
     // vol_integrate_host: the frames are copied on a stream of the library's own
     cudaStream_t copy_stream;
 };
 
+#ifndef VF_PIPELINE
+#define VF_PIPELINE true
+#endif
 // one kernel launch; `dependent` = programmatic dependent launch on the previous kernel of the stream
 template <typename... Args>
 static cudaError_t launch(void (*kernel)(const Params, Args...), dim3 grid, int block, cudaStream_t s, bool dependent, const Params &p, Args... args)
@@ -241,10 +249,12 @@ extern "C" int vol_create(vol_t **out, const int32_t dims_geo[3], int32_t r, con
     // one 128-byte statistics record (8 words, then 12 counters: read back together by vol_frame_stats*), then the queue control words
     static_assert(sizeof(uint32_t) * vf::ST_N + sizeof(unsigned long long) * vf::CNT_N == VOL_STATS_RAW_BYTES && vf::CTRL_Q0 * 4 == VOL_STATS_RAW_BYTES,
                   "raw statistics record: 8 words, then 12 counters");
-    if (cudaMalloc(&p.ctrl, sizeof(uint32_t) * vf::CTRL_N) != cudaSuccess) rc = VOL_E_OOM;
+    if (cudaMalloc(&v->ctrl_base, sizeof(uint32_t) * vf::CTRL_N * vf::CTRL_SETS) != cudaSuccess) rc = VOL_E_OOM;
+    if (rc == VOL_OK && cudaMemset(v->ctrl_base, 0, sizeof(uint32_t) * vf::CTRL_N * vf::CTRL_SETS) != cudaSuccess) rc = VOL_E_CUDA;
+    for (int i = 0; i < vf::CTRL_SETS && rc == VOL_OK; ++i)                                                 // "no valid depth yet"
+        if (cudaMemset(v->ctrl_base + i * vf::CTRL_N + vf::Q_DMIN, 0xff, sizeof(uint32_t)) != cudaSuccess) rc = VOL_E_CUDA;
+    if (rc == VOL_OK) { p.ctrl = v->ctrl_base; p.ctrl_next = v->ctrl_base + vf::CTRL_N; v->ctrl_last = v->ctrl_base; }
     if (rc == VOL_OK) p.counters = reinterpret_cast<unsigned long long *>(p.ctrl + vf::ST_N);
-    if (rc == VOL_OK && cudaMemset(p.ctrl, 0, sizeof(uint32_t) * vf::CTRL_N) != cudaSuccess) rc = VOL_E_CUDA;
-    if (rc == VOL_OK && cudaMemset(p.ctrl + vf::Q_DMIN0, 0xff, sizeof(uint32_t) * 2) != cudaSuccess) rc = VOL_E_CUDA;   // "no valid depth yet"
     if (rc != VOL_OK) { cudaGetLastError(); return fail(rc); }
 
     cudaDeviceProp prop;
@@ -268,6 +278,17 @@ extern "C" int vol_create(vol_t **out, const int32_t dims_geo[3], int32_t r, con
     return VOL_OK;
 }
 
+static void free_scratch(vol *v)
+{
+    for (int i = 0; i < 2; ++i) {
+        if (v->scr_pixmap[i]) cudaFree(v->scr_pixmap[i]);
+        if (v->scr_pyr[i]) cudaFree(v->scr_pyr[i]);
+        if (v->scr_depthf[i]) cudaFree(v->scr_depthf[i]);
+        if (v->scr_jobs[i]) cudaFree(v->scr_jobs[i]);
+        v->scr_pixmap[i] = nullptr; v->scr_pyr[i] = nullptr; v->scr_depthf[i] = nullptr; v->scr_jobs[i] = nullptr;
+    }
+}
+
 extern "C" void vol_destroy(vol_t *v)
 {
     if (!v) return;
@@ -278,16 +299,13 @@ extern "C" void vol_destroy(vol_t *v)
     if (v->p.work_geo) cudaFree(v->p.work_geo);
     if (v->p.work_col) cudaFree(v->p.work_col);
     if (v->p.marks) cudaFree(v->p.marks);
-    if (v->p.jobs) cudaFree(v->p.jobs);
     if (v->p.tile_neg) cudaFree(v->p.tile_neg);
     if (v->p.tile_sat) cudaFree(v->p.tile_sat);
     if (v->p.tile_skip) cudaFree(v->p.tile_skip);
     for (int i = 0; i < 4; ++i) if (v->p.sec_map[i]) cudaFree(v->p.sec_map[i]);
     if (v->p.brick_neg) cudaFree(v->p.brick_neg);
-    if (v->p.ctrl) cudaFree(v->p.ctrl);
-    if (v->p.pixmap) cudaFree(v->p.pixmap);
-    if (v->p.pyr) cudaFree(v->p.pyr);
-    if (v->p.depthf) cudaFree(v->p.depthf);
+    if (v->ctrl_base) cudaFree(v->ctrl_base);
+    free_scratch(v);
     for (int i = 0; i < N_STAGE; ++i) {
         if (v->stage_depth[i]) cudaFree(v->stage_depth[i]);
         if (v->stage_rgb[i]) cudaFree(v->stage_rgb[i]);
@@ -301,20 +319,15 @@ extern "C" void vol_destroy(vol_t *v)
     delete v;
 }
 
-// (re)allocate the per-frame-size scratch: pixel map + depth pyramid
+// (re)allocate the per-frame-size scratch (both sets): pixel map, float depth map, depth pyramid, shell-mark jobs
 static int ensure_scratch(vol *v, int wd, int hd)
 {
-    if (v->scratch_wd == wd && v->scratch_hd == hd && v->p.pixmap) return VOL_OK;
+    if (v->scratch_wd == wd && v->scratch_hd == hd && v->scr_pixmap[0]) return VOL_OK;
     Params &p = v->p;
     v->scratch_wd = v->scratch_hd = 0;                       // nothing is valid until every allocation below has succeeded
-    if (p.pixmap) { CK(cudaDeviceSynchronize()); cudaFree(p.pixmap); p.pixmap = nullptr; }
-    if (p.pyr) { cudaFree(p.pyr); p.pyr = nullptr; }
-    if (p.depthf) { cudaFree(p.depthf); p.depthf = nullptr; }
-    if (p.jobs) { cudaFree(p.jobs); p.jobs = nullptr; }
-    CK(cudaMalloc(&p.depthf, sizeof(float) * (size_t)wd * hd));
+    if (v->scr_pixmap[0]) CK(cudaDeviceSynchronize());
+    free_scratch(v);
     p.jobs_cap = (uint32_t)((size_t)((wd + 3) / 4 * 4) * (size_t)((hd + 3) / 4 * 4));     // one per pixel at most
-    CK(cudaMalloc(&p.jobs, sizeof(uint4) * (size_t)p.jobs_cap));
-    CK(cudaMalloc(&p.pixmap, sizeof(float4) * (size_t)wd * hd));
     int l = 0; size_t off = 0;
     for (; l < 3; ++l) {                                     // blocks of 8, 16, 32 pixels
         const int bs = 8 << l;
@@ -323,7 +336,12 @@ static int ensure_scratch(vol *v, int wd, int hd)
     }
     p.pyr_levels = 3;
     v->pyr_entries = off;
-    CK(cudaMalloc(&p.pyr, sizeof(uint32_t) * off));
+    for (int i = 0; i < 2; ++i) {
+        CK(cudaMalloc(&v->scr_depthf[i], sizeof(float) * (size_t)wd * hd));
+        CK(cudaMalloc(&v->scr_jobs[i], sizeof(uint4) * (size_t)p.jobs_cap));
+        CK(cudaMalloc(&v->scr_pixmap[i], sizeof(float4) * (size_t)wd * hd));
+        CK(cudaMalloc(&v->scr_pyr[i], sizeof(uint32_t) * off));
+    }
     v->scratch_wd = wd; v->scratch_hd = hd;
     return VOL_OK;
 }
@@ -357,6 +375,10 @@ static int integrate_impl(vol_t *v, const uint16_t *depth_u16_dev, int32_t wd, i
     box_extents(p.R, 0.5 * vf::TX * p.vs, 0.5 * vf::TY * p.vs, 0.5 * vf::TZ * p.vs, slack, p.tile_ex, p.tile_ey, p.tile_ez);
     box_extents(p.R, 0.5 * (vf::TX / vf::SUBX) * p.vs, 0.5 * vf::TY * p.vs, 0.5 * (vf::TZ / vf::SUBZ) * p.vs, slack, p.sub_ex, p.sub_ey, p.sub_ez);
     p.parity = (int)(v->frame_seq & 1u);
+    p.pixmap = v->scr_pixmap[p.parity]; p.depthf = v->scr_depthf[p.parity]; p.pyr = v->scr_pyr[p.parity]; p.jobs = v->scr_jobs[p.parity];
+    p.ctrl = v->ctrl_base + (size_t)(v->frame_seq % (unsigned)vf::CTRL_SETS) * vf::CTRL_N;
+    p.ctrl_next = v->ctrl_base + (size_t)((v->frame_seq + 1u) % (unsigned)vf::CTRL_SETS) * vf::CTRL_N;
+    p.counters = reinterpret_cast<unsigned long long *>(p.ctrl + vf::ST_N);
     p.counting = v->counting ? 1 : 0;
     p.sigma_g = (float)((double)p.sigma * 1.0001 + slack);
     camera_to_world(p.R, p.t, p.Rw, p.tw);
@@ -372,14 +394,16 @@ static int integrate_impl(vol_t *v, const uint16_t *depth_u16_dev, int32_t wd, i
     const dim3 g0((wd + 31) / 32, (hd + 31) / 32);
     const int g2 = v->fused_blocks;
     const bool cnt = v->counting;
-    // k_fused is launched with programmatic stream serialization: its CTAs may be scheduled while the pre-pass drains (it
-    // signals griddepcontrol.launch_dependents), and they wait for its completion and memory flush with griddepcontrol.wait
-    // before touching anything it wrote.
+    // Both kernels are launched with programmatic stream serialization.  k_fused's CTAs may be scheduled while the pre-pass
+    // drains (it signals griddepcontrol.launch_dependents), and they wait for its completion and memory flush with
+    // griddepcontrol.wait before touching anything it wrote.  The pre-pass of the NEXT frame, if it follows directly on the
+    // stream, may start while this frame's k_fused is running out of work -- it touches nothing that kernel uses (scratch
+    // set, control block) and does not complete before it (k_prepass); behind anything else it starts in stream order.
 #define VF_LAUNCH(RR)                                                                   \
     do {                                                                                \
         const FusedFn kf = fused_kernel<RR>(cnt, p.variant);                            \
-        CK(launch(vf::k_prepass<RR>, g0, 256, s, false, p));                            \
-        ++v->frame_seq;                                                                 \
+        CK(launch(vf::k_prepass<RR>, g0, 256, s, VF_PIPELINE, p));                            \
+        ++v->frame_seq; v->ctrl_last = p.ctrl;                                          \
         if (v->profiling) { CK(cudaEventRecord(v->ev[1], s)); CK(cudaEventRecord(v->ev[2], s)); } \
         if (rgb_ready) {   /* everything but the colour items now, those once the HD frame has arrived */ \
             CK(launch(kf, dim3(g2), vf::CTA, s, true, p, (int)vf::PHASE_GEO));          \
@@ -639,7 +663,7 @@ extern "C" int vol_frame_stats_async(vol_t *v, void *raw_host, void *stream)
     if (!v || !raw_host) return VOL_E_ARG;
     int rc = set_device(v); if (rc) return rc;
     cudaStream_t s = (cudaStream_t)stream;
-    CK(cudaMemcpyAsync(raw_host, v->p.ctrl, VOL_STATS_RAW_BYTES, cudaMemcpyDeviceToHost, s));
+    CK(cudaMemcpyAsync(raw_host, v->ctrl_last, VOL_STATS_RAW_BYTES, cudaMemcpyDeviceToHost, s));
     return VOL_OK;
 }
 

@@ -73,11 +73,14 @@ def run_sequence(c, frames, counting=True, check_every=1, **kw):
     return g, o
 
 
-def sampled_full_size(c, frames, n_cols, seed, alternate_host=False, variant=0, frame_fn=None, mu=None, sigma=None, expect_colour=True):
+def sampled_full_size(c, frames, n_cols, seed, alternate_host=False, variant=0, frame_fn=None, mu=None, sigma=None, expect_colour=True,
+                      burst=0):
     """Full-size volumes in the launch configuration bench.py times (device-resident frames, counters off), compared on a
     seeded sample: every voxel of n_cols random 8 x 8 (x, y) geometry columns and all their colour children.  Voxels never
     interact, so the oracle run on the sample alone gives their exact state (ref_integrate_subset).
-    frame_fn(c, i) supplies frame i (default: the configuration's scan); mu / sigma override the configuration's."""
+    frame_fn(c, i) supplies frame i (default: the configuration's scan); mu / sigma override the configuration's.
+    burst > 0: the frames are made resident `burst` at a time and then enqueued with nothing between the calls, as in
+    bench.py's timed region (the next frame's pre-pass then runs under the tail of the fused kernel)."""
     import paper_1602_06645_b200 as vf
     frame_fn = frame_fn or synth.frame
     mu = c.mu if mu is None else mu
@@ -98,9 +101,19 @@ def sampled_full_size(c, frames, n_cols, seed, alternate_host=False, variant=0, 
     o = oracle.RefVolume(c.dims_geo, r, c.origin, c.extent, mu, c.w_max, sigma=sigma, allocate=False, variant=variant)
     g = vf.Volume(c.dims_geo, r, c.origin, c.extent, mu, c.w_max, sigma=sigma, variant=variant)
     try:
+        pending = []
         for n, fi in enumerate(frames):
             depth, rgb, T = frame_fn(c, fi)
-            if alternate_host and n % 2:                          # every other frame through vol_integrate_host
+            if burst:
+                pending.append((to_dev(depth), to_dev(rgb), T))
+                if len(pending) == burst or n == len(frames) - 1:
+                    import torch
+                    torch.cuda.synchronize()
+                    for dd, dr, Tp in pending:
+                        g.integrate(dd, c.wd, c.hd, dr, c.wh, c.hh, Tp, c.K_depth, c.K_rgb, c.T_depth_rgb)
+                    torch.cuda.synchronize()
+                    pending = []
+            elif alternate_host and n % 2:                          # every other frame through vol_integrate_host
                 g.integrate_host(depth, rgb, T, c.K_depth, c.K_rgb, c.T_depth_rgb)
             else:
                 g.integrate(to_dev(depth), c.wd, c.hd, to_dev(rgb), c.wh, c.hh, T, c.K_depth, c.K_rgb, c.T_depth_rgb)

@@ -174,6 +174,43 @@ def test_host_frames_enqueued_back_to_back():
         compare_states(g, o, f"back to back, repeat {rep}")
 
 
+def test_device_frames_pipelined_back_to_back():
+    """vol_integrate with device-resident frames enqueued directly one after the other: the pre-pass of frame n + 1 is a
+    programmatic dependent launch and runs under the tail of frame n's fused kernel (two scratch sets, three control
+    blocks).  24 frames of config 3's noisy orbit (the volume large enough for the fused kernel to run for tens of
+    microseconds), no counters, nothing between the calls, on a stream of its own, repeated.  The state must equal the oracle's, byte for byte, every time; and the
+    statistics record read back asynchronously after a frame must be that frame's even when two more frames follow it."""
+    import torch
+    c = synth.config(3).scaled(192, 2)
+    frames = [synth.frame(c, fi) for fi in range(0, 240, 10)]
+    g, o = make_pair(c)
+    for d, rgb, T in frames:
+        o.integrate(d, rgb, T, c.K_depth, c.K_rgb, c.T_depth_rgb)
+    dev = [(to_dev(d), to_dev(rgb), T) for d, rgb, T in frames]
+    stream = torch.cuda.Stream()
+    torch.cuda.synchronize()
+    for rep in range(4):
+        g.reset(stream)
+        for dd, dr, T in dev:
+            g.integrate(dd, c.wd, c.hd, dr, c.wh, c.hh, T, c.K_depth, c.K_rgb, c.T_depth_rgb, stream=stream)
+        stream.synchronize()
+        compare_states(g, o, f"pipelined, repeat {rep}")
+    # statistics of frame n, read in stream order, while frames n + 1 and n + 2 are already enqueued behind it
+    g.reset(stream)
+    raw = torch.zeros((len(dev), 16), dtype=torch.int64).pin_memory()
+    for n, (dd, dr, T) in enumerate(dev):
+        g.integrate(dd, c.wd, c.hd, dr, c.wh, c.hh, T, c.K_depth, c.K_rgb, c.T_depth_rgb, stream=stream)
+        g.frame_stats_async(raw[n], stream)
+    stream.synchronize()
+    tiles = [g.decode_stats(raw[n]).tiles_geo for n in range(len(dev))]
+    g.reset(stream)
+    for n, (dd, dr, T) in enumerate(dev):
+        g.integrate(dd, c.wd, c.hd, dr, c.wh, c.hh, T, c.K_depth, c.K_rgb, c.T_depth_rgb, stream=stream)
+        assert g.frame_stats(stream).tiles_geo == tiles[n] > 0, n
+    compare_states(g, o, "with statistics")
+    g.close()
+
+
 def test_shards_reassemble_to_the_unsharded_volume():
     """z-slab sharding (VOL_SLAB layers dealt round-robin): two shards run one after the other on this GPU hold exactly
     the slabs of the unsharded result; no voxel is owned twice or dropped."""
@@ -229,6 +266,13 @@ def test_cfg3_full_size_whole_sequence_sampled():
     alternating between the device and the host entry point; geometry weights reach w_max = 128 on the way."""
     ng, nc = _sampled_full_size(synth.config(3), range(300), 40, 31, alternate_host=True)
     assert ng > 100000 and nc > 100000
+
+
+def test_cfg3_full_size_pipelined_sampled():
+    """The benchmark workload the way bench.py's timed region runs it: device-resident frames, 16 at a time, enqueued with
+    nothing between the calls (the pre-pass of frame n + 1 under the tail of frame n's fused kernel), 64 frames."""
+    ng, nc = _sampled_full_size(synth.config(3), range(64), 40, 33, burst=16)
+    assert ng > 100000 and nc > 30000
 
 
 def test_cfg2_cfg4_cfg5_full_size_whole_sequences_sampled():
