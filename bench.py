@@ -1,15 +1,22 @@
 #!/usr/bin/env python
 """bench.py -- fused TSDF + colour-volume integration throughput on B200 (one JSON line on stdout).
 
-A *step* is one pass of the whole hot path (S0-S9: pre-pass, tile classification, fused integrate) over one synthetic
-RGB-D frame.  Workload at N = 1: BASELINE.json configs[2] ("cfg3": geometry 512^3 over a 3 m cube, colour 1024^3,
-640x480 depth, 1920x1080 RGB, 20 primitives on a plane, jittered orbit) -- the configuration the 70 % target is quoted on.
+A *step* is one pass of the whole hot path (S0-S9: per-pixel pre-pass, then ONE persistent fused kernel that classifies
+tiles, sets and scans the shell marks and integrates both volumes) over one synthetic RGB-D frame.  Workload at N = 1:
+BASELINE.json configs[2] ("cfg3": geometry 512^3 over a 3 m cube, colour 1024^3, 640x480 depth, 1920x1080 RGB, 20
+primitives on a plane, jittered orbit) -- the configuration the 70 % target is quoted on.
 
-  value     whole-job voxel updates/s = (N_geo + N_col) voxels brought up to date per frame x frames / device time,
-            inputs resident in HBM, CUDA events on the launching stream, L2 flushed between timed frames
+  value     whole-job voxel updates/s = (N_geo + N_col) voxels brought up to date per frame x frames / device time:
+            exactly K steps enqueued one after the other between two CUDA events on the launching stream, inputs resident
+            in HBM.  No L2 flush: the K frames differ and every step touches > 100 MB of volumes of 2.7 GB.
+  flushed   the same K frames timed one by one with a 512 MiB flush before each (round 1's method; per_frame_ms)
+  steady_state  the same after the arc has been swept until the weights are saturated (gate closed, stores skipped)
+  stress    three saturating frames: free space, inside the truncation band, colour shell
   e2e       the same metric through vol_integrate_host (pinned HOST frames copied in, per-frame stats copied out)
-  roofline  fused kernel: algorithmic bytes per launch (4 B x voxels read + 4 B x voxels changed + the two input images)
-            / its mean launch time (CUDA events inside the library), against the measured HBM copy peak
+  roofline  fused kernel: algorithmic bytes per launch (4 B x voxels read + 4 B x voxels changed + the two input images;
+            sector_exact: 32 B x sectors touched) / its mean launch time (CUDA events inside the library, one frame at a
+            time), against the measured HBM copy peak; step_frac: the same bytes over the whole step; traffic / issue: ncu
+            figures from profiles/traffic.csv, quoted only if captured with the kernel sources this run was built from
   cpu_baseline  the CPU oracle, as it stands, on the first full-size frames of the same workload (rank 0, N = 1 only)
 
 N > 1 (torchrun): every rank integrates an independent scan of the same configuration (replicas, no data-path
