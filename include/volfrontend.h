@@ -96,6 +96,24 @@ int vol_frontend_track(vol_frontend_t *fe, const float T_init[16], const int32_t
  * vol_frontend_track; every pointer nullable.  HOST values, no device work. */
 int vol_frontend_track_info(const vol_frontend_t *fe, int32_t *status_out, int32_t *level_out, double *conditioning_out);
 
+/* One F5 step that ALLOCATES NOTHING -- for callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving
+ * loops, harnesses that forbid it).  No front-end object: the caller passes the maps of one level and receives the sums, all
+ * DEVICE memory.  V_dev / N_dev: vertex and normal map of the current (measured) frame, Vp_dev / Np_dev: of the prediction;
+ * each w*h pixels of 4 floats (x, y, z, 0), 16-byte aligned, row-major, invalid = normal (0, 0, 0) -- the layout the front end
+ * keeps on the device.  K: HOST, intrinsics of THIS level.  T_pred_cur: HOST, current camera -> prediction camera.  dist_m /
+ * cos_min: the F5 gates (<= 0 selects 0.10 / 0.94).  sums_dev: DEVICE, VOL_ICP_SUMS doubles, written in stream order.
+ * Asynchronous on `stream`; calls no cudaMalloc, cudaFree, cudaMallocHost or any other allocating routine, and does not
+ * synchronise.  The same sums as vol_frontend_icp_step up to binary64 summation order (blocks' partial sums are added in a
+ * fixed order, so the result is bit-reproducible as well).
+ * Limit: the step's scratch (29 doubles per block of 32 x 8 pixels) is a static device array of VOL_ICP_STATIC_MAX_BLOCKS
+ * slots, 1.8 MiB, held by every GPU that loads the library until the process exits; ceil(w / 32) * ceil(h / 8) beyond that
+ * is VOL_E_TOOBIG (vol_strerror names the sizes) -- 8192 blocks cover maps up to 1920 x 1088 or 2048 x 1024.  The device is
+ * the CURRENT device (ordinals 0..63).  ALL calls share the one array per device: calls that may overlap on the GPU (two
+ * streams, two host threads on two streams) RACE on it and return garbage; order them on one stream or with events. */
+#define VOL_ICP_STATIC_MAX_BLOCKS 8192
+int vol_icp_step_static(const float *V_dev, const float *N_dev, const float *Vp_dev, const float *Np_dev, int32_t w, int32_t h,
+                        const float K[9], const float T_pred_cur[16], float dist_m, float cos_min, double *sums_dev, void *stream);
+
 /* Copy the maps of one level to the host (tests, debugging): which = 0 measured, 1 predicted; depth_host: wl*hl floats,
  * vertex_host / normal_host: wl*hl*3 floats; any may be NULL.  Synchronises `stream`. */
 int vol_frontend_maps(const vol_frontend_t *fe, int32_t which, int32_t level, float *depth_host, float *vertex_host,

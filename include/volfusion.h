@@ -55,6 +55,7 @@ extern "C" {
 #define VOL_E_LOST  -4   /* vol_frontend_track only: the arguments were valid but the pose could not be estimated (too few
                             correspondences, normal equations not positive definite or too close to singular); the
                             volumes and the front end are intact and the caller may re-localise or skip the frame */
+#define VOL_E_TOOBIG -5  /* vol_icp_step_static only: the maps need more scratch than the fixed static array holds */
 
 /* geometry layers per shard slab (and per culling tile along z): rank `shard_rank` of `shard_world` owns the
  * geometry layers k with (k / VOL_SLAB) % shard_world == shard_rank, and the r*VOL_SLAB colour layers under each */

@@ -19,7 +19,7 @@ _SRC_DIR = os.path.join(_HERE, "csrc")
 _SO = os.path.join(_HERE, "libvolfusion.so")
 _lib = None
 
-VOL_OK, VOL_E_ARG, VOL_E_OOM, VOL_E_CUDA, VOL_E_LOST = 0, -1, -2, -3, -4
+VOL_OK, VOL_E_ARG, VOL_E_OOM, VOL_E_CUDA, VOL_E_LOST, VOL_E_TOOBIG = 0, -1, -2, -3, -4, -5
 VOL_SLAB = 8
 VOL_STATS_RAW_BYTES = 128
 
@@ -31,7 +31,8 @@ EXPORTS = ["vol_create", "vol_integrate", "vol_integrate_host", "vol_raycast", "
            "vol_launches_per_frame", "vol_selftest", "vol_destroy", "vol_strerror",
            # include/volfrontend.h
            "vol_frontend_create", "vol_frontend_destroy", "vol_frontend_measure", "vol_frontend_predict_depth", "vol_frontend_predict",
-           "vol_frontend_icp_step", "vol_frontend_track", "vol_frontend_track_info", "vol_frontend_maps"]
+           "vol_frontend_icp_step", "vol_frontend_track", "vol_frontend_track_info", "vol_frontend_maps",
+           "vol_icp_step_static"]
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
@@ -117,6 +118,7 @@ def lib():
         L.vol_frontend_track.argtypes = [P, P, P, P, P, P, P]
         L.vol_frontend_track_info.argtypes = [P, P, P, P]
         L.vol_frontend_maps.argtypes = [P, I32, I32, P, P, P, P]
+        L.vol_icp_step_static.argtypes = [P, P, P, P, I32, I32, P, P, F, F, P, P]
         for name in EXPORTS:
             if name not in ("vol_destroy", "vol_strerror", "vol_frontend_destroy"):
                 getattr(L, name).restype = ctypes.c_int
@@ -313,6 +315,17 @@ class FrontendOpts(ctypes.Structure):
 
 
 ICP_SUMS = 29
+
+
+ICP_STATIC_MAX_BLOCKS = 8192
+
+
+def icp_step_static(V, N, Vp, Np, w, h, K, T_pred_cur, sums_out, dist_m=0.0, cos_min=0.0, stream=None):
+    """vol_icp_step_static: one F5 step without any allocation.  V, N, Vp, Np: CUDA float32 tensors of w*h*4 (x, y, z, 0);
+    K: intrinsics of this level; sums_out: CUDA float64 tensor of ICP_SUMS, written in stream order (asynchronous)."""
+    Kc, T = _f32(K, 9), _f32(T_pred_cur, 16)
+    _check(lib().vol_icp_step_static(_dev_ptr(V), _dev_ptr(N), _dev_ptr(Vp), _dev_ptr(Np), int(w), int(h), Kc.ctypes.data, T.ctypes.data,
+                                     float(dist_m), float(cos_min), _dev_ptr(sums_out), _stream_ptr(stream)), "vol_icp_step_static")
 
 
 class Frontend:

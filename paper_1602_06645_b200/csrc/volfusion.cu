@@ -156,6 +156,7 @@ extern "C" const char *vol_strerror(int code)
         case VOL_E_OOM: return g_err[0] ? g_err : "out of device memory";
         case VOL_E_CUDA: return g_err[0] ? g_err : "CUDA error";
         case VOL_E_LOST: return g_err[0] ? g_err : "tracking lost";
+        case VOL_E_TOOBIG: return g_err[0] ? g_err : "input larger than the static scratch";
         default: return "unknown error code";
     }
 }
@@ -798,3 +799,4 @@ extern "C" int vol_trace_dump(unsigned long long *host)
 #endif
 
 #include "frontend_host.cuh"
+#include "noalloc.cuh"
