@@ -115,7 +115,8 @@ __device__ __forceinline__ bool shell_box(const Params &p, float xa, float xb, f
 //      larger than a compact piece's (a smooth surface seen head-on).  Otherwise the patch is cut into its 4 rows or its 4
 //      columns, whichever have the smaller depth ranges (a surface seen at a grazing angle: the pieces of the strips are
 //      staggered along the view direction, and their boxes follow the shear that one box for the patch would fill in) --
-//      or, if even those ranges exceed STRIP_RANGE_MAX (a depth edge), into its pixels.
+//      or, if even those ranges exceed STRIP_RANGE_MAX (a depth edge), into its pixels.  (With a sigma so large that even a compact
+//      patch's box spans more than MARK_FINE_MAX cells, the patches of a CTA's 32 x 32 region are merged into one job.)
 //      The fused kernel's warps turn the jobs into marks: bits of the colour cells that meet a job's box.  Marks are
 //      consumed (and cleared) by the fused kernel.
 constexpr float PATCH_SPREAD_MAX = 2.4f, STRIP_RANGE_MAX = 0.02f;
@@ -125,12 +126,12 @@ template <int R>
 __global__ void __launch_bounds__(256) k_prepass(const __grid_constant__ Params p)
 {
     __shared__ uint32_t s_mn[16], s_mx[16];
-    __shared__ uint32_t s_njobs, s_base;
+    __shared__ uint32_t s_njobs, s_base, s_rlo, s_rhi;      // s_rlo / s_rhi: depth range (float bits) of the region job, see (c)
     __shared__ uint4 s_jobs[1024];      // mark jobs: {x | y << 15 | JOB_* << 30 of the first pixel, depth range of its eligible pixels}
     const int t = threadIdx.x, tx = t & 31, tq = t >> 5;
     pdl_launch_dependents();
     if (t < 16) { s_mn[t] = 0xffffu; s_mx[t] = 0u; }
-    if (t == 0) s_njobs = 0u;
+    if (t == 0) { s_njobs = 0u; s_rlo = 0x7f800000u; s_rhi = 0u; }
     // the control block of the NEXT frame starts at zero ("no valid depth yet" for the minimum); this frame's was cleared by the
     // pre-pass before it (params.cuh, CTRL_SETS)
     if (blockIdx.x == 0 && blockIdx.y == 0)
@@ -223,7 +224,12 @@ __global__ void __launch_bounds__(256) k_prepass(const __grid_constant__ Params 
                 const float c = (float)CLY * p.vc, wfoot = 4.0f * zhi / p.fx;
                 const float n0 = (2.0f * p.sigma / c + 2.0f) * (wfoot / c + 2.0f) * (0.5f * wfoot / c + 2.0f);
                 const uint32_t xy = (uint32_t)xp | ((uint32_t)yp << 15);
-                if ((float)ncell <= PATCH_SPREAD_MAX * n0) {
+                if (n0 > (float)MARK_FINE_MAX) {
+                    // sigma is so large that even a compact patch's box spans thousands of cells (mark_box then works tile
+                    // by tile): the boxes of neighbouring patches are nearly the same, and the CTA's whole 32 x 32 region
+                    // becomes ONE job with the union of their depth ranges (positive floats order like their bit patterns)
+                    if ((tx & 3) == 0) { atomicMin(&s_rlo, __float_as_uint(zlo)); atomicMax(&s_rhi, __float_as_uint(zhi)); }
+                } else if ((float)ncell <= PATCH_SPREAD_MAX * n0) {
                     if ((tx & 3) == 0) s_jobs[atomicAdd(&s_njobs, 1u)] = make_uint4(xy | ((uint32_t)JOB_PATCH << 30), __float_as_uint(zlo), __float_as_uint(zhi), 0u);
                 } else if (fminf(rmax, cmax) <= STRIP_RANGE_MAX) {
                     if (rmax <= cmax) {                               // rows: lane m of the patch queues row m
@@ -244,6 +250,9 @@ __global__ void __launch_bounds__(256) k_prepass(const __grid_constant__ Params 
             }
         }
     }
+    __syncthreads();
+    if (t == 0 && s_rhi >= s_rlo && s_rhi != 0u)             // the region job: fourth word = 1
+        s_jobs[s_njobs++] = make_uint4((uint32_t)(blockIdx.x * 32) | ((uint32_t)(blockIdx.y * 32) << 15) | ((uint32_t)JOB_PATCH << 30), s_rlo, s_rhi, 1u);
     __syncthreads();
     {   // append this CTA's jobs to the frame's queue (one reservation per CTA)
         const uint32_t njobs = s_njobs;
@@ -393,7 +402,8 @@ __device__ __forceinline__ void mark_chunk(const Params &p, uint32_t chunk, uint
     const uint4 job = __ldcg(p.jobs + j);
     const float xa = (float)(job.x & 0x7fffu), ya = (float)((job.x >> 15) & 0x7fffu);
     const uint32_t shape = job.x >> 30;
-    const float ex = shape == JOB_PATCH || shape == JOB_ROW ? 3.0f : 0.0f, ey = shape == JOB_PATCH || shape == JOB_COLUMN ? 3.0f : 0.0f;
+    float ex = shape == JOB_PATCH || shape == JOB_ROW ? 3.0f : 0.0f, ey = shape == JOB_PATCH || shape == JOB_COLUMN ? 3.0f : 0.0f;
+    if (job.w != 0u) { ex = fminf(31.0f, p.wd_f - 1.0f - xa); ey = fminf(31.0f, p.hd_f - 1.0f - ya); }      // a CTA's 32 x 32 region (k_prepass)
     int i0, i1, j0, j1, k0, k1;
     if (shell_box(p, xa, xa + ex, ya, ya + ey, __uint_as_float(job.y), __uint_as_float(job.z), i0, i1, j0, j1, k0, k1))
         mark_box<R>(p, i0, i1, j0, j1, k0, k1, lane & 3, 4);
