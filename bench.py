@@ -102,6 +102,12 @@ def ncu_record(workload):
     return None
 
 
+def ncu_block(workload):
+    """traffic / warp instructions of k_fused for a secondary workload, from profiles/traffic.csv (null on another build)"""
+    rec = ncu_record(workload)
+    return {"traffic": rec["dram_bytes"] if rec else None, "warp_instructions_per_launch": rec["warp_instructions"] if rec else None}
+
+
 def issue_roofline(rec, fused_ms_mean, sm_mhz, n_sms):
     """The bound the fused kernel actually runs into: warp instructions issued per second against
     SMs x 4 schedulers x 1 instruction per cycle at the SM clock seen during the run.  The instruction count per launch comes
@@ -438,7 +444,7 @@ def run_ours(args, rank, world, local_rank):
                   "kernel_ms_mean": {"prepass": float(s_kms[:, 0].mean()), "fused": float(s_kms[:, 2].mean())},
                   "per_frame_mean": {k: float(s_cnt[:, i].mean()) for i, k in enumerate(STAT_KEYS)},
                   "algorithmic_bytes": float(av.mean()),
-                  "roofline": roofline_block(av, asec, tch, tchs, s_kms[:, 2], s_ms, peak),
+                  "roofline": dict(roofline_block(av, asec, tch, tchs, s_kms[:, 2], s_ms, peak), **ncu_block(c.name + "-steady")),
                   "note": "the timed frames again after the arc has been swept back and forth: geometry weights saturated at w_max, "
                           "colour gate mostly closed (col_changed << col_read), stores skipped where the word does not change"}
 
@@ -506,7 +512,7 @@ def run_ours(args, rank, world, local_rank):
                             "fused_ms": float(s_kms[:, 2].mean()),
                             "mu_m": s_mu, "sigma_m": s_sigma, "algorithmic_bytes": float(av.mean()),
                             "geo_read": float(s_cnt[:, 0].mean()), "col_read": float(s_cnt[:, 2].mean()),
-                            "roofline": roofline_block(av, asec, tch, tchs, s_kms[:, 2], s_ms, peak)}
+                            "roofline": dict(roofline_block(av, asec, tch, tchs, s_kms[:, 2], s_ms, peak), **ncu_block(f"{c.name}-stress-{kind}"))}
             svol.close()
             del svol, sfr
             torch.cuda.empty_cache()
