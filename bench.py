@@ -541,20 +541,27 @@ def run_ours(args, rank, world, local_rank):
         T_prev, dd_last = np.asarray(frames[nfr - 2][4], np.float32), frames[nfr - 1][2]
         tms = {"measure": [], "predict": [], "track": []}
         evs = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
+        T_rel, trk_rms, trk_cnt, lost = np.eye(4, dtype=np.float32), float("nan"), 0, None
         for rep in range(6):
             evs[0].record(stream)
             fe.measure(dd_last, c.K_depth, stream=stream)
             evs[1].record(stream)
             fe.predict(vol, T_prev, c.K_depth, 0.3, 8.0, stream=stream)
             evs[2].record(stream)
-            T_rel, trk_rms, trk_cnt = fe.track(stream=stream)
+            try:
+                T_rel, trk_rms, trk_cnt = fe.track(stream=stream)
+            except vf.VolError as e:                          # VOL_E_LOST: e.g. the sphere of config 1 (rotations about its centre unobservable)
+                if e.code != vf.VOL_E_LOST:
+                    raise
+                lost = str(e)
             evs[3].record(stream)
             torch.cuda.synchronize()
             if rep >= 2:
                 for k, name in enumerate(("measure", "predict", "track")):
                     tms[name].append(float(evs[k].elapsed_time(evs[k + 1])))
         T_trk = T_prev.astype(np.float64) @ T_rel.astype(np.float64)
-        tracking = {"measure_ms": float(np.mean(tms["measure"])), "predict_ms": float(np.mean(tms["predict"])),
+        trk_status, trk_level, trk_cond = fe.track_info()
+        tracking = {"status": "lost: " + lost if lost else "ok", "conditioning": trk_cond, "measure_ms": float(np.mean(tms["measure"])), "predict_ms": float(np.mean(tms["predict"])),
                     "track_ms": float(np.mean(tms["track"])), "icp_steps": 19, "correspondences": int(trk_cnt), "rms_mm": 1e3 * trk_rms,
                     "pose_error_mm": 1e3 * float(np.linalg.norm(T_trk[:3, 3] - np.asarray(T_last, np.float64)[:3, 3])),
                     "motion_mm": 1e3 * float(np.linalg.norm(T_prev[:3, 3] - np.asarray(T_last, np.float32)[:3, 3])),
