@@ -72,6 +72,8 @@ def _load():
         lib.ref_sample_colour_trilinear.argtypes = [P, P, P, ctypes.c_int64, P]
         lib.ref_raycast.restype = ctypes.c_int
         lib.ref_raycast.argtypes = [P, P, P, ctypes.c_int32, ctypes.c_int32, P, P, ctypes.c_float, ctypes.c_float, P, P]
+        lib.ref_raycast_trilinear.restype = ctypes.c_int
+        lib.ref_raycast_trilinear.argtypes = [P, P, P, ctypes.c_int32, ctypes.c_int32, P, P, ctypes.c_float, ctypes.c_float, P, P]
         _lib = lib
     return _lib
 
@@ -176,6 +178,17 @@ class RefVolume:
                                  T.ctypes.data, Kc.ctypes.data, float(t_near), float(t_far), depth.ctypes.data, rgb.ctypes.data)
         if rc != 0:
             raise ValueError("ref_raycast: bad arguments")
+        return depth, rgb
+
+    def raycast_trilinear(self, w, h, T_world_cam, K, t_near, t_far):
+        """ref_raycast_trilinear (reading R7): as raycast(), the TSDF of a sample interpolated from the 8 surrounding voxels."""
+        T, Kc = _f32(T_world_cam, 16), _f32(K, 9)
+        depth = np.zeros((h, w), dtype=np.float32)
+        rgb = np.zeros((h, w, 3), dtype=np.uint8)
+        rc = _load().ref_raycast_trilinear(ctypes.addressof(self.desc), self.geo.ctypes.data, self.col.ctypes.data, int(w), int(h),
+                                           T.ctypes.data, Kc.ctypes.data, float(t_near), float(t_far), depth.ctypes.data, rgb.ctypes.data)
+        if rc != 0:
+            raise ValueError("ref_raycast_trilinear: bad arguments")
         return depth, rgb
 
     def frame_constants(self, T_world_depth, T_depth_rgb):

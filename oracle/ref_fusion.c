@@ -423,6 +423,83 @@ int ref_raycast(const ref_vol_t *v, const uint32_t *geo, const uint32_t *col, in
     return 0;
 }
 
+/* ref_raycast_trilinear -- the same ray caster with reading R3 replaced by R7 (round 2):
+ *   R7  the TSDF at a sample is the TRILINEAR interpolation of the 8 voxels whose centres surround the point: grid coordinate
+ *       g = (p - origin) / vs - 1/2 per axis (voxel centres at integers, A1), b = floor(g), f = g - b; corner c = 0..7 is voxel
+ *       b + (c & 1, (c >> 1) & 1, c >> 2) with weight (wz * wy) * wx, w = f on the far side and 1 - f on the near side;
+ *       F = sum over c, in that order, of weight * q (fmaf).  If any of the 8 voxels lies outside the volume or was never
+ *       observed (w = 0) the sample is "unknown".
+ * R1, R2, R4 (on these F), R5 and R6 are unchanged.  A TSDF that is linear in space (a plane inside the truncation band) is
+ * reproduced exactly by the interpolation, so the zero crossing of R4 is the plane itself for any t_near -- no voxel-sized
+ * terraces, which is what the tracker's prediction needs (F8 is not applied to these maps).  ** parity unpinned by the paper ** */
+int ref_raycast_trilinear(const ref_vol_t *v, const uint32_t *geo, const uint32_t *col, int32_t w, int32_t h,
+                          const float T_world_cam[16], const float K[9], float t_near, float t_far,
+                          float *depth_out, uint8_t *rgb_out)
+{
+    if (!v || !geo || !col || !T_world_cam || !K || !depth_out || w <= 0 || h <= 0) return -1;
+    if (!(t_near >= 0.0f) || !(t_far >= t_near)) return -1;
+    const float fx = K[0], fy = K[4], cx = K[2], cy = K[5];
+    const float vs = v->extent / (float)v->nx, vc = vs / (float)v->r;
+    const float inv_vs = 1.0f / vs, inv_vc = 1.0f / vc;
+    const int cnx = v->nx * v->r, cny = v->ny * v->r, cnz = v->nz * v->r;
+    const int n[3] = {v->nx, v->ny, v->nz};
+#pragma omp parallel for schedule(dynamic, 4)
+    for (int y = 0; y < h; ++y)
+        for (int x = 0; x < w; ++x) {
+            const float dx = ((float)x - cx) / fx, dy = ((float)y - cy) / fy;                     /* R1 */
+            float dw[3], ow[3];
+            for (int a = 0; a < 3; ++a) {
+                dw[a] = fmaf(T_world_cam[4 * a + 1], dy, fmaf(T_world_cam[4 * a + 0], dx, T_world_cam[4 * a + 2]));
+                ow[a] = T_world_cam[4 * a + 3];
+            }
+            float depth = 0.0f, t_prev = 0.0f, f_prev = 0.0f;
+            int known_prev = 0;
+            uint8_t rgb[3] = {0, 0, 0};
+            for (int k = 0;; ++k) {
+                const float t = fmaf((float)k, vs, t_near);                                       /* R2 */
+                if (t > t_far) break;
+                float b[3], fr[3];
+                int in = 1;
+                for (int a = 0; a < 3; ++a) {                                                     /* R7 */
+                    const float g = (fmaf(t, dw[a], ow[a]) - v->origin[a]) * inv_vs - 0.5f;
+                    b[a] = floorf(g);
+                    fr[a] = g - b[a];
+                    in = in && b[a] >= 0.0f && b[a] <= (float)(n[a] - 2);                         /* false for NaN / inf as well */
+                }
+                int known = in; float f = 0.0f;
+                if (in) {
+                    const int i0 = (int)b[0], j0 = (int)b[1], k0 = (int)b[2];
+                    for (int c = 0; c < 8; ++c) {
+                        const uint32_t word = geo[((size_t)(k0 + (c >> 2)) * (size_t)v->ny + (size_t)(j0 + ((c >> 1) & 1))) * (size_t)v->nx + (size_t)(i0 + (c & 1))];
+                        if ((int16_t)(word >> 16) == 0) known = 0;
+                        const float wx = (c & 1) ? fr[0] : 1.0f - fr[0];
+                        const float wy = (c & 2) ? fr[1] : 1.0f - fr[1];
+                        const float wz = (c & 4) ? fr[2] : 1.0f - fr[2];
+                        f = fmaf((wz * wy) * wx, (float)(int16_t)(word & 0xffffu), f);
+                    }
+                    if (!known) f = 0.0f;
+                }
+                if (known && known_prev && f_prev > 0.0f && !(f > 0.0f)) {                        /* R4 */
+                    depth = fmaf(vs, f_prev / (f_prev - f), t_prev);
+                    break;
+                }
+                known_prev = known; t_prev = t; f_prev = f;
+            }
+            if (depth > 0.0f) {                                                                   /* R5 */
+                const float hx = floorf((fmaf(depth, dw[0], ow[0]) - v->origin[0]) * inv_vc);
+                const float hy = floorf((fmaf(depth, dw[1], ow[1]) - v->origin[1]) * inv_vc);
+                const float hz = floorf((fmaf(depth, dw[2], ow[2]) - v->origin[2]) * inv_vc);
+                if (hx >= 0.0f && hx < (float)cnx && hy >= 0.0f && hy < (float)cny && hz >= 0.0f && hz < (float)cnz) {
+                    const uint32_t cw = col[((size_t)(int)hz * (size_t)cny + (size_t)(int)hy) * (size_t)cnx + (size_t)(int)hx];
+                    if ((cw >> 24) != 0) { rgb[0] = (uint8_t)cw; rgb[1] = (uint8_t)(cw >> 8); rgb[2] = (uint8_t)(cw >> 16); }
+                }
+            }
+            depth_out[(size_t)y * (size_t)w + (size_t)x] = depth;
+            if (rgb_out) { uint8_t *o = rgb_out + ((size_t)y * (size_t)w + (size_t)x) * 3; o[0] = rgb[0]; o[1] = rgb[1]; o[2] = rgb[2]; }
+        }
+    return 0;
+}
+
 /* ------------------------------------------------------------------------------------------ */
 /* ref_sample_colour -- NEXT row: colour-volume lookup at world points     */
 /* ------------------------------------------------------------------------------------------ */
