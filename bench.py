@@ -533,11 +533,34 @@ def run_ours(args, rank, world, local_rank):
     torch.cuda.synchronize()
     raycast_ms = float(r0.elapsed_time(r1)) / 10.0
     raycast_hit = float((rc_depth > 0).float().mean())
+    for _ in range(3):
+        vol.raycast_trilinear(c.wd, c.hd, T_last, c.K_depth, 0.3, 8.0, rc_depth, rc_rgb, stream=stream)
+    torch.cuda.synchronize()
+    r0.record(stream)
+    for _ in range(10):
+        vol.raycast_trilinear(c.wd, c.hd, T_last, c.K_depth, 0.3, 8.0, rc_depth, rc_rgb, stream=stream)
+    r1.record(stream)
+    torch.cuda.synchronize()
+    raycast_tri_ms = float(r0.elapsed_time(r1)) / 10.0
+    # the same right after a frame has been integrated: the casters' skip flags are rebuilt from the volume first
+    rc_fresh = {}
+    for name, fn in (("nearest", vol.raycast), ("trilinear", vol.raycast_trilinear)):
+        ts = []
+        for fr in frames[-4:]:
+            win.integrate(fr)
+            r0.record(stream)
+            fn(c.wd, c.hd, T_last, c.K_depth, 0.3, 8.0, rc_depth, None, stream=stream)
+            r1.record(stream)
+            torch.cuda.synchronize()
+            ts.append(float(r0.elapsed_time(r1)))
+        rc_fresh[name] = float(np.mean(ts[1:]))
+    vol.raycast(c.wd, c.hd, T_last, c.K_depth, 0.3, 8.0, rc_depth, rc_rgb, stream=stream)       # (the sampling figures below use these hits)
+    torch.cuda.synchronize()
     # ---- NEXT row: the tracker -- front end of the last frame, prediction ray-cast from the pose before
     #      it, coarse-to-fine ICP (19 steps, each a kernel and a 232-byte read-back); the tracked pose against the true one
     tracking = None
     if not stress_kind and nfr >= 2:
-        fe = vf.Frontend(c.wd, c.hd, 3, device=local_rank)
+        fe = vf.Frontend(c.wd, c.hd, 3, device=local_rank, trilinear_prediction=True)
         T_prev, dd_last = np.asarray(frames[nfr - 2][4], np.float32), frames[nfr - 1][2]
         tms = {"measure": [], "predict": [], "track": []}
         evs = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
@@ -565,6 +588,7 @@ def run_ours(args, rank, world, local_rank):
                     "track_ms": float(np.mean(tms["track"])), "icp_steps": 19, "correspondences": int(trk_cnt), "rms_mm": 1e3 * trk_rms,
                     "pose_error_mm": 1e3 * float(np.linalg.norm(T_trk[:3, 3] - np.asarray(T_last, np.float64)[:3, 3])),
                     "motion_mm": 1e3 * float(np.linalg.norm(T_prev[:3, 3] - np.asarray(T_last, np.float32)[:3, 3])),
+                    "prediction": "vol_raycast_trilinear, no F8 (opts.trilinear_prediction)",
                     "note": "vol_frontend_measure / _predict / _track (SURVEY 8(f) rank 4) of the last frame against the fused volumes, "
                             "not part of the timed step"}
         fe.close()
@@ -664,7 +688,10 @@ def run_ours(args, rank, world, local_rank):
                                         "mode": "vol_integrate_host + vol_frame_stats (synchronises) per frame (a live scan)"}},
         "tracking": tracking,
         "raycast": {"ms": raycast_ms, "rays_per_s": c.wd * c.hd / (raycast_ms * 1e-3), "image": f"{c.wd}x{c.hd}", "hit_fraction": raycast_hit,
-                    "note": "vol_raycast of the fused volumes (SURVEY 8(f) rank 1), not part of the timed step"},
+                    "trilinear_ms": raycast_tri_ms, "after_a_new_frame_ms": rc_fresh,
+                    "note": "vol_raycast / vol_raycast_trilinear of the fused volumes (SURVEY 8(f) rank 1), not part of the timed step; "
+                            "ms: repeated casts of an unchanged volume; after_a_new_frame_ms: depth only, including the rebuild of the "
+                            "casters' skip flags that the first cast after a vol_integrate does"},
         "sample_colour": None if sample_ms is None else {
             "ms": sample_ms, "points": int(sp_pts.shape[0]), "points_per_s": sp_pts.shape[0] / (sample_ms * 1e-3), "filled_fraction": sample_filled,
             "trilinear_ms": sample_tri_ms,

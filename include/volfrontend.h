@@ -45,6 +45,9 @@ typedef struct {
     float   cos_min;        /* F5 normal gate (cosine); <= 0 selects 0.94 */
     int32_t device;         /* CUDA device ordinal; < 0 = current device */
     float   cond_min;       /* F6 conditioning gate, see vol_frontend_track; <= 0 selects VOL_ICP_COND_MIN; must be < 1 */
+    int32_t trilinear_prediction;   /* != 0: vol_frontend_predict casts its rays with vol_raycast_trilinear (reading R7) and builds the
+                                       maps from that depth map directly, without F8 (which exists to smooth the voxel-sized terraces
+                                       of the nearest-voxel ray caster) */
 } vol_frontend_opts_t;
 
 #define VOL_ICP_COND_MIN 1e-3f
@@ -64,7 +67,8 @@ int vol_frontend_measure(vol_frontend_t *fe, const uint16_t *depth_u16_dev, cons
 int vol_frontend_predict_depth(vol_frontend_t *fe, const float *depth_m_dev, const float K[9], int32_t filter, void *stream);
 
 /* The same with the ray casting included: vol_raycast of `v` from T_world_cam (the pose the prediction is made from,
- * normally the previous frame's), then vol_frontend_predict_depth with the filter (F8).  Unsharded volumes only.  Asynchronous. */
+ * normally the previous frame's), then vol_frontend_predict_depth with the filter (F8) -- or, with
+ * opts.trilinear_prediction, vol_raycast_trilinear and no filter.  Unsharded volumes only.  Asynchronous. */
 int vol_frontend_predict(vol_frontend_t *fe, const vol_t *v, const float T_world_cam[16], const float K[9], float t_near_m,
                          float t_far_m, void *stream);
 

@@ -161,6 +161,14 @@ int vol_integrate_host(vol_t *v, const uint16_t *depth_u16_host, int32_t wd, int
 int vol_raycast(const vol_t *v, int32_t w, int32_t h, const float T_world_cam[16], const float K[9], float t_near_m,
                 float t_far_m, float *depth_dev, uint8_t *rgb8_dev, void *stream);
 
+/* The same with the TSDF of a sample interpolated trilinearly from the 8 voxels whose centres surround it (reading R7; a
+ * sample with a never-observed or outside voxel among the 8 is unknown).  A plane inside the truncation band is rendered
+ * at its exact depth whatever the phase of the samples, and the depth map has no voxel-sized terraces: the tracker can
+ * build its prediction from it without the millimetre rounding and bilateral pass that the nearest-voxel map needs (F8).
+ * Same arguments, same rules. */
+int vol_raycast_trilinear(const vol_t *v, int32_t w, int32_t h, const float T_world_cam[16], const float K[9], float t_near_m,
+                float t_far_m, float *depth_dev, uint8_t *rgb8_dev, void *stream);
+
 /* Look up the colour volume at n world points ("given the 3D world positions, the RGB value of any pixel can
  * be found by accessing the colour volume" -- the positions of a polygon's texture map are V_a + i V_aV_green + j V_aV_blue
  * of eq. 11-14, computed by the caller).  points_dev: DEVICE, n x 3 float32 (x, y, z in world metres); words_dev: DEVICE,

@@ -26,7 +26,7 @@ VOL_STATS_RAW_BYTES = 128
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "--fmad=false", "-std=c++17",
               "-Xcompiler", "-fPIC,-ffp-contract=off", "-shared"]
 
-EXPORTS = ["vol_create", "vol_integrate", "vol_integrate_host", "vol_raycast", "vol_sample_colour", "vol_sample_colour_trilinear", "vol_download", "vol_download_voxels", "vol_upload",
+EXPORTS = ["vol_create", "vol_integrate", "vol_integrate_host", "vol_raycast", "vol_raycast_trilinear", "vol_sample_colour", "vol_sample_colour_trilinear", "vol_download", "vol_download_voxels", "vol_upload",
            "vol_reset", "vol_info", "vol_shard_layers", "vol_set_counting", "vol_frame_stats", "vol_frame_stats_async", "vol_stats_decode", "vol_set_profiling", "vol_last_kernel_ms",
            "vol_launches_per_frame", "vol_selftest", "vol_destroy", "vol_strerror",
            # include/volfrontend.h
@@ -88,6 +88,7 @@ def lib():
         L.vol_integrate.argtypes = [P, P, I32, I32, P, I32, I32, P, P, P, P, P]
         L.vol_integrate_host.argtypes = L.vol_integrate.argtypes
         L.vol_raycast.argtypes = [P, I32, I32, P, P, F, F, P, P, P]
+        L.vol_raycast_trilinear.argtypes = [P, I32, I32, P, P, F, F, P, P, P]
         L.vol_sample_colour.argtypes = [P, P, I64, P, P]
         L.vol_sample_colour_trilinear.argtypes = [P, P, I64, P, P]
         L.vol_download.argtypes = [P, P, ctypes.c_size_t, P, ctypes.c_size_t, P]
@@ -226,6 +227,13 @@ class Volume:
         _check(lib().vol_raycast(self._h, int(w), int(h), T.ctypes.data, Kc.ctypes.data, float(t_near), float(t_far),
                                  _dev_ptr(depth_dev), None if rgb_dev is None else _dev_ptr(rgb_dev), _stream_ptr(stream)), "vol_raycast")
 
+    def raycast_trilinear(self, w, h, T_world_cam, K, t_near, t_far, depth_dev, rgb_dev=None, stream=None):
+        """vol_raycast_trilinear: as raycast(), the TSDF of a sample interpolated from the 8 surrounding voxels (reading R7)."""
+        T, Kc = _f32(T_world_cam, 16), _f32(K, 9)
+        _check(lib().vol_raycast_trilinear(self._h, int(w), int(h), T.ctypes.data, Kc.ctypes.data, float(t_near), float(t_far),
+                                           _dev_ptr(depth_dev), None if rgb_dev is None else _dev_ptr(rgb_dev), _stream_ptr(stream)),
+               "vol_raycast_trilinear")
+
     def sample_colour(self, points_dev, n, words_dev, stream=None):
         """vol_sample_colour: points_dev = CUDA float32 tensor [n, 3] (world), words_dev = CUDA int32/uint32 tensor [n]."""
         _check(lib().vol_sample_colour(self._h, _dev_ptr(points_dev), int(n), _dev_ptr(words_dev), _stream_ptr(stream)), "vol_sample_colour")
@@ -311,7 +319,8 @@ class Volume:
 
 class FrontendOpts(ctypes.Structure):
     _fields_ = [("sigma_s_px", ctypes.c_float), ("sigma_r_m", ctypes.c_float), ("dist_m", ctypes.c_float),
-                ("cos_min", ctypes.c_float), ("device", ctypes.c_int32), ("cond_min", ctypes.c_float)]
+                ("cos_min", ctypes.c_float), ("device", ctypes.c_int32), ("cond_min", ctypes.c_float),
+                ("trilinear_prediction", ctypes.c_int32)]
 
 
 ICP_SUMS = 29
@@ -332,10 +341,10 @@ class Frontend:
     """include/volfrontend.h: depth front end (bilateral filter, vertex / normal map pyramid) and ICP tracking against a
     ray-cast prediction -- the measured and predicted map pyramids of one image size on one GPU."""
 
-    def __init__(self, w, h, levels=3, sigma_s_px=0.0, sigma_r_m=0.0, dist_m=0.0, cos_min=0.0, device=-1, cond_min=0.0):
+    def __init__(self, w, h, levels=3, sigma_s_px=0.0, sigma_r_m=0.0, dist_m=0.0, cos_min=0.0, device=-1, cond_min=0.0, trilinear_prediction=False):
         self._h = ctypes.c_void_p()
         self.w, self.h, self.levels = int(w), int(h), int(levels)
-        opts = FrontendOpts(float(sigma_s_px), float(sigma_r_m), float(dist_m), float(cos_min), int(device), float(cond_min))
+        opts = FrontendOpts(float(sigma_s_px), float(sigma_r_m), float(dist_m), float(cos_min), int(device), float(cond_min), int(bool(trilinear_prediction)))
         rc = lib().vol_frontend_create(ctypes.byref(self._h), self.w, self.h, self.levels, ctypes.byref(opts))
         if rc != VOL_OK:
             self._h = ctypes.c_void_p()

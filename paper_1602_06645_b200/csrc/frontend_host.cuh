@@ -21,6 +21,7 @@ struct vol_frontend {
     unsigned long long *track_acc; size_t track_steps;      // vol_frontend_track: one set of accumulators per step
     double *track_out, *track_out_pinned;                   // FE_TRACK_OUT doubles: T (3 x 4), rms, count, status, level, conditioning
     double cond_min;
+    bool trilinear_prediction;
     int last_status, last_level; double last_cond;          // of the most recent vol_frontend_track
     int track_blocks;                                       // co-resident blocks of k_icp_track
 };
@@ -72,6 +73,7 @@ extern "C" int vol_frontend_create(vol_frontend_t **out, int32_t w, int32_t h, i
     memset(fe, 0, sizeof *fe);
     fe->device = device; fe->w = w; fe->h = h; fe->levels = levels;
     fe->sigma_s = sigma_s; fe->sigma_r = sigma_r; fe->dist_m = dist_m; fe->cos_min = cos_min; fe->cond_min = (double)cond_min;
+    fe->trilinear_prediction = opts && opts->trilinear_prediction != 0;
     // F1 tables: binary64, rounded once
     const double ss = (double)sigma_s, sr = (double)sigma_r * 1000.0;
     fe->kmax = (int)std::ceil(3.0 * sr);
@@ -157,9 +159,11 @@ extern "C" int vol_frontend_predict(vol_frontend_t *fe, const vol_t *v, const fl
                                     float t_far_m, void *stream)
 {
     if (!fe || !v || fe->device != v->device) return VOL_E_ARG;
-    int rc = vol_raycast(v, fe->w, fe->h, T_world_cam, K, t_near_m, t_far_m, fe->ray_depth, nullptr, stream);
+    const bool tri = fe->trilinear_prediction;
+    int rc = tri ? vol_raycast_trilinear(v, fe->w, fe->h, T_world_cam, K, t_near_m, t_far_m, fe->ray_depth, nullptr, stream)
+                 : vol_raycast(v, fe->w, fe->h, T_world_cam, K, t_near_m, t_far_m, fe->ray_depth, nullptr, stream);
     if (rc) return rc;
-    return vol_frontend_predict_depth(fe, fe->ray_depth, K, 1, stream);
+    return vol_frontend_predict_depth(fe, fe->ray_depth, K, tri ? 0 : 1, stream);
 }
 
 static vf::IcpLevel fe_level(const vol_frontend *fe, int level)

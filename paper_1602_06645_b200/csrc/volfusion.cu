@@ -54,6 +54,10 @@ struct vol {
     // while the fused kernel of the frame before it is still reading its own set
     float4 *scr_pixmap[2]; float *scr_depthf[2]; uint32_t *scr_pyr[2]; uint4 *scr_jobs[2];
     uint32_t *ctrl_base, *ctrl_last;    // ctrl_last: block of the most recent frame (vol_frame_stats*)
+    // ray casting: exact "holds an observed tsdf <= 0" flags per sub-box (raycast.cuh, k_sub_neg), rebuilt by the first ray
+    // cast after the geometry volume has changed (content_version counts vol_integrate*, vol_upload, vol_reset)
+    uint8_t *sub_neg, *tile_any, *brick_any, *sub_dil, *tile_dil, *brick_dil; int sbx, sby, sbz;
+    mutable unsigned long long content_version, sub_neg_version, dil_version;
     cudaEvent_t ev[4];
     bool ev_valid;
     // vol_integrate_host: the frames are copied on a stream of the library's own
@@ -241,11 +245,15 @@ extern "C" int vol_create(vol_t **out, const int32_t dims_geo[3], int32_t r, con
     if (rc == VOL_OK && cudaMemset(p.marks, 0, sizeof(uint32_t) * nw) != cudaSuccess) rc = VOL_E_CUDA;
     if (cudaMalloc(&p.tile_sat, nt) != cudaSuccess || cudaMalloc(&p.tile_skip, nt) != cudaSuccess) rc = VOL_E_OOM;
     if (rc == VOL_OK && (cudaMemset(p.tile_sat, 0, nt) != cudaSuccess || cudaMemset(p.tile_skip, 0, nt) != cudaSuccess)) rc = VOL_E_CUDA;
+    v->sbx = p.tiles_x * vf::SUBX; v->sby = p.tiles_y; v->sbz = (p.n_tiles > 0 ? p.n_tiles / (p.tiles_x * p.tiles_y) : 0) * vf::SUBZ;
+    if (cudaMalloc(&v->sub_neg, nt * vf::SUBX * vf::SUBZ) != cudaSuccess || cudaMalloc(&v->tile_any, nt) != cudaSuccess ||
+        cudaMalloc(&v->sub_dil, nt * vf::SUBX * vf::SUBZ) != cudaSuccess || cudaMalloc(&v->tile_dil, nt) != cudaSuccess) rc = VOL_E_OOM;
+    v->content_version = 1; v->sub_neg_version = 0;
     if (cudaMalloc(&p.tile_neg, nt) != cudaSuccess) rc = VOL_E_OOM;
     if (rc == VOL_OK && cudaMemset(p.tile_neg, 0, nt) != cudaSuccess) rc = VOL_E_CUDA;
     p.bricks_x = p.tiles_x; p.bricks_y = (p.tiles_y + 7) / 8; p.bricks_z = (my_slabs + 3) / 4;
     const size_t nb = (size_t)p.bricks_x * p.bricks_y * p.bricks_z + 1;
-    if (cudaMalloc(&p.brick_neg, nb) != cudaSuccess) rc = VOL_E_OOM;
+    if (cudaMalloc(&p.brick_neg, nb) != cudaSuccess || cudaMalloc(&v->brick_any, nb) != cudaSuccess || cudaMalloc(&v->brick_dil, nb) != cudaSuccess) rc = VOL_E_OOM;
     if (rc == VOL_OK && cudaMemset(p.brick_neg, 0, nb) != cudaSuccess) rc = VOL_E_CUDA;
     // one 128-byte statistics record (8 words, then 12 counters: read back together by vol_frame_stats*), then the queue control words
     static_assert(sizeof(uint32_t) * vf::ST_N + sizeof(unsigned long long) * vf::CNT_N == VOL_STATS_RAW_BYTES && vf::CTRL_Q0 * 4 == VOL_STATS_RAW_BYTES,
@@ -301,6 +309,12 @@ extern "C" void vol_destroy(vol_t *v)
     if (v->p.work_col) cudaFree(v->p.work_col);
     if (v->p.marks) cudaFree(v->p.marks);
     if (v->p.tile_neg) cudaFree(v->p.tile_neg);
+    if (v->sub_neg) cudaFree(v->sub_neg);
+    if (v->tile_any) cudaFree(v->tile_any);
+    if (v->brick_any) cudaFree(v->brick_any);
+    if (v->sub_dil) cudaFree(v->sub_dil);
+    if (v->tile_dil) cudaFree(v->tile_dil);
+    if (v->brick_dil) cudaFree(v->brick_dil);
     if (v->p.tile_sat) cudaFree(v->p.tile_sat);
     if (v->p.tile_skip) cudaFree(v->p.tile_skip);
     for (int i = 0; i < 4; ++i) if (v->p.sec_map[i]) cudaFree(v->p.sec_map[i]);
@@ -404,7 +418,7 @@ static int integrate_impl(vol_t *v, const uint16_t *depth_u16_dev, int32_t wd, i
     do {                                                                                \
         const FusedFn kf = fused_kernel<RR>(cnt, p.variant);                            \
         CK(launch(vf::k_prepass<RR>, g0, 256, s, VF_PIPELINE, p));                            \
-        ++v->frame_seq; v->ctrl_last = p.ctrl;                                          \
+        ++v->frame_seq; ++v->content_version; v->ctrl_last = p.ctrl;                    \
         if (v->profiling) { CK(cudaEventRecord(v->ev[1], s)); CK(cudaEventRecord(v->ev[2], s)); } \
         if (rgb_ready) {   /* everything but the colour items now, those once the HD frame has arrived */ \
             CK(launch(kf, dim3(g2), vf::CTA, s, true, p, (int)vf::PHASE_GEO));          \
@@ -480,8 +494,8 @@ extern "C" int vol_integrate_host(vol_t *v, const uint16_t *depth_u16_host, int3
     return VOL_OK;
 }
 
-extern "C" int vol_raycast(const vol_t *v, int32_t w, int32_t h, const float T_world_cam[16], const float K[9], float t_near_m,
-                           float t_far_m, float *depth_dev, uint8_t *rgb8_dev, void *stream)
+static int raycast_impl(const vol_t *v, int32_t w, int32_t h, const float T_world_cam[16], const float K[9], float t_near_m,
+                        float t_far_m, float *depth_dev, uint8_t *rgb8_dev, void *stream, bool trilinear)
 {
     if (!v || !T_world_cam || !K || !depth_dev) return VOL_E_ARG;
     if (w <= 0 || h <= 0 || w > 16384 || h > 16384 || !intrinsics_ok(K)) return VOL_E_ARG;
@@ -495,10 +509,40 @@ extern "C" int vol_raycast(const vol_t *v, int32_t w, int32_t h, const float T_w
     for (int i = 0; i < 12; ++i) q.T[i] = T_world_cam[i];
     q.t_near = t_near_m; q.t_far = t_far_m; q.depth = depth_dev; q.rgb = rgb8_dev;
     if (v->p.n_tiles == 0) return VOL_OK;
+    q.sub_neg = v->sub_neg; q.sbx = v->sbx; q.sby = v->sby; q.tile_any = v->tile_any; q.brick_any = v->brick_any;
+    if (v->sub_neg_version != v->content_version) {            // (stream-ordered with the calls that changed the volume: volfusion.h)
+        CK(cudaMemsetAsync(v->brick_any, 0, (size_t)v->p.bricks_x * v->p.bricks_y * v->p.bricks_z, (cudaStream_t)stream));
+        vf::k_sub_neg<<<(v->p.n_tiles + 7) / 8, 256, 0, (cudaStream_t)stream>>>(v->p, v->sub_neg, v->sbx, v->sby, v->sbz, v->tile_any, v->brick_any);
+        v->sub_neg_version = v->content_version;
+    }
+    q.sub_dil = v->sub_dil; q.tile_dil = v->tile_dil; q.brick_dil = v->brick_dil;
+    if (trilinear && v->dil_version != v->content_version) {
+        const int tz = v->p.n_tiles / (v->p.tiles_x * v->p.tiles_y);
+        const long long ns = (long long)v->sbx * v->sby * v->sbz, nb = (long long)v->p.bricks_x * v->p.bricks_y * v->p.bricks_z;
+        const unsigned b0 = (unsigned)((ns + 255) / 256), b1 = (unsigned)((v->p.n_tiles + 255) / 256), b2 = (unsigned)((nb + 255) / 256);
+        const vf::DilateJob j0 = {v->sub_neg, v->sub_dil, v->sbx, v->sby, v->sbz, 0u};
+        const vf::DilateJob j1 = {v->tile_any, v->tile_dil, v->p.tiles_x, v->p.tiles_y, tz, b0};
+        const vf::DilateJob j2 = {v->brick_any, v->brick_dil, v->p.bricks_x, v->p.bricks_y, v->p.bricks_z, b0 + b1};
+        vf::k_dilate<<<b0 + b1 + b2, 256, 0, (cudaStream_t)stream>>>(j0, j1, j2);
+        v->dil_version = v->content_version;
+    }
     const dim3 grid((w + 7) / 8, (h + 7) / 8);
-    vf::k_raycast<<<grid, 64, 0, (cudaStream_t)stream>>>(v->p, q);
+    if (trilinear) vf::k_raycast_trilinear<<<grid, 64, 0, (cudaStream_t)stream>>>(v->p, q);
+    else vf::k_raycast<<<grid, 64, 0, (cudaStream_t)stream>>>(v->p, q);
     CK(cudaGetLastError());
     return VOL_OK;
+}
+
+extern "C" int vol_raycast(const vol_t *v, int32_t w, int32_t h, const float T_world_cam[16], const float K[9], float t_near_m,
+                           float t_far_m, float *depth_dev, uint8_t *rgb8_dev, void *stream)
+{
+    return raycast_impl(v, w, h, T_world_cam, K, t_near_m, t_far_m, depth_dev, rgb8_dev, stream, false);
+}
+
+extern "C" int vol_raycast_trilinear(const vol_t *v, int32_t w, int32_t h, const float T_world_cam[16], const float K[9], float t_near_m,
+                                     float t_far_m, float *depth_dev, uint8_t *rgb8_dev, void *stream)
+{
+    return raycast_impl(v, w, h, T_world_cam, K, t_near_m, t_far_m, depth_dev, rgb8_dev, stream, true);
 }
 
 extern "C" int vol_sample_colour(const vol_t *v, const float *points_dev, int64_t n, uint32_t *words_dev, void *stream)
@@ -544,6 +588,7 @@ extern "C" int vol_upload(vol_t *v, const void *geo_host, const void *col_host, 
     cudaStream_t s = (cudaStream_t)stream;
     if (geo_host && v->geo_bytes) CK(cudaMemcpyAsync(v->p.geo, geo_host, v->geo_bytes, cudaMemcpyHostToDevice, s));
     if (col_host && v->col_bytes) CK(cudaMemcpyAsync(v->p.col, col_host, v->col_bytes, cudaMemcpyHostToDevice, s));
+    ++v->content_version;
     if (geo_host && v->p.n_tiles > 0) {                       // unknown content: no tile or brick may be skipped
         CK(cudaMemsetAsync(v->p.tile_sat, 0, (size_t)v->p.n_tiles, s));
         CK(cudaMemsetAsync(v->p.tile_neg, 1, (size_t)v->p.n_tiles, s));
@@ -558,6 +603,7 @@ extern "C" int vol_reset(vol_t *v, void *stream)
     if (!v) return VOL_E_ARG;
     int rc = set_device(v); if (rc) return rc;
     cudaStream_t s = (cudaStream_t)stream;
+    ++v->content_version;
     if (v->geo_bytes) CK(cudaMemsetAsync(v->p.geo, 0, v->geo_bytes, s));
     if (v->col_bytes) CK(cudaMemsetAsync(v->p.col, 0, v->col_bytes, s));
     if (v->p.n_tiles > 0) {
@@ -798,5 +844,8 @@ extern "C" int vol_trace_dump(unsigned long long *host)
 }
 #endif
 
+#ifdef VF_RAYSTAT
+extern "C" int vol_raystat_dump(unsigned long long *out) { cudaDeviceSynchronize(); cudaMemcpyFromSymbol(out, vf::g_raystat, sizeof(unsigned long long) * 8); unsigned long long z[8] = {0}; cudaMemcpyToSymbol(vf::g_raystat, z, sizeof z); return 0; }
+#endif
 #include "frontend_host.cuh"
 #include "noalloc.cuh"

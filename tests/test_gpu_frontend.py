@@ -230,6 +230,50 @@ def test_closed_loop_on_the_benchmark_workload():
     fe.close(); g.close()
 
 
+def test_trilinear_prediction_maps_and_closed_loop():
+    """opts.trilinear_prediction: the predicted maps are F2-F4 of vol_raycast_trilinear's depth map, without F8 -- bit for bit
+    the oracle's pyramid of its own trilinear ray cast (config 2 scaled); and the closed loop on config 3 at full size, 40
+    frames, CUDA path only, stays within a few millimetres of the true trajectory with this prediction too."""
+    import paper_1602_06645_b200 as vf
+    from parity_util import integrate_both, make_pair
+    c = synth.config(2).scaled(128, 2)
+    g, o = make_pair(c)
+    for fi in (0, 4, 8):
+        depth, rgb, T = synth.frame(c, fi)
+        integrate_both(g, o, c, depth, rgb, T, counting=False)
+    fe = vf.Frontend(c.wd, c.hd, 3, trilinear_prediction=True)
+    Tp = synth.frame(c, 6)[2]
+    fe.predict(g, Tp, c.K_depth, 0.3, 8.0)
+    od, _ = o.raycast_trilinear(c.wd, c.hd, Tp, c.K_depth, 0.3, 8.0)
+    assert (od > 0).mean() > 0.2
+    assert_pyramids_identical(fe, 1, ofe.pyramid(od, c.K_depth, 3), "trilinear prediction")
+    fe.close(); g.close()
+    c = synth.config(3)
+    g = vf.Volume(c.dims_geo, c.r, c.origin, c.extent, c.mu, c.w_max)
+    fe = vf.Frontend(c.wd, c.hd, 3, trilinear_prediction=True)
+    Tg, worst, worst_ang, counts = None, 0.0, 0.0, []
+    for i in range(40):
+        depth, rgb, T_true = synth.frame(c, i)
+        dd, dr = to_dev(depth), to_dev(rgb)
+        if i == 0:
+            Tg = T_true.astype(np.float32)
+        else:
+            fe.predict(g, Tg, c.K_depth, 0.3, 8.0)
+            fe.measure(dd, c.K_depth)
+            Trel, rms, cnt = fe.track()
+            counts.append(cnt)
+            assert cnt > 60000 and rms < 1.5e-3, (i, cnt, rms)
+            Tg = synth.rigid32(Tg.astype(np.float64) @ Trel.astype(np.float64))
+        g.integrate(dd, c.wd, c.hd, dr, c.wh, c.hh, Tg, c.K_depth, c.K_rgb, c.T_depth_rgb)
+        err = np.linalg.inv(T_true.astype(np.float64)) @ Tg.astype(np.float64)
+        worst = max(worst, float(np.linalg.norm(Tg[:3, 3] - T_true[:3, 3])))
+        worst_ang = max(worst_ang, math.degrees(math.acos(min(1.0, (np.trace(err[:3, :3]) - 1) / 2))))
+    print("correspondences:", counts[:3], "...", counts[-3:])
+    print(f"config 3 closed loop with the trilinear prediction, 40 frames: worst drift {1e3 * worst:.2f} mm, {worst_ang:.3f} degrees")
+    assert worst < 0.005 and worst_ang < 0.3
+    fe.close(); g.close()
+
+
 def test_frontend_rejects_bad_calls():
     """Validation precedes any launch: maps that do not exist yet, levels out of range, a non-rigid estimate, a negative
     iteration count, a volume on shards -- each is VOL_E_ARG and leaves the front end usable."""

@@ -8,13 +8,13 @@ from parity_util import integrate_both, make_pair
 pytestmark = pytest.mark.gpu
 
 
-def cast_both(g, o, w, h, T, K, t_near, t_far, with_rgb=True):
+def cast_both(g, o, w, h, T, K, t_near, t_far, with_rgb=True, trilinear=False):
     import torch
     dd = torch.full((h * w,), -1.0, dtype=torch.float32, device="cuda")
     dr = torch.full((h * w * 3,), 7, dtype=torch.uint8, device="cuda") if with_rgb else None
-    g.raycast(w, h, T, K, t_near, t_far, dd, dr)
+    (g.raycast_trilinear if trilinear else g.raycast)(w, h, T, K, t_near, t_far, dd, dr)
     torch.cuda.synchronize()
-    od, orgb = o.raycast(w, h, T, K, t_near, t_far)
+    od, orgb = (o.raycast_trilinear if trilinear else o.raycast)(w, h, T, K, t_near, t_far)
     gd = dd.cpu().numpy().reshape(h, w)
     assert np.array_equal(gd.view(np.uint32), od.view(np.uint32)), f"{int((gd.view(np.uint32) != od.view(np.uint32)).sum())} depths differ"
     if with_rgb:
@@ -30,20 +30,22 @@ def fused_pair(c, frames):
     return g, o
 
 
-def test_raycast_cfg1_views():
+@pytest.mark.parametrize("tri", [False, True])
+def test_raycast_cfg1_views(tri):
     """Config 1 after its 5 frames: the scan's own camera, an oblique camera, a camera inside the volume, a ragged image
-    size (not a multiple of the 8 x 8 pixel CTA), t_near on and off the voxel grid."""
+    size (not a multiple of the 8 x 8 pixel CTA), t_near on and off the voxel grid.  Both readings of the TSDF sample:
+    nearest voxel (R3) and trilinear (R7)."""
     c = synth.config(1)
     g, o = fused_pair(c, range(5))
-    d, rgb = cast_both(g, o, c.wd, c.hd, synth.frame(c, 2)[2], c.K_depth, 0.4, 3.0)
+    d, rgb = cast_both(g, o, c.wd, c.hd, synth.frame(c, 2)[2], c.K_depth, 0.4, 3.0, trilinear=tri)
     assert (d > 0).sum() > 2000 and (rgb.sum(axis=2) > 0).sum() > 2000
     T = synth.rigid32(synth.look_at((0.25, -0.15, 0.1), (0.0, 0.0, 1.5), up=(0.0, -1.0, 0.0)))
-    d, _ = cast_both(g, o, 157, 93, T, c.K_depth, 0.3125, 2.75)
+    d, _ = cast_both(g, o, 157, 93, T, c.K_depth, 0.3125, 2.75, trilinear=tri)
     assert (d > 0).sum() > 2000
     T = synth.rigid32(synth.look_at((0.1, 0.3, 1.15), (0.0, 0.0, 1.5), up=(0.0, -1.0, 0.0)))     # inside the cube
-    cast_both(g, o, c.wd, c.hd, T, c.K_depth, 0.0, 1.0)
-    cast_both(g, o, c.wd, c.hd, T, c.K_depth, 0.05, 0.05)                                          # a single sample: no pair, no hit
-    cast_both(g, o, 64, 48, T, c.K_rgb, 0.0, 2.0, with_rgb=False)                                  # depth only
+    cast_both(g, o, c.wd, c.hd, T, c.K_depth, 0.0, 1.0, trilinear=tri)
+    cast_both(g, o, c.wd, c.hd, T, c.K_depth, 0.05, 0.05, trilinear=tri)                           # a single sample: no pair, no hit
+    cast_both(g, o, 64, 48, T, c.K_rgb, 0.0, 2.0, with_rgb=False, trilinear=tri)                   # depth only
 
 
 def test_raycast_cfg2_r3_and_empty_volume():
@@ -60,6 +62,10 @@ def test_raycast_cfg2_r3_and_empty_volume():
     want = synth.frame(c, 15)[0].astype(np.float32) * 1e-3
     both = (d > 0) & (want > 0)
     assert np.median(np.abs(d[both] - want[both])) < 2.0 * c.extent / 96                          # it is the scene that was fused
+    dt, _ = cast_both(g, o, c.wd, c.hd, synth.frame(c, 15)[2], c.K_depth, 0.2, 4.0, trilinear=True)
+    both = (dt > 0) & (want > 0)
+    assert (dt > 0).mean() > 0.2 and np.median(np.abs(dt[both] - want[both])) < 1.0 * c.extent / 96
+    cast_both(g, o, 301, 203, synth.frame(c, 33)[2], c.K_depth / np.array([[2, 1, 2], [1, 2, 2], [1, 1, 1]], np.float32), 0.37, 3.1, trilinear=True)
 
 
 def test_raycast_rejects_bad_arguments():
@@ -73,6 +79,9 @@ def test_raycast_rejects_bad_arguments():
     for args in ((Tbad, c.K_depth, 0.1, 2.0), (I4, c.K_depth, 2.0, 1.0), (I4, c.K_depth, -1.0, 1.0)):
         with pytest.raises(vf.VolError) as e:
             g.raycast(c.wd, c.hd, args[0], args[1], args[2], args[3], dd)
+        assert e.value.code == vf.VOL_E_ARG
+        with pytest.raises(vf.VolError) as e:
+            g.raycast_trilinear(c.wd, c.hd, args[0], args[1], args[2], args[3], dd)
         assert e.value.code == vf.VOL_E_ARG
     shard = vf.Volume(c.dims_geo, c.r, c.origin, c.extent, c.mu, c.w_max, shard_rank=0, shard_world=2)
     with pytest.raises(vf.VolError):
@@ -93,6 +102,8 @@ def test_raycast_cfg3_full_size():
         check_counters(st, cnt, f"cfg3 full size, frame {fi}")
     compare_states(g, o, "cfg3 full size, every voxel")
     d, rgb = cast_both(g, o, c.wd, c.hd, synth.frame(c, 3)[2], c.K_depth, 0.3, 5.0)
+    assert (d > 0).mean() > 0.5 and (rgb.sum(axis=2) > 0).mean() > 0.3
+    d, rgb = cast_both(g, o, c.wd, c.hd, synth.frame(c, 3)[2], c.K_depth, 0.3, 5.0, trilinear=True)
     assert (d > 0).mean() > 0.5 and (rgb.sum(axis=2) > 0).mean() > 0.3
     g.close()
 
