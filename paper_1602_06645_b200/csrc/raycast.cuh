@@ -245,12 +245,6 @@ __global__ void __launch_bounds__(64) k_raycast(const __grid_constant__ Params p
 // three levels are dilated by one box towards +x, +y, +z (k_dilate) and looked up once, for the base corner's box; a jump ends
 // at the last sample whose base corner is still inside that box.
 struct TriSample { float t, f; bool known, in; int i0, j0, k0; float fx, fy, fz; };
-#ifdef VF_RAYSTAT
-__device__ unsigned long long g_raystat[8];
-#define RS(i) atomicAdd(&g_raystat[i], 1ull)
-#else
-#define RS(i) do { } while (0)
-#endif
 
 // R2 + the index part of R7 for sample k: canonical arithmetic, identical to the oracle's
 __device__ __forceinline__ TriSample tri_sample(const Params &p, const float (&dw)[3], const float (&ow)[3], float vs, float inv_vs, float t_near, int k)
@@ -340,8 +334,7 @@ __global__ void __launch_bounds__(64) k_raycast_trilinear(const __grid_constant_
         while (k <= k1) {
             TriSample cur = tri_sample(p, dw, ow, vs, inv_vs, q.t_near, k);               // R2
             if (cur.t > q.t_far) break;
-            RS(0);
-            if (!cur.in) { RS(1); prev = cur; prev_pending = false; ++k; continue; }             // unknown sample
+            if (!cur.in) { prev = cur; prev_pending = false; ++k; continue; }             // unknown sample
             // can any corner hold an observed tsdf <= 0?  One look-up per level, in the dilated flags, for the box of the BASE
             // corner: brick, then tile, then sub-box
             const unsigned ax0 = (unsigned)cur.i0, ay0 = (unsigned)cur.j0, az0 = (unsigned)cur.k0;
@@ -365,14 +358,11 @@ __global__ void __launch_bounds__(64) k_raycast_trilinear(const __grid_constant_
                     else if (gd[a] < -1e-9f) t_exit = fminf(t_exit, (lo + 0.55f - go[a]) * rgd[a]);
                 }
                 const int kn = (int)fminf(floorf((t_exit - q.t_near) * inv_vs) - 1.0f, (float)k1);
-                if (kn > k) RS(3);
                 k = max(k, kn) + 1;
                 prev_pending = true;
                 continue;
             }
-            RS(4);
-            if (!tri_value(p, cur, false)) { prev_pending = true; ++k; continue; }
-            RS(5);         // all 8 values > 0: not a candidate
+            if (!tri_value(p, cur, false)) { prev_pending = true; ++k; continue; }         // all 8 values > 0: not a candidate
             if (cur.known && !(cur.f > 0.0f)) {                                            // candidate: needs F_prev
                 if (prev_pending) {
                     prev = tri_sample(p, dw, ow, vs, inv_vs, q.t_near, k - 1);

@@ -844,8 +844,5 @@ extern "C" int vol_trace_dump(unsigned long long *host)
 }
 #endif
 
-#ifdef VF_RAYSTAT
-extern "C" int vol_raystat_dump(unsigned long long *out) { cudaDeviceSynchronize(); cudaMemcpyFromSymbol(out, vf::g_raystat, sizeof(unsigned long long) * 8); unsigned long long z[8] = {0}; cudaMemcpyToSymbol(vf::g_raystat, z, sizeof z); return 0; }
-#endif
 #include "frontend_host.cuh"
 #include "noalloc.cuh"
