@@ -20,7 +20,8 @@ primitives on a plane, jittered orbit) -- the configuration the 70 % target is q
   cpu_baseline  the CPU oracle, as it stands, on the first full-size frames of the same workload (rank 0, N = 1 only)
 
 N > 1 (torchrun): every rank integrates an independent scan of the same configuration (replicas, no data-path
-collective), value = sum over ranks / max-over-ranks time, "scaling": "weak".
+collective), value = sum over ranks / max-over-ranks time, "scaling": "weak".  With --shard the N
+ranks integrate ONE scan as z-slab shards ("strong"); --shard-of R,W times one such shard alone on one GPU.
 `--impl reference` times the CPU oracle alone (rank 0), each step a bounded sample of the workload.
 """
 import argparse
@@ -59,6 +60,11 @@ def parse():
                     help="time ONE saturating frame kind of SURVEY 8(d) item 5 as the main workload instead of the scan "
                          "(the default run reports all three under \"stress\")")
     ap.add_argument("--no-stress", action="store_true", help="skip the three saturating frames")
+    ap.add_argument("--shard", action="store_true",
+                    help="N > 1: ONE scan on N GPUs -- rank k owns the z-slabs k mod N of both volumes (vol_opts_t.shard_*), every rank "
+                         "receives every frame; value = one scan's voxels / max-over-ranks time, scaling = strong")
+    ap.add_argument("--shard-of", default=None, metavar="R,W",
+                    help="single process: time shard R of W alone on this GPU (what rank R of a W-GPU --shard run would do)")
     ap.add_argument("--steady-frames", type=int, default=150,
                     help="frames swept back and forth over the arc before the steady-state window (0 = skip it)")
     return ap.parse_args()
@@ -234,7 +240,7 @@ def run_reference(args, rank):
     ms = 1e3 * float(np.mean(t))
     val = nvox / (ms * 1e-3)
     out = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
-           "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+           "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "strong" if args.shard else "weak", "vs_baseline": None,
            "dtype": "f32", "data": "synthetic",
            "config": {"workload": workload_name(c), "sample_per_step": sample},
            "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
@@ -377,7 +383,12 @@ def run_ours(args, rank, world, local_rank):
     c.variant = args.variant
     W, K = args.warmup, args.steps
     nfr = W + K
-    first = args.first_frame + 7 * rank                       # replicas scan different parts of the trajectory
+    shard_rank, shard_world = (rank, world) if args.shard else (0, 1)
+    if args.shard_of:
+        shard_rank, shard_world = (int(t) for t in args.shard_of.split(","))
+    sharded = shard_world > 1
+    scans = 1 if args.shard else world                        # independent scans in the job
+    first = args.first_frame + (0 if args.shard else 7 * rank)     # replicas scan different parts of the trajectory
     sampler = ClockSampler(local_rank) if rank == 0 else None
     if sampler:
         sampler.start()
@@ -402,7 +413,7 @@ def run_ours(args, rank, world, local_rank):
     mu, sigma = synth.stress_params(c, stress_kind) if stress_kind else (c.mu, c.sigma)
     frames = [upload(synth.stress_frame(c, i, stress_kind) if stress_kind else synth.frame(c, (first + i) % c.n_frames)) for i in range(nfr)]
     vol = vf.Volume(c.dims_geo, c.r, c.origin, c.extent, mu, c.w_max, sigma=sigma, gate=c.gate, device=local_rank,
-                    variant=getattr(c, "variant", 0))
+                    variant=getattr(c, "variant", 0), shard_rank=shard_rank, shard_world=shard_world)
     warm, timed = frames[:W], frames[W:]
     win = Window(vol, timed, c, stream, flush_buf, not args.no_flush)
 
@@ -491,7 +502,7 @@ def run_ours(args, rank, world, local_rank):
     # ---- the saturating frames of SURVEY 8(d) item 5, on volumes of the same size (each kind with the mu / sigma it needs):
     #      counted, profiled and timed like the scan, a few frames each.  Parity: tests/test_gpu_parity.py::test_stress_*.
     stress = None
-    if world == 1 and not stress_kind and not args.no_stress:
+    if world == 1 and not sharded and not stress_kind and not args.no_stress:
         stress = {}
         for kind in synth.STRESS_KINDS:
             s_mu, s_sigma = synth.stress_params(c, kind)
@@ -517,112 +528,116 @@ def run_ours(args, rank, world, local_rank):
             del svol, sfr
             torch.cuda.empty_cache()
 
-    # ---- NEXT row, outside the timed regions: vol_raycast of the volumes as they stand now, from the
-    #      last frame's pose, one 640 x 480 (depth-camera sized) image per call
-    rc_depth = torch.empty(c.wd * c.hd, dtype=torch.float32, device="cuda")
-    rc_rgb = torch.empty(c.wd * c.hd * 3, dtype=torch.uint8, device="cuda")
-    T_last = frames[nfr - 1][4]
-    for _ in range(3):
-        vol.raycast(c.wd, c.hd, T_last, c.K_depth, 0.3, 8.0, rc_depth, rc_rgb, stream=stream)
-    r0 = torch.cuda.Event(enable_timing=True); r1 = torch.cuda.Event(enable_timing=True)
-    torch.cuda.synchronize()
-    r0.record(stream)
-    for _ in range(10):
-        vol.raycast(c.wd, c.hd, T_last, c.K_depth, 0.3, 8.0, rc_depth, rc_rgb, stream=stream)
-    r1.record(stream)
-    torch.cuda.synchronize()
-    raycast_ms = float(r0.elapsed_time(r1)) / 10.0
-    raycast_hit = float((rc_depth > 0).float().mean())
-    for _ in range(3):
-        vol.raycast_trilinear(c.wd, c.hd, T_last, c.K_depth, 0.3, 8.0, rc_depth, rc_rgb, stream=stream)
-    torch.cuda.synchronize()
-    r0.record(stream)
-    for _ in range(10):
-        vol.raycast_trilinear(c.wd, c.hd, T_last, c.K_depth, 0.3, 8.0, rc_depth, rc_rgb, stream=stream)
-    r1.record(stream)
-    torch.cuda.synchronize()
-    raycast_tri_ms = float(r0.elapsed_time(r1)) / 10.0
-    # the same right after a frame has been integrated: the casters' skip flags are rebuilt from the volume first
-    rc_fresh = {}
-    for name, fn in (("nearest", vol.raycast), ("trilinear", vol.raycast_trilinear)):
-        ts = []
-        for fr in frames[-4:]:
-            win.integrate(fr)
+    # (a shard does not hold the whole volume: the rows beyond the hot path are measured on unsharded volumes only)
+    raycast_ms = raycast_hit = raycast_tri_ms = rc_fresh = tracking = sample_ms = sample_filled = sample_tri_ms = None
+    sp_pts = None
+    if not sharded:
+        # ---- NEXT row, outside the timed regions: vol_raycast of the volumes as they stand now, from the
+        #      last frame's pose, one 640 x 480 (depth-camera sized) image per call
+        rc_depth = torch.empty(c.wd * c.hd, dtype=torch.float32, device="cuda")
+        rc_rgb = torch.empty(c.wd * c.hd * 3, dtype=torch.uint8, device="cuda")
+        T_last = frames[nfr - 1][4]
+        for _ in range(3):
+            vol.raycast(c.wd, c.hd, T_last, c.K_depth, 0.3, 8.0, rc_depth, rc_rgb, stream=stream)
+        r0 = torch.cuda.Event(enable_timing=True); r1 = torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        r0.record(stream)
+        for _ in range(10):
+            vol.raycast(c.wd, c.hd, T_last, c.K_depth, 0.3, 8.0, rc_depth, rc_rgb, stream=stream)
+        r1.record(stream)
+        torch.cuda.synchronize()
+        raycast_ms = float(r0.elapsed_time(r1)) / 10.0
+        raycast_hit = float((rc_depth > 0).float().mean())
+        for _ in range(3):
+            vol.raycast_trilinear(c.wd, c.hd, T_last, c.K_depth, 0.3, 8.0, rc_depth, rc_rgb, stream=stream)
+        torch.cuda.synchronize()
+        r0.record(stream)
+        for _ in range(10):
+            vol.raycast_trilinear(c.wd, c.hd, T_last, c.K_depth, 0.3, 8.0, rc_depth, rc_rgb, stream=stream)
+        r1.record(stream)
+        torch.cuda.synchronize()
+        raycast_tri_ms = float(r0.elapsed_time(r1)) / 10.0
+        # the same right after a frame has been integrated: the casters' skip flags are rebuilt from the volume first
+        rc_fresh = {}
+        for name, fn in (("nearest", vol.raycast), ("trilinear", vol.raycast_trilinear)):
+            ts = []
+            for fr in frames[-4:]:
+                win.integrate(fr)
+                r0.record(stream)
+                fn(c.wd, c.hd, T_last, c.K_depth, 0.3, 8.0, rc_depth, None, stream=stream)
+                r1.record(stream)
+                torch.cuda.synchronize()
+                ts.append(float(r0.elapsed_time(r1)))
+            rc_fresh[name] = float(np.mean(ts[1:]))
+        vol.raycast(c.wd, c.hd, T_last, c.K_depth, 0.3, 8.0, rc_depth, rc_rgb, stream=stream)       # (the sampling figures below use these hits)
+        torch.cuda.synchronize()
+        # ---- NEXT row: the tracker -- front end of the last frame, prediction ray-cast from the pose before
+        #      it, coarse-to-fine ICP (19 steps, each a kernel and a 232-byte read-back); the tracked pose against the true one
+        tracking = None
+        if not stress_kind and nfr >= 2:
+            fe = vf.Frontend(c.wd, c.hd, 3, device=local_rank, trilinear_prediction=True)
+            T_prev, dd_last = np.asarray(frames[nfr - 2][4], np.float32), frames[nfr - 1][2]
+            tms = {"measure": [], "predict": [], "track": []}
+            evs = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
+            T_rel, trk_rms, trk_cnt, lost = np.eye(4, dtype=np.float32), float("nan"), 0, None
+            for rep in range(6):
+                evs[0].record(stream)
+                fe.measure(dd_last, c.K_depth, stream=stream)
+                evs[1].record(stream)
+                fe.predict(vol, T_prev, c.K_depth, 0.3, 8.0, stream=stream)
+                evs[2].record(stream)
+                try:
+                    T_rel, trk_rms, trk_cnt = fe.track(stream=stream)
+                except vf.VolError as e:                          # VOL_E_LOST: e.g. the sphere of config 1 (rotations about its centre unobservable)
+                    if e.code != vf.VOL_E_LOST:
+                        raise
+                    lost = str(e)
+                evs[3].record(stream)
+                torch.cuda.synchronize()
+                if rep >= 2:
+                    for k, name in enumerate(("measure", "predict", "track")):
+                        tms[name].append(float(evs[k].elapsed_time(evs[k + 1])))
+            T_trk = T_prev.astype(np.float64) @ T_rel.astype(np.float64)
+            trk_status, trk_level, trk_cond = fe.track_info()
+            tracking = {"status": "lost: " + lost if lost else "ok", "conditioning": trk_cond, "measure_ms": float(np.mean(tms["measure"])), "predict_ms": float(np.mean(tms["predict"])),
+                        "track_ms": float(np.mean(tms["track"])), "icp_steps": 19, "correspondences": int(trk_cnt), "rms_mm": 1e3 * trk_rms,
+                        "pose_error_mm": 1e3 * float(np.linalg.norm(T_trk[:3, 3] - np.asarray(T_last, np.float64)[:3, 3])),
+                        "motion_mm": 1e3 * float(np.linalg.norm(T_prev[:3, 3] - np.asarray(T_last, np.float32)[:3, 3])),
+                        "prediction": "vol_raycast_trilinear, no F8 (opts.trilinear_prediction)",
+                        "note": "vol_frontend_measure / _predict / _track (SURVEY 8(f) rank 4) of the last frame against the fused volumes, "
+                                "not part of the timed step"}
+            fe.close()
+        # ---- NEXT row: vol_sample_colour at surface points -- the ray-cast hit points, 8 jittered copies
+        #      each (about the density of a texture map with Size_pixel = one colour voxel), as a polygon texture map would ask
+        Tl = torch.from_numpy(np.asarray(T_last, np.float32)).cuda()
+        yy, xx = torch.meshgrid(torch.arange(c.hd, device="cuda", dtype=torch.float32), torch.arange(c.wd, device="cuda", dtype=torch.float32), indexing="ij")
+        zz = rc_depth.reshape(c.hd, c.wd)
+        cam = torch.stack([(xx - float(c.K_depth[0, 2])) / float(c.K_depth[0, 0]) * zz, (yy - float(c.K_depth[1, 2])) / float(c.K_depth[1, 1]) * zz, zz], dim=-1)
+        hit_pts = (cam.reshape(-1, 3) @ Tl[:3, :3].T + Tl[:3, 3])[rc_depth > 0]
+        gen = torch.Generator(device="cuda"); gen.manual_seed(1)
+        sp_pts = (hit_pts.repeat(8, 1) + (torch.rand(hit_pts.shape[0] * 8, 3, device="cuda", generator=gen) - 0.5) * (2.0 * c.voxel / c.r)).contiguous()
+        sp_out = torch.empty(sp_pts.shape[0], dtype=torch.int32, device="cuda")
+        sample_ms, sample_filled, sample_tri_ms = None, None, None
+        if sp_pts.shape[0] > 0:
+            for _ in range(3):
+                vol.sample_colour(sp_pts, sp_pts.shape[0], sp_out, stream=stream)
+            torch.cuda.synchronize()
             r0.record(stream)
-            fn(c.wd, c.hd, T_last, c.K_depth, 0.3, 8.0, rc_depth, None, stream=stream)
+            for _ in range(10):
+                vol.sample_colour(sp_pts, sp_pts.shape[0], sp_out, stream=stream)
             r1.record(stream)
             torch.cuda.synchronize()
-            ts.append(float(r0.elapsed_time(r1)))
-        rc_fresh[name] = float(np.mean(ts[1:]))
-    vol.raycast(c.wd, c.hd, T_last, c.K_depth, 0.3, 8.0, rc_depth, rc_rgb, stream=stream)       # (the sampling figures below use these hits)
-    torch.cuda.synchronize()
-    # ---- NEXT row: the tracker -- front end of the last frame, prediction ray-cast from the pose before
-    #      it, coarse-to-fine ICP (19 steps, each a kernel and a 232-byte read-back); the tracked pose against the true one
-    tracking = None
-    if not stress_kind and nfr >= 2:
-        fe = vf.Frontend(c.wd, c.hd, 3, device=local_rank, trilinear_prediction=True)
-        T_prev, dd_last = np.asarray(frames[nfr - 2][4], np.float32), frames[nfr - 1][2]
-        tms = {"measure": [], "predict": [], "track": []}
-        evs = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
-        T_rel, trk_rms, trk_cnt, lost = np.eye(4, dtype=np.float32), float("nan"), 0, None
-        for rep in range(6):
-            evs[0].record(stream)
-            fe.measure(dd_last, c.K_depth, stream=stream)
-            evs[1].record(stream)
-            fe.predict(vol, T_prev, c.K_depth, 0.3, 8.0, stream=stream)
-            evs[2].record(stream)
-            try:
-                T_rel, trk_rms, trk_cnt = fe.track(stream=stream)
-            except vf.VolError as e:                          # VOL_E_LOST: e.g. the sphere of config 1 (rotations about its centre unobservable)
-                if e.code != vf.VOL_E_LOST:
-                    raise
-                lost = str(e)
-            evs[3].record(stream)
+            sample_ms = float(r0.elapsed_time(r1)) / 10.0
+            sample_filled = float(((sp_out.view(torch.int32) >> 24) != 0).float().mean())
+            for _ in range(3):
+                vol.sample_colour_trilinear(sp_pts, sp_pts.shape[0], sp_out, stream=stream)
             torch.cuda.synchronize()
-            if rep >= 2:
-                for k, name in enumerate(("measure", "predict", "track")):
-                    tms[name].append(float(evs[k].elapsed_time(evs[k + 1])))
-        T_trk = T_prev.astype(np.float64) @ T_rel.astype(np.float64)
-        trk_status, trk_level, trk_cond = fe.track_info()
-        tracking = {"status": "lost: " + lost if lost else "ok", "conditioning": trk_cond, "measure_ms": float(np.mean(tms["measure"])), "predict_ms": float(np.mean(tms["predict"])),
-                    "track_ms": float(np.mean(tms["track"])), "icp_steps": 19, "correspondences": int(trk_cnt), "rms_mm": 1e3 * trk_rms,
-                    "pose_error_mm": 1e3 * float(np.linalg.norm(T_trk[:3, 3] - np.asarray(T_last, np.float64)[:3, 3])),
-                    "motion_mm": 1e3 * float(np.linalg.norm(T_prev[:3, 3] - np.asarray(T_last, np.float32)[:3, 3])),
-                    "prediction": "vol_raycast_trilinear, no F8 (opts.trilinear_prediction)",
-                    "note": "vol_frontend_measure / _predict / _track (SURVEY 8(f) rank 4) of the last frame against the fused volumes, "
-                            "not part of the timed step"}
-        fe.close()
-    # ---- NEXT row: vol_sample_colour at surface points -- the ray-cast hit points, 8 jittered copies
-    #      each (about the density of a texture map with Size_pixel = one colour voxel), as a polygon texture map would ask
-    Tl = torch.from_numpy(np.asarray(T_last, np.float32)).cuda()
-    yy, xx = torch.meshgrid(torch.arange(c.hd, device="cuda", dtype=torch.float32), torch.arange(c.wd, device="cuda", dtype=torch.float32), indexing="ij")
-    zz = rc_depth.reshape(c.hd, c.wd)
-    cam = torch.stack([(xx - float(c.K_depth[0, 2])) / float(c.K_depth[0, 0]) * zz, (yy - float(c.K_depth[1, 2])) / float(c.K_depth[1, 1]) * zz, zz], dim=-1)
-    hit_pts = (cam.reshape(-1, 3) @ Tl[:3, :3].T + Tl[:3, 3])[rc_depth > 0]
-    gen = torch.Generator(device="cuda"); gen.manual_seed(1)
-    sp_pts = (hit_pts.repeat(8, 1) + (torch.rand(hit_pts.shape[0] * 8, 3, device="cuda", generator=gen) - 0.5) * (2.0 * c.voxel / c.r)).contiguous()
-    sp_out = torch.empty(sp_pts.shape[0], dtype=torch.int32, device="cuda")
-    sample_ms, sample_filled, sample_tri_ms = None, None, None
-    if sp_pts.shape[0] > 0:
-        for _ in range(3):
-            vol.sample_colour(sp_pts, sp_pts.shape[0], sp_out, stream=stream)
-        torch.cuda.synchronize()
-        r0.record(stream)
-        for _ in range(10):
-            vol.sample_colour(sp_pts, sp_pts.shape[0], sp_out, stream=stream)
-        r1.record(stream)
-        torch.cuda.synchronize()
-        sample_ms = float(r0.elapsed_time(r1)) / 10.0
-        sample_filled = float(((sp_out.view(torch.int32) >> 24) != 0).float().mean())
-        for _ in range(3):
-            vol.sample_colour_trilinear(sp_pts, sp_pts.shape[0], sp_out, stream=stream)
-        torch.cuda.synchronize()
-        r0.record(stream)
-        for _ in range(10):
-            vol.sample_colour_trilinear(sp_pts, sp_pts.shape[0], sp_out, stream=stream)
-        r1.record(stream)
-        torch.cuda.synchronize()
-        sample_tri_ms = float(r0.elapsed_time(r1)) / 10.0
+            r0.record(stream)
+            for _ in range(10):
+                vol.sample_colour_trilinear(sp_pts, sp_pts.shape[0], sp_out, stream=stream)
+            r1.record(stream)
+            torch.cuda.synchronize()
+            sample_tri_ms = float(r0.elapsed_time(r1)) / 10.0
     total_ms, flushed_ms, e2e_ms, e2e_serial_ms = max_over_ranks([total_ms, flushed_ms, e2e_ms, e2e_serial_ms], world, "cuda")
     clocks = sampler.stop() if sampler else None
     if clocks is not None and nvml is not None and nvml.sm:
@@ -636,8 +651,8 @@ def run_ours(args, rank, world, local_rank):
 
     nvox = int(np.prod(c.dims_geo)) * (1 + c.r ** 3)
     ms_per_step = total_ms / K
-    value = whole_job_value(nvox, K, world, total_ms)
-    e2e_value = whole_job_value(nvox, K, world, e2e_ms)
+    value = whole_job_value(nvox, K, scans, total_ms)
+    e2e_value = whole_job_value(nvox, K, scans, e2e_ms)
     fused_ms = kms[:, 2]
     av, asec, tch, tchs = bytes_of(cnt, frame_bytes)
     wl_key = c.name + (f"-stress-{stress_kind}" if stress_kind else "") + (f"-variant{args.variant}" if args.variant else "")
@@ -652,7 +667,7 @@ def run_ours(args, rank, world, local_rank):
                  "issue": issue_roofline(rec, float(fused_ms.mean()), (clocks or {}).get("sm_mhz"), n_sms)})
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
-        "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "strong" if args.shard else "weak", "vs_baseline": None,
         "dtype": "f32", "data": "synthetic",
         "config": {"workload": workload_name(c) + (f" -- STRESS: saturating frame ({stress_kind})" if stress_kind else ""),
                    "value_kind": "visited: (N_geo + N_col) voxels brought up to date per frame x frames / device time -- about 1 % of them "
@@ -660,13 +675,16 @@ def run_ours(args, rank, world, local_rank):
                    "frames": "one saturating pose, the wall moving" if stress_kind else f"{first}..{first + nfr - 1} of the seeded trajectory",
                    "l2": "no flush: inputs larger than L2 -- K distinct frames of 6.8 MB, each touching > 100 MB of volumes of 2.7 GB "
                          "(126 MB L2); the figure with a 512 MiB flush before every frame is under \"flushed\"",
-                   "parallelism": "single GPU" if world == 1 else f"{world} replicas (independent scans), no data-path collective"},
-        "frames_per_s": world * K / (total_ms * 1e-3),
-        "applied_updates_per_s": world * float(cnt[:, 0].sum() + cnt[:, 2].sum()) / (total_ms * 1e-3),
+                   "parallelism": (f"shard {shard_rank} of {shard_world} alone (z-slabs {shard_rank} mod {shard_world}): its share of one scan" if args.shard_of else
+                                   "single GPU" if world == 1 else
+                                   f"one scan on {world} z-slab shards, every rank receives every frame, no data-path collective; counters are rank 0's shard" if args.shard else
+                                   f"{world} replicas (independent scans), no data-path collective")},
+        "frames_per_s": scans * K / (total_ms * 1e-3),
+        "applied_updates_per_s": scans * float(cnt[:, 0].sum() + cnt[:, 2].sum()) / (total_ms * 1e-3),
         "per_frame_ms": {"median": float(np.median(per_frame_ms)), "p95": float(np.percentile(per_frame_ms, 95)), "min": float(per_frame_ms.min())},
         "kernel_ms_mean": {"prepass": float(kms[:, 0].mean()), "fused": float(fused_ms.mean())},
         "flushed": None if args.no_flush else {
-            "ms_per_step": flushed_ms / K, "value": whole_job_value(nvox, K, world, flushed_ms),
+            "ms_per_step": flushed_ms / K, "value": whole_job_value(nvox, K, scans, flushed_ms),
             "note": "the same K frames timed one by one (a pair of events around each, L2 flushed by a 512 MiB memset before each; "
                     "per_frame_ms are these): round 1's headline method.  Nothing can overlap from one frame to the next "
                     "here; in the timed region proper the next frame's pre-pass starts under the tail of the fused kernel "
@@ -684,10 +702,10 @@ def run_ours(args, rank, world, local_rank):
                 "d2h_bytes_per_step": vf.VOL_STATS_RAW_BYTES,
                 "mode": "vol_integrate_host + vol_frame_stats_async per frame, frames enqueued back to back (a recorded "
                         "sequence): the copies of frame n + 1 overlap the kernels of frame n",
-                "one_frame_at_a_time": {"value": whole_job_value(nvox, K, world, e2e_serial_ms), "ms_per_step": e2e_serial_ms / K,
+                "one_frame_at_a_time": {"value": whole_job_value(nvox, K, scans, e2e_serial_ms), "ms_per_step": e2e_serial_ms / K,
                                         "mode": "vol_integrate_host + vol_frame_stats (synchronises) per frame (a live scan)"}},
         "tracking": tracking,
-        "raycast": {"ms": raycast_ms, "rays_per_s": c.wd * c.hd / (raycast_ms * 1e-3), "image": f"{c.wd}x{c.hd}", "hit_fraction": raycast_hit,
+        "raycast": None if raycast_ms is None else {"ms": raycast_ms, "rays_per_s": c.wd * c.hd / (raycast_ms * 1e-3), "image": f"{c.wd}x{c.hd}", "hit_fraction": raycast_hit,
                     "trilinear_ms": raycast_tri_ms, "after_a_new_frame_ms": rc_fresh,
                     "note": "vol_raycast / vol_raycast_trilinear of the fused volumes (SURVEY 8(f) rank 1), not part of the timed step; "
                             "ms: repeated casts of an unchanged volume; after_a_new_frame_ms: depth only, including the rebuild of the "
