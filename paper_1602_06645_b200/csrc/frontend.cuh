@@ -18,12 +18,32 @@ constexpr int ICP_SUMS = 29;                  // 21 (upper triangle of A) + 6 (b
 struct LevelK { float fx, fy, cx, cy; };
 
 // F1: bilateral filter of the raw depth.  ws: 49 spatial weights [dy + 3][dx + 3]; wr: kmax + 1 range weights over whole mm.
-__global__ void __launch_bounds__(256) k_bilateral(const uint16_t *__restrict__ depth, int w, int h, const float *__restrict__ ws,
+// A CTA filters 32 x 8 pixels from a shared-memory tile of 38 x 14 (the 7 x 7 windows of neighbouring pixels overlap in 42 of
+// their 49 pixels).  FROM_FLOAT: the input is float metres and F8's rounding to whole millimetres (half-even, clamped to
+// 65535) is done while the tile is loaded.
+template <bool FROM_FLOAT>
+__global__ void __launch_bounds__(256) k_bilateral(const void *__restrict__ in, int w, int h, const float *__restrict__ ws,
                                                    const float *__restrict__ wr, int kmax, float *__restrict__ out)
 {
-    const int x = blockIdx.x * 32 + (threadIdx.x & 31), y = blockIdx.y * 8 + (threadIdx.x >> 5);
+    constexpr int TW = 32 + 2 * FE_RADIUS, TH = 8 + 2 * FE_RADIUS;
+    __shared__ uint16_t tile[TH][TW + 2];
+    __shared__ float s_ws[49];
+    const int x0 = blockIdx.x * 32 - FE_RADIUS, y0 = blockIdx.y * 8 - FE_RADIUS;
+    for (int i = threadIdx.x; i < TW * TH; i += 256) {
+        const int tx = i % TW, ty = i / TW, xx = x0 + tx, yy = y0 + ty;
+        uint16_t v = 0;                                       // outside the image: never used (the window is clipped below)
+        if (xx >= 0 && xx < w && yy >= 0 && yy < h) {
+            if (FROM_FLOAT) v = (uint16_t)fminf(rintf(__fmul_rn(__ldg(static_cast<const float *>(in) + (size_t)yy * w + xx), 1000.0f)), 65535.0f);
+            else v = __ldg(static_cast<const uint16_t *>(in) + (size_t)yy * w + xx);
+        }
+        tile[ty][tx] = v;
+    }
+    if (threadIdx.x < 49) s_ws[threadIdx.x] = __ldg(ws + threadIdx.x);
+    __syncthreads();
+    const int lx = threadIdx.x & 31, ly = threadIdx.x >> 5;
+    const int x = blockIdx.x * 32 + lx, y = blockIdx.y * 8 + ly;
     if (x >= w || y >= h) return;
-    const int d = (int)__ldg(depth + (size_t)y * w + x);
+    const int d = (int)tile[ly + FE_RADIUS][lx + FE_RADIUS];
     float r = 0.0f;
     if (d > 0) {
         float sw = 0.0f, sd = 0.0f;
@@ -35,10 +55,10 @@ __global__ void __launch_bounds__(256) k_bilateral(const uint16_t *__restrict__ 
             for (int dx = -FE_RADIUS; dx <= FE_RADIUS; ++dx) {
                 const int xx = x + dx;
                 if (xx < 0 || xx >= w) continue;
-                const int q = (int)__ldg(depth + (size_t)yy * w + xx);
+                const int q = (int)tile[ly + FE_RADIUS + dy][lx + FE_RADIUS + dx];
                 const int delta = abs(q - d);
                 if (q > 0 && delta <= kmax) {
-                    const float wgt = __fmul_rn(__ldg(ws + (dy + FE_RADIUS) * 7 + (dx + FE_RADIUS)), __ldg(wr + delta));
+                    const float wgt = __fmul_rn(s_ws[(dy + FE_RADIUS) * 7 + (dx + FE_RADIUS)], __ldg(wr + delta));
                     sw = __fadd_rn(sw, wgt);
                     sd = __fadd_rn(sd, __fmul_rn(wgt, (float)q));
                 }
@@ -49,21 +69,10 @@ __global__ void __launch_bounds__(256) k_bilateral(const uint16_t *__restrict__ 
     out[(size_t)y * w + x] = r;
 }
 
-// F8: float metres -> whole millimetres (half-even, clamped), the input format of F1
-__global__ void __launch_bounds__(256) k_to_millimetres(const float *__restrict__ in, int n, uint16_t *__restrict__ out)
+// F2 for one output pixel: the 2 x 2 block (v[0] = the block's first pixel) -> its mean over the valid pixels within thr of v[0]
+__device__ __forceinline__ float fe_half_sample(const float (&v)[4], float thr)
 {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < n) out[i] = (uint16_t)fminf(rintf(__fmul_rn(__ldg(in + i), 1000.0f)), 65535.0f);
-}
-
-// F2: next pyramid level (w, h = size of the OUTPUT level)
-__global__ void __launch_bounds__(256) k_half_sample(const float *__restrict__ in, int w, int h, float thr, float *__restrict__ out)
-{
-    const int x = blockIdx.x * 32 + (threadIdx.x & 31), y = blockIdx.y * 8 + (threadIdx.x >> 5);
-    if (x >= w || y >= h) return;
-    const float2 r0 = __ldg(reinterpret_cast<const float2 *>(in + (size_t)(2 * y) * (2 * w) + 2 * x));
-    const float2 r1 = __ldg(reinterpret_cast<const float2 *>(in + (size_t)(2 * y + 1) * (2 * w) + 2 * x));
-    const float c = r0.x, v[4] = {r0.x, r0.y, r1.x, r1.y};
+    const float c = v[0];
     float res = 0.0f;
     if (c > 0.0f) {
         float s = 0.0f, n = 0.0f;
@@ -72,7 +81,31 @@ __global__ void __launch_bounds__(256) k_half_sample(const float *__restrict__ i
             if (v[i] > 0.0f && fabsf(__fsub_rn(v[i], c)) <= thr) { s = __fadd_rn(s, v[i]); n = __fadd_rn(n, 1.0f); }
         res = __fdiv_rn(s, n);
     }
-    out[(size_t)y * w + x] = res;
+    return res;
+}
+
+// F2, every level in ONE launch: a thread owns one pixel of the coarsest level, i.e. a square block of 2^(levels-1) pixels
+// of level 0, and builds the levels of that block one after the other (level l reads the values the same thread has just
+// written for level l - 1).  D[l]: depth map of level l, w0 x h0 the size of level 0.
+struct PyramidParams { float *D[FE_MAX_LEVELS]; int levels, w0, h0; float thr; };
+__global__ void __launch_bounds__(256) k_pyramid_depth(const __grid_constant__ PyramidParams q)
+{
+    const int top = q.levels - 1, wt = q.w0 >> top, ht = q.h0 >> top;
+    const int X = blockIdx.x * 32 + (threadIdx.x & 31), Y = blockIdx.y * 8 + (threadIdx.x >> 5);
+    if (X >= wt || Y >= ht) return;
+    for (int l = 1; l <= top; ++l) {
+        const int wl = q.w0 >> l, side = 1 << (top - l);                  // this thread's block at level l is side x side
+        const float *in = q.D[l - 1];
+        float *out = q.D[l];
+        for (int by = 0; by < side; ++by)
+            for (int bx = 0; bx < side; ++bx) {
+                const int x = X * side + bx, y = Y * side + by;
+                const float2 r0 = *reinterpret_cast<const float2 *>(in + (size_t)(2 * y) * (2 * wl) + 2 * x);
+                const float2 r1 = *reinterpret_cast<const float2 *>(in + (size_t)(2 * y + 1) * (2 * wl) + 2 * x);
+                const float v[4] = {r0.x, r0.y, r1.x, r1.y};
+                out[(size_t)y * wl + x] = fe_half_sample(v, q.thr);
+            }
+    }
 }
 
 // F3 = eq. 7: the vertex of pixel (x, y) with depth D
@@ -81,11 +114,20 @@ __device__ __forceinline__ float3 fe_vertex(const LevelK k, int x, int y, float 
     return make_float3(__fdiv_rn(__fmul_rn(__fsub_rn((float)x, k.cx), D), k.fx), __fdiv_rn(__fmul_rn(__fsub_rn((float)y, k.cy), D), k.fy), D);
 }
 
-// F3 + F4 of one level: V (xyz, w = 0) and N (eq. 8 normalised; zero where a neighbour is missing or invalid)
-__global__ void __launch_bounds__(256) k_vertex_normal(const float *__restrict__ D, int w, int h, const LevelK k, float4 *__restrict__ V,
-                                                       float4 *__restrict__ N)
+// F3 + F4 of every level in ONE launch: V (xyz, w = 0) and N (eq. 8 normalised; zero where a neighbour is missing or invalid).
+// The CTAs of the levels follow one another in the grid (first_block).
+struct MapLevel { const float *D; float4 *V, *N; int w, h; LevelK k; unsigned first_block, blocks_x; };
+struct MapParams { MapLevel lv[FE_MAX_LEVELS]; int levels; };
+__global__ void __launch_bounds__(256) k_vertex_normal(const __grid_constant__ MapParams q)
 {
-    const int x = blockIdx.x * 32 + (threadIdx.x & 31), y = blockIdx.y * 8 + (threadIdx.x >> 5);
+    int l = 0;
+    while (l + 1 < q.levels && blockIdx.x >= q.lv[l + 1].first_block) ++l;
+    const MapLevel &m = q.lv[l];
+    const unsigned blk = blockIdx.x - m.first_block;
+    const int w = m.w, h = m.h;
+    const LevelK k = m.k;
+    const float *__restrict__ D = m.D;
+    const int x = (int)(blk % m.blocks_x) * 32 + (threadIdx.x & 31), y = (int)(blk / m.blocks_x) * 8 + (threadIdx.x >> 5);
     if (x >= w || y >= h) return;
     const size_t o = (size_t)y * w + x;
     const float d0 = __ldg(D + o);
@@ -107,7 +149,7 @@ __global__ void __launch_bounds__(256) k_vertex_normal(const float *__restrict__
             }
         }
     }
-    V[o] = v; N[o] = n;
+    m.V[o] = v; m.N[o] = n;
 }
 
 

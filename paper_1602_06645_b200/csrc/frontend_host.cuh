@@ -16,7 +16,6 @@ struct vol_frontend {
     vf::LevelK k[2][vf::FE_MAX_LEVELS];
     bool have[2];
     float *ray_depth;                                       // vol_frontend_predict: the ray-cast depth map
-    uint16_t *pred_mm;                                      // F8: the prediction in whole millimetres
     unsigned long long *acc_dev, *acc_pinned;               // vol_frontend_icp_step: ICP_ACC integer accumulators
     unsigned long long *track_acc; size_t track_steps;      // vol_frontend_track: one set of accumulators per step
     double *track_out, *track_out_pinned;                   // FE_TRACK_OUT doubles: T (3 x 4), rms, count, status, level, conditioning
@@ -41,7 +40,6 @@ extern "C" void vol_frontend_destroy(vol_frontend_t *fe)
             if (fe->N[s][l]) cudaFree(fe->N[s][l]);
         }
     if (fe->ray_depth) cudaFree(fe->ray_depth);
-    if (fe->pred_mm) cudaFree(fe->pred_mm);
     if (fe->acc_dev) cudaFree(fe->acc_dev);
     if (fe->acc_pinned) cudaFreeHost(fe->acc_pinned);
     if (fe->track_acc) cudaFree(fe->track_acc);
@@ -87,7 +85,6 @@ extern "C" int vol_frontend_create(vol_frontend_t **out, int32_t w, int32_t h, i
     auto fail = [&](int code) { delete[] wr; vol_frontend_destroy(fe); return code; };
     bool okc = cudaMalloc(&fe->ws, sizeof ws) == cudaSuccess && cudaMalloc(&fe->wr, sizeof(float) * (fe->kmax + 1)) == cudaSuccess &&
                cudaMalloc(&fe->ray_depth, sizeof(float) * (size_t)w * h) == cudaSuccess &&
-               cudaMalloc(&fe->pred_mm, sizeof(uint16_t) * (size_t)w * h) == cudaSuccess &&
                cudaMalloc(&fe->acc_dev, sizeof(unsigned long long) * vf::ICP_ACC) == cudaSuccess &&
                cudaMallocHost(&fe->acc_pinned, sizeof(unsigned long long) * vf::ICP_ACC) == cudaSuccess &&
                cudaMalloc(&fe->track_out, sizeof(double) * FE_TRACK_OUT) == cudaSuccess &&
@@ -110,22 +107,32 @@ extern "C" int vol_frontend_create(vol_frontend_t **out, int32_t w, int32_t h, i
     return VOL_OK;
 }
 
-// F2-F4 for every level of side s, from its level-0 depth map
+// F2-F4 for every level of side s, from its level-0 depth map: two launches (all depth levels, then all vertex / normal maps)
 static int fe_build_pyramid(vol_frontend *fe, int s, const float K[9], cudaStream_t st)
 {
     vf::LevelK k = {K[0], K[4], K[2], K[5]};
-    const float thr = 3.0f * fe->sigma_r;
+    vf::PyramidParams pq; vf::MapParams mq;
+    memset(&pq, 0, sizeof pq); memset(&mq, 0, sizeof mq);
+    pq.levels = mq.levels = fe->levels; pq.w0 = fe->w; pq.h0 = fe->h; pq.thr = 3.0f * fe->sigma_r;
+    unsigned first = 0;
     for (int l = 0; l < fe->levels; ++l) {
         const int w = fe->w >> l, h = fe->h >> l;
-        const dim3 grid((w + 31) / 32, (h + 7) / 8);
         if (l > 0) {
             k.fx = k.fx * 0.5f; k.fy = k.fy * 0.5f;
             k.cx = (k.cx - 0.5f) * 0.5f; k.cy = (k.cy - 0.5f) * 0.5f;
-            vf::k_half_sample<<<grid, 256, 0, st>>>(fe->D[s][l - 1], w, h, thr, fe->D[s][l]);
         }
         fe->k[s][l] = k;
-        vf::k_vertex_normal<<<grid, 256, 0, st>>>(fe->D[s][l], w, h, k, fe->V[s][l], fe->N[s][l]);
+        pq.D[l] = fe->D[s][l];
+        vf::MapLevel &m = mq.lv[l];
+        m.D = fe->D[s][l]; m.V = fe->V[s][l]; m.N = fe->N[s][l]; m.w = w; m.h = h; m.k = k;
+        m.first_block = first; m.blocks_x = (unsigned)((w + 31) / 32);
+        first += m.blocks_x * (unsigned)((h + 7) / 8);
     }
+    if (fe->levels > 1) {
+        const int top = fe->levels - 1, wt = fe->w >> top, ht = fe->h >> top;
+        vf::k_pyramid_depth<<<dim3((wt + 31) / 32, (ht + 7) / 8), 256, 0, st>>>(pq);
+    }
+    vf::k_vertex_normal<<<first, 256, 0, st>>>(mq);
     CK(cudaGetLastError());
     fe->have[s] = true;
     return VOL_OK;
@@ -136,7 +143,7 @@ extern "C" int vol_frontend_measure(vol_frontend_t *fe, const uint16_t *depth_u1
     if (!fe || !depth_u16_dev || !K || !intrinsics_ok(K)) return VOL_E_ARG;
     int rc = fe_set_device(fe); if (rc) return rc;
     cudaStream_t st = (cudaStream_t)stream;
-    vf::k_bilateral<<<dim3((fe->w + 31) / 32, (fe->h + 7) / 8), 256, 0, st>>>(depth_u16_dev, fe->w, fe->h, fe->ws, fe->wr, fe->kmax, fe->D[0][0]);
+    vf::k_bilateral<false><<<dim3((fe->w + 31) / 32, (fe->h + 7) / 8), 256, 0, st>>>(depth_u16_dev, fe->w, fe->h, fe->ws, fe->wr, fe->kmax, fe->D[0][0]);
     return fe_build_pyramid(fe, 0, K, st);
 }
 
@@ -146,9 +153,8 @@ extern "C" int vol_frontend_predict_depth(vol_frontend_t *fe, const float *depth
     int rc = fe_set_device(fe); if (rc) return rc;
     cudaStream_t st = (cudaStream_t)stream;
     const int n = fe->w * fe->h;
-    if (filter) {                                            // F8
-        vf::k_to_millimetres<<<(n + 255) / 256, 256, 0, st>>>(depth_m_dev, n, fe->pred_mm);
-        vf::k_bilateral<<<dim3((fe->w + 31) / 32, (fe->h + 7) / 8), 256, 0, st>>>(fe->pred_mm, fe->w, fe->h, fe->ws, fe->wr, fe->kmax, fe->D[1][0]);
+    if (filter) {                                            // F8: rounding to millimetres inside the filter's tile load
+        vf::k_bilateral<true><<<dim3((fe->w + 31) / 32, (fe->h + 7) / 8), 256, 0, st>>>(depth_m_dev, fe->w, fe->h, fe->ws, fe->wr, fe->kmax, fe->D[1][0]);
     } else {
         CK(cudaMemcpyAsync(fe->D[1][0], depth_m_dev, sizeof(float) * (size_t)n, cudaMemcpyDeviceToDevice, st));
     }
