@@ -145,7 +145,7 @@ struct Counts { unsigned long long n[CNT_N]; };
 #ifndef VF_COL_BATCH
 #define VF_COL_BATCH 4
 #endif
-constexpr uint32_t COL_BATCH = VF_COL_BATCH, COL_BATCH_TAIL = 12, GEO_BATCH = 2;
+constexpr uint32_t COL_BATCH = VF_COL_BATCH, COL_BATCH_TAIL = 12, GEO_BATCH = 1;
 // per-warp state of the consumer loop (shared memory; written by lane 0 between __syncwarp()s, read by every lane): the items
 // need every register, and what is kept in shared memory is not spilled to (cached, evictable) local memory around them
 enum : uint32_t { F_GEO_DONE = 1u, F_COL_DONE = 2u, F_MARKS_SET = 4u, F_SCAN_CLAIMED = 8u, F_COL_READY = 16u, F_CLS_COMPLETE = 32u };
@@ -677,7 +677,7 @@ __global__ void __launch_bounds__(CTA, VF_MIN_CTAS) k_fused(const __grid_constan
     // ---- consumer: colour items once they exist (they are the longer ones), geometry items otherwise.
     // Every access to the queues is an L2 round trip of the order of a microsecond under load, so a round of the loop first
     // ISSUES whatever it may need (the progress counter it is watching, the slot of its geometry ticket) and only then looks at
-    // the answers; tickets are drawn for several items at once.  The state of the loop lives in shared memory: the items need
+    // the answers; colour tickets are drawn for several items at once (geometry tickets one by one: measured, balance is worth more).  The state of the loop lives in shared memory: the items need
     // every register, and what is kept in shared memory is not spilled to (cached, evictable) local memory around them.
     volatile WarpState &ws = s_state[threadIdx.x >> 5];
     if (lane == 0) {
