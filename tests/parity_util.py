@@ -34,7 +34,59 @@ def integrate_both(g, o, c, depth, rgb, T, counting=True):
     return st, cnt
 
 
-def compare_states(g, o, where=""):
+def describe_mismatches(geo, og, col, oc, o, frame=None, limit=4):
+    """Text for a failing comparison: the first differing voxels of each volume with their indices and the fields
+    of both words; with frame = (c, depth, T_world_depth) also, in binary64, where the voxel projects in that depth frame and
+    how far it is from the decisions that gate its update: geometry (u, v), sdf + mu; colour (u, v), d^2 - sigma^2."""
+    lines = []
+    ctx = None
+    if frame is not None:
+        c, depth, T = frame
+        Ti = np.linalg.inv(np.asarray(T, np.float64).reshape(4, 4))
+        K = np.asarray(c.K_depth, np.float64).reshape(3, 3)
+        ctx = (c, np.asarray(depth), Ti, K)
+
+    def project(idx, dims, vs):
+        nx, ny, _ = dims
+        i, j, k = int(idx % nx), int((idx // nx) % ny), int(idx // (nx * ny))
+        txt = f"({i}, {j}, {k})"
+        if ctx is None:
+            return txt, None
+        c, depth, Ti, K = ctx
+        pw = np.asarray(o.desc.origin, np.float64) + (np.array([i, j, k]) + 0.5) * vs
+        pc = Ti[:3, :3] @ pw + Ti[:3, 3]
+        if pc[2] <= 0:
+            return txt + " behind the camera", None
+        u, v = K[0, 0] * pc[0] / pc[2] + K[0, 2], K[1, 1] * pc[1] / pc[2] + K[1, 2]
+        ui, vi = int(np.floor(u + 0.5)), int(np.floor(v + 0.5))
+        inside = 0 <= ui < depth.shape[1] and 0 <= vi < depth.shape[0]
+        d = float(depth[vi, ui]) * 1e-3 if inside else 0.0
+        return txt + f" -> (u, v) = ({u:.4f}, {v:.4f}), Z = {pc[2]:.6f}, D = {d:.3f}", (pc, ui, vi, d, K)
+
+    vs = float(o.desc.extent) / int(o.desc.nx)
+    for name, a, b, dims, size, fields in (("geometry", geo, og, (int(o.desc.nx), int(o.desc.ny), int(o.desc.nz)), vs,
+                                            lambda w: f"q = {int(np.int16(w & 0xffff))}, w = {int(w >> 16)}"),
+                                           ("colour", col, oc, tuple(int(x) * int(o.desc.r) for x in (o.desc.nx, o.desc.ny, o.desc.nz)), vs / int(o.desc.r),
+                                            lambda w: f"rgb = ({int(w & 255)}, {int((w >> 8) & 255)}, {int((w >> 16) & 255)}), wq = {int(w >> 24)}")):
+        bad = np.flatnonzero(a.reshape(-1) != b.reshape(-1))
+        if bad.size == 0:
+            continue
+        lines.append(f"{name}: {bad.size} words differ")
+        for idx in bad[:limit]:
+            where, pr = project(int(idx), dims, size)
+            extra = ""
+            if pr is not None and pr[3] > 0:
+                pc, ui, vi, d, K = pr
+                if name == "geometry":
+                    extra = f", sdf + mu = {d - pc[2] + float(o.desc.mu):.6f}"
+                else:
+                    pvd = np.array([(ui - K[0, 2]) * d / K[0, 0], (vi - K[1, 2]) * d / K[1, 1], d])
+                    extra = f", d^2 - sigma^2 = {float(((pc - pvd) ** 2).sum()) - float(o.desc.sigma) ** 2:.3e}"
+            lines.append(f"  voxel {where}{extra}: CUDA {fields(int(a.reshape(-1)[idx]))} | oracle {fields(int(b.reshape(-1)[idx]))}")
+    return "\n".join(lines)
+
+
+def compare_states(g, o, where="", frame=None):
     """Parity bar (BASELINE.json north_star): geometry weight and colour weight bit-exact, TSDF within 1e-5 after
     dequantisation (one q step is 3.05e-5, so this means identical q), colour channels within 1 LSB.  Under the
     canonical arithmetic the words are in fact byte-identical, which is what is asserted; the looser bar is evaluated
@@ -43,13 +95,15 @@ def compare_states(g, o, where=""):
     og, oc = o.geo, o.col
     assert geo.shape == og.shape and col.shape == oc.shape
     dq = np.abs(oracle.geo_q(geo) - oracle.geo_q(og))
+    if not (np.array_equal(geo, og) and np.array_equal(col, oc)):
+        print(describe_mismatches(geo, og, col, oc, o, frame))          # shown by pytest with the failing assertion below
     assert np.array_equal(oracle.geo_w(geo), oracle.geo_w(og)), f"{where}: geometry weights differ"
     assert dq.max() / 32767.0 <= 1e-5, f"{where}: TSDF differs, max |dq| = {dq.max()} at {int((dq > 0).sum())} voxels"
     assert np.array_equal(oracle.col_w(col), oracle.col_w(oc)), f"{where}: colour weights differ at {int((oracle.col_w(col) != oracle.col_w(oc)).sum())} voxels"
     dc = np.abs(oracle.col_rgb(col) - oracle.col_rgb(oc))
     assert dc.max() <= 1, f"{where}: colour differs by {dc.max()}"
     n_bad = int((geo != og).sum()) + int((col != oc).sum())
-    assert n_bad == 0, f"{where}: {n_bad} words not byte-identical"
+    assert n_bad == 0, f"{where}: {n_bad} words not byte-identical\n" + describe_mismatches(geo, og, col, oc, o, frame)
     return geo, col
 
 
@@ -69,7 +123,7 @@ def run_sequence(c, frames, counting=True, check_every=1, **kw):
         if counting:
             check_counters(st, cnt, f"{c.name} frame {fi}")
         if (n + 1) % check_every == 0 or n == len(frames) - 1:
-            compare_states(g, o, f"{c.name} frame {fi}")
+            compare_states(g, o, f"{c.name} frame {fi}", frame=(c, depth, T))
     return g, o
 
 

@@ -69,3 +69,24 @@ def test_no_cpu_fallback_without_a_gpu():
     with pytest.raises(vf.VolError) as e:
         vf.Volume((8, 8, 8), 2, (0, 0, 0), 1.0, 0.1, 128)
     assert e.value.code == vf.VOL_E_CUDA
+
+
+def test_parity_harness_describes_a_mismatch():
+    """tests/parity_util.describe_mismatches (SURVEY 8(c) diagnostics): a word changed by hand is reported with its voxel
+    index, both words' fields and where the voxel stands relative to the decisions that gate its update."""
+    import numpy as np
+    import oracle
+    import synth
+    from parity_util import describe_mismatches
+    c = synth.config(1).scaled(32, 2)
+    o = oracle.RefVolume(c.dims_geo, c.r, c.origin, c.extent, c.mu, c.w_max)
+    depth, rgb, T = synth.frame(c, 0)
+    o.integrate(depth, rgb, T, c.K_depth, c.K_rgb, c.T_depth_rgb)
+    geo, col = o.geo.copy(), o.col.copy()
+    assert describe_mismatches(geo, o.geo, col, o.col, o) == ""
+    gi, ci = np.flatnonzero(geo)[100], np.flatnonzero(col)[50]
+    geo.reshape(-1)[gi] ^= 1
+    col.reshape(-1)[ci] ^= 0x100
+    txt = describe_mismatches(geo, o.geo, col, o.col, o, (c, depth, T))
+    assert "geometry: 1 words differ" in txt and "colour: 1 words differ" in txt
+    assert "sdf + mu" in txt and "d^2 - sigma^2" in txt and "(u, v)" in txt and "oracle q =" in txt
