@@ -220,6 +220,7 @@ __device__ __forceinline__ void icp_accumulate(double (&s)[ICP_SUMS], const floa
 // the blocks arrive (binary64 atomicAdd would).  |a| is far below 2^42 for maps in metres (at most 2^19 pixels x (10 m)^2);
 // it is clamped there so that a corrupt map cannot overflow the integers.
 constexpr int ICP_ACC = 2 * ICP_SUMS;          // int64 words per set of accumulators: hi[ICP_SUMS], lo[ICP_SUMS]
+constexpr int TRACK_STRIDE = 64;               // k_icp_track: words per step -- ICP_ACC accumulators, then the step's arrival counter
 
 __device__ __forceinline__ void icp_publish(double a, unsigned long long *acc)
 {
@@ -334,7 +335,7 @@ __device__ inline int icp_se3_update(double *T, const double *sums, double cond_
 }
 
 // F7 in ONE cooperative launch (vol_frontend_track): every step is a grid-stride pass over the level's pixels into its own
-// set of accumulators (all zeroed before the launch), one grid-wide barrier, and the 6 x 6 solve -- done redundantly by one
+// set of accumulators (all zeroed before the launch), one grid-wide barrier (an arrival counter), and the 6 x 6 solve -- done redundantly by one
 // thread of every block (29 values in, 12 out: cheaper than a second barrier to broadcast the result).
 struct TrackParams {
     IcpLevel lv[FE_MAX_LEVELS];
@@ -342,7 +343,7 @@ struct TrackParams {
     float dist2, cos_min;
     double T0[12];                  // initial estimate
     double cond_min;                // icp_se3_update's threshold
-    unsigned long long *acc;        // total steps x ICP_ACC integer accumulators, zeroed
+    unsigned long long *acc;        // total steps x TRACK_STRIDE words (accumulators and arrival counter of every step), zeroed
     double *out;                    // 12 (T) + rms + count + status (0 ok, 1 too few correspondences, 2 not positive definite,
                                     // 3 unobservable) + level + conditioning of the last step solved
 };
@@ -350,7 +351,6 @@ struct TrackParams {
 __global__ void __launch_bounds__(256) k_icp_track(const __grid_constant__ TrackParams q)
 {
     __shared__ double sh[8][ICP_SUMS], shT[16];
-    cooperative_groups::grid_group grid = cooperative_groups::this_grid();
     double T[12];
 #pragma unroll
     for (int i = 0; i < 12; ++i) T[i] = q.T0[i];
@@ -371,11 +371,17 @@ __global__ void __launch_bounds__(256) k_icp_track(const __grid_constant__ Track
                 float J[6], r;
                 if (x < lv.w && y < lv.h && icp_pixel(lv, R, t, q.dist2, q.cos_min, x, y, J, r)) icp_accumulate(s, J, r);
             }
-            unsigned long long *acc = q.acc + (size_t)step * ICP_ACC;
-            icp_block_reduce(s, sh, acc);
-            __threadfence();
-            grid.sync();
+            unsigned long long *acc = q.acc + (size_t)step * TRACK_STRIDE;
+            icp_block_reduce(s, sh, acc);                        // (ends with a block barrier: this block's reductions have been issued)
             if (threadIdx.x == 0) {                              // one thread per block solves; the others take its result
+                // the grid-wide barrier of this step: one arrival counter per step (zeroed with the accumulators), bumped with
+                // release semantics -- cumulative over the block's reductions through the block barrier above -- and polled with
+                // acquire loads.  All blocks are co-resident (cooperative launch).  Lighter than grid.sync(): no system-scope
+                // fence, no L1 invalidation, and only the thread that needs the sums waits for them.
+                unsigned *arrive = reinterpret_cast<unsigned *>(acc + ICP_ACC);
+                asm volatile("red.release.gpu.global.add.u32 [%0], 1;" ::"l"(arrive) : "memory");
+                unsigned seen;
+                do { asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(seen) : "l"(arrive) : "memory"); } while (seen < gridDim.x);
                 double g[ICP_SUMS];
 #pragma unroll
                 for (int i = 0; i < ICP_SUMS; ++i) g[i] = icp_total((long long)__ldcg(acc + i), (long long)__ldcg(acc + ICP_SUMS + i));

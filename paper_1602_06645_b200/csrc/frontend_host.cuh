@@ -102,7 +102,7 @@ extern "C" int vol_frontend_create(vol_frontend_t **out, int32_t w, int32_t h, i
     int occ = 0, sms = 0;
     if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, vf::k_icp_track, 256, 0) != cudaSuccess || occ < 1 ||
         cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device) != cudaSuccess) { vol_frontend_destroy(fe); return VOL_E_CUDA; }
-    fe->track_blocks = occ * sms;
+    fe->track_blocks = (occ < 2 ? occ : 2) * sms;           // two blocks per SM: measured equal to full occupancy, a quarter of the reductions
     *out = fe;
     return VOL_OK;
 }
@@ -222,7 +222,7 @@ extern "C" int vol_frontend_track(vol_frontend_t *fe, const float T_init[16], co
     cudaStream_t st = (cudaStream_t)stream;
     if (steps > fe->track_steps) {
         if (fe->track_acc) { CK(cudaDeviceSynchronize()); cudaFree(fe->track_acc); fe->track_acc = nullptr; fe->track_steps = 0; }
-        CK(cudaMalloc(&fe->track_acc, steps * vf::ICP_ACC * sizeof(unsigned long long)));
+        CK(cudaMalloc(&fe->track_acc, steps * vf::TRACK_STRIDE * sizeof(unsigned long long)));
         fe->track_steps = steps;
     }
     vf::TrackParams q;
@@ -232,7 +232,7 @@ extern "C" int vol_frontend_track(vol_frontend_t *fe, const float T_init[16], co
     q.dist2 = fe->dist_m * fe->dist_m; q.cos_min = fe->cos_min;
     for (int i = 0; i < 12; ++i) q.T0[i] = T_init ? (double)T_init[i] : (i % 5 == 0 ? 1.0 : 0.0);
     q.acc = fe->track_acc; q.out = fe->track_out; q.cond_min = fe->cond_min;
-    if (steps > 0) CK(cudaMemsetAsync(fe->track_acc, 0, steps * vf::ICP_ACC * sizeof(unsigned long long), st));
+    if (steps > 0) CK(cudaMemsetAsync(fe->track_acc, 0, steps * vf::TRACK_STRIDE * sizeof(unsigned long long), st));
     const int tiles0 = ((fe->w + 31) / 32) * ((fe->h + 7) / 8);
     const int blocks = fe->track_blocks < tiles0 ? fe->track_blocks : tiles0;
     void *args[] = {&q};
