@@ -43,7 +43,7 @@ METRIC = "fused_voxel_updates_per_s"
 UNIT = "voxel updates/s"
 
 
-def parse():
+def parse(argv=None):
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=30)
@@ -67,7 +67,7 @@ def parse():
                     help="single process: time shard R of W alone on this GPU (what rank R of a W-GPU --shard run would do)")
     ap.add_argument("--steady-frames", type=int, default=150,
                     help="frames swept back and forth over the arc before the steady-state window (0 = skip it)")
-    return ap.parse_args()
+    return ap.parse_args(argv)
 
 
 def peaks():

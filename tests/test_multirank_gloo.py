@@ -63,7 +63,10 @@ def test_two_ranks_timing_and_shards():
             assert all((k // 8) % world == r for k in o)             # VOL_SLAB = 8 layers dealt round-robin
     sys.path.insert(0, ROOT)
     import bench
-    assert bench.whole_job_value(1000, 10, 2, 5.0) == 2 * 1000 * 10 / 5e-3
+    assert bench.whole_job_value(1000, 10, 2, 5.0) == 2 * 1000 * 10 / 5e-3      # replicas: every rank fuses a scan of its own
+    assert bench.whole_job_value(1000, 10, 1, 5.0) == 1000 * 10 / 5e-3          # --shard: ONE scan, whatever the number of ranks
+    args = bench.parse(["--gpus", "2", "--shard"])
+    assert args.shard and args.shard_of is None and bench.parse(["--shard-of", "1,4"]).shard_of == "1,4"
 
 
 def test_shard_layers_rejects_bad_arguments():
