@@ -68,6 +68,38 @@ def test_raycast_cfg2_r3_and_empty_volume():
     cast_both(g, o, 301, 203, synth.frame(c, 33)[2], c.K_depth / np.array([[2, 1, 2], [1, 2, 2], [1, 1, 1]], np.float32), 0.37, 3.1, trilinear=True)
 
 
+def test_raycast_skip_flags_follow_the_volume():
+    """The casters' skip flags are rebuilt whenever the geometry volume has changed -- by vol_integrate, by vol_upload (content
+    the integration never saw: every tile must be looked at) and by vol_reset (nothing left to hit) -- and not otherwise: casts
+    between changes, from different cameras, both readings, always equal the oracle's."""
+    import paper_1602_06645_b200 as vf
+    c = synth.config(2).scaled(96, 2)
+    g, o = fused_pair(c, (0, 10))
+    Ta, Tb = synth.frame(c, 5)[2], synth.frame(c, 40)[2]
+    for tri in (False, True):
+        cast_both(g, o, c.wd, c.hd, Ta, c.K_depth, 0.2, 4.0, trilinear=tri)
+        cast_both(g, o, c.wd, c.hd, Tb, c.K_depth, 0.2, 4.0, trilinear=tri)            # flags reused
+    depth, rgb, T = synth.frame(c, 20)
+    integrate_both(g, o, c, depth, rgb, T, counting=False)                          # the volume changes: rebuilt
+    for tri in (True, False):
+        d, _ = cast_both(g, o, c.wd, c.hd, Tb, c.K_depth, 0.2, 4.0, trilinear=tri)
+        assert (d > 0).mean() > 0.1
+    # a second volume receives the state through vol_upload: no integration has flagged anything there
+    h = vf.Volume(c.dims_geo, c.r, c.origin, c.extent, c.mu, c.w_max)
+    cast_both(h, type(o)(c.dims_geo, c.r, c.origin, c.extent, c.mu, c.w_max), 80, 60, Ta, c.K_depth / np.array([[8, 1, 8], [1, 8, 8], [1, 1, 1]], np.float32), 0.2, 4.0)
+    h.upload(o.geo, o.col)
+    for tri in (False, True):
+        d, _ = cast_both(h, o, c.wd, c.hd, Ta, c.K_depth, 0.2, 4.0, trilinear=tri)
+        assert (d > 0).mean() > 0.1
+    h.reset()
+    import torch
+    dd = torch.full((c.wd * c.hd,), -1.0, dtype=torch.float32, device="cuda")
+    for fn in (h.raycast, h.raycast_trilinear):
+        fn(c.wd, c.hd, Ta, c.K_depth, 0.2, 4.0, dd)
+        assert float(dd.abs().max()) == 0.0                                         # empty again
+    h.close(); g.close()
+
+
 def test_raycast_rejects_bad_arguments():
     import torch
     import paper_1602_06645_b200 as vf
