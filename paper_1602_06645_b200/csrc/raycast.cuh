@@ -40,7 +40,7 @@ __global__ void __launch_bounds__(256) k_dilate(const __grid_constant__ DilateJo
 
 // The finest level of the ray casters' skip hierarchy, rebuilt (when the volume has changed) just before a ray cast: for
 // every tile that the integration flagged (tile_neg: "may hold an observed voxel with tsdf <= 0" -- a loose, one-sided test
-// against the depth range of the tile's footprint, accumulated over all frames) the tile's voxels are read once and each of
+// against the depth range of the tile's footprint, accumulated since the last rebuild) the tile's voxels are read once and each of
 // its 8 sub-boxes gets the exact answer.  One warp per tile, lane = (x, y) column of a sub-box.  A ray then reads voxels
 // only in the shell of sub-boxes around the zero crossing (and behind it) instead of in every flagged tile it crosses.
 __global__ void __launch_bounds__(256) k_sub_neg(const __grid_constant__ Params p, uint8_t *__restrict__ sub_neg, int sbx_n, int sby_n, int sbz_n,
@@ -100,6 +100,10 @@ __global__ void __launch_bounds__(256) k_sub_neg(const __grid_constant__ Params 
     if (lane == 0) {
         tile_any[tile] = tile_has ? 1 : 0;
         if (tile_has) brick_any[((ttz / 4) * p.bricks_y + tty / 8) * p.bricks_x + ttx] = 1;     // (zeroed before the launch)
+        // The exact answer also replaces the integration's loose flag, so that the next rebuild reads only the tiles that hold
+        // such a voxel now or were flagged since.  Safe: a tile can only receive a tsdf <= 0 in a frame whose classification
+        // flags it again (prepass.cuh sets the flag every time its condition holds, not only the first time).
+        if (flagged && !tile_has) p.tile_neg[tile] = 0;
     }
 }
 
