@@ -157,7 +157,10 @@ int vol_integrate_host(vol_t *v, const uint16_t *depth_u16_host, int32_t wd, int
  * colour voxel containing the hit point gives the colour.
  * depth_dev: DEVICE, w*h float32, metres along the camera's z axis, 0 = no surface; rgb8_dev: DEVICE, w*h*3 bytes R,G,B
  * (black where there is no surface or no colour), nullable.  T_world_cam / K: HOST, as for vol_integrate.  Unsharded
- * volumes only (VOL_E_ARG otherwise).  Asynchronous on `stream`; reads the volumes, writes nothing else. */
+ * volumes only (VOL_E_ARG otherwise).  Asynchronous on `stream`; reads the volumes and writes, beside its outputs, only
+ * per-volume scratch of its own: the first cast after the geometry volume has changed (vol_integrate*, vol_upload,
+ * vol_reset) rebuilds the flags that let rays skip bricks, tiles and 8 x 4 x 4 sub-boxes without an observed tsdf <= 0
+ * (about 30 us on a 512^3 volume) -- which is why ray casts on one volume fall under the stream-ordering rule above too. */
 int vol_raycast(const vol_t *v, int32_t w, int32_t h, const float T_world_cam[16], const float K[9], float t_near_m,
                 float t_far_m, float *depth_dev, uint8_t *rgb8_dev, void *stream);
 
