@@ -8,7 +8,8 @@ primitives on a plane, jittered orbit) -- the configuration the 70 % target is q
 
   value     whole-job voxel updates/s = (N_geo + N_col) voxels brought up to date per frame x frames / device time:
             exactly K steps enqueued one after the other between two CUDA events on the launching stream, inputs resident
-            in HBM.  No L2 flush: the K frames differ and every step touches > 100 MB of volumes of 2.7 GB.
+            in HBM.  No L2 flush kernel: three volumes take the steps in turn, so consecutive steps work on different
+            4.8 GB of memory (inputs larger than L2); --single-volume keeps them on one.
   flushed   the same K frames timed one by one with a 512 MiB flush before each (round 1's method; per_frame_ms)
   steady_state  the same after the arc has been swept until the weights are saturated (gate closed, stores skipped)
   stress    three saturating frames: free space, inside the truncation band, colour shell
@@ -65,6 +66,7 @@ def parse(argv=None):
                          "receives every frame; value = one scan's voxels / max-over-ranks time, scaling = strong")
     ap.add_argument("--shard-of", default=None, metavar="R,W",
                     help="single process: time shard R of W alone on this GPU (what rank R of a W-GPU --shard run would do)")
+    ap.add_argument("--single-volume", action="store_true", help="all timed steps on one volume (default: three volumes take them in turn)")
     ap.add_argument("--steady-frames", type=int, default=150,
                     help="frames swept back and forth over the arc before the steady-state window (0 = skip it)")
     return ap.parse_args(argv)
@@ -288,47 +290,58 @@ def bytes_of(cnt, frame_bytes):
 
 
 class Window:
-    """Counts, per-kernel times and the timed pass of one list of frames on one volume."""
+    """Counts, per-kernel times and the timed passes of one list of frames.  Step s integrates frame s into volume s mod N of
+    `vols`: with N = 3 volumes taking the steps in turn, a volume's lines are touched again only after two other steps have
+    moved their own ~290 MB through the 126 MB L2 -- the inputs of consecutive timed steps are larger than L2 without any
+    flush kernel between them.  Every pass uses the same schedule, so the counters belong to exactly the timed steps."""
 
-    def __init__(self, vol, frames, c, stream, flush_buf, flush):
-        self.vol, self.frames, self.c, self.stream, self.flush_buf, self.flush = vol, frames, c, stream, flush_buf, flush
+    def __init__(self, vols, frames, c, stream, flush_buf, flush):
+        self.vols = vols if isinstance(vols, (list, tuple)) else [vols]
+        self.vol = self.vols[0]
+        self.frames, self.c, self.stream, self.flush_buf, self.flush = frames, c, stream, flush_buf, flush
 
-    def integrate(self, fr):
+    def integrate(self, fr, s=0):
         _, _, dd, dr, T = fr
         c = self.c
-        self.vol.integrate(dd, c.wd, c.hd, dr, c.wh, c.hh, T, c.K_depth, c.K_rgb, c.T_depth_rgb, stream=self.stream)
+        v = self.vols[s % len(self.vols)]
+        v.integrate(dd, c.wd, c.hd, dr, c.wh, c.hh, T, c.K_depth, c.K_rgb, c.T_depth_rgb, stream=self.stream)
+        return v
 
     def count(self):
-        """(untimed) per-frame counters of exactly these frames, from the counting variant"""
-        self.vol.set_counting(True)
+        """(untimed) per-step counters of exactly these steps, from the counting variant"""
+        for v in self.vols:
+            v.set_counting(True)
         rows = []
-        for fr in self.frames:
-            self.integrate(fr)
-            rows.append(stats_row(self.vol.frame_stats(self.stream)))
-        self.vol.set_counting(False)
+        for s, fr in enumerate(self.frames):
+            v = self.integrate(fr, s)
+            rows.append(stats_row(v.frame_stats(self.stream)))
+        for v in self.vols:
+            v.set_counting(False)
         return np.array(rows, dtype=np.float64)
 
     def kernel_times(self):
         """(untimed) per-kernel times (library-side CUDA events on the launching stream)"""
-        self.vol.set_profiling(True)
+        for v in self.vols:
+            v.set_profiling(True)
         kms = []
-        for fr in self.frames:
+        for s, fr in enumerate(self.frames):
             if self.flush:
                 self.flush_buf.zero_()
-            self.integrate(fr)
-            kms.append(self.vol.last_kernel_ms())
-        self.vol.set_profiling(False)
+            v = self.integrate(fr, s)
+            kms.append(v.last_kernel_ms())
+        for v in self.vols:
+            v.set_profiling(False)
         return np.array(kms)
 
     def back_to_back(self, torch, barrier, nvml=None):
-        """the same frames enqueued with nothing between them (no flush kernel, no event): one pair of events around all of
-        them.  Only here can the pre-pass of frame n + 1 start under the tail of frame n's fused kernel (programmatic
-        dependent launch).  The frames differ from one another and the volumes are far larger than L2."""
+        """THE timed pass: the steps enqueued with nothing between them (no flush kernel, no event): one pair of events around
+        all of them.  Only here can the pre-pass of step n + 1 start under the tail of step n's fused kernel (programmatic
+        dependent launch)."""
         t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         barrier()
         t0.record(self.stream)
-        for fr in self.frames:
-            self.integrate(fr)
+        for s, fr in enumerate(self.frames):
+            self.integrate(fr, s)
         t1.record(self.stream)
         while nvml and not t1.query():
             nvml.sample()
@@ -336,14 +349,14 @@ class Window:
         return float(t0.elapsed_time(t1)) / len(self.frames)
 
     def timed(self, torch, barrier, nvml=None):
-        """THE timed pass: events around every frame, L2 flushed between frames"""
+        """the same steps one by one: events around every step, L2 flushed (512 MiB memset) before each"""
         ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in self.frames]
         barrier()
         for n, fr in enumerate(self.frames):
             if self.flush:
                 self.flush_buf.zero_()
             ev[n][0].record(self.stream)
-            self.integrate(fr)
+            self.integrate(fr, n)
             ev[n][1].record(self.stream)
             if nvml and n % 4 == 3:
                 nvml.sample()                                     # the device is busy with the frames enqueued so far
@@ -415,12 +428,17 @@ def run_ours(args, rank, world, local_rank):
     vol = vf.Volume(c.dims_geo, c.r, c.origin, c.extent, mu, c.w_max, sigma=sigma, gate=c.gate, device=local_rank,
                     variant=getattr(c, "variant", 0), shard_rank=shard_rank, shard_world=shard_world)
     warm, timed = frames[:W], frames[W:]
-    win = Window(vol, timed, c, stream, flush_buf, not args.no_flush)
+    # Three volumes take the timed steps in turn (Window): their 3 x (N_geo + N_col) x 4 bytes must fit beside everything else
+    n_rot = 1 if (stress_kind or args.single_volume or 3 * 4 * int(np.prod(c.dims_geo)) * (1 + c.r ** 3) > 100e9) else 3
+    vols = [vol] + [vf.Volume(c.dims_geo, c.r, c.origin, c.extent, mu, c.w_max, sigma=sigma, gate=c.gate, device=local_rank,
+                              variant=getattr(c, "variant", 0), shard_rank=shard_rank, shard_world=shard_world) for _ in range(n_rot - 1)]
+    win = Window(vols, timed, c, stream, flush_buf, not args.no_flush)
 
     def warm_up():
-        vol.reset(stream)
-        for fr in warm:
-            win.integrate(fr)
+        for n, v in enumerate(vols):
+            v.reset(stream)
+            for fr in warm:
+                win.integrate(fr, n)
 
     # ---- pass 1 (untimed): per-frame voxel and sector counters of exactly the timed frames -> algorithmic bytes
     warm_up()
@@ -445,7 +463,8 @@ def run_ours(args, rank, world, local_rank):
     if args.steady_frames > 0 and not stress_kind:
         order = list(range(nfr)) + list(range(nfr - 2, 0, -1))
         for n in range(args.steady_frames):
-            win.integrate(frames[order[n % len(order)]])
+            for k in range(len(vols)):
+                win.integrate(frames[order[n % len(order)]], k)
         s_cnt = win.count()
         s_kms = win.kernel_times()
         s_flushed = win.timed(torch, barrier)
@@ -673,8 +692,11 @@ def run_ours(args, rank, world, local_rank):
                    "value_kind": "visited: (N_geo + N_col) voxels brought up to date per frame x frames / device time -- about 1 % of them "
                                  "are touched (applied_updates_per_s counts those); the reference arm uses the same convention",
                    "frames": "one saturating pose, the wall moving" if stress_kind else f"{first}..{first + nfr - 1} of the seeded trajectory",
-                   "l2": "no flush: inputs larger than L2 -- K distinct frames of 6.8 MB, each touching > 100 MB of volumes of 2.7 GB "
-                         "(126 MB L2); the figure with a 512 MiB flush before every frame is under \"flushed\"",
+                   "l2": (f"no flush: inputs larger than L2 -- {n_rot} volumes of {4e-9 * nvox:.1f} GB take the K steps in turn, each step a "
+                          "distinct frame (6.8 MB) that moves > 100 MB of its volume, so a volume's lines are touched again only "
+                          "after the other volumes' steps have gone through the 126 MB L2" if n_rot > 1 else
+                          "no flush, one volume: K distinct frames, each moving its own part of the volume") +
+                         "; the figure with a 512 MiB flush before every step is under \"flushed\"",
                    "parallelism": (f"shard {shard_rank} of {shard_world} alone (z-slabs {shard_rank} mod {shard_world}): its share of one scan" if args.shard_of else
                                    "single GPU" if world == 1 else
                                    f"one scan on {world} z-slab shards, every rank receives every frame, no data-path collective; counters are rank 0's shard" if args.shard else
